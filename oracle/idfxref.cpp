@@ -1,0 +1,962 @@
+// idfxref — the ORACLE for the idfx B200 library.
+//
+// TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may build, load or call anything in this directory.
+// The CUDA path (paper_2304_13746_b200/) shares no source, header, table or helper with it.
+//
+// What it is: a plain, slow, single-threaded fp64 CPU implementation of one RK2 cycle of the
+// second-order Godunov finite-volume scheme of IDEFIX (Lesur et al., arXiv 2304.13746) for
+// compressible HD and ideal MHD on a uniform periodic 3D Cartesian grid, written step by step in the
+// paper's order.  Citations "PAPER.md:<line>" refer to /root/reference/PAPER.md; "O<n>" / "G<n>" refer
+// to SURVEY.md §8(c) (the written-out formulas and the readings of points the paper leaves open;
+// they are restated in DESIGN.md).
+//
+// Pins (tests/test_oracle_*.py, all `-m "not gpu"`): flux consistency F(U,U)=F(U); HLL/HLLC/HLLD
+// fan-integral identity; HLLC p* continuity; isolated contact and rotational discontinuities; Roe
+// L·R=I, A·r=λr against a finite-difference Jacobian, Σλαr = F_R−F_L; MHD-Roe(B=0) = 5-wave HD Roe;
+// limiter properties; exact Sod solution along x, y, z; direction symmetry; uniform state; conservation;
+// div B; Eᶜ plane-parallel identity; RK2 amplification factor; closed-form dt; 2nd-order convergence of
+// linear fast/Alfvén waves.
+// PARITY UNPINNED (the paper fixes none of these and prints no number that depends on them, see
+// DESIGN.md "Readings"): the limiter flavour (G2), the Davis wave-speed estimate (G5), the HLLD
+// degeneracy threshold (G6), the Roe fallback/degenerate-eigenvector conventions (G7), the face→cell
+// mapping of c_max in dt (G8), un-lagged dt (G9) and the reference E^c state (G10).
+//
+// Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC idfxref.cpp -o libidfxref.so
+#include <algorithm>
+#include <cmath>
+#include <cstddef>
+#include <cstring>
+#include <vector>
+
+#define IDFXREF_API extern "C" __attribute__((visibility("default")))
+
+namespace {
+
+constexpr int NG = 2;  // ghost layers: PLM needs 2 ("number of ghost cells ... adjusted")
+
+enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3 };
+enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2 };
+enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2 };
+enum { OK = 0, ERR_INVALID_ARG = -1, ERR_UNSUPPORTED = -2, ERR_UNPHYSICAL = -5 };
+
+// ---------------------------------------------------------------------------------------------
+// Point-wise physics.  A 1D state along direction d is W = (rho, u, v, w, p, By, Bz) with u the
+// normal velocity and (By, Bz) the transverse field after cyclic permutation; Bn is the normal field.
+// The conserved vector is U = (rho, rho u, rho v, rho w, E, By, Bz).
+// ---------------------------------------------------------------------------------------------
+
+// O1 / PAPER.md:61: E = p/(gamma-1) + rho v^2/2 + B^2/2.
+void cons_from_prim(const double W[7], double Bn, double g, double U[7]) {
+  const double rho = W[0], u = W[1], v = W[2], w = W[3], p = W[4], By = W[5], Bz = W[6];
+  U[0] = rho;
+  U[1] = rho * u;
+  U[2] = rho * v;
+  U[3] = rho * w;
+  U[4] = p / (g - 1.0) + 0.5 * rho * (u * u + v * v + w * w) + 0.5 * (Bn * Bn + By * By + Bz * Bz);
+  U[5] = By;
+  U[6] = Bz;
+}
+
+// O4 / PAPER.md:43-53 (Eq. 1-4, ideal part), P = p + B^2/2.
+void phys_flux(const double W[7], double Bn, const double U[7], double F[7]) {
+  const double rho = W[0], u = W[1], v = W[2], w = W[3], p = W[4], By = W[5], Bz = W[6];
+  const double pT = p + 0.5 * (Bn * Bn + By * By + Bz * Bz);
+  F[0] = rho * u;
+  F[1] = rho * u * u + pT - Bn * Bn;
+  F[2] = rho * u * v - Bn * By;
+  F[3] = rho * u * w - Bn * Bz;
+  F[4] = (U[4] + pT) * u - Bn * (u * Bn + v * By + w * Bz);
+  F[5] = u * By - v * Bn;
+  F[6] = u * Bz - w * Bn;
+}
+
+// O4: a^2 = gamma p / rho; c_f^2 = (1/2)[a^2 + b^2 + sqrt((a^2+b^2)^2 - 4 a^2 Bn^2/rho)], b^2 = |B|^2/rho.
+// With B = 0 this is exactly a.
+double fast_speed(const double W[7], double Bn, double g) {
+  const double rho = W[0], p = W[4], By = W[5], Bz = W[6];
+  const double a2 = g * p / rho;
+  const double b2 = (Bn * Bn + By * By + Bz * Bz) / rho;
+  const double s = a2 + b2;
+  double disc = s * s - 4.0 * a2 * Bn * Bn / rho;
+  if (disc < 0.0) disc = 0.0;
+  return std::sqrt(0.5 * (s + std::sqrt(disc)));
+}
+
+// O4 / G5 (Davis): S_L = min(u_L - c_L, u_R - c_R), S_R = max(u_L + c_L, u_R + c_R).
+void davis_speeds(const double WL[7], const double WR[7], double Bn, double g, double& SL, double& SR) {
+  const double cL = fast_speed(WL, Bn, g), cR = fast_speed(WR, Bn, g);
+  SL = std::min(WL[1] - cL, WR[1] - cR);
+  SR = std::max(WL[1] + cL, WR[1] + cR);
+}
+
+// O5 HLL.
+void hll_flux(const double UL[7], const double UR[7], const double FL[7], const double FR[7], double SL,
+              double SR, double F[7]) {
+  if (SL >= 0.0) {
+    for (int n = 0; n < 7; ++n) F[n] = FL[n];
+  } else if (SR <= 0.0) {
+    for (int n = 0; n < 7; ++n) F[n] = FR[n];
+  } else {
+    for (int n = 0; n < 7; ++n) F[n] = (SR * FL[n] - SL * FR[n] + SL * SR * (UR[n] - UL[n])) / (SR - SL);
+  }
+}
+
+// O6 HLLC, hydrodynamics only (Toro et al. 1994).  Star states are returned for the pins.
+struct HllcFan {
+  double SL, SS, SR;
+  double UsL[5], UsR[5];
+};
+
+void hllc_fan(const double WL[7], const double WR[7], const double UL[7], const double UR[7], double SL,
+              double SR, HllcFan& f) {
+  const double rL = WL[0], uL = WL[1], pL = WL[4];
+  const double rR = WR[0], uR = WR[1], pR = WR[4];
+  const double SS = (pR - pL + rL * uL * (SL - uL) - rR * uR * (SR - uR)) / (rL * (SL - uL) - rR * (SR - uR));
+  f.SL = SL;
+  f.SS = SS;
+  f.SR = SR;
+  {
+    const double fac = rL * (SL - uL) / (SL - SS);
+    f.UsL[0] = fac;
+    f.UsL[1] = fac * SS;
+    f.UsL[2] = fac * WL[2];
+    f.UsL[3] = fac * WL[3];
+    f.UsL[4] = fac * (UL[4] / rL + (SS - uL) * (SS + pL / (rL * (SL - uL))));
+  }
+  {
+    const double fac = rR * (SR - uR) / (SR - SS);
+    f.UsR[0] = fac;
+    f.UsR[1] = fac * SS;
+    f.UsR[2] = fac * WR[2];
+    f.UsR[3] = fac * WR[3];
+    f.UsR[4] = fac * (UR[4] / rR + (SS - uR) * (SS + pR / (rR * (SR - uR))));
+  }
+}
+
+void hllc_flux(const double WL[7], const double WR[7], const double UL[7], const double UR[7],
+               const double FL[7], const double FR[7], double SL, double SR, double F[7]) {
+  F[5] = 0.0;
+  F[6] = 0.0;
+  if (SL >= 0.0) {
+    for (int n = 0; n < 5; ++n) F[n] = FL[n];
+    return;
+  }
+  if (SR <= 0.0) {
+    for (int n = 0; n < 5; ++n) F[n] = FR[n];
+    return;
+  }
+  HllcFan f;
+  hllc_fan(WL, WR, UL, UR, SL, SR, f);
+  if (f.SS >= 0.0) {
+    for (int n = 0; n < 5; ++n) F[n] = FL[n] + SL * (f.UsL[n] - UL[n]);
+  } else {
+    for (int n = 0; n < 5; ++n) F[n] = FR[n] + SR * (f.UsR[n] - UR[n]);
+  }
+}
+
+// O7 HLLD (Miyoshi & Kusano 2005).  The five speeds and four intermediate states are
+// returned for the pins.
+struct HlldFan {
+  double SL, SsL, SM, SsR, SR;
+  double UsL[7], UssL[7], UssR[7], UsR[7];
+};
+
+void hlld_fan(const double WL[7], const double WR[7], double Bn, const double UL[7], const double UR[7],
+              double SL, double SR, HlldFan& f) {
+  const double rL = WL[0], uL = WL[1], vL = WL[2], wL = WL[3], pL = WL[4], ByL = WL[5], BzL = WL[6];
+  const double rR = WR[0], uR = WR[1], vR = WR[2], wR = WR[3], pR = WR[4], ByR = WR[5], BzR = WR[6];
+  const double pTL = pL + 0.5 * (Bn * Bn + ByL * ByL + BzL * BzL);
+  const double pTR = pR + 0.5 * (Bn * Bn + ByR * ByR + BzR * BzR);
+  const double sgn = (Bn >= 0.0) ? 1.0 : -1.0;
+
+  const double D = (SR - uR) * rR - (SL - uL) * rL;
+  const double SM = ((SR - uR) * rR * uR - (SL - uL) * rL * uL - pTR + pTL) / D;
+  const double pTs =
+      ((SR - uR) * rR * pTL - (SL - uL) * rL * pTR + rL * rR * (SR - uR) * (SL - uL) * (uR - uL)) / D;
+
+  // star states, K = L, R
+  double rsL, vsL, wsL, BysL, BzsL, EsL;
+  double rsR, vsR, wsR, BysR, BzsR, EsR;
+  {
+    rsL = rL * (SL - uL) / (SL - SM);
+    const double dK = rL * (SL - uL) * (SL - SM) - Bn * Bn;
+    if (std::fabs(dK) < 1e-12 * rL * (SL - uL) * (SL - uL)) {  // G6
+      vsL = vL;
+      wsL = wL;
+      BysL = ByL;
+      BzsL = BzL;
+    } else {
+      vsL = vL - Bn * ByL * (SM - uL) / dK;
+      wsL = wL - Bn * BzL * (SM - uL) / dK;
+      const double num = rL * (SL - uL) * (SL - uL) - Bn * Bn;
+      BysL = ByL * num / dK;
+      BzsL = BzL * num / dK;
+    }
+    const double vB = uL * Bn + vL * ByL + wL * BzL;
+    const double vBs = SM * Bn + vsL * BysL + wsL * BzsL;
+    EsL = ((SL - uL) * UL[4] - pTL * uL + pTs * SM + Bn * (vB - vBs)) / (SL - SM);
+  }
+  {
+    rsR = rR * (SR - uR) / (SR - SM);
+    const double dK = rR * (SR - uR) * (SR - SM) - Bn * Bn;
+    if (std::fabs(dK) < 1e-12 * rR * (SR - uR) * (SR - uR)) {  // G6
+      vsR = vR;
+      wsR = wR;
+      BysR = ByR;
+      BzsR = BzR;
+    } else {
+      vsR = vR - Bn * ByR * (SM - uR) / dK;
+      wsR = wR - Bn * BzR * (SM - uR) / dK;
+      const double num = rR * (SR - uR) * (SR - uR) - Bn * Bn;
+      BysR = ByR * num / dK;
+      BzsR = BzR * num / dK;
+    }
+    const double vB = uR * Bn + vR * ByR + wR * BzR;
+    const double vBs = SM * Bn + vsR * BysR + wsR * BzsR;
+    EsR = ((SR - uR) * UR[4] - pTR * uR + pTs * SM + Bn * (vB - vBs)) / (SR - SM);
+  }
+  const double sqL = std::sqrt(rsL), sqR = std::sqrt(rsR);
+  f.SL = SL;
+  f.SR = SR;
+  f.SM = SM;
+  f.SsL = SM - std::fabs(Bn) / sqL;
+  f.SsR = SM + std::fabs(Bn) / sqR;
+
+  // double-star states
+  const double inv = 1.0 / (sqL + sqR);
+  const double vss = (sqL * vsL + sqR * vsR + (BysR - BysL) * sgn) * inv;
+  const double wss = (sqL * wsL + sqR * wsR + (BzsR - BzsL) * sgn) * inv;
+  const double Byss = (sqL * BysR + sqR * BysL + sqL * sqR * (vsR - vsL) * sgn) * inv;
+  const double Bzss = (sqL * BzsR + sqR * BzsL + sqL * sqR * (wsR - wsL) * sgn) * inv;
+  const double vBss = SM * Bn + vss * Byss + wss * Bzss;
+  const double vBsL = SM * Bn + vsL * BysL + wsL * BzsL;
+  const double vBsR = SM * Bn + vsR * BysR + wsR * BzsR;
+  const double EssL = EsL - sqL * (vBsL - vBss) * sgn;
+  const double EssR = EsR + sqR * (vBsR - vBss) * sgn;
+
+  f.UsL[0] = rsL; f.UsL[1] = rsL * SM; f.UsL[2] = rsL * vsL; f.UsL[3] = rsL * wsL; f.UsL[4] = EsL;
+  f.UsL[5] = BysL; f.UsL[6] = BzsL;
+  f.UsR[0] = rsR; f.UsR[1] = rsR * SM; f.UsR[2] = rsR * vsR; f.UsR[3] = rsR * wsR; f.UsR[4] = EsR;
+  f.UsR[5] = BysR; f.UsR[6] = BzsR;
+  f.UssL[0] = rsL; f.UssL[1] = rsL * SM; f.UssL[2] = rsL * vss; f.UssL[3] = rsL * wss; f.UssL[4] = EssL;
+  f.UssL[5] = Byss; f.UssL[6] = Bzss;
+  f.UssR[0] = rsR; f.UssR[1] = rsR * SM; f.UssR[2] = rsR * vss; f.UssR[3] = rsR * wss; f.UssR[4] = EssR;
+  f.UssR[5] = Byss; f.UssR[6] = Bzss;
+}
+
+void hlld_flux(const double WL[7], const double WR[7], double Bn, const double UL[7], const double UR[7],
+               const double FL[7], const double FR[7], double SL, double SR, double F[7]) {
+  if (SL >= 0.0) {
+    for (int n = 0; n < 7; ++n) F[n] = FL[n];
+    return;
+  }
+  if (SR <= 0.0) {
+    for (int n = 0; n < 7; ++n) F[n] = FR[n];
+    return;
+  }
+  HlldFan f;
+  hlld_fan(WL, WR, Bn, UL, UR, SL, SR, f);
+  // selection in exactly the order of O7
+  if (f.SsL >= 0.0) {
+    for (int n = 0; n < 7; ++n) F[n] = FL[n] + SL * (f.UsL[n] - UL[n]);
+  } else if (f.SsR <= 0.0) {
+    for (int n = 0; n < 7; ++n) F[n] = FR[n] + SR * (f.UsR[n] - UR[n]);
+  } else if (f.SM >= 0.0) {
+    for (int n = 0; n < 7; ++n)
+      F[n] = FL[n] + f.SsL * f.UssL[n] - (f.SsL - SL) * f.UsL[n] - SL * UL[n];
+  } else {
+    for (int n = 0; n < 7; ++n)
+      F[n] = FR[n] + f.SsR * f.UssR[n] - (f.SsR - SR) * f.UsR[n] - SR * UR[n];
+  }
+}
+
+// O8 Roe ("approximate linear Roe Riemann solver (Cargo & Gallice 1997)").
+// Eigen-system in primitive variables W = (rho,u,v,w,p,By,Bz) at the Roe-averaged state, plus the
+// matrices M = dU/dW and Minv = dW/dU of the shifted equation of state (O8).  Returns false when
+// a~^2 <= 0 (G7: the caller then falls back to HLL).
+struct RoeSys {
+  double lam[7];
+  double R[7][7];  // R[k][:] = k-th right eigenvector (primitive)
+  double L[7][7];  // L[k][:] = k-th left eigenvector (primitive)
+  double M[7][7];
+  double Minv[7][7];
+};
+
+bool roe_system(const double WL[7], const double WR[7], double Bn, const double UL[7], const double UR[7],
+                double g, RoeSys& s) {
+  const double rL = WL[0], rR = WR[0];
+  const double sL = std::sqrt(rL), sR = std::sqrt(rR);
+  const double isum = 1.0 / (sL + sR);
+  const double rb = sL * sR;
+  const double ub = (sL * WL[1] + sR * WR[1]) * isum;
+  const double vb = (sL * WL[2] + sR * WR[2]) * isum;
+  const double wb = (sL * WL[3] + sR * WR[3]) * isum;
+  const double pTL = WL[4] + 0.5 * (Bn * Bn + WL[5] * WL[5] + WL[6] * WL[6]);
+  const double pTR = WR[4] + 0.5 * (Bn * Bn + WR[5] * WR[5] + WR[6] * WR[6]);
+  const double HL = (UL[4] + pTL) / rL, HR = (UR[4] + pTR) / rR;
+  const double Hb = (sL * HL + sR * HR) * isum;
+  const double Byb = (sR * WL[5] + sL * WR[5]) * isum;  // weights swapped (O8)
+  const double Bzb = (sR * WL[6] + sL * WR[6]) * isum;
+  const double dBy = WR[5] - WL[5], dBz = WR[6] - WL[6];
+  const double X = (dBy * dBy + dBz * dBz) * 0.5 * isum * isum;
+  const double Xp = (g - 2.0) * X;
+  const double v2 = ub * ub + vb * vb + wb * wb;
+  const double a2 = (g - 1.0) * (Hb - 0.5 * v2 - (Bn * Bn + Byb * Byb + Bzb * Bzb) / rb) - Xp;
+  if (!(a2 > 0.0)) return false;
+  const double a = std::sqrt(a2);
+
+  const double bn2 = Bn * Bn / rb;
+  const double bt2 = (Byb * Byb + Bzb * Bzb) / rb;
+  const double sum = a2 + bn2 + bt2;
+  double disc = sum * sum - 4.0 * a2 * bn2;
+  if (disc < 0.0) disc = 0.0;
+  const double Cf2 = 0.5 * (sum + std::sqrt(disc));
+  const double Cs2 = a2 * bn2 / Cf2;
+  const double Cf = std::sqrt(Cf2), Cs = std::sqrt(Cs2);
+  const double CA = std::sqrt(bn2);
+
+  double af, as;
+  if (Cf2 - Cs2 <= 0.0) {
+    af = 1.0;
+    as = 0.0;
+  } else {
+    double af2 = (a2 - Cs2) / (Cf2 - Cs2), as2 = (Cf2 - a2) / (Cf2 - Cs2);
+    af2 = std::min(1.0, std::max(0.0, af2));
+    as2 = std::min(1.0, std::max(0.0, as2));
+    af = std::sqrt(af2);
+    as = std::sqrt(as2);
+  }
+  const double Bt = std::sqrt(Byb * Byb + Bzb * Bzb);
+  double by, bz;
+  if (Bt == 0.0) {
+    by = bz = 1.0 / std::sqrt(2.0);
+  } else {
+    by = Byb / Bt;
+    bz = Bzb / Bt;
+  }
+  const double S = (Bn >= 0.0) ? 1.0 : -1.0;
+  const double sr = std::sqrt(rb);
+  const double Cff = Cf * af, Css = Cs * as, Qf = Cf * af * S, Qs = Cs * as * S;
+  const double Af = a * af * sr, As = a * as * sr;
+
+  s.lam[0] = ub - Cf; s.lam[1] = ub - CA; s.lam[2] = ub - Cs; s.lam[3] = ub;
+  s.lam[4] = ub + Cs; s.lam[5] = ub + CA; s.lam[6] = ub + Cf;
+
+  const double i2a2 = 1.0 / (2.0 * a2);
+  for (int k = 0; k < 7; ++k)
+    for (int n = 0; n < 7; ++n) s.R[k][n] = s.L[k][n] = 0.0;
+  // fast, sign = -1 for k=0 (u - Cf), +1 for k=6
+  for (int pm = 0; pm < 2; ++pm) {
+    const int k = pm ? 6 : 0;
+    const double sg = pm ? 1.0 : -1.0;
+    double* r = s.R[k];
+    double* l = s.L[k];
+    r[0] = rb * af; r[1] = sg * Cff; r[2] = -sg * Qs * by; r[3] = -sg * Qs * bz; r[4] = rb * a2 * af;
+    r[5] = As * by; r[6] = As * bz;
+    l[0] = 0.0; l[1] = sg * Cff * i2a2; l[2] = -sg * Qs * by * i2a2; l[3] = -sg * Qs * bz * i2a2;
+    l[4] = af / rb * i2a2; l[5] = As * by / rb * i2a2; l[6] = As * bz / rb * i2a2;
+  }
+  // Alfven, k=1 (u - CA), k=5 (u + CA)
+  for (int pm = 0; pm < 2; ++pm) {
+    const int k = pm ? 5 : 1;
+    const double sg = pm ? 1.0 : -1.0;
+    double* r = s.R[k];
+    double* l = s.L[k];
+    r[2] = sg * bz; r[3] = -sg * by; r[5] = -S * sr * bz; r[6] = S * sr * by;
+    l[2] = 0.5 * sg * bz; l[3] = -0.5 * sg * by; l[5] = -0.5 * S * bz / sr; l[6] = 0.5 * S * by / sr;
+  }
+  // slow, k=2 (u - Cs), k=4 (u + Cs)
+  for (int pm = 0; pm < 2; ++pm) {
+    const int k = pm ? 4 : 2;
+    const double sg = pm ? 1.0 : -1.0;
+    double* r = s.R[k];
+    double* l = s.L[k];
+    r[0] = rb * as; r[1] = sg * Css; r[2] = sg * Qf * by; r[3] = sg * Qf * bz; r[4] = rb * a2 * as;
+    r[5] = -Af * by; r[6] = -Af * bz;
+    l[0] = 0.0; l[1] = sg * Css * i2a2; l[2] = sg * Qf * by * i2a2; l[3] = sg * Qf * bz * i2a2;
+    l[4] = as / rb * i2a2; l[5] = -Af * by / rb * i2a2; l[6] = -Af * bz / rb * i2a2;
+  }
+  // entropy
+  s.R[3][0] = 1.0;
+  s.L[3][0] = 1.0;
+  s.L[3][4] = -1.0 / a2;
+
+  for (int r = 0; r < 7; ++r)
+    for (int c = 0; c < 7; ++c) s.M[r][c] = s.Minv[r][c] = 0.0;
+  const double gm1 = g - 1.0;
+  s.M[0][0] = 1.0;
+  s.M[1][0] = ub; s.M[1][1] = rb;
+  s.M[2][0] = vb; s.M[2][2] = rb;
+  s.M[3][0] = wb; s.M[3][3] = rb;
+  s.M[4][0] = 0.5 * v2 + Xp / gm1; s.M[4][1] = rb * ub; s.M[4][2] = rb * vb; s.M[4][3] = rb * wb;
+  s.M[4][4] = 1.0 / gm1; s.M[4][5] = Byb; s.M[4][6] = Bzb;
+  s.M[5][5] = 1.0;
+  s.M[6][6] = 1.0;
+  s.Minv[0][0] = 1.0;
+  s.Minv[1][0] = -ub / rb; s.Minv[1][1] = 1.0 / rb;
+  s.Minv[2][0] = -vb / rb; s.Minv[2][2] = 1.0 / rb;
+  s.Minv[3][0] = -wb / rb; s.Minv[3][3] = 1.0 / rb;
+  s.Minv[4][0] = gm1 * 0.5 * v2 - Xp; s.Minv[4][1] = -gm1 * ub; s.Minv[4][2] = -gm1 * vb;
+  s.Minv[4][3] = -gm1 * wb; s.Minv[4][4] = gm1; s.Minv[4][5] = -gm1 * Byb; s.Minv[4][6] = -gm1 * Bzb;
+  s.Minv[5][5] = 1.0;
+  s.Minv[6][6] = 1.0;
+  return true;
+}
+
+// F = (F_L+F_R)/2 - (1/2) sum_k |lambda_k| alpha_k r_k, alpha = L (Minv dU), r^cons = M r  (O8, no entropy fix).
+bool roe_flux(const double WL[7], const double WR[7], double Bn, const double UL[7], const double UR[7],
+              const double FL[7], const double FR[7], double g, double F[7]) {
+  RoeSys s;
+  if (!roe_system(WL, WR, Bn, UL, UR, g, s)) return false;
+  double dU[7], dW[7], acc[7];
+  for (int n = 0; n < 7; ++n) dU[n] = UR[n] - UL[n];
+  for (int r = 0; r < 7; ++r) {
+    double t = 0.0;
+    for (int c = 0; c < 7; ++c) t += s.Minv[r][c] * dU[c];
+    dW[r] = t;
+  }
+  for (int n = 0; n < 7; ++n) acc[n] = 0.0;
+  for (int k = 0; k < 7; ++k) {
+    double alpha = 0.0;
+    for (int n = 0; n < 7; ++n) alpha += s.L[k][n] * dW[n];
+    const double c = std::fabs(s.lam[k]) * alpha;
+    for (int n = 0; n < 7; ++n) acc[n] += c * s.R[k][n];
+  }
+  for (int r = 0; r < 7; ++r) {
+    double t = 0.0;
+    for (int c = 0; c < 7; ++c) t += s.M[r][c] * acc[c];
+    F[r] = 0.5 * (FL[r] + FR[r]) - 0.5 * t;
+  }
+  return true;
+}
+
+// One Riemann problem: flux F and the face signal speed c_face = max(|S_L|,|S_R|) for every solver (O4).
+// Returns 1 when the Roe solver fell back to HLL (G7), else 0.
+int riemann(int solver, double g, const double WL[7], const double WR[7], double Bn, double F[7],
+            double& cface) {
+  double UL[7], UR[7], FL[7], FR[7], SL, SR;
+  cons_from_prim(WL, Bn, g, UL);
+  cons_from_prim(WR, Bn, g, UR);
+  phys_flux(WL, Bn, UL, FL);
+  phys_flux(WR, Bn, UR, FR);
+  davis_speeds(WL, WR, Bn, g, SL, SR);
+  cface = std::max(std::fabs(SL), std::fabs(SR));
+  int fallback = 0;
+  switch (solver) {
+    case SOLVER_HLL: hll_flux(UL, UR, FL, FR, SL, SR, F); break;
+    case SOLVER_HLLC: hllc_flux(WL, WR, UL, UR, FL, FR, SL, SR, F); break;
+    case SOLVER_HLLD: hlld_flux(WL, WR, Bn, UL, UR, FL, FR, SL, SR, F); break;
+    default:
+      if (!roe_flux(WL, WR, Bn, UL, UR, FL, FR, g, F)) {
+        hll_flux(UL, UR, FL, FR, SL, SR, F);
+        fallback = 1;
+      }
+  }
+  return fallback;
+}
+
+// O3 limited slope (G2): zero at extrema; van Leer = harmonic mean; minmod = smaller one.
+double slope(int limiter, double dm, double dp) {
+  if (limiter == LIM_FLAT) return 0.0;
+  if (dm * dp <= 0.0) return 0.0;
+  if (limiter == LIM_VANLEER) return 2.0 * dm * dp / (dm + dp);
+  const double s = (dm > 0.0) ? 1.0 : -1.0;
+  return s * std::min(std::fabs(dm), std::fabs(dp));
+}
+
+// ---------------------------------------------------------------------------------------------
+// Grid-level scheme
+// ---------------------------------------------------------------------------------------------
+typedef std::vector<double> Arr;
+
+struct Ctx {
+  int n[3];
+  double dx, g;
+  int solver, limiter, emf;
+  bool mhd;
+  int p[3];
+  size_t st[3];  // strides in doubles: st[0] = 1
+  size_t N;
+  Arr U[5], U0[5], U1[5], Us[5];    // master conserved state, saved state, stage-1 state, scratch
+  Arr Bf[3], Bf0[3], Bf1[3], Bfs[3];
+  Arr V[8];                         // rho, vx, vy, vz, p, Bcx, Bcy, Bcz
+  Arr F[3][7];                      // face fluxes per direction in that direction's local ordering
+  Arr cf[3];                        // c_face per direction
+  Arr E[3];                         // edge EMFs: E[0] at (i, j-1/2, k-1/2), E[1] at (i-1/2, j, k-1/2), E[2] at (i-1/2, j-1/2, k)
+  double last_dt;
+  int status;
+  long long roe_fallbacks;
+
+  size_t at(int i, int j, int k) const {
+    return (size_t)(k + NG) * st[2] + (size_t)(j + NG) * st[1] + (size_t)(i + NG);
+  }
+};
+
+inline int pmod(int a, int n) {
+  int r = a % n;
+  return r < 0 ? r + n : r;
+}
+
+// a1 / O2(i): periodic fill, 2 layers, x then y then z (PAPER.md:233 sequential per-dimension order).
+void fill_periodic(const Ctx& c, Arr& a) {
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int gI = 1; gI <= NG; ++gI) {
+        a[c.at(-gI, j, k)] = a[c.at(pmod(-gI, nx), j, k)];
+        a[c.at(nx - 1 + gI, j, k)] = a[c.at(pmod(nx - 1 + gI, nx), j, k)];
+      }
+  for (int k = 0; k < nz; ++k)
+    for (int gI = 1; gI <= NG; ++gI)
+      for (int i = -NG; i < nx + NG; ++i) {
+        a[c.at(i, -gI, k)] = a[c.at(i, pmod(-gI, ny), k)];
+        a[c.at(i, ny - 1 + gI, k)] = a[c.at(i, pmod(ny - 1 + gI, ny), k)];
+      }
+  for (int gI = 1; gI <= NG; ++gI)
+    for (int j = -NG; j < ny + NG; ++j)
+      for (int i = -NG; i < nx + NG; ++i) {
+        a[c.at(i, j, -gI)] = a[c.at(i, j, pmod(-gI, nz))];
+        a[c.at(i, j, nz - 1 + gI)] = a[c.at(i, j, pmod(nz - 1 + gI, nz))];
+      }
+}
+
+// a2 / O1: Bc = mean of the two bounding faces (G1); v = m/rho; p = (gamma-1)(E - rho v^2/2 - Bc^2/2).
+// Needs the face ghosts of Bf (face index n).  Prims are computed on active cells and then filled
+// periodically, which is bit-identical to computing them in the ghosts from filled U and Bf (O2 (i)-(ii)).
+void compute_prims(Ctx& c, const Arr U[5], const Arr Bf[3]) {
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        const size_t q = c.at(i, j, k);
+        double bx = 0.0, by = 0.0, bz = 0.0;
+        if (c.mhd) {
+          bx = 0.5 * (Bf[0][q] + Bf[0][q + c.st[0]]);
+          by = 0.5 * (Bf[1][q] + Bf[1][q + c.st[1]]);
+          bz = 0.5 * (Bf[2][q] + Bf[2][q + c.st[2]]);
+        }
+        const double rho = U[0][q];
+        const double vx = U[1][q] / rho, vy = U[2][q] / rho, vz = U[3][q] / rho;
+        const double p =
+            (c.g - 1.0) * (U[4][q] - 0.5 * rho * (vx * vx + vy * vy + vz * vz) - 0.5 * (bx * bx + by * by + bz * bz));
+        if (!(rho > 0.0) || !(p > 0.0)) c.status = ERR_UNPHYSICAL;
+        c.V[0][q] = rho; c.V[1][q] = vx; c.V[2][q] = vy; c.V[3][q] = vz; c.V[4][q] = p;
+        c.V[5][q] = bx; c.V[6][q] = by; c.V[7][q] = bz;
+      }
+  for (int n = 0; n < (c.mhd ? 8 : 5); ++n) fill_periodic(c, c.V[n]);
+}
+
+// a3+a4 / O3-O8: face states and Riemann flux on every face of direction d whose 4-cell stencil exists:
+// index 0..n along d, and one transverse ghost layer (needed by the EMFs).
+void sweep(Ctx& c, int d, const Arr Bf[3], bool want_flux) {
+  const int a = d, b = (d + 1) % 3, e = (d + 2) % 3;
+  int lo[3], hi[3];
+  lo[a] = 0; hi[a] = c.n[a];
+  lo[b] = -1; hi[b] = c.n[b];
+  lo[e] = -1; hi[e] = c.n[e];
+  const size_t sa = c.st[a];
+  const Arr* q[7] = {&c.V[0], &c.V[1 + a], &c.V[1 + b], &c.V[1 + e], &c.V[4], &c.V[5 + b], &c.V[5 + e]};
+  const int nq = c.mhd ? 7 : 5;
+  int ijk[3];
+  for (ijk[2] = lo[2]; ijk[2] <= hi[2]; ++ijk[2])
+    for (ijk[1] = lo[1]; ijk[1] <= hi[1]; ++ijk[1])
+      for (ijk[0] = lo[0]; ijk[0] <= hi[0]; ++ijk[0]) {
+        const size_t i0 = c.at(ijk[0], ijk[1], ijk[2]);  // cell to the right of the face
+        double WL[7] = {0, 0, 0, 0, 0, 0, 0}, WR[7] = {0, 0, 0, 0, 0, 0, 0};
+        for (int n = 0; n < nq; ++n) {
+          const double* v = q[n]->data();
+          const double qm2 = v[i0 - 2 * sa], qm1 = v[i0 - sa], q0 = v[i0], qp1 = v[i0 + sa];
+          const double sm = slope(c.limiter, qm1 - qm2, q0 - qm1);   // slope of cell i-1
+          const double s0 = slope(c.limiter, q0 - qm1, qp1 - q0);    // slope of cell i
+          WL[n] = qm1 + 0.5 * sm;
+          WR[n] = q0 - 0.5 * s0;
+        }
+        const double Bn = c.mhd ? Bf[a][i0] : 0.0;  // G3: staggered value on both sides
+        if (!(WL[0] > 0.0) || !(WR[0] > 0.0) || !(WL[4] > 0.0) || !(WR[4] > 0.0)) c.status = ERR_UNPHYSICAL;
+        if (want_flux) {
+          double F[7], cface;
+          c.roe_fallbacks += riemann(c.solver, c.g, WL, WR, Bn, F, cface);
+          for (int n = 0; n < 7; ++n) c.F[d][n][i0] = F[n];
+          c.cf[d][i0] = cface;
+        } else {
+          double SL, SR;
+          davis_speeds(WL, WR, Bn, c.g, SL, SR);
+          c.cf[d][i0] = std::max(std::fabs(SL), std::fabs(SR));
+        }
+      }
+}
+
+// a6 / O10: edge EMF E_c at (a-1/2, b-1/2) with (a,b,c) cyclic.
+void edge_emf(Ctx& c, int comp) {
+  const int a = (comp + 1) % 3, b = (comp + 2) % 3;
+  const size_t ea = c.st[a], eb = c.st[b];
+  int lo[3] = {0, 0, 0}, hi[3];
+  hi[a] = c.n[a]; hi[b] = c.n[b]; hi[comp] = c.n[comp] - 1;
+  // face-centred EMFs from the Riemann fluxes of B: E_c^(a) = -F_a[B_b] = -F[a][5]; E_c^(b) = +F_b[B_a] = +F[b][6]
+  const double* Fa5 = c.F[a][5].data();
+  const double* Fb6 = c.F[b][6].data();
+  const double* Fa0 = c.F[a][0].data();
+  const double* Fb0 = c.F[b][0].data();
+  const double* va = c.V[1 + a].data();
+  const double* vb = c.V[1 + b].data();
+  const double* Ba = c.V[5 + a].data();
+  const double* Bb = c.V[5 + b].data();
+  auto Ea = [&](size_t P) { return -Fa5[P]; };
+  auto Eb = [&](size_t P) { return Fb6[P]; };
+  auto Ec = [&](size_t Q) { return vb[Q] * Ba[Q] - va[Q] * Bb[Q]; };  // -(v x B)_c at the cell centre (G10)
+  auto upwind = [](double flux, double gm, double gp) {
+    if (flux > 0.0) return gm;
+    if (flux < 0.0) return gp;
+    return 0.5 * (gm + gp);
+  };
+  int ijk[3];
+  for (ijk[2] = lo[2]; ijk[2] <= hi[2]; ++ijk[2])
+    for (ijk[1] = lo[1]; ijk[1] <= hi[1]; ++ijk[1])
+      for (ijk[0] = lo[0]; ijk[0] <= hi[0]; ++ijk[0]) {
+        const size_t P = c.at(ijk[0], ijk[1], ijk[2]);
+        double e = 0.25 * (Ea(P) + Ea(P - eb) + Eb(P) + Eb(P - ea));
+        if (c.emf == EMF_UCT) {
+          // d/db at the a-face (ia-1/2): quarter points ib-1/4 (cells P-ea, P) and ib-3/4 (cells P-ea-eb, P-eb)
+          const double gbp_m = 2.0 * (Ec(P - ea) - Eb(P - ea));          // g_b+ of cell P-ea
+          const double gbp_p = 2.0 * (Ec(P) - Eb(P));                    // g_b+ of cell P
+          const double gbm_m = 2.0 * (Eb(P - ea) - Ec(P - ea - eb));     // g_b- of cell P-ea-eb
+          const double gbm_p = 2.0 * (Eb(P) - Ec(P - eb));               // g_b- of cell P-eb
+          const double Gb_q1 = upwind(Fa0[P], gbp_m, gbp_p);             // (ia-1/2, ib-1/4)
+          const double Gb_q3 = upwind(Fa0[P - eb], gbm_m, gbm_p);        // (ia-1/2, ib-3/4)
+          // d/da at the b-face (ib-1/2): quarter points ia-1/4 (cells P-eb, P) and ia-3/4 (cells P-ea-eb, P-ea)
+          const double gap_m = 2.0 * (Ec(P - eb) - Ea(P - eb));          // g_a+ of cell P-eb
+          const double gap_p = 2.0 * (Ec(P) - Ea(P));                    // g_a+ of cell P
+          const double gam_m = 2.0 * (Ea(P - eb) - Ec(P - ea - eb));     // g_a- of cell P-ea-eb
+          const double gam_p = 2.0 * (Ea(P) - Ec(P - ea));               // g_a- of cell P-ea
+          const double Ga_q1 = upwind(Fb0[P], gap_m, gap_p);             // (ia-1/4, ib-1/2)
+          const double Ga_q3 = upwind(Fb0[P - ea], gam_m, gam_p);        // (ia-3/4, ib-1/2)
+          e += 0.125 * (Gb_q3 - Gb_q1) + 0.125 * (Ga_q3 - Ga_q1);
+        }
+        c.E[comp][P] = e;
+      }
+}
+
+// O2: U* = S_dt(U), Bf* = S_dt(Bf).  `Uin`/`Bin` are modified only in their ghost zones.
+void stage(Ctx& c, Arr Uin[5], Arr Bin[3], double dt, Arr Uout[5], Arr Bout[3]) {
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  for (int n = 0; n < 5; ++n) fill_periodic(c, Uin[n]);
+  if (c.mhd)
+    for (int n = 0; n < 3; ++n) fill_periodic(c, Bin[n]);
+  compute_prims(c, Uin, Bin);
+  for (int d = 0; d < 3; ++d) sweep(c, d, Bin, true);
+  // a5 / Eq. 5: flux divergence; local flux ordering (rho, m_n, m_t1, m_t2, E) -> global momentum
+  const double dtdx = dt / c.dx;
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        const size_t q = c.at(i, j, k);
+        double div[5] = {0, 0, 0, 0, 0};
+        for (int d = 0; d < 3; ++d) {
+          const int a = d, b = (d + 1) % 3, e = (d + 2) % 3;
+          const size_t s = c.st[d];
+          div[0] += c.F[d][0][q + s] - c.F[d][0][q];
+          div[1 + a] += c.F[d][1][q + s] - c.F[d][1][q];
+          div[1 + b] += c.F[d][2][q + s] - c.F[d][2][q];
+          div[1 + e] += c.F[d][3][q + s] - c.F[d][3][q];
+          div[4] += c.F[d][4][q + s] - c.F[d][4][q];
+        }
+        for (int n = 0; n < 5; ++n) Uout[n][q] = Uin[n][q] - dtdx * div[n];
+      }
+  if (!c.mhd) return;
+  for (int comp = 0; comp < 3; ++comp) edge_emf(c, comp);
+  // a7 / O11 / Eq. 6: discrete Stokes theorem on each face
+  const size_t sx = c.st[0], sy = c.st[1], sz = c.st[2];
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        const size_t q = c.at(i, j, k);
+        Bout[0][q] = Bin[0][q] - dtdx * ((c.E[2][q + sy] - c.E[2][q]) - (c.E[1][q + sz] - c.E[1][q]));
+        Bout[1][q] = Bin[1][q] - dtdx * ((c.E[0][q + sz] - c.E[0][q]) - (c.E[2][q + sx] - c.E[2][q]));
+        Bout[2][q] = Bin[2][q] - dtdx * ((c.E[1][q + sx] - c.E[1][q]) - (c.E[0][q + sy] - c.E[0][q]));
+      }
+}
+
+// a9 / O9 / Eq. 10: dt = cfl / max_cells sum_d c_d/dx, c_d = max over the cell's two faces (G8).
+double compute_dt(Ctx& c, double cfl) {
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  for (int n = 0; n < 5; ++n) fill_periodic(c, c.U[n]);
+  if (c.mhd)
+    for (int n = 0; n < 3; ++n) fill_periodic(c, c.Bf[n]);
+  compute_prims(c, c.U, c.Bf);
+  for (int d = 0; d < 3; ++d) sweep(c, d, c.Bf, false);
+  double mx = 0.0;
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        const size_t q = c.at(i, j, k);
+        double s = 0.0;
+        for (int d = 0; d < 3; ++d) s += std::max(c.cf[d][q], c.cf[d][q + c.st[d]]);
+        mx = std::max(mx, s / c.dx);
+      }
+  return cfl / mx;
+}
+
+// a8 / O12 / Eq. 9 with Tab. 1: RK2, w1=1, w1^0=0, w2=w2^0=1/2.
+void step(Ctx& c, double dt) {
+  const int nb = c.mhd ? 3 : 0;
+  for (int n = 0; n < 5; ++n) c.U0[n] = c.U[n];
+  for (int n = 0; n < nb; ++n) c.Bf0[n] = c.Bf[n];
+  stage(c, c.U0, c.Bf0, dt, c.U1, c.Bf1);
+  stage(c, c.U1, c.Bf1, dt, c.Us, c.Bfs);
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        const size_t q = c.at(i, j, k);
+        for (int n = 0; n < 5; ++n) c.U[n][q] = 0.5 * c.U0[n][q] + 0.5 * c.Us[n][q];
+        for (int n = 0; n < nb; ++n) c.Bf[n][q] = 0.5 * c.Bf0[n][q] + 0.5 * c.Bfs[n][q];
+      }
+  c.last_dt = dt;
+}
+
+}  // namespace
+
+// =============================================================================================
+// C ABI (host pointers everywhere).  Layouts as in include/idfx.h: [var][nz][ny][nx], x fastest;
+// bface[d][k][j][i] is the d-component on the LEFT d-face of cell (i,j,k).
+// =============================================================================================
+struct idfxref_ctx {
+  Ctx c;
+};
+
+IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, double gamma, int solver,
+                                        int limiter, int emf_mode) {
+  if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(gamma > 1.0)) return nullptr;
+  if (solver < 0 || solver > 3 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 2) return nullptr;
+  const bool mhd = emf_mode != EMF_NONE;
+  if (mhd && solver == SOLVER_HLLC) return nullptr;
+  if (!mhd && solver == SOLVER_HLLD) return nullptr;
+  idfxref_ctx* h = new idfxref_ctx;
+  Ctx& c = h->c;
+  c.n[0] = nx; c.n[1] = ny; c.n[2] = nz;
+  c.dx = dx; c.g = gamma; c.solver = solver; c.limiter = limiter; c.emf = emf_mode; c.mhd = mhd;
+  for (int d = 0; d < 3; ++d) c.p[d] = c.n[d] + 2 * NG;
+  c.st[0] = 1; c.st[1] = (size_t)c.p[0]; c.st[2] = (size_t)c.p[0] * c.p[1];
+  c.N = c.st[2] * c.p[2];
+  for (int n = 0; n < 5; ++n) {
+    c.U[n].assign(c.N, 0.0); c.U0[n].assign(c.N, 0.0); c.U1[n].assign(c.N, 0.0); c.Us[n].assign(c.N, 0.0);
+  }
+  for (int n = 0; n < 8; ++n) c.V[n].assign(c.N, 0.0);
+  for (int d = 0; d < 3; ++d) {
+    c.Bf[d].assign(c.N, 0.0); c.Bf0[d].assign(c.N, 0.0); c.Bf1[d].assign(c.N, 0.0); c.Bfs[d].assign(c.N, 0.0);
+    for (int n = 0; n < 7; ++n) c.F[d][n].assign(c.N, 0.0);
+    c.cf[d].assign(c.N, 0.0);
+    c.E[d].assign(c.N, 0.0);
+  }
+  c.last_dt = 0.0; c.status = OK; c.roe_fallbacks = 0;
+  return h;
+}
+
+IDFXREF_API void idfxref_destroy(idfxref_ctx* h) { delete h; }
+
+// O1 set_state: Bc from faces, then U from prims.
+IDFXREF_API int idfxref_set_state(idfxref_ctx* h, const double* prim, const double* bface) {
+  if (!h || !prim) return ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  if (c.mhd && !bface) return ERR_INVALID_ARG;
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  const size_t nc = (size_t)nx * ny * nz;
+  if (c.mhd) {
+    for (int d = 0; d < 3; ++d) {
+      for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+          for (int i = 0; i < nx; ++i) c.Bf[d][c.at(i, j, k)] = bface[d * nc + ((size_t)k * ny + j) * nx + i];
+      fill_periodic(c, c.Bf[d]);
+    }
+  }
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        const size_t q = c.at(i, j, k), s = ((size_t)k * ny + j) * nx + i;
+        double bx = 0, by = 0, bz = 0;
+        if (c.mhd) {
+          bx = 0.5 * (c.Bf[0][q] + c.Bf[0][q + c.st[0]]);
+          by = 0.5 * (c.Bf[1][q] + c.Bf[1][q + c.st[1]]);
+          bz = 0.5 * (c.Bf[2][q] + c.Bf[2][q + c.st[2]]);
+        }
+        const double rho = prim[0 * nc + s], vx = prim[1 * nc + s], vy = prim[2 * nc + s], vz = prim[3 * nc + s],
+                     p = prim[4 * nc + s];
+        if (!(rho > 0.0) || !(p > 0.0)) c.status = ERR_UNPHYSICAL;
+        c.U[0][q] = rho; c.U[1][q] = rho * vx; c.U[2][q] = rho * vy; c.U[3][q] = rho * vz;
+        c.U[4][q] = p / (c.g - 1.0) + 0.5 * rho * (vx * vx + vy * vy + vz * vz) + 0.5 * (bx * bx + by * by + bz * bz);
+      }
+  return OK;
+}
+
+IDFXREF_API int idfxref_get_conserved(idfxref_ctx* h, double* cons, double* bface) {
+  if (!h || !cons) return ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  const size_t nc = (size_t)nx * ny * nz;
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        const size_t q = c.at(i, j, k), s = ((size_t)k * ny + j) * nx + i;
+        for (int n = 0; n < 5; ++n) cons[n * nc + s] = c.U[n][q];
+        if (c.mhd && bface)
+          for (int d = 0; d < 3; ++d) bface[d * nc + s] = c.Bf[d][q];
+      }
+  return OK;
+}
+
+IDFXREF_API int idfxref_get_state(idfxref_ctx* h, double* prim, double* bface) {
+  if (!h || !prim) return ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  const size_t nc = (size_t)nx * ny * nz;
+  if (c.mhd)
+    for (int d = 0; d < 3; ++d) fill_periodic(c, c.Bf[d]);
+  compute_prims(c, c.U, c.Bf);
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        const size_t q = c.at(i, j, k), s = ((size_t)k * ny + j) * nx + i;
+        for (int n = 0; n < 5; ++n) prim[n * nc + s] = c.V[n][q];
+        if (c.mhd && bface)
+          for (int d = 0; d < 3; ++d) bface[d * nc + s] = c.Bf[d][q];
+      }
+  return OK;
+}
+
+IDFXREF_API int idfxref_compute_dt(idfxref_ctx* h, double cfl, double* dt_out) {
+  if (!h || !dt_out || !(cfl > 0.0) || !(cfl < 1.0)) return ERR_INVALID_ARG;
+  *dt_out = compute_dt(h->c, cfl);
+  return h->c.status;
+}
+
+IDFXREF_API int idfxref_step(idfxref_ctx* h, double dt) {
+  if (!h || !(dt > 0.0)) return ERR_INVALID_ARG;
+  step(h->c, dt);
+  return h->c.status;
+}
+
+// G9: advance = nsteps x { dt = compute_dt(cfl); step(dt) }, dt evaluated on the current state each time.
+IDFXREF_API int idfxref_advance(idfxref_ctx* h, int nsteps, double cfl) {
+  if (!h || nsteps < 0 || !(cfl > 0.0) || !(cfl < 1.0)) return ERR_INVALID_ARG;
+  for (int s = 0; s < nsteps; ++s) step(h->c, compute_dt(h->c, cfl));
+  return h->c.status;
+}
+
+IDFXREF_API int idfxref_last_dt(const idfxref_ctx* h, double* dt_out) {
+  if (!h || !dt_out) return ERR_INVALID_ARG;
+  *dt_out = h->c.last_dt;
+  return OK;
+}
+
+IDFXREF_API int idfxref_status(const idfxref_ctx* h) { return h ? h->c.status : ERR_INVALID_ARG; }
+IDFXREF_API long long idfxref_roe_fallbacks(const idfxref_ctx* h) { return h ? h->c.roe_fallbacks : -1; }
+
+// Edge EMFs of the most recent stage, emf[c][k][j][i] = E_c at the lower edges of cell (i,j,k)
+// (E_x at (i, j-1/2, k-1/2), E_y at (i-1/2, j, k-1/2), E_z at (i-1/2, j-1/2, k)).
+IDFXREF_API int idfxref_get_emf(const idfxref_ctx* h, double* emf) {
+  if (!h || !emf) return ERR_INVALID_ARG;
+  const Ctx& c = h->c;
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  const size_t nc = (size_t)nx * ny * nz;
+  for (int comp = 0; comp < 3; ++comp)
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) emf[comp * nc + ((size_t)k * ny + j) * nx + i] = c.E[comp][c.at(i, j, k)];
+  return OK;
+}
+
+// Face fluxes of the most recent stage in direction d, flux[n][k][j][i] on the LEFT d-face of cell (i,j,k),
+// local ordering n = (rho, m_n, m_t1, m_t2, E, B_t1, B_t2); cface likewise.
+IDFXREF_API int idfxref_get_flux(const idfxref_ctx* h, int d, double* flux, double* cface) {
+  if (!h || d < 0 || d > 2) return ERR_INVALID_ARG;
+  const Ctx& c = h->c;
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  const size_t nc = (size_t)nx * ny * nz;
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        const size_t q = c.at(i, j, k), s = ((size_t)k * ny + j) * nx + i;
+        if (flux)
+          for (int n = 0; n < 7; ++n) flux[n * nc + s] = c.F[d][n][q];
+        if (cface) cface[s] = c.cf[d][q];
+      }
+  return OK;
+}
+
+// ---- point-wise entry points used only by the pins --------------------------------------------
+IDFXREF_API void idfxref_cons_from_prim(double gamma, const double* W, double Bn, double* U) {
+  cons_from_prim(W, Bn, gamma, U);
+}
+IDFXREF_API void idfxref_phys_flux(double gamma, const double* W, double Bn, double* F) {
+  double U[7];
+  cons_from_prim(W, Bn, gamma, U);
+  phys_flux(W, Bn, U, F);
+}
+// Flux as a function of the conserved vector (for finite-difference Jacobians).
+IDFXREF_API void idfxref_flux_from_cons(double gamma, const double* U, double Bn, double* F) {
+  double W[7];
+  W[0] = U[0]; W[1] = U[1] / U[0]; W[2] = U[2] / U[0]; W[3] = U[3] / U[0];
+  W[5] = U[5]; W[6] = U[6];
+  W[4] = (gamma - 1.0) * (U[4] - 0.5 * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / U[0] -
+                          0.5 * (Bn * Bn + U[5] * U[5] + U[6] * U[6]));
+  phys_flux(W, Bn, U, F);
+}
+IDFXREF_API int idfxref_riemann(int solver, double gamma, const double* WL, const double* WR, double Bn,
+                                double* F, double* cface) {
+  return riemann(solver, gamma, WL, WR, Bn, F, *cface);
+}
+IDFXREF_API void idfxref_wave_speeds(double gamma, const double* WL, const double* WR, double Bn, double* SL,
+                                     double* SR) {
+  davis_speeds(WL, WR, Bn, gamma, *SL, *SR);
+}
+IDFXREF_API double idfxref_slope(int limiter, double dm, double dp) { return slope(limiter, dm, dp); }
+// speeds[3] = (S_L, S*, S_R); states[2][5] = (U*_L, U*_R)
+IDFXREF_API void idfxref_hllc_fan(double gamma, const double* WL, const double* WR, double* speeds,
+                                  double* states) {
+  double UL[7], UR[7], SL, SR;
+  cons_from_prim(WL, 0.0, gamma, UL);
+  cons_from_prim(WR, 0.0, gamma, UR);
+  davis_speeds(WL, WR, 0.0, gamma, SL, SR);
+  HllcFan f;
+  hllc_fan(WL, WR, UL, UR, SL, SR, f);
+  speeds[0] = f.SL; speeds[1] = f.SS; speeds[2] = f.SR;
+  for (int n = 0; n < 5; ++n) { states[n] = f.UsL[n]; states[5 + n] = f.UsR[n]; }
+}
+// speeds[5] = (S_L, S*_L, S_M, S*_R, S_R); states[4][7] = (U*_L, U**_L, U**_R, U*_R)
+IDFXREF_API void idfxref_hlld_fan(double gamma, const double* WL, const double* WR, double Bn, double* speeds,
+                                  double* states) {
+  double UL[7], UR[7], SL, SR;
+  cons_from_prim(WL, Bn, gamma, UL);
+  cons_from_prim(WR, Bn, gamma, UR);
+  davis_speeds(WL, WR, Bn, gamma, SL, SR);
+  HlldFan f;
+  hlld_fan(WL, WR, Bn, UL, UR, SL, SR, f);
+  speeds[0] = f.SL; speeds[1] = f.SsL; speeds[2] = f.SM; speeds[3] = f.SsR; speeds[4] = f.SR;
+  for (int n = 0; n < 7; ++n) {
+    states[n] = f.UsL[n]; states[7 + n] = f.UssL[n]; states[14 + n] = f.UssR[n]; states[21 + n] = f.UsR[n];
+  }
+}
+// lam[7]; Rc[7][7] with Rc[k][:] the k-th right eigenvector in CONSERVED variables (M r_k);
+// Lc[7][7] with Lc[k][:] the k-th left eigenvector in conserved variables (l_k Minv).  Returns 0 if a~^2 <= 0.
+IDFXREF_API int idfxref_roe_system(double gamma, const double* WL, const double* WR, double Bn, double* lam,
+                                   double* Rc, double* Lc) {
+  double UL[7], UR[7];
+  cons_from_prim(WL, Bn, gamma, UL);
+  cons_from_prim(WR, Bn, gamma, UR);
+  RoeSys s;
+  if (!roe_system(WL, WR, Bn, UL, UR, gamma, s)) return 0;
+  for (int k = 0; k < 7; ++k) {
+    lam[k] = s.lam[k];
+    for (int n = 0; n < 7; ++n) {
+      double r = 0.0, l = 0.0;
+      for (int m = 0; m < 7; ++m) {
+        r += s.M[n][m] * s.R[k][m];
+        l += s.L[k][m] * s.Minv[m][n];
+      }
+      Rc[k * 7 + n] = r;
+      Lc[k * 7 + n] = l;
+    }
+  }
+  return 1;
+}
