@@ -1,0 +1,110 @@
+/* idfx.h — C ABI of the B200-native (sm_100a) Godunov HD / ideal-MHD step of IDEFIX
+ * (Lesur et al., arXiv 2304.13746).  Citations "PAPER.md:<line>" refer to the paper text; "O<n>" / "G<n>"
+ * to the written-out formulas and readings in DESIGN.md (same numbering as SURVEY.md §8(c)).
+ *
+ * What one context is: a uniform periodic Cartesian box of nx*ny*nz cells with spacing dx in all three
+ * directions, gamma-law gas, advanced by the explicit RK2 cycle of PAPER.md:130-145 (Eq. 9, Tab. 1):
+ *   cycle:  dt = cfl / max_cells sum_d c_max,d/dx                  (Eq. 10 without eta)
+ *           U1 = S_dt(U0);  U = U0/2 + S_dt(U1)/2                  (Eq. 9, w2 = w2^0 = 1/2)
+ *   S_dt:   periodic ghost fill -> cell-centred B and cons->prim -> PLM reconstruction of primitives to faces
+ *            -> Riemann solver per face -> flux divergence (Eq. 5)
+ *           -> edge EMFs -> constrained-transport update of the face-centred B (Eq. 6).
+ * Every step of that path runs in CUDA kernels of this library; there is no CPU fallback.
+ *
+ * Conventions
+ *   - All arithmetic is IEEE fp64.  No floors are applied (G13): rho <= 0, p <= 0 or NaN met in the
+ *     cons->prim conversion raises a sticky device flag reported as IDFX_ERR_UNPHYSICAL.
+ *   - Array layout: structure of arrays, [var][nz][ny][nx] contiguous, x fastest, no padding.
+ *       prim  : [5] = rho, vx, vy, vz, p           cons : [5] = rho, mx, my, mz, E
+ *       bface : [3]; bface[d][k][j][i] is B_d on the LEFT d-face of cell (i,j,k), i.e. B_x at (i-1/2, j, k).
+ *               Periodic, so face n coincides with face 0 and every component has nx*ny*nz entries.
+ *     The caller must supply a discretely divergence-free bface; the library never cleans it, and its
+ *     CT update keeps the discrete divergence at round-off.
+ *   - E = p/(gamma-1) + rho v^2/2 + Bc^2/2 with Bc the mean of the two bounding faces (G1).
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers (pageable or pinned).
+ *   - Ownership: the caller owns every buffer it passes, including the workspace (allocate it with
+ *     whatever owns device memory in the application, e.g. a torch tensor).  The context owns no large
+ *     device allocation; it owns CUDA graphs, TMA descriptors and a few hundred bytes of host memory.
+ *   - All work is enqueued on the stream given to idfx_bind (a cudaStream_t cast to void*, NULL = legacy
+ *     default stream).  Only idfx_compute_dt, idfx_last_dt, idfx_status, idfx_get_state_host and
+ *     idfx_launch_count synchronise with the host.
+ *   - Errors: every int-returning call returns IDFX_OK or a negative code; nothing throws or aborts.
+ *     idfx_last_error() gives a thread-local message for the last failure.
+ */
+#ifndef IDFX_H
+#define IDFX_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct idfx_ctx idfx_ctx;
+
+/* Riemann solvers.  HLLC is hydrodynamics-only; in MHD it is replaced by HLLD. */
+enum { IDFX_SOLVER_HLL = 0, IDFX_SOLVER_HLLC = 1, IDFX_SOLVER_HLLD = 2, IDFX_SOLVER_ROE = 3 };
+/* Reconstruction: flat (1st order), PLM with minmod or van Leer (harmonic mean, G2) slopes. */
+enum { IDFX_LIMITER_FLAT = 0, IDFX_LIMITER_MINMOD = 1, IDFX_LIMITER_VANLEER = 2 };
+/* EMF reconstruction.  IDFX_EMF_NONE selects hydrodynamics (no magnetic field at all). */
+enum { IDFX_EMF_NONE = 0, IDFX_EMF_ARITHMETIC = 1, IDFX_EMF_UCT_CONTACT = 2 };
+enum {
+  IDFX_OK = 0,
+  IDFX_ERR_INVALID_ARG = -1,
+  IDFX_ERR_UNSUPPORTED = -2, /* solver / emf_mode combination that does not exist (HLLC+MHD, HLLD+HD) */
+  IDFX_ERR_NOT_BOUND = -3,   /* call needs idfx_bind first */
+  IDFX_ERR_CUDA = -4,        /* a CUDA runtime call failed; see idfx_last_error() */
+  IDFX_ERR_UNPHYSICAL = -5   /* sticky: rho <= 0 or p <= 0 or NaN was met on the device */
+};
+
+/* Creates a context.  Requirements: nx, ny, nz >= 4; dx > 0; gamma > 1; valid enums; HD (emf_mode NONE)
+ * with HLL/HLLC/ROE, MHD with HLL/HLLD/ROE.  Returns NULL on error (idfx_last_error() says why).
+ * Host-only: touches no device memory. */
+idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solver, int limiter, int emf_mode);
+
+/* Device bytes the caller must supply to idfx_bind (internal padded state, stage buffers, fluxes, EMFs). */
+size_t idfx_workspace_bytes(const idfx_ctx* ctx);
+
+/* Binds a caller-owned device workspace (>= idfx_workspace_bytes, 256-byte aligned) and a stream.
+ * Zeroes the workspace on that stream.  Must precede every call below. */
+int idfx_bind(idfx_ctx* ctx, void* d_workspace, size_t bytes, void* cuda_stream);
+
+/* Copy-in of the state (O1): Bc from faces, then conserved variables from the primitives.
+ * d_bface may be NULL only when emf_mode is NONE (it is ignored then). */
+int idfx_set_state(idfx_ctx* ctx, const double* d_prim, const double* d_bface);
+int idfx_set_state_host(idfx_ctx* ctx, const double* h_prim, const double* h_bface);
+
+/* Copy-out: primitives re-derived from the conserved state and the face field; bface bit-exact. */
+int idfx_get_state(idfx_ctx* ctx, double* d_prim, double* d_bface);
+int idfx_get_state_host(idfx_ctx* ctx, double* h_prim, double* h_bface); /* synchronises */
+/* Copy-out of the master state as it is stored: conserved cell variables and face B. */
+int idfx_get_conserved(idfx_ctx* ctx, double* d_cons, double* d_bface);
+
+/* dt of Eq. 10 on the CURRENT state (O9): cfl / max_cells [ sum_d c_d / dx ], with c_d of a
+ * cell the larger c_face of its two d-faces (G8) and c_face = max(|S_L|,|S_R|) of the Davis estimate (G5).
+ * 0 < cfl < 1.  Writes *h_dt_out; synchronises. */
+int idfx_compute_dt(idfx_ctx* ctx, double cfl, double* h_dt_out);
+
+/* One RK2 cycle with the given dt > 0 (O12). */
+int idfx_step(idfx_ctx* ctx, double dt);
+
+/* nsteps cycles, each with dt evaluated on the state at the start of that cycle (G9); dt never leaves the
+ * device.  Equivalent to nsteps x { idfx_compute_dt; idfx_step }. */
+int idfx_advance(idfx_ctx* ctx, int nsteps, double cfl);
+
+/* dt used by the most recent cycle (synchronises). */
+int idfx_last_dt(idfx_ctx* ctx, double* h_dt_out);
+
+/* Synchronises; IDFX_OK, IDFX_ERR_UNPHYSICAL (sticky device flag) or IDFX_ERR_CUDA. */
+int idfx_status(idfx_ctx* ctx);
+
+/* Number of kernels of this library launched on behalf of ctx since idfx_bind (graph replays included). */
+long long idfx_launch_count(const idfx_ctx* ctx);
+
+const char* idfx_last_error(void);
+void idfx_destroy(idfx_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IDFX_H */

@@ -1,0 +1,913 @@
+// idfx.cu — kernels and C ABI of the idfx CUDA path (sm_100a, fp64).  Interface: include/idfx.h.
+//
+// Data layout in HBM: structure of arrays; every field is a padded box
+// [nz+4][ny+4][pitch] doubles with 2 ghost layers in y and z and, in x, the active cells starting at
+// column IOFF = 16 (a 128-byte boundary) with ghost columns 14,15 and nx+16,nx+17; pitch is a multiple of
+// 16 doubles.  All fields live in the caller's workspace.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/idfx.h"
+#include "physics.cuh"
+
+namespace idfx {
+
+constexpr int NG = 2;
+constexpr int IOFF = 16;
+
+struct Geom {
+  int nx, ny, nz;
+  int sy;         // row pitch in doubles
+  long long sz;   // plane stride in doubles
+  long long np;   // padded field size in doubles
+  long long nc;   // nx*ny*nz
+  double dx, gamma;
+  __host__ __device__ __forceinline__ long long at(int i, int j, int k) const {
+    return (long long)(k + NG) * sz + (long long)(j + NG) * sy + (i + IOFF);
+  }
+};
+
+// flat thread index -> active cell
+__device__ __forceinline__ bool cell_of_thread(const Geom& g, int& i, int& j, int& k) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= g.nc) return false;
+  i = (int)(t % g.nx);
+  const long long r = t / g.nx;
+  j = (int)(r % g.ny);
+  k = (int)(r / g.ny);
+  return true;
+}
+
+struct DevScalars {
+  unsigned long long smax_bits;  // bit pattern of max_cells sum_d c_d/dx (positive doubles order like integers)
+  double dt_used;
+  int flag;
+};
+
+// ---------------------------------------------------------------------------------------------
+// copy-in / copy-out between the caller's contiguous arrays and the padded fields
+// ---------------------------------------------------------------------------------------------
+struct FieldList {
+  double* f[11];
+  int n;
+};
+
+__global__ void k_pack(Geom g, FieldList dst, const double* __restrict__ src) {
+  int i, j, k;
+  if (!cell_of_thread(g, i, j, k)) return;
+  const long long c = g.at(i, j, k);
+  const long long s = ((long long)k * g.ny + j) * g.nx + i;
+  for (int n = 0; n < dst.n; ++n) dst.f[n][c] = src[n * g.nc + s];
+}
+
+__global__ void k_unpack(Geom g, FieldList srcf, double* __restrict__ dst) {
+  int i, j, k;
+  if (!cell_of_thread(g, i, j, k)) return;
+  const long long c = g.at(i, j, k);
+  const long long s = ((long long)k * g.ny + j) * g.nx + i;
+  for (int n = 0; n < srcf.n; ++n) dst[n * g.nc + s] = srcf.f[n][c];
+}
+
+// a1: periodic ghost fill of a list of fields, one thread per ghost cell.  Every ghost cell copies from its
+// wrapped active image, which equals the sequential x, y, z fill of O2 (i).
+__global__ void k_fill_ghost(Geom g, FieldList fl) {
+  const int px = g.nx + 2 * NG, py = g.ny + 2 * NG;
+  const long long nZ = 2LL * NG * py * px;             // k in ghost
+  const long long nY = (long long)g.nz * 2 * NG * px;  // k active, j in ghost
+  const long long nX = (long long)g.nz * g.ny * 2 * NG;
+  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  int i, j, k;
+  if (t < nZ) {
+    i = (int)(t % px) - NG;
+    const long long r = t / px;
+    j = (int)(r % py) - NG;
+    const int kk = (int)(r / py);
+    k = kk < NG ? kk - NG : g.nz + kk - NG;
+  } else if ((t -= nZ) < nY) {
+    i = (int)(t % px) - NG;
+    const long long r = t / px;
+    const int jj = (int)(r % (2 * NG));
+    j = jj < NG ? jj - NG : g.ny + jj - NG;
+    k = (int)(r / (2 * NG));
+  } else if ((t -= nY) < nX) {
+    const int ii = (int)(t % (2 * NG));
+    i = ii < NG ? ii - NG : g.nx + ii - NG;
+    const long long r = t / (2 * NG);
+    j = (int)(r % g.ny);
+    k = (int)(r / g.ny);
+  } else {
+    return;
+  }
+  const int is = (i + g.nx) % g.nx, js = (j + g.ny) % g.ny, ks = (k + g.nz) % g.nz;
+  const long long d = g.at(i, j, k), s = g.at(is, js, ks);
+  for (int n = 0; n < fl.n; ++n) fl.f[n][d] = fl.f[n][s];
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2: cell-centred B and cons <-> prim
+// ---------------------------------------------------------------------------------------------
+struct StateArgs {
+  double* U[5];
+  double* V[8];
+  const double* Bf[3];
+  DevScalars* sc;
+};
+
+// set_state (O1): V[0..4] hold the primitives; writes Bc into V[5..7] and the conserved state into U.
+template <bool MHD>
+__global__ void k_cons_from_prim(Geom g, StateArgs a) {
+  int i, j, k;
+  if (!cell_of_thread(g, i, j, k)) return;
+  const long long c = g.at(i, j, k);
+  double bx = 0.0, by = 0.0, bz = 0.0;
+  if (MHD) {
+    // right faces through the periodic image (face ghosts are not filled yet)
+    bx = 0.5 * (a.Bf[0][c] + a.Bf[0][g.at(i + 1 == g.nx ? 0 : i + 1, j, k)]);
+    by = 0.5 * (a.Bf[1][c] + a.Bf[1][g.at(i, j + 1 == g.ny ? 0 : j + 1, k)]);
+    bz = 0.5 * (a.Bf[2][c] + a.Bf[2][g.at(i, j, k + 1 == g.nz ? 0 : k + 1)]);
+    a.V[5][c] = bx;
+    a.V[6][c] = by;
+    a.V[7][c] = bz;
+  }
+  const double rho = a.V[0][c], vx = a.V[1][c], vy = a.V[2][c], vz = a.V[3][c], p = a.V[4][c];
+  if (!(rho > 0.0) || !(p > 0.0)) a.sc->flag = 1;
+  a.U[0][c] = rho;
+  a.U[1][c] = rho * vx;
+  a.U[2][c] = rho * vy;
+  a.U[3][c] = rho * vz;
+  a.U[4][c] = p / (g.gamma - 1.0) + 0.5 * rho * (vx * vx + vy * vy + vz * vz) + 0.5 * (bx * bx + by * by + bz * bz);
+}
+
+__device__ __forceinline__ void prim_from_cons(double gm1, double rho, double mx, double my, double mz, double E,
+                                               double bx, double by, double bz, double& vx, double& vy, double& vz,
+                                               double& p) {
+  const double ir = 1.0 / rho;
+  vx = mx * ir;
+  vy = my * ir;
+  vz = mz * ir;
+  p = gm1 * (E - 0.5 * rho * (vx * vx + vy * vy + vz * vz) - 0.5 * (bx * bx + by * by + bz * bz));
+}
+
+// get_state: primitives from the master state (Bf ghosts are valid whenever this runs).
+template <bool MHD>
+__global__ void k_prim_from_cons(Geom g, StateArgs a) {
+  int i, j, k;
+  if (!cell_of_thread(g, i, j, k)) return;
+  const long long c = g.at(i, j, k);
+  double bx = 0.0, by = 0.0, bz = 0.0;
+  if (MHD) {
+    bx = 0.5 * (a.Bf[0][c] + a.Bf[0][c + 1]);
+    by = 0.5 * (a.Bf[1][c] + a.Bf[1][c + g.sy]);
+    bz = 0.5 * (a.Bf[2][c] + a.Bf[2][c + g.sz]);
+    a.V[5][c] = bx;
+    a.V[6][c] = by;
+    a.V[7][c] = bz;
+  }
+  double vx, vy, vz, p;
+  const double rho = a.U[0][c];
+  prim_from_cons(g.gamma - 1.0, rho, a.U[1][c], a.U[2][c], a.U[3][c], a.U[4][c], bx, by, bz, vx, vy, vz, p);
+  a.V[0][c] = rho;
+  a.V[1][c] = vx;
+  a.V[2][c] = vy;
+  a.V[3][c] = vz;
+  a.V[4][c] = p;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3 + a4: reconstruct -> Riemann -> flux on the left face of every active cell, one direction.
+// q[] are the primitive fields permuted for the sweep direction (rho, u, v, w, p, B_t1, B_t2), bn the
+// staggered normal field, sd the stride along the sweep.  Faces in the ghost layers are never computed:
+// they are periodic images of these and consumers wrap their indices instead.
+// ---------------------------------------------------------------------------------------------
+struct FluxArgs {
+  const double* q[7];
+  const double* bn;
+  long long sd;
+  double* F[7];  // local ordering (rho, m_n, m_t1, m_t2, E, B_t1, B_t2); F[5], F[6] unused in HD
+  double* cf;    // c_face
+};
+
+template <int SOLVER, int LIM, bool MHD, bool SPEED_ONLY>
+__global__ void __launch_bounds__(128) k_flux_face(Geom g, FluxArgs a) {
+  int i, j, k;
+  if (!cell_of_thread(g, i, j, k)) return;
+  const long long c = g.at(i, j, k);
+  constexpr int NQ = MHD ? 7 : 5;
+  double WL[7], WR[7];
+#pragma unroll
+  for (int n = 0; n < NQ; ++n) {
+    const double* __restrict__ q = a.q[n];
+    const double qm2 = q[c - 2 * a.sd], qm1 = q[c - a.sd], q0 = q[c], qp1 = q[c + a.sd];
+    const double sm = limited_slope<LIM>(qm1 - qm2, q0 - qm1);
+    const double s0 = limited_slope<LIM>(q0 - qm1, qp1 - q0);
+    WL[n] = qm1 + 0.5 * sm;
+    WR[n] = q0 - 0.5 * s0;
+  }
+  if (!MHD) WL[5] = WL[6] = WR[5] = WR[6] = 0.0;
+  const double Bn = MHD ? a.bn[c] : 0.0;  // G3
+  if (SPEED_ONLY) {
+    double SL, SR;
+    outer_speeds<MHD>(WL, WR, Bn, g.gamma, SL, SR);
+    a.cf[c] = fmax(fabs(SL), fabs(SR));
+  } else {
+    double F[7];
+    a.cf[c] = riemann<SOLVER, MHD>(WL, WR, Bn, g.gamma, F);
+#pragma unroll
+    for (int n = 0; n < NQ; ++n) a.F[n][c] = F[n];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5: flux divergence R = sum_d [F_d(i+1/2) - F_d(i-1/2)] (Eq. 5); a9: block max of sum_d c_d/dx
+// ---------------------------------------------------------------------------------------------
+struct RhsArgs {
+  const double* F[3][5];
+  const double* cf[3];
+  double* R[5];
+  DevScalars* sc;
+};
+
+__device__ __forceinline__ double block_max_128(double v) {
+  __shared__ double red[4];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  return fmax(fmax(red[0], red[1]), fmax(red[2], red[3]));
+}
+
+template <bool WANT_R, bool WANT_DT>
+__global__ void __launch_bounds__(128) k_rhs(Geom g, RhsArgs a) {
+  int i, j, k;
+  const bool active = cell_of_thread(g, i, j, k);
+  double s = 0.0;
+  if (active) {
+    const long long c = g.at(i, j, k);
+    const long long cp[3] = {g.at(i + 1 == g.nx ? 0 : i + 1, j, k), g.at(i, j + 1 == g.ny ? 0 : j + 1, k),
+                             g.at(i, j, k + 1 == g.nz ? 0 : k + 1)};
+    if (WANT_R) {
+      double r[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        r[0] += a.F[d][0][cp[d]] - a.F[d][0][c];
+        r[1 + d] += a.F[d][1][cp[d]] - a.F[d][1][c];
+        r[1 + (d + 1) % 3] += a.F[d][2][cp[d]] - a.F[d][2][c];
+        r[1 + (d + 2) % 3] += a.F[d][3][cp[d]] - a.F[d][3][c];
+        r[4] += a.F[d][4][cp[d]] - a.F[d][4][c];
+      }
+#pragma unroll
+      for (int n = 0; n < 5; ++n) a.R[n][c] = r[n];
+    }
+    if (WANT_DT) {
+#pragma unroll
+      for (int d = 0; d < 3; ++d) s += fmax(a.cf[d][c], a.cf[d][cp[d]]);  // G8
+      s /= g.dx;
+    }
+  }
+  if (WANT_DT) {
+    const double m = block_max_128(s);
+    if (threadIdx.x == 0) atomicMax(&a.sc->smax_bits, (unsigned long long)__double_as_longlong(m));
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a6: edge EMFs (O10).  Thread (i,j,k) owns the three lower edges of its cell:
+//   E[0] = E_x(i, j-1/2, k-1/2), E[1] = E_y(i-1/2, j, k-1/2), E[2] = E_z(i-1/2, j-1/2, k).
+// For component c with (a,b,c) cyclic:  E_c^(a) = -F_a[B_b] = -FB[a][0],  E_c^(b) = +F_b[B_a] = +FB[b][1].
+// ---------------------------------------------------------------------------------------------
+struct EmfArgs {
+  const double* FB[3][2];  // FB[d][0] = F_d[B_t1], FB[d][1] = F_d[B_t2] on the left d-faces
+  const double* FM[3];     // mass flux F_d[rho]
+  const double* v[3];
+  const double* Bc[3];
+  double* E[3];
+};
+
+template <bool UCT>
+__global__ void __launch_bounds__(128) k_emf(Geom g, EmfArgs a) {
+  int idx[3];
+  if (!cell_of_thread(g, idx[0], idx[1], idx[2])) return;
+  const int n[3] = {g.nx, g.ny, g.nz};
+  const long long st[3] = {1, g.sy, g.sz};
+  const long long P = g.at(idx[0], idx[1], idx[2]);
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const int ia = (c + 1) % 3, ib = (c + 2) % 3;
+    // periodic images of the neighbours one step down in a and in b (flux arrays have no ghosts)
+    const long long da = idx[ia] == 0 ? (long long)(n[ia] - 1) * st[ia] : -st[ia];
+    const long long db = idx[ib] == 0 ? (long long)(n[ib] - 1) * st[ib] : -st[ib];
+    const double* __restrict__ Fa = a.FB[ia][0];
+    const double* __restrict__ Fb = a.FB[ib][1];
+    const double EaP = -Fa[P], EaPb = -Fa[P + db];  // a-faces at (ia-1/2, ib) and (ia-1/2, ib-1)
+    const double EbP = Fb[P], EbPa = Fb[P + da];    // b-faces at (ia, ib-1/2) and (ia-1, ib-1/2)
+    double e = 0.25 * (EaP + EaPb + EbP + EbPa);
+    if (UCT) {
+      // cell-centred reference EMF -(v x B)_c = v_b B_a - v_a B_b from the stage-input primitives (G10);
+      // V has ghosts, so plain offsets
+      const double* __restrict__ va = a.v[ia];
+      const double* __restrict__ vb = a.v[ib];
+      const double* __restrict__ Ba = a.Bc[ia];
+      const double* __restrict__ Bb = a.Bc[ib];
+      const long long Qa = P - st[ia], Qb = P - st[ib], Qab = P - st[ia] - st[ib];
+      const double Ec = vb[P] * Ba[P] - va[P] * Bb[P];
+      const double Eca = vb[Qa] * Ba[Qa] - va[Qa] * Bb[Qa];
+      const double Ecb = vb[Qb] * Ba[Qb] - va[Qb] * Bb[Qb];
+      const double Ecab = vb[Qab] * Ba[Qab] - va[Qab] * Bb[Qab];
+      const double fa = a.FM[ia][P], fab = a.FM[ia][P + db];  // mass flux through the two a-faces
+      const double fb = a.FM[ib][P], fba = a.FM[ib][P + da];  // and the two b-faces
+      // d/db on the a-face, quarter points ib-1/4 (cells P-a | P) and ib-3/4 (cells P-a-b | P-b)
+      const double gbp_m = 2.0 * (Eca - EbPa), gbp_p = 2.0 * (Ec - EbP);
+      const double gbm_m = 2.0 * (EbPa - Ecab), gbm_p = 2.0 * (EbP - Ecb);
+      const double Gb1 = fa > 0.0 ? gbp_m : (fa < 0.0 ? gbp_p : 0.5 * (gbp_m + gbp_p));
+      const double Gb3 = fab > 0.0 ? gbm_m : (fab < 0.0 ? gbm_p : 0.5 * (gbm_m + gbm_p));
+      // d/da on the b-face, quarter points ia-1/4 (cells P-b | P) and ia-3/4 (cells P-a-b | P-a)
+      const double gap_m = 2.0 * (Ecb - EaPb), gap_p = 2.0 * (Ec - EaP);
+      const double gam_m = 2.0 * (EaPb - Ecab), gam_p = 2.0 * (EaP - Eca);
+      const double Ga1 = fb > 0.0 ? gap_m : (fb < 0.0 ? gap_p : 0.5 * (gap_m + gap_p));
+      const double Ga3 = fba > 0.0 ? gam_m : (fba < 0.0 ? gam_p : 0.5 * (gam_m + gam_p));
+      e += 0.125 * (Gb3 - Gb1) + 0.125 * (Ga3 - Ga1);
+    }
+    a.E[c][P] = e;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5 (apply) + a7 (CT, Eq. 6) + a8 (RK2 combine, Eq. 9) + a2 (cons->prim of the result), one pass.
+// Stage 1: Unew = U0 - dt/dx R.  Stage 2: Unew = U0/2 + (U1 - dt/dx R)/2; same for the face field.
+// The thread also evaluates the CT update of its cell's three RIGHT faces (owned by the neighbours) so
+// that the cell-centred field of the new state is available without another pass.
+// ---------------------------------------------------------------------------------------------
+struct UpdateArgs {
+  const double* Uin[5];   // state the stage started from (U0 in stage 1, U1 in stage 2)
+  const double* U0[5];    // saved state (stage 2 only)
+  const double* R[5];
+  double* Uout[5];
+  const double* Bin[3];   // ghosts filled
+  const double* B0[3];    // ghosts filled (stage 2 only)
+  const double* E[3];     // active lower edges only
+  double* Bout[3];
+  double* V[8];
+  DevScalars* sc;
+  double dt_fixed;        // > 0: use it; otherwise dt = cfl / smax
+  double cfl;
+};
+
+template <bool MHD, bool STAGE2>
+__global__ void __launch_bounds__(128) k_update(Geom g, UpdateArgs a) {
+  int i, j, k;
+  if (!cell_of_thread(g, i, j, k)) return;
+  const long long c = g.at(i, j, k);
+  double dt = a.dt_fixed;
+  if (!(dt > 0.0)) dt = a.cfl / __longlong_as_double((long long)a.sc->smax_bits);
+  if (!STAGE2 && blockIdx.x == 0 && threadIdx.x == 0) a.sc->dt_used = dt;
+  const double dtdx = dt / g.dx;
+
+  double u[5];
+#pragma unroll
+  for (int n = 0; n < 5; ++n) {
+    const double us = a.Uin[n][c] - dtdx * a.R[n][c];
+    u[n] = STAGE2 ? 0.5 * a.U0[n][c] + 0.5 * us : us;
+    a.Uout[n][c] = u[n];
+  }
+  double bc[3] = {0.0, 0.0, 0.0};
+  if (MHD) {
+    const int ip = i + 1 == g.nx ? 0 : i + 1, jp = j + 1 == g.ny ? 0 : j + 1, kp = k + 1 == g.nz ? 0 : k + 1;
+    // edge values on the 2x2x2 corner box of the cell (periodic images on the upper side)
+    auto Ex = [&](int jj, int kk) { return a.E[0][g.at(i, jj, kk)]; };
+    auto Ey = [&](int ii, int kk) { return a.E[1][g.at(ii, j, kk)]; };
+    auto Ez = [&](int ii, int jj) { return a.E[2][g.at(ii, jj, k)]; };
+    const double ex00 = Ex(j, k), ex10 = Ex(jp, k), ex01 = Ex(j, kp), ex11 = Ex(jp, kp);
+    const double ey00 = Ey(i, k), ey10 = Ey(ip, k), ey01 = Ey(i, kp), ey11 = Ey(ip, kp);
+    const double ez00 = Ez(i, j), ez10 = Ez(ip, j), ez01 = Ez(i, jp), ez11 = Ez(ip, jp);
+    // O11, left faces then right faces
+    const double cxl = (ez01 - ez00) - (ey01 - ey00), cxr = (ez11 - ez10) - (ey11 - ey10);
+    const double cyl = (ex01 - ex00) - (ez10 - ez00), cyr = (ex11 - ex10) - (ez11 - ez01);
+    const double czl = (ey10 - ey00) - (ex10 - ex00), czr = (ey11 - ey01) - (ex11 - ex01);
+    const double curlL[3] = {cxl, cyl, czl}, curlR[3] = {cxr, cyr, czr};
+    const long long st[3] = {1, g.sy, g.sz};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      double bl = a.Bin[d][c] - dtdx * curlL[d];
+      double br = a.Bin[d][c + st[d]] - dtdx * curlR[d];
+      if (STAGE2) {
+        bl = 0.5 * a.B0[d][c] + 0.5 * bl;
+        br = 0.5 * a.B0[d][c + st[d]] + 0.5 * br;
+      }
+      a.Bout[d][c] = bl;
+      bc[d] = 0.5 * (bl + br);
+      a.V[5 + d][c] = bc[d];
+    }
+  }
+  double vx, vy, vz, p;
+  prim_from_cons(g.gamma - 1.0, u[0], u[1], u[2], u[3], u[4], bc[0], bc[1], bc[2], vx, vy, vz, p);
+  if (!(u[0] > 0.0) || !(p > 0.0)) a.sc->flag = 1;
+  a.V[0][c] = u[0];
+  a.V[1][c] = vx;
+  a.V[2][c] = vy;
+  a.V[3][c] = vz;
+  a.V[4][c] = p;
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+thread_local char g_err[512] = "";
+
+void set_err(const char* fmt, const char* a = "", const char* b = "") { snprintf(g_err, sizeof(g_err), fmt, a, b); }
+
+// field slots in the workspace
+enum {
+  F_UA = 0,    // 5: conserved state at the start of the cycle (and its result)
+  F_UB = 5,    // 5: stage-1 state
+  F_BA = 10,   // 3 x 3: face-field buffers that rotate between B0 / B1 / result
+  F_BB = 13,
+  F_BC = 16,
+  F_V = 19,    // 8: primitives + cell-centred B of the stage input
+  F_R = 27,    // 5: flux divergence
+  F_FB = 32,   // 6: face fluxes of B, [d][0..1]
+  F_E = 38,    // 3: edge EMFs
+  F_FH = 41,   // 15: face fluxes of (rho, m, E), [d][0..4]
+  F_CF = 56,   // 3: c_face
+  F_COUNT = 59
+};
+
+}  // namespace idfx
+
+using namespace idfx;
+
+struct idfx_ctx {
+  Geom g;
+  int solver, limiter, emf;
+  bool mhd;
+  double* ws = nullptr;
+  size_t ws_bytes = 0;
+  cudaStream_t stream = nullptr;
+  bool bound = false;
+  DevScalars* sc = nullptr;
+  int bcur = 0;  // which of the three face-field buffers holds the current state
+  long long launches = 0;
+  double* field(int slot) const { return ws + (size_t)slot * (size_t)g.np; }
+  double* bbuf(int which, int d) const { return field(F_BA + 3 * which + d); }
+};
+
+#define CK(call)                                                          \
+  do {                                                                    \
+    cudaError_t e_ = (call);                                              \
+    if (e_ != cudaSuccess) {                                              \
+      set_err("CUDA error: %s at %s", cudaGetErrorString(e_), #call);     \
+      return IDFX_ERR_CUDA;                                               \
+    }                                                                     \
+  } while (0)
+
+namespace {
+
+inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+
+int check_bound(const idfx_ctx* c) {
+  if (!c) {
+    set_err("null context");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  if (!c->bound) {
+    set_err("context has no workspace: call idfx_bind first");
+    return IDFX_ERR_NOT_BOUND;
+  }
+  return IDFX_OK;
+}
+
+template <int SOLVER, int LIM, bool MHD>
+void launch_flux_sl(idfx_ctx* c, const FluxArgs& a, bool speed_only) {
+  const unsigned nb = blocks_for(c->g.nc, 128);
+  if (speed_only)
+    k_flux_face<SOLVER, LIM, MHD, true><<<nb, 128, 0, c->stream>>>(c->g, a);
+  else
+    k_flux_face<SOLVER, LIM, MHD, false><<<nb, 128, 0, c->stream>>>(c->g, a);
+}
+
+template <int SOLVER, bool MHD>
+void launch_flux_s(idfx_ctx* c, const FluxArgs& a, bool speed_only) {
+  switch (c->limiter) {
+    case LIM_FLAT: launch_flux_sl<SOLVER, LIM_FLAT, MHD>(c, a, speed_only); break;
+    case LIM_MINMOD: launch_flux_sl<SOLVER, LIM_MINMOD, MHD>(c, a, speed_only); break;
+    default: launch_flux_sl<SOLVER, LIM_VANLEER, MHD>(c, a, speed_only);
+  }
+}
+
+void launch_flux(idfx_ctx* c, int d, const double* const Bf[3], bool speed_only) {
+  const int ia = d, ib = (d + 1) % 3, ie = (d + 2) % 3;
+  const long long st[3] = {1, c->g.sy, c->g.sz};
+  FluxArgs a;
+  double* V = c->field(F_V);
+  const long long np = c->g.np;
+  a.q[0] = V;
+  a.q[1] = V + (1 + ia) * np;
+  a.q[2] = V + (1 + ib) * np;
+  a.q[3] = V + (1 + ie) * np;
+  a.q[4] = V + 4 * np;
+  a.q[5] = V + (5 + ib) * np;
+  a.q[6] = V + (5 + ie) * np;
+  a.bn = c->mhd ? Bf[ia] : nullptr;
+  a.sd = st[d];
+  for (int n = 0; n < 5; ++n) a.F[n] = c->field(F_FH + 5 * d + n);
+  a.F[5] = c->field(F_FB + 2 * d);
+  a.F[6] = c->field(F_FB + 2 * d + 1);
+  a.cf = c->field(F_CF + d);
+  if (c->mhd) {
+    if (c->solver == SOLVER_HLL) launch_flux_s<SOLVER_HLL, true>(c, a, speed_only);
+    else if (c->solver == SOLVER_HLLD) launch_flux_s<SOLVER_HLLD, true>(c, a, speed_only);
+    else launch_flux_s<SOLVER_ROE, true>(c, a, speed_only);
+  } else {
+    if (c->solver == SOLVER_HLL) launch_flux_s<SOLVER_HLL, false>(c, a, speed_only);
+    else if (c->solver == SOLVER_HLLC) launch_flux_s<SOLVER_HLLC, false>(c, a, speed_only);
+    else launch_flux_s<SOLVER_ROE, false>(c, a, speed_only);
+  }
+  c->launches++;
+}
+
+void launch_rhs(idfx_ctx* c, bool want_r, bool want_dt) {
+  RhsArgs a;
+  for (int d = 0; d < 3; ++d) {
+    for (int n = 0; n < 5; ++n) a.F[d][n] = c->field(F_FH + 5 * d + n);
+    a.cf[d] = c->field(F_CF + d);
+  }
+  for (int n = 0; n < 5; ++n) a.R[n] = c->field(F_R + n);
+  a.sc = c->sc;
+  const unsigned nb = blocks_for(c->g.nc, 128);
+  if (want_r && want_dt) k_rhs<true, true><<<nb, 128, 0, c->stream>>>(c->g, a);
+  else if (want_r) k_rhs<true, false><<<nb, 128, 0, c->stream>>>(c->g, a);
+  else k_rhs<false, true><<<nb, 128, 0, c->stream>>>(c->g, a);
+  c->launches++;
+}
+
+void launch_emf(idfx_ctx* c) {
+  EmfArgs a;
+  for (int d = 0; d < 3; ++d) {
+    a.FB[d][0] = c->field(F_FB + 2 * d);
+    a.FB[d][1] = c->field(F_FB + 2 * d + 1);
+    a.FM[d] = c->field(F_FH + 5 * d);
+    a.v[d] = c->field(F_V + 1 + d);
+    a.Bc[d] = c->field(F_V + 5 + d);
+    a.E[d] = c->field(F_E + d);
+  }
+  const unsigned nb = blocks_for(c->g.nc, 128);
+  if (c->emf == EMF_UCT) k_emf<true><<<nb, 128, 0, c->stream>>>(c->g, a);
+  else k_emf<false><<<nb, 128, 0, c->stream>>>(c->g, a);
+  c->launches++;
+}
+
+void launch_fill(idfx_ctx* c, int which_b) {
+  FieldList fl;
+  fl.n = 0;
+  for (int n = 0; n < (c->mhd ? 8 : 5); ++n) fl.f[fl.n++] = c->field(F_V + n);
+  if (c->mhd)
+    for (int d = 0; d < 3; ++d) fl.f[fl.n++] = c->bbuf(which_b, d);
+  const Geom& g = c->g;
+  const long long px = g.nx + 2 * NG, py = g.ny + 2 * NG;
+  const long long nt = 2LL * NG * py * px + (long long)g.nz * 2 * NG * px + (long long)g.nz * g.ny * 2 * NG;
+  k_fill_ghost<<<blocks_for(nt, 128), 128, 0, c->stream>>>(g, fl);
+  c->launches++;
+}
+
+// One stage S_dt (O2) followed by the RK combine.  bin: face buffer of the stage input; b0: saved face
+// buffer; bout: destination.
+void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fixed, double cfl, bool want_dt) {
+  const double* Bf[3] = {c->bbuf(bin, 0), c->bbuf(bin, 1), c->bbuf(bin, 2)};
+  for (int d = 0; d < 3; ++d) launch_flux(c, d, Bf, false);
+  launch_rhs(c, true, want_dt);
+  if (c->mhd) launch_emf(c);
+  UpdateArgs a;
+  for (int n = 0; n < 5; ++n) {
+    a.Uin[n] = c->field((stage2 ? F_UB : F_UA) + n);
+    a.U0[n] = c->field(F_UA + n);
+    a.R[n] = c->field(F_R + n);
+    a.Uout[n] = c->field((stage2 ? F_UA : F_UB) + n);
+  }
+  for (int d = 0; d < 3; ++d) {
+    a.Bin[d] = c->bbuf(bin, d);
+    a.B0[d] = c->bbuf(b0, d);
+    a.E[d] = c->field(F_E + d);
+    a.Bout[d] = c->bbuf(bout, d);
+  }
+  for (int n = 0; n < 8; ++n) a.V[n] = c->field(F_V + n);
+  a.sc = c->sc;
+  a.dt_fixed = dt_fixed;
+  a.cfl = cfl;
+  const unsigned nb = blocks_for(c->g.nc, 128);
+  if (c->mhd) {
+    if (stage2) k_update<true, true><<<nb, 128, 0, c->stream>>>(c->g, a);
+    else k_update<true, false><<<nb, 128, 0, c->stream>>>(c->g, a);
+  } else {
+    if (stage2) k_update<false, true><<<nb, 128, 0, c->stream>>>(c->g, a);
+    else k_update<false, false><<<nb, 128, 0, c->stream>>>(c->g, a);
+  }
+  c->launches++;
+  launch_fill(c, bout);
+}
+
+// One RK2 cycle.  dt_fixed > 0: that dt; otherwise dt = cfl / max found by stage 1 (never leaves the device).
+int run_cycle(idfx_ctx* c, double dt_fixed, double cfl) {
+  const bool want_dt = !(dt_fixed > 0.0);
+  if (want_dt) CK(cudaMemsetAsync(&c->sc->smax_bits, 0, sizeof(unsigned long long), c->stream));
+  const int b0 = c->bcur, b1 = (c->bcur + 1) % 3, b2 = (c->bcur + 2) % 3;
+  run_stage(c, false, b0, b0, b1, dt_fixed, cfl, want_dt);
+  run_stage(c, true, b1, b0, b2, dt_fixed, cfl, false);
+  c->bcur = b2;
+  CK(cudaGetLastError());
+  return IDFX_OK;
+}
+
+int copy3d(idfx_ctx* c, double* field, const double* contig_in, double* contig_out, cudaMemcpyKind kind) {
+  const Geom& g = c->g;
+  cudaMemcpy3DParms p;
+  memset(&p, 0, sizeof(p));
+  cudaPitchedPtr pad = make_cudaPitchedPtr((void*)(field + g.at(0, 0, 0)), (size_t)g.sy * 8, g.nx, g.ny + 2 * NG);
+  p.extent = make_cudaExtent((size_t)g.nx * 8, g.ny, g.nz);
+  p.kind = kind;
+  if (contig_in) {
+    p.srcPtr = make_cudaPitchedPtr((void*)contig_in, (size_t)g.nx * 8, g.nx, g.ny);
+    p.dstPtr = pad;
+  } else {
+    p.srcPtr = pad;
+    p.dstPtr = make_cudaPitchedPtr((void*)contig_out, (size_t)g.nx * 8, g.nx, g.ny);
+  }
+  CK(cudaMemcpy3DAsync(&p, c->stream));
+  return IDFX_OK;
+}
+
+// after the primitives (V[0..4]) and the face field (current buffer, active part) are in place
+int finish_set_state(idfx_ctx* c) {
+  StateArgs a;
+  for (int n = 0; n < 5; ++n) a.U[n] = c->field(F_UA + n);
+  for (int n = 0; n < 8; ++n) a.V[n] = c->field(F_V + n);
+  for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
+  a.sc = c->sc;
+  const unsigned nb = blocks_for(c->g.nc, 128);
+  if (c->mhd) k_cons_from_prim<true><<<nb, 128, 0, c->stream>>>(c->g, a);
+  else k_cons_from_prim<false><<<nb, 128, 0, c->stream>>>(c->g, a);
+  c->launches++;
+  launch_fill(c, c->bcur);
+  CK(cudaGetLastError());
+  return IDFX_OK;
+}
+
+int refresh_prims(idfx_ctx* c) {
+  StateArgs a;
+  for (int n = 0; n < 5; ++n) a.U[n] = c->field(F_UA + n);
+  for (int n = 0; n < 8; ++n) a.V[n] = c->field(F_V + n);
+  for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
+  a.sc = c->sc;
+  const unsigned nb = blocks_for(c->g.nc, 128);
+  if (c->mhd) k_prim_from_cons<true><<<nb, 128, 0, c->stream>>>(c->g, a);
+  else k_prim_from_cons<false><<<nb, 128, 0, c->stream>>>(c->g, a);
+  c->launches++;
+  CK(cudaGetLastError());
+  return IDFX_OK;
+}
+
+}  // namespace
+
+// =============================================================================================
+// C ABI
+// =============================================================================================
+extern "C" {
+
+const char* idfx_last_error(void) { return g_err; }
+
+idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solver, int limiter, int emf_mode) {
+  if (nx < 4 || ny < 4 || nz < 4) {
+    set_err("idfx_create: nx, ny, nz must be >= 4");
+    return nullptr;
+  }
+  if (!(dx > 0.0) || !(gamma > 1.0)) {
+    set_err("idfx_create: need dx > 0 and gamma > 1");
+    return nullptr;
+  }
+  if (solver < 0 || solver > 3 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 2) {
+    set_err("idfx_create: unknown solver, limiter or emf_mode");
+    return nullptr;
+  }
+  const bool mhd = emf_mode != EMF_NONE;
+  if ((mhd && solver == SOLVER_HLLC) || (!mhd && solver == SOLVER_HLLD)) {
+    set_err("idfx_create: unsupported combination (HLLC is HD-only, HLLD is MHD-only)");
+    return nullptr;
+  }
+  idfx_ctx* c = new (std::nothrow) idfx_ctx;
+  if (!c) return nullptr;
+  Geom& g = c->g;
+  g.nx = nx;
+  g.ny = ny;
+  g.nz = nz;
+  g.dx = dx;
+  g.gamma = gamma;
+  g.sy = ((nx + IOFF + NG + 15) / 16) * 16;
+  g.sz = (long long)g.sy * (ny + 2 * NG);
+  g.np = ((g.sz * (nz + 2 * NG) + 31) / 32) * 32;
+  g.nc = (long long)nx * ny * nz;
+  c->solver = solver;
+  c->limiter = limiter;
+  c->emf = emf_mode;
+  c->mhd = mhd;
+  return c;
+}
+
+size_t idfx_workspace_bytes(const idfx_ctx* c) {
+  if (!c) return 0;
+  return (size_t)F_COUNT * (size_t)c->g.np * sizeof(double) + 256;
+}
+
+int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
+  if (!c || !d_workspace) {
+    set_err("idfx_bind: null argument");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  if (bytes < idfx_workspace_bytes(c) || ((size_t)d_workspace & 255) != 0) {
+    set_err("idfx_bind: workspace too small or not 256-byte aligned");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  c->ws = (double*)d_workspace;
+  c->ws_bytes = bytes;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->sc = (DevScalars*)(c->ws + (size_t)F_COUNT * (size_t)c->g.np);
+  c->bcur = 0;
+  c->launches = 0;
+  CK(cudaMemsetAsync(d_workspace, 0, idfx_workspace_bytes(c), c->stream));
+  c->bound = true;
+  return IDFX_OK;
+}
+
+int idfx_set_state(idfx_ctx* c, const double* d_prim, const double* d_bface) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!d_prim || (c->mhd && !d_bface)) {
+    set_err("idfx_set_state: null state pointer");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  const unsigned nb = blocks_for(c->g.nc, 128);
+  FieldList fl;
+  fl.n = 5;
+  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(F_V + n);
+  k_pack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_prim);
+  c->launches++;
+  if (c->mhd) {
+    fl.n = 3;
+    for (int d = 0; d < 3; ++d) fl.f[d] = c->bbuf(c->bcur, d);
+    k_pack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_bface);
+    c->launches++;
+  }
+  return finish_set_state(c);
+}
+
+int idfx_set_state_host(idfx_ctx* c, const double* h_prim, const double* h_bface) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!h_prim || (c->mhd && !h_bface)) {
+    set_err("idfx_set_state_host: null state pointer");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  for (int n = 0; n < 5; ++n)
+    if ((rc = copy3d(c, c->field(F_V + n), h_prim + (size_t)n * c->g.nc, nullptr, cudaMemcpyHostToDevice))) return rc;
+  if (c->mhd)
+    for (int d = 0; d < 3; ++d)
+      if ((rc = copy3d(c, c->bbuf(c->bcur, d), h_bface + (size_t)d * c->g.nc, nullptr, cudaMemcpyHostToDevice)))
+        return rc;
+  return finish_set_state(c);
+}
+
+int idfx_get_state(idfx_ctx* c, double* d_prim, double* d_bface) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!d_prim) {
+    set_err("idfx_get_state: null output");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  if ((rc = refresh_prims(c))) return rc;
+  const unsigned nb = blocks_for(c->g.nc, 128);
+  FieldList fl;
+  fl.n = 5;
+  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(F_V + n);
+  k_unpack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_prim);
+  c->launches++;
+  if (c->mhd && d_bface) {
+    fl.n = 3;
+    for (int d = 0; d < 3; ++d) fl.f[d] = c->bbuf(c->bcur, d);
+    k_unpack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_bface);
+    c->launches++;
+  }
+  CK(cudaGetLastError());
+  return IDFX_OK;
+}
+
+int idfx_get_state_host(idfx_ctx* c, double* h_prim, double* h_bface) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!h_prim) {
+    set_err("idfx_get_state_host: null output");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  if ((rc = refresh_prims(c))) return rc;
+  for (int n = 0; n < 5; ++n)
+    if ((rc = copy3d(c, c->field(F_V + n), nullptr, h_prim + (size_t)n * c->g.nc, cudaMemcpyDeviceToHost))) return rc;
+  if (c->mhd && h_bface)
+    for (int d = 0; d < 3; ++d)
+      if ((rc = copy3d(c, c->bbuf(c->bcur, d), nullptr, h_bface + (size_t)d * c->g.nc, cudaMemcpyDeviceToHost)))
+        return rc;
+  CK(cudaStreamSynchronize(c->stream));
+  return IDFX_OK;
+}
+
+int idfx_get_conserved(idfx_ctx* c, double* d_cons, double* d_bface) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!d_cons) {
+    set_err("idfx_get_conserved: null output");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  const unsigned nb = blocks_for(c->g.nc, 128);
+  FieldList fl;
+  fl.n = 5;
+  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(F_UA + n);
+  k_unpack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_cons);
+  c->launches++;
+  if (c->mhd && d_bface) {
+    fl.n = 3;
+    for (int d = 0; d < 3; ++d) fl.f[d] = c->bbuf(c->bcur, d);
+    k_unpack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_bface);
+    c->launches++;
+  }
+  CK(cudaGetLastError());
+  return IDFX_OK;
+}
+
+int idfx_compute_dt(idfx_ctx* c, double cfl, double* h_dt_out) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!h_dt_out || !(cfl > 0.0) || !(cfl < 1.0)) {
+    set_err("idfx_compute_dt: need 0 < cfl < 1 and a non-null output");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  CK(cudaMemsetAsync(&c->sc->smax_bits, 0, sizeof(unsigned long long), c->stream));
+  const double* Bf[3] = {c->bbuf(c->bcur, 0), c->bbuf(c->bcur, 1), c->bbuf(c->bcur, 2)};
+  for (int d = 0; d < 3; ++d) launch_flux(c, d, Bf, true);
+  launch_rhs(c, false, true);
+  CK(cudaGetLastError());
+  unsigned long long bits = 0;
+  CK(cudaMemcpyAsync(&bits, &c->sc->smax_bits, sizeof(bits), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  double smax;
+  memcpy(&smax, &bits, sizeof(smax));
+  *h_dt_out = cfl / smax;
+  return IDFX_OK;
+}
+
+int idfx_step(idfx_ctx* c, double dt) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!(dt > 0.0)) {
+    set_err("idfx_step: dt must be > 0");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  return run_cycle(c, dt, 0.0);
+}
+
+int idfx_advance(idfx_ctx* c, int nsteps, double cfl) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (nsteps < 0 || !(cfl > 0.0) || !(cfl < 1.0)) {
+    set_err("idfx_advance: need nsteps >= 0 and 0 < cfl < 1");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  for (int s = 0; s < nsteps; ++s)
+    if ((rc = run_cycle(c, 0.0, cfl))) return rc;
+  return IDFX_OK;
+}
+
+int idfx_last_dt(idfx_ctx* c, double* h_dt_out) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!h_dt_out) return IDFX_ERR_INVALID_ARG;
+  CK(cudaMemcpyAsync(h_dt_out, &c->sc->dt_used, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return IDFX_OK;
+}
+
+int idfx_status(idfx_ctx* c) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  int flag = 0;
+  CK(cudaMemcpyAsync(&flag, &c->sc->flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  if (flag) {
+    set_err("unphysical state (rho <= 0, p <= 0 or NaN) met on the device");
+    return IDFX_ERR_UNPHYSICAL;
+  }
+  return IDFX_OK;
+}
+
+long long idfx_launch_count(const idfx_ctx* c) { return c ? c->launches : 0; }
+
+void idfx_destroy(idfx_ctx* c) { delete c; }
+
+}  // extern "C"

@@ -1,0 +1,404 @@
+// physics.cuh — point-wise device functions of the idfx CUDA path (sm_100a, fp64).
+//
+// Reconstruction, ideal HD/MHD fluxes and the approximate Riemann solvers
+// of PAPER.md:81: HLL, HLLC (HD), HLLD (MHD), Roe.  Formulas and readings: DESIGN.md O3-O8 / G2-G7.
+// A 1D state along the sweep direction is W = (rho, u, v, w, p, By, Bz): u normal velocity, (By,Bz) the
+// transverse field after cyclic permutation, Bn the normal (staggered) field.  Fluxes come back in the same
+// local ordering F = (rho, m_n, m_t1, m_t2, E, B_t1, B_t2).
+//
+// This file shares nothing with oracle/: the solvers are written for registers (reciprocals reused,
+// analytic Roe projections instead of 7x7 matrix loops, one-sided HLLD star states).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace idfx {
+
+enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3 };
+enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2 };
+enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2 };
+
+#define IDFX_DEV __device__ __forceinline__
+
+// O3 / G2: limited slope from the backward and forward differences.
+template <int LIM>
+IDFX_DEV double limited_slope(double dm, double dp) {
+  if (LIM == LIM_FLAT) return 0.0;
+  const double prod = dm * dp;
+  if (LIM == LIM_VANLEER) {
+    const bool mono = prod > 0.0;
+    const double den = mono ? (dm + dp) : 1.0;  // keeps the division off its slow path at extrema
+    const double s = (2.0 * prod) / den;
+    return mono ? s : 0.0;
+  } else {
+    const double s = (fabs(dm) < fabs(dp)) ? dm : dp;
+    return (prod > 0.0) ? s : 0.0;
+  }
+}
+
+// Conserved vector, physical flux and total pressure of one side.
+template <bool MHD>
+IDFX_DEV void side_cons_flux(const double W[7], double Bn, double igm1, double U[7], double F[7], double& pT) {
+  const double rho = W[0], u = W[1], v = W[2], w = W[3], p = W[4];
+  const double mu = rho * u;
+  const double ke = 0.5 * rho * (u * u + v * v + w * w);
+  U[0] = rho;
+  U[1] = mu;
+  U[2] = rho * v;
+  U[3] = rho * w;
+  if (MHD) {
+    const double By = W[5], Bz = W[6];
+    const double pb = 0.5 * (Bn * Bn + By * By + Bz * Bz);
+    const double vB = u * Bn + v * By + w * Bz;
+    pT = p + pb;
+    U[4] = p * igm1 + ke + pb;
+    U[5] = By;
+    U[6] = Bz;
+    F[0] = mu;
+    F[1] = mu * u + pT - Bn * Bn;
+    F[2] = mu * v - Bn * By;
+    F[3] = mu * w - Bn * Bz;
+    F[4] = (U[4] + pT) * u - Bn * vB;
+    F[5] = u * By - v * Bn;
+    F[6] = u * Bz - w * Bn;
+  } else {
+    pT = p;
+    U[4] = p * igm1 + ke;
+    U[5] = U[6] = 0.0;
+    F[0] = mu;
+    F[1] = mu * u + p;
+    F[2] = mu * v;
+    F[3] = mu * w;
+    F[4] = (U[4] + p) * u;
+    F[5] = F[6] = 0.0;
+  }
+}
+
+// O4: sound speed (HD) or fast magnetosonic speed along the sweep direction (MHD).
+template <bool MHD>
+IDFX_DEV double signal_speed(const double W[7], double Bn, double g) {
+  const double ir = 1.0 / W[0];
+  const double a2 = g * W[4] * ir;
+  if (!MHD) return sqrt(a2);
+  const double bn2 = Bn * Bn * ir;
+  const double b2 = bn2 + (W[5] * W[5] + W[6] * W[6]) * ir;
+  const double s = a2 + b2;
+  const double disc = fmax(s * s - 4.0 * a2 * bn2, 0.0);
+  return sqrt(0.5 * (s + sqrt(disc)));
+}
+
+// O4 / G5: Davis estimate of the outer speeds; c_face = max(|S_L|,|S_R|) for every solver.
+template <bool MHD>
+IDFX_DEV void outer_speeds(const double WL[7], const double WR[7], double Bn, double g, double& SL, double& SR) {
+  const double cL = signal_speed<MHD>(WL, Bn, g), cR = signal_speed<MHD>(WR, Bn, g);
+  SL = fmin(WL[1] - cL, WR[1] - cR);
+  SR = fmax(WL[1] + cL, WR[1] + cR);
+}
+
+// O5: HLL average inside the fan (caller handles S_L >= 0 and S_R <= 0).
+template <int NV>
+IDFX_DEV void hll_inner(const double UL[7], const double UR[7], const double FL[7], const double FR[7], double SL,
+                        double SR, double F[7]) {
+  const double inv = 1.0 / (SR - SL);
+  const double ss = SL * SR;
+#pragma unroll
+  for (int n = 0; n < NV; ++n) F[n] = (SR * FL[n] - SL * FR[n] + ss * (UR[n] - UL[n])) * inv;
+}
+
+// O6: HLLC (hydrodynamics).  Only the star state on the side of the contact is built.
+IDFX_DEV void hllc_inner(const double WL[7], const double WR[7], const double UL[7], const double UR[7],
+                         const double FL[7], const double FR[7], double SL, double SR, double F[7]) {
+  const double qL = WL[0] * (SL - WL[1]);  // rho_L (S_L - u_L)
+  const double qR = WR[0] * (SR - WR[1]);
+  const double SS = (WR[4] - WL[4] + qL * WL[1] - qR * WR[1]) / (qL - qR);
+  const bool left = SS >= 0.0;
+  const double SK = left ? SL : SR;
+  const double qK = left ? qL : qR;
+  const double rK = left ? WL[0] : WR[0], uK = left ? WL[1] : WR[1], vK = left ? WL[2] : WR[2];
+  const double wK = left ? WL[3] : WR[3], pK = left ? WL[4] : WR[4], EK = left ? UL[4] : UR[4];
+  const double fac = qK / (SK - SS);
+  double Us[5];
+  Us[0] = fac;
+  Us[1] = fac * SS;
+  Us[2] = fac * vK;
+  Us[3] = fac * wK;
+  Us[4] = fac * (EK / rK + (SS - uK) * (SS + pK / qK));
+#pragma unroll
+  for (int n = 0; n < 5; ++n) {
+    const double Fk = left ? FL[n] : FR[n];
+    const double Uk = left ? UL[n] : UR[n];
+    F[n] = Fk + SK * (Us[n] - Uk);
+  }
+}
+
+// O7 / G6: HLLD (MHD), for S_L < 0 < S_R.  The starred transverse components are needed from both sides
+// (they enter the double-star state); energies and the final flux only on the side that is selected.
+IDFX_DEV void hlld_inner(const double WL[7], const double WR[7], double Bn, const double UL[7], const double UR[7],
+                         const double FL[7], const double FR[7], double pTL, double pTR, double SL, double SR,
+                         double F[7]) {
+  const double uL = WL[1], uR = WR[1];
+  const double sL = SL - uL, sR = SR - uR;
+  const double qL = WL[0] * sL, qR = WR[0] * sR;  // rho_K (S_K - u_K)
+  const double iD = 1.0 / (qR - qL);
+  const double SM = (qR * uR - qL * uL - pTR + pTL) * iD;
+  const double pTs = (qR * pTL - qL * pTR + qL * qR * (uR - uL)) * iD;
+  const double Bn2 = Bn * Bn;
+
+  const double iL = 1.0 / (SL - SM), iR = 1.0 / (SR - SM);
+  const double rsL = qL * iL, rsR = qR * iR;  // rho*_K
+  double vsL, wsL, BysL, BzsL, vsR, wsR, BysR, BzsR;
+  {
+    const double d = qL * (SL - SM) - Bn2;
+    const bool deg = fabs(d) < 1e-12 * qL * sL;
+    const double id = 1.0 / (deg ? 1.0 : d);
+    const double f = deg ? 0.0 : Bn * (SM - uL) * id;
+    const double h = deg ? 1.0 : (qL * sL - Bn2) * id;
+    vsL = WL[2] - WL[5] * f;
+    wsL = WL[3] - WL[6] * f;
+    BysL = WL[5] * h;
+    BzsL = WL[6] * h;
+  }
+  {
+    const double d = qR * (SR - SM) - Bn2;
+    const bool deg = fabs(d) < 1e-12 * qR * sR;
+    const double id = 1.0 / (deg ? 1.0 : d);
+    const double f = deg ? 0.0 : Bn * (SM - uR) * id;
+    const double h = deg ? 1.0 : (qR * sR - Bn2) * id;
+    vsR = WR[2] - WR[5] * f;
+    wsR = WR[3] - WR[6] * f;
+    BysR = WR[5] * h;
+    BzsR = WR[6] * h;
+  }
+  const double sqL = sqrt(rsL), sqR = sqrt(rsR);
+  const double aBn = fabs(Bn);
+  const double SsL = SM - aBn / sqL, SsR = SM + aBn / sqR;
+
+  // side selection in the order of O7: S*_L >= 0 -> U*_L ; S*_R <= 0 -> U*_R ; S_M >= 0 -> U**_L ; else U**_R
+  const bool starL = SsL >= 0.0;
+  const bool starR = !starL && (SsR <= 0.0);
+  const bool left = starL || (!starR && SM >= 0.0);
+  const bool dstar = !starL && !starR;
+
+  const double SK = left ? SL : SR, sK = left ? sL : sR, iK = left ? iL : iR;
+  const double rsK = left ? rsL : rsR, sqK = left ? sqL : sqR;
+  const double uK = left ? uL : uR, vK = left ? WL[2] : WR[2], wK = left ? WL[3] : WR[3];
+  const double ByK = left ? WL[5] : WR[5], BzK = left ? WL[6] : WR[6];
+  const double EK = left ? UL[4] : UR[4], pTK = left ? pTL : pTR;
+  const double vsK = left ? vsL : vsR, wsK = left ? wsL : wsR;
+  const double BysK = left ? BysL : BysR, BzsK = left ? BzsL : BzsR;
+
+  const double vBK = uK * Bn + vK * ByK + wK * BzK;
+  const double vBsK = SM * Bn + vsK * BysK + wsK * BzsK;
+  const double EsK = (sK * EK - pTK * uK + pTs * SM + Bn * (vBK - vBsK)) * iK;
+
+  double Us[7];
+  Us[0] = rsK;
+  Us[1] = rsK * SM;
+  Us[2] = rsK * vsK;
+  Us[3] = rsK * wsK;
+  Us[4] = EsK;
+  Us[5] = BysK;
+  Us[6] = BzsK;
+  if (!dstar) {
+#pragma unroll
+    for (int n = 0; n < 7; ++n) {
+      const double Fk = left ? FL[n] : FR[n];
+      const double Uk = left ? UL[n] : UR[n];
+      F[n] = Fk + SK * (Us[n] - Uk);
+    }
+    return;
+  }
+  const double sgn = (Bn >= 0.0) ? 1.0 : -1.0;
+  const double inv = 1.0 / (sqL + sqR);
+  const double vss = (sqL * vsL + sqR * vsR + (BysR - BysL) * sgn) * inv;
+  const double wss = (sqL * wsL + sqR * wsR + (BzsR - BzsL) * sgn) * inv;
+  const double sqq = sqL * sqR;
+  const double Byss = (sqL * BysR + sqR * BysL + sqq * (vsR - vsL) * sgn) * inv;
+  const double Bzss = (sqL * BzsR + sqR * BzsL + sqq * (wsR - wsL) * sgn) * inv;
+  const double vBss = SM * Bn + vss * Byss + wss * Bzss;
+  // E**_L = E*_L - sqrt(rho*_L)(vB*_L - vB**) sgn ;  E**_R = E*_R + sqrt(rho*_R)(vB*_R - vB**) sgn
+  const double EssK = left ? (EsK - sqK * (vBsK - vBss) * sgn) : (EsK + sqK * (vBsK - vBss) * sgn);
+  const double SsK = left ? SsL : SsR;
+  double Uss[7];
+  Uss[0] = rsK;
+  Uss[1] = rsK * SM;
+  Uss[2] = rsK * vss;
+  Uss[3] = rsK * wss;
+  Uss[4] = EssK;
+  Uss[5] = Byss;
+  Uss[6] = Bzss;
+#pragma unroll
+  for (int n = 0; n < 7; ++n) {
+    const double Fk = left ? FL[n] : FR[n];
+    const double Uk = left ? UL[n] : UR[n];
+    F[n] = Fk + SsK * Uss[n] - (SsK - SK) * Us[n] - SK * Uk;
+  }
+}
+
+// O8 / G7: Roe solver with the exact Roe averages of the shifted equation of state, no entropy fix.
+// Returns false when a~^2 <= 0 (caller falls back to HLL).  Projections are written out analytically:
+// dW = Minv dU, alpha_k = l_k . dW, primitive sum s = sum |lambda_k| alpha_k r_k, flux jump = M s.
+template <bool MHD>
+IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const double UL[7], const double UR[7],
+                        const double FL[7], const double FR[7], double pTL, double pTR, double g, double F[7]) {
+  const double sL = sqrt(WL[0]), sR = sqrt(WR[0]);
+  const double isum = 1.0 / (sL + sR);
+  const double rb = sL * sR;
+  const double irb = 1.0 / rb;
+  const double ub = (sL * WL[1] + sR * WR[1]) * isum;
+  const double vb = (sL * WL[2] + sR * WR[2]) * isum;
+  const double wb = (sL * WL[3] + sR * WR[3]) * isum;
+  const double HL = (UL[4] + pTL) / WL[0], HR = (UR[4] + pTR) / WR[0];
+  const double Hb = (sL * HL + sR * HR) * isum;
+  const double v2h = 0.5 * (ub * ub + vb * vb + wb * wb);
+  const double gm1 = g - 1.0;
+  double Byb = 0.0, Bzb = 0.0, Xp = 0.0, bt2 = 0.0, bn2 = 0.0;
+  const double dBy = UR[5] - UL[5], dBz = UR[6] - UL[6];
+  if (MHD) {
+    Byb = (sR * WL[5] + sL * WR[5]) * isum;
+    Bzb = (sR * WL[6] + sL * WR[6]) * isum;
+    Xp = (g - 2.0) * (dBy * dBy + dBz * dBz) * 0.5 * isum * isum;
+    bt2 = (Byb * Byb + Bzb * Bzb) * irb;
+    bn2 = Bn * Bn * irb;
+  }
+  const double a2 = gm1 * (Hb - v2h - (bn2 + bt2)) - Xp;
+  if (!(a2 > 0.0)) return false;
+
+  // jumps in the linearised primitive variables
+  const double dr = UR[0] - UL[0];
+  const double dmx = UR[1] - UL[1], dmy = UR[2] - UL[2], dmz = UR[3] - UL[3], dE = UR[4] - UL[4];
+  const double du = (dmx - ub * dr) * irb;
+  const double dv = (dmy - vb * dr) * irb;
+  const double dw = (dmz - wb * dr) * irb;
+  const double dp = gm1 * (v2h * dr - ub * dmx - vb * dmy - wb * dmz + dE - Byb * dBy - Bzb * dBz) - Xp * dr;
+
+  double s0, s1, s2, s3, s4, s5 = 0.0, s6 = 0.0;
+  if (!MHD) {
+    const double a = sqrt(a2);
+    const double ia2 = 1.0 / a2;
+    // acoustic waves u -+ a: r = (rb, -+a, 0, 0, rb a2), l = (0, -+a, 0, 0, 1/rb)/(2 a2)
+    const double am = (-a * du + dp * irb) * 0.5 * ia2;
+    const double ap = (a * du + dp * irb) * 0.5 * ia2;
+    const double lm = fabs(ub - a) * am, lp = fabs(ub + a) * ap, l0 = fabs(ub);
+    const double a0 = dr - dp * ia2;
+    s0 = rb * (lm + lp) + l0 * a0;
+    s1 = a * (lp - lm);
+    s2 = l0 * dv;
+    s3 = l0 * dw;
+    s4 = rb * a2 * (lm + lp);
+  } else {
+    const double a = sqrt(a2);
+    const double sum = a2 + bn2 + bt2;
+    const double disc = sqrt(fmax(sum * sum - 4.0 * a2 * bn2, 0.0));
+    const double Cf2 = 0.5 * (sum + disc);
+    const double Cs2 = a2 * bn2 / Cf2;
+    const double Cf = sqrt(Cf2), Cs = sqrt(Cs2), CA = sqrt(bn2);
+    double af = 1.0, as = 0.0;
+    const double den = Cf2 - Cs2;
+    if (den > 0.0) {
+      const double iden = 1.0 / den;
+      af = sqrt(fmin(1.0, fmax(0.0, (a2 - Cs2) * iden)));
+      as = sqrt(fmin(1.0, fmax(0.0, (Cf2 - a2) * iden)));
+    }
+    const double Bt = sqrt(Byb * Byb + Bzb * Bzb);
+    double by = 0.70710678118654752440, bz = 0.70710678118654752440;
+    if (Bt != 0.0) {
+      const double iBt = 1.0 / Bt;
+      by = Byb * iBt;
+      bz = Bzb * iBt;
+    }
+    const double S = (Bn >= 0.0) ? 1.0 : -1.0;
+    const double sr = sqrt(rb), isr = 1.0 / sr;
+    const double Cff = Cf * af, Css = Cs * as, Qf = Cff * S, Qs = Css * S;
+    const double Af = a * af * sr, As = a * as * sr;
+    const double i2a2 = 0.5 / a2;
+
+    const double dvt = by * dv + bz * dw;        // beta . dv_t
+    const double dBt = (by * dBy + bz * dBz);    // beta . dB_t
+    const double dvx = -bz * dv + by * dw;       // (beta_perp) . dv_t
+    const double dBx = (-bz * dBy + by * dBz);   // (beta_perp) . dB_t
+    // wave strengths
+    const double tf = (af * dp + As * dBt) * irb;
+    const double afm = (-Cff * du + Qs * dvt + tf) * i2a2;
+    const double afp = (Cff * du - Qs * dvt + tf) * i2a2;
+    const double ts = (as * dp - Af * dBt) * irb;
+    const double asm_ = (-Css * du - Qf * dvt + ts) * i2a2;
+    const double asp = (Css * du + Qf * dvt + ts) * i2a2;
+    const double aAm = 0.5 * (dvx + S * dBx * isr);     // l_A- = (0,0,-bz,+by,0,-S bz/sr, S by/sr)/2
+    const double aAp = 0.5 * (-dvx + S * dBx * isr);
+    const double a0 = dr - dp / a2;
+    // |lambda| alpha
+    const double Lfm = fabs(ub - Cf) * afm, Lfp = fabs(ub + Cf) * afp;
+    const double Lsm = fabs(ub - Cs) * asm_, Lsp = fabs(ub + Cs) * asp;
+    const double LAm = fabs(ub - CA) * aAm, LAp = fabs(ub + CA) * aAp;
+    const double L0 = fabs(ub) * a0;
+    // primitive-space sum; components along beta (t) and beta_perp (x) for v_t and B_t
+    const double fsum = Lfm + Lfp, ssum = Lsm + Lsp;
+    s0 = rb * (af * fsum + as * ssum) + L0;
+    s1 = Cff * (Lfp - Lfm) + Css * (Lsp - Lsm);
+    const double vt = Qs * (Lfm - Lfp) + Qf * (Lsp - Lsm);   // along beta
+    const double vx = LAm - LAp;                             // along beta_perp: r_A-+ = (.., -+bz, +-by, ..)
+    s2 = by * vt - bz * vx;
+    s3 = bz * vt + by * vx;
+    s4 = rb * a2 * (af * fsum + as * ssum);
+    const double Bt_ = As * fsum - Af * ssum;                // along beta
+    const double Bx_ = S * sr * (LAm + LAp);                 // along beta_perp
+    s5 = by * Bt_ - bz * Bx_;
+    s6 = bz * Bt_ + by * Bx_;
+  }
+  // conserved-variable jump M s, F = (F_L + F_R)/2 - (M s)/2
+  const double j0 = s0;
+  const double j1 = ub * s0 + rb * s1;
+  const double j2 = vb * s0 + rb * s2;
+  const double j3 = wb * s0 + rb * s3;
+  const double j4 = (v2h + Xp / gm1) * s0 + rb * (ub * s1 + vb * s2 + wb * s3) + s4 / gm1 + Byb * s5 + Bzb * s6;
+  F[0] = 0.5 * (FL[0] + FR[0] - j0);
+  F[1] = 0.5 * (FL[1] + FR[1] - j1);
+  F[2] = 0.5 * (FL[2] + FR[2] - j2);
+  F[3] = 0.5 * (FL[3] + FR[3] - j3);
+  F[4] = 0.5 * (FL[4] + FR[4] - j4);
+  F[5] = MHD ? 0.5 * (FL[5] + FR[5] - s5) : 0.0;
+  F[6] = MHD ? 0.5 * (FL[6] + FR[6] - s6) : 0.0;
+  return true;
+}
+
+// One Riemann problem.  Returns the flux in F and c_face = max(|S_L|,|S_R|).
+template <int SOLVER, bool MHD>
+IDFX_DEV double riemann(const double WL[7], const double WR[7], double Bn, double g, double F[7]) {
+  const double igm1 = 1.0 / (g - 1.0);
+  double UL[7], UR[7], FL[7], FR[7], pTL, pTR, SL, SR;
+  side_cons_flux<MHD>(WL, Bn, igm1, UL, FL, pTL);
+  side_cons_flux<MHD>(WR, Bn, igm1, UR, FR, pTR);
+  outer_speeds<MHD>(WL, WR, Bn, g, SL, SR);
+  const double cface = fmax(fabs(SL), fabs(SR));
+  constexpr int NV = MHD ? 7 : 5;
+  if (SOLVER == SOLVER_ROE) {
+    if (!roe_inner<MHD>(WL, WR, Bn, UL, UR, FL, FR, pTL, pTR, g, F)) {
+      if (SL >= 0.0) {
+#pragma unroll
+        for (int n = 0; n < 7; ++n) F[n] = FL[n];
+      } else if (SR <= 0.0) {
+#pragma unroll
+        for (int n = 0; n < 7; ++n) F[n] = FR[n];
+      } else {
+        F[5] = F[6] = 0.0;
+        hll_inner<NV>(UL, UR, FL, FR, SL, SR, F);
+      }
+    }
+    return cface;
+  }
+  if (SL >= 0.0) {
+#pragma unroll
+    for (int n = 0; n < 7; ++n) F[n] = FL[n];
+  } else if (SR <= 0.0) {
+#pragma unroll
+    for (int n = 0; n < 7; ++n) F[n] = FR[n];
+  } else {
+    if (!MHD) F[5] = F[6] = 0.0;
+    if (SOLVER == SOLVER_HLL) hll_inner<NV>(UL, UR, FL, FR, SL, SR, F);
+    if (SOLVER == SOLVER_HLLC) hllc_inner(WL, WR, UL, UR, FL, FR, SL, SR, F);
+    if (SOLVER == SOLVER_HLLD) hlld_inner(WL, WR, Bn, UL, UR, FL, FR, pTL, pTR, SL, SR, F);
+  }
+  return cface;
+}
+
+}  // namespace idfx

@@ -1,0 +1,151 @@
+"""Thin ctypes binding over the C-ABI library (include/idfx.h) — argument marshalling only.
+
+Every step of the method runs in the CUDA kernels of libidfx.so; torch is used for device memory (the
+workspace and the state tensors) and for the stream.  There is no CPU fallback: if the library is
+missing or no CUDA device is present, calls raise.
+"""
+import ctypes
+import os
+
+import torch
+
+SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE = 0, 1, 2, 3
+LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER = 0, 1, 2
+EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT = 0, 1, 2
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_NOT_BOUND, ERR_CUDA, ERR_UNPHYSICAL = 0, -1, -2, -3, -4, -5
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libidfx.so")
+
+# every symbol include/idfx.h declares
+SYMBOLS = (
+    "idfx_create", "idfx_workspace_bytes", "idfx_bind", "idfx_set_state", "idfx_set_state_host",
+    "idfx_get_state", "idfx_get_state_host", "idfx_get_conserved", "idfx_compute_dt", "idfx_step",
+    "idfx_advance", "idfx_last_dt", "idfx_status", "idfx_launch_count", "idfx_last_error", "idfx_destroy",
+)
+
+_lib = None
+
+
+class IdfxError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("idfx error %d: %s" % (code, msg))
+        self.code = code
+
+
+def lib():
+    """Loads libidfx.so (built by paper_2304_13746_b200/build.py or __graft_entry__.build())."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("%s is missing: run `python -m paper_2304_13746_b200.build` (nvcc, sm_100a)" % LIB_PATH)
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci, cd, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+        dp = ctypes.POINTER(ctypes.c_double)
+        L.idfx_create.restype = vp
+        L.idfx_create.argtypes = [ci, ci, ci, cd, cd, ci, ci, ci]
+        L.idfx_workspace_bytes.restype = sz
+        L.idfx_workspace_bytes.argtypes = [vp]
+        L.idfx_bind.argtypes = [vp, vp, sz, vp]
+        for n in ("idfx_set_state", "idfx_set_state_host", "idfx_get_state", "idfx_get_state_host", "idfx_get_conserved"):
+            getattr(L, n).argtypes = [vp, vp, vp]
+        L.idfx_compute_dt.argtypes = [vp, cd, dp]
+        L.idfx_step.argtypes = [vp, cd]
+        L.idfx_advance.argtypes = [vp, ci, cd]
+        L.idfx_last_dt.argtypes = [vp, dp]
+        L.idfx_status.argtypes = [vp]
+        L.idfx_launch_count.argtypes = [vp]
+        L.idfx_launch_count.restype = ctypes.c_longlong
+        L.idfx_last_error.restype = ctypes.c_char_p
+        L.idfx_destroy.argtypes = [vp]
+        L.idfx_destroy.restype = None
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != OK:
+        raise IdfxError(rc, lib().idfx_last_error().decode())
+
+
+class Idfx:
+    """One periodic nx*ny*nz box on one GPU.  Tensors are float64, [var][nz][ny][nx]."""
+
+    def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode, device="cuda:0", stream=None):
+        self.L = lib()
+        self.h = self.L.idfx_create(nx, ny, nz, dx, gamma, solver, limiter, emf_mode)
+        if not self.h:
+            raise IdfxError(ERR_INVALID_ARG, self.L.idfx_last_error().decode())
+        if not torch.cuda.is_available():
+            raise RuntimeError("idfx needs a CUDA device; there is no CPU fallback")
+        self.device = torch.device(device)
+        self.shape = (nz, ny, nx)
+        self.mhd = emf_mode != EMF_NONE
+        nbytes = self.L.idfx_workspace_bytes(self.h)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        with torch.cuda.device(self.device):
+            s = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.stream = s
+        _check(self.L.idfx_bind(self.h, self.workspace.data_ptr(), nbytes, s.cuda_stream))
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.idfx_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        self.close()
+
+    def _dev(self, t, nvar):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == (nvar,) + self.shape
+        return t.data_ptr()
+
+    def _host(self, t, nvar):
+        assert (not t.is_cuda) and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == (nvar,) + self.shape
+        return t.data_ptr()
+
+    def set_state(self, prim, bface=None):
+        host = not prim.is_cuda
+        f = self.L.idfx_set_state_host if host else self.L.idfx_set_state
+        p = self._host if host else self._dev
+        _check(f(self.h, p(prim, 5), p(bface, 3) if bface is not None else None))
+
+    def get_state(self, out_prim=None, out_bface=None, host=False):
+        dev = "cpu" if host else self.device
+        if out_prim is None:
+            out_prim = torch.empty((5,) + self.shape, dtype=torch.float64, device=dev, pin_memory=host)
+        if out_bface is None and self.mhd:
+            out_bface = torch.empty((3,) + self.shape, dtype=torch.float64, device=dev, pin_memory=host)
+        f = self.L.idfx_get_state_host if host else self.L.idfx_get_state
+        p = self._host if host else self._dev
+        _check(f(self.h, p(out_prim, 5), p(out_bface, 3) if out_bface is not None else None))
+        return out_prim, out_bface
+
+    def get_conserved(self):
+        cons = torch.empty((5,) + self.shape, dtype=torch.float64, device=self.device)
+        bface = torch.empty((3,) + self.shape, dtype=torch.float64, device=self.device) if self.mhd else None
+        _check(self.L.idfx_get_conserved(self.h, cons.data_ptr(), bface.data_ptr() if self.mhd else None))
+        return cons, bface
+
+    def compute_dt(self, cfl):
+        dt = ctypes.c_double()
+        _check(self.L.idfx_compute_dt(self.h, cfl, ctypes.byref(dt)))
+        return dt.value
+
+    def step(self, dt):
+        _check(self.L.idfx_step(self.h, dt))
+
+    def advance(self, nsteps, cfl):
+        _check(self.L.idfx_advance(self.h, nsteps, cfl))
+
+    def last_dt(self):
+        dt = ctypes.c_double()
+        _check(self.L.idfx_last_dt(self.h, ctypes.byref(dt)))
+        return dt.value
+
+    def status(self):
+        return self.L.idfx_status(self.h)
+
+    def launch_count(self):
+        return self.L.idfx_launch_count(self.h)
