@@ -1,0 +1,289 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the whole hot path (one "step" = one full RK2 cycle including its dt evaluation)
+on BASELINE config 5: 512^3 periodic ideal MHD, fp64, PLM van Leer + HLLD + CT (upwind-contact EMF) + RK2, CFL 0.3,
+seeded random-phase synthetic input.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--n 512] [--workload config5]
+
+Prints ONE JSON line (rank 0).  `value` = cell-updates/s with the state resident in HBM; `e2e` = the same job
+through the C ABI with HOST buffers (set_state_host -> advance -> get_state_host inside the timed region).
+N > 1: independent replicas, one per GPU, no collective on the data path (replicas only);
+only the timing is reduced (max over ranks).
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 3D MHD cell-updates/s"
+UNIT = "cell-updates/s"
+ALGO_BYTES_PER_CELL_UPDATE = 320.0          # 40 doubles per MHD cell-update
+# algorithmic flops of one reconstruct+Riemann face solve and of the other kernels, per cell per launch
+# (counted from the formulas); used for the "alu" roofline of the flux kernels
+ALGO_FLOPS_PER_CELL = {"flux_x": 700.0, "flux_y": 700.0, "flux_z": 700.0}
+# algorithmic (compulsory) bytes per cell per launch of each kernel class, DESIGN.md "Kernels"
+ALGO_BYTES_PER_CELL = {"flux_x": 8 * 16.0, "flux_y": 8 * 16.0, "flux_z": 8 * 16.0, "rhs_dtmax": 8 * 23.0,
+                       "edge_emf": 8 * 18.0, "ct_update_prim": 8 * 36.0}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config5")
+    ap.add_argument("--n", type=int, default=None, help="override the grid size (development only)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[1]))
+                smax.append(float(f[2]))
+                power.append(float(f[3]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_rate(cfg_name, n, steps, warmup):
+    """cell-updates/s of the CPU oracle as it stands, one thread, on the recipe of `cfg_name` at n^3."""
+    from oracle import idfxref
+    from paper_2304_13746_b200 import inputs
+    prim, b, cfg = inputs.make(cfg_name, n=n)
+    ref = idfxref.Oracle(n, n, n, cfg["dx"], cfg["gamma"], cfg["solver"], cfg["limiter"], cfg["emf"])
+    ref.set_state(prim.numpy(), None if b is None else b.numpy())
+    if warmup:
+        ref.advance(warmup, cfg["cfl"])
+    t0 = time.perf_counter()
+    ref.advance(steps, cfg["cfl"])
+    el = time.perf_counter() - t0
+    assert ref.status() == 0
+    return n ** 3 * steps / el, el
+
+
+def run_reference(args):
+    """Reference arm of this tier = the oracle, timed on the host cores on a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = 64
+    rate, el = oracle_rate(args.workload, n, args.steps, args.warmup)
+    sample = "%s recipe at %d^3 (bounded sample of the 512^3 workload), %d timed steps after %d warm-up" % (
+        args.workload, n, args.steps, args.warmup)
+    out = {
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": el / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config5: 512^3 MHD HLLD + PLM van Leer + CT upwind-contact + RK2, CFL 0.3",
+                   "sample": sample},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2304_13746_b200 import idfx, inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    prim, bface, cfg = inputs.make(args.workload, n=args.n, device=dev)
+    n, cfl = cfg["n"], cfg["cfl"]
+    cells = n ** 3
+    sim = idfx.Idfx(n, n, n, cfg["dx"], cfg["gamma"], cfg["solver"], cfg["limiter"], cfg["emf"], device=dev)
+    sim.set_state(prim, bface)
+    K, W = args.steps, max(args.warmup, 0)
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps -------------------
+    sim.advance(W, cfl)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    l0 = sim.launch_count()
+    e0.record()
+    sim.advance(K, cfl)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = sim.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    assert sim.status() == 0, "unphysical state during the timed region"
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = cells * K * world / (ms * 1e-3)
+
+    # ---- per-kernel durations over K more steps (CUDA events around every launch, on the launch stream) ----
+    sim.profile(True)
+    sim.advance(K, cfl)
+    prof = sim.profile_read()
+    sim.profile(False)
+    peaks, peak_kind = load_peaks()
+    hbm_peak = float(peaks["hbm_gbs"])
+    fp64_tflops, fp64_tinst = idfx.probe_fp64()
+    tot_ms = sum(v[0] for v in prof.values())
+    kernels = {}
+    for name, (kms, cnt) in prof.items():
+        if cnt == 0:
+            continue
+        avg = kms / cnt
+        ent = {"launches_per_step": cnt / K, "avg_ms": avg, "share": kms / tot_ms}
+        if name in ALGO_BYTES_PER_CELL:
+            ent["algo_GBps"] = ALGO_BYTES_PER_CELL[name] * cells / (avg * 1e-3) * 1e-9
+        if name in ALGO_FLOPS_PER_CELL:
+            ent["algo_TFLOPs"] = ALGO_FLOPS_PER_CELL[name] * cells / (avg * 1e-3) * 1e-12
+        kernels[name] = ent
+    dom = max(kernels, key=lambda k: kernels[k]["share"] / kernels[k]["launches_per_step"])
+    if dom in ALGO_FLOPS_PER_CELL:
+        roof = {"kernel": dom, "bound": "alu", "achieved": kernels[dom]["algo_TFLOPs"], "peak": fp64_tflops,
+                "unit": "TFLOP/s", "frac": kernels[dom]["algo_TFLOPs"] / fp64_tflops, "traffic": None,
+                "peak_source": "fp64 DFMA probe measured in this run (idfx_probe_fp64)"}
+    else:
+        roof = {"kernel": dom, "bound": "hbm", "achieved": kernels[dom]["algo_GBps"], "peak": hbm_peak,
+                "unit": "GB/s", "frac": kernels[dom]["algo_GBps"] / hbm_peak, "traffic": None,
+                "peak_source": "MEASURED_PEAKS.json (%s)" % peak_kind}
+    step_hbm = ALGO_BYTES_PER_CELL_UPDATE * value / world * 1e-9
+    roof_step = {"bound": "hbm", "achieved": step_hbm, "peak": hbm_peak, "unit": "GB/s", "frac": step_hbm / hbm_peak,
+                 "what": "whole step: 320 algorithmic B per cell-update x cell-updates/s per GPU, of %s" % peak_kind}
+
+    # ---- end to end through the C ABI with host buffers --------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        h_prim, h_b = prim.cpu().pin_memory(), bface.cpu().pin_memory() if bface is not None else None
+        o_prim = torch.empty_like(h_prim).pin_memory()
+        o_b = torch.empty_like(h_b).pin_memory() if h_b is not None else None
+        del prim, bface
+        barrier()
+        t0 = time.perf_counter()
+        sim.set_state(h_prim, h_b)              # idfx_set_state_host: H2D inside the timed region
+        sim.advance(K, cfl)
+        sim.get_state(o_prim, o_b, host=True)   # idfx_get_state_host: D2H, synchronises
+        el = time.perf_counter() - t0
+        t = torch.tensor([el], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        el = float(t.item())
+        nbytes = h_prim.numel() * 8 + (h_b.numel() * 8 if h_b is not None else 0)
+        e2e = {"value": cells * K * world / el, "unit": UNIT, "h2d_bytes_per_step": nbytes / K,
+               "d2h_bytes_per_step": nbytes / K,
+               "what": "set_state_host + advance(K) + get_state_host; the state crosses PCIe once per job, bytes amortised over K steps"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        sn, ssteps = 128, 2
+        rate, el = oracle_rate(args.workload, sn, ssteps, 0)
+        cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": el,
+               "sample": "%s recipe at %d^3, %d steps (oracle/idfxref.cpp as it stands, 1 thread of %d host cores)" % (
+                   args.workload, sn, ssteps, os.cpu_count() or 0)}
+
+    if rank == 0:
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "%s: %d^3 periodic ideal MHD, PLM van Leer + HLLD + CT upwind-contact + RK2, CFL %.2f, "
+                                   "seeded random-phase v and B=curl A (|k|<=8, Mach 1, beta 10)" % (args.workload, n, cfl),
+                       "grid": [n, n, n], "cells_per_gpu": cells, "parallelism": "replicas x%d" % world,
+                       "l2": "inputs (%.1f GB state) larger than L2, no flush needed" % (8 * 8 * cells * 1e-9)},
+            "gpu_launches": launches, "clocks": clocks, "e2e": e2e,
+            "roofline": roof, "roofline_step_hbm": roof_step, "kernels": kernels,
+            "fp64_probe": {"tflops": fp64_tflops, "tinst_per_s": fp64_tinst},
+            "cpu_baseline": cpu,
+            "context": "paper: >1e8 cell/s on one V100 (PAPER.md:17), 1.21e8 per V100 in Tab. 4 (PAPER.md:389); other hardware, not the target",
+        }
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

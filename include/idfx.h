@@ -26,8 +26,9 @@
  *     whatever owns device memory in the application, e.g. a torch tensor).  The context owns no large
  *     device allocation; it owns CUDA graphs, TMA descriptors and a few hundred bytes of host memory.
  *   - All work is enqueued on the stream given to idfx_bind (a cudaStream_t cast to void*, NULL = legacy
- *     default stream).  Only idfx_compute_dt, idfx_last_dt, idfx_status, idfx_get_state_host and
- *     idfx_launch_count synchronise with the host.
+ *     default stream).  Only idfx_compute_dt, idfx_last_dt, idfx_status, idfx_set_state_host and
+ *     idfx_get_state_host synchronise with the host (the host-buffer calls return when the copy is done,
+ *     so the caller may reuse or free its buffers immediately).
  *   - Errors: every int-returning call returns IDFX_OK or a negative code; nothing throws or aborts.
  *     idfx_last_error() gives a thread-local message for the last failure.
  */
@@ -72,7 +73,7 @@ int idfx_bind(idfx_ctx* ctx, void* d_workspace, size_t bytes, void* cuda_stream)
 /* Copy-in of the state (O1): Bc from faces, then conserved variables from the primitives.
  * d_bface may be NULL only when emf_mode is NONE (it is ignored then). */
 int idfx_set_state(idfx_ctx* ctx, const double* d_prim, const double* d_bface);
-int idfx_set_state_host(idfx_ctx* ctx, const double* h_prim, const double* h_bface);
+int idfx_set_state_host(idfx_ctx* ctx, const double* h_prim, const double* h_bface); /* synchronises */
 
 /* Copy-out: primitives re-derived from the conserved state and the face field; bface bit-exact. */
 int idfx_get_state(idfx_ctx* ctx, double* d_prim, double* d_bface);
@@ -100,6 +101,15 @@ int idfx_status(idfx_ctx* ctx);
 
 /* Number of kernels of this library launched on behalf of ctx since idfx_bind (graph replays included). */
 long long idfx_launch_count(const idfx_ctx* ctx);
+
+/* Per-kernel timing for the roofline report.  While enabled, every kernel launch of ctx is bracketed by a
+ * CUDA-event pair on the bound stream.  idfx_profile_enable(ctx, 1) clears the accumulators and starts,
+ * (ctx, 0) stops.  idfx_profile_read synchronises and returns the summed device time in milliseconds and
+ * the number of launches of kernel class kernel_id; idfx_profile_kernel_name gives the class names
+ * ("flux_x", "flux_y", "flux_z", "rhs_dtmax", "edge_emf", "ct_update_prim", "ghost_fill", "state_io"), NULL past the end. */
+int idfx_profile_enable(idfx_ctx* ctx, int on);
+int idfx_profile_read(idfx_ctx* ctx, int kernel_id, double* h_ms_total, long long* h_launches);
+const char* idfx_profile_kernel_name(int kernel_id);
 
 const char* idfx_last_error(void);
 void idfx_destroy(idfx_ctx* ctx);

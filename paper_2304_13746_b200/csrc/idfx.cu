@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "../../include/idfx.h"
 #include "physics.cuh"
@@ -151,7 +152,8 @@ __device__ __forceinline__ void prim_from_cons(double gm1, double rho, double mx
   p = gm1 * (E - 0.5 * rho * (vx * vx + vy * vy + vz * vz) - 0.5 * (bx * bx + by * by + bz * bz));
 }
 
-// get_state: primitives from the master state (Bf ghosts are valid whenever this runs).
+// get_state: primitives from the master state into scratch fields (Bf ghosts are valid whenever this runs).
+// The stage-input primitives V are left untouched so that reading the state never perturbs the run.
 template <bool MHD>
 __global__ void k_prim_from_cons(Geom g, StateArgs a) {
   int i, j, k;
@@ -162,9 +164,6 @@ __global__ void k_prim_from_cons(Geom g, StateArgs a) {
     bx = 0.5 * (a.Bf[0][c] + a.Bf[0][c + 1]);
     by = 0.5 * (a.Bf[1][c] + a.Bf[1][c + g.sy]);
     bz = 0.5 * (a.Bf[2][c] + a.Bf[2][c + g.sz]);
-    a.V[5][c] = bx;
-    a.V[6][c] = by;
-    a.V[7][c] = bz;
   }
   double vx, vy, vz, p;
   const double rho = a.U[0][c];
@@ -438,6 +437,11 @@ enum {
 
 using namespace idfx;
 
+// kernel classes for idfx_profile_* (order = idfx_profile_kernel_name)
+enum { K_FLUX_X = 0, K_FLUX_Y, K_FLUX_Z, K_RHS, K_EMF, K_UPDATE, K_FILL, K_STATE, K_COUNT };
+static const char* const kKernelNames[K_COUNT] = {"flux_x", "flux_y", "flux_z", "rhs_dtmax", "edge_emf",
+                                                  "ct_update_prim", "ghost_fill", "state_io"};
+
 struct idfx_ctx {
   Geom g;
   int solver, limiter, emf;
@@ -449,9 +453,62 @@ struct idfx_ctx {
   DevScalars* sc = nullptr;
   int bcur = 0;  // which of the three face-field buffers holds the current state
   long long launches = 0;
+  // optional per-kernel timing with CUDA events on the bound stream (idfx_profile_*)
+  bool prof_on = false;
+  struct ProfRec { cudaEvent_t a, b; int id; };
+  std::vector<ProfRec> prof_pending;
+  std::vector<cudaEvent_t> prof_free;
+  double prof_ms[K_COUNT] = {0};
+  long long prof_n[K_COUNT] = {0};
   double* field(int slot) const { return ws + (size_t)slot * (size_t)g.np; }
   double* bbuf(int which, int d) const { return field(F_BA + 3 * which + d); }
 };
+
+namespace {
+cudaEvent_t prof_event(idfx_ctx* c) {
+  if (!c->prof_free.empty()) {
+    cudaEvent_t e = c->prof_free.back();
+    c->prof_free.pop_back();
+    return e;
+  }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+void prof_drain(idfx_ctx* c) {
+  for (auto& r : c->prof_pending) {
+    float ms = 0.f;
+    cudaEventSynchronize(r.b);
+    cudaEventElapsedTime(&ms, r.a, r.b);
+    c->prof_ms[r.id] += ms;
+    c->prof_n[r.id] += 1;
+    c->prof_free.push_back(r.a);
+    c->prof_free.push_back(r.b);
+  }
+  c->prof_pending.clear();
+}
+// brackets one kernel launch: counts it and, when profiling is on, times it with an event pair
+struct LaunchScope {
+  idfx_ctx* c;
+  int id;
+  cudaEvent_t a = nullptr;
+  LaunchScope(idfx_ctx* c_, int id_) : c(c_), id(id_) {
+    if (c->prof_on) {
+      a = prof_event(c);
+      cudaEventRecord(a, c->stream);
+    }
+  }
+  ~LaunchScope() {
+    c->launches++;
+    if (c->prof_on) {
+      cudaEvent_t b = prof_event(c);
+      cudaEventRecord(b, c->stream);
+      c->prof_pending.push_back({a, b, id});
+      if (c->prof_pending.size() >= 4096) prof_drain(c);
+    }
+  }
+};
+}  // namespace
 
 #define CK(call)                                                          \
   do {                                                                    \
@@ -515,6 +572,7 @@ void launch_flux(idfx_ctx* c, int d, const double* const Bf[3], bool speed_only)
   a.F[5] = c->field(F_FB + 2 * d);
   a.F[6] = c->field(F_FB + 2 * d + 1);
   a.cf = c->field(F_CF + d);
+  LaunchScope ls(c, K_FLUX_X + d);
   if (c->mhd) {
     if (c->solver == SOLVER_HLL) launch_flux_s<SOLVER_HLL, true>(c, a, speed_only);
     else if (c->solver == SOLVER_HLLD) launch_flux_s<SOLVER_HLLD, true>(c, a, speed_only);
@@ -524,7 +582,6 @@ void launch_flux(idfx_ctx* c, int d, const double* const Bf[3], bool speed_only)
     else if (c->solver == SOLVER_HLLC) launch_flux_s<SOLVER_HLLC, false>(c, a, speed_only);
     else launch_flux_s<SOLVER_ROE, false>(c, a, speed_only);
   }
-  c->launches++;
 }
 
 void launch_rhs(idfx_ctx* c, bool want_r, bool want_dt) {
@@ -536,10 +593,10 @@ void launch_rhs(idfx_ctx* c, bool want_r, bool want_dt) {
   for (int n = 0; n < 5; ++n) a.R[n] = c->field(F_R + n);
   a.sc = c->sc;
   const unsigned nb = blocks_for(c->g.nc, 128);
+  LaunchScope ls(c, K_RHS);
   if (want_r && want_dt) k_rhs<true, true><<<nb, 128, 0, c->stream>>>(c->g, a);
   else if (want_r) k_rhs<true, false><<<nb, 128, 0, c->stream>>>(c->g, a);
   else k_rhs<false, true><<<nb, 128, 0, c->stream>>>(c->g, a);
-  c->launches++;
 }
 
 void launch_emf(idfx_ctx* c) {
@@ -553,9 +610,9 @@ void launch_emf(idfx_ctx* c) {
     a.E[d] = c->field(F_E + d);
   }
   const unsigned nb = blocks_for(c->g.nc, 128);
+  LaunchScope ls(c, K_EMF);
   if (c->emf == EMF_UCT) k_emf<true><<<nb, 128, 0, c->stream>>>(c->g, a);
   else k_emf<false><<<nb, 128, 0, c->stream>>>(c->g, a);
-  c->launches++;
 }
 
 void launch_fill(idfx_ctx* c, int which_b) {
@@ -567,8 +624,8 @@ void launch_fill(idfx_ctx* c, int which_b) {
   const Geom& g = c->g;
   const long long px = g.nx + 2 * NG, py = g.ny + 2 * NG;
   const long long nt = 2LL * NG * py * px + (long long)g.nz * 2 * NG * px + (long long)g.nz * g.ny * 2 * NG;
+  LaunchScope ls(c, K_FILL);
   k_fill_ghost<<<blocks_for(nt, 128), 128, 0, c->stream>>>(g, fl);
-  c->launches++;
 }
 
 // One stage S_dt (O2) followed by the RK combine.  bin: face buffer of the stage input; b0: saved face
@@ -596,6 +653,8 @@ void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fi
   a.dt_fixed = dt_fixed;
   a.cfl = cfl;
   const unsigned nb = blocks_for(c->g.nc, 128);
+  {
+    LaunchScope ls(c, K_UPDATE);
   if (c->mhd) {
     if (stage2) k_update<true, true><<<nb, 128, 0, c->stream>>>(c->g, a);
     else k_update<true, false><<<nb, 128, 0, c->stream>>>(c->g, a);
@@ -603,7 +662,7 @@ void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fi
     if (stage2) k_update<false, true><<<nb, 128, 0, c->stream>>>(c->g, a);
     else k_update<false, false><<<nb, 128, 0, c->stream>>>(c->g, a);
   }
-  c->launches++;
+  }
   launch_fill(c, bout);
 }
 
@@ -645,9 +704,10 @@ int finish_set_state(idfx_ctx* c) {
   for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
   a.sc = c->sc;
   const unsigned nb = blocks_for(c->g.nc, 128);
+  { LaunchScope ls(c, K_STATE);
   if (c->mhd) k_cons_from_prim<true><<<nb, 128, 0, c->stream>>>(c->g, a);
   else k_cons_from_prim<false><<<nb, 128, 0, c->stream>>>(c->g, a);
-  c->launches++;
+  }
   launch_fill(c, c->bcur);
   CK(cudaGetLastError());
   return IDFX_OK;
@@ -656,13 +716,15 @@ int finish_set_state(idfx_ctx* c) {
 int refresh_prims(idfx_ctx* c) {
   StateArgs a;
   for (int n = 0; n < 5; ++n) a.U[n] = c->field(F_UA + n);
-  for (int n = 0; n < 8; ++n) a.V[n] = c->field(F_V + n);
+  for (int n = 0; n < 8; ++n) a.V[n] = nullptr;
+  for (int n = 0; n < 5; ++n) a.V[n] = c->field(F_R + n);  // scratch: R is dead between cycles
   for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
   a.sc = c->sc;
   const unsigned nb = blocks_for(c->g.nc, 128);
+  { LaunchScope ls(c, K_STATE);
   if (c->mhd) k_prim_from_cons<true><<<nb, 128, 0, c->stream>>>(c->g, a);
   else k_prim_from_cons<false><<<nb, 128, 0, c->stream>>>(c->g, a);
-  c->launches++;
+  }
   CK(cudaGetLastError());
   return IDFX_OK;
 }
@@ -749,13 +811,15 @@ int idfx_set_state(idfx_ctx* c, const double* d_prim, const double* d_bface) {
   FieldList fl;
   fl.n = 5;
   for (int n = 0; n < 5; ++n) fl.f[n] = c->field(F_V + n);
+  { LaunchScope ls(c, K_STATE);
   k_pack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_prim);
-  c->launches++;
+  }
   if (c->mhd) {
     fl.n = 3;
     for (int d = 0; d < 3; ++d) fl.f[d] = c->bbuf(c->bcur, d);
+    { LaunchScope ls(c, K_STATE);
     k_pack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_bface);
-    c->launches++;
+    }
   }
   return finish_set_state(c);
 }
@@ -773,7 +837,9 @@ int idfx_set_state_host(idfx_ctx* c, const double* h_prim, const double* h_bface
     for (int d = 0; d < 3; ++d)
       if ((rc = copy3d(c, c->bbuf(c->bcur, d), h_bface + (size_t)d * c->g.nc, nullptr, cudaMemcpyHostToDevice)))
         return rc;
-  return finish_set_state(c);
+  if ((rc = finish_set_state(c))) return rc;
+  CK(cudaStreamSynchronize(c->stream));  // the caller may reuse its host buffers as soon as this returns
+  return IDFX_OK;
 }
 
 int idfx_get_state(idfx_ctx* c, double* d_prim, double* d_bface) {
@@ -787,14 +853,16 @@ int idfx_get_state(idfx_ctx* c, double* d_prim, double* d_bface) {
   const unsigned nb = blocks_for(c->g.nc, 128);
   FieldList fl;
   fl.n = 5;
-  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(F_V + n);
+  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(F_R + n);
+  { LaunchScope ls(c, K_STATE);
   k_unpack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_prim);
-  c->launches++;
+  }
   if (c->mhd && d_bface) {
     fl.n = 3;
     for (int d = 0; d < 3; ++d) fl.f[d] = c->bbuf(c->bcur, d);
+    { LaunchScope ls(c, K_STATE);
     k_unpack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_bface);
-    c->launches++;
+    }
   }
   CK(cudaGetLastError());
   return IDFX_OK;
@@ -809,7 +877,7 @@ int idfx_get_state_host(idfx_ctx* c, double* h_prim, double* h_bface) {
   }
   if ((rc = refresh_prims(c))) return rc;
   for (int n = 0; n < 5; ++n)
-    if ((rc = copy3d(c, c->field(F_V + n), nullptr, h_prim + (size_t)n * c->g.nc, cudaMemcpyDeviceToHost))) return rc;
+    if ((rc = copy3d(c, c->field(F_R + n), nullptr, h_prim + (size_t)n * c->g.nc, cudaMemcpyDeviceToHost))) return rc;
   if (c->mhd && h_bface)
     for (int d = 0; d < 3; ++d)
       if ((rc = copy3d(c, c->bbuf(c->bcur, d), nullptr, h_bface + (size_t)d * c->g.nc, cudaMemcpyDeviceToHost)))
@@ -829,13 +897,15 @@ int idfx_get_conserved(idfx_ctx* c, double* d_cons, double* d_bface) {
   FieldList fl;
   fl.n = 5;
   for (int n = 0; n < 5; ++n) fl.f[n] = c->field(F_UA + n);
+  { LaunchScope ls(c, K_STATE);
   k_unpack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_cons);
-  c->launches++;
+  }
   if (c->mhd && d_bface) {
     fl.n = 3;
     for (int d = 0; d < 3; ++d) fl.f[d] = c->bbuf(c->bcur, d);
+    { LaunchScope ls(c, K_STATE);
     k_unpack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_bface);
-    c->launches++;
+    }
   }
   CK(cudaGetLastError());
   return IDFX_OK;
@@ -908,6 +978,40 @@ int idfx_status(idfx_ctx* c) {
 
 long long idfx_launch_count(const idfx_ctx* c) { return c ? c->launches : 0; }
 
-void idfx_destroy(idfx_ctx* c) { delete c; }
+int idfx_profile_enable(idfx_ctx* c, int on) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  prof_drain(c);
+  for (int k = 0; k < K_COUNT; ++k) {
+    c->prof_ms[k] = 0.0;
+    c->prof_n[k] = 0;
+  }
+  c->prof_on = on != 0;
+  return IDFX_OK;
+}
+
+int idfx_profile_read(idfx_ctx* c, int kernel_id, double* h_ms_total, long long* h_launches) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (kernel_id < 0 || kernel_id >= K_COUNT || !h_ms_total || !h_launches) {
+    set_err("idfx_profile_read: bad kernel id or null output");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  prof_drain(c);
+  *h_ms_total = c->prof_ms[kernel_id];
+  *h_launches = c->prof_n[kernel_id];
+  return IDFX_OK;
+}
+
+const char* idfx_profile_kernel_name(int kernel_id) {
+  return (kernel_id >= 0 && kernel_id < K_COUNT) ? kKernelNames[kernel_id] : nullptr;
+}
+
+void idfx_destroy(idfx_ctx* c) {
+  if (!c) return;
+  prof_drain(c);
+  for (cudaEvent_t e : c->prof_free) cudaEventDestroy(e);
+  delete c;
+}
 
 }  // extern "C"

@@ -22,6 +22,8 @@ SYMBOLS = (
     "idfx_create", "idfx_workspace_bytes", "idfx_bind", "idfx_set_state", "idfx_set_state_host",
     "idfx_get_state", "idfx_get_state_host", "idfx_get_conserved", "idfx_compute_dt", "idfx_step",
     "idfx_advance", "idfx_last_dt", "idfx_status", "idfx_launch_count", "idfx_last_error", "idfx_destroy",
+    "idfx_profile_enable", "idfx_profile_read", "idfx_profile_kernel_name",
+    "idfx_probe_fp64",
 )
 
 _lib = None
@@ -56,6 +58,11 @@ def lib():
         L.idfx_status.argtypes = [vp]
         L.idfx_launch_count.argtypes = [vp]
         L.idfx_launch_count.restype = ctypes.c_longlong
+        L.idfx_profile_enable.argtypes = [vp, ci]
+        L.idfx_profile_read.argtypes = [vp, ci, dp, ctypes.POINTER(ctypes.c_longlong)]
+        L.idfx_profile_kernel_name.argtypes = [ci]
+        L.idfx_profile_kernel_name.restype = ctypes.c_char_p
+        L.idfx_probe_fp64.argtypes = [vp, ci, dp, dp]
         L.idfx_last_error.restype = ctypes.c_char_p
         L.idfx_destroy.argtypes = [vp]
         L.idfx_destroy.restype = None
@@ -66,6 +73,15 @@ def lib():
 def _check(rc):
     if rc != OK:
         raise IdfxError(rc, lib().idfx_last_error().decode())
+
+
+def probe_fp64(repeats=5):
+    """(TFLOP/s, 1e12 fp64 instructions/s) of chains of independent DFMAs on the current device."""
+    tf, ti = ctypes.c_double(), ctypes.c_double()
+    rc = lib().idfx_probe_fp64(torch.cuda.current_stream().cuda_stream, repeats, ctypes.byref(tf), ctypes.byref(ti))
+    if rc != OK:
+        raise IdfxError(rc, "fp64 probe failed")
+    return tf.value, ti.value
 
 
 class Idfx:
@@ -149,3 +165,19 @@ class Idfx:
 
     def launch_count(self):
         return self.L.idfx_launch_count(self.h)
+
+    def profile(self, on):
+        _check(self.L.idfx_profile_enable(self.h, 1 if on else 0))
+
+    def profile_read(self):
+        """{kernel class: (total ms, launches)} accumulated since profile(True)."""
+        out = {}
+        k = 0
+        while True:
+            name = self.L.idfx_profile_kernel_name(k)
+            if name is None:
+                return out
+            ms, n = ctypes.c_double(), ctypes.c_longlong()
+            _check(self.L.idfx_profile_read(self.h, k, ctypes.byref(ms), ctypes.byref(n)))
+            out[name.decode()] = (ms.value, n.value)
+            k += 1

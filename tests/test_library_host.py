@@ -22,8 +22,9 @@ def L():
 
 
 def test_exports_every_declared_symbol(L):
-    header = open(os.path.join(ROOT, "include", "idfx.h")).read()
-    declared = set(re.findall(r"\b(idfx_[a-z_]+)\s*\(", header))
+    inc = os.path.join(ROOT, "include")
+    header = "".join(open(os.path.join(inc, f)).read() for f in sorted(os.listdir(inc)) if f.endswith(".h"))
+    declared = set(re.findall(r"\b(idfx_[a-z0-9_]+)\s*\(", header))
     assert declared == set(idfx.SYMBOLS)
     raw = ctypes.CDLL(idfx.LIB_PATH)
     for s in declared:
