@@ -1,0 +1,49 @@
+// common.cuh — geometry of the padded fields and the device scalars shared by all kernels of the idfx CUDA path.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace idfx {
+
+constexpr int NG = 2;
+constexpr int IOFF = 16;
+
+struct Geom {
+  int nx, ny, nz;
+  int sy;         // row pitch in doubles
+  long long sz;   // plane stride in doubles
+  long long np;   // padded field size in doubles
+  long long nc;   // nx*ny*nz
+  double dx, gamma;
+  __host__ __device__ __forceinline__ long long at(int i, int j, int k) const {
+    return (long long)(k + NG) * sz + (long long)(j + NG) * sy + (i + IOFF);
+  }
+};
+
+// flat thread index -> active cell
+__device__ __forceinline__ bool cell_of_thread(const Geom& g, int& i, int& j, int& k) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= g.nc) return false;
+  i = (int)(t % g.nx);
+  const long long r = t / g.nx;
+  j = (int)(r % g.ny);
+  k = (int)(r / g.ny);
+  return true;
+}
+
+struct DevScalars {
+  unsigned long long smax_bits;  // bit pattern of max_cells sum_d c_d/dx (positive doubles order like integers)
+  double dt_used;
+  int flag;
+};
+
+// block-wide maximum for blocks of exactly 128 threads; every thread must call it
+__device__ __forceinline__ double block_max_128(double v) {
+  __shared__ double red[4];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  return fmax(fmax(red[0], red[1]), fmax(red[2], red[3]));
+}
+
+}  // namespace idfx

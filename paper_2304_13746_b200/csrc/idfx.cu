@@ -12,41 +12,11 @@
 #include <vector>
 
 #include "../../include/idfx.h"
+#include "common.cuh"
 #include "physics.cuh"
+#include "flux_march.cuh"
 
 namespace idfx {
-
-constexpr int NG = 2;
-constexpr int IOFF = 16;
-
-struct Geom {
-  int nx, ny, nz;
-  int sy;         // row pitch in doubles
-  long long sz;   // plane stride in doubles
-  long long np;   // padded field size in doubles
-  long long nc;   // nx*ny*nz
-  double dx, gamma;
-  __host__ __device__ __forceinline__ long long at(int i, int j, int k) const {
-    return (long long)(k + NG) * sz + (long long)(j + NG) * sy + (i + IOFF);
-  }
-};
-
-// flat thread index -> active cell
-__device__ __forceinline__ bool cell_of_thread(const Geom& g, int& i, int& j, int& k) {
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= g.nc) return false;
-  i = (int)(t % g.nx);
-  const long long r = t / g.nx;
-  j = (int)(r % g.ny);
-  k = (int)(r / g.ny);
-  return true;
-}
-
-struct DevScalars {
-  unsigned long long smax_bits;  // bit pattern of max_cells sum_d c_d/dx (positive doubles order like integers)
-  double dt_used;
-  int flag;
-};
 
 // ---------------------------------------------------------------------------------------------
 // copy-in / copy-out between the caller's contiguous arrays and the padded fields
@@ -228,15 +198,6 @@ struct RhsArgs {
   double* R[5];
   DevScalars* sc;
 };
-
-__device__ __forceinline__ double block_max_128(double v) {
-  __shared__ double red[4];
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
-  __syncthreads();
-  return fmax(fmax(red[0], red[1]), fmax(red[2], red[3]));
-}
 
 template <bool WANT_R, bool WANT_DT>
 __global__ void __launch_bounds__(128) k_rhs(Geom g, RhsArgs a) {
@@ -428,9 +389,11 @@ enum {
   F_R = 27,    // 5: flux divergence
   F_FB = 32,   // 6: face fluxes of B, [d][0..1]
   F_E = 38,    // 3: edge EMFs
-  F_FH = 41,   // 15: face fluxes of (rho, m, E), [d][0..4]
-  F_CF = 56,   // 3: c_face
-  F_COUNT = 59
+  F_FX = 41,   // 5: x-face fluxes of (rho, m, E); F_FX+0 doubles as the x mass flux
+  F_CFX = 46,  // 1: c_face of the x sweep
+  F_FM = 47,   // 3: face mass fluxes of the y, z sweeps at +1, +2 (slot +0 unused)
+  F_CS = 50,   // 1: sum_d c_d per cell (x and y parts)
+  F_COUNT = 51
 };
 
 }  // namespace idfx
@@ -535,68 +498,142 @@ int check_bound(const idfx_ctx* c) {
   return IDFX_OK;
 }
 
-template <int SOLVER, int LIM, bool MHD>
-void launch_flux_sl(idfx_ctx* c, const FluxArgs& a, bool speed_only) {
-  const unsigned nb = blocks_for(c->g.nc, 128);
-  if (speed_only)
-    k_flux_face<SOLVER, LIM, MHD, true><<<nb, 128, 0, c->stream>>>(c->g, a);
-  else
-    k_flux_face<SOLVER, LIM, MHD, false><<<nb, 128, 0, c->stream>>>(c->g, a);
+// ---- standalone dt (idfx_compute_dt): signal speeds on every face, then the per-cell sum and the max ----
+template <int LIM, bool MHD>
+void launch_speed_l(idfx_ctx* c, const FluxArgs& a) {
+  k_flux_face<SOLVER_HLL, LIM, MHD, true><<<blocks_for(c->g.nc, 128), 128, 0, c->stream>>>(c->g, a);
 }
 
-template <int SOLVER, bool MHD>
-void launch_flux_s(idfx_ctx* c, const FluxArgs& a, bool speed_only) {
-  switch (c->limiter) {
-    case LIM_FLAT: launch_flux_sl<SOLVER, LIM_FLAT, MHD>(c, a, speed_only); break;
-    case LIM_MINMOD: launch_flux_sl<SOLVER, LIM_MINMOD, MHD>(c, a, speed_only); break;
-    default: launch_flux_sl<SOLVER, LIM_VANLEER, MHD>(c, a, speed_only);
-  }
-}
-
-void launch_flux(idfx_ctx* c, int d, const double* const Bf[3], bool speed_only) {
+void launch_speed(idfx_ctx* c, int d, const double* const Bf[3]) {
   const int ia = d, ib = (d + 1) % 3, ie = (d + 2) % 3;
   const long long st[3] = {1, c->g.sy, c->g.sz};
   FluxArgs a;
-  double* V = c->field(F_V);
-  const long long np = c->g.np;
-  a.q[0] = V;
-  a.q[1] = V + (1 + ia) * np;
-  a.q[2] = V + (1 + ib) * np;
-  a.q[3] = V + (1 + ie) * np;
-  a.q[4] = V + 4 * np;
-  a.q[5] = V + (5 + ib) * np;
-  a.q[6] = V + (5 + ie) * np;
+  a.q[0] = c->field(F_V);
+  a.q[1] = c->field(F_V + 1 + ia);
+  a.q[2] = c->field(F_V + 1 + ib);
+  a.q[3] = c->field(F_V + 1 + ie);
+  a.q[4] = c->field(F_V + 4);
+  a.q[5] = c->field(F_V + 5 + ib);
+  a.q[6] = c->field(F_V + 5 + ie);
   a.bn = c->mhd ? Bf[ia] : nullptr;
   a.sd = st[d];
-  for (int n = 0; n < 5; ++n) a.F[n] = c->field(F_FH + 5 * d + n);
-  a.F[5] = c->field(F_FB + 2 * d);
-  a.F[6] = c->field(F_FB + 2 * d + 1);
-  a.cf = c->field(F_CF + d);
+  for (int n = 0; n < 7; ++n) a.F[n] = nullptr;
+  a.cf = c->field(F_R + d);  // scratch: R is dead between cycles
   LaunchScope ls(c, K_FLUX_X + d);
   if (c->mhd) {
-    if (c->solver == SOLVER_HLL) launch_flux_s<SOLVER_HLL, true>(c, a, speed_only);
-    else if (c->solver == SOLVER_HLLD) launch_flux_s<SOLVER_HLLD, true>(c, a, speed_only);
-    else launch_flux_s<SOLVER_ROE, true>(c, a, speed_only);
+    if (c->limiter == LIM_FLAT) launch_speed_l<LIM_FLAT, true>(c, a);
+    else if (c->limiter == LIM_MINMOD) launch_speed_l<LIM_MINMOD, true>(c, a);
+    else launch_speed_l<LIM_VANLEER, true>(c, a);
   } else {
-    if (c->solver == SOLVER_HLL) launch_flux_s<SOLVER_HLL, false>(c, a, speed_only);
-    else if (c->solver == SOLVER_HLLC) launch_flux_s<SOLVER_HLLC, false>(c, a, speed_only);
-    else launch_flux_s<SOLVER_ROE, false>(c, a, speed_only);
+    if (c->limiter == LIM_FLAT) launch_speed_l<LIM_FLAT, false>(c, a);
+    else if (c->limiter == LIM_MINMOD) launch_speed_l<LIM_MINMOD, false>(c, a);
+    else launch_speed_l<LIM_VANLEER, false>(c, a);
   }
 }
 
-void launch_rhs(idfx_ctx* c, bool want_r, bool want_dt) {
+void launch_dtmax(idfx_ctx* c) {
   RhsArgs a;
   for (int d = 0; d < 3; ++d) {
-    for (int n = 0; n < 5; ++n) a.F[d][n] = c->field(F_FH + 5 * d + n);
-    a.cf[d] = c->field(F_CF + d);
+    for (int n = 0; n < 5; ++n) a.F[d][n] = nullptr;
+    a.cf[d] = c->field(F_R + d);
   }
-  for (int n = 0; n < 5; ++n) a.R[n] = c->field(F_R + n);
+  for (int n = 0; n < 5; ++n) a.R[n] = nullptr;
   a.sc = c->sc;
-  const unsigned nb = blocks_for(c->g.nc, 128);
   LaunchScope ls(c, K_RHS);
-  if (want_r && want_dt) k_rhs<true, true><<<nb, 128, 0, c->stream>>>(c->g, a);
-  else if (want_r) k_rhs<true, false><<<nb, 128, 0, c->stream>>>(c->g, a);
-  else k_rhs<false, true><<<nb, 128, 0, c->stream>>>(c->g, a);
+  k_rhs<false, true><<<blocks_for(c->g.nc, 128), 128, 0, c->stream>>>(c->g, a);
+}
+
+// ---- the three flux sweeps of one stage --------------------------------------------------------
+template <int SOLVER, int LIM, bool MHD>
+void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
+  const Geom& g = c->g;
+  const bool uct = c->emf == EMF_UCT;
+  {  // x: faces 0..nx of every row
+    FluxXArgs a;
+    a.q[0] = c->field(F_V);
+    a.q[1] = c->field(F_V + 1);
+    a.q[2] = c->field(F_V + 2);
+    a.q[3] = c->field(F_V + 3);
+    a.q[4] = c->field(F_V + 4);
+    a.q[5] = c->field(F_V + 6);
+    a.q[6] = c->field(F_V + 7);
+    a.bn = MHD ? Bf[0] : nullptr;
+    for (int n = 0; n < 5; ++n) a.FH[n] = c->field(F_FX + n);
+    a.FB[0] = c->field(F_FB + 0);
+    a.FB[1] = c->field(F_FB + 1);
+    a.cf = c->field(F_CFX);
+    const int gx = (g.nx + 1 + 30) / 31;
+    const long long nrows = (long long)g.ny * g.nz;
+    long long rpw = gx * nrows / 9472;
+    rpw = rpw < 1 ? 1 : (rpw > 32 ? 32 : rpw);
+    a.rows_per_warp = (int)rpw;
+    dim3 grid(gx, (unsigned)((nrows + 4 * rpw - 1) / (4 * rpw)));
+    LaunchScope ls(c, K_FLUX_X);
+    k_flux_x<SOLVER, LIM, MHD><<<grid, 128, 0, c->stream>>>(g, a);
+  }
+  for (int d = 1; d < 3; ++d) {  // y then z: marching pencils
+    const int ib = (d + 1) % 3, ie = (d + 2) % 3;
+    FluxMArgs a;
+    a.q[0] = c->field(F_V);
+    a.q[1] = c->field(F_V + 1 + d);
+    a.q[2] = c->field(F_V + 1 + ib);
+    a.q[3] = c->field(F_V + 1 + ie);
+    a.q[4] = c->field(F_V + 4);
+    a.q[5] = c->field(F_V + 5 + ib);
+    a.q[6] = c->field(F_V + 5 + ie);
+    a.bn = MHD ? Bf[d] : nullptr;
+    a.sd = d == 1 ? g.sy : g.sz;
+    a.st = d == 1 ? g.sz : g.sy;
+    a.ns = d == 1 ? g.ny : g.nz;
+    a.nt = d == 1 ? g.nz : g.ny;
+    for (int n = 0; n < 5; ++n) {
+      a.FX[n] = c->field(F_FX + n);
+      a.R[n] = c->field(F_R + n);
+    }
+    a.cfx = c->field(F_CFX);
+    a.csum = c->field(F_CS);
+    a.FB[0] = c->field(F_FB + 2 * d);
+    a.FB[1] = c->field(F_FB + 2 * d + 1);
+    a.FM = c->field(F_FM + d);
+    a.sc = c->sc;
+    const long long per_chunk = (long long)((g.nx + 31) / 32) * ((a.nt + 3) / 4);
+    long long nch = (148 * 16 + per_chunk - 1) / per_chunk;
+    const long long maxch = a.ns / 8 > 0 ? a.ns / 8 : 1;
+    nch = nch < 1 ? 1 : (nch > maxch ? maxch : nch);
+    a.chunk = (int)((a.ns + nch - 1) / nch);
+    dim3 grid((g.nx + 31) / 32, (a.nt + 3) / 4, (unsigned)((a.ns + a.chunk - 1) / a.chunk));
+    LaunchScope ls(c, K_FLUX_X + d);
+    if (d == 1) {
+      if (want_dt) k_flux_march<SOLVER, LIM, MHD, 1, true, true><<<grid, 128, 0, c->stream>>>(g, a);
+      else if (uct) k_flux_march<SOLVER, LIM, MHD, 1, false, true><<<grid, 128, 0, c->stream>>>(g, a);
+      else k_flux_march<SOLVER, LIM, MHD, 1, false, false><<<grid, 128, 0, c->stream>>>(g, a);
+    } else {
+      if (want_dt) k_flux_march<SOLVER, LIM, MHD, 2, true, true><<<grid, 128, 0, c->stream>>>(g, a);
+      else if (uct) k_flux_march<SOLVER, LIM, MHD, 2, false, true><<<grid, 128, 0, c->stream>>>(g, a);
+      else k_flux_march<SOLVER, LIM, MHD, 2, false, false><<<grid, 128, 0, c->stream>>>(g, a);
+    }
+  }
+}
+
+template <int SOLVER, bool MHD>
+void launch_sweeps_s(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
+  switch (c->limiter) {
+    case LIM_FLAT: launch_sweeps_t<SOLVER, LIM_FLAT, MHD>(c, Bf, want_dt); break;
+    case LIM_MINMOD: launch_sweeps_t<SOLVER, LIM_MINMOD, MHD>(c, Bf, want_dt); break;
+    default: launch_sweeps_t<SOLVER, LIM_VANLEER, MHD>(c, Bf, want_dt);
+  }
+}
+
+void launch_sweeps(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
+  if (c->mhd) {
+    if (c->solver == SOLVER_HLL) launch_sweeps_s<SOLVER_HLL, true>(c, Bf, want_dt);
+    else if (c->solver == SOLVER_HLLD) launch_sweeps_s<SOLVER_HLLD, true>(c, Bf, want_dt);
+    else launch_sweeps_s<SOLVER_ROE, true>(c, Bf, want_dt);
+  } else {
+    if (c->solver == SOLVER_HLL) launch_sweeps_s<SOLVER_HLL, false>(c, Bf, want_dt);
+    else if (c->solver == SOLVER_HLLC) launch_sweeps_s<SOLVER_HLLC, false>(c, Bf, want_dt);
+    else launch_sweeps_s<SOLVER_ROE, false>(c, Bf, want_dt);
+  }
 }
 
 void launch_emf(idfx_ctx* c) {
@@ -604,7 +641,7 @@ void launch_emf(idfx_ctx* c) {
   for (int d = 0; d < 3; ++d) {
     a.FB[d][0] = c->field(F_FB + 2 * d);
     a.FB[d][1] = c->field(F_FB + 2 * d + 1);
-    a.FM[d] = c->field(F_FH + 5 * d);
+    a.FM[d] = d == 0 ? c->field(F_FX) : c->field(F_FM + d);
     a.v[d] = c->field(F_V + 1 + d);
     a.Bc[d] = c->field(F_V + 5 + d);
     a.E[d] = c->field(F_E + d);
@@ -632,8 +669,7 @@ void launch_fill(idfx_ctx* c, int which_b) {
 // buffer; bout: destination.
 void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fixed, double cfl, bool want_dt) {
   const double* Bf[3] = {c->bbuf(bin, 0), c->bbuf(bin, 1), c->bbuf(bin, 2)};
-  for (int d = 0; d < 3; ++d) launch_flux(c, d, Bf, false);
-  launch_rhs(c, true, want_dt);
+  launch_sweeps(c, Bf, want_dt);
   if (c->mhd) launch_emf(c);
   UpdateArgs a;
   for (int n = 0; n < 5; ++n) {
@@ -920,8 +956,8 @@ int idfx_compute_dt(idfx_ctx* c, double cfl, double* h_dt_out) {
   }
   CK(cudaMemsetAsync(&c->sc->smax_bits, 0, sizeof(unsigned long long), c->stream));
   const double* Bf[3] = {c->bbuf(c->bcur, 0), c->bbuf(c->bcur, 1), c->bbuf(c->bcur, 2)};
-  for (int d = 0; d < 3; ++d) launch_flux(c, d, Bf, true);
-  launch_rhs(c, false, true);
+  for (int d = 0; d < 3; ++d) launch_speed(c, d, Bf);
+  launch_dtmax(c);
   CK(cudaGetLastError());
   unsigned long long bits = 0;
   CK(cudaMemcpyAsync(&bits, &c->sc->smax_bits, sizeof(bits), cudaMemcpyDeviceToHost, c->stream));
