@@ -14,6 +14,13 @@
 #include "common.cuh"
 #include "physics.cuh"
 
+#ifndef IDFX_MINB_X
+#define IDFX_MINB_X 2
+#endif
+#ifndef IDFX_MINB_M
+#define IDFX_MINB_M 2
+#endif
+
 namespace idfx {
 
 struct FluxXArgs {
@@ -27,7 +34,7 @@ struct FluxXArgs {
 
 // lane l of a warp owns cell ci = f0 - 1 + l of one row; lanes 1..31 solve the left face of their cell.
 template <int SOLVER, int LIM, bool MHD>
-__global__ void __launch_bounds__(128) k_flux_x(Geom g, FluxXArgs a) {
+__global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a) {
   constexpr int NQ = MHD ? 7 : 5;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int f0 = 31 * blockIdx.x;
@@ -107,7 +114,7 @@ struct FluxMArgs {
 
 // DIR = 1: y sweep, R = dF_x + dF_y (and csum = c_x + c_y).  DIR = 2: z sweep, R += dF_z (and the dt reduction).
 template <int SOLVER, int LIM, bool MHD, int DIR, bool WANT_DT, bool WANT_FM>
-__global__ void __launch_bounds__(128) k_flux_march(Geom g, FluxMArgs a) {
+__global__ void __launch_bounds__(128, IDFX_MINB_M) k_flux_march(Geom g, FluxMArgs a) {
   constexpr int NQ = MHD ? 7 : 5;
   // local momentum components (n, t1, t2) -> global slot in R
   constexpr int PN = 1 + DIR, PT1 = 1 + (DIR + 1) % 3, PT2 = 1 + (DIR + 2) % 3;
@@ -120,19 +127,14 @@ __global__ void __launch_bounds__(128) k_flux_march(Geom g, FluxMArgs a) {
   if (active) {
     const long long sd = a.sd;
     long long c = g.at(i, 0, 0) + (long long)t * a.st + (long long)(s0 - 2) * sd;  // cell s0-2
-    double qm[7], q0[7], qp[7], WL[7];
+    double dm[7], q0[7], qp[7], WL[7];  // dm = q(s) - q(s-1): the forward difference of the previous cell
 #pragma unroll
     for (int n = 0; n < NQ; ++n) {
-      qm[n] = a.q[n][c];
-      q0[n] = a.q[n][c + sd];
-      qp[n] = a.q[n][c + 2 * sd];
-    }
-#pragma unroll
-    for (int n = 0; n < NQ; ++n) {
-      const double s = limited_slope<LIM>(q0[n] - qm[n], qp[n] - q0[n]);  // slope of cell s0-1
-      WL[n] = q0[n] + 0.5 * s;
-      qm[n] = q0[n];
-      q0[n] = qp[n];
+      const double qm = a.q[n][c];
+      const double qc = a.q[n][c + sd];
+      q0[n] = a.q[n][c + 2 * sd];
+      dm[n] = q0[n] - qc;
+      WL[n] = qc + 0.5 * limited_slope<LIM>(qc - qm, dm[n]);  // slope of cell s0-1
     }
     c += 2 * sd;  // cell s0 = right cell of face s0
 #pragma unroll
@@ -166,9 +168,11 @@ __global__ void __launch_bounds__(128) k_flux_march(Geom g, FluxMArgs a) {
       double WR[7], WLn[7];
 #pragma unroll
       for (int n = 0; n < NQ; ++n) {
-        const double sl = limited_slope<LIM>(q0[n] - qm[n], qp[n] - q0[n]);
+        const double dp = qp[n] - q0[n];
+        const double sl = limited_slope<LIM>(dm[n], dp);
         WR[n] = q0[n] - 0.5 * sl;
         WLn[n] = q0[n] + 0.5 * sl;
+        dm[n] = dp;
       }
       if (!MHD) WR[5] = WR[6] = 0.0;
       double F[7];
@@ -196,7 +200,6 @@ __global__ void __launch_bounds__(128) k_flux_march(Geom g, FluxMArgs a) {
 #pragma unroll
       for (int n = 0; n < NQ; ++n) {
         WL[n] = WLn[n];
-        qm[n] = q0[n];
         q0[n] = qp[n];
         qp[n] = qn[n];
       }

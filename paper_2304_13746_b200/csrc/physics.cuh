@@ -19,6 +19,49 @@ enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2 };
 
 #define IDFX_DEV __device__ __forceinline__
 
+// Reciprocal and square root without the IEEE slow paths: hardware seed (upper 32 bits, ~2^-20) refined by two
+// Newton steps in fp64, result within ~1 ulp.  All operands on this path are normal, finite and non-negative
+// where a root is taken; zero is handled explicitly.  -DIDFX_PRECISE_MATH restores the correctly rounded forms.
+IDFX_DEV double rcp(double x) {
+#ifdef IDFX_PRECISE_MATH
+  return 1.0 / x;
+#else
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-x, y, 1.0);
+  return fma(y, e, y);
+#endif
+}
+
+// 1/sqrt(x) for x > 0
+IDFX_DEV double rsqrt_pos(double x) {
+#ifdef IDFX_PRECISE_MATH
+  return 1.0 / sqrt(x);
+#else
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double h = 0.5 * x;
+  double e = fma(-h * y, y, 0.5);  // (1 - x y^2)/2
+  y = fma(y, e, y);
+  e = fma(-h * y, y, 0.5);
+  return fma(y, e, y);
+#endif
+}
+
+// sqrt(x) for x >= 0 (exactly 0 for x below 1e-300)
+IDFX_DEV double sqrt_nn(double x) {
+#ifdef IDFX_PRECISE_MATH
+  return sqrt(x);
+#else
+  const double y = rsqrt_pos(fmax(x, 1e-300));
+  double s = x * y;
+  s = fma(fma(-s, s, x), 0.5 * y, s);  // one correction step
+  return x > 1e-300 ? s : 0.0;
+#endif
+}
+
 // O3 / G2: limited slope from the backward and forward differences.
 template <int LIM>
 IDFX_DEV double limited_slope(double dm, double dp) {
@@ -27,7 +70,7 @@ IDFX_DEV double limited_slope(double dm, double dp) {
   if (LIM == LIM_VANLEER) {
     const bool mono = prod > 0.0;
     const double den = mono ? (dm + dp) : 1.0;  // keeps the division off its slow path at extrema
-    const double s = (2.0 * prod) / den;
+    const double s = (2.0 * prod) * rcp(den);
     return mono ? s : 0.0;
   } else {
     const double s = (fabs(dm) < fabs(dp)) ? dm : dp;
@@ -76,14 +119,14 @@ IDFX_DEV void side_cons_flux(const double W[7], double Bn, double igm1, double U
 // O4: sound speed (HD) or fast magnetosonic speed along the sweep direction (MHD).
 template <bool MHD>
 IDFX_DEV double signal_speed(const double W[7], double Bn, double g) {
-  const double ir = 1.0 / W[0];
+  const double ir = rcp(W[0]);
   const double a2 = g * W[4] * ir;
-  if (!MHD) return sqrt(a2);
+  if (!MHD) return sqrt_nn(a2);
   const double bn2 = Bn * Bn * ir;
   const double b2 = bn2 + (W[5] * W[5] + W[6] * W[6]) * ir;
   const double s = a2 + b2;
   const double disc = fmax(s * s - 4.0 * a2 * bn2, 0.0);
-  return sqrt(0.5 * (s + sqrt(disc)));
+  return sqrt_nn(0.5 * (s + sqrt_nn(disc)));
 }
 
 // O4 / G5: Davis estimate of the outer speeds; c_face = max(|S_L|,|S_R|) for every solver.
@@ -98,7 +141,7 @@ IDFX_DEV void outer_speeds(const double WL[7], const double WR[7], double Bn, do
 template <int NV>
 IDFX_DEV void hll_inner(const double UL[7], const double UR[7], const double FL[7], const double FR[7], double SL,
                         double SR, double F[7]) {
-  const double inv = 1.0 / (SR - SL);
+  const double inv = rcp(SR - SL);
   const double ss = SL * SR;
 #pragma unroll
   for (int n = 0; n < NV; ++n) F[n] = (SR * FL[n] - SL * FR[n] + ss * (UR[n] - UL[n])) * inv;
@@ -109,19 +152,19 @@ IDFX_DEV void hllc_inner(const double WL[7], const double WR[7], const double UL
                          const double FL[7], const double FR[7], double SL, double SR, double F[7]) {
   const double qL = WL[0] * (SL - WL[1]);  // rho_L (S_L - u_L)
   const double qR = WR[0] * (SR - WR[1]);
-  const double SS = (WR[4] - WL[4] + qL * WL[1] - qR * WR[1]) / (qL - qR);
+  const double SS = (WR[4] - WL[4] + qL * WL[1] - qR * WR[1]) * rcp(qL - qR);
   const bool left = SS >= 0.0;
   const double SK = left ? SL : SR;
   const double qK = left ? qL : qR;
   const double rK = left ? WL[0] : WR[0], uK = left ? WL[1] : WR[1], vK = left ? WL[2] : WR[2];
   const double wK = left ? WL[3] : WR[3], pK = left ? WL[4] : WR[4], EK = left ? UL[4] : UR[4];
-  const double fac = qK / (SK - SS);
+  const double fac = qK * rcp(SK - SS);
   double Us[5];
   Us[0] = fac;
   Us[1] = fac * SS;
   Us[2] = fac * vK;
   Us[3] = fac * wK;
-  Us[4] = fac * (EK / rK + (SS - uK) * (SS + pK / qK));
+  Us[4] = fac * (EK * rcp(rK) + (SS - uK) * (SS + pK * rcp(qK)));
 #pragma unroll
   for (int n = 0; n < 5; ++n) {
     const double Fk = left ? FL[n] : FR[n];
@@ -138,18 +181,18 @@ IDFX_DEV void hlld_inner(const double WL[7], const double WR[7], double Bn, cons
   const double uL = WL[1], uR = WR[1];
   const double sL = SL - uL, sR = SR - uR;
   const double qL = WL[0] * sL, qR = WR[0] * sR;  // rho_K (S_K - u_K)
-  const double iD = 1.0 / (qR - qL);
+  const double iD = rcp(qR - qL);
   const double SM = (qR * uR - qL * uL - pTR + pTL) * iD;
   const double pTs = (qR * pTL - qL * pTR + qL * qR * (uR - uL)) * iD;
   const double Bn2 = Bn * Bn;
 
-  const double iL = 1.0 / (SL - SM), iR = 1.0 / (SR - SM);
+  const double iL = rcp(SL - SM), iR = rcp(SR - SM);
   const double rsL = qL * iL, rsR = qR * iR;  // rho*_K
   double vsL, wsL, BysL, BzsL, vsR, wsR, BysR, BzsR;
   {
     const double d = qL * (SL - SM) - Bn2;
     const bool deg = fabs(d) < 1e-12 * qL * sL;
-    const double id = 1.0 / (deg ? 1.0 : d);
+    const double id = rcp(deg ? 1.0 : d);
     const double f = deg ? 0.0 : Bn * (SM - uL) * id;
     const double h = deg ? 1.0 : (qL * sL - Bn2) * id;
     vsL = WL[2] - WL[5] * f;
@@ -160,7 +203,7 @@ IDFX_DEV void hlld_inner(const double WL[7], const double WR[7], double Bn, cons
   {
     const double d = qR * (SR - SM) - Bn2;
     const bool deg = fabs(d) < 1e-12 * qR * sR;
-    const double id = 1.0 / (deg ? 1.0 : d);
+    const double id = rcp(deg ? 1.0 : d);
     const double f = deg ? 0.0 : Bn * (SM - uR) * id;
     const double h = deg ? 1.0 : (qR * sR - Bn2) * id;
     vsR = WR[2] - WR[5] * f;
@@ -168,9 +211,10 @@ IDFX_DEV void hlld_inner(const double WL[7], const double WR[7], double Bn, cons
     BysR = WR[5] * h;
     BzsR = WR[6] * h;
   }
-  const double sqL = sqrt(rsL), sqR = sqrt(rsR);
+  const double ysL = rsqrt_pos(rsL), ysR = rsqrt_pos(rsR);  // 1/sqrt(rho*_K)
+  const double sqL = rsL * ysL, sqR = rsR * ysR;
   const double aBn = fabs(Bn);
-  const double SsL = SM - aBn / sqL, SsR = SM + aBn / sqR;
+  const double SsL = SM - aBn * ysL, SsR = SM + aBn * ysR;
 
   // side selection in the order of O7: S*_L >= 0 -> U*_L ; S*_R <= 0 -> U*_R ; S_M >= 0 -> U**_L ; else U**_R
   const bool starL = SsL >= 0.0;
@@ -208,7 +252,7 @@ IDFX_DEV void hlld_inner(const double WL[7], const double WR[7], double Bn, cons
     return;
   }
   const double sgn = (Bn >= 0.0) ? 1.0 : -1.0;
-  const double inv = 1.0 / (sqL + sqR);
+  const double inv = rcp(sqL + sqR);
   const double vss = (sqL * vsL + sqR * vsR + (BysR - BysL) * sgn) * inv;
   const double wss = (sqL * wsL + sqR * wsR + (BzsR - BzsL) * sgn) * inv;
   const double sqq = sqL * sqR;
@@ -240,17 +284,17 @@ IDFX_DEV void hlld_inner(const double WL[7], const double WR[7], double Bn, cons
 template <bool MHD>
 IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const double UL[7], const double UR[7],
                         const double FL[7], const double FR[7], double pTL, double pTR, double g, double F[7]) {
-  const double sL = sqrt(WL[0]), sR = sqrt(WR[0]);
-  const double isum = 1.0 / (sL + sR);
+  const double sL = sqrt_nn(WL[0]), sR = sqrt_nn(WR[0]);
+  const double isum = rcp(sL + sR);
   const double rb = sL * sR;
-  const double irb = 1.0 / rb;
+  const double irb = rcp(rb);
   const double ub = (sL * WL[1] + sR * WR[1]) * isum;
   const double vb = (sL * WL[2] + sR * WR[2]) * isum;
   const double wb = (sL * WL[3] + sR * WR[3]) * isum;
-  const double HL = (UL[4] + pTL) / WL[0], HR = (UR[4] + pTR) / WR[0];
+  const double HL = (UL[4] + pTL) * rcp(WL[0]), HR = (UR[4] + pTR) * rcp(WR[0]);
   const double Hb = (sL * HL + sR * HR) * isum;
   const double v2h = 0.5 * (ub * ub + vb * vb + wb * wb);
-  const double gm1 = g - 1.0;
+  const double gm1 = g - 1.0, igm1 = rcp(gm1);
   double Byb = 0.0, Bzb = 0.0, Xp = 0.0, bt2 = 0.0, bn2 = 0.0;
   const double dBy = UR[5] - UL[5], dBz = UR[6] - UL[6];
   if (MHD) {
@@ -273,8 +317,8 @@ IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const
 
   double s0, s1, s2, s3, s4, s5 = 0.0, s6 = 0.0;
   if (!MHD) {
-    const double a = sqrt(a2);
-    const double ia2 = 1.0 / a2;
+    const double a = sqrt_nn(a2);
+    const double ia2 = rcp(a2);
     // acoustic waves u -+ a: r = (rb, -+a, 0, 0, rb a2), l = (0, -+a, 0, 0, 1/rb)/(2 a2)
     const double am = (-a * du + dp * irb) * 0.5 * ia2;
     const double ap = (a * du + dp * irb) * 0.5 * ia2;
@@ -286,31 +330,32 @@ IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const
     s3 = l0 * dw;
     s4 = rb * a2 * (lm + lp);
   } else {
-    const double a = sqrt(a2);
+    const double a = sqrt_nn(a2);
+    const double ia2 = rcp(a2);
     const double sum = a2 + bn2 + bt2;
-    const double disc = sqrt(fmax(sum * sum - 4.0 * a2 * bn2, 0.0));
+    const double disc = sqrt_nn(fmax(sum * sum - 4.0 * a2 * bn2, 0.0));
     const double Cf2 = 0.5 * (sum + disc);
-    const double Cs2 = a2 * bn2 / Cf2;
-    const double Cf = sqrt(Cf2), Cs = sqrt(Cs2), CA = sqrt(bn2);
+    const double Cs2 = a2 * bn2 * rcp(Cf2);
+    const double Cf = sqrt_nn(Cf2), Cs = sqrt_nn(Cs2), CA = sqrt_nn(bn2);
     double af = 1.0, as = 0.0;
     const double den = Cf2 - Cs2;
     if (den > 0.0) {
-      const double iden = 1.0 / den;
-      af = sqrt(fmin(1.0, fmax(0.0, (a2 - Cs2) * iden)));
-      as = sqrt(fmin(1.0, fmax(0.0, (Cf2 - a2) * iden)));
+      const double iden = rcp(den);
+      af = sqrt_nn(fmin(1.0, fmax(0.0, (a2 - Cs2) * iden)));
+      as = sqrt_nn(fmin(1.0, fmax(0.0, (Cf2 - a2) * iden)));
     }
-    const double Bt = sqrt(Byb * Byb + Bzb * Bzb);
+    const double Bt2 = Byb * Byb + Bzb * Bzb;
     double by = 0.70710678118654752440, bz = 0.70710678118654752440;
-    if (Bt != 0.0) {
-      const double iBt = 1.0 / Bt;
+    if (Bt2 > 1e-300) {
+      const double iBt = rsqrt_pos(Bt2);
       by = Byb * iBt;
       bz = Bzb * iBt;
     }
     const double S = (Bn >= 0.0) ? 1.0 : -1.0;
-    const double sr = sqrt(rb), isr = 1.0 / sr;
+    const double isr = rsqrt_pos(rb), sr = rb * isr;
     const double Cff = Cf * af, Css = Cs * as, Qf = Cff * S, Qs = Css * S;
     const double Af = a * af * sr, As = a * as * sr;
-    const double i2a2 = 0.5 / a2;
+    const double i2a2 = 0.5 * ia2;
 
     const double dvt = by * dv + bz * dw;        // beta . dv_t
     const double dBt = (by * dBy + bz * dBz);    // beta . dB_t
@@ -325,7 +370,7 @@ IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const
     const double asp = (Css * du + Qf * dvt + ts) * i2a2;
     const double aAm = 0.5 * (dvx + S * dBx * isr);     // l_A- = (0,0,-bz,+by,0,-S bz/sr, S by/sr)/2
     const double aAp = 0.5 * (-dvx + S * dBx * isr);
-    const double a0 = dr - dp / a2;
+    const double a0 = dr - dp * ia2;
     // |lambda| alpha
     const double Lfm = fabs(ub - Cf) * afm, Lfp = fabs(ub + Cf) * afp;
     const double Lsm = fabs(ub - Cs) * asm_, Lsp = fabs(ub + Cs) * asp;
@@ -350,7 +395,7 @@ IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const
   const double j1 = ub * s0 + rb * s1;
   const double j2 = vb * s0 + rb * s2;
   const double j3 = wb * s0 + rb * s3;
-  const double j4 = (v2h + Xp / gm1) * s0 + rb * (ub * s1 + vb * s2 + wb * s3) + s4 / gm1 + Byb * s5 + Bzb * s6;
+  const double j4 = (v2h + Xp * igm1) * s0 + rb * (ub * s1 + vb * s2 + wb * s3) + s4 * igm1 + Byb * s5 + Bzb * s6;
   F[0] = 0.5 * (FL[0] + FR[0] - j0);
   F[1] = 0.5 * (FL[1] + FR[1] - j1);
   F[2] = 0.5 * (FL[2] + FR[2] - j2);
@@ -364,7 +409,7 @@ IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const
 // One Riemann problem.  Returns the flux in F and c_face = max(|S_L|,|S_R|).
 template <int SOLVER, bool MHD>
 IDFX_DEV double riemann(const double WL[7], const double WR[7], double Bn, double g, double F[7]) {
-  const double igm1 = 1.0 / (g - 1.0);
+  const double igm1 = rcp(g - 1.0);
   double UL[7], UR[7], FL[7], FR[7], pTL, pTR, SL, SR;
   side_cons_flux<MHD>(WL, Bn, igm1, UL, FL, pTL);
   side_cons_flux<MHD>(WR, Bn, igm1, UR, FR, pTR);
