@@ -23,6 +23,9 @@
 
 namespace idfx {
 
+// pulls a line into L1 ahead of its use; costs no register
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 struct FluxXArgs {
   const double* q[7];  // rho, vx, vy, vz, p, Bc_y, Bc_z
   const double* bn;    // B_x on x-faces
@@ -152,6 +155,13 @@ __global__ void __launch_bounds__(128, IDFX_MINB_M) k_flux_march(Geom g, FluxMAr
         if (MHD) Bnn = a.bn[c + sd];
       }
       const long long cu = c - sd;  // cell s-1, completed by this face
+      if (s + 1 < s1) {  // lines of the iteration after next, and of the next cell update, into L1
+#pragma unroll
+        for (int n = 0; n < NQ; ++n) prefetch_l1(a.q[n] + c + 3 * sd);
+        if (MHD) prefetch_l1(a.bn + c + 2 * sd);
+#pragma unroll
+        for (int n = 0; n < 5; ++n) prefetch_l1(DIR == 1 ? a.FX[n] + c + 1 : a.R[n] + c);
+      }
       double r_in[5], cs_in = 0.0;
       if (s > s0) {
         if (DIR == 1) {
