@@ -173,111 +173,6 @@ IDFX_DEV void hllc_inner(const double WL[7], const double WR[7], const double UL
   }
 }
 
-// O7 / G6: HLLD (MHD), for S_L < 0 < S_R.  The starred transverse components are needed from both sides
-// (they enter the double-star state); energies and the final flux only on the side that is selected.
-IDFX_DEV void hlld_inner(const double WL[7], const double WR[7], double Bn, const double UL[7], const double UR[7],
-                         const double FL[7], const double FR[7], double pTL, double pTR, double SL, double SR,
-                         double F[7]) {
-  const double uL = WL[1], uR = WR[1];
-  const double sL = SL - uL, sR = SR - uR;
-  const double qL = WL[0] * sL, qR = WR[0] * sR;  // rho_K (S_K - u_K)
-  const double iD = rcp(qR - qL);
-  const double SM = (qR * uR - qL * uL - pTR + pTL) * iD;
-  const double pTs = (qR * pTL - qL * pTR + qL * qR * (uR - uL)) * iD;
-  const double Bn2 = Bn * Bn;
-
-  const double iL = rcp(SL - SM), iR = rcp(SR - SM);
-  const double rsL = qL * iL, rsR = qR * iR;  // rho*_K
-  double vsL, wsL, BysL, BzsL, vsR, wsR, BysR, BzsR;
-  {
-    const double d = qL * (SL - SM) - Bn2;
-    const bool deg = fabs(d) < 1e-12 * qL * sL;
-    const double id = rcp(deg ? 1.0 : d);
-    const double f = deg ? 0.0 : Bn * (SM - uL) * id;
-    const double h = deg ? 1.0 : (qL * sL - Bn2) * id;
-    vsL = WL[2] - WL[5] * f;
-    wsL = WL[3] - WL[6] * f;
-    BysL = WL[5] * h;
-    BzsL = WL[6] * h;
-  }
-  {
-    const double d = qR * (SR - SM) - Bn2;
-    const bool deg = fabs(d) < 1e-12 * qR * sR;
-    const double id = rcp(deg ? 1.0 : d);
-    const double f = deg ? 0.0 : Bn * (SM - uR) * id;
-    const double h = deg ? 1.0 : (qR * sR - Bn2) * id;
-    vsR = WR[2] - WR[5] * f;
-    wsR = WR[3] - WR[6] * f;
-    BysR = WR[5] * h;
-    BzsR = WR[6] * h;
-  }
-  const double ysL = rsqrt_pos(rsL), ysR = rsqrt_pos(rsR);  // 1/sqrt(rho*_K)
-  const double sqL = rsL * ysL, sqR = rsR * ysR;
-  const double aBn = fabs(Bn);
-  const double SsL = SM - aBn * ysL, SsR = SM + aBn * ysR;
-
-  // side selection in the order of O7: S*_L >= 0 -> U*_L ; S*_R <= 0 -> U*_R ; S_M >= 0 -> U**_L ; else U**_R
-  const bool starL = SsL >= 0.0;
-  const bool starR = !starL && (SsR <= 0.0);
-  const bool left = starL || (!starR && SM >= 0.0);
-  const bool dstar = !starL && !starR;
-
-  const double SK = left ? SL : SR, sK = left ? sL : sR, iK = left ? iL : iR;
-  const double rsK = left ? rsL : rsR, sqK = left ? sqL : sqR;
-  const double uK = left ? uL : uR, vK = left ? WL[2] : WR[2], wK = left ? WL[3] : WR[3];
-  const double ByK = left ? WL[5] : WR[5], BzK = left ? WL[6] : WR[6];
-  const double EK = left ? UL[4] : UR[4], pTK = left ? pTL : pTR;
-  const double vsK = left ? vsL : vsR, wsK = left ? wsL : wsR;
-  const double BysK = left ? BysL : BysR, BzsK = left ? BzsL : BzsR;
-
-  const double vBK = uK * Bn + vK * ByK + wK * BzK;
-  const double vBsK = SM * Bn + vsK * BysK + wsK * BzsK;
-  const double EsK = (sK * EK - pTK * uK + pTs * SM + Bn * (vBK - vBsK)) * iK;
-
-  double Us[7];
-  Us[0] = rsK;
-  Us[1] = rsK * SM;
-  Us[2] = rsK * vsK;
-  Us[3] = rsK * wsK;
-  Us[4] = EsK;
-  Us[5] = BysK;
-  Us[6] = BzsK;
-  if (!dstar) {
-#pragma unroll
-    for (int n = 0; n < 7; ++n) {
-      const double Fk = left ? FL[n] : FR[n];
-      const double Uk = left ? UL[n] : UR[n];
-      F[n] = Fk + SK * (Us[n] - Uk);
-    }
-    return;
-  }
-  const double sgn = (Bn >= 0.0) ? 1.0 : -1.0;
-  const double inv = rcp(sqL + sqR);
-  const double vss = (sqL * vsL + sqR * vsR + (BysR - BysL) * sgn) * inv;
-  const double wss = (sqL * wsL + sqR * wsR + (BzsR - BzsL) * sgn) * inv;
-  const double sqq = sqL * sqR;
-  const double Byss = (sqL * BysR + sqR * BysL + sqq * (vsR - vsL) * sgn) * inv;
-  const double Bzss = (sqL * BzsR + sqR * BzsL + sqq * (wsR - wsL) * sgn) * inv;
-  const double vBss = SM * Bn + vss * Byss + wss * Bzss;
-  // E**_L = E*_L - sqrt(rho*_L)(vB*_L - vB**) sgn ;  E**_R = E*_R + sqrt(rho*_R)(vB*_R - vB**) sgn
-  const double EssK = left ? (EsK - sqK * (vBsK - vBss) * sgn) : (EsK + sqK * (vBsK - vBss) * sgn);
-  const double SsK = left ? SsL : SsR;
-  double Uss[7];
-  Uss[0] = rsK;
-  Uss[1] = rsK * SM;
-  Uss[2] = rsK * vss;
-  Uss[3] = rsK * wss;
-  Uss[4] = EssK;
-  Uss[5] = Byss;
-  Uss[6] = Bzss;
-#pragma unroll
-  for (int n = 0; n < 7; ++n) {
-    const double Fk = left ? FL[n] : FR[n];
-    const double Uk = left ? UL[n] : UR[n];
-    F[n] = Fk + SsK * Uss[n] - (SsK - SK) * Us[n] - SK * Uk;
-  }
-}
-
 // O8 / G7: Roe solver with the exact Roe averages of the shifted equation of state, no entropy fix.
 // Returns false when a~^2 <= 0 (caller falls back to HLL).  Projections are written out analytically:
 // dW = Minv dU, alpha_k = l_k . dW, primitive sum s = sum |lambda_k| alpha_k r_k, flux jump = M s.
@@ -406,9 +301,126 @@ IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const
   return true;
 }
 
+// O7 / G5 / G6: the whole HLLD problem written one-sided and branch-free.  Total pressures, outer speeds, S_M, p_T*
+// and the starred transverse components need both sides; conserved vector, physical flux, E*, E** and the flux
+// combination are evaluated only for the side K the selection of O7 picks (K = L when S_L >= 0, R when S_R <= 0).
+IDFX_DEV double hlld_onesided(const double WL[7], const double WR[7], double Bn, double g, double F[7]) {
+  const double Bn2 = Bn * Bn;
+  const double pbL = 0.5 * (Bn2 + WL[5] * WL[5] + WL[6] * WL[6]);
+  const double pbR = 0.5 * (Bn2 + WR[5] * WR[5] + WR[6] * WR[6]);
+  const double pTL = WL[4] + pbL, pTR = WR[4] + pbR;
+  const double uL = WL[1], uR = WR[1];
+  double cL, cR;
+  {
+    const double ir = rcp(WL[0]);
+    const double a2 = g * WL[4] * ir, bn2 = Bn2 * ir, sm = a2 + 2.0 * pbL * ir;
+    cL = sqrt_nn(0.5 * (sm + sqrt_nn(fmax(sm * sm - 4.0 * a2 * bn2, 0.0))));
+  }
+  {
+    const double ir = rcp(WR[0]);
+    const double a2 = g * WR[4] * ir, bn2 = Bn2 * ir, sm = a2 + 2.0 * pbR * ir;
+    cR = sqrt_nn(0.5 * (sm + sqrt_nn(fmax(sm * sm - 4.0 * a2 * bn2, 0.0))));
+  }
+  const double SL = fmin(uL - cL, uR - cR), SR = fmax(uL + cL, uR + cR);
+  const double cface = fmax(fabs(SL), fabs(SR));
+
+  const double sL = SL - uL, sR = SR - uR;
+  const double qL = WL[0] * sL, qR = WR[0] * sR;  // rho_K (S_K - u_K)
+  const double iD = rcp(qR - qL);
+  const double SM = (qR * uR - qL * uL - pTR + pTL) * iD;
+  const double pTs = (qR * pTL - qL * pTR + qL * qR * (uR - uL)) * iD;
+  const double iL = rcp(SL - SM), iR = rcp(SR - SM);
+  const double rsL = qL * iL, rsR = qR * iR;  // rho*_K
+  double vsL, wsL, BysL, BzsL, vsR, wsR, BysR, BzsR;
+  {
+    const double d = qL * (SL - SM) - Bn2;
+    const bool deg = fabs(d) < 1e-12 * qL * sL;
+    const double id = rcp(deg ? 1.0 : d);
+    const double f = deg ? 0.0 : Bn * (SM - uL) * id;
+    const double h = deg ? 1.0 : (qL * sL - Bn2) * id;
+    vsL = WL[2] - WL[5] * f;
+    wsL = WL[3] - WL[6] * f;
+    BysL = WL[5] * h;
+    BzsL = WL[6] * h;
+  }
+  {
+    const double d = qR * (SR - SM) - Bn2;
+    const bool deg = fabs(d) < 1e-12 * qR * sR;
+    const double id = rcp(deg ? 1.0 : d);
+    const double f = deg ? 0.0 : Bn * (SM - uR) * id;
+    const double h = deg ? 1.0 : (qR * sR - Bn2) * id;
+    vsR = WR[2] - WR[5] * f;
+    wsR = WR[3] - WR[6] * f;
+    BysR = WR[5] * h;
+    BzsR = WR[6] * h;
+  }
+  const double ysL = rsqrt_pos(fabs(rsL)), ysR = rsqrt_pos(fabs(rsR));  // 1/sqrt(rho*_K); |.| only guards unused lanes
+  const double sqL = fabs(rsL) * ysL, sqR = fabs(rsR) * ysR;
+  const double aBn = fabs(Bn);
+  const double SsL = SM - aBn * ysL, SsR = SM + aBn * ysR;
+
+  // selection in the order of O7
+  const bool pureL = SL >= 0.0, pureR = !pureL && SR <= 0.0;
+  const bool starL = SsL >= 0.0, starR = !starL && SsR <= 0.0;
+  const bool pure = pureL || pureR;
+  const bool left = pureL || (!pureR && (starL || (!starR && SM >= 0.0)));
+  const bool dstar = !pure && !starL && !starR;
+
+  // side K: conserved vector and physical flux
+  const double rK = left ? WL[0] : WR[0], uK = left ? uL : uR, vK = left ? WL[2] : WR[2];
+  const double wK = left ? WL[3] : WR[3], pK = left ? WL[4] : WR[4];
+  const double ByK = left ? WL[5] : WR[5], BzK = left ? WL[6] : WR[6];
+  const double pbK = left ? pbL : pbR, pTK = left ? pTL : pTR;
+  const double muK = rK * uK;
+  const double EK = pK * rcp(g - 1.0) + 0.5 * rK * (uK * uK + vK * vK + wK * wK) + pbK;
+  const double vBK = uK * Bn + vK * ByK + wK * BzK;
+  double UK[7], FK[7];
+  UK[0] = rK; UK[1] = muK; UK[2] = rK * vK; UK[3] = rK * wK; UK[4] = EK; UK[5] = ByK; UK[6] = BzK;
+  FK[0] = muK;
+  FK[1] = muK * uK + pTK - Bn2;
+  FK[2] = muK * vK - Bn * ByK;
+  FK[3] = muK * wK - Bn * BzK;
+  FK[4] = (EK + pTK) * uK - Bn * vBK;
+  FK[5] = uK * ByK - vK * Bn;
+  FK[6] = uK * BzK - wK * Bn;
+
+  // star and double-star states of side K
+  const double SK = left ? SL : SR, sK = left ? sL : sR, iK = left ? iL : iR;
+  const double rsK = left ? rsL : rsR, sqK = left ? sqL : sqR, SsK = left ? SsL : SsR;
+  const double vsK = left ? vsL : vsR, wsK = left ? wsL : wsR;
+  const double BysK = left ? BysL : BysR, BzsK = left ? BzsL : BzsR;
+  const double vBsK = SM * Bn + vsK * BysK + wsK * BzsK;
+  const double EsK = (sK * EK - pTK * uK + pTs * SM + Bn * (vBK - vBsK)) * iK;
+  const double sgn = (Bn >= 0.0) ? 1.0 : -1.0;
+  const double inv = rcp(sqL + sqR);
+  const double sqq = sqL * sqR;
+  const double vss = (sqL * vsL + sqR * vsR + (BysR - BysL) * sgn) * inv;
+  const double wss = (sqL * wsL + sqR * wsR + (BzsR - BzsL) * sgn) * inv;
+  const double Byss = (sqL * BysR + sqR * BysL + sqq * (vsR - vsL) * sgn) * inv;
+  const double Bzss = (sqL * BzsR + sqR * BzsL + sqq * (wsR - wsL) * sgn) * inv;
+  const double vBss = SM * Bn + vss * Byss + wss * Bzss;
+  // E**_L = E*_L - sqrt(rho*_L)(vB*_L - vB**) sgn ;  E**_R = E*_R + sqrt(rho*_R)(vB*_R - vB**) sgn
+  const double sside = left ? -sgn : sgn;
+  const double EssK = EsK + sside * sqK * (vBsK - vBss);
+  double Us[7], Uss[7];
+  Us[0] = rsK; Us[1] = rsK * SM; Us[2] = rsK * vsK; Us[3] = rsK * wsK; Us[4] = EsK; Us[5] = BysK; Us[6] = BzsK;
+  Uss[0] = rsK; Uss[1] = Us[1]; Uss[2] = rsK * vss; Uss[3] = rsK * wss; Uss[4] = EssK; Uss[5] = Byss; Uss[6] = Bzss;
+  // star:        F = F_K + S_K (U* - U_K)
+  // double star: F = F_K + S*_K U** - (S*_K - S_K) U* - S_K U_K
+  const double c1 = dstar ? SK - SsK : SK;
+  const double c2 = dstar ? SsK : 0.0;
+#pragma unroll
+  for (int n = 0; n < 7; ++n) {
+    const double f = FK[n] + c1 * Us[n] + c2 * Uss[n] - SK * UK[n];
+    F[n] = pure ? FK[n] : f;
+  }
+  return cface;
+}
+
 // One Riemann problem.  Returns the flux in F and c_face = max(|S_L|,|S_R|).
 template <int SOLVER, bool MHD>
 IDFX_DEV double riemann(const double WL[7], const double WR[7], double Bn, double g, double F[7]) {
+  if (SOLVER == SOLVER_HLLD) return hlld_onesided(WL, WR, Bn, g, F);
   const double igm1 = rcp(g - 1.0);
   double UL[7], UR[7], FL[7], FR[7], pTL, pTR, SL, SR;
   side_cons_flux<MHD>(WL, Bn, igm1, UL, FL, pTL);
@@ -441,7 +453,6 @@ IDFX_DEV double riemann(const double WL[7], const double WR[7], double Bn, doubl
     if (!MHD) F[5] = F[6] = 0.0;
     if (SOLVER == SOLVER_HLL) hll_inner<NV>(UL, UR, FL, FR, SL, SR, F);
     if (SOLVER == SOLVER_HLLC) hllc_inner(WL, WR, UL, UR, FL, FR, SL, SR, F);
-    if (SOLVER == SOLVER_HLLD) hlld_inner(WL, WR, Bn, UL, UR, FL, FR, pTL, pTR, SL, SR, F);
   }
   return cface;
 }
