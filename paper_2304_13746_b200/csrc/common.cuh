@@ -36,6 +36,8 @@ struct DevScalars {
   int flag;
 };
 
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // block-wide maximum for blocks of exactly 128 threads; every thread must call it
 __device__ __forceinline__ double block_max_128(double v) {
   __shared__ double red[4];

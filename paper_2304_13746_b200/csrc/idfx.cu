@@ -22,7 +22,7 @@ namespace idfx {
 // copy-in / copy-out between the caller's contiguous arrays and the padded fields
 // ---------------------------------------------------------------------------------------------
 struct FieldList {
-  double* f[11];
+  double* f[14];
   int n;
 };
 
@@ -82,7 +82,7 @@ __global__ void k_fill_ghost(Geom g, FieldList fl) {
 // ---------------------------------------------------------------------------------------------
 struct StateArgs {
   double* U[5];
-  double* V[8];
+  double* V[11];  // rho, v, p, Bc, Ec = -(v x Bc)
   const double* Bf[3];
   DevScalars* sc;
 };
@@ -104,6 +104,11 @@ __global__ void k_cons_from_prim(Geom g, StateArgs a) {
     a.V[7][c] = bz;
   }
   const double rho = a.V[0][c], vx = a.V[1][c], vy = a.V[2][c], vz = a.V[3][c], p = a.V[4][c];
+  if (MHD) {
+    a.V[8][c] = vz * by - vy * bz;
+    a.V[9][c] = vx * bz - vz * bx;
+    a.V[10][c] = vy * bx - vx * by;
+  }
   if (!(rho > 0.0) || !(p > 0.0)) a.sc->flag = 1;
   a.U[0][c] = rho;
   a.U[1][c] = rho * vx;
@@ -241,20 +246,16 @@ __global__ void __launch_bounds__(128) k_rhs(Geom g, RhsArgs a) {
 struct EmfArgs {
   const double* FB[3][2];  // FB[d][0] = F_d[B_t1], FB[d][1] = F_d[B_t2] on the left d-faces
   const double* FM[3];     // mass flux F_d[rho]
-  const double* v[3];
-  const double* Bc[3];
+  const double* Ec[3];     // cell-centred reference EMF -(v x Bc) of the stage input, with ghosts (G10)
   double* E[3];
 };
 
+// E_c on the lower (a-1/2, b-1/2) edge of active cell idx, (a,b,c) cyclic (O10)
 template <bool UCT>
-__global__ void __launch_bounds__(128) k_emf(Geom g, EmfArgs a) {
-  int idx[3];
-  if (!cell_of_thread(g, idx[0], idx[1], idx[2])) return;
+__device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& a, const int idx[3], int c) {
   const int n[3] = {g.nx, g.ny, g.nz};
   const long long st[3] = {1, g.sy, g.sz};
   const long long P = g.at(idx[0], idx[1], idx[2]);
-#pragma unroll
-  for (int c = 0; c < 3; ++c) {
     const int ia = (c + 1) % 3, ib = (c + 2) % 3;
     // periodic images of the neighbours one step down in a and in b (flux arrays have no ghosts)
     const long long da = idx[ia] == 0 ? (long long)(n[ia] - 1) * st[ia] : -st[ia];
@@ -265,17 +266,9 @@ __global__ void __launch_bounds__(128) k_emf(Geom g, EmfArgs a) {
     const double EbP = Fb[P], EbPa = Fb[P + da];    // b-faces at (ia, ib-1/2) and (ia-1, ib-1/2)
     double e = 0.25 * (EaP + EaPb + EbP + EbPa);
     if (UCT) {
-      // cell-centred reference EMF -(v x B)_c = v_b B_a - v_a B_b from the stage-input primitives (G10);
-      // V has ghosts, so plain offsets
-      const double* __restrict__ va = a.v[ia];
-      const double* __restrict__ vb = a.v[ib];
-      const double* __restrict__ Ba = a.Bc[ia];
-      const double* __restrict__ Bb = a.Bc[ib];
-      const long long Qa = P - st[ia], Qb = P - st[ib], Qab = P - st[ia] - st[ib];
-      const double Ec = vb[P] * Ba[P] - va[P] * Bb[P];
-      const double Eca = vb[Qa] * Ba[Qa] - va[Qa] * Bb[Qa];
-      const double Ecb = vb[Qb] * Ba[Qb] - va[Qb] * Bb[Qb];
-      const double Ecab = vb[Qab] * Ba[Qab] - va[Qab] * Bb[Qab];
+      // cell-centred reference EMF of the stage input (G10), stored with ghosts next to the primitives
+      const double* __restrict__ Ecc = a.Ec[c];
+      const double Ec = Ecc[P], Eca = Ecc[P - st[ia]], Ecb = Ecc[P - st[ib]], Ecab = Ecc[P - st[ia] - st[ib]];
       const double fa = a.FM[ia][P], fab = a.FM[ia][P + db];  // mass flux through the two a-faces
       const double fb = a.FM[ib][P], fba = a.FM[ib][P + da];  // and the two b-faces
       // d/db on the a-face, quarter points ib-1/4 (cells P-a | P) and ib-3/4 (cells P-a-b | P-b)
@@ -290,8 +283,16 @@ __global__ void __launch_bounds__(128) k_emf(Geom g, EmfArgs a) {
       const double Ga3 = fba > 0.0 ? gam_m : (fba < 0.0 ? gam_p : 0.5 * (gam_m + gam_p));
       e += 0.125 * (Gb3 - Gb1) + 0.125 * (Ga3 - Ga1);
     }
-    a.E[c][P] = e;
-  }
+    return e;
+}
+
+template <bool UCT>
+__global__ void __launch_bounds__(128) k_emf(Geom g, EmfArgs a) {
+  int idx[3];
+  if (!cell_of_thread(g, idx[0], idx[1], idx[2])) return;
+  const long long P = g.at(idx[0], idx[1], idx[2]);
+#pragma unroll
+  for (int c = 0; c < 3; ++c) a.E[c][P] = edge_emf<UCT>(g, a, idx, c);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -309,7 +310,7 @@ struct UpdateArgs {
   const double* B0[3];    // ghosts filled (stage 2 only)
   const double* E[3];     // active lower edges only
   double* Bout[3];
-  double* V[8];
+  double* V[11];
   DevScalars* sc;
   double dt_fixed;        // > 0: use it; otherwise dt = cfl / smax
   double cfl;
@@ -372,6 +373,108 @@ __global__ void __launch_bounds__(128) k_update(Geom g, UpdateArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// a6 + a5 (apply) + a7 + a8 + a2 + a1 fused for MHD: one CTA owns a TX x TY x TZ tile of cells.
+// Phase 1 evaluates every edge EMF of the tile's edge lattice once (upper lattice planes are recomputed by the
+// neighbouring tile: 29 % more edge evaluations, no DRAM cost) into shared memory; phase 2 is k_update with the
+// edges read from shared memory, so the edge EMFs never travel to HBM; the result's ghost images (V and the new
+// face field) are written by the owners of the boundary cells, which replaces the separate ghost-fill pass.
+// ---------------------------------------------------------------------------------------------
+constexpr int CT_TX = 32, CT_TY = 8, CT_TZ = 4;
+constexpr int CT_LX = CT_TX + 1, CT_LY = CT_TY + 1, CT_LZ = CT_TZ + 1;
+
+template <bool UCT, bool STAGE2>
+__global__ void __launch_bounds__(256) k_ct_update(Geom g, EmfArgs ea, UpdateArgs a) {
+  __shared__ double sE[3][CT_LZ][CT_LY][CT_LX];
+  const int i0 = blockIdx.x * CT_TX, j0 = blockIdx.y * CT_TY, k0 = blockIdx.z * CT_TZ;
+  // ---- phase 1: edge lattice ----
+  for (int p = threadIdx.x; p < CT_LZ * CT_LY * CT_LX; p += 256) {
+    const int li = p % CT_LX, lj = (p / CT_LX) % CT_LY, lk = p / (CT_LX * CT_LY);
+    const int I = i0 + li, J = j0 + lj, K = k0 + lk;
+    if (I > g.nx || J > g.ny || K > g.nz) continue;
+    // periodic image of lattice index n is index 0
+    const int idx[3] = {I == g.nx ? 0 : I, J == g.ny ? 0 : J, K == g.nz ? 0 : K};
+    if (li < CT_TX) sE[0][lk][lj][li] = edge_emf<UCT>(g, ea, idx, 0);
+    if (lj < CT_TY) sE[1][lk][lj][li] = edge_emf<UCT>(g, ea, idx, 1);
+    if (lk < CT_TZ) sE[2][lk][lj][li] = edge_emf<UCT>(g, ea, idx, 2);
+  }
+  __syncthreads();
+  // ---- phase 2: one (i, j) column of TZ cells per thread ----
+  const int li = threadIdx.x % CT_TX, lj = threadIdx.x / CT_TX;
+  const int i = i0 + li, j = j0 + lj;
+  if (i >= g.nx || j >= g.ny) return;
+  double dt = a.dt_fixed;
+  if (!(dt > 0.0)) dt = a.cfl / __longlong_as_double((long long)a.sc->smax_bits);
+  if (!STAGE2 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) a.sc->dt_used = dt;
+  const double dtdx = dt / g.dx;
+  const long long st[3] = {1, g.sy, g.sz};
+  // ghost images of this column in x and y
+  const long long gx = i < NG ? (long long)g.nx : (i >= g.nx - NG ? -(long long)g.nx : 0);
+  const long long gy = j < NG ? (long long)g.ny * g.sy : (j >= g.ny - NG ? -(long long)g.ny * g.sy : 0);
+#pragma unroll
+  for (int lk = 0; lk < CT_TZ; ++lk) {
+    const int k = k0 + lk;
+    if (k >= g.nz) break;
+    const long long c = g.at(i, j, k);
+    double u[5];
+#pragma unroll
+    for (int n = 0; n < 5; ++n) {
+      const double us = a.Uin[n][c] - dtdx * a.R[n][c];
+      u[n] = STAGE2 ? 0.5 * a.U0[n][c] + 0.5 * us : us;
+      a.Uout[n][c] = u[n];
+    }
+    const double ex00 = sE[0][lk][lj][li], ex10 = sE[0][lk][lj + 1][li];
+    const double ex01 = sE[0][lk + 1][lj][li], ex11 = sE[0][lk + 1][lj + 1][li];
+    const double ey00 = sE[1][lk][lj][li], ey10 = sE[1][lk][lj][li + 1];
+    const double ey01 = sE[1][lk + 1][lj][li], ey11 = sE[1][lk + 1][lj][li + 1];
+    const double ez00 = sE[2][lk][lj][li], ez10 = sE[2][lk][lj][li + 1];
+    const double ez01 = sE[2][lk][lj + 1][li], ez11 = sE[2][lk][lj + 1][li + 1];
+    // O11, left faces then right faces
+    const double curlL[3] = {(ez01 - ez00) - (ey01 - ey00), (ex01 - ex00) - (ez10 - ez00), (ey10 - ey00) - (ex10 - ex00)};
+    const double curlR[3] = {(ez11 - ez10) - (ey11 - ey10), (ex11 - ex10) - (ez11 - ez01), (ey11 - ey01) - (ex11 - ex01)};
+    double v[11];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      double bl = a.Bin[d][c] - dtdx * curlL[d];
+      double br = a.Bin[d][c + st[d]] - dtdx * curlR[d];
+      if (STAGE2) {
+        bl = 0.5 * a.B0[d][c] + 0.5 * bl;
+        br = 0.5 * a.B0[d][c + st[d]] + 0.5 * br;
+      }
+      v[5 + d] = 0.5 * (bl + br);
+      a.Bout[d][c] = bl;
+      // images of the new face value
+      const long long gz = k < NG ? (long long)g.nz * g.sz : (k >= g.nz - NG ? -(long long)g.nz * g.sz : 0);
+#pragma unroll
+      for (int m = 1; m < 8; ++m) {
+        const long long off = ((m & 1) ? gx : 0) + ((m & 2) ? gy : 0) + ((m & 4) ? gz : 0);
+        const bool ok = (!(m & 1) || gx != 0) && (!(m & 2) || gy != 0) && (!(m & 4) || gz != 0);
+        if (ok) a.Bout[d][c + off] = bl;
+      }
+    }
+    prim_from_cons(g.gamma - 1.0, u[0], u[1], u[2], u[3], u[4], v[5], v[6], v[7], v[1], v[2], v[3], v[4]);
+    v[0] = u[0];
+    v[8] = v[3] * v[6] - v[2] * v[7];
+    v[9] = v[1] * v[7] - v[3] * v[5];
+    v[10] = v[2] * v[5] - v[1] * v[6];
+    if (!(u[0] > 0.0) || !(v[4] > 0.0)) a.sc->flag = 1;
+    const long long gz = k < NG ? (long long)g.nz * g.sz : (k >= g.nz - NG ? -(long long)g.nz * g.sz : 0);
+#pragma unroll
+    for (int n = 0; n < 11; ++n) a.V[n][c] = v[n];
+    if (gx != 0 || gy != 0 || gz != 0) {
+#pragma unroll
+      for (int m = 1; m < 8; ++m) {
+        const long long off = ((m & 1) ? gx : 0) + ((m & 2) ? gy : 0) + ((m & 4) ? gz : 0);
+        const bool ok = (!(m & 1) || gx != 0) && (!(m & 2) || gy != 0) && (!(m & 4) || gz != 0);
+        if (ok) {
+#pragma unroll
+          for (int n = 0; n < 11; ++n) a.V[n][c + off] = v[n];
+        }
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
 thread_local char g_err[512] = "";
@@ -385,15 +488,15 @@ enum {
   F_BA = 10,   // 3 x 3: face-field buffers that rotate between B0 / B1 / result
   F_BB = 13,
   F_BC = 16,
-  F_V = 19,    // 8: primitives + cell-centred B of the stage input
-  F_R = 27,    // 5: flux divergence
-  F_FB = 32,   // 6: face fluxes of B, [d][0..1]
-  F_E = 38,    // 3: edge EMFs
-  F_FX = 41,   // 5: x-face fluxes of (rho, m, E); F_FX+0 doubles as the x mass flux
-  F_CFX = 46,  // 1: c_face of the x sweep
-  F_FM = 47,   // 3: face mass fluxes of the y, z sweeps at +1, +2 (slot +0 unused)
-  F_CS = 50,   // 1: sum_d c_d per cell (x and y parts)
-  F_COUNT = 51
+  F_V = 19,    // 11: primitives, cell-centred B and Ec = -(v x Bc) of the stage input
+  F_V2 = 30,   // 11: second buffer (MHD: the fused CT/update kernel reads the stage input while writing the result)
+  F_R = 41,    // 5: flux divergence
+  F_FB = 46,   // 6: face fluxes of B, [d][0..1]
+  F_FX = 52,   // 5: x-face fluxes of (rho, m, E); F_FX+0 doubles as the x mass flux
+  F_CFX = 57,  // 1: c_face of the x sweep
+  F_FM = 58,   // 3: face mass fluxes of the y, z sweeps at +1, +2 (slot +0 unused)
+  F_CS = 61,   // 1: sum_d c_d per cell (x and y parts)
+  F_COUNT = 62
 };
 
 }  // namespace idfx
@@ -415,6 +518,7 @@ struct idfx_ctx {
   bool bound = false;
   DevScalars* sc = nullptr;
   int bcur = 0;  // which of the three face-field buffers holds the current state
+  int vcur = 0;  // which primitive buffer holds the stage input
   long long launches = 0;
   // optional per-kernel timing with CUDA events on the bound stream (idfx_profile_*)
   bool prof_on = false;
@@ -425,6 +529,8 @@ struct idfx_ctx {
   long long prof_n[K_COUNT] = {0};
   double* field(int slot) const { return ws + (size_t)slot * (size_t)g.np; }
   double* bbuf(int which, int d) const { return field(F_BA + 3 * which + d); }
+  double* vfield(int n) const { return field((vcur ? F_V2 : F_V) + n); }
+  double* vfield_out(int n) const { return field((vcur ? F_V : F_V2) + n); }
 };
 
 namespace {
@@ -508,13 +614,13 @@ void launch_speed(idfx_ctx* c, int d, const double* const Bf[3]) {
   const int ia = d, ib = (d + 1) % 3, ie = (d + 2) % 3;
   const long long st[3] = {1, c->g.sy, c->g.sz};
   FluxArgs a;
-  a.q[0] = c->field(F_V);
-  a.q[1] = c->field(F_V + 1 + ia);
-  a.q[2] = c->field(F_V + 1 + ib);
-  a.q[3] = c->field(F_V + 1 + ie);
-  a.q[4] = c->field(F_V + 4);
-  a.q[5] = c->field(F_V + 5 + ib);
-  a.q[6] = c->field(F_V + 5 + ie);
+  a.q[0] = c->vfield(0);
+  a.q[1] = c->vfield(1 + ia);
+  a.q[2] = c->vfield(1 + ib);
+  a.q[3] = c->vfield(1 + ie);
+  a.q[4] = c->vfield(4);
+  a.q[5] = c->vfield(5 + ib);
+  a.q[6] = c->vfield(5 + ie);
   a.bn = c->mhd ? Bf[ia] : nullptr;
   a.sd = st[d];
   for (int n = 0; n < 7; ++n) a.F[n] = nullptr;
@@ -550,13 +656,13 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
   const bool uct = c->emf == EMF_UCT;
   {  // x: faces 0..nx of every row
     FluxXArgs a;
-    a.q[0] = c->field(F_V);
-    a.q[1] = c->field(F_V + 1);
-    a.q[2] = c->field(F_V + 2);
-    a.q[3] = c->field(F_V + 3);
-    a.q[4] = c->field(F_V + 4);
-    a.q[5] = c->field(F_V + 6);
-    a.q[6] = c->field(F_V + 7);
+    a.q[0] = c->vfield(0);
+    a.q[1] = c->vfield(1);
+    a.q[2] = c->vfield(2);
+    a.q[3] = c->vfield(3);
+    a.q[4] = c->vfield(4);
+    a.q[5] = c->vfield(6);
+    a.q[6] = c->vfield(7);
     a.bn = MHD ? Bf[0] : nullptr;
     for (int n = 0; n < 5; ++n) a.FH[n] = c->field(F_FX + n);
     a.FB[0] = c->field(F_FB + 0);
@@ -574,13 +680,13 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
   for (int d = 1; d < 3; ++d) {  // y then z: marching pencils
     const int ib = (d + 1) % 3, ie = (d + 2) % 3;
     FluxMArgs a;
-    a.q[0] = c->field(F_V);
-    a.q[1] = c->field(F_V + 1 + d);
-    a.q[2] = c->field(F_V + 1 + ib);
-    a.q[3] = c->field(F_V + 1 + ie);
-    a.q[4] = c->field(F_V + 4);
-    a.q[5] = c->field(F_V + 5 + ib);
-    a.q[6] = c->field(F_V + 5 + ie);
+    a.q[0] = c->vfield(0);
+    a.q[1] = c->vfield(1 + d);
+    a.q[2] = c->vfield(1 + ib);
+    a.q[3] = c->vfield(1 + ie);
+    a.q[4] = c->vfield(4);
+    a.q[5] = c->vfield(5 + ib);
+    a.q[6] = c->vfield(5 + ie);
     a.bn = MHD ? Bf[d] : nullptr;
     a.sd = d == 1 ? g.sy : g.sz;
     a.st = d == 1 ? g.sz : g.sy;
@@ -636,26 +742,22 @@ void launch_sweeps(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
   }
 }
 
-void launch_emf(idfx_ctx* c) {
+EmfArgs emf_args(idfx_ctx* c) {
   EmfArgs a;
   for (int d = 0; d < 3; ++d) {
     a.FB[d][0] = c->field(F_FB + 2 * d);
     a.FB[d][1] = c->field(F_FB + 2 * d + 1);
     a.FM[d] = d == 0 ? c->field(F_FX) : c->field(F_FM + d);
-    a.v[d] = c->field(F_V + 1 + d);
-    a.Bc[d] = c->field(F_V + 5 + d);
-    a.E[d] = c->field(F_E + d);
+    a.Ec[d] = c->vfield(8 + d);
+    a.E[d] = nullptr;
   }
-  const unsigned nb = blocks_for(c->g.nc, 128);
-  LaunchScope ls(c, K_EMF);
-  if (c->emf == EMF_UCT) k_emf<true><<<nb, 128, 0, c->stream>>>(c->g, a);
-  else k_emf<false><<<nb, 128, 0, c->stream>>>(c->g, a);
+  return a;
 }
 
 void launch_fill(idfx_ctx* c, int which_b) {
   FieldList fl;
   fl.n = 0;
-  for (int n = 0; n < (c->mhd ? 8 : 5); ++n) fl.f[fl.n++] = c->field(F_V + n);
+  for (int n = 0; n < (c->mhd ? 11 : 5); ++n) fl.f[fl.n++] = c->vfield(n);
   if (c->mhd)
     for (int d = 0; d < 3; ++d) fl.f[fl.n++] = c->bbuf(which_b, d);
   const Geom& g = c->g;
@@ -670,7 +772,6 @@ void launch_fill(idfx_ctx* c, int which_b) {
 void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fixed, double cfl, bool want_dt) {
   const double* Bf[3] = {c->bbuf(bin, 0), c->bbuf(bin, 1), c->bbuf(bin, 2)};
   launch_sweeps(c, Bf, want_dt);
-  if (c->mhd) launch_emf(c);
   UpdateArgs a;
   for (int n = 0; n < 5; ++n) {
     a.Uin[n] = c->field((stage2 ? F_UB : F_UA) + n);
@@ -681,25 +782,35 @@ void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fi
   for (int d = 0; d < 3; ++d) {
     a.Bin[d] = c->bbuf(bin, d);
     a.B0[d] = c->bbuf(b0, d);
-    a.E[d] = c->field(F_E + d);
+    a.E[d] = nullptr;
     a.Bout[d] = c->bbuf(bout, d);
   }
-  for (int n = 0; n < 8; ++n) a.V[n] = c->field(F_V + n);
   a.sc = c->sc;
   a.dt_fixed = dt_fixed;
   a.cfl = cfl;
-  const unsigned nb = blocks_for(c->g.nc, 128);
-  {
-    LaunchScope ls(c, K_UPDATE);
+  const Geom& g = c->g;
   if (c->mhd) {
-    if (stage2) k_update<true, true><<<nb, 128, 0, c->stream>>>(c->g, a);
-    else k_update<true, false><<<nb, 128, 0, c->stream>>>(c->g, a);
+    // edge EMFs + CT + RK combine + cons->prim + ghost images in one kernel; V is double-buffered because the
+    // EMFs of neighbouring tiles still read the stage-input primitives while this tile writes the result's
+    const EmfArgs ea = emf_args(c);
+    for (int n = 0; n < 11; ++n) a.V[n] = c->vfield_out(n);
+    dim3 grid((g.nx + CT_TX - 1) / CT_TX, (g.ny + CT_TY - 1) / CT_TY, (g.nz + CT_TZ - 1) / CT_TZ);
+    const bool uct = c->emf == EMF_UCT;
+    LaunchScope ls(c, K_UPDATE);
+    if (uct && stage2) k_ct_update<true, true><<<grid, 256, 0, c->stream>>>(g, ea, a);
+    else if (uct) k_ct_update<true, false><<<grid, 256, 0, c->stream>>>(g, ea, a);
+    else if (stage2) k_ct_update<false, true><<<grid, 256, 0, c->stream>>>(g, ea, a);
+    else k_ct_update<false, false><<<grid, 256, 0, c->stream>>>(g, ea, a);
+    c->vcur ^= 1;
   } else {
-    if (stage2) k_update<false, true><<<nb, 128, 0, c->stream>>>(c->g, a);
-    else k_update<false, false><<<nb, 128, 0, c->stream>>>(c->g, a);
+    for (int n = 0; n < 11; ++n) a.V[n] = c->vfield(n);
+    {
+      LaunchScope ls(c, K_UPDATE);
+      if (stage2) k_update<false, true><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
+      else k_update<false, false><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
+    }
+    launch_fill(c, bout);
   }
-  }
-  launch_fill(c, bout);
 }
 
 // One RK2 cycle.  dt_fixed > 0: that dt; otherwise dt = cfl / max found by stage 1 (never leaves the device).
@@ -736,7 +847,7 @@ int copy3d(idfx_ctx* c, double* field, const double* contig_in, double* contig_o
 int finish_set_state(idfx_ctx* c) {
   StateArgs a;
   for (int n = 0; n < 5; ++n) a.U[n] = c->field(F_UA + n);
-  for (int n = 0; n < 8; ++n) a.V[n] = c->field(F_V + n);
+  for (int n = 0; n < 11; ++n) a.V[n] = c->vfield(n);
   for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
   a.sc = c->sc;
   const unsigned nb = blocks_for(c->g.nc, 128);
@@ -752,7 +863,7 @@ int finish_set_state(idfx_ctx* c) {
 int refresh_prims(idfx_ctx* c) {
   StateArgs a;
   for (int n = 0; n < 5; ++n) a.U[n] = c->field(F_UA + n);
-  for (int n = 0; n < 8; ++n) a.V[n] = nullptr;
+  for (int n = 0; n < 11; ++n) a.V[n] = nullptr;
   for (int n = 0; n < 5; ++n) a.V[n] = c->field(F_R + n);  // scratch: R is dead between cycles
   for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
   a.sc = c->sc;
@@ -830,6 +941,7 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
   c->stream = (cudaStream_t)cuda_stream;
   c->sc = (DevScalars*)(c->ws + (size_t)F_COUNT * (size_t)c->g.np);
   c->bcur = 0;
+  c->vcur = 0;
   c->launches = 0;
   CK(cudaMemsetAsync(d_workspace, 0, idfx_workspace_bytes(c), c->stream));
   c->bound = true;
@@ -846,7 +958,7 @@ int idfx_set_state(idfx_ctx* c, const double* d_prim, const double* d_bface) {
   const unsigned nb = blocks_for(c->g.nc, 128);
   FieldList fl;
   fl.n = 5;
-  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(F_V + n);
+  for (int n = 0; n < 5; ++n) fl.f[n] = c->vfield(n);
   { LaunchScope ls(c, K_STATE);
   k_pack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_prim);
   }
@@ -868,7 +980,7 @@ int idfx_set_state_host(idfx_ctx* c, const double* h_prim, const double* h_bface
     return IDFX_ERR_INVALID_ARG;
   }
   for (int n = 0; n < 5; ++n)
-    if ((rc = copy3d(c, c->field(F_V + n), h_prim + (size_t)n * c->g.nc, nullptr, cudaMemcpyHostToDevice))) return rc;
+    if ((rc = copy3d(c, c->vfield(n), h_prim + (size_t)n * c->g.nc, nullptr, cudaMemcpyHostToDevice))) return rc;
   if (c->mhd)
     for (int d = 0; d < 3; ++d)
       if ((rc = copy3d(c, c->bbuf(c->bcur, d), h_bface + (size_t)d * c->g.nc, nullptr, cudaMemcpyHostToDevice)))
