@@ -124,6 +124,13 @@ def run_config(idfx, R, name, n=None, steps=None):
     assert sim.status() == 0 and ref.status() == 0
     assert abs(sim.last_dt() - ref.last_dt()) <= TOL_DT * ref.last_dt()
     assert_state_close(sim, ref, TOL, name)
+    cons, bf = sim.get_conserved()
+    rc, rb = ref.get_conserved()
+    worst = max(rel_err(cons[v].cpu().numpy(), rc[v]) for v in range(5))
+    if rb is not None:
+        worst = max(worst, float(np.abs(bf.cpu().numpy() - rb).max() / np.abs(rb).max()))
+    print("%s n=%d steps=%d: worst relative error %.3e, dt rel diff %.1e" % (
+        name, N, steps, worst, abs(sim.last_dt() - ref.last_dt()) / ref.last_dt()))
     return sim, ref
 
 
