@@ -50,15 +50,21 @@ IDFX_DEV double rsqrt_pos(double x) {
 #endif
 }
 
-// sqrt(x) for x >= 0 (exactly 0 for x below 1e-300)
+// sqrt(x) for x >= 0: x * rsqrt(max(x, tiny)); exact 0 stays 0 and no select is needed
 IDFX_DEV double sqrt_nn(double x) {
 #ifdef IDFX_PRECISE_MATH
   return sqrt(x);
 #else
-  const double y = rsqrt_pos(fmax(x, 1e-300));
-  double s = x * y;
-  s = fma(fma(-s, s, x), 0.5 * y, s);  // one correction step
-  return x > 1e-300 ? s : 0.0;
+  return x * rsqrt_pos(fmax(x, 1e-300));
+#endif
+}
+
+// sqrt(x) for x > 0
+IDFX_DEV double sqrt_pos(double x) {
+#ifdef IDFX_PRECISE_MATH
+  return sqrt(x);
+#else
+  return x * rsqrt_pos(x);
 #endif
 }
 
@@ -121,12 +127,12 @@ template <bool MHD>
 IDFX_DEV double signal_speed(const double W[7], double Bn, double g) {
   const double ir = rcp(W[0]);
   const double a2 = g * W[4] * ir;
-  if (!MHD) return sqrt_nn(a2);
+  if (!MHD) return sqrt_pos(a2);
   const double bn2 = Bn * Bn * ir;
   const double b2 = bn2 + (W[5] * W[5] + W[6] * W[6]) * ir;
   const double s = a2 + b2;
   const double disc = fmax(s * s - 4.0 * a2 * bn2, 0.0);
-  return sqrt_nn(0.5 * (s + sqrt_nn(disc)));
+  return sqrt_pos(0.5 * (s + sqrt_nn(disc)));
 }
 
 // O4 / G5: Davis estimate of the outer speeds; c_face = max(|S_L|,|S_R|) for every solver.
@@ -179,7 +185,7 @@ IDFX_DEV void hllc_inner(const double WL[7], const double WR[7], const double UL
 template <bool MHD>
 IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const double UL[7], const double UR[7],
                         const double FL[7], const double FR[7], double pTL, double pTR, double g, double F[7]) {
-  const double sL = sqrt_nn(WL[0]), sR = sqrt_nn(WR[0]);
+  const double sL = sqrt_pos(WL[0]), sR = sqrt_pos(WR[0]);
   const double isum = rcp(sL + sR);
   const double rb = sL * sR;
   const double irb = rcp(rb);
@@ -212,7 +218,7 @@ IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const
 
   double s0, s1, s2, s3, s4, s5 = 0.0, s6 = 0.0;
   if (!MHD) {
-    const double a = sqrt_nn(a2);
+    const double a = sqrt_pos(a2);
     const double ia2 = rcp(a2);
     // acoustic waves u -+ a: r = (rb, -+a, 0, 0, rb a2), l = (0, -+a, 0, 0, 1/rb)/(2 a2)
     const double am = (-a * du + dp * irb) * 0.5 * ia2;
@@ -225,7 +231,7 @@ IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const
     s3 = l0 * dw;
     s4 = rb * a2 * (lm + lp);
   } else {
-    const double a = sqrt_nn(a2);
+    const double a = sqrt_pos(a2);
     const double ia2 = rcp(a2);
     const double sum = a2 + bn2 + bt2;
     const double disc = sqrt_nn(fmax(sum * sum - 4.0 * a2 * bn2, 0.0));
@@ -314,12 +320,12 @@ IDFX_DEV double hlld_onesided(const double WL[7], const double WR[7], double Bn,
   {
     const double ir = rcp(WL[0]);
     const double a2 = g * WL[4] * ir, bn2 = Bn2 * ir, sm = a2 + 2.0 * pbL * ir;
-    cL = sqrt_nn(0.5 * (sm + sqrt_nn(fmax(sm * sm - 4.0 * a2 * bn2, 0.0))));
+    cL = sqrt_pos(0.5 * (sm + sqrt_nn(fmax(sm * sm - 4.0 * a2 * bn2, 0.0))));
   }
   {
     const double ir = rcp(WR[0]);
     const double a2 = g * WR[4] * ir, bn2 = Bn2 * ir, sm = a2 + 2.0 * pbR * ir;
-    cR = sqrt_nn(0.5 * (sm + sqrt_nn(fmax(sm * sm - 4.0 * a2 * bn2, 0.0))));
+    cR = sqrt_pos(0.5 * (sm + sqrt_nn(fmax(sm * sm - 4.0 * a2 * bn2, 0.0))));
   }
   const double SL = fmin(uL - cL, uR - cR), SR = fmax(uL + cL, uR + cR);
   const double cface = fmax(fabs(SL), fabs(SR));
