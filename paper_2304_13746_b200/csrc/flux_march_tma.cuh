@@ -1,0 +1,209 @@
+// flux_march_tma.cuh — the y / z marching sweep (flux_march.cuh) with its stencil planes staged through shared
+// memory by TMA.  Each CTA owns a 32 (x) by 4 (transverse) strip of pencils; per sweep plane one elected thread
+// issues two cp.async.bulk.tensor.4d loads (8 primitive fields and the staggered normal field, 9 KB) into a
+// 5-stage ring guarded by full / empty mbarriers, three planes ahead of the consumers.  Consumers read only their
+// own element of every field, so the ring replaces the register prefetch and the per-load address arithmetic.
+// MHD only (the HD sweeps keep the register-prefetch kernel).
+#pragma once
+#include <cuda.h>
+
+#include <cstdint>
+
+#include "common.cuh"
+#include "flux_march.cuh"
+#include "physics.cuh"
+
+namespace idfx {
+
+#ifndef IDFX_MINB_T
+#define IDFX_MINB_T 3
+#endif
+constexpr int TMA_NST = 5;               // ring stages
+constexpr int TMA_SLACK = 2;             // a stage is refilled two planes after it was consumed
+constexpr int TMA_PLANE_V = 8 * 4 * 32;  // doubles of the primitive box (8 fields x 4 rows x 32 columns)
+constexpr int TMA_PLANE = TMA_PLANE_V + 4 * 32;
+constexpr uint32_t TMA_PLANE_BYTES = TMA_PLANE * 8;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
+                                            int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar))
+      : "memory");
+}
+
+struct FluxTArgs {
+  int fV0;              // first field of the stage-input primitive buffer inside the V tensor map (0 or 11)
+  int fB;               // field of the normal face component inside the B tensor map
+  int ns, nt, chunk;
+  long long sd, st;
+  const double* FX[5];
+  const double* cfx;
+  double* R[5];
+  double* csum;
+  double* FB[2];
+  double* FM;
+  DevScalars* sc;
+};
+
+template <int SOLVER, int LIM, int DIR, bool WANT_DT, bool WANT_FM>
+__global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, FluxTArgs a, const __grid_constant__ CUtensorMap mapV,
+                                                           const __grid_constant__ CUtensorMap mapB) {
+  __shared__ alignas(128) double ring[TMA_NST][TMA_PLANE];
+  __shared__ uint64_t full[TMA_NST], empty[TMA_NST];
+  constexpr int PN = 1 + DIR, PT1 = 1 + (DIR + 1) % 3, PT2 = 1 + (DIR + 2) % 3;
+  // primitive field ids inside the box, in the sweep's local order (rho, u, v, w, p, B_t1, B_t2)
+  constexpr int FQ[7] = {0, 1 + DIR, 1 + (DIR + 1) % 3, 1 + (DIR + 2) % 3, 4, 5 + (DIR + 1) % 3, 5 + (DIR + 2) % 3};
+  const int lx = threadIdx.x & 31, lt = threadIdx.x >> 5;
+  const int i = blockIdx.x * 32 + lx;
+  const int t = blockIdx.y * 4 + lt;
+  const int s0 = blockIdx.z * a.chunk;
+  const int s1 = min(s0 + a.chunk, a.ns);
+  const bool active = i < g.nx && t < a.nt;
+  const int np = s1 - s0 + 4;  // planes s0-2 .. s1+1
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int st = 0; st < TMA_NST; ++st) {
+      mbar_init(&full[st], 1);
+      mbar_init(&empty[st], 128);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+  const int cx = IOFF + blockIdx.x * 32, ct = NG + blockIdx.y * 4, cs0 = NG + s0 - 2;
+  auto issue = [&](int j) {
+    uint64_t* bar = &full[j % TMA_NST];
+    double* dst = ring[j % TMA_NST];
+    mbar_expect_tx(bar, TMA_PLANE_BYTES);
+    if (DIR == 1) {
+      tma_load_4d(dst, &mapV, bar, cx, cs0 + j, ct, a.fV0);
+      tma_load_4d(dst + TMA_PLANE_V, &mapB, bar, cx, cs0 + j, ct, a.fB);
+    } else {
+      tma_load_4d(dst, &mapV, bar, cx, ct, cs0 + j, a.fV0);
+      tma_load_4d(dst + TMA_PLANE_V, &mapB, bar, cx, ct, cs0 + j, a.fB);
+    }
+  };
+  if (threadIdx.x == 0)
+    for (int j = 0; j < min(np, TMA_NST); ++j) issue(j);
+  const int so = lt * 32 + lx;  // this thread's element inside one field of a plane
+  // waits for plane j, copies this thread's 7 primitives and normal field out, releases the stage
+  auto consume = [&](int j, double q[7], double& bn) {
+    const int st = j % TMA_NST;
+    mbar_wait(&full[st], (j / TMA_NST) & 1);
+    const double* p = ring[st];
+#pragma unroll
+    for (int n = 0; n < 7; ++n) q[n] = p[FQ[n] * 128 + so];
+    bn = p[TMA_PLANE_V + so];
+    mbar_arrive(&empty[st]);
+    if (threadIdx.x == 0) {
+      const int jr = j - TMA_SLACK;
+      if (jr >= 0 && jr + TMA_NST < np) {
+        mbar_wait(&empty[jr % TMA_NST], (jr / TMA_NST) & 1);
+        issue(jr + TMA_NST);
+      }
+    }
+  };
+
+  double smax = 0.0;
+  double dm[7], q0[7], WL[7], Bn, dummy;
+  {
+    double qm[7], qc[7];
+    consume(0, qm, dummy);
+    consume(1, qc, dummy);
+    consume(2, q0, Bn);
+#pragma unroll
+    for (int n = 0; n < 7; ++n) {
+      dm[n] = q0[n] - qc[n];
+      WL[n] = qc[n] + 0.5 * limited_slope<LIM>(qc[n] - qm[n], dm[n]);  // slope of cell s0-1
+    }
+  }
+  long long c = g.at(min(i, g.nx - 1), 0, 0) + (long long)min(t, a.nt - 1) * a.st + (long long)s0 * a.sd;
+  const long long sd = a.sd;
+  double Fp[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, cfp = 0.0;
+  for (int s = s0; s <= s1; ++s, c += sd) {
+    double qp[7], Bnn;
+    consume(s - s0 + 3, qp, Bnn);  // plane s+1
+    if (active) {
+      const long long cu = c - sd;  // cell s-1, completed by this face
+      if (s + 1 < s1) {
+#pragma unroll
+        for (int n = 0; n < 5; ++n) prefetch_l1(DIR == 1 ? a.FX[n] + c + 1 : a.R[n] + c);
+      }
+      double r_in[5], cs_in = 0.0;
+      if (s > s0) {
+        if (DIR == 1) {
+#pragma unroll
+          for (int n = 0; n < 5; ++n) r_in[n] = a.FX[n][cu + 1] - a.FX[n][cu];
+          if (WANT_DT) cs_in = fmax(a.cfx[cu], a.cfx[cu + 1]);
+        } else {
+#pragma unroll
+          for (int n = 0; n < 5; ++n) r_in[n] = a.R[n][cu];
+          if (WANT_DT) cs_in = a.csum[cu];
+        }
+      }
+      double WR[7], WLn[7];
+#pragma unroll
+      for (int n = 0; n < 7; ++n) {
+        const double dp = qp[n] - q0[n];
+        const double sl = limited_slope<LIM>(dm[n], dp);
+        WR[n] = q0[n] - 0.5 * sl;
+        WLn[n] = q0[n] + 0.5 * sl;
+        dm[n] = dp;
+      }
+      double F[7];
+      const double cf = riemann<SOLVER, true>(WL, WR, Bn, g.gamma, F);
+      if (s < s1) {  // faces s0..s1-1 belong to this chunk
+        a.FB[0][c] = F[5];
+        a.FB[1][c] = F[6];
+        if (WANT_FM) a.FM[c] = F[0];
+      }
+      if (s > s0) {
+        a.R[0][cu] = r_in[0] + (F[0] - Fp[0]);
+        a.R[PN][cu] = r_in[PN] + (F[1] - Fp[1]);
+        a.R[PT1][cu] = r_in[PT1] + (F[2] - Fp[2]);
+        a.R[PT2][cu] = r_in[PT2] + (F[3] - Fp[3]);
+        a.R[4][cu] = r_in[4] + (F[4] - Fp[4]);
+        if (WANT_DT) {
+          const double cs = cs_in + fmax(cfp, cf);  // G8
+          if (DIR == 1) a.csum[cu] = cs;
+          else smax = fmax(smax, cs);
+        }
+      }
+#pragma unroll
+      for (int n = 0; n < 5; ++n) Fp[n] = F[n];
+      cfp = cf;
+#pragma unroll
+      for (int n = 0; n < 7; ++n) WL[n] = WLn[n];
+    }
+#pragma unroll
+    for (int n = 0; n < 7; ++n) q0[n] = qp[n];
+    Bn = Bnn;
+  }
+  if (WANT_DT && DIR == 2) {
+    const double m = block_max_128(smax / g.dx);
+    if (threadIdx.x == 0) atomicMax(&a.sc->smax_bits, (unsigned long long)__double_as_longlong(m));
+  }
+}
+
+}  // namespace idfx

@@ -7,6 +7,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -15,6 +16,7 @@
 #include "common.cuh"
 #include "physics.cuh"
 #include "flux_march.cuh"
+#include "flux_march_tma.cuh"
 
 namespace idfx {
 
@@ -520,6 +522,8 @@ struct idfx_ctx {
   DevScalars* sc = nullptr;
   int bcur = 0;  // which of the three face-field buffers holds the current state
   int vcur = 0;  // which primitive buffer holds the stage input
+  bool use_tma = false;            // y/z sweeps stage their planes through shared memory with TMA (MHD)
+  CUtensorMap mapV[3], mapB[3];    // per sweep direction (1 = y, 2 = z): boxes over the V and face-B field groups
   long long launches = 0;
   // optional per-kernel timing with CUDA events on the bound stream (idfx_profile_*)
   bool prof_on = false;
@@ -593,6 +597,43 @@ namespace {
 
 inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 4D tensor maps (x, y, z, field) over groups of equally spaced padded fields; one box = one sweep plane of a
+// 32 x 4 strip of pencils.
+int make_tensor_maps(idfx_ctx* c) {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess) {
+    set_err("cuTensorMapEncodeTiled is not available from this driver");
+    return IDFX_ERR_CUDA;
+  }
+  EncodeTiledFn enc = (EncodeTiledFn)fn;
+  const Geom& g = c->g;
+  const cuuint64_t py = g.ny + 2 * NG, pz = g.nz + 2 * NG;
+  const cuuint64_t strides[3] = {(cuuint64_t)g.sy * 8, (cuuint64_t)g.sz * 8, (cuuint64_t)g.np * 8};
+  const cuuint32_t es[4] = {1, 1, 1, 1};
+  for (int d = 1; d < 3; ++d) {
+    const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, 22}, dimB[4] = {(cuuint64_t)g.sy, py, pz, 9};
+    const cuuint32_t boxV[4] = {32, d == 1 ? 1u : 4u, d == 1 ? 4u : 1u, 8};
+    const cuuint32_t boxB[4] = {32, d == 1 ? 1u : 4u, d == 1 ? 4u : 1u, 1};
+    CUresult r1 = enc(&c->mapV[d], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_V), dimV, strides, boxV, es,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r2 = enc(&c->mapB[d], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_BA), dimB, strides, boxB, es,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r1 != CUDA_SUCCESS || r2 != CUDA_SUCCESS) {
+      set_err("cuTensorMapEncodeTiled failed");
+      return IDFX_ERR_CUDA;
+    }
+  }
+  return IDFX_OK;
+}
+
 int check_bound(const idfx_ctx* c) {
   if (!c) {
     set_err("null context");
@@ -648,6 +689,22 @@ void launch_dtmax(idfx_ctx* c) {
   a.sc = c->sc;
   LaunchScope ls(c, K_RHS);
   k_rhs<false, true><<<blocks_for(c->g.nc, 128), 128, 0, c->stream>>>(c->g, a);
+}
+
+template <int SOLVER, int LIM, bool MHD>
+void launch_march_tma(idfx_ctx* c, int d, dim3 grid, const FluxTArgs& ta, bool want_dt, bool uct) {
+  if constexpr (MHD) {
+    const Geom& g = c->g;
+    if (d == 1) {
+      if (want_dt) k_flux_march_tma<SOLVER, LIM, 1, true, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
+      else if (uct) k_flux_march_tma<SOLVER, LIM, 1, false, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
+      else k_flux_march_tma<SOLVER, LIM, 1, false, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
+    } else {
+      if (want_dt) k_flux_march_tma<SOLVER, LIM, 2, true, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
+      else if (uct) k_flux_march_tma<SOLVER, LIM, 2, false, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
+      else k_flux_march_tma<SOLVER, LIM, 2, false, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
+    }
+  }
 }
 
 // ---- the three flux sweeps of one stage --------------------------------------------------------
@@ -710,6 +767,16 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
     a.chunk = (int)((a.ns + nch - 1) / nch);
     dim3 grid((g.nx + 31) / 32, (a.nt + 3) / 4, (unsigned)((a.ns + a.chunk - 1) / a.chunk));
     LaunchScope ls(c, K_FLUX_X + d);
+    if (MHD && c->use_tma) {
+      FluxTArgs ta;
+      ta.fV0 = c->vcur ? 11 : 0;
+      ta.fB = (int)((Bf[d] - c->field(F_BA)) / g.np);
+      ta.ns = a.ns; ta.nt = a.nt; ta.chunk = a.chunk; ta.sd = a.sd; ta.st = a.st;
+      for (int n = 0; n < 5; ++n) { ta.FX[n] = a.FX[n]; ta.R[n] = a.R[n]; }
+      ta.cfx = a.cfx; ta.csum = a.csum; ta.FB[0] = a.FB[0]; ta.FB[1] = a.FB[1]; ta.FM = a.FM; ta.sc = a.sc;
+      launch_march_tma<SOLVER, LIM, MHD>(c, d, grid, ta, want_dt, uct);
+      continue;
+    }
     if (d == 1) {
       if (want_dt) k_flux_march<SOLVER, LIM, MHD, 1, true, true><<<grid, 128, 0, c->stream>>>(g, a);
       else if (uct) k_flux_march<SOLVER, LIM, MHD, 1, false, true><<<grid, 128, 0, c->stream>>>(g, a);
@@ -945,6 +1012,12 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
   c->vcur = 0;
   c->launches = 0;
   CK(cudaMemsetAsync(d_workspace, 0, idfx_workspace_bytes(c), c->stream));
+  const char* env = getenv("IDFX_TMA");
+  c->use_tma = c->mhd && !(env && env[0] == '0');  // IDFX_TMA=0 selects the register-prefetch sweeps (A/B only)
+  if (c->use_tma) {
+    int rc = make_tensor_maps(c);
+    if (rc) return rc;
+  }
   c->bound = true;
   return IDFX_OK;
 }
