@@ -249,7 +249,6 @@ struct EmfArgs {
   const double* FB[3][2];  // FB[d][0] = F_d[B_t1], FB[d][1] = F_d[B_t2] on the left d-faces
   const double* FM[3];     // mass flux F_d[rho]
   const double* Ec[3];     // cell-centred reference EMF -(v x Bc) of the stage input, with ghosts (G10)
-  double* E[3];
 };
 
 // E_c on the lower (a-1/2, b-1/2) edge of active cell idx, (a,b,c) cyclic (O10)
@@ -288,20 +287,9 @@ __device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& a, cons
     return e;
 }
 
-template <bool UCT>
-__global__ void __launch_bounds__(128) k_emf(Geom g, EmfArgs a) {
-  int idx[3];
-  if (!cell_of_thread(g, idx[0], idx[1], idx[2])) return;
-  const long long P = g.at(idx[0], idx[1], idx[2]);
-#pragma unroll
-  for (int c = 0; c < 3; ++c) a.E[c][P] = edge_emf<UCT>(g, a, idx, c);
-}
-
 // ---------------------------------------------------------------------------------------------
-// a5 (apply) + a7 (CT, Eq. 6) + a8 (RK2 combine, Eq. 9) + a2 (cons->prim of the result), one pass.
+// a5 (apply) + a7 (CT, Eq. 6) + a8 (RK2 combine, Eq. 9) + a2 (cons->prim of the result).
 // Stage 1: Unew = U0 - dt/dx R.  Stage 2: Unew = U0/2 + (U1 - dt/dx R)/2; same for the face field.
-// The thread also evaluates the CT update of its cell's three RIGHT faces (owned by the neighbours) so
-// that the cell-centred field of the new state is available without another pass.
 // ---------------------------------------------------------------------------------------------
 struct UpdateArgs {
   const double* Uin[5];   // state the stage started from (U0 in stage 1, U1 in stage 2)
@@ -310,7 +298,6 @@ struct UpdateArgs {
   double* Uout[5];
   const double* Bin[3];   // ghosts filled
   const double* B0[3];    // ghosts filled (stage 2 only)
-  const double* E[3];     // active lower edges only
   double* Bout[3];
   double* V[11];
   DevScalars* sc;
@@ -318,8 +305,9 @@ struct UpdateArgs {
   double cfl;
 };
 
-template <bool MHD, bool STAGE2>
-__global__ void __launch_bounds__(128) k_update(Geom g, UpdateArgs a) {
+// Hydrodynamics: apply the flux divergence, RK2 combine, cons->prim.  (MHD uses k_ct_update below.)
+template <bool STAGE2>
+__global__ void __launch_bounds__(128) k_update_hd(Geom g, UpdateArgs a) {
   int i, j, k;
   if (!cell_of_thread(g, i, j, k)) return;
   const long long c = g.at(i, j, k);
@@ -327,7 +315,6 @@ __global__ void __launch_bounds__(128) k_update(Geom g, UpdateArgs a) {
   if (!(dt > 0.0)) dt = a.cfl / __longlong_as_double((long long)a.sc->smax_bits);
   if (!STAGE2 && blockIdx.x == 0 && threadIdx.x == 0) a.sc->dt_used = dt;
   const double dtdx = dt / g.dx;
-
   double u[5];
 #pragma unroll
   for (int n = 0; n < 5; ++n) {
@@ -335,37 +322,8 @@ __global__ void __launch_bounds__(128) k_update(Geom g, UpdateArgs a) {
     u[n] = STAGE2 ? 0.5 * a.U0[n][c] + 0.5 * us : us;
     a.Uout[n][c] = u[n];
   }
-  double bc[3] = {0.0, 0.0, 0.0};
-  if (MHD) {
-    const int ip = i + 1 == g.nx ? 0 : i + 1, jp = j + 1 == g.ny ? 0 : j + 1, kp = k + 1 == g.nz ? 0 : k + 1;
-    // edge values on the 2x2x2 corner box of the cell (periodic images on the upper side)
-    auto Ex = [&](int jj, int kk) { return a.E[0][g.at(i, jj, kk)]; };
-    auto Ey = [&](int ii, int kk) { return a.E[1][g.at(ii, j, kk)]; };
-    auto Ez = [&](int ii, int jj) { return a.E[2][g.at(ii, jj, k)]; };
-    const double ex00 = Ex(j, k), ex10 = Ex(jp, k), ex01 = Ex(j, kp), ex11 = Ex(jp, kp);
-    const double ey00 = Ey(i, k), ey10 = Ey(ip, k), ey01 = Ey(i, kp), ey11 = Ey(ip, kp);
-    const double ez00 = Ez(i, j), ez10 = Ez(ip, j), ez01 = Ez(i, jp), ez11 = Ez(ip, jp);
-    // O11, left faces then right faces
-    const double cxl = (ez01 - ez00) - (ey01 - ey00), cxr = (ez11 - ez10) - (ey11 - ey10);
-    const double cyl = (ex01 - ex00) - (ez10 - ez00), cyr = (ex11 - ex10) - (ez11 - ez01);
-    const double czl = (ey10 - ey00) - (ex10 - ex00), czr = (ey11 - ey01) - (ex11 - ex01);
-    const double curlL[3] = {cxl, cyl, czl}, curlR[3] = {cxr, cyr, czr};
-    const long long st[3] = {1, g.sy, g.sz};
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-      double bl = a.Bin[d][c] - dtdx * curlL[d];
-      double br = a.Bin[d][c + st[d]] - dtdx * curlR[d];
-      if (STAGE2) {
-        bl = 0.5 * a.B0[d][c] + 0.5 * bl;
-        br = 0.5 * a.B0[d][c + st[d]] + 0.5 * br;
-      }
-      a.Bout[d][c] = bl;
-      bc[d] = 0.5 * (bl + br);
-      a.V[5 + d][c] = bc[d];
-    }
-  }
   double vx, vy, vz, p;
-  prim_from_cons(g.gamma - 1.0, u[0], u[1], u[2], u[3], u[4], bc[0], bc[1], bc[2], vx, vy, vz, p);
+  prim_from_cons(g.gamma - 1.0, u[0], u[1], u[2], u[3], u[4], 0.0, 0.0, 0.0, vx, vy, vz, p);
   if (!(u[0] > 0.0) || !(p > 0.0)) a.sc->flag = 1;
   a.V[0][c] = u[0];
   a.V[1][c] = vx;
@@ -817,7 +775,6 @@ EmfArgs emf_args(idfx_ctx* c) {
     a.FB[d][1] = c->field(F_FB + 2 * d + 1);
     a.FM[d] = d == 0 ? c->field(F_FX) : c->field(F_FM + d);
     a.Ec[d] = c->vfield(8 + d);
-    a.E[d] = nullptr;
   }
   return a;
 }
@@ -850,7 +807,6 @@ void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fi
   for (int d = 0; d < 3; ++d) {
     a.Bin[d] = c->bbuf(bin, d);
     a.B0[d] = c->bbuf(b0, d);
-    a.E[d] = nullptr;
     a.Bout[d] = c->bbuf(bout, d);
   }
   a.sc = c->sc;
@@ -874,8 +830,8 @@ void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fi
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield(n);
     {
       LaunchScope ls(c, K_UPDATE);
-      if (stage2) k_update<false, true><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
-      else k_update<false, false><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
+      if (stage2) k_update_hd<true><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
+      else k_update_hd<false><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
     }
     launch_fill(c, bout);
   }
