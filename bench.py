@@ -108,6 +108,22 @@ class ClockSampler:
                 "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(seconds_or_ms, world, device):
+    """Elapsed time of the job = the slowest rank's (replicas run independently; this is the only collective)."""
+    if world <= 1:
+        return float(seconds_or_ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([seconds_or_ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_rate(cells_per_rank, steps, world, elapsed_s):
+    """Whole-job throughput of `world` independent replicas (weak scaling): all cell-updates / slowest rank's time."""
+    return cells_per_rank * steps * world / elapsed_s
+
+
 def oracle_rate(cfg_name, n, steps, warmup):
     """cell-updates/s of the CPU oracle as it stands, one thread, on the recipe of `cfg_name` at n^3."""
     from oracle import idfxref
@@ -188,11 +204,8 @@ def run_ours(args):
     launches = sim.launch_count() - l0
     ms = e0.elapsed_time(e1)
     assert sim.status() == 0, "unphysical state during the timed region"
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = cells * K * world / (ms * 1e-3)
+    ms = max_over_ranks(ms, world, dev)
+    value = aggregate_rate(cells, K, world, ms * 1e-3)
 
     # ---- per-kernel durations over K more steps (CUDA events around every launch, on the launch stream) ----
     sim.profile(True)
@@ -246,12 +259,9 @@ def run_ours(args):
         sim.advance(K, cfl)
         sim.get_state(o_prim, o_b, host=True)   # idfx_get_state_host: D2H, synchronises
         el = time.perf_counter() - t0
-        t = torch.tensor([el], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        el = float(t.item())
+        el = max_over_ranks(el, world, dev)
         nbytes = h_prim.numel() * 8 + (h_b.numel() * 8 if h_b is not None else 0)
-        e2e = {"value": cells * K * world / el, "unit": UNIT, "h2d_bytes_per_step": nbytes / K,
+        e2e = {"value": aggregate_rate(cells, K, world, el), "unit": UNIT, "h2d_bytes_per_step": nbytes / K,
                "d2h_bytes_per_step": nbytes / K,
                "what": "set_state_host + advance(K) + get_state_host; the state crosses PCIe once per job, bytes amortised over K steps"}
 
