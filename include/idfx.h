@@ -90,7 +90,9 @@ int idfx_compute_dt(idfx_ctx* ctx, double cfl, double* h_dt_out);
 int idfx_step(idfx_ctx* ctx, double dt);
 
 /* nsteps cycles, each with dt evaluated on the state at the start of that cycle (G9); dt never leaves the
- * device.  Equivalent to nsteps x { idfx_compute_dt; idfx_step }. */
+ * device.  Equivalent to nsteps x { idfx_compute_dt; idfx_step }.  When the bound stream is not the default stream the
+ * cycle (8 kernels + one memset) is captured once per buffer-rotation state into a CUDA graph and replayed
+ * (IDFX_GRAPH=0 in the environment disables this). */
 int idfx_advance(idfx_ctx* ctx, int nsteps, double cfl);
 
 /* dt used by the most recent cycle (synchronises). */

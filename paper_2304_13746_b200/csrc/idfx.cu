@@ -480,6 +480,11 @@ struct idfx_ctx {
   DevScalars* sc = nullptr;
   int bcur = 0;  // which of the three face-field buffers holds the current state
   int vcur = 0;  // which primitive buffer holds the stage input
+  // one captured CUDA graph per buffer rotation state (3 face-field rotations x 2 primitive buffers)
+  cudaGraphExec_t graph[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  long long graph_launches[6] = {0, 0, 0, 0, 0, 0};
+  double graph_cfl = 0.0;
+  bool use_graph = true;
   bool use_tma = false;            // y/z sweeps stage their planes through shared memory with TMA (MHD)
   CUtensorMap mapV[3], mapB[3];    // per sweep direction (1 = y, 2 = z): boxes over the V and face-B field groups
   long long launches = 0;
@@ -590,6 +595,13 @@ int make_tensor_maps(idfx_ctx* c) {
     }
   }
   return IDFX_OK;
+}
+
+void drop_graphs(idfx_ctx* c) {
+  for (int k = 0; k < 6; ++k) {
+    if (c->graph[k]) cudaGraphExecDestroy(c->graph[k]);
+    c->graph[k] = nullptr;
+  }
 }
 
 int check_bound(const idfx_ctx* c) {
@@ -968,6 +980,11 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
   c->vcur = 0;
   c->launches = 0;
   CK(cudaMemsetAsync(d_workspace, 0, idfx_workspace_bytes(c), c->stream));
+  drop_graphs(c);
+  const char* genv = getenv("IDFX_GRAPH");
+  // the legacy default stream cannot be captured: graphs only on a stream of the caller's own
+  c->use_graph = !(genv && genv[0] == '0') && c->stream != nullptr && c->stream != cudaStreamLegacy &&
+                 c->stream != cudaStreamPerThread;
   const char* env = getenv("IDFX_TMA");
   c->use_tma = c->mhd && !(env && env[0] == '0');  // IDFX_TMA=0 selects the register-prefetch sweeps (A/B only)
   if (c->use_tma) {
@@ -1127,8 +1144,40 @@ int idfx_advance(idfx_ctx* c, int nsteps, double cfl) {
     set_err("idfx_advance: need nsteps >= 0 and 0 < cfl < 1");
     return IDFX_ERR_INVALID_ARG;
   }
-  for (int s = 0; s < nsteps; ++s)
-    if ((rc = run_cycle(c, 0.0, cfl))) return rc;
+  if (c->graph_cfl != cfl) {
+    drop_graphs(c);
+    c->graph_cfl = cfl;
+  }
+  for (int s = 0; s < nsteps; ++s) {
+    if (!c->use_graph || c->prof_on) {
+      if ((rc = run_cycle(c, 0.0, cfl))) return rc;
+      continue;
+    }
+    // the cycle is a fixed sequence of 8 kernels + 1 memset whose arguments depend only on the buffer rotation
+    // state: capture it once per state, then replay (dt never leaves the device, so nothing else varies)
+    const int key = c->bcur * 2 + c->vcur;
+    if (!c->graph[key]) {
+      const int b = c->bcur, v = c->vcur;
+      const long long l0 = c->launches;
+      cudaGraph_t gr = nullptr;
+      CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+      rc = run_cycle(c, 0.0, cfl);
+      cudaError_t e = cudaStreamEndCapture(c->stream, &gr);
+      if (rc || e != cudaSuccess || !gr) {
+        set_err("CUDA graph capture of the cycle failed: %s", cudaGetErrorString(e));
+        return IDFX_ERR_CUDA;
+      }
+      CK(cudaGraphInstantiate(&c->graph[key], gr, 0));
+      cudaGraphDestroy(gr);
+      c->graph_launches[key] = c->launches - l0;
+      c->launches = l0;  // nothing ran during capture
+      c->bcur = b;
+      c->vcur = v;
+    }
+    CK(cudaGraphLaunch(c->graph[key], c->stream));
+    c->launches += c->graph_launches[key];
+    c->bcur = (c->bcur + 2) % 3;  // as run_cycle leaves it; vcur toggles twice per cycle
+  }
   return IDFX_OK;
 }
 
@@ -1188,6 +1237,7 @@ const char* idfx_profile_kernel_name(int kernel_id) {
 void idfx_destroy(idfx_ctx* c) {
   if (!c) return;
   prof_drain(c);
+  drop_graphs(c);
   for (cudaEvent_t e : c->prof_free) cudaEventDestroy(e);
   delete c;
 }

@@ -99,10 +99,28 @@ class Idfx:
         self.mhd = emf_mode != EMF_NONE
         nbytes = self.L.idfx_workspace_bytes(self.h)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        # The library enqueues on its own stream (a non-default stream can be captured into CUDA graphs); every call
+        # below orders that stream after the caller's current stream and the caller's stream after it.
         with torch.cuda.device(self.device):
-            s = stream if stream is not None else torch.cuda.current_stream(self.device)
-        self.stream = s
-        _check(self.L.idfx_bind(self.h, self.workspace.data_ptr(), nbytes, s.cuda_stream))
+            self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
+        _check(self.L.idfx_bind(self.h, self.workspace.data_ptr(), nbytes, self.stream.cuda_stream))
+
+    class _Ordered:
+        def __init__(self, sim):
+            self.sim = sim
+
+        def __enter__(self):
+            self.cur = torch.cuda.current_stream(self.sim.device)
+            if self.cur != self.sim.stream:
+                self.sim.stream.wait_stream(self.cur)
+
+        def __exit__(self, *exc):
+            if self.cur != self.sim.stream:
+                self.cur.wait_stream(self.sim.stream)
+            return False
+
+    def _ordered(self):
+        return Idfx._Ordered(self)
 
     def close(self):
         if getattr(self, "h", None):
@@ -125,7 +143,8 @@ class Idfx:
         host = not prim.is_cuda
         f = self.L.idfx_set_state_host if host else self.L.idfx_set_state
         p = self._host if host else self._dev
-        _check(f(self.h, p(prim, 5), p(bface, 3) if bface is not None else None))
+        with self._ordered():
+            _check(f(self.h, p(prim, 5), p(bface, 3) if bface is not None else None))
 
     def get_state(self, out_prim=None, out_bface=None, host=False):
         dev = "cpu" if host else self.device
@@ -135,25 +154,30 @@ class Idfx:
             out_bface = torch.empty((3,) + self.shape, dtype=torch.float64, device=dev, pin_memory=host)
         f = self.L.idfx_get_state_host if host else self.L.idfx_get_state
         p = self._host if host else self._dev
-        _check(f(self.h, p(out_prim, 5), p(out_bface, 3) if out_bface is not None else None))
+        with self._ordered():
+            _check(f(self.h, p(out_prim, 5), p(out_bface, 3) if out_bface is not None else None))
         return out_prim, out_bface
 
     def get_conserved(self):
         cons = torch.empty((5,) + self.shape, dtype=torch.float64, device=self.device)
         bface = torch.empty((3,) + self.shape, dtype=torch.float64, device=self.device) if self.mhd else None
-        _check(self.L.idfx_get_conserved(self.h, cons.data_ptr(), bface.data_ptr() if self.mhd else None))
+        with self._ordered():
+            _check(self.L.idfx_get_conserved(self.h, cons.data_ptr(), bface.data_ptr() if self.mhd else None))
         return cons, bface
 
     def compute_dt(self, cfl):
         dt = ctypes.c_double()
-        _check(self.L.idfx_compute_dt(self.h, cfl, ctypes.byref(dt)))
+        with self._ordered():
+            _check(self.L.idfx_compute_dt(self.h, cfl, ctypes.byref(dt)))
         return dt.value
 
     def step(self, dt):
-        _check(self.L.idfx_step(self.h, dt))
+        with self._ordered():
+            _check(self.L.idfx_step(self.h, dt))
 
     def advance(self, nsteps, cfl):
-        _check(self.L.idfx_advance(self.h, nsteps, cfl))
+        with self._ordered():
+            _check(self.L.idfx_advance(self.h, nsteps, cfl))
 
     def last_dt(self):
         dt = ctypes.c_double()
