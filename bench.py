@@ -35,6 +35,11 @@ ALGO_FLOPS_PER_CELL = {"flux_x": 360.0, "flux_y": 360.0, "flux_z": 360.0}
 ALGO_BYTES_PER_CELL = {"flux_x": 8 * 16.0, "flux_y": 8 * 21.0, "flux_z": 8 * 21.0, "ct_update_prim": 8 * 48.0}
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch (mean of the stage-1 and stage-2 launch) from the committed
+# ncu --set full capture of this command at 512^3 (profiles/r01_ncu_full_512.md); only valid for that workload
+NCU_TRAFFIC_BYTES_512 = {"flux_x": 17.81e9, "flux_y": 25.72e9, "flux_z": 24.91e9, "ct_update_prim": 56.86e9}
+
+
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -230,13 +235,16 @@ def run_ours(args):
     def roof_of(name):
         k = kernels[name]
         hbm = {"kernel": name, "bound": "hbm", "achieved": k["algo_GBps"], "peak": hbm_peak, "unit": "GB/s",
-               "frac": k["algo_GBps"] / hbm_peak, "traffic": None, "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % peak_kind}
+               "frac": k["algo_GBps"] / hbm_peak, "traffic": k.get("ncu_dram_bytes"), "peak_source": "MEASURED_PEAKS.json hbm_gbs (%s)" % peak_kind}
         if name not in ALGO_FLOPS_PER_CELL:
             return hbm
         alu = {"kernel": name, "bound": "alu", "achieved": k["algo_TFLOPs"], "peak": fp64_tflops, "unit": "TFLOP/s",
-               "frac": k["algo_TFLOPs"] / fp64_tflops, "traffic": None,
+               "frac": k["algo_TFLOPs"] / fp64_tflops, "traffic": k.get("ncu_dram_bytes"),
                "peak_source": "fp64 DFMA probe measured in this run (idfx_probe_fp64)", "hbm_frac": hbm["frac"]}
         return alu
+    if n == 512 and args.workload == "config5":
+        for k in kernels:
+            kernels[k]["ncu_dram_bytes"] = NCU_TRAFFIC_BYTES_512.get(k)
     per_launch = {k: v["avg_ms"] for k, v in kernels.items() if k in ALGO_BYTES_PER_CELL}
     dom = max(per_launch, key=per_launch.get)
     roof = roof_of(dom)
