@@ -341,13 +341,22 @@ __global__ void __launch_bounds__(128) k_update_hd(Geom g, UpdateArgs a) {
 // ---------------------------------------------------------------------------------------------
 constexpr int CT_TX = 32, CT_TY = 4, CT_TZ = 4;  // 32x8x4 and 32x8x8 tiles measured the same
 constexpr int CT_THREADS = CT_TX * CT_TY;
+#ifndef IDFX_MINB_CT
+#define IDFX_MINB_CT 8
+#endif
+#ifndef IDFX_CT_UNROLL
+#define IDFX_CT_UNROLL 1
+#endif
+#define IDFX_PRAGMA_(x) _Pragma(#x)
+#define IDFX_UNROLL(n) IDFX_PRAGMA_(unroll n)
 constexpr int CT_LX = CT_TX + 1, CT_LY = CT_TY + 1, CT_LZ = CT_TZ + 1;
 
 template <bool UCT, bool STAGE2>
-__global__ void __launch_bounds__(CT_THREADS) k_ct_update(Geom g, EmfArgs ea, UpdateArgs a) {
+__global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, EmfArgs ea, UpdateArgs a) {
   __shared__ double sE[3][CT_LZ][CT_LY][CT_LX];
   const int i0 = blockIdx.x * CT_TX, j0 = blockIdx.y * CT_TY, k0 = blockIdx.z * CT_TZ;
   // ---- phase 1: edge lattice ----
+  IDFX_UNROLL(IDFX_CT_UNROLL)
   for (int p = threadIdx.x; p < CT_LZ * CT_LY * CT_LX; p += CT_THREADS) {
     const int li = p % CT_LX, lj = (p / CT_LX) % CT_LY, lk = p / (CT_LX * CT_LY);
     const int I = i0 + li, J = j0 + lj, K = k0 + lk;
