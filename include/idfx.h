@@ -43,8 +43,9 @@ extern "C" {
 
 typedef struct idfx_ctx idfx_ctx;
 
-/* Riemann solvers.  HLLC is hydrodynamics-only; in MHD it is replaced by HLLD. */
-enum { IDFX_SOLVER_HLL = 0, IDFX_SOLVER_HLLC = 1, IDFX_SOLVER_HLLD = 2, IDFX_SOLVER_ROE = 3 };
+/* Riemann solvers, here listed by number; the paper orders them from most to least diffusive:
+ * Rusanov (local Lax-Friedrichs), HLL, HLLC / HLLD, Roe.  HLLC is hydrodynamics-only; in MHD it is replaced by HLLD. */
+enum { IDFX_SOLVER_HLL = 0, IDFX_SOLVER_HLLC = 1, IDFX_SOLVER_HLLD = 2, IDFX_SOLVER_ROE = 3, IDFX_SOLVER_RUSANOV = 4 };
 /* Reconstruction: flat (1st order), PLM with minmod or van Leer (harmonic mean, G2) slopes. */
 enum { IDFX_LIMITER_FLAT = 0, IDFX_LIMITER_MINMOD = 1, IDFX_LIMITER_VANLEER = 2 };
 /* EMF reconstruction.  IDFX_EMF_NONE selects hydrodynamics (no magnetic field at all). */
@@ -59,7 +60,7 @@ enum {
 };
 
 /* Creates a context.  Requirements: nx, ny, nz >= 4; dx > 0; gamma > 1; valid enums; HD (emf_mode NONE)
- * with HLL/HLLC/ROE, MHD with HLL/HLLD/ROE.  Returns NULL on error (idfx_last_error() says why).
+ * with RUSANOV/HLL/HLLC/ROE, MHD with RUSANOV/HLL/HLLD/ROE.  Returns NULL on error (idfx_last_error() says why).
  * Host-only: touches no device memory. */
 idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solver, int limiter, int emf_mode);
 

@@ -14,7 +14,7 @@
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): flux consistency F(U,U)=F(U); HLL/HLLC/HLLD
 // fan-integral identity; HLLC p* continuity; isolated contact and rotational discontinuities; Roe
 // L·R=I, A·r=λr against a finite-difference Jacobian, Σλαr = F_R−F_L; MHD-Roe(B=0) = 5-wave HD Roe;
-// limiter properties; exact Sod solution along x, y, z; direction symmetry; uniform state; conservation;
+// Rusanov = HLL with symmetric speeds; limiter properties; exact Sod solution along x, y, z; direction symmetry; uniform state; conservation;
 // div B; Eᶜ plane-parallel identity; RK2 amplification factor; closed-form dt; 2nd-order convergence of
 // linear fast/Alfvén waves.
 // PARITY UNPINNED (the paper fixes none of these and prints no number that depends on them, see
@@ -35,7 +35,7 @@ namespace {
 
 constexpr int NG = 2;  // ghost layers: PLM needs 2 ("number of ghost cells ... adjusted")
 
-enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3 };
+enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_RUSANOV = 4 };
 enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2 };
 enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2 };
 enum { OK = 0, ERR_INVALID_ARG = -1, ERR_UNSUPPORTED = -2, ERR_UNPHYSICAL = -5 };
@@ -100,6 +100,13 @@ void hll_flux(const double UL[7], const double UR[7], const double FL[7], const 
   } else {
     for (int n = 0; n < 7; ++n) F[n] = (SR * FL[n] - SL * FR[n] + SL * SR * (UR[n] - UL[n])) / (SR - SL);
   }
+}
+
+// Rusanov / local Lax-Friedrichs flux ("Lax-Friedrichs Rusanov flux (Rusanov 1962)", the most diffusive
+// solver of the paper's list): F = (F_L + F_R)/2 - (c_face/2)(U_R - U_L) with c_face = max(|S_L|,|S_R|) (O4).
+void rusanov_flux(const double UL[7], const double UR[7], const double FL[7], const double FR[7], double cface,
+                  double F[7]) {
+  for (int n = 0; n < 7; ++n) F[n] = 0.5 * (FL[n] + FR[n]) - 0.5 * cface * (UR[n] - UL[n]);
 }
 
 // O6 HLLC, hydrodynamics only (Toro et al. 1994).  Star states are returned for the pins.
@@ -447,6 +454,7 @@ int riemann(int solver, double g, const double WL[7], const double WR[7], double
     case SOLVER_HLL: hll_flux(UL, UR, FL, FR, SL, SR, F); break;
     case SOLVER_HLLC: hllc_flux(WL, WR, UL, UR, FL, FR, SL, SR, F); break;
     case SOLVER_HLLD: hlld_flux(WL, WR, Bn, UL, UR, FL, FR, SL, SR, F); break;
+    case SOLVER_RUSANOV: rusanov_flux(UL, UR, FL, FR, cface, F); break;
     default:
       if (!roe_flux(WL, WR, Bn, UL, UR, FL, FR, g, F)) {
         hll_flux(UL, UR, FL, FR, SL, SR, F);
@@ -728,7 +736,7 @@ struct idfxref_ctx {
 IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, double gamma, int solver,
                                         int limiter, int emf_mode) {
   if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(gamma > 1.0)) return nullptr;
-  if (solver < 0 || solver > 3 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 2) return nullptr;
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 2) return nullptr;
   const bool mhd = emf_mode != EMF_NONE;
   if (mhd && solver == SOLVER_HLLC) return nullptr;
   if (!mhd && solver == SOLVER_HLLD) return nullptr;

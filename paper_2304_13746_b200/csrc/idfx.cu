@@ -780,10 +780,12 @@ void launch_sweeps_s(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
 void launch_sweeps(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
   if (c->mhd) {
     if (c->solver == SOLVER_HLL) launch_sweeps_s<SOLVER_HLL, true>(c, Bf, want_dt);
+    else if (c->solver == SOLVER_RUSANOV) launch_sweeps_s<SOLVER_RUSANOV, true>(c, Bf, want_dt);
     else if (c->solver == SOLVER_HLLD) launch_sweeps_s<SOLVER_HLLD, true>(c, Bf, want_dt);
     else launch_sweeps_s<SOLVER_ROE, true>(c, Bf, want_dt);
   } else {
     if (c->solver == SOLVER_HLL) launch_sweeps_s<SOLVER_HLL, false>(c, Bf, want_dt);
+    else if (c->solver == SOLVER_RUSANOV) launch_sweeps_s<SOLVER_RUSANOV, false>(c, Bf, want_dt);
     else if (c->solver == SOLVER_HLLC) launch_sweeps_s<SOLVER_HLLC, false>(c, Bf, want_dt);
     else launch_sweeps_s<SOLVER_ROE, false>(c, Bf, want_dt);
   }
@@ -939,7 +941,7 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
     set_err("idfx_create: need dx > 0 and gamma > 1");
     return nullptr;
   }
-  if (solver < 0 || solver > 3 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 2) {
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 2) {
     set_err("idfx_create: unknown solver, limiter or emf_mode");
     return nullptr;
   }

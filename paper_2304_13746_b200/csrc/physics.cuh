@@ -13,7 +13,7 @@
 
 namespace idfx {
 
-enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3 };
+enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_RUSANOV = 4 };
 enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2 };
 enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2 };
 
@@ -434,6 +434,12 @@ IDFX_DEV double riemann(const double WL[7], const double WR[7], double Bn, doubl
   outer_speeds<MHD>(WL, WR, Bn, g, SL, SR);
   const double cface = fmax(fabs(SL), fabs(SR));
   constexpr int NV = MHD ? 7 : 5;
+  if (SOLVER == SOLVER_RUSANOV) {  // local Lax-Friedrichs: central flux minus c_face/2 times the jump
+    const double hc = 0.5 * cface;
+#pragma unroll
+    for (int n = 0; n < 7; ++n) F[n] = n < NV ? 0.5 * (FL[n] + FR[n]) - hc * (UR[n] - UL[n]) : 0.0;
+    return cface;
+  }
   if (SOLVER == SOLVER_ROE) {
     if (!roe_inner<MHD>(WL, WR, Bn, UL, UR, FL, FR, pTL, pTR, g, F)) {
       if (SL >= 0.0) {

@@ -13,7 +13,7 @@ from paper_2304_13746_b200 import inputs
 
 pytestmark = pytest.mark.gpu
 
-HLL, HLLC, HLLD, ROE = 0, 1, 2, 3
+HLL, HLLC, HLLD, ROE, RUSANOV = 0, 1, 2, 3, 4
 FLAT, MINMOD, VANLEER = 0, 1, 2
 EMF_NONE, EMF_ARITH, EMF_UCT = 0, 1, 2
 TOL = 1e-10
@@ -90,7 +90,7 @@ COMBOS = [
     (ROE, VANLEER, EMF_NONE), (ROE, MINMOD, EMF_NONE),
     (HLL, VANLEER, EMF_ARITH), (HLL, MINMOD, EMF_UCT), (HLLD, VANLEER, EMF_ARITH), (HLLD, VANLEER, EMF_UCT),
     (HLLD, MINMOD, EMF_UCT), (HLLD, FLAT, EMF_ARITH), (ROE, VANLEER, EMF_ARITH), (ROE, VANLEER, EMF_UCT),
-    (ROE, MINMOD, EMF_ARITH),
+    (ROE, MINMOD, EMF_ARITH), (RUSANOV, VANLEER, EMF_NONE), (RUSANOV, VANLEER, EMF_UCT), (RUSANOV, MINMOD, EMF_ARITH),
 ]
 
 

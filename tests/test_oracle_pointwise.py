@@ -7,7 +7,7 @@ import os
 import numpy as np
 import pytest
 
-HLL, HLLC, HLLD, ROE = 0, 1, 2, 3
+HLL, HLLC, HLLD, ROE, RUSANOV = 0, 1, 2, 3, 4
 FLAT, MINMOD, VANLEER = 0, 1, 2
 G = 5.0 / 3.0
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
@@ -57,7 +57,8 @@ def test_phys_flux_matches_equations(R):
         np.testing.assert_allclose(R.cons_from_prim(G, W, Bn), cons_np(W, Bn, G), rtol=1e-15)
 
 
-@pytest.mark.parametrize("solver,mhd", [(HLL, False), (HLLC, False), (ROE, False), (HLL, True), (HLLD, True), (ROE, True)])
+@pytest.mark.parametrize("solver,mhd", [(HLL, False), (HLLC, False), (ROE, False), (RUSANOV, False), (HLL, True),
+                                        (HLLD, True), (ROE, True), (RUSANOV, True)])
 def test_flux_consistency(R, solver, mhd):
     """F_solver(U, U) = F(U) (north_star pin)."""
     rng = np.random.default_rng(2)
@@ -118,6 +119,33 @@ def test_hll_supersonic_and_formula(R):
         for solver in (HLL, HLLD, ROE):
             F = R.riemann(solver, G, a, b, 0.3)[0]
             np.testing.assert_allclose(F, flux_np(s, 0.3, G), rtol=1e-12)
+
+
+def test_rusanov_is_central_flux_minus_half_cface_jump(R):
+    """PAPER.md:81 "Lax-Friedrichs Rusanov flux": F = (F_L+F_R)/2 - (c/2)(U_R-U_L), c = max(|u|+c_f) of the two sides;
+    identical to HLL when the fan is symmetric (S_R = -S_L), and never less diffusive than HLL."""
+    rng = np.random.default_rng(41)
+    for _ in range(200):
+        WL, WR, Bn = rand_state(rng), rand_state(rng), rng.uniform(-1, 1)
+        F, c, fb = R.riemann(RUSANOV, G, WL, WR, Bn)
+
+        def cf(W):
+            a2, b2 = G * W[4] / W[0], (Bn * Bn + W[5] ** 2 + W[6] ** 2) / W[0]
+            return np.sqrt(0.5 * (a2 + b2 + np.sqrt((a2 + b2) ** 2 - 4 * a2 * Bn * Bn / W[0])))
+        lam = max(abs(WL[1]) + cf(WL), abs(WR[1]) + cf(WR))
+        assert c == pytest.approx(lam, rel=1e-13) and fb == 0
+        ref = 0.5 * (flux_np(WL, Bn, G) + flux_np(WR, Bn, G)) - 0.5 * lam * (cons_np(WR, Bn, G) - cons_np(WL, Bn, G))
+        np.testing.assert_allclose(F, ref, rtol=1e-13, atol=1e-13)
+    # symmetric fan: same speeds on both sides and u = 0  =>  S_R = -S_L  =>  HLL = Rusanov
+    for _ in range(50):
+        WL = rand_state(rng)
+        WL[1] = 0.0
+        WR = WL.copy()
+        WR[2:4] = rng.uniform(-1, 1, 2)          # a shear and a rotation of B_t keep |u| + c_f equal
+        th = rng.uniform(0, 2 * np.pi)
+        bt = np.hypot(WL[5], WL[6])
+        WR[5], WR[6] = bt * np.cos(th), bt * np.sin(th)
+        np.testing.assert_allclose(R.riemann(RUSANOV, G, WL, WR, 0.4)[0], R.riemann(HLL, G, WL, WR, 0.4)[0], atol=1e-13)
 
 
 def test_hllc_fan_integral_and_pressure(R):
