@@ -48,8 +48,9 @@ typedef struct idfx_ctx idfx_ctx;
 enum { IDFX_SOLVER_HLL = 0, IDFX_SOLVER_HLLC = 1, IDFX_SOLVER_HLLD = 2, IDFX_SOLVER_ROE = 3, IDFX_SOLVER_RUSANOV = 4 };
 /* Reconstruction: flat (1st order), PLM with minmod or van Leer (harmonic mean, G2) slopes. */
 enum { IDFX_LIMITER_FLAT = 0, IDFX_LIMITER_MINMOD = 1, IDFX_LIMITER_VANLEER = 2 };
-/* EMF reconstruction.  IDFX_EMF_NONE selects hydrodynamics (no magnetic field at all). */
-enum { IDFX_EMF_NONE = 0, IDFX_EMF_ARITHMETIC = 1, IDFX_EMF_UCT_CONTACT = 2 };
+/* EMF reconstruction: arithmetic average of the face fluxes, and the E^0 and E^c (upwind-contact)
+ * schemes of Gardiner & Stone 2005.  IDFX_EMF_NONE selects hydrodynamics (no magnetic field at all). */
+enum { IDFX_EMF_NONE = 0, IDFX_EMF_ARITHMETIC = 1, IDFX_EMF_UCT_CONTACT = 2, IDFX_EMF_UCT_0 = 3 };
 enum {
   IDFX_OK = 0,
   IDFX_ERR_INVALID_ARG = -1,

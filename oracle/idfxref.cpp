@@ -37,7 +37,7 @@ constexpr int NG = 2;  // ghost layers: PLM needs 2 ("number of ghos
 
 enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_RUSANOV = 4 };
 enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2 };
-enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2 };
+enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3 };
 enum { OK = 0, ERR_INVALID_ARG = -1, ERR_UNSUPPORTED = -2, ERR_UNPHYSICAL = -5 };
 
 // ---------------------------------------------------------------------------------------------
@@ -624,6 +624,12 @@ void edge_emf(Ctx& c, int comp) {
       for (ijk[0] = lo[0]; ijk[0] <= hi[0]; ++ijk[0]) {
         const size_t P = c.at(ijk[0], ijk[1], ijk[2]);
         double e = 0.25 * (Ea(P) + Ea(P - eb) + Eb(P) + Eb(P - ea));
+        if (c.emf == EMF_UCT0) {
+          // E^0 of Gardiner & Stone 2005: the E^c construction with the two candidate gradients
+          // averaged instead of upwinded, which collapses to (1/2) sum of the four face values - (1/4) sum of the
+          // four cell-centred reference values
+          e = 0.5 * (Ea(P) + Ea(P - eb) + Eb(P) + Eb(P - ea)) - 0.25 * (Ec(P) + Ec(P - ea) + Ec(P - eb) + Ec(P - ea - eb));
+        }
         if (c.emf == EMF_UCT) {
           // d/db at the a-face (ia-1/2): quarter points ib-1/4 (cells P-ea, P) and ib-3/4 (cells P-ea-eb, P-eb)
           const double gbp_m = 2.0 * (Ec(P - ea) - Eb(P - ea));          // g_b+ of cell P-ea
@@ -736,7 +742,7 @@ struct idfxref_ctx {
 IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, double gamma, int solver,
                                         int limiter, int emf_mode) {
   if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(gamma > 1.0)) return nullptr;
-  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 2) return nullptr;
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 3) return nullptr;
   const bool mhd = emf_mode != EMF_NONE;
   if (mhd && solver == SOLVER_HLLC) return nullptr;
   if (!mhd && solver == SOLVER_HLLD) return nullptr;

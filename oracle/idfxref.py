@@ -16,7 +16,7 @@ _LIB = os.path.join(_HERE, "libidfxref.so")
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
 LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER = 0, 1, 2
-EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT = 0, 1, 2
+EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0 = 0, 1, 2, 3
 OK, ERR_UNPHYSICAL = 0, -5
 
 _lib = None

@@ -252,7 +252,7 @@ struct EmfArgs {
 };
 
 // E_c on the lower (a-1/2, b-1/2) edge of active cell idx, (a,b,c) cyclic (O10)
-template <bool UCT>
+template <int MODE>
 __device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& a, const int idx[3], int c) {
   const int n[3] = {g.nx, g.ny, g.nz};
   const long long st[3] = {1, g.sy, g.sz};
@@ -266,7 +266,13 @@ __device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& a, cons
     const double EaP = -Fa[P], EaPb = -Fa[P + db];  // a-faces at (ia-1/2, ib) and (ia-1/2, ib-1)
     const double EbP = Fb[P], EbPa = Fb[P + da];    // b-faces at (ia, ib-1/2) and (ia-1, ib-1/2)
     double e = 0.25 * (EaP + EaPb + EbP + EbPa);
-    if (UCT) {
+    if (MODE == EMF_UCT0) {
+      // E^0: averaged instead of upwinded gradients = (1/2) sum of faces - (1/4) sum of cell-centred references
+      const double* __restrict__ Ecc = a.Ec[c];
+      e = 0.5 * (EaP + EaPb + EbP + EbPa) -
+          0.25 * (Ecc[P] + Ecc[P - st[ia]] + Ecc[P - st[ib]] + Ecc[P - st[ia] - st[ib]]);
+    }
+    if (MODE == EMF_UCT) {
       // cell-centred reference EMF of the stage input (G10), stored with ghosts next to the primitives
       const double* __restrict__ Ecc = a.Ec[c];
       const double Ec = Ecc[P], Eca = Ecc[P - st[ia]], Ecb = Ecc[P - st[ib]], Ecab = Ecc[P - st[ia] - st[ib]];
@@ -351,7 +357,7 @@ constexpr int CT_THREADS = CT_TX * CT_TY;
 #define IDFX_UNROLL(n) IDFX_PRAGMA_(unroll n)
 constexpr int CT_LX = CT_TX + 1, CT_LY = CT_TY + 1, CT_LZ = CT_TZ + 1;
 
-template <bool UCT, bool STAGE2>
+template <int MODE, bool STAGE2>
 __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, EmfArgs ea, UpdateArgs a) {
   __shared__ double sE[3][CT_LZ][CT_LY][CT_LX];
   const int i0 = blockIdx.x * CT_TX, j0 = blockIdx.y * CT_TY, k0 = blockIdx.z * CT_TZ;
@@ -363,9 +369,9 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
     if (I > g.nx || J > g.ny || K > g.nz) continue;
     // periodic image of lattice index n is index 0
     const int idx[3] = {I == g.nx ? 0 : I, J == g.ny ? 0 : J, K == g.nz ? 0 : K};
-    if (li < CT_TX) sE[0][lk][lj][li] = edge_emf<UCT>(g, ea, idx, 0);
-    if (lj < CT_TY) sE[1][lk][lj][li] = edge_emf<UCT>(g, ea, idx, 1);
-    if (lk < CT_TZ) sE[2][lk][lj][li] = edge_emf<UCT>(g, ea, idx, 2);
+    if (li < CT_TX) sE[0][lk][lj][li] = edge_emf<MODE>(g, ea, idx, 0);
+    if (lj < CT_TY) sE[1][lk][lj][li] = edge_emf<MODE>(g, ea, idx, 1);
+    if (lk < CT_TZ) sE[2][lk][lj][li] = edge_emf<MODE>(g, ea, idx, 2);
   }
   __syncthreads();
   // ---- phase 2: one (i, j) column of TZ cells per thread ----
@@ -842,12 +848,17 @@ void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fi
     const EmfArgs ea = emf_args(c);
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield_out(n);
     dim3 grid((g.nx + CT_TX - 1) / CT_TX, (g.ny + CT_TY - 1) / CT_TY, (g.nz + CT_TZ - 1) / CT_TZ);
-    const bool uct = c->emf == EMF_UCT;
     LaunchScope ls(c, K_UPDATE);
-    if (uct && stage2) k_ct_update<true, true><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
-    else if (uct) k_ct_update<true, false><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
-    else if (stage2) k_ct_update<false, true><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
-    else k_ct_update<false, false><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
+    if (c->emf == EMF_UCT) {
+      if (stage2) k_ct_update<EMF_UCT, true><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
+      else k_ct_update<EMF_UCT, false><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
+    } else if (c->emf == EMF_UCT0) {
+      if (stage2) k_ct_update<EMF_UCT0, true><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
+      else k_ct_update<EMF_UCT0, false><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
+    } else {
+      if (stage2) k_ct_update<EMF_ARITH, true><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
+      else k_ct_update<EMF_ARITH, false><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
+    }
     c->vcur ^= 1;
   } else {
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield(n);
@@ -941,7 +952,7 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
     set_err("idfx_create: need dx > 0 and gamma > 1");
     return nullptr;
   }
-  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 2) {
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 3) {
     set_err("idfx_create: unknown solver, limiter or emf_mode");
     return nullptr;
   }

@@ -11,7 +11,7 @@ import torch
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
 LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER = 0, 1, 2
-EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT = 0, 1, 2
+EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0 = 0, 1, 2, 3
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_NOT_BOUND, ERR_CUDA, ERR_UNPHYSICAL = 0, -1, -2, -3, -4, -5
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
 
 HLL, HLLC, HLLD, ROE, RUSANOV = 0, 1, 2, 3, 4
 FLAT, MINMOD, VANLEER = 0, 1, 2
-EMF_NONE, EMF_ARITH, EMF_UCT = 0, 1, 2
+EMF_NONE, EMF_ARITH, EMF_UCT, EMF_UCT0 = 0, 1, 2, 3
 TOL = 1e-10
 TOL_DT = 1e-12
 
@@ -91,6 +91,7 @@ COMBOS = [
     (HLL, VANLEER, EMF_ARITH), (HLL, MINMOD, EMF_UCT), (HLLD, VANLEER, EMF_ARITH), (HLLD, VANLEER, EMF_UCT),
     (HLLD, MINMOD, EMF_UCT), (HLLD, FLAT, EMF_ARITH), (ROE, VANLEER, EMF_ARITH), (ROE, VANLEER, EMF_UCT),
     (ROE, MINMOD, EMF_ARITH), (RUSANOV, VANLEER, EMF_NONE), (RUSANOV, VANLEER, EMF_UCT), (RUSANOV, MINMOD, EMF_ARITH),
+    (HLLD, VANLEER, EMF_UCT0), (ROE, MINMOD, EMF_UCT0),
 ]
 
 
