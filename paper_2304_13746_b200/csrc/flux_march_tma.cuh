@@ -64,9 +64,14 @@ struct FluxTArgs {
   double* FB[2];
   double* FM;
   DevScalars* sc;
+  // APPLY (stage 2 of the z sweep): the completed divergence is applied at once, U = U0/2 + (U1 - dt/dx R)/2
+  const double* Uin[5];
+  const double* U0[5];
+  double* Uout[5];
+  double dt_fixed, cfl;
 };
 
-template <int SOLVER, int LIM, int DIR, bool WANT_DT, bool WANT_FM>
+template <int SOLVER, int LIM, int DIR, bool WANT_DT, bool WANT_FM, bool APPLY>
 __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, FluxTArgs a, const __grid_constant__ CUtensorMap mapV,
                                                            const __grid_constant__ CUtensorMap mapB) {
   __shared__ alignas(128) double ring[TMA_NST][TMA_PLANE];
@@ -125,7 +130,12 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
     }
   };
 
-  double smax = 0.0;
+  double smax = 0.0, dtdx = 0.0;
+  if (APPLY) {
+    double dt = a.dt_fixed;
+    if (!(dt > 0.0)) dt = a.cfl / __longlong_as_double((long long)a.sc->smax_bits);
+    dtdx = dt / g.dx;
+  }
   double dm[7], q0[7], WL[7], Bn, dummy;
   {
     double qm[7], qc[7];
@@ -149,6 +159,21 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
       if (s + 1 < s1) {
 #pragma unroll
         for (int n = 0; n < 5; ++n) prefetch_l1(DIR == 1 ? a.FX[n] + c + 1 : a.R[n] + c);
+        if (APPLY) {
+#pragma unroll
+          for (int n = 0; n < 5; ++n) {
+            prefetch_l1(a.Uin[n] + c);
+            prefetch_l1(a.U0[n] + c);
+          }
+        }
+      }
+      double uin[5], u0[5];
+      if (APPLY && s > s0) {
+#pragma unroll
+        for (int n = 0; n < 5; ++n) {
+          uin[n] = a.Uin[n][cu];
+          u0[n] = a.U0[n][cu];
+        }
       }
       double r_in[5], cs_in = 0.0;
       if (s > s0) {
@@ -179,11 +204,17 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
         if (WANT_FM) a.FM[c] = F[0];
       }
       if (s > s0) {
-        a.R[0][cu] = r_in[0] + (F[0] - Fp[0]);
-        a.R[PN][cu] = r_in[PN] + (F[1] - Fp[1]);
-        a.R[PT1][cu] = r_in[PT1] + (F[2] - Fp[2]);
-        a.R[PT2][cu] = r_in[PT2] + (F[3] - Fp[3]);
-        a.R[4][cu] = r_in[4] + (F[4] - Fp[4]);
+        double rt[5];
+        rt[0] = r_in[0] + (F[0] - Fp[0]);
+        rt[PN] = r_in[PN] + (F[1] - Fp[1]);
+        rt[PT1] = r_in[PT1] + (F[2] - Fp[2]);
+        rt[PT2] = r_in[PT2] + (F[3] - Fp[3]);
+        rt[4] = r_in[4] + (F[4] - Fp[4]);
+#pragma unroll
+        for (int n = 0; n < 5; ++n) {
+          if (APPLY) a.Uout[n][cu] = 0.5 * u0[n] + 0.5 * (uin[n] - dtdx * rt[n]);  // Eq. 9, w2 = w2^0 = 1/2
+          else a.R[n][cu] = rt[n];
+        }
         if (WANT_DT) {
           const double cs = cs_in + fmax(cfp, cf);  // G8
           if (DIR == 1) a.csum[cu] = cs;

@@ -357,7 +357,8 @@ constexpr int CT_THREADS = CT_TX * CT_TY;
 #define IDFX_UNROLL(n) IDFX_PRAGMA_(unroll n)
 constexpr int CT_LX = CT_TX + 1, CT_LY = CT_TY + 1, CT_LZ = CT_TZ + 1;
 
-template <int MODE, bool STAGE2>
+// UDONE: the conserved state was already combined by the z sweep (stage 2); only read it back for the primitives.
+template <int MODE, bool STAGE2, bool UDONE>
 __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, EmfArgs ea, UpdateArgs a) {
   __shared__ double sE[3][CT_LZ][CT_LY][CT_LX];
   const int i0 = blockIdx.x * CT_TX, j0 = blockIdx.y * CT_TY, k0 = blockIdx.z * CT_TZ;
@@ -394,9 +395,13 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
     double u[5];
 #pragma unroll
     for (int n = 0; n < 5; ++n) {
-      const double us = a.Uin[n][c] - dtdx * a.R[n][c];
-      u[n] = STAGE2 ? 0.5 * a.U0[n][c] + 0.5 * us : us;
-      a.Uout[n][c] = u[n];
+      if (UDONE) {
+        u[n] = a.Uout[n][c];
+      } else {
+        const double us = a.Uin[n][c] - dtdx * a.R[n][c];
+        u[n] = STAGE2 ? 0.5 * a.U0[n][c] + 0.5 * us : us;
+        a.Uout[n][c] = u[n];
+      }
     }
     const double ex00 = sE[0][lk][lj][li], ex10 = sE[0][lk][lj + 1][li];
     const double ex01 = sE[0][lk + 1][lj][li], ex11 = sE[0][lk + 1][lj + 1][li];
@@ -677,24 +682,32 @@ void launch_dtmax(idfx_ctx* c) {
 }
 
 template <int SOLVER, int LIM, bool MHD>
-void launch_march_tma(idfx_ctx* c, int d, dim3 grid, const FluxTArgs& ta, bool want_dt, bool uct) {
+void launch_march_tma(idfx_ctx* c, int d, dim3 grid, const FluxTArgs& ta, bool want_dt, bool uct, bool apply) {
   if constexpr (MHD) {
     const Geom& g = c->g;
     if (d == 1) {
-      if (want_dt) k_flux_march_tma<SOLVER, LIM, 1, true, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
-      else if (uct) k_flux_march_tma<SOLVER, LIM, 1, false, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
-      else k_flux_march_tma<SOLVER, LIM, 1, false, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
+      if (want_dt) k_flux_march_tma<SOLVER, LIM, 1, true, true, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
+      else if (uct) k_flux_march_tma<SOLVER, LIM, 1, false, true, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
+      else k_flux_march_tma<SOLVER, LIM, 1, false, false, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
+    } else if (apply) {
+      if (uct) k_flux_march_tma<SOLVER, LIM, 2, false, true, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
+      else k_flux_march_tma<SOLVER, LIM, 2, false, false, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
     } else {
-      if (want_dt) k_flux_march_tma<SOLVER, LIM, 2, true, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
-      else if (uct) k_flux_march_tma<SOLVER, LIM, 2, false, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
-      else k_flux_march_tma<SOLVER, LIM, 2, false, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
+      if (want_dt) k_flux_march_tma<SOLVER, LIM, 2, true, true, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
+      else if (uct) k_flux_march_tma<SOLVER, LIM, 2, false, true, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
+      else k_flux_march_tma<SOLVER, LIM, 2, false, false, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
     }
   }
 }
 
 // ---- the three flux sweeps of one stage --------------------------------------------------------
+struct ApplyInfo {
+  bool on;  // stage 2 with the TMA sweeps: the z sweep applies the divergence and the RK2 combine itself
+  double dt_fixed, cfl;
+};
+
 template <int SOLVER, int LIM, bool MHD>
-void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
+void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const ApplyInfo& ap) {
   const Geom& g = c->g;
   const bool uct = c->emf == EMF_UCT;
   {  // x: faces 0..nx of every row
@@ -759,7 +772,14 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
       ta.ns = a.ns; ta.nt = a.nt; ta.chunk = a.chunk; ta.sd = a.sd; ta.st = a.st;
       for (int n = 0; n < 5; ++n) { ta.FX[n] = a.FX[n]; ta.R[n] = a.R[n]; }
       ta.cfx = a.cfx; ta.csum = a.csum; ta.FB[0] = a.FB[0]; ta.FB[1] = a.FB[1]; ta.FM = a.FM; ta.sc = a.sc;
-      launch_march_tma<SOLVER, LIM, MHD>(c, d, grid, ta, want_dt, uct);
+      for (int n = 0; n < 5; ++n) {
+        ta.Uin[n] = c->field(F_UB + n);
+        ta.U0[n] = c->field(F_UA + n);
+        ta.Uout[n] = c->field(F_UA + n);
+      }
+      ta.dt_fixed = ap.dt_fixed;
+      ta.cfl = ap.cfl;
+      launch_march_tma<SOLVER, LIM, MHD>(c, d, grid, ta, want_dt, uct, ap.on && d == 2);
       continue;
     }
     if (d == 1) {
@@ -775,25 +795,25 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
 }
 
 template <int SOLVER, bool MHD>
-void launch_sweeps_s(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
+void launch_sweeps_s(idfx_ctx* c, const double* const Bf[3], bool want_dt, const ApplyInfo& ap) {
   switch (c->limiter) {
-    case LIM_FLAT: launch_sweeps_t<SOLVER, LIM_FLAT, MHD>(c, Bf, want_dt); break;
-    case LIM_MINMOD: launch_sweeps_t<SOLVER, LIM_MINMOD, MHD>(c, Bf, want_dt); break;
-    default: launch_sweeps_t<SOLVER, LIM_VANLEER, MHD>(c, Bf, want_dt);
+    case LIM_FLAT: launch_sweeps_t<SOLVER, LIM_FLAT, MHD>(c, Bf, want_dt, ap); break;
+    case LIM_MINMOD: launch_sweeps_t<SOLVER, LIM_MINMOD, MHD>(c, Bf, want_dt, ap); break;
+    default: launch_sweeps_t<SOLVER, LIM_VANLEER, MHD>(c, Bf, want_dt, ap);
   }
 }
 
-void launch_sweeps(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
+void launch_sweeps(idfx_ctx* c, const double* const Bf[3], bool want_dt, const ApplyInfo& ap) {
   if (c->mhd) {
-    if (c->solver == SOLVER_HLL) launch_sweeps_s<SOLVER_HLL, true>(c, Bf, want_dt);
-    else if (c->solver == SOLVER_RUSANOV) launch_sweeps_s<SOLVER_RUSANOV, true>(c, Bf, want_dt);
-    else if (c->solver == SOLVER_HLLD) launch_sweeps_s<SOLVER_HLLD, true>(c, Bf, want_dt);
-    else launch_sweeps_s<SOLVER_ROE, true>(c, Bf, want_dt);
+    if (c->solver == SOLVER_HLL) launch_sweeps_s<SOLVER_HLL, true>(c, Bf, want_dt, ap);
+    else if (c->solver == SOLVER_RUSANOV) launch_sweeps_s<SOLVER_RUSANOV, true>(c, Bf, want_dt, ap);
+    else if (c->solver == SOLVER_HLLD) launch_sweeps_s<SOLVER_HLLD, true>(c, Bf, want_dt, ap);
+    else launch_sweeps_s<SOLVER_ROE, true>(c, Bf, want_dt, ap);
   } else {
-    if (c->solver == SOLVER_HLL) launch_sweeps_s<SOLVER_HLL, false>(c, Bf, want_dt);
-    else if (c->solver == SOLVER_RUSANOV) launch_sweeps_s<SOLVER_RUSANOV, false>(c, Bf, want_dt);
-    else if (c->solver == SOLVER_HLLC) launch_sweeps_s<SOLVER_HLLC, false>(c, Bf, want_dt);
-    else launch_sweeps_s<SOLVER_ROE, false>(c, Bf, want_dt);
+    if (c->solver == SOLVER_HLL) launch_sweeps_s<SOLVER_HLL, false>(c, Bf, want_dt, ap);
+    else if (c->solver == SOLVER_RUSANOV) launch_sweeps_s<SOLVER_RUSANOV, false>(c, Bf, want_dt, ap);
+    else if (c->solver == SOLVER_HLLC) launch_sweeps_s<SOLVER_HLLC, false>(c, Bf, want_dt, ap);
+    else launch_sweeps_s<SOLVER_ROE, false>(c, Bf, want_dt, ap);
   }
 }
 
@@ -821,11 +841,19 @@ void launch_fill(idfx_ctx* c, int which_b) {
   k_fill_ghost<<<blocks_for(nt, 128), 128, 0, c->stream>>>(g, fl);
 }
 
+template <int MODE>
+void launch_ct(idfx_ctx* c, dim3 grid, const EmfArgs& ea, const UpdateArgs& a, bool stage2, bool udone) {
+  if (udone) k_ct_update<MODE, true, true><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
+  else if (stage2) k_ct_update<MODE, true, false><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
+  else k_ct_update<MODE, false, false><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
+}
+
 // One stage S_dt (O2) followed by the RK combine.  bin: face buffer of the stage input; b0: saved face
 // buffer; bout: destination.
 void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fixed, double cfl, bool want_dt) {
   const double* Bf[3] = {c->bbuf(bin, 0), c->bbuf(bin, 1), c->bbuf(bin, 2)};
-  launch_sweeps(c, Bf, want_dt);
+  const ApplyInfo ap = {stage2 && c->mhd && c->use_tma, dt_fixed, cfl};
+  launch_sweeps(c, Bf, want_dt, ap);
   UpdateArgs a;
   for (int n = 0; n < 5; ++n) {
     a.Uin[n] = c->field((stage2 ? F_UB : F_UA) + n);
@@ -848,17 +876,11 @@ void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fi
     const EmfArgs ea = emf_args(c);
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield_out(n);
     dim3 grid((g.nx + CT_TX - 1) / CT_TX, (g.ny + CT_TY - 1) / CT_TY, (g.nz + CT_TZ - 1) / CT_TZ);
+    const bool udone = stage2 && c->use_tma;  // the TMA z sweep of stage 2 applied the divergence itself
     LaunchScope ls(c, K_UPDATE);
-    if (c->emf == EMF_UCT) {
-      if (stage2) k_ct_update<EMF_UCT, true><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
-      else k_ct_update<EMF_UCT, false><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
-    } else if (c->emf == EMF_UCT0) {
-      if (stage2) k_ct_update<EMF_UCT0, true><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
-      else k_ct_update<EMF_UCT0, false><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
-    } else {
-      if (stage2) k_ct_update<EMF_ARITH, true><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
-      else k_ct_update<EMF_ARITH, false><<<grid, CT_THREADS, 0, c->stream>>>(g, ea, a);
-    }
+    if (c->emf == EMF_UCT) launch_ct<EMF_UCT>(c, grid, ea, a, stage2, udone);
+    else if (c->emf == EMF_UCT0) launch_ct<EMF_UCT0>(c, grid, ea, a, stage2, udone);
+    else launch_ct<EMF_ARITH>(c, grid, ea, a, stage2, udone);
     c->vcur ^= 1;
   } else {
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield(n);
