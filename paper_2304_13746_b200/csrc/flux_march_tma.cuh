@@ -237,4 +237,96 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// x sweep with TMA-staged rows.  A CTA owns a window of 31 x-faces (cells f0-1 .. f0+30, one lane each, plus one halo
+// cell on either side) of four consecutive rows (one warp per row) and marches over z planes; per plane two boxes
+// (36 columns x 4 rows x 8 primitive fields, and the B_x faces) land in a 4-stage ring.  Lanes read their three-cell
+// stencil from shared memory, so no edge loads and no shuffles of the primitives are needed; only the left face state
+// comes from the neighbouring lane by shuffle.  Lanes 1..31 solve the left face of their cell.
+// ---------------------------------------------------------------------------------------------
+constexpr int TX_NST = 4, TX_SLACK = 1;
+constexpr int TX_W = 36;
+constexpr int TX_PLANE_V = 8 * 4 * TX_W;
+constexpr int TX_PLANE = TX_PLANE_V + 4 * TX_W;
+constexpr uint32_t TX_PLANE_BYTES = TX_PLANE * 8;
+
+struct FluxXTArgs {
+  int fV0, fB;   // first primitive field inside the V tensor map; field of B_x inside the B tensor map
+  int chunk;     // z planes per CTA
+  double* FH[5];
+  double* FB[2];
+  double* cf;
+};
+
+template <int SOLVER, int LIM>
+__global__ void __launch_bounds__(128, 4) k_flux_x_tma(Geom g, FluxXTArgs a, const __grid_constant__ CUtensorMap mapV,
+                                                       const __grid_constant__ CUtensorMap mapB) {
+  __shared__ alignas(128) double ring[TX_NST][TX_PLANE];
+  __shared__ uint64_t full[TX_NST], empty[TX_NST];
+  constexpr int FQ[7] = {0, 1, 2, 3, 4, 6, 7};  // rho, vx, vy, vz, p, Bc_y, Bc_z
+  const int lane = threadIdx.x & 31, row = threadIdx.x >> 5;
+  const int f0 = 31 * blockIdx.x;
+  const int ci = f0 - 1 + lane;
+  const int j = blockIdx.y * 4 + row;
+  const int k0 = blockIdx.z * a.chunk;
+  const int np = min(k0 + a.chunk, g.nz) - k0;
+  const bool solve = lane >= 1 && ci <= g.nx && j < g.ny;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int st = 0; st < TX_NST; ++st) {
+      mbar_init(&full[st], 1);
+      mbar_init(&empty[st], 128);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+  // TMA needs the box to start on a 16-byte boundary: shift odd windows one column left (36 >= 34 + 1 columns)
+  const int sh = f0 & 1;
+  const int cx = IOFF + f0 - 2 - sh, cy = NG + blockIdx.y * 4, cz0 = NG + k0;
+  auto issue = [&](int p) {
+    uint64_t* bar = &full[p % TX_NST];
+    double* dst = ring[p % TX_NST];
+    mbar_expect_tx(bar, TX_PLANE_BYTES);
+    tma_load_4d(dst, &mapV, bar, cx, cy, cz0 + p, a.fV0);
+    tma_load_4d(dst + TX_PLANE_V, &mapB, bar, cx, cy, cz0 + p, a.fB);
+  };
+  if (threadIdx.x == 0)
+    for (int p = 0; p < min(np, TX_NST); ++p) issue(p);
+  const int so = row * TX_W + lane + sh;  // stencil cells ci-1, ci, ci+1 sit at so, so+1, so+2
+  long long c = g.at(min(ci, g.nx + 1), min(j, g.ny - 1), k0);
+  for (int p = 0; p < np; ++p, c += g.sz) {
+    const int st = p % TX_NST;
+    mbar_wait(&full[st], (p / TX_NST) & 1);
+    const double* r = ring[st];
+    double WL[7], WR[7];
+#pragma unroll
+    for (int n = 0; n < 7; ++n) {
+      const double* f = r + FQ[n] * (4 * TX_W) + so;
+      const double qm = f[0], q = f[1], qp = f[2];
+      const double sl = limited_slope<LIM>(q - qm, qp - q);
+      WR[n] = q - 0.5 * sl;
+      WL[n] = __shfl_up_sync(0xffffffffu, q + 0.5 * sl, 1);
+    }
+    const double Bn = r[TX_PLANE_V + so + 1];
+    mbar_arrive(&empty[st]);
+    if (threadIdx.x == 0) {
+      const int pr = p - TX_SLACK;
+      if (pr >= 0 && pr + TX_NST < np) {
+        mbar_wait(&empty[pr % TX_NST], (pr / TX_NST) & 1);
+        issue(pr + TX_NST);
+      }
+    }
+    if (solve) {
+      double F[7];
+      const double cface = riemann<SOLVER, true>(WL, WR, Bn, g.gamma, F);
+#pragma unroll
+      for (int n = 0; n < 5; ++n) a.FH[n][c] = F[n];
+      a.FB[0][c] = F[5];
+      a.FB[1][c] = F[6];
+      a.cf[c] = cface;
+    }
+  }
+}
+
 }  // namespace idfx

@@ -599,15 +599,18 @@ int make_tensor_maps(idfx_ctx* c) {
   const cuuint64_t py = g.ny + 2 * NG, pz = g.nz + 2 * NG;
   const cuuint64_t strides[3] = {(cuuint64_t)g.sy * 8, (cuuint64_t)g.sz * 8, (cuuint64_t)g.np * 8};
   const cuuint32_t es[4] = {1, 1, 1, 1};
-  for (int d = 1; d < 3; ++d) {
+  for (int d = 0; d < 3; ++d) {
     const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, 22}, dimB[4] = {(cuuint64_t)g.sy, py, pz, 9};
-    const cuuint32_t boxV[4] = {32, d == 1 ? 1u : 4u, d == 1 ? 4u : 1u, 8};
-    const cuuint32_t boxB[4] = {32, d == 1 ? 1u : 4u, d == 1 ? 4u : 1u, 1};
+    // x sweep: 36 columns x 4 rows of one z plane; y sweep: 32 x 1 x 4; z sweep: 32 x 4 x 1
+    const cuuint32_t bx = d == 0 ? (cuuint32_t)TX_W : 32u, by = d == 1 ? 1u : 4u, bz = d == 1 ? 4u : 1u;
+    const cuuint32_t boxV[4] = {bx, by, bz, 8};
+    const cuuint32_t boxB[4] = {bx, by, bz, 1};
+    const CUtensorMapL2promotion promo = d == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE : CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
     CUresult r1 = enc(&c->mapV[d], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_V), dimV, strides, boxV, es,
-                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     CUresult r2 = enc(&c->mapB[d], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_BA), dimB, strides, boxB, es,
-                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r1 != CUDA_SUCCESS || r2 != CUDA_SUCCESS) {
       set_err("cuTensorMapEncodeTiled failed");
@@ -682,6 +685,11 @@ void launch_dtmax(idfx_ctx* c) {
 }
 
 template <int SOLVER, int LIM, bool MHD>
+void launch_x_tma(idfx_ctx* c, dim3 grid, const FluxXTArgs& ta) {
+  if constexpr (MHD) k_flux_x_tma<SOLVER, LIM><<<grid, 128, 0, c->stream>>>(c->g, ta, c->mapV[0], c->mapB[0]);
+}
+
+template <int SOLVER, int LIM, bool MHD>
 void launch_march_tma(idfx_ctx* c, int d, dim3 grid, const FluxTArgs& ta, bool want_dt, bool uct, bool apply) {
   if constexpr (MHD) {
     const Geom& g = c->g;
@@ -731,7 +739,24 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const
     a.rows_per_warp = (int)rpw;
     dim3 grid(gx, (unsigned)((nrows + 4 * rpw - 1) / (4 * rpw)));
     LaunchScope ls(c, K_FLUX_X);
-    k_flux_x<SOLVER, LIM, MHD><<<grid, 128, 0, c->stream>>>(g, a);
+    if (MHD && c->use_tma) {
+      FluxXTArgs ta;
+      ta.fV0 = c->vcur ? 11 : 0;
+      ta.fB = (int)((Bf[0] - c->field(F_BA)) / g.np);
+      for (int n = 0; n < 5; ++n) ta.FH[n] = a.FH[n];
+      ta.FB[0] = a.FB[0];
+      ta.FB[1] = a.FB[1];
+      ta.cf = a.cf;
+      const long long per_chunk = (long long)gx * ((g.ny + 3) / 4);
+      long long nch = (148 * 16 + per_chunk - 1) / per_chunk;
+      const long long maxch = g.nz / 8 > 0 ? g.nz / 8 : 1;
+      nch = nch < 1 ? 1 : (nch > maxch ? maxch : nch);
+      ta.chunk = (int)((g.nz + nch - 1) / nch);
+      dim3 tgrid(gx, (g.ny + 3) / 4, (unsigned)((g.nz + ta.chunk - 1) / ta.chunk));
+      launch_x_tma<SOLVER, LIM, MHD>(c, tgrid, ta);
+    } else {
+      k_flux_x<SOLVER, LIM, MHD><<<grid, 128, 0, c->stream>>>(g, a);
+    }
   }
   for (int d = 1; d < 3; ++d) {  // y then z: marching pencils
     const int ib = (d + 1) % 3, ie = (d + 2) % 3;
