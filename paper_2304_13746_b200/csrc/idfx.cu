@@ -739,7 +739,9 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const
     a.rows_per_warp = (int)rpw;
     dim3 grid(gx, (unsigned)((nrows + 4 * rpw - 1) / (4 * rpw)));
     LaunchScope ls(c, K_FLUX_X);
-    if (MHD && c->use_tma) {
+    // Measured: the TMA rows win up to 256^3 (0.64 vs 0.69 ms), but at 512^3 their 36-column boxes for 31 faces cost
+    // 23 GB instead of 18 GB of DRAM traffic per launch and lose (5.6 vs 4.9 ms under ncu): long rows use the shuffle kernel.
+    if (MHD && c->use_tma && g.nx <= 384) {
       FluxXTArgs ta;
       ta.fV0 = c->vcur ? 11 : 0;
       ta.fB = (int)((Bf[0] - c->field(F_BA)) / g.np);
