@@ -39,7 +39,7 @@ ALGO_BYTES_PER_CELL = {"flux_x": 8 * 16.0, "flux_y": 8 * 21.0, "flux_z": 8 * 26.
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (mean of the stage-1 and stage-2 launch) from the committed
 # ncu --set full capture of this command at 512^3 (profiles/r01_ncu_full_512.md); only valid for that workload
-NCU_TRAFFIC_BYTES_512 = {"flux_x": 17.81e9, "flux_y": 25.72e9, "flux_z": 24.91e9, "ct_update_prim": 56.86e9}
+NCU_TRAFFIC_BYTES_512 = {"flux_x": 17.81e9, "flux_y": 25.70e9, "flux_z": 31.44e9, "ct_update_prim": 50.04e9}
 
 
 def parse_args():
