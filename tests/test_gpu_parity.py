@@ -243,3 +243,28 @@ def test_minimum_size_box(idfx, R):
     sim.advance(3, 0.3)
     ref.advance(3, 0.3)
     assert_state_close(sim, ref, TOL)
+
+
+def test_alternate_code_paths_in_a_subprocess(idfx):
+    """IDFX_TMA=0 (register-prefetch sweeps + separate R path in stage 2) and IDFX_GRAPH=0 (no CUDA-graph replay) are
+    A/B switches read at idfx_bind; run one MHD parity case under each in a fresh process."""
+    import os
+    import subprocess
+    import sys
+    code = (
+        "import sys, numpy as np, torch\n"
+        "sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+        "from oracle import idfxref as R\n"
+        "from paper_2304_13746_b200 import idfx\n"
+        "import test_gpu_parity as T\n"
+        "prim, b, dx = T.smooth_ic(37, 21, 13, 11)\n"
+        "sim, ref = T.make_pair(idfx, R, 37, 21, 13, dx, 5.0 / 3.0, T.HLLD, T.VANLEER, T.EMF_UCT, prim, b)\n"
+        "sim.advance(3, 0.4); ref.advance(3, 0.4)\n"
+        "T.assert_state_close(sim, ref, T.TOL)\n"
+        "assert abs(sim.last_dt() - ref.last_dt()) <= T.TOL_DT * ref.last_dt()\n"
+        "print('ok')\n"
+    ) % (os.path.dirname(os.path.dirname(os.path.abspath(__file__))), os.path.dirname(os.path.abspath(__file__)))
+    for env_add in ({"IDFX_TMA": "0"}, {"IDFX_GRAPH": "0"}, {"IDFX_TMA": "0", "IDFX_GRAPH": "0"}):
+        p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300,
+                           env=dict(os.environ, **env_add))
+        assert p.returncode == 0 and "ok" in p.stdout, (env_add, p.stderr[-2000:])
