@@ -30,11 +30,11 @@ ALGO_BYTES_PER_CELL_UPDATE = 320.0          # 40 doubles per M
 # Algorithmic work per cell per launch of each kernel class.
 # Sweeps: one PLM + HLLD face solve = 360 flops (+, -, x, /, sqrt counted once each in O3-O7, one E*, one U**).
 ALGO_FLOPS_PER_CELL = {"flux_x": 360.0, "flux_y": 360.0, "flux_z": 360.0}
-# Compulsory doubles read + written per cell (MHD, E^c): x: V7+Bn | Fx5 FB2 cf1; y: V7+Bn+Fx5 | R5 FB2 FM1;
-# z stage 1: V7+Bn+R5 | R5 FB2 FM1 (21), stage 2 also applies the RK2 combine: + U1 5 + U0 5 | U5 instead of R5 (31);
-# fused CT/update stage 1: R5 U0 5 Bin3 FB6 FM3 Ec3 | U5 B3 V11 (44), stage 2: U5 Bin3 B0 3 FB6 FM3 Ec3 | B3 V11 (37).
-# Values are the means over the two stages.
-ALGO_BYTES_PER_CELL = {"flux_x": 8 * 16.0, "flux_y": 8 * 21.0, "flux_z": 8 * 26.0, "ct_update_prim": 8 * 40.5}
+# Compulsory doubles read + written per cell (MHD, E^c; sg = 1-byte sign of the face mass flux):
+# x: V7+Bn | Fx5 FB2 cf1 sg; y: V7+Bn+Fx5 | R5 FB2 sg; z stage 1: V7+Bn+R5 | R5 FB2 sg (20 1/8), stage 2 also applies the
+# RK2 combine: + U1 5 + U0 5 | U5 instead of R5 (30 1/8); fused CT/update stage 1: R5 U0 5 Bin3 FB6 sg3 Ec3 | U5 B3 V11
+# (41 3/8), stage 2: U5 Bin3 B0 3 FB6 sg3 Ec3 | B3 V11 (34 3/8).  Values are the means over the two stages.
+ALGO_BYTES_PER_CELL = {"flux_x": 8 * 16.125, "flux_y": 8 * 20.125, "flux_z": 8 * 25.125, "ct_update_prim": 8 * 37.875}
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (mean of the stage-1 and stage-2 launch) from the committed

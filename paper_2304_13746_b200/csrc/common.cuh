@@ -38,6 +38,9 @@ struct DevScalars {
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
+// sign of a face mass flux as one byte (+1, -1, 0): all the upwind-contact EMF needs of it (G10)
+__device__ __forceinline__ signed char flux_sign(double f) { return f > 0.0 ? 1 : (f < 0.0 ? -1 : 0); }
+
 // block-wide maximum for blocks of exactly 128 threads; every thread must call it
 __device__ __forceinline__ double block_max_128(double v) {
   __shared__ double red[4];

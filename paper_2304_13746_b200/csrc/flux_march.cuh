@@ -15,7 +15,7 @@
 #include "physics.cuh"
 
 #ifndef IDFX_MINB_X
-#define IDFX_MINB_X 2
+#define IDFX_MINB_X 3
 #endif
 #ifndef IDFX_MINB_M
 #define IDFX_MINB_M 2
@@ -32,6 +32,7 @@ struct FluxXArgs {
   double* FH[5];       // F_x of (rho, mx, my, mz, E) on faces 0..nx (face nx is written too)
   double* FB[2];       // F_x[B_y], F_x[B_z]
   double* cf;          // c_face
+  signed char* sg;     // sign of the mass flux (upwind-contact EMF only, else null)
   int rows_per_warp;
 };
 
@@ -96,6 +97,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a
         a.FB[1][c] = F[6];
       }
       a.cf[c] = cface;
+      if (a.sg) a.sg[c] = flux_sign(F[0]);
     }
   }
 }
@@ -111,7 +113,7 @@ struct FluxMArgs {
   double* R[5];         // flux divergence, global ordering (rho, mx, my, mz, E)
   double* csum;         // sum_d c_d of the cell, accumulated over x and y
   double* FB[2];        // face fluxes of B_t1, B_t2
-  double* FM;           // face mass flux (upwind-contact EMF only)
+  signed char* SG;      // sign of the face mass flux (upwind-contact EMF only)
   DevScalars* sc;
 };
 
@@ -190,7 +192,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_M) k_flux_march(Geom g, FluxMAr
       if (s < s1 && MHD) {  // faces s0..s1-1 belong to this chunk
         a.FB[0][c] = F[5];
         a.FB[1][c] = F[6];
-        if (WANT_FM) a.FM[c] = F[0];
+        if (WANT_FM) a.SG[c] = flux_sign(F[0]);
       }
       if (s > s0) {
         a.R[0][cu] = r_in[0] + (F[0] - Fp[0]);

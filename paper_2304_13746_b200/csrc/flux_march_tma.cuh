@@ -62,7 +62,7 @@ struct FluxTArgs {
   double* R[5];
   double* csum;
   double* FB[2];
-  double* FM;
+  signed char* SG;      // sign of the face mass flux (upwind-contact EMF only)
   DevScalars* sc;
   // APPLY (stage 2 of the z sweep): the completed divergence is applied at once, U = U0/2 + (U1 - dt/dx R)/2
   const double* Uin[5];
@@ -201,7 +201,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
       if (s < s1) {  // faces s0..s1-1 belong to this chunk
         a.FB[0][c] = F[5];
         a.FB[1][c] = F[6];
-        if (WANT_FM) a.FM[c] = F[0];
+        if (WANT_FM) a.SG[c] = flux_sign(F[0]);
       }
       if (s > s0) {
         double rt[5];
@@ -256,6 +256,7 @@ struct FluxXTArgs {
   double* FH[5];
   double* FB[2];
   double* cf;
+  signed char* sg;  // sign of the mass flux (upwind-contact EMF only, else null)
 };
 
 template <int SOLVER, int LIM>
@@ -325,6 +326,7 @@ __global__ void __launch_bounds__(128, 4) k_flux_x_tma(Geom g, FluxXTArgs a, con
       a.FB[0][c] = F[5];
       a.FB[1][c] = F[6];
       a.cf[c] = cface;
+      if (a.sg) a.sg[c] = flux_sign(F[0]);
     }
   }
 }

@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(128) k_rhs(Geom g, RhsArgs a) {
 // ---------------------------------------------------------------------------------------------
 struct EmfArgs {
   const double* FB[3][2];  // FB[d][0] = F_d[B_t1], FB[d][1] = F_d[B_t2] on the left d-faces
-  const double* FM[3];     // mass flux F_d[rho]
+  const signed char* SG[3];  // sign of the mass flux F_d[rho] on the left d-faces
   const double* Ec[3];     // cell-centred reference EMF -(v x Bc) of the stage input, with ghosts (G10)
 };
 
@@ -276,18 +276,18 @@ __device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& a, cons
       // cell-centred reference EMF of the stage input (G10), stored with ghosts next to the primitives
       const double* __restrict__ Ecc = a.Ec[c];
       const double Ec = Ecc[P], Eca = Ecc[P - st[ia]], Ecb = Ecc[P - st[ib]], Ecab = Ecc[P - st[ia] - st[ib]];
-      const double fa = a.FM[ia][P], fab = a.FM[ia][P + db];  // mass flux through the two a-faces
-      const double fb = a.FM[ib][P], fba = a.FM[ib][P + da];  // and the two b-faces
+      const int fa = a.SG[ia][P], fab = a.SG[ia][P + db];  // sign of the mass flux through the two a-faces
+      const int fb = a.SG[ib][P], fba = a.SG[ib][P + da];  // and the two b-faces
       // d/db on the a-face, quarter points ib-1/4 (cells P-a | P) and ib-3/4 (cells P-a-b | P-b)
       const double gbp_m = 2.0 * (Eca - EbPa), gbp_p = 2.0 * (Ec - EbP);
       const double gbm_m = 2.0 * (EbPa - Ecab), gbm_p = 2.0 * (EbP - Ecb);
-      const double Gb1 = fa > 0.0 ? gbp_m : (fa < 0.0 ? gbp_p : 0.5 * (gbp_m + gbp_p));
-      const double Gb3 = fab > 0.0 ? gbm_m : (fab < 0.0 ? gbm_p : 0.5 * (gbm_m + gbm_p));
+      const double Gb1 = fa > 0 ? gbp_m : (fa < 0 ? gbp_p : 0.5 * (gbp_m + gbp_p));
+      const double Gb3 = fab > 0 ? gbm_m : (fab < 0 ? gbm_p : 0.5 * (gbm_m + gbm_p));
       // d/da on the b-face, quarter points ia-1/4 (cells P-b | P) and ia-3/4 (cells P-a-b | P-a)
       const double gap_m = 2.0 * (Ecb - EaPb), gap_p = 2.0 * (Ec - EaP);
       const double gam_m = 2.0 * (EaPb - Ecab), gam_p = 2.0 * (EaP - Eca);
-      const double Ga1 = fb > 0.0 ? gap_m : (fb < 0.0 ? gap_p : 0.5 * (gap_m + gap_p));
-      const double Ga3 = fba > 0.0 ? gam_m : (fba < 0.0 ? gam_p : 0.5 * (gam_m + gam_p));
+      const double Ga1 = fb > 0 ? gap_m : (fb < 0 ? gap_p : 0.5 * (gap_m + gap_p));
+      const double Ga3 = fba > 0 ? gam_m : (fba < 0 ? gam_p : 0.5 * (gam_m + gam_p));
       e += 0.125 * (Gb3 - Gb1) + 0.125 * (Ga3 - Ga1);
     }
     return e;
@@ -475,9 +475,9 @@ enum {
   F_FB = 46,   // 6: face fluxes of B, [d][0..1]
   F_FX = 52,   // 5: x-face fluxes of (rho, m, E); F_FX+0 doubles as the x mass flux
   F_CFX = 57,  // 1: c_face of the x sweep
-  F_FM = 58,   // 3: face mass fluxes of the y, z sweeps at +1, +2 (slot +0 unused)
-  F_CS = 61,   // 1: sum_d c_d per cell (x and y parts)
-  F_COUNT = 62
+  F_SG = 58,   // 1 slot holding three byte fields: sign of the face mass flux of the x, y, z sweeps (E^c only)
+  F_CS = 59,   // 1: sum_d c_d per cell (x and y parts)
+  F_COUNT = 60
 };
 
 }  // namespace idfx
@@ -517,6 +517,7 @@ struct idfx_ctx {
   long long prof_n[K_COUNT] = {0};
   double* field(int slot) const { return ws + (size_t)slot * (size_t)g.np; }
   double* bbuf(int which, int d) const { return field(F_BA + 3 * which + d); }
+  signed char* sgn(int d) const { return (signed char*)field(F_SG) + (size_t)d * (size_t)g.np; }
   double* vfield(int n) const { return field((vcur ? F_V2 : F_V) + n); }
   double* vfield_out(int n) const { return field((vcur ? F_V : F_V2) + n); }
 };
@@ -732,6 +733,7 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const
     a.FB[0] = c->field(F_FB + 0);
     a.FB[1] = c->field(F_FB + 1);
     a.cf = c->field(F_CFX);
+    a.sg = uct ? c->sgn(0) : nullptr;
     const int gx = (g.nx + 1 + 30) / 31;
     const long long nrows = (long long)g.ny * g.nz;
     long long rpw = gx * nrows / 9472;
@@ -749,6 +751,7 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const
       ta.FB[0] = a.FB[0];
       ta.FB[1] = a.FB[1];
       ta.cf = a.cf;
+      ta.sg = a.sg;
       const long long per_chunk = (long long)gx * ((g.ny + 3) / 4);
       long long nch = (148 * 16 + per_chunk - 1) / per_chunk;
       const long long maxch = g.nz / 8 > 0 ? g.nz / 8 : 1;
@@ -783,7 +786,7 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const
     a.csum = c->field(F_CS);
     a.FB[0] = c->field(F_FB + 2 * d);
     a.FB[1] = c->field(F_FB + 2 * d + 1);
-    a.FM = c->field(F_FM + d);
+    a.SG = c->sgn(d);
     a.sc = c->sc;
     const long long per_chunk = (long long)((g.nx + 31) / 32) * ((a.nt + 3) / 4);
     long long nch = (148 * 16 + per_chunk - 1) / per_chunk;
@@ -798,7 +801,7 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const
       ta.fB = (int)((Bf[d] - c->field(F_BA)) / g.np);
       ta.ns = a.ns; ta.nt = a.nt; ta.chunk = a.chunk; ta.sd = a.sd; ta.st = a.st;
       for (int n = 0; n < 5; ++n) { ta.FX[n] = a.FX[n]; ta.R[n] = a.R[n]; }
-      ta.cfx = a.cfx; ta.csum = a.csum; ta.FB[0] = a.FB[0]; ta.FB[1] = a.FB[1]; ta.FM = a.FM; ta.sc = a.sc;
+      ta.cfx = a.cfx; ta.csum = a.csum; ta.FB[0] = a.FB[0]; ta.FB[1] = a.FB[1]; ta.SG = a.SG; ta.sc = a.sc;
       for (int n = 0; n < 5; ++n) {
         ta.Uin[n] = c->field(F_UB + n);
         ta.U0[n] = c->field(F_UA + n);
@@ -849,7 +852,7 @@ EmfArgs emf_args(idfx_ctx* c) {
   for (int d = 0; d < 3; ++d) {
     a.FB[d][0] = c->field(F_FB + 2 * d);
     a.FB[d][1] = c->field(F_FB + 2 * d + 1);
-    a.FM[d] = d == 0 ? c->field(F_FX) : c->field(F_FM + d);
+    a.SG[d] = c->sgn(d);
     a.Ec[d] = c->vfield(8 + d);
   }
   return a;
