@@ -31,7 +31,7 @@ struct FluxXArgs {
   const double* bn;    // B_x on x-faces
   double* FH[5];       // F_x of (rho, mx, my, mz, E) on faces 0..nx (face nx is written too)
   double* FB[2];       // F_x[B_y], F_x[B_z]
-  double* cf;          // c_face
+  double* cf;          // c_face (stage 1 only, else null)
   signed char* sg;     // sign of the mass flux (upwind-contact EMF only, else null)
   int rows_per_warp;
 };
@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a
         a.FB[0][c] = F[5];
         a.FB[1][c] = F[6];
       }
-      a.cf[c] = cface;
+      if (a.cf) a.cf[c] = cface;  // only the dt evaluation of stage 1 reads it
       if (a.sg) a.sg[c] = flux_sign(F[0]);
     }
   }

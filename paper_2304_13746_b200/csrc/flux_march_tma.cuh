@@ -325,7 +325,7 @@ __global__ void __launch_bounds__(128, 4) k_flux_x_tma(Geom g, FluxXTArgs a, con
       for (int n = 0; n < 5; ++n) a.FH[n][c] = F[n];
       a.FB[0][c] = F[5];
       a.FB[1][c] = F[6];
-      a.cf[c] = cface;
+      if (a.cf) a.cf[c] = cface;  // only the dt evaluation of stage 1 reads it
       if (a.sg) a.sg[c] = flux_sign(F[0]);
     }
   }

@@ -732,7 +732,7 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const
     for (int n = 0; n < 5; ++n) a.FH[n] = c->field(F_FX + n);
     a.FB[0] = c->field(F_FB + 0);
     a.FB[1] = c->field(F_FB + 1);
-    a.cf = c->field(F_CFX);
+    a.cf = want_dt ? c->field(F_CFX) : nullptr;
     a.sg = uct ? c->sgn(0) : nullptr;
     const int gx = (g.nx + 1 + 30) / 31;
     const long long nrows = (long long)g.ny * g.nz;
