@@ -345,7 +345,12 @@ __global__ void __launch_bounds__(128) k_update_hd(Geom g, UpdateArgs a) {
 // edges read from shared memory, so the edge EMFs never travel to HBM; the result's ghost images (V and the new
 // face field) are written by the owners of the boundary cells, which replaces the separate ghost-fill pass.
 // ---------------------------------------------------------------------------------------------
-constexpr int CT_TX = 32, CT_TY = 4, CT_TZ = 4;  // 32x8x4 and 32x8x8 tiles measured the same
+#ifndef IDFX_CT_TX
+#define IDFX_CT_TX 32
+#define IDFX_CT_TY 4
+#define IDFX_CT_TZ 4
+#endif
+constexpr int CT_TX = IDFX_CT_TX, CT_TY = IDFX_CT_TY, CT_TZ = IDFX_CT_TZ;
 constexpr int CT_THREADS = CT_TX * CT_TY;
 #ifndef IDFX_MINB_CT
 #define IDFX_MINB_CT 8
