@@ -4,8 +4,9 @@
 // cpu_baseline / --impl reference legs may build, load or call anything in this directory.
 // The CUDA path (paper_2304_13746_b200/) shares no source, header, table or helper with it.
 //
-// What it is: a plain, slow, single-threaded fp64 CPU implementation of one RK2 cycle of the
-// second-order Godunov finite-volume scheme of IDEFIX (Lesur et al., arXiv 2304.13746) for
+// What it is: a plain, slow, single-threaded fp64 CPU implementation of one explicit cycle (RK2 by default;
+// Euler and RK3 of Tab. 1 as options) of the
+// Godunov finite-volume scheme of IDEFIX (Lesur et al., arXiv 2304.13746) for
 // compressible HD and ideal MHD on a uniform periodic 3D Cartesian grid, written step by step in the
 // paper's order.  Citations "PAPER.md:<line>" refer to /root/reference/PAPER.md; "O<n>" / "G<n>" refer
 // to SURVEY.md §8(c) (the written-out formulas and the readings of points the paper leaves open;
@@ -16,11 +17,14 @@
 // L·R=I, A·r=λr against a finite-difference Jacobian, Σλαr = F_R−F_L; MHD-Roe(B=0) = 5-wave HD Roe;
 // Rusanov = HLL with symmetric speeds; limiter properties; exact Sod solution along x, y, z; direction symmetry; uniform state; conservation;
 // div B; Eᶜ plane-parallel identity; RK2 amplification factor; closed-form dt; 2nd-order convergence of
-// linear fast/Alfvén waves.
+// linear fast/Alfvén waves.  Options (tests/test_oracle_options.py): Euler/RK2/RK3 amplification polynomials and temporal
+// order; LimO3 exact for parabolas, bounded at jumps, 3rd-order linear-wave convergence with RK3; vector-potential CT
+// equal to face CT up to rounding with div B that does not accumulate; advance_to lands on t_end.
 // PARITY UNPINNED (the paper fixes none of these and prints no number that depends on them, see
 // DESIGN.md "Readings"): the limiter flavour (G2), the Davis wave-speed estimate (G5), the HLLD
 // degeneracy threshold (G6), the Roe fallback/degenerate-eigenvector conventions (G7), the face→cell
-// mapping of c_max in dt (G8), un-lagged dt (G9) and the reference E^c state (G10).
+// mapping of c_max in dt (G8), un-lagged dt (G9), the reference E^c state (G10), and the LimO3 constants
+// (1.6, r = 1, eps = 1e-12; G18: PAPER.md:79 only names the scheme of Cada & Torrilhon 2009).
 //
 // Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC idfxref.cpp -o libidfxref.so
 #include <algorithm>
@@ -36,7 +40,9 @@ namespace {
 constexpr int NG = 2;  // ghost layers: PLM needs 2 ("number of ghost cells ... adjusted")
 
 enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_RUSANOV = 4 };
-enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2 };
+enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3 };
+enum { OPT_INTEGRATOR = 0, OPT_CT_FORM = 1 };  // idfxref_set_option
+enum { CT_FACE = 0, CT_POTENTIAL = 1 };
 enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3 };
 enum { OK = 0, ERR_INVALID_ARG = -1, ERR_UNSUPPORTED = -2, ERR_UNPHYSICAL = -5 };
 
@@ -473,6 +479,41 @@ double slope(int limiter, double dm, double dp) {
   return s * std::min(std::fabs(dm), std::fabs(dp));
 }
 
+// LimO3 ("LimO3 (Cada & Torrilhon 2009)"; reading G18).  With d- = q_i - q_{i-1},
+// d+ = q_{i+1} - q_i and theta = d-/d+, the value at the upper face of cell i is q_i + phi(theta) d+ / 2, where the
+// unlimited third-order weight is phi^(theta) = (2 + theta)/3 (exact for cell averages of a parabola) and the limited
+// one phi_O3 = max(0, min(phi^, max(-theta/2, min(2 theta, phi^, 1.6)))).  The limiter is switched off where the data
+// are smooth: eta = (d-^2 + d+^2)/(r dx)^2 with r = 1; eta <= 1 - eps -> phi^, eta >= 1 + eps -> phi_O3, linear blend
+// in between, eps = 1e-12.  The lower face is the mirror image (d- and d+ exchanged, sign flipped).
+// Returns phi(theta) * dplus, the full increment; the face value is q + half of it.
+double limo3_increment(double dminus, double dplus, double dx) {
+  const double eps = 1e-12, r = 1.0;
+  const double unlimited = (2.0 * dplus + dminus) / 3.0;  // phi^(theta) d+
+  double limited = 0.0;
+  if (dplus != 0.0) {
+    const double theta = dminus / dplus;
+    const double phat = (2.0 + theta) / 3.0;
+    const double phi = std::max(0.0, std::min(phat, std::max(-0.5 * theta, std::min(std::min(2.0 * theta, phat), 1.6))));
+    limited = phi * dplus;
+  }
+  const double eta = (dminus * dminus + dplus * dplus) / ((r * dx) * (r * dx));
+  if (eta <= 1.0 - eps) return unlimited;
+  if (eta >= 1.0 + eps) return limited;
+  return 0.5 * ((1.0 - (eta - 1.0) / eps) * unlimited + (1.0 + (eta - 1.0) / eps) * limited);
+}
+
+// S2: values of the reconstruction of cell i at its lower and upper faces from (q_{i-1}, q_i, q_{i+1}).
+void reconstruct(int limiter, double qm, double q0, double qp, double dx, double& lower, double& upper) {
+  if (limiter == LIM_LIMO3) {
+    upper = q0 + 0.5 * limo3_increment(q0 - qm, qp - q0, dx);
+    lower = q0 - 0.5 * limo3_increment(qp - q0, q0 - qm, dx);
+    return;
+  }
+  const double s = slope(limiter, q0 - qm, qp - q0);
+  lower = q0 - 0.5 * s;
+  upper = q0 + 0.5 * s;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Grid-level scheme
 // ---------------------------------------------------------------------------------------------
@@ -492,6 +533,11 @@ struct Ctx {
   Arr F[3][7];                      // face fluxes per direction in that direction's local ordering
   Arr cf[3];                        // c_face per direction
   Arr E[3];                         // edge EMFs: E[0] at (i, j-1/2, k-1/2), E[1] at (i-1/2, j, k-1/2), E[2] at (i-1/2, j-1/2, k)
+  int nstages;                      // 1 Euler, 2 RK2, 3 RK3 (Tab. 1)
+  int ct_form;                      // CT_FACE: Eq. 6; CT_POTENTIAL: Eq. 7-8
+  Arr A[3], A0[3], As[3], Bref[3];  // CT_POTENTIAL: edge potential accumulated since set_state (same places as E),
+                                    // its saved and scratch copies, and the face field given to set_state (G19)
+  double t;                         // time since set_state
   double last_dt;
   int status;
   long long roe_fallbacks;
@@ -575,10 +621,9 @@ void sweep(Ctx& c, int d, const Arr Bf[3], bool want_flux) {
         for (int n = 0; n < nq; ++n) {
           const double* v = q[n]->data();
           const double qm2 = v[i0 - 2 * sa], qm1 = v[i0 - sa], q0 = v[i0], qp1 = v[i0 + sa];
-          const double sm = slope(c.limiter, qm1 - qm2, q0 - qm1);   // slope of cell i-1
-          const double s0 = slope(c.limiter, q0 - qm1, qp1 - q0);    // slope of cell i
-          WL[n] = qm1 + 0.5 * sm;
-          WR[n] = q0 - 0.5 * s0;
+          double lo_unused, hi_unused;
+          reconstruct(c.limiter, qm2, qm1, q0, c.dx, lo_unused, WL[n]);   // cell i-1 at its upper face
+          reconstruct(c.limiter, qm1, q0, qp1, c.dx, WR[n], hi_unused);   // cell i at its lower face
         }
         const double Bn = c.mhd ? Bf[a][i0] : 0.0;  // G3: staggered value on both sides
         if (!(WL[0] > 0.0) || !(WR[0] > 0.0) || !(WL[4] > 0.0) || !(WR[4] > 0.0)) c.status = ERR_UNPHYSICAL;
@@ -651,8 +696,9 @@ void edge_emf(Ctx& c, int comp) {
       }
 }
 
-// O2: U* = S_dt(U), Bf* = S_dt(Bf).  `Uin`/`Bin` are modified only in their ghost zones.
-void stage(Ctx& c, Arr Uin[5], Arr Bin[3], double dt, Arr Uout[5], Arr Bout[3]) {
+// O2: U* = S_dt(U), Bf* = S_dt(Bf) (CT_FACE) or A* = S_dt(A) (CT_POTENTIAL).  `Uin`/`Bin` are modified only in
+// their ghost zones.
+void stage(Ctx& c, Arr Uin[5], Arr Bin[3], const Arr Ain[3], double dt, Arr Uout[5], Arr Bout[3], Arr Aout[3]) {
   const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
   for (int n = 0; n < 5; ++n) fill_periodic(c, Uin[n]);
   if (c.mhd)
@@ -679,6 +725,20 @@ void stage(Ctx& c, Arr Uin[5], Arr Bin[3], double dt, Arr Uout[5], Arr Bout[3]) 
       }
   if (!c.mhd) return;
   for (int comp = 0; comp < 3; ++comp) edge_emf(c, comp);
+  if (c.ct_form == CT_POTENTIAL) {
+    // Eq. 7: dA/dt = -E on every edge where E was evaluated (the lattice of the active faces)
+    for (int comp = 0; comp < 3; ++comp) {
+      int hi[3] = {c.n[0], c.n[1], c.n[2]};
+      hi[comp] = c.n[comp] - 1;
+      for (int k = 0; k <= hi[2]; ++k)
+        for (int j = 0; j <= hi[1]; ++j)
+          for (int i = 0; i <= hi[0]; ++i) {
+            const size_t q = c.at(i, j, k);
+            Aout[comp][q] = Ain[comp][q] - dt * c.E[comp][q];
+          }
+    }
+    return;
+  }
   // a7 / O11 / Eq. 6: discrete Stokes theorem on each face
   const size_t sx = c.st[0], sy = c.st[1], sz = c.st[2];
   for (int k = 0; k < nz; ++k)
@@ -711,22 +771,55 @@ double compute_dt(Ctx& c, double cfl) {
   return cfl / mx;
 }
 
-// a8 / O12 / Eq. 9 with Tab. 1: RK2, w1=1, w1^0=0, w2=w2^0=1/2.
+// Eq. 8 with the gauge of G19: Bf = Bref + curl A on the active faces (same differences as Eq. 6).
+void field_from_potential(const Ctx& c, const Arr A[3], Arr Bout[3]) {
+  const size_t sx = c.st[0], sy = c.st[1], sz = c.st[2];
+  for (int k = 0; k < c.n[2]; ++k)
+    for (int j = 0; j < c.n[1]; ++j)
+      for (int i = 0; i < c.n[0]; ++i) {
+        const size_t q = c.at(i, j, k);
+        Bout[0][q] = c.Bref[0][q] + ((A[2][q + sy] - A[2][q]) - (A[1][q + sz] - A[1][q])) / c.dx;
+        Bout[1][q] = c.Bref[1][q] + ((A[0][q + sz] - A[0][q]) - (A[2][q + sx] - A[2][q])) / c.dx;
+        Bout[2][q] = c.Bref[2][q] + ((A[1][q + sx] - A[1][q]) - (A[0][q + sy] - A[0][q])) / c.dx;
+      }
+}
+
+// a8 / O12 / Eq. 9 with Tab. 1: U_s = w_s S_dt(U_{s-1}) + w_s^0 U_0.
+//   Euler: w1 = 1, w1^0 = 0.   RK2: + w2 = w2^0 = 1/2.   RK3: w2 = 1/4, w2^0 = 3/4, w3 = 2/3, w3^0 = 1/3.
 void step(Ctx& c, double dt) {
+  static const double W[3][3] = {{1.0, 0.0, 0.0}, {1.0, 0.5, 0.0}, {1.0, 0.25, 2.0 / 3.0}};
+  static const double W0[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.5, 0.0}, {0.0, 0.75, 1.0 / 3.0}};
   const int nb = c.mhd ? 3 : 0;
+  const bool pot = c.mhd && c.ct_form == CT_POTENTIAL;
   for (int n = 0; n < 5; ++n) c.U0[n] = c.U[n];
   for (int n = 0; n < nb; ++n) c.Bf0[n] = c.Bf[n];
-  stage(c, c.U0, c.Bf0, dt, c.U1, c.Bf1);
-  stage(c, c.U1, c.Bf1, dt, c.Us, c.Bfs);
+  if (pot)
+    for (int n = 0; n < 3; ++n) c.A0[n] = c.A[n];
   const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
-  for (int k = 0; k < nz; ++k)
-    for (int j = 0; j < ny; ++j)
-      for (int i = 0; i < nx; ++i) {
-        const size_t q = c.at(i, j, k);
-        for (int n = 0; n < 5; ++n) c.U[n][q] = 0.5 * c.U0[n][q] + 0.5 * c.Us[n][q];
-        for (int n = 0; n < nb; ++n) c.Bf[n][q] = 0.5 * c.Bf0[n][q] + 0.5 * c.Bfs[n][q];
-      }
+  for (int s = 0; s < c.nstages; ++s) {
+    const double w = W[c.nstages - 1][s], w0 = W0[c.nstages - 1][s];
+    const bool last = s == c.nstages - 1;
+    Arr* Uin = s == 0 ? c.U0 : c.U1;
+    Arr* Bin = s == 0 ? c.Bf0 : c.Bf1;
+    stage(c, Uin, Bin, c.A, dt, c.Us, c.Bfs, c.As);
+    Arr* Unew = last ? c.U : c.U1;
+    Arr* Bnew = last ? c.Bf : c.Bf1;
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+          const size_t q = c.at(i, j, k);
+          for (int n = 0; n < 5; ++n) Unew[n][q] = w0 == 0.0 ? c.Us[n][q] : w0 * c.U0[n][q] + w * c.Us[n][q];
+          if (!pot)
+            for (int n = 0; n < nb; ++n) Bnew[n][q] = w0 == 0.0 ? c.Bfs[n][q] : w0 * c.Bf0[n][q] + w * c.Bfs[n][q];
+        }
+    if (pot) {
+      for (int n = 0; n < 3; ++n)
+        for (size_t q = 0; q < c.N; ++q) c.A[n][q] = w0 == 0.0 ? c.As[n][q] : w0 * c.A0[n][q] + w * c.As[n][q];
+      field_from_potential(c, c.A, Bnew);
+    }
+  }
   c.last_dt = dt;
+  c.t += dt;
 }
 
 }  // namespace
@@ -742,7 +835,7 @@ struct idfxref_ctx {
 IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, double gamma, int solver,
                                         int limiter, int emf_mode) {
   if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(gamma > 1.0)) return nullptr;
-  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 3) return nullptr;
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 3 || emf_mode < 0 || emf_mode > 3) return nullptr;
   const bool mhd = emf_mode != EMF_NONE;
   if (mhd && solver == SOLVER_HLLC) return nullptr;
   if (!mhd && solver == SOLVER_HLLD) return nullptr;
@@ -763,11 +856,32 @@ IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, doubl
     c.cf[d].assign(c.N, 0.0);
     c.E[d].assign(c.N, 0.0);
   }
+  c.nstages = 2; c.ct_form = CT_FACE; c.t = 0.0;
   c.last_dt = 0.0; c.status = OK; c.roe_fallbacks = 0;
   return h;
 }
 
 IDFXREF_API void idfxref_destroy(idfxref_ctx* h) { delete h; }
+
+// Options beyond the create() arguments; call before set_state.  OPT_INTEGRATOR: number of stages 1..3 (Tab. 1);
+// OPT_CT_FORM: CT_FACE (Eq. 6) or CT_POTENTIAL (Eq. 7-8).
+IDFXREF_API int idfxref_set_option(idfxref_ctx* h, int option, int value) {
+  if (!h) return ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  if (option == OPT_INTEGRATOR && value >= 1 && value <= 3) {
+    c.nstages = value;
+    return OK;
+  }
+  if (option == OPT_CT_FORM && (value == CT_FACE || (value == CT_POTENTIAL && c.mhd))) {
+    c.ct_form = value;
+    if (value == CT_POTENTIAL)
+      for (int d = 0; d < 3; ++d) {
+        c.A[d].assign(c.N, 0.0); c.A0[d].assign(c.N, 0.0); c.As[d].assign(c.N, 0.0); c.Bref[d].assign(c.N, 0.0);
+      }
+    return OK;
+  }
+  return ERR_INVALID_ARG;
+}
 
 // O1 set_state: Bc from faces, then U from prims.
 IDFXREF_API int idfxref_set_state(idfxref_ctx* h, const double* prim, const double* bface) {
@@ -782,8 +896,13 @@ IDFXREF_API int idfxref_set_state(idfxref_ctx* h, const double* prim, const doub
         for (int j = 0; j < ny; ++j)
           for (int i = 0; i < nx; ++i) c.Bf[d][c.at(i, j, k)] = bface[d * nc + ((size_t)k * ny + j) * nx + i];
       fill_periodic(c, c.Bf[d]);
+      if (c.ct_form == CT_POTENTIAL) {  // G19: the potential is counted from this state on
+        c.Bref[d] = c.Bf[d];
+        std::fill(c.A[d].begin(), c.A[d].end(), 0.0);
+      }
     }
   }
+  c.t = 0.0;
   for (int k = 0; k < nz; ++k)
     for (int j = 0; j < ny; ++j)
       for (int i = 0; i < nx; ++i) {
@@ -855,6 +974,49 @@ IDFXREF_API int idfxref_advance(idfxref_ctx* h, int nsteps, double cfl) {
   if (!h || nsteps < 0 || !(cfl > 0.0) || !(cfl < 1.0)) return ERR_INVALID_ARG;
   for (int s = 0; s < nsteps; ++s) step(h->c, compute_dt(h->c, cfl));
   return h->c.status;
+}
+
+// Cycles with the CFL step until t_end: a step that would reach or pass t_end is shortened to land on it.
+IDFXREF_API int idfxref_advance_to(idfxref_ctx* h, double t_end, double cfl, int max_steps, int* nsteps_out) {
+  if (!h || max_steps < 0 || !(cfl > 0.0) || !(cfl < 1.0)) return ERR_INVALID_ARG;
+  Ctx& c = h->c;
+  int n = 0;
+  while (c.t < t_end && n < max_steps) {
+    double dt = compute_dt(c, cfl);
+    const double remaining = t_end - c.t;
+    const bool lands = dt >= remaining;
+    if (lands) dt = remaining;
+    step(c, dt);
+    if (lands) c.t = t_end;
+    ++n;
+  }
+  if (nsteps_out) *nsteps_out = n;
+  return c.status;
+}
+
+IDFXREF_API int idfxref_time(const idfxref_ctx* h, double* t_out) {
+  if (!h || !t_out) return ERR_INVALID_ARG;
+  *t_out = h->c.t;
+  return OK;
+}
+
+// Edge potential accumulated since set_state (CT_POTENTIAL), layout as idfxref_get_emf.
+IDFXREF_API int idfxref_get_potential(const idfxref_ctx* h, double* pot) {
+  if (!h || !pot || h->c.ct_form != CT_POTENTIAL) return ERR_INVALID_ARG;
+  const Ctx& c = h->c;
+  const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  const size_t nc = (size_t)nx * ny * nz;
+  for (int comp = 0; comp < 3; ++comp)
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) pot[comp * nc + ((size_t)k * ny + j) * nx + i] = c.A[comp][c.at(i, j, k)];
+  return OK;
+}
+
+// Point-wise S2 for the pins: values of cell i's reconstruction at its lower and upper faces.
+IDFXREF_API void idfxref_reconstruct(int limiter, double qm, double q0, double qp, double dx, double* lower,
+                                     double* upper) {
+  reconstruct(limiter, qm, q0, qp, dx, *lower, *upper);
 }
 
 IDFXREF_API int idfxref_last_dt(const idfxref_ctx* h, double* dt_out) {

@@ -15,7 +15,9 @@ _SRC = os.path.join(_HERE, "idfxref.cpp")
 _LIB = os.path.join(_HERE, "libidfxref.so")
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
-LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER = 0, 1, 2
+LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3 = 0, 1, 2, 3
+OPT_INTEGRATOR, OPT_CT_FORM = 0, 1
+CT_FACE, CT_POTENTIAL = 0, 1
 EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0 = 0, 1, 2, 3
 OK, ERR_UNPHYSICAL = 0, -5
 
@@ -72,6 +74,12 @@ def lib():
         L.idfxref_hlld_fan.argtypes = [cd, dp, dp, cd, dp, dp]
         L.idfxref_hlld_fan.restype = None
         L.idfxref_roe_system.argtypes = [cd, dp, dp, cd, dp, dp, dp]
+        L.idfxref_set_option.argtypes = [vp, ci, ci]
+        L.idfxref_advance_to.argtypes = [vp, cd, cd, ci, ctypes.POINTER(ci)]
+        L.idfxref_time.argtypes = [vp, dp]
+        L.idfxref_get_potential.argtypes = [vp, dp]
+        L.idfxref_reconstruct.argtypes = [ci, cd, cd, cd, cd, dp, dp]
+        L.idfxref_reconstruct.restype = None
         _lib = L
     return _lib
 
@@ -87,13 +95,17 @@ def _c(a):
 class Oracle:
     """One oracle context: a periodic nx*ny*nz box (arrays are [var][nz][ny][nx])."""
 
-    def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode):
+    def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode, nstages=2, ct_form=CT_FACE):
         self.L = lib()
         self.shape = (nz, ny, nx)
         self.mhd = emf_mode != EMF_NONE
         self.h = self.L.idfxref_create(nx, ny, nz, dx, gamma, solver, limiter, emf_mode)
         if not self.h:
             raise ValueError("idfxref_create rejected the arguments")
+        if nstages != 2 and self.L.idfxref_set_option(self.h, OPT_INTEGRATOR, nstages) != OK:
+            raise ValueError("bad number of stages")
+        if ct_form != CT_FACE and self.L.idfxref_set_option(self.h, OPT_CT_FORM, ct_form) != OK:
+            raise ValueError("bad CT form")
 
     def close(self):
         if self.h:
@@ -133,6 +145,23 @@ class Oracle:
 
     def advance(self, nsteps, cfl):
         return self.L.idfxref_advance(self.h, nsteps, cfl)
+
+    def advance_to(self, t_end, cfl, max_steps=1 << 30):
+        """Returns (status, number of cycles taken)."""
+        n = ctypes.c_int()
+        rc = self.L.idfxref_advance_to(self.h, t_end, cfl, max_steps, ctypes.byref(n))
+        return rc, n.value
+
+    def time(self):
+        t = ctypes.c_double()
+        self.L.idfxref_time(self.h, ctypes.byref(t))
+        return t.value
+
+    def get_potential(self):
+        pot = np.empty((3,) + self.shape)
+        if self.L.idfxref_get_potential(self.h, _p(pot)) != OK:
+            raise ValueError("no vector potential in this context")
+        return pot
 
     def last_dt(self):
         dt = ctypes.c_double()
@@ -199,6 +228,13 @@ def wave_speeds(gamma, WL, WR, Bn=0.0):
 
 def slope(limiter, dm, dp):
     return lib().idfxref_slope(limiter, dm, dp)
+
+
+def reconstruct(limiter, qm, q0, qp, dx):
+    """(value at the lower face, value at the upper face) of cell i's reconstruction."""
+    lo, hi = ctypes.c_double(), ctypes.c_double()
+    lib().idfxref_reconstruct(limiter, qm, q0, qp, dx, ctypes.byref(lo), ctypes.byref(hi))
+    return lo.value, hi.value
 
 
 def hllc_fan(gamma, WL, WR):

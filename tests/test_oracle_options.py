@@ -1,0 +1,228 @@
+"""Pins for the oracle's optional parts: the Euler / RK2 / RK3 weights of Tab. 1,
+the LimO3 reconstruction, the vector-potential form of CT (Eq. 7-8) and the
+run-to-a-time driver.  Expected values are closed forms (stability polynomials, point values of a parabola),
+convergence orders, or the equivalence the paper states ("mathematically equivalent to the original CT")."""
+import math
+
+import numpy as np
+import pytest
+
+from test_oracle_scheme import (EMF_ARITH, EMF_NONE, EMF_UCT, FLAT, G53, HLL, HLLD, VANLEER, curl_np, divb,
+                                linear_wave_mode, smooth_mhd_ic)
+
+LIMO3 = 3
+
+
+# =================================================================================================
+# Tab. 1: the stability polynomial of each integrator on a linear problem
+# =================================================================================================
+@pytest.mark.parametrize("nstages", [1, 2, 3])
+def test_rk_amplification_polynomials(R, nstages):
+    """Supersonic uniform flow + flat reconstruction + HLL = first-order upwind advection of rho (linear).  One
+    cycle multiplies Fourier mode m by sum_{q<=s} z^q/q!, z = -(u dt/dx)(1 - exp(-i k dx)): Euler 1 + z, RK2
+    + z^2/2, RK3 + z^3/6 (Gottlieb & Shu 1998, the schemes Tab. 1 encodes)."""
+    n = 16
+    dx = 1.0 / n
+    x = (np.arange(n) + 0.5) * dx
+    prim = np.zeros((5, 1, 1, n))
+    prim[0, 0, 0] = 1.0 + 0.1 * np.cos(2 * np.pi * x) + 0.05 * np.sin(4 * np.pi * x)
+    prim[1] = 3.0
+    prim[4] = 0.1
+    o = R.Oracle(n, 1, 1, dx, 1.4, HLL, FLAT, EMF_NONE, nstages=nstages)
+    o.set_state(prim)
+    dt = 0.37 * dx / 3.0
+    o.step(dt)
+    f0, f1 = np.fft.fft(prim[0].ravel()), np.fft.fft(o.get_state()[0][0].ravel())
+    for m in (1, 2):
+        z = -(3.0 * dt / dx) * (1 - np.exp(-2j * np.pi * m / n))
+        poly = sum(z ** q / math.factorial(q) for q in range(nstages + 1))
+        assert f1[m] / f0[m] == pytest.approx(poly, abs=1e-13)
+    assert o.time() == dt
+
+
+def nonlinear_1d_ic(n, amp=0.05):
+    dx = 1.0 / n
+    c = np.cos(2 * np.pi * (np.arange(n) + 0.5) * dx)
+    s = np.sin(2 * np.pi * (np.arange(n) + 0.5) * dx)
+    prim = np.empty((5, 1, 1, n))
+    prim[0, 0, 0] = 1 + amp * c
+    prim[1, 0, 0] = amp * s
+    prim[2, 0, 0] = 0.5 * amp * c
+    prim[3, 0, 0] = -0.3 * amp * s
+    prim[4, 0, 0] = 0.6 + amp * 0.4 * c
+    bf = np.empty((3, 1, 1, n))
+    bf[0], bf[1, 0, 0], bf[2, 0, 0] = 1.0, 1.5 + amp * s, amp * 0.5 * c
+    return prim, bf
+
+
+@pytest.mark.parametrize("nstages", [1, 2, 3])
+def test_temporal_order_of_the_integrators(R, nstages):
+    """Fixed grid, smooth nonlinear MHD flow, time step halved: the difference to a finely stepped run falls as
+    dt^s for the s-stage scheme, for the cell variables and for the face field alike."""
+    n, T = 32, 0.02
+    prim, bf = nonlinear_1d_ic(n)
+
+    def run(nsteps):
+        o = R.Oracle(n, 1, 1, 1.0 / n, G53, HLL, LIMO3, EMF_UCT, nstages=nstages)
+        o.set_state(prim, bf)
+        for _ in range(nsteps):
+            assert o.step(T / nsteps) == 0
+        u, b = o.get_conserved()
+        return np.concatenate([u.ravel(), b.ravel()])
+
+    ref = run(1024 if nstages == 1 else 256)
+    e = [np.abs(run(k) - ref).max() for k in (4, 8, 16)]
+    for a, b in zip(e[:-1], e[1:]):
+        assert math.log2(a / b) == pytest.approx(nstages, abs=0.25), (nstages, e)
+
+
+# =================================================================================================
+# LimO3
+# =================================================================================================
+def test_limo3_reproduces_a_parabola_where_the_data_are_smooth(R):
+    """Cell averages of q(x) = a + b x + c x^2 on a uniform grid: the unlimited weight (2 + theta)/3 returns the point
+    values of q at both faces exactly (third order); dx = 0.1 and small coefficients keep eta < 1."""
+    a, b, c, dx = 0.7, 0.31, -0.23, 0.1
+    avg = lambda xc: a + b * xc + c * (xc * xc + dx * dx / 12.0)
+    q = lambda x: a + b * x + c * x * x
+    for xc in (-0.35, 0.0, 0.2, 1.05):
+        lo, hi = R.reconstruct(LIMO3, avg(xc - dx), avg(xc), avg(xc + dx), dx)
+        assert lo == pytest.approx(q(xc - dx / 2), abs=2e-16 * 8)
+        assert hi == pytest.approx(q(xc + dx / 2), abs=2e-16 * 8)
+
+
+def test_limo3_limited_branch_values(R):
+    """Steep data (eta > 1): phi = max(0, min((2+theta)/3, max(-theta/2, min(2 theta, (2+theta)/3, 1.6)))).  Linear data keep
+    phi = 1; a monotone kink is capped by 2 theta on one side and by 1.6 on the other; extrema with theta in (-2, 0)
+    keep a reduced, non-zero increment (the scheme does not clip extrema) and theta <= -2 gives zero."""
+    dx = 1e-3
+    # (qm, q0, qp) -> expected phi(theta) for the upper face and phi(1/theta) for the lower one
+    cases = [((0.0, 1.0, 2.0), 1.0, 1.0),            # theta = 1
+             ((0.0, 10.0, 11.0), 1.6, 0.2),          # theta = 10: cap 1.6;   1/theta = 0.1: 2 theta
+             ((0.0, 1.0, 5.0), 0.5, 1.6),            # theta = 1/4: 2 theta;  1/theta = 4: min(phat = 2, 1.6)
+             ((0.0, 1.0, 0.0), 1.0 / 3.0, 1.0 / 3.0),  # theta = -1: min(1/3, 1/2)
+             ((0.0, 3.0, 2.0), 0.0, 0.5 / 3.0),      # theta = -3 -> 0;  1/theta = -1/3: min(5/9, 1/6)
+             ((0.0, 1.0, 1.0), 0.0, 0.0)]            # d+ = 0
+    for (qm, q0, qp), phi_up, phi_lo in cases:
+        lo, hi = R.reconstruct(LIMO3, qm, q0, qp, dx)
+        assert hi == pytest.approx(q0 + 0.5 * phi_up * (qp - q0), abs=1e-15)
+        assert lo == pytest.approx(q0 - 0.5 * phi_lo * (q0 - qm), abs=1e-15)
+
+
+def test_limo3_symmetries_and_bounds(R):
+    rng = np.random.default_rng(5)
+    for _ in range(2000):
+        qm, q0, qp = rng.normal(size=3) * 10.0 ** rng.integers(-3, 2)
+        dx = 10.0 ** rng.integers(-4, 1)
+        lo, hi = R.reconstruct(LIMO3, qm, q0, qp, dx)
+        lo_r, hi_r = R.reconstruct(LIMO3, qp, q0, qm, dx)      # mirror image
+        assert (lo, hi) == (hi_r, lo_r)
+        lo_n, hi_n = R.reconstruct(LIMO3, -qm, -q0, -qp, dx)   # odd in the data
+        assert (lo_n, hi_n) == (-lo, -hi)
+        lo_s, hi_s = R.reconstruct(LIMO3, qm + 1.0, q0 + 1.0, qp + 1.0, dx)
+        assert lo_s == pytest.approx(lo + 1.0, abs=1e-12 * max(1.0, abs(q0))) and hi_s == pytest.approx(hi + 1.0, abs=1e-12 * max(1.0, abs(q0)))
+        if (qm - q0) ** 2 + (qp - q0) ** 2 > 1.01 * dx * dx:   # limited: 0 <= phi <= 1.6, and monotone data stay bounded
+            slack = 4e-16 * max(abs(q0), abs(qp)) * abs(qp - q0)   # hi is rounded at the size of q0
+            assert -slack <= (hi - q0) * (qp - q0) <= 0.8 * (qp - q0) ** 2 + slack
+            if (q0 - qm) * (qp - q0) > 0:
+                assert min(q0, qp) <= hi <= max(q0, qp) and min(qm, q0) <= lo <= max(qm, q0)
+
+
+def run_wave_1d(R, n, limiter, nstages, kind="fast", cfl=0.4, eps=1e-6):
+    speed, r = linear_wave_mode(kind)
+    dx = 1.0 / n
+    c = np.cos(2 * np.pi * (np.arange(n) + 0.5) * dx).reshape(1, 1, n)
+    prim = np.empty((5, 1, 1, n))
+    prim[0] = 1 + eps * r[0] * c
+    prim[1], prim[2], prim[3] = eps * r[1] * c, eps * r[2] * c, eps * r[3] * c
+    prim[4] = 0.6 + eps * r[4] * c
+    bf = np.empty((3, 1, 1, n))
+    bf[0], bf[1], bf[2] = 1.0, 1.5 + eps * r[5] * c, eps * r[6] * c
+    o = R.Oracle(n, 1, 1, dx, G53, HLLD, limiter, EMF_UCT, nstages=nstages)
+    o.set_state(prim, bf)
+    period = 1.0 / speed
+    nsteps = int(math.ceil(period / o.compute_dt(cfl)))
+    for _ in range(nsteps):
+        assert o.step(period / nsteps) == 0
+    p1, b1 = o.get_state()
+    tot = [np.abs(p1[v] - prim[v]).mean() for v in range(5)] + [np.abs(b1[d] - bf[d]).mean() for d in range(3)]
+    return math.sqrt(sum(t * t for t in tot)) / eps
+
+
+@pytest.mark.parametrize("kind", ["fast", "alfven"])
+def test_rk3_limo3_linear_wave_is_third_order(R, kind):
+    """The paper's most accurate combination short of PPM (Fig. 7): third-order convergence, and an
+    error well below the second-order scheme's at the same resolution."""
+    errs = [run_wave_1d(R, n, LIMO3, 3, kind) for n in (32, 64)]
+    assert math.log2(errs[0] / errs[1]) >= 2.8, errs
+    assert errs[1] < 0.2 * run_wave_1d(R, 64, VANLEER, 2, kind)
+
+
+# =================================================================================================
+# Eq. 7-8: vector-potential form of CT
+# =================================================================================================
+@pytest.mark.parametrize("nstages,emf", [(2, EMF_UCT), (3, EMF_ARITH), (1, EMF_UCT)])
+def test_vector_potential_form_equals_face_form(R, nstages, emf):
+    """"mathematically equivalent to the original CT algorithm": same run in both forms, differences at
+    rounding level only; and the potential is what Eq. 7 says, checked on one Euler step against the stored EMFs."""
+    n = 12
+    prim, b = smooth_mhd_ic(n, seed=11)
+    outs = []
+    for form in (R.CT_FACE, R.CT_POTENTIAL):
+        o = R.Oracle(n, n, n, 1.0 / n, G53, HLLD, VANLEER, emf, nstages=nstages, ct_form=form)
+        o.set_state(prim, b)
+        assert o.advance(6, 0.3) == 0
+        outs.append(o.get_conserved())
+    for x, y in zip(outs[0], outs[1]):
+        assert np.abs(x - y).max() <= 2e-14 * np.abs(x).max()
+    o = R.Oracle(n, n, n, 1.0 / n, G53, HLLD, VANLEER, emf, nstages=1, ct_form=R.CT_POTENTIAL)
+    o.set_state(prim, b)
+    dt = 0.5 * o.compute_dt(0.3)
+    o.step(dt)
+    np.testing.assert_array_equal(o.get_potential(), -dt * o.get_emf())
+    a = o.get_potential()
+    bnew = o.get_conserved()[1]
+    np.testing.assert_allclose(bnew, b + curl_np(a[0], a[1], a[2], 1.0 / n), rtol=0, atol=1e-15)
+
+
+def test_vector_potential_divb_does_not_accumulate(R):
+    """"prevents roundoff errors from accumulating in div B": after many cycles the divergence of the
+    potential form is still one rounding of the face values, while the face form has drifted above it."""
+    n = 8
+    prim, b = smooth_mhd_ic(n, seed=3)
+    res = {}
+    for form in (R.CT_FACE, R.CT_POTENTIAL):
+        o = R.Oracle(n, n, n, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT, ct_form=form)
+        o.set_state(prim, b)
+        assert o.advance(150, 0.3) == 0
+        bf = o.get_conserved()[1]
+        res[form] = np.abs(divb(bf)).max() / np.abs(bf).max()
+    assert res[R.CT_POTENTIAL] <= 8 * 2.2e-16      # sum of six face values, each rounded once
+    assert res[R.CT_FACE] > res[R.CT_POTENTIAL]
+
+
+# =================================================================================================
+# run to a given time (the paper's runs are "to t = ...")
+# =================================================================================================
+def test_advance_to_lands_on_t_end(R):
+    n = 8
+    prim, b = smooth_mhd_ic(n, seed=7)
+    o = R.Oracle(n, n, n, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT)
+    o.set_state(prim, b)
+    t_end = 3.6 * o.compute_dt(0.3)
+    rc, nsteps = o.advance_to(t_end, 0.3)
+    assert rc == 0 and o.time() == t_end and 4 <= nsteps <= 5
+    # the same by hand: CFL steps, the last one shortened
+    o2 = R.Oracle(n, n, n, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT)
+    o2.set_state(prim, b)
+    t = 0.0
+    for _ in range(nsteps):
+        dt = min(o2.compute_dt(0.3), t_end - t)
+        o2.step(dt)
+        t += dt
+    for x, y in zip(o.get_conserved(), o2.get_conserved()):
+        np.testing.assert_array_equal(x, y)
+    # max_steps stops early
+    o.set_state(prim, b)
+    rc, k = o.advance_to(t_end, 0.3, max_steps=2)
+    assert k == 2 and 0.0 < o.time() < t_end
