@@ -3,7 +3,8 @@
  * to the written-out formulas and readings in DESIGN.md (same numbering as SURVEY.md §8(c)).
  *
  * What one context is: a uniform periodic Cartesian box of nx*ny*nz cells with spacing dx in all three
- * directions, gamma-law gas, advanced by the explicit RK2 cycle of PAPER.md:130-145 (Eq. 9, Tab. 1):
+ * directions, gamma-law gas, advanced by the explicit multi-stage cycle of PAPER.md:130-145 (Eq. 9, Tab. 1; RK2 unless
+ * idfx_set_option selects Euler or RK3):
  *   cycle:  dt = cfl / max_cells sum_d c_max,d/dx                  (Eq. 10 without eta)
  *           U1 = S_dt(U0);  U = U0/2 + S_dt(U1)/2                  (Eq. 9, w2 = w2^0 = 1/2)
  *   S_dt:   periodic ghost fill -> cell-centred B and cons->prim -> PLM reconstruction of primitives to faces
@@ -12,8 +13,8 @@
  * Every step of that path runs in CUDA kernels of this library; there is no CPU fallback.
  *
  * Conventions
- *   - All arithmetic is IEEE fp64.  No floors are applied (G13): rho <= 0, p <= 0 or NaN met in the
- *     cons->prim conversion raises a sticky device flag reported as IDFX_ERR_UNPHYSICAL.
+ *   - All arithmetic is IEEE fp64.  No floors are applied (G13) unless IDFX_OPT_PRESSURE_FLOOR is set: rho <= 0, p <= 0
+ *     or NaN met in the cons->prim conversion raises a sticky device flag reported as IDFX_ERR_UNPHYSICAL.
  *   - Array layout: structure of arrays, [var][nz][ny][nx] contiguous, x fastest, no padding.
  *       prim  : [5] = rho, vx, vy, vz, p           cons : [5] = rho, mx, my, mz, E
  *       bface : [3]; bface[d][k][j][i] is B_d on the LEFT d-face of cell (i,j,k), i.e. B_x at (i-1/2, j, k).
@@ -26,8 +27,8 @@
  *     whatever owns device memory in the application, e.g. a torch tensor).  The context owns no large
  *     device allocation; it owns CUDA graphs, TMA descriptors and a few hundred bytes of host memory.
  *   - All work is enqueued on the stream given to idfx_bind (a cudaStream_t cast to void*, NULL = legacy
- *     default stream).  Only idfx_compute_dt, idfx_last_dt, idfx_status, idfx_set_state_host and
- *     idfx_get_state_host synchronise with the host (the host-buffer calls return when the copy is done,
+ *     default stream).  Only idfx_compute_dt, idfx_last_dt, idfx_status, idfx_advance_to, idfx_time, idfx_floor_count,
+ *     idfx_set_state_host and idfx_get_state_host synchronise with the host (the host-buffer calls return when the copy is done,
  *     so the caller may reuse or free its buffers immediately).
  *   - Errors: every int-returning call returns IDFX_OK or a negative code; nothing throws or aborts.
  *     idfx_last_error() gives a thread-local message for the last failure.
@@ -46,8 +47,9 @@ typedef struct idfx_ctx idfx_ctx;
 /* Riemann solvers, here listed by number; the paper orders them from most to least diffusive:
  * Rusanov (local Lax-Friedrichs), HLL, HLLC / HLLD, Roe.  HLLC is hydrodynamics-only; in MHD it is replaced by HLLD. */
 enum { IDFX_SOLVER_HLL = 0, IDFX_SOLVER_HLLC = 1, IDFX_SOLVER_HLLD = 2, IDFX_SOLVER_ROE = 3, IDFX_SOLVER_RUSANOV = 4 };
-/* Reconstruction: flat (1st order), PLM with minmod or van Leer (harmonic mean, G2) slopes. */
-enum { IDFX_LIMITER_FLAT = 0, IDFX_LIMITER_MINMOD = 1, IDFX_LIMITER_VANLEER = 2 };
+/* Reconstruction: flat (1st order), PLM with minmod or van Leer (harmonic mean, G2) slopes, and the compact
+ * third-order LimO3 of Cada & Torrilhon 2009 (same 3-cell stencil and 2 ghost layers; constants in reading G18). */
+enum { IDFX_LIMITER_FLAT = 0, IDFX_LIMITER_MINMOD = 1, IDFX_LIMITER_VANLEER = 2, IDFX_LIMITER_LIMO3 = 3 };
 /* EMF reconstruction: arithmetic average of the face fluxes, and the E^0 and E^c (upwind-contact)
  * schemes of Gardiner & Stone 2005.  IDFX_EMF_NONE selects hydrodynamics (no magnetic field at all). */
 enum { IDFX_EMF_NONE = 0, IDFX_EMF_ARITHMETIC = 1, IDFX_EMF_UCT_CONTACT = 2, IDFX_EMF_UCT_0 = 3 };
@@ -64,6 +66,25 @@ enum {
  * with RUSANOV/HLL/HLLC/ROE, MHD with RUSANOV/HLL/HLLD/ROE.  Returns NULL on error (idfx_last_error() says why).
  * Host-only: touches no device memory. */
 idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solver, int limiter, int emf_mode);
+
+/* Options beyond the arguments of idfx_create.
+ *   IDFX_OPT_INTEGRATOR: number of stages of the explicit integrator of Tab. 1: 1 = Euler,
+ *     2 = RK2 (default), 3 = RK3 (w2 = 1/4, w2^0 = 3/4, w3 = 2/3, w3^0 = 1/3).  May be changed at any time between cycles.
+ *   IDFX_OPT_CT_FORM: IDFX_CT_FACE (default) evolves the face field with Eq. 6; IDFX_CT_POTENTIAL evolves the
+ *     edge-centred vector potential, dA/dt = -E, and sets B = B_ref + curl A after every stage (Eq. 7-8),
+ *     so that round-off cannot accumulate in div B.  B_ref is the face field given to idfx_set_state and A counts from
+ *     zero there (reading G19: a periodic A cannot carry a mean field).  MHD only; must be chosen BEFORE
+ *     idfx_workspace_bytes / idfx_bind (it needs 12 more fields). */
+enum { IDFX_OPT_INTEGRATOR = 0, IDFX_OPT_CT_FORM = 1, IDFX_OPT_PRESSURE_FLOOR = 2 };
+enum { IDFX_CT_FACE = 0, IDFX_CT_POTENTIAL = 1 };
+int idfx_set_option(idfx_ctx* ctx, int option, int value);
+/* Real-valued options.  IDFX_OPT_PRESSURE_FLOOR (default 0 = none, reading G13): when > 0, a pressure below it met in
+ * the cons->prim conversion is raised to it and the total energy of the cell is rewritten to match (energy is then no
+ * longer conserved in that cell; idfx_floor_count says how often this happened since idfx_set_state).  The paper describes
+ * no such fix, but without one its own 3D Orszag-Tang run with HLLD meets p < 0 before t = 1 (DESIGN.md,
+ * reading G20).  May be changed between cycles. */
+int idfx_set_option_real(idfx_ctx* ctx, int option, double value);
+int idfx_floor_count(idfx_ctx* ctx, long long* h_count_out); /* synchronises */
 
 /* Device bytes the caller must supply to idfx_bind (internal padded state, stage buffers, fluxes, EMFs). */
 size_t idfx_workspace_bytes(const idfx_ctx* ctx);
@@ -88,14 +109,28 @@ int idfx_get_conserved(idfx_ctx* ctx, double* d_cons, double* d_bface);
  * 0 < cfl < 1.  Writes *h_dt_out; synchronises. */
 int idfx_compute_dt(idfx_ctx* ctx, double cfl, double* h_dt_out);
 
-/* One RK2 cycle with the given dt > 0 (O12). */
+/* One cycle of the integrator (RK2 by default) with the given dt > 0 (O12). */
 int idfx_step(idfx_ctx* ctx, double dt);
 
 /* nsteps cycles, each with dt evaluated on the state at the start of that cycle (G9); dt never leaves the
  * device.  Equivalent to nsteps x { idfx_compute_dt; idfx_step }.  When the bound stream is not the default stream the
- * cycle (8 kernels + one memset) is captured once per buffer-rotation state into a CUDA graph and replayed
+ * cycle (9 kernels for RK2 MHD) is captured once per buffer-rotation state into a CUDA graph and replayed
  * (IDFX_GRAPH=0 in the environment disables this). */
 int idfx_advance(idfx_ctx* ctx, int nsteps, double cfl);
+
+/* Cycles with the CFL step until the time t_end (time counts from 0 at idfx_set_state; the paper's runs are "to t = ...",
+ * PAPER.md:346): a step that would reach or pass t_end is shortened on the device to land on it exactly.  Stops early
+ * after max_steps cycles.  Cycles are enqueued in batches and the device clock is read back between batches
+ * (synchronises); a cycle enqueued past t_end leaves the state bit-for-bit unchanged.  Writes the number of cycles
+ * taken by this call and the time reached (either may be NULL). */
+int idfx_advance_to(idfx_ctx* ctx, double t_end, double cfl, int max_steps, int* h_nsteps_out, double* h_t_out);
+
+/* Time reached since idfx_set_state (synchronises). */
+int idfx_time(idfx_ctx* ctx, double* h_t_out);
+
+/* IDFX_CT_POTENTIAL only: the edge potential accumulated since idfx_set_state, d_pot[c][k][j][i] = A_c on the lower
+ * edges of cell (i,j,k): A_x at (i, j-1/2, k-1/2), A_y at (i-1/2, j, k-1/2), A_z at (i-1/2, j-1/2, k). */
+int idfx_get_potential(idfx_ctx* ctx, double* d_pot);
 
 /* dt used by the most recent cycle (synchronises). */
 int idfx_last_dt(idfx_ctx* ctx, double* h_dt_out);

@@ -41,7 +41,7 @@ constexpr int NG = 2;  // ghost layers: PLM needs 2 ("number of ghos
 
 enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_RUSANOV = 4 };
 enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3 };
-enum { OPT_INTEGRATOR = 0, OPT_CT_FORM = 1 };  // idfxref_set_option
+enum { OPT_INTEGRATOR = 0, OPT_CT_FORM = 1, OPT_PRESSURE_FLOOR = 2 };  // idfxref_set_option / idfxref_set_option_real
 enum { CT_FACE = 0, CT_POTENTIAL = 1 };
 enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3 };
 enum { OK = 0, ERR_INVALID_ARG = -1, ERR_UNSUPPORTED = -2, ERR_UNPHYSICAL = -5 };
@@ -538,6 +538,8 @@ struct Ctx {
   Arr A[3], A0[3], As[3], Bref[3];  // CT_POTENTIAL: edge potential accumulated since set_state (same places as E),
                                     // its saved and scratch copies, and the face field given to set_state (G19)
   double t;                         // time since set_state
+  double pfloor;                    // optional pressure floor (0 = none, G13); see compute_prims
+  long long nfloor;                 // how often it acted since set_state
   double last_dt;
   int status;
   long long roe_fallbacks;
@@ -578,7 +580,8 @@ void fill_periodic(const Ctx& c, Arr& a) {
 // a2 / O1: Bc = mean of the two bounding faces (G1); v = m/rho; p = (gamma-1)(E - rho v^2/2 - Bc^2/2).
 // Needs the face ghosts of Bf (face index n).  Prims are computed on active cells and then filled
 // periodically, which is bit-identical to computing them in the ghosts from filled U and Bf (O2 (i)-(ii)).
-void compute_prims(Ctx& c, const Arr U[5], const Arr Bf[3]) {
+// Optional (reading G20, off by default): a pressure below c.pfloor is raised to it and E is rewritten to match.
+void compute_prims(Ctx& c, Arr U[5], const Arr Bf[3]) {
   const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
   for (int k = 0; k < nz; ++k)
     for (int j = 0; j < ny; ++j)
@@ -592,8 +595,16 @@ void compute_prims(Ctx& c, const Arr U[5], const Arr Bf[3]) {
         }
         const double rho = U[0][q];
         const double vx = U[1][q] / rho, vy = U[2][q] / rho, vz = U[3][q] / rho;
-        const double p =
+        double p =
             (c.g - 1.0) * (U[4][q] - 0.5 * rho * (vx * vx + vy * vy + vz * vz) - 0.5 * (bx * bx + by * by + bz * bz));
+        if (c.pfloor > 0.0 && p < c.pfloor) {
+          // a cell floored before recomputes to the floor within rounding: its energy is left as it is
+          if (p < c.pfloor * (1.0 - 1e-9)) {
+            U[4][q] = c.pfloor / (c.g - 1.0) + 0.5 * rho * (vx * vx + vy * vy + vz * vz) + 0.5 * (bx * bx + by * by + bz * bz);
+            c.nfloor += 1;
+          }
+          p = c.pfloor;
+        }
         if (!(rho > 0.0) || !(p > 0.0)) c.status = ERR_UNPHYSICAL;
         c.V[0][q] = rho; c.V[1][q] = vx; c.V[2][q] = vy; c.V[3][q] = vz; c.V[4][q] = p;
         c.V[5][q] = bx; c.V[6][q] = by; c.V[7][q] = bz;
@@ -818,6 +829,10 @@ void step(Ctx& c, double dt) {
       field_from_potential(c, c.A, Bnew);
     }
   }
+  if (c.pfloor > 0.0) {  // G20: the floor belongs to the cons->prim conversion of the result, so the state a cycle
+    for (int n = 0; n < nb; ++n) fill_periodic(c, c.Bf[n]);  // leaves behind is already fixed
+    compute_prims(c, c.U, c.Bf);
+  }
   c.last_dt = dt;
   c.t += dt;
 }
@@ -856,7 +871,7 @@ IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, doubl
     c.cf[d].assign(c.N, 0.0);
     c.E[d].assign(c.N, 0.0);
   }
-  c.nstages = 2; c.ct_form = CT_FACE; c.t = 0.0;
+  c.nstages = 2; c.ct_form = CT_FACE; c.t = 0.0; c.pfloor = 0.0; c.nfloor = 0;
   c.last_dt = 0.0; c.status = OK; c.roe_fallbacks = 0;
   return h;
 }
@@ -903,6 +918,7 @@ IDFXREF_API int idfxref_set_state(idfxref_ctx* h, const double* prim, const doub
     }
   }
   c.t = 0.0;
+  c.nfloor = 0;
   for (int k = 0; k < nz; ++k)
     for (int j = 0; j < ny; ++j)
       for (int i = 0; i < nx; ++i) {
@@ -975,6 +991,14 @@ IDFXREF_API int idfxref_advance(idfxref_ctx* h, int nsteps, double cfl) {
   for (int s = 0; s < nsteps; ++s) step(h->c, compute_dt(h->c, cfl));
   return h->c.status;
 }
+
+IDFXREF_API int idfxref_set_option_real(idfxref_ctx* h, int option, double value) {
+  if (!h || option != OPT_PRESSURE_FLOOR || !(value >= 0.0)) return ERR_INVALID_ARG;
+  h->c.pfloor = value;
+  return OK;
+}
+
+IDFXREF_API long long idfxref_floor_count(const idfxref_ctx* h) { return h ? h->c.nfloor : -1; }
 
 // Cycles with the CFL step until t_end: a step that would reach or pass t_end is shortened to land on it.
 IDFXREF_API int idfxref_advance_to(idfxref_ctx* h, double t_end, double cfl, int max_steps, int* nsteps_out) {

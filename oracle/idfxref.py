@@ -16,7 +16,7 @@ _LIB = os.path.join(_HERE, "libidfxref.so")
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
 LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3 = 0, 1, 2, 3
-OPT_INTEGRATOR, OPT_CT_FORM = 0, 1
+OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR = 0, 1, 2
 CT_FACE, CT_POTENTIAL = 0, 1
 EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0 = 0, 1, 2, 3
 OK, ERR_UNPHYSICAL = 0, -5
@@ -75,6 +75,9 @@ def lib():
         L.idfxref_hlld_fan.restype = None
         L.idfxref_roe_system.argtypes = [cd, dp, dp, cd, dp, dp, dp]
         L.idfxref_set_option.argtypes = [vp, ci, ci]
+        L.idfxref_set_option_real.argtypes = [vp, ci, cd]
+        L.idfxref_floor_count.argtypes = [vp]
+        L.idfxref_floor_count.restype = ctypes.c_longlong
         L.idfxref_advance_to.argtypes = [vp, cd, cd, ci, ctypes.POINTER(ci)]
         L.idfxref_time.argtypes = [vp, dp]
         L.idfxref_get_potential.argtypes = [vp, dp]
@@ -95,7 +98,7 @@ def _c(a):
 class Oracle:
     """One oracle context: a periodic nx*ny*nz box (arrays are [var][nz][ny][nx])."""
 
-    def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode, nstages=2, ct_form=CT_FACE):
+    def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode, nstages=2, ct_form=CT_FACE, pressure_floor=0.0):
         self.L = lib()
         self.shape = (nz, ny, nx)
         self.mhd = emf_mode != EMF_NONE
@@ -106,6 +109,8 @@ class Oracle:
             raise ValueError("bad number of stages")
         if ct_form != CT_FACE and self.L.idfxref_set_option(self.h, OPT_CT_FORM, ct_form) != OK:
             raise ValueError("bad CT form")
+        if pressure_floor and self.L.idfxref_set_option_real(self.h, OPT_PRESSURE_FLOOR, pressure_floor) != OK:
+            raise ValueError("bad pressure floor")
 
     def close(self):
         if self.h:
@@ -151,6 +156,9 @@ class Oracle:
         n = ctypes.c_int()
         rc = self.L.idfxref_advance_to(self.h, t_end, cfl, max_steps, ctypes.byref(n))
         return rc, n.value
+
+    def floor_count(self):
+        return self.L.idfxref_floor_count(self.h)
 
     def time(self):
         t = ctypes.c_double()

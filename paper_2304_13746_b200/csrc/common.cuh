@@ -14,6 +14,7 @@ struct Geom {
   long long np;   // padded field size in doubles
   long long nc;   // nx*ny*nz
   double dx, gamma;
+  double pfloor;  // > 0: pressures below it are raised to it in cons->prim and E is rewritten (idfx_set_option_real); 0: none (G13)
   __host__ __device__ __forceinline__ long long at(int i, int j, int k) const {
     return (long long)(k + NG) * sz + (long long)(j + NG) * sy + (i + IOFF);
   }
@@ -32,9 +33,36 @@ __device__ __forceinline__ bool cell_of_thread(const Geom& g, int& i, int& j, in
 
 struct DevScalars {
   unsigned long long smax_bits;  // bit pattern of max_cells sum_d c_d/dx (positive doubles order like integers)
-  double dt_used;
+  double dt_used;                // dt of the running cycle, written by the update kernel of its first stage
   int flag;
+  int pad_;
+  double t;                      // time at the start of the running cycle (committed by k_cycle_begin)
+  double t_next;                 // time at its end
+  double t_end;                  // +inf, or the target of idfx_advance_to: a step that would pass it lands on it
+  long long ncycles;             // cycles with dt > 0 since set_state
+  unsigned long long nfloor;     // cells raised to the pressure floor since set_state
 };
+
+// dt of the cycle as the first stage's update kernel sees it (every thread evaluates the same expression):
+// the fixed step, or Eq. 10 from the reduced maximum, shortened to land on t_end.
+__device__ __forceinline__ double first_stage_dt(const DevScalars* sc, double dt_fixed, double cfl, bool& lands) {
+  double dt = dt_fixed;
+  lands = false;
+  if (!(dt > 0.0)) {
+    dt = cfl / __longlong_as_double((long long)sc->smax_bits);
+    const double remaining = sc->t_end - sc->t;
+    lands = dt >= remaining;
+    if (lands) dt = remaining;
+  }
+  return dt;
+}
+
+// thread 0 of block 0 of that kernel publishes it
+__device__ __forceinline__ void publish_dt(DevScalars* sc, double dt, bool lands) {
+  sc->dt_used = dt;
+  sc->t_next = lands ? sc->t_end : sc->t + dt;
+  if (dt > 0.0) sc->ncycles += 1;
+}
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 

@@ -40,6 +40,7 @@ struct FluxXArgs {
 template <int SOLVER, int LIM, bool MHD>
 __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a) {
   constexpr int NQ = MHD ? 7 : 5;
+  const double dx2 = g.dx * g.dx;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int f0 = 31 * blockIdx.x;
   const int ci = f0 - 1 + lane;
@@ -82,9 +83,9 @@ __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a
       double qp = __shfl_down_sync(0xffffffffu, q[n], 1);
       if (lane == 0) qm = qe[n];
       if (lane == 31) qp = qe[n];
-      const double s = limited_slope<LIM>(q[n] - qm, qp - q[n]);
-      WR[n] = q[n] - 0.5 * s;
-      WL[n] = __shfl_up_sync(0xffffffffu, q[n] + 0.5 * s, 1);
+      double up;
+      face_values<LIM>(q[n], q[n] - qm, qp - q[n], dx2, WR[n], up);
+      WL[n] = __shfl_up_sync(0xffffffffu, up, 1);
     }
     if (!MHD) WL[5] = WL[6] = WR[5] = WR[6] = 0.0;
     if (solve) {
@@ -121,6 +122,7 @@ struct FluxMArgs {
 template <int SOLVER, int LIM, bool MHD, int DIR, bool WANT_DT, bool WANT_FM>
 __global__ void __launch_bounds__(128, IDFX_MINB_M) k_flux_march(Geom g, FluxMArgs a) {
   constexpr int NQ = MHD ? 7 : 5;
+  const double dx2 = g.dx * g.dx;
   // local momentum components (n, t1, t2) -> global slot in R
   constexpr int PN = 1 + DIR, PT1 = 1 + (DIR + 1) % 3, PT2 = 1 + (DIR + 2) % 3;
   const int i = blockIdx.x * 32 + (threadIdx.x & 31);
@@ -139,7 +141,8 @@ __global__ void __launch_bounds__(128, IDFX_MINB_M) k_flux_march(Geom g, FluxMAr
       const double qc = a.q[n][c + sd];
       q0[n] = a.q[n][c + 2 * sd];
       dm[n] = q0[n] - qc;
-      WL[n] = qc + 0.5 * limited_slope<LIM>(qc - qm, dm[n]);  // slope of cell s0-1
+      double lo_unused;
+      face_values<LIM>(qc, qc - qm, dm[n], dx2, lo_unused, WL[n]);  // cell s0-1 at its upper face
     }
     c += 2 * sd;  // cell s0 = right cell of face s0
 #pragma unroll
@@ -181,9 +184,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_M) k_flux_march(Geom g, FluxMAr
 #pragma unroll
       for (int n = 0; n < NQ; ++n) {
         const double dp = qp[n] - q0[n];
-        const double sl = limited_slope<LIM>(dm[n], dp);
-        WR[n] = q0[n] - 0.5 * sl;
-        WLn[n] = q0[n] + 0.5 * sl;
+        face_values<LIM>(q0[n], dm[n], dp, dx2, WR[n], WLn[n]);
         dm[n] = dp;
       }
       if (!MHD) WR[5] = WR[6] = 0.0;

@@ -64,11 +64,11 @@ struct FluxTArgs {
   double* FB[2];
   signed char* SG;      // sign of the face mass flux (upwind-contact EMF only)
   DevScalars* sc;
-  // APPLY (stage 2 of the z sweep): the completed divergence is applied at once, U = U0/2 + (U1 - dt/dx R)/2
+  // APPLY (stages >= 2 of the z sweep): the completed divergence is applied at once, U_s = w0 U_0 + w (U_{s-1} - dt/dx R)
   const double* Uin[5];
   const double* U0[5];
   double* Uout[5];
-  double dt_fixed, cfl;
+  double w, w0;
 };
 
 template <int SOLVER, int LIM, int DIR, bool WANT_DT, bool WANT_FM, bool APPLY>
@@ -76,6 +76,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
                                                            const __grid_constant__ CUtensorMap mapB) {
   __shared__ alignas(128) double ring[TMA_NST][TMA_PLANE];
   __shared__ uint64_t full[TMA_NST], empty[TMA_NST];
+  const double dx2 = g.dx * g.dx;
   constexpr int PN = 1 + DIR, PT1 = 1 + (DIR + 1) % 3, PT2 = 1 + (DIR + 2) % 3;
   // primitive field ids inside the box, in the sweep's local order (rho, u, v, w, p, B_t1, B_t2)
   constexpr int FQ[7] = {0, 1 + DIR, 1 + (DIR + 1) % 3, 1 + (DIR + 2) % 3, 4, 5 + (DIR + 1) % 3, 5 + (DIR + 2) % 3};
@@ -131,11 +132,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
   };
 
   double smax = 0.0, dtdx = 0.0;
-  if (APPLY) {
-    double dt = a.dt_fixed;
-    if (!(dt > 0.0)) dt = a.cfl / __longlong_as_double((long long)a.sc->smax_bits);
-    dtdx = dt / g.dx;
-  }
+  if (APPLY) dtdx = a.sc->dt_used / g.dx;  // published by the first stage's update kernel
   double dm[7], q0[7], WL[7], Bn, dummy;
   {
     double qm[7], qc[7];
@@ -145,7 +142,8 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
 #pragma unroll
     for (int n = 0; n < 7; ++n) {
       dm[n] = q0[n] - qc[n];
-      WL[n] = qc[n] + 0.5 * limited_slope<LIM>(qc[n] - qm[n], dm[n]);  // slope of cell s0-1
+      double lo_unused;
+      face_values<LIM>(qc[n], qc[n] - qm[n], dm[n], dx2, lo_unused, WL[n]);  // cell s0-1 at its upper face
     }
   }
   long long c = g.at(min(i, g.nx - 1), 0, 0) + (long long)min(t, a.nt - 1) * a.st + (long long)s0 * a.sd;
@@ -191,9 +189,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
 #pragma unroll
       for (int n = 0; n < 7; ++n) {
         const double dp = qp[n] - q0[n];
-        const double sl = limited_slope<LIM>(dm[n], dp);
-        WR[n] = q0[n] - 0.5 * sl;
-        WLn[n] = q0[n] + 0.5 * sl;
+        face_values<LIM>(q0[n], dm[n], dp, dx2, WR[n], WLn[n]);
         dm[n] = dp;
       }
       double F[7];
@@ -212,7 +208,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
         rt[4] = r_in[4] + (F[4] - Fp[4]);
 #pragma unroll
         for (int n = 0; n < 5; ++n) {
-          if (APPLY) a.Uout[n][cu] = 0.5 * u0[n] + 0.5 * (uin[n] - dtdx * rt[n]);  // Eq. 9, w2 = w2^0 = 1/2
+          if (APPLY) a.Uout[n][cu] = dtdx == 0.0 ? u0[n] : a.w0 * u0[n] + a.w * (uin[n] - dtdx * rt[n]);  // Eq. 9
           else a.R[n][cu] = rt[n];
         }
         if (WANT_DT) {
@@ -264,6 +260,7 @@ __global__ void __launch_bounds__(128, 4) k_flux_x_tma(Geom g, FluxXTArgs a, con
                                                        const __grid_constant__ CUtensorMap mapB) {
   __shared__ alignas(128) double ring[TX_NST][TX_PLANE];
   __shared__ uint64_t full[TX_NST], empty[TX_NST];
+  const double dx2 = g.dx * g.dx;
   constexpr int FQ[7] = {0, 1, 2, 3, 4, 6, 7};  // rho, vx, vy, vz, p, Bc_y, Bc_z
   const int lane = threadIdx.x & 31, row = threadIdx.x >> 5;
   const int f0 = 31 * blockIdx.x;
@@ -305,9 +302,9 @@ __global__ void __launch_bounds__(128, 4) k_flux_x_tma(Geom g, FluxXTArgs a, con
     for (int n = 0; n < 7; ++n) {
       const double* f = r + FQ[n] * (4 * TX_W) + so;
       const double qm = f[0], q = f[1], qp = f[2];
-      const double sl = limited_slope<LIM>(q - qm, qp - q);
-      WR[n] = q - 0.5 * sl;
-      WL[n] = __shfl_up_sync(0xffffffffu, q + 0.5 * sl, 1);
+      double up;
+      face_values<LIM>(q, q - qm, qp - q, dx2, WR[n], up);
+      WL[n] = __shfl_up_sync(0xffffffffu, up, 1);
     }
     const double Bn = r[TX_PLANE_V + so + 1];
     mbar_arrive(&empty[st]);

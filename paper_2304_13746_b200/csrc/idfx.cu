@@ -6,6 +6,7 @@
 // 16 doubles.  All fields live in the caller's workspace.
 #include <cuda_runtime.h>
 
+#include <cstddef>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -130,6 +131,17 @@ __device__ __forceinline__ void prim_from_cons(double gm1, double rho, double mx
 }
 
 // get_state: primitives from the master state into scratch fields (Bf ghosts are valid whenever this runs).
+// Optional pressure floor (off unless idfx_set_option_real sets it; the paper describes none, reading G13/G20): a pressure
+// below the floor is raised to it and the total energy rewritten to match.  Returns true when it acted.
+__device__ __forceinline__ bool pressure_floor(const Geom& g, DevScalars* sc, double rho, double vx, double vy, double vz,
+                                               double bx, double by, double bz, double& p, double& E) {
+  if (!(g.pfloor > 0.0) || !(p < g.pfloor)) return false;
+  p = g.pfloor;
+  E = p / (g.gamma - 1.0) + 0.5 * rho * (vx * vx + vy * vy + vz * vz) + 0.5 * (bx * bx + by * by + bz * bz);
+  atomicAdd(&sc->nfloor, 1ull);
+  return true;
+}
+
 // The stage-input primitives V are left untouched so that reading the state never perturbs the run.
 template <bool MHD>
 __global__ void k_prim_from_cons(Geom g, StateArgs a) {
@@ -145,6 +157,7 @@ __global__ void k_prim_from_cons(Geom g, StateArgs a) {
   double vx, vy, vz, p;
   const double rho = a.U[0][c];
   prim_from_cons(g.gamma - 1.0, rho, a.U[1][c], a.U[2][c], a.U[3][c], a.U[4][c], bx, by, bz, vx, vy, vz, p);
+  if (g.pfloor > 0.0 && p < g.pfloor) p = g.pfloor;  // a floored cell recomputes to the floor within rounding
   a.V[0][c] = rho;
   a.V[1][c] = vx;
   a.V[2][c] = vy;
@@ -172,15 +185,15 @@ __global__ void __launch_bounds__(128) k_flux_face(Geom g, FluxArgs a) {
   if (!cell_of_thread(g, i, j, k)) return;
   const long long c = g.at(i, j, k);
   constexpr int NQ = MHD ? 7 : 5;
+  const double dx2 = g.dx * g.dx;
   double WL[7], WR[7];
 #pragma unroll
   for (int n = 0; n < NQ; ++n) {
     const double* __restrict__ q = a.q[n];
     const double qm2 = q[c - 2 * a.sd], qm1 = q[c - a.sd], q0 = q[c], qp1 = q[c + a.sd];
-    const double sm = limited_slope<LIM>(qm1 - qm2, q0 - qm1);
-    const double s0 = limited_slope<LIM>(q0 - qm1, qp1 - q0);
-    WL[n] = qm1 + 0.5 * sm;
-    WR[n] = q0 - 0.5 * s0;
+    double lo_unused, hi_unused;
+    face_values<LIM>(qm1, qm1 - qm2, q0 - qm1, dx2, lo_unused, WL[n]);
+    face_values<LIM>(q0, q0 - qm1, qp1 - q0, dx2, WR[n], hi_unused);
   }
   if (!MHD) WL[5] = WL[6] = WR[5] = WR[6] = 0.0;
   const double Bn = MHD ? a.bn[c] : 0.0;  // G3
@@ -307,8 +320,13 @@ struct UpdateArgs {
   double* Bout[3];
   double* V[11];
   DevScalars* sc;
-  double dt_fixed;        // > 0: use it; otherwise dt = cfl / smax
+  const double* Ain[3];   // vector-potential form (Eq. 7-8): edge potential of the stage input, the saved one, the result,
+  const double* A0[3];
+  double* Aout[3];
+  const double* Bref[3];  // and the face field the potential is counted from (ghosts filled)
+  double dt_fixed;        // > 0: use it; otherwise dt = cfl / smax (first stage; later stages read sc->dt_used)
   double cfl;
+  double w, w0;           // Eq. 9: U_s = w U* + w0 U_0 (stages >= 2)
 };
 
 // Hydrodynamics: apply the flux divergence, RK2 combine, cons->prim.  (MHD uses k_ct_update below.)
@@ -317,19 +335,25 @@ __global__ void __launch_bounds__(128) k_update_hd(Geom g, UpdateArgs a) {
   int i, j, k;
   if (!cell_of_thread(g, i, j, k)) return;
   const long long c = g.at(i, j, k);
-  double dt = a.dt_fixed;
-  if (!(dt > 0.0)) dt = a.cfl / __longlong_as_double((long long)a.sc->smax_bits);
-  if (!STAGE2 && blockIdx.x == 0 && threadIdx.x == 0) a.sc->dt_used = dt;
+  double dt;
+  if (STAGE2) {
+    dt = a.sc->dt_used;
+  } else {
+    bool lands;
+    dt = first_stage_dt(a.sc, a.dt_fixed, a.cfl, lands);
+    if (blockIdx.x == 0 && threadIdx.x == 0) publish_dt(a.sc, dt, lands);
+  }
   const double dtdx = dt / g.dx;
   double u[5];
 #pragma unroll
   for (int n = 0; n < 5; ++n) {
     const double us = a.Uin[n][c] - dtdx * a.R[n][c];
-    u[n] = STAGE2 ? 0.5 * a.U0[n][c] + 0.5 * us : us;
+    u[n] = STAGE2 ? (dt == 0.0 ? a.U0[n][c] : a.w0 * a.U0[n][c] + a.w * us) : us;
     a.Uout[n][c] = u[n];
   }
   double vx, vy, vz, p;
   prim_from_cons(g.gamma - 1.0, u[0], u[1], u[2], u[3], u[4], 0.0, 0.0, 0.0, vx, vy, vz, p);
+  if (pressure_floor(g, a.sc, u[0], vx, vy, vz, 0.0, 0.0, 0.0, p, u[4])) a.Uout[4][c] = u[4];
   if (!(u[0] > 0.0) || !(p > 0.0)) a.sc->flag = 1;
   a.V[0][c] = u[0];
   a.V[1][c] = vx;
@@ -362,11 +386,22 @@ constexpr int CT_THREADS = CT_TX * CT_TY;
 #define IDFX_UNROLL(n) IDFX_PRAGMA_(unroll n)
 constexpr int CT_LX = CT_TX + 1, CT_LY = CT_TY + 1, CT_LZ = CT_TZ + 1;
 
-// UDONE: the conserved state was already combined by the z sweep (stage 2); only read it back for the primitives.
-template <int MODE, bool STAGE2, bool UDONE>
+// UDONE: the conserved state was already combined by the z sweep (stages >= 2); only read it back for the primitives.
+// VP: vector-potential form (Eq. 7-8): the lattice holds the new potential A = w (A_in - dt E) + w0 A_0 instead of E
+// and the face field is B_ref + curl A, so its divergence is one rounding of the face values at any time.
+template <int MODE, bool STAGE2, bool UDONE, bool VP>
 __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, EmfArgs ea, UpdateArgs a) {
   __shared__ double sE[3][CT_LZ][CT_LY][CT_LX];
   const int i0 = blockIdx.x * CT_TX, j0 = blockIdx.y * CT_TY, k0 = blockIdx.z * CT_TZ;
+  double dt;
+  if (STAGE2) {
+    dt = a.sc->dt_used;
+  } else {
+    bool lands;
+    dt = first_stage_dt(a.sc, a.dt_fixed, a.cfl, lands);
+    if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) publish_dt(a.sc, dt, lands);
+  }
+  const bool idle = STAGE2 && dt == 0.0;  // a cycle at t_end (idfx_advance_to ran past it): hand U_0 on unchanged
   // ---- phase 1: edge lattice ----
   IDFX_UNROLL(IDFX_CT_UNROLL)
   for (int p = threadIdx.x; p < CT_LZ * CT_LY * CT_LX; p += CT_THREADS) {
@@ -375,18 +410,26 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
     if (I > g.nx || J > g.ny || K > g.nz) continue;
     // periodic image of lattice index n is index 0
     const int idx[3] = {I == g.nx ? 0 : I, J == g.ny ? 0 : J, K == g.nz ? 0 : K};
-    if (li < CT_TX) sE[0][lk][lj][li] = edge_emf<MODE>(g, ea, idx, 0);
-    if (lj < CT_TY) sE[1][lk][lj][li] = edge_emf<MODE>(g, ea, idx, 1);
-    if (lk < CT_TZ) sE[2][lk][lj][li] = edge_emf<MODE>(g, ea, idx, 2);
+    const bool on[3] = {li < CT_TX, lj < CT_TY, lk < CT_TZ};
+    const bool owned = on[0] && on[1] && on[2] && I < g.nx && J < g.ny && K < g.nz;
+    const long long P = g.at(idx[0], idx[1], idx[2]);
+#pragma unroll
+    for (int comp = 0; comp < 3; ++comp) {
+      if (!on[comp]) continue;
+      double e = edge_emf<MODE>(g, ea, idx, comp);
+      if (VP) {
+        e = a.Ain[comp][P] - dt * e;  // Eq. 7
+        if (STAGE2) e = idle ? a.A0[comp][P] : a.w0 * a.A0[comp][P] + a.w * e;
+        if (owned) a.Aout[comp][P] = e;
+      }
+      sE[comp][lk][lj][li] = e;
+    }
   }
   __syncthreads();
   // ---- phase 2: one (i, j) column of TZ cells per thread ----
   const int li = threadIdx.x % CT_TX, lj = threadIdx.x / CT_TX;
   const int i = i0 + li, j = j0 + lj;
   if (i >= g.nx || j >= g.ny) return;
-  double dt = a.dt_fixed;
-  if (!(dt > 0.0)) dt = a.cfl / __longlong_as_double((long long)a.sc->smax_bits);
-  if (!STAGE2 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) a.sc->dt_used = dt;
   const double dtdx = dt / g.dx;
   const long long st[3] = {1, g.sy, g.sz};
   // ghost images of this column in x and y
@@ -404,7 +447,7 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
         u[n] = a.Uout[n][c];
       } else {
         const double us = a.Uin[n][c] - dtdx * a.R[n][c];
-        u[n] = STAGE2 ? 0.5 * a.U0[n][c] + 0.5 * us : us;
+        u[n] = STAGE2 ? (idle ? a.U0[n][c] : a.w0 * a.U0[n][c] + a.w * us) : us;
         a.Uout[n][c] = u[n];
       }
     }
@@ -420,11 +463,17 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
     double v[11];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-      double bl = a.Bin[d][c] - dtdx * curlL[d];
-      double br = a.Bin[d][c + st[d]] - dtdx * curlR[d];
-      if (STAGE2) {
-        bl = 0.5 * a.B0[d][c] + 0.5 * bl;
-        br = 0.5 * a.B0[d][c + st[d]] + 0.5 * br;
+      double bl, br;
+      if (VP) {
+        bl = a.Bref[d][c] + curlL[d] / g.dx;  // Eq. 8
+        br = a.Bref[d][c + st[d]] + curlR[d] / g.dx;
+      } else {
+        bl = a.Bin[d][c] - dtdx * curlL[d];  // Eq. 6
+        br = a.Bin[d][c + st[d]] - dtdx * curlR[d];
+        if (STAGE2) {
+          bl = idle ? a.B0[d][c] : a.w0 * a.B0[d][c] + a.w * bl;
+          br = idle ? a.B0[d][c + st[d]] : a.w0 * a.B0[d][c + st[d]] + a.w * br;
+        }
       }
       v[5 + d] = 0.5 * (bl + br);
       a.Bout[d][c] = bl;
@@ -438,6 +487,7 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
       }
     }
     prim_from_cons(g.gamma - 1.0, u[0], u[1], u[2], u[3], u[4], v[5], v[6], v[7], v[1], v[2], v[3], v[4]);
+    if (pressure_floor(g, a.sc, u[0], v[1], v[2], v[3], v[5], v[6], v[7], v[4], u[4])) a.Uout[4][c] = u[4];
     v[0] = u[0];
     v[8] = v[3] * v[6] - v[2] * v[7];
     v[9] = v[1] * v[7] - v[3] * v[5];
@@ -457,6 +507,14 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
         }
       }
     }
+  }
+}
+
+// First launch of every cycle: commits the time reached by the previous one and resets the dt reduction.
+__global__ void k_cycle_begin(DevScalars* sc) {
+  if (threadIdx.x == 0) {
+    sc->t = sc->t_next;
+    sc->smax_bits = 0ull;
   }
 }
 
@@ -482,7 +540,11 @@ enum {
   F_CFX = 57,  // 1: c_face of the x sweep
   F_SG = 58,   // 1 slot holding three byte fields: sign of the face mass flux of the x, y, z sweeps (E^c only)
   F_CS = 59,   // 1: sum_d c_d per cell (x and y parts)
-  F_COUNT = 60
+  F_COUNT = 60,
+  // vector-potential form only (idfx_set_option(IDFX_OPT_CT_FORM, IDFX_CT_POTENTIAL)):
+  F_AA = 60,   // 3 x 3: edge-potential buffers, rotating like the face-field buffers
+  F_BREF = 69, // 3: the face field given to set_state (ghosts filled)
+  F_COUNT_VP = 72
 };
 
 }  // namespace idfx
@@ -503,8 +565,14 @@ struct idfx_ctx {
   cudaStream_t stream = nullptr;
   bool bound = false;
   DevScalars* sc = nullptr;
+  int nstages = 2;  // Tab. 1: 1 Euler, 2 RK2, 3 RK3
+  bool vp = false;  // Eq. 7-8 instead of Eq. 6
+  int fixed_batch = 0;  // IDFX_ADVANCE_BATCH: cycles per batch of idfx_advance_to (tests: forces cycles past t_end)
+  int nfields() const { return vp ? F_COUNT_VP : F_COUNT; }
+  double* abuf(int which, int d) const { return field(F_AA + 3 * which + d); }
   int bcur = 0;  // which of the three face-field buffers holds the current state
   int vcur = 0;  // which primitive buffer holds the stage input
+  int graph_bnext[6] = {0, 0, 0, 0, 0, 0}, graph_vnext[6] = {0, 0, 0, 0, 0, 0};  // rotation state a replayed cycle leaves
   // one captured CUDA graph per buffer rotation state (3 face-field rotations x 2 primitive buffers)
   cudaGraphExec_t graph[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   long long graph_launches[6] = {0, 0, 0, 0, 0, 0};
@@ -670,10 +738,12 @@ void launch_speed(idfx_ctx* c, int d, const double* const Bf[3]) {
   if (c->mhd) {
     if (c->limiter == LIM_FLAT) launch_speed_l<LIM_FLAT, true>(c, a);
     else if (c->limiter == LIM_MINMOD) launch_speed_l<LIM_MINMOD, true>(c, a);
+    else if (c->limiter == LIM_LIMO3) launch_speed_l<LIM_LIMO3, true>(c, a);
     else launch_speed_l<LIM_VANLEER, true>(c, a);
   } else {
     if (c->limiter == LIM_FLAT) launch_speed_l<LIM_FLAT, false>(c, a);
     else if (c->limiter == LIM_MINMOD) launch_speed_l<LIM_MINMOD, false>(c, a);
+    else if (c->limiter == LIM_LIMO3) launch_speed_l<LIM_LIMO3, false>(c, a);
     else launch_speed_l<LIM_VANLEER, false>(c, a);
   }
 }
@@ -716,8 +786,9 @@ void launch_march_tma(idfx_ctx* c, int d, dim3 grid, const FluxTArgs& ta, bool w
 
 // ---- the three flux sweeps of one stage --------------------------------------------------------
 struct ApplyInfo {
-  bool on;  // stage 2 with the TMA sweeps: the z sweep applies the divergence and the RK2 combine itself
-  double dt_fixed, cfl;
+  bool on;  // stages >= 2 with the TMA sweeps: the z sweep applies the divergence and the RK combine itself
+  double w, w0;
+  int uin, uout;  // first slots of the stage-input and result conserved fields
 };
 
 template <int SOLVER, int LIM, bool MHD>
@@ -808,12 +879,12 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const
       for (int n = 0; n < 5; ++n) { ta.FX[n] = a.FX[n]; ta.R[n] = a.R[n]; }
       ta.cfx = a.cfx; ta.csum = a.csum; ta.FB[0] = a.FB[0]; ta.FB[1] = a.FB[1]; ta.SG = a.SG; ta.sc = a.sc;
       for (int n = 0; n < 5; ++n) {
-        ta.Uin[n] = c->field(F_UB + n);
+        ta.Uin[n] = c->field(ap.uin + n);
         ta.U0[n] = c->field(F_UA + n);
-        ta.Uout[n] = c->field(F_UA + n);
+        ta.Uout[n] = c->field(ap.uout + n);
       }
-      ta.dt_fixed = ap.dt_fixed;
-      ta.cfl = ap.cfl;
+      ta.w = ap.w;
+      ta.w0 = ap.w0;
       launch_march_tma<SOLVER, LIM, MHD>(c, d, grid, ta, want_dt, uct, ap.on && d == 2);
       continue;
     }
@@ -834,6 +905,7 @@ void launch_sweeps_s(idfx_ctx* c, const double* const Bf[3], bool want_dt, const
   switch (c->limiter) {
     case LIM_FLAT: launch_sweeps_t<SOLVER, LIM_FLAT, MHD>(c, Bf, want_dt, ap); break;
     case LIM_MINMOD: launch_sweeps_t<SOLVER, LIM_MINMOD, MHD>(c, Bf, want_dt, ap); break;
+    case LIM_LIMO3: launch_sweeps_t<SOLVER, LIM_LIMO3, MHD>(c, Bf, want_dt, ap); break;
     default: launch_sweeps_t<SOLVER, LIM_VANLEER, MHD>(c, Bf, want_dt, ap);
   }
 }
@@ -876,34 +948,52 @@ void launch_fill(idfx_ctx* c, int which_b) {
   k_fill_ghost<<<blocks_for(nt, 128), 128, 0, c->stream>>>(g, fl);
 }
 
-template <int MODE>
-void launch_ct(idfx_ctx* c, dim3 grid, const EmfArgs& ea, const UpdateArgs& a, bool stage2, bool udone) {
-  if (udone) k_ct_update<MODE, true, true><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
-  else if (stage2) k_ct_update<MODE, true, false><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
-  else k_ct_update<MODE, false, false><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
+template <int MODE, bool VP>
+void launch_ct_v(idfx_ctx* c, dim3 grid, const EmfArgs& ea, const UpdateArgs& a, bool stage2, bool udone) {
+  if (udone) k_ct_update<MODE, true, true, VP><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
+  else if (stage2) k_ct_update<MODE, true, false, VP><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
+  else k_ct_update<MODE, false, false, VP><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
 }
 
-// One stage S_dt (O2) followed by the RK combine.  bin: face buffer of the stage input; b0: saved face
-// buffer; bout: destination.
-void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fixed, double cfl, bool want_dt) {
+template <int MODE>
+void launch_ct(idfx_ctx* c, dim3 grid, const EmfArgs& ea, const UpdateArgs& a, bool stage2, bool udone) {
+  if (c->vp) launch_ct_v<MODE, true>(c, grid, ea, a, stage2, udone);
+  else launch_ct_v<MODE, false>(c, grid, ea, a, stage2, udone);
+}
+
+// One stage S_dt (O2) followed by the RK combine of Eq. 9.  s: stage index (0-based); bin: face buffer of the stage
+// input; b0: saved face buffer; bout: destination.  Conserved fields: U_0 lives in F_UA for the whole cycle, the
+// intermediate stages in F_UB, the last stage writes the result back to F_UA.
+void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, double cfl, bool want_dt) {
+  static const double W[3][3] = {{1.0, 0.0, 0.0}, {1.0, 0.5, 0.0}, {1.0, 0.25, 2.0 / 3.0}};      // Tab. 1
+  static const double W0[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.5, 0.0}, {0.0, 0.75, 1.0 / 3.0}};
+  const bool combine = s > 0, last = s == c->nstages - 1;
+  const int uin = s == 0 ? F_UA : F_UB, uout = last ? F_UA : F_UB;
+  const double w = W[c->nstages - 1][s], w0 = W0[c->nstages - 1][s];
   const double* Bf[3] = {c->bbuf(bin, 0), c->bbuf(bin, 1), c->bbuf(bin, 2)};
-  const ApplyInfo ap = {stage2 && c->mhd && c->use_tma, dt_fixed, cfl};
+  const ApplyInfo ap = {combine && c->mhd && c->use_tma, w, w0, uin, uout};
   launch_sweeps(c, Bf, want_dt, ap);
   UpdateArgs a;
   for (int n = 0; n < 5; ++n) {
-    a.Uin[n] = c->field((stage2 ? F_UB : F_UA) + n);
+    a.Uin[n] = c->field(uin + n);
     a.U0[n] = c->field(F_UA + n);
     a.R[n] = c->field(F_R + n);
-    a.Uout[n] = c->field((stage2 ? F_UA : F_UB) + n);
+    a.Uout[n] = c->field(uout + n);
   }
   for (int d = 0; d < 3; ++d) {
     a.Bin[d] = c->bbuf(bin, d);
     a.B0[d] = c->bbuf(b0, d);
     a.Bout[d] = c->bbuf(bout, d);
+    a.Ain[d] = c->vp ? c->abuf(bin, d) : nullptr;
+    a.A0[d] = c->vp ? c->abuf(b0, d) : nullptr;
+    a.Aout[d] = c->vp ? c->abuf(bout, d) : nullptr;
+    a.Bref[d] = c->vp ? c->field(F_BREF + d) : nullptr;
   }
   a.sc = c->sc;
   a.dt_fixed = dt_fixed;
   a.cfl = cfl;
+  a.w = w;
+  a.w0 = w0;
   const Geom& g = c->g;
   if (c->mhd) {
     // edge EMFs + CT + RK combine + cons->prim + ghost images in one kernel; V is double-buffered because the
@@ -911,31 +1001,39 @@ void run_stage(idfx_ctx* c, bool stage2, int bin, int b0, int bout, double dt_fi
     const EmfArgs ea = emf_args(c);
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield_out(n);
     dim3 grid((g.nx + CT_TX - 1) / CT_TX, (g.ny + CT_TY - 1) / CT_TY, (g.nz + CT_TZ - 1) / CT_TZ);
-    const bool udone = stage2 && c->use_tma;  // the TMA z sweep of stage 2 applied the divergence itself
+    const bool udone = ap.on;  // the TMA z sweep applied the divergence itself
     LaunchScope ls(c, K_UPDATE);
-    if (c->emf == EMF_UCT) launch_ct<EMF_UCT>(c, grid, ea, a, stage2, udone);
-    else if (c->emf == EMF_UCT0) launch_ct<EMF_UCT0>(c, grid, ea, a, stage2, udone);
-    else launch_ct<EMF_ARITH>(c, grid, ea, a, stage2, udone);
+    if (c->emf == EMF_UCT) launch_ct<EMF_UCT>(c, grid, ea, a, combine, udone);
+    else if (c->emf == EMF_UCT0) launch_ct<EMF_UCT0>(c, grid, ea, a, combine, udone);
+    else launch_ct<EMF_ARITH>(c, grid, ea, a, combine, udone);
     c->vcur ^= 1;
   } else {
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield(n);
     {
       LaunchScope ls(c, K_UPDATE);
-      if (stage2) k_update_hd<true><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
+      if (combine) k_update_hd<true><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
       else k_update_hd<false><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
     }
     launch_fill(c, bout);
   }
 }
 
-// One RK2 cycle.  dt_fixed > 0: that dt; otherwise dt = cfl / max found by stage 1 (never leaves the device).
+// One cycle of the integrator.  dt_fixed > 0: that dt; otherwise dt = cfl / max found by stage 1, shortened to land on
+// t_end (never leaves the device).
 int run_cycle(idfx_ctx* c, double dt_fixed, double cfl) {
   const bool want_dt = !(dt_fixed > 0.0);
-  if (want_dt) CK(cudaMemsetAsync(&c->sc->smax_bits, 0, sizeof(unsigned long long), c->stream));
+  {
+    LaunchScope ls(c, K_STATE);
+    k_cycle_begin<<<1, 32, 0, c->stream>>>(c->sc);
+  }
   const int b0 = c->bcur, b1 = (c->bcur + 1) % 3, b2 = (c->bcur + 2) % 3;
-  run_stage(c, false, b0, b0, b1, dt_fixed, cfl, want_dt);
-  run_stage(c, true, b1, b0, b2, dt_fixed, cfl, false);
-  c->bcur = b2;
+  int bin = b0;
+  for (int s = 0; s < c->nstages; ++s) {
+    const int bout = bin == b1 ? b2 : b1;  // never b0 (saved) and never the stage input
+    run_stage(c, s, bin, b0, bout, dt_fixed, cfl, want_dt && s == 0);
+    bin = bout;
+  }
+  c->bcur = bin;
   CK(cudaGetLastError());
   return IDFX_OK;
 }
@@ -958,6 +1056,17 @@ int copy3d(idfx_ctx* c, double* field, const double* contig_in, double* contig_o
   return IDFX_OK;
 }
 
+// t = 0, no target time, no cycles counted; the sticky error flag and the dt scalars are left alone
+int reset_clock(idfx_ctx* c) {
+  DevScalars h;
+  memset(&h, 0, sizeof(h));
+  h.t_end = INFINITY;
+  const size_t off = offsetof(DevScalars, t);
+  // pageable source: staged before the call returns
+  CK(cudaMemcpyAsync((char*)c->sc + off, (const char*)&h + off, sizeof(h) - off, cudaMemcpyHostToDevice, c->stream));
+  return IDFX_OK;
+}
+
 // after the primitives (V[0..4]) and the face field (current buffer, active part) are in place
 int finish_set_state(idfx_ctx* c) {
   StateArgs a;
@@ -972,7 +1081,12 @@ int finish_set_state(idfx_ctx* c) {
   }
   launch_fill(c, c->bcur);
   CK(cudaGetLastError());
-  return IDFX_OK;
+  if (c->vp) {  // G19: the potential is counted from this state on
+    const size_t fb = (size_t)c->g.np * sizeof(double);
+    CK(cudaMemsetAsync(c->field(F_AA), 0, 9 * fb, c->stream));
+    CK(cudaMemcpyAsync(c->field(F_BREF), c->bbuf(c->bcur, 0), 3 * fb, cudaMemcpyDeviceToDevice, c->stream));
+  }
+  return reset_clock(c);
 }
 
 int refresh_prims(idfx_ctx* c) {
@@ -1009,7 +1123,7 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
     set_err("idfx_create: need dx > 0 and gamma > 1");
     return nullptr;
   }
-  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 2 || emf_mode < 0 || emf_mode > 3) {
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 3 || emf_mode < 0 || emf_mode > 3) {
     set_err("idfx_create: unknown solver, limiter or emf_mode");
     return nullptr;
   }
@@ -1026,6 +1140,7 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
   g.nz = nz;
   g.dx = dx;
   g.gamma = gamma;
+  g.pfloor = 0.0;
   g.sy = ((nx + IOFF + NG + 15) / 16) * 16;
   g.sz = (long long)g.sy * (ny + 2 * NG);
   g.np = ((g.sz * (nz + 2 * NG) + 31) / 32) * 32;
@@ -1039,7 +1154,7 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
 
 size_t idfx_workspace_bytes(const idfx_ctx* c) {
   if (!c) return 0;
-  return (size_t)F_COUNT * (size_t)c->g.np * sizeof(double) + 256;
+  return (size_t)c->nfields() * (size_t)c->g.np * sizeof(double) + 256;
 }
 
 int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
@@ -1054,16 +1169,19 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
   c->ws = (double*)d_workspace;
   c->ws_bytes = bytes;
   c->stream = (cudaStream_t)cuda_stream;
-  c->sc = (DevScalars*)(c->ws + (size_t)F_COUNT * (size_t)c->g.np);
+  c->sc = (DevScalars*)(c->ws + (size_t)c->nfields() * (size_t)c->g.np);
   c->bcur = 0;
   c->vcur = 0;
   c->launches = 0;
   CK(cudaMemsetAsync(d_workspace, 0, idfx_workspace_bytes(c), c->stream));
+  if (int rc = reset_clock(c)) return rc;
   drop_graphs(c);
   const char* genv = getenv("IDFX_GRAPH");
   // the legacy default stream cannot be captured: graphs only on a stream of the caller's own
   c->use_graph = !(genv && genv[0] == '0') && c->stream != nullptr && c->stream != cudaStreamLegacy &&
                  c->stream != cudaStreamPerThread;
+  const char* benv = getenv("IDFX_ADVANCE_BATCH");
+  c->fixed_batch = benv ? atoi(benv) : 0;
   const char* env = getenv("IDFX_TMA");
   c->use_tma = c->mhd && !(env && env[0] == '0');  // IDFX_TMA=0 selects the register-prefetch sweeps (A/B only)
   if (c->use_tma) {
@@ -1216,13 +1334,9 @@ int idfx_step(idfx_ctx* c, double dt) {
   return run_cycle(c, dt, 0.0);
 }
 
-int idfx_advance(idfx_ctx* c, int nsteps, double cfl) {
-  int rc = check_bound(c);
-  if (rc) return rc;
-  if (nsteps < 0 || !(cfl > 0.0) || !(cfl < 1.0)) {
-    set_err("idfx_advance: need nsteps >= 0 and 0 < cfl < 1");
-    return IDFX_ERR_INVALID_ARG;
-  }
+// nsteps cycles with the CFL step, replayed from CUDA graphs where possible
+static int advance_cycles(idfx_ctx* c, int nsteps, double cfl) {
+  int rc;
   if (c->graph_cfl != cfl) {
     drop_graphs(c);
     c->graph_cfl = cfl;
@@ -1232,8 +1346,8 @@ int idfx_advance(idfx_ctx* c, int nsteps, double cfl) {
       if ((rc = run_cycle(c, 0.0, cfl))) return rc;
       continue;
     }
-    // the cycle is a fixed sequence of 8 kernels + 1 memset whose arguments depend only on the buffer rotation
-    // state: capture it once per state, then replay (dt never leaves the device, so nothing else varies)
+    // the cycle is a fixed sequence of kernels whose arguments depend only on the buffer rotation state: capture it
+    // once per state, then replay (dt and the clock never leave the device, so nothing else varies)
     const int key = c->bcur * 2 + c->vcur;
     if (!c->graph[key]) {
       const int b = c->bcur, v = c->vcur;
@@ -1250,13 +1364,142 @@ int idfx_advance(idfx_ctx* c, int nsteps, double cfl) {
       cudaGraphDestroy(gr);
       c->graph_launches[key] = c->launches - l0;
       c->launches = l0;  // nothing ran during capture
+      c->graph_bnext[key] = c->bcur;
+      c->graph_vnext[key] = c->vcur;
       c->bcur = b;
       c->vcur = v;
     }
     CK(cudaGraphLaunch(c->graph[key], c->stream));
     c->launches += c->graph_launches[key];
-    c->bcur = (c->bcur + 2) % 3;  // as run_cycle leaves it; vcur toggles twice per cycle
+    c->bcur = c->graph_bnext[key];  // as run_cycle leaves them
+    c->vcur = c->graph_vnext[key];
   }
+  return IDFX_OK;
+}
+
+static int read_scalars(idfx_ctx* c, DevScalars* h) {
+  CK(cudaMemcpyAsync(h, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return IDFX_OK;
+}
+
+int idfx_advance(idfx_ctx* c, int nsteps, double cfl) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (nsteps < 0 || !(cfl > 0.0) || !(cfl < 1.0)) {
+    set_err("idfx_advance: need nsteps >= 0 and 0 < cfl < 1");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  return advance_cycles(c, nsteps, cfl);
+}
+
+int idfx_advance_to(idfx_ctx* c, double t_end, double cfl, int max_steps, int* h_nsteps_out, double* h_t_out) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (max_steps < 0 || !(cfl > 0.0) || !(cfl < 1.0) || !(t_end == t_end)) {
+    set_err("idfx_advance_to: need max_steps >= 0, 0 < cfl < 1 and a t_end that is not NaN");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  DevScalars h;
+  if ((rc = read_scalars(c, &h))) return rc;
+  const long long n0 = h.ncycles;
+  CK(cudaMemcpyAsync(&c->sc->t_end, &t_end, sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  long long done = 0;
+  double dt_last = 0.0;
+  while (h.t_next < t_end && done < max_steps) {
+    // batch size: most of the cycles the last dt says are left, at least one, never past max_steps
+    long long batch = dt_last > 0.0 ? (long long)(0.9 * (t_end - h.t_next) / dt_last) : 1;
+    batch = batch < 1 ? 1 : (batch > 64 ? 64 : batch);
+    if (c->fixed_batch > 0) batch = c->fixed_batch;
+    if (batch > max_steps - done) batch = max_steps - done;
+    if ((rc = advance_cycles(c, (int)batch, cfl))) break;
+    if ((rc = read_scalars(c, &h))) break;
+    if (h.flag) break;  // unphysical state: idfx_status reports it
+    done = h.ncycles - n0;
+    dt_last = h.dt_used;
+    if (!(dt_last > 0.0) && h.t_next < t_end) break;  // cannot progress (dt = 0 or NaN)
+  }
+  const double inf = INFINITY;
+  cudaMemcpyAsync(&c->sc->t_end, &inf, sizeof(double), cudaMemcpyHostToDevice, c->stream);
+  if (h_nsteps_out) *h_nsteps_out = (int)done;
+  if (h_t_out) *h_t_out = h.t_next;
+  return rc;
+}
+
+int idfx_time(idfx_ctx* c, double* h_t_out) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!h_t_out) return IDFX_ERR_INVALID_ARG;
+  DevScalars h;
+  if ((rc = read_scalars(c, &h))) return rc;
+  *h_t_out = h.t_next;
+  return IDFX_OK;
+}
+
+int idfx_set_option(idfx_ctx* c, int option, int value) {
+  if (!c) {
+    set_err("null context");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  if (option == 0 /* IDFX_OPT_INTEGRATOR */ && value >= 1 && value <= 3) {
+    if (value != c->nstages) drop_graphs(c);
+    c->nstages = value;
+    return IDFX_OK;
+  }
+  if (option == 1 /* IDFX_OPT_CT_FORM */ && (value == 0 || value == 1)) {
+    if (c->bound) {
+      set_err("idfx_set_option: the CT form must be chosen before idfx_bind");
+      return IDFX_ERR_INVALID_ARG;
+    }
+    if (value == 1 && !c->mhd) {
+      set_err("idfx_set_option: the vector-potential form needs a magnetic field");
+      return IDFX_ERR_UNSUPPORTED;
+    }
+    c->vp = value == 1;
+    return IDFX_OK;
+  }
+  set_err("idfx_set_option: unknown option or value");
+  return IDFX_ERR_INVALID_ARG;
+}
+
+int idfx_set_option_real(idfx_ctx* c, int option, double value) {
+  if (!c) {
+    set_err("null context");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  if (option == 2 /* IDFX_OPT_PRESSURE_FLOOR */ && value >= 0.0) {
+    if (value != c->g.pfloor) drop_graphs(c);  // kernel arguments are baked into the captured cycles
+    c->g.pfloor = value;
+    return IDFX_OK;
+  }
+  set_err("idfx_set_option_real: unknown option or value");
+  return IDFX_ERR_INVALID_ARG;
+}
+
+int idfx_floor_count(idfx_ctx* c, long long* h_count_out) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!h_count_out) return IDFX_ERR_INVALID_ARG;
+  DevScalars h;
+  if ((rc = read_scalars(c, &h))) return rc;
+  *h_count_out = (long long)h.nfloor;
+  return IDFX_OK;
+}
+
+int idfx_get_potential(idfx_ctx* c, double* d_pot) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if (!c->vp || !d_pot) {
+    set_err("idfx_get_potential: needs IDFX_CT_POTENTIAL and a non-null output");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  FieldList fl;
+  fl.n = 3;
+  for (int d = 0; d < 3; ++d) fl.f[d] = c->abuf(c->bcur, d);
+  { LaunchScope ls(c, K_STATE);
+  k_unpack<<<blocks_for(c->g.nc, 128), 128, 0, c->stream>>>(c->g, fl, d_pot);
+  }
+  CK(cudaGetLastError());
   return IDFX_OK;
 }
 

@@ -14,7 +14,7 @@
 namespace idfx {
 
 enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_RUSANOV = 4 };
-enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2 };
+enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3 };
 enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3 };
 
 #define IDFX_DEV __device__ __forceinline__
@@ -81,6 +81,37 @@ IDFX_DEV double limited_slope(double dm, double dp) {
   } else {
     const double s = (fabs(dm) < fabs(dp)) ? dm : dp;
     return (prod > 0.0) ? s : 0.0;
+  }
+}
+
+// LimO3 (Cada & Torrilhon 2009; reading G18): phi(theta) * dplus with theta = dminus/dplus,
+// written without the division: with s = sign(dplus), a = |dplus|, b = s dminus and P = (2a + b)/3,
+//   limited = s max(0, min(P, max(-b/2, min(2b, P, 1.6 a)))),  unlimited = (2 dplus + dminus)/3,
+// the unlimited value where eta = (dminus^2 + dplus^2)/dx^2 < 1 (smooth data), a linear blend within 1e-12 of eta = 1.
+IDFX_DEV double limo3_increment(double dminus, double dplus, double dx2) {
+  const double unl = (2.0 * dplus + dminus) * (1.0 / 3.0);
+  const double a = fabs(dplus), b = dplus < 0.0 ? -dminus : dminus;
+  const double P = (2.0 * a + b) * (1.0 / 3.0);
+  const double l = fmax(0.0, fmin(P, fmax(-0.5 * b, fmin(fmin(2.0 * b, P), 1.6 * a))));
+  const double lim = dplus < 0.0 ? -l : l;
+  const double num = dminus * dminus + dplus * dplus;
+  const double eps = 1e-12;
+  if (num <= (1.0 - eps) * dx2) return unl;
+  if (num >= (1.0 + eps) * dx2) return lim;
+  const double x = (num / dx2 - 1.0) / eps;  // rare: the blend zone
+  return 0.5 * ((1.0 - x) * unl + (1.0 + x) * lim);
+}
+
+// S2: values of cell i's reconstruction at its lower and upper faces; dm = q_i - q_{i-1}, dp = q_{i+1} - q_i.
+template <int LIM>
+IDFX_DEV void face_values(double q, double dm, double dp, double dx2, double& lower, double& upper) {
+  if (LIM == LIM_LIMO3) {
+    upper = q + 0.5 * limo3_increment(dm, dp, dx2);
+    lower = q - 0.5 * limo3_increment(dp, dm, dx2);
+  } else {
+    const double s = limited_slope<LIM>(dm, dp);
+    lower = q - 0.5 * s;
+    upper = q + 0.5 * s;
   }
 }
 

@@ -10,7 +10,9 @@ import os
 import torch
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
-LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER = 0, 1, 2
+LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3 = 0, 1, 2, 3
+OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR = 0, 1, 2
+CT_FACE, CT_POTENTIAL = 0, 1
 EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0 = 0, 1, 2, 3
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_NOT_BOUND, ERR_CUDA, ERR_UNPHYSICAL = 0, -1, -2, -3, -4, -5
 
@@ -23,6 +25,7 @@ SYMBOLS = (
     "idfx_get_state", "idfx_get_state_host", "idfx_get_conserved", "idfx_compute_dt", "idfx_step",
     "idfx_advance", "idfx_last_dt", "idfx_status", "idfx_launch_count", "idfx_last_error", "idfx_destroy",
     "idfx_profile_enable", "idfx_profile_read", "idfx_profile_kernel_name",
+    "idfx_set_option", "idfx_advance_to", "idfx_time", "idfx_get_potential", "idfx_set_option_real", "idfx_floor_count",
     "idfx_probe_fp64",
 )
 
@@ -55,6 +58,12 @@ def lib():
         L.idfx_step.argtypes = [vp, cd]
         L.idfx_advance.argtypes = [vp, ci, cd]
         L.idfx_last_dt.argtypes = [vp, dp]
+        L.idfx_set_option.argtypes = [vp, ci, ci]
+        L.idfx_advance_to.argtypes = [vp, cd, cd, ci, ctypes.POINTER(ci), dp]
+        L.idfx_time.argtypes = [vp, dp]
+        L.idfx_get_potential.argtypes = [vp, vp]
+        L.idfx_set_option_real.argtypes = [vp, ci, cd]
+        L.idfx_floor_count.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong)]
         L.idfx_status.argtypes = [vp]
         L.idfx_launch_count.argtypes = [vp]
         L.idfx_launch_count.restype = ctypes.c_longlong
@@ -87,11 +96,18 @@ def probe_fp64(repeats=5):
 class Idfx:
     """One periodic nx*ny*nz box on one GPU.  Tensors are float64, [var][nz][ny][nx]."""
 
-    def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode, device="cuda:0", stream=None):
+    def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode, device="cuda:0", stream=None, nstages=2,
+                 ct_form=CT_FACE, pressure_floor=0.0):
         self.L = lib()
         self.h = self.L.idfx_create(nx, ny, nz, dx, gamma, solver, limiter, emf_mode)
         if not self.h:
             raise IdfxError(ERR_INVALID_ARG, self.L.idfx_last_error().decode())
+        if nstages != 2:
+            _check(self.L.idfx_set_option(self.h, OPT_INTEGRATOR, nstages))
+        if ct_form != CT_FACE:
+            _check(self.L.idfx_set_option(self.h, OPT_CT_FORM, ct_form))
+        if pressure_floor:
+            _check(self.L.idfx_set_option_real(self.h, OPT_PRESSURE_FLOOR, pressure_floor))
         if not torch.cuda.is_available():
             raise RuntimeError("idfx needs a CUDA device; there is no CPU fallback")
         self.device = torch.device(device)
@@ -178,6 +194,32 @@ class Idfx:
     def advance(self, nsteps, cfl):
         with self._ordered():
             _check(self.L.idfx_advance(self.h, nsteps, cfl))
+
+    def set_integrator(self, nstages):
+        _check(self.L.idfx_set_option(self.h, OPT_INTEGRATOR, nstages))
+
+    def advance_to(self, t_end, cfl, max_steps=(1 << 31) - 1):
+        """Returns (number of cycles taken, time reached)."""
+        n, t = ctypes.c_int(), ctypes.c_double()
+        with self._ordered():
+            _check(self.L.idfx_advance_to(self.h, t_end, cfl, max_steps, ctypes.byref(n), ctypes.byref(t)))
+        return n.value, t.value
+
+    def floor_count(self):
+        n = ctypes.c_longlong()
+        _check(self.L.idfx_floor_count(self.h, ctypes.byref(n)))
+        return n.value
+
+    def time(self):
+        t = ctypes.c_double()
+        _check(self.L.idfx_time(self.h, ctypes.byref(t)))
+        return t.value
+
+    def get_potential(self):
+        pot = torch.empty((3,) + self.shape, dtype=torch.float64, device=self.device)
+        with self._ordered():
+            _check(self.L.idfx_get_potential(self.h, pot.data_ptr()))
+        return pot
 
     def last_dt(self):
         dt = ctypes.c_double()

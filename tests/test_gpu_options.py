@@ -1,0 +1,160 @@
+"""Parity of the CUDA path against the oracle for the optional parts: Euler / RK3 (Tab. 1), the
+LimO3 reconstruction, the vector-potential form of CT (Eq. 7-8), idfx_advance_to, and the paper's 3D Orszag-Tang run
+(PAPER.md:346).  Same bar as tests/test_gpu_parity.py: 1e-10 relative on the conserved variables and the face field,
+1e-12 on dt and on the time reached."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2304_13746_b200 import inputs
+from test_gpu_parity import (EMF_ARITH, EMF_NONE, EMF_UCT, EMF_UCT0, HLL, HLLC, HLLD, MINMOD, ROE, TOL, TOL_DT, VANLEER,
+                             assert_state_close, idfx, smooth_ic)  # noqa: F401  (idfx is a fixture)
+
+pytestmark = pytest.mark.gpu
+
+LIMO3 = 3
+G53 = 5.0 / 3.0
+
+
+def pair(idfx, R, shape, dx, solver, limiter, emf, prim, b, nstages=2, ct_form=0):
+    nx, ny, nz = shape
+    sim = idfx.Idfx(nx, ny, nz, dx, G53, solver, limiter, emf, nstages=nstages, ct_form=ct_form)
+    sim.set_state(torch.from_numpy(prim).cuda(), None if b is None else torch.from_numpy(b).cuda())
+    ref = R.Oracle(nx, ny, nz, dx, G53, solver, limiter, emf, nstages=nstages, ct_form=ct_form)
+    ref.set_state(prim, b)
+    return sim, ref
+
+
+OPTION_COMBOS = [
+    # solver, limiter, emf, stages, CT form
+    (HLLD, VANLEER, EMF_UCT, 3, 0), (HLLD, LIMO3, EMF_UCT, 3, 0), (HLLD, LIMO3, EMF_UCT, 2, 0), (ROE, LIMO3, EMF_ARITH, 3, 0),
+    (HLL, LIMO3, EMF_UCT0, 1, 0), (HLLD, VANLEER, EMF_UCT, 1, 0), (HLLC, LIMO3, EMF_NONE, 3, 0), (HLL, MINMOD, EMF_NONE, 1, 0),
+    (ROE, LIMO3, EMF_NONE, 2, 0),
+    (HLLD, VANLEER, EMF_UCT, 2, 1), (HLLD, LIMO3, EMF_UCT, 3, 1), (ROE, VANLEER, EMF_ARITH, 1, 1), (HLL, MINMOD, EMF_UCT0, 3, 1),
+]
+
+
+@pytest.mark.parametrize("solver,limiter,emf,nstages,ct_form", OPTION_COMBOS)
+def test_option_combinations_ragged_box(idfx, R, solver, limiter, emf, nstages, ct_form):
+    nx, ny, nz = 37, 21, 13
+    prim, b, dx = smooth_ic(nx, ny, nz, 23, emf != EMF_NONE)
+    sim, ref = pair(idfx, R, (nx, ny, nz), dx, solver, limiter, emf, prim, b, nstages, ct_form)
+    for s in range(4):
+        sim.advance(1, 0.35)
+        ref.advance(1, 0.35)
+        assert abs(sim.last_dt() - ref.last_dt()) <= TOL_DT * ref.last_dt()
+        assert_state_close(sim, ref, TOL, "step %d" % s)
+    assert sim.status() == 0 and ref.status() == 0
+    assert abs(sim.time() - ref.time()) <= TOL_DT * ref.time()
+    if ct_form == 1:
+        a_g, a_r = sim.get_potential().cpu().numpy(), ref.get_potential()
+        assert np.abs(a_g - a_r).max() <= TOL * np.abs(a_r).max()
+
+
+def test_limo3_on_steep_data(idfx, R):
+    """Random-phase Mach-1 turbulence at 40^3 after a few cycles has cells on both sides of the LimO3 smoothness switch
+    (eta = 1) and at its limited branches; the two implementations (theta form / division-free form) must agree."""
+    prim, b, cfg = inputs.make("config3", n=40)
+    sim, ref = pair(idfx, R, (40, 40, 40), cfg["dx"], HLLD, LIMO3, EMF_UCT, prim.numpy(), b.numpy(), 3, 0)
+    sim.advance(6, 0.3)
+    ref.advance(6, 0.3)
+    assert_state_close(sim, ref, TOL, "config3 recipe, LimO3 + RK3")
+    p = ref.get_state()[0]
+    d = np.diff(p[0], axis=2)
+    eta = (d[:, :, 1:] ** 2 + d[:, :, :-1] ** 2) / cfg["dx"] ** 2
+    assert (eta > 1).any() and (eta < 1).any()      # both branches were exercised
+
+
+@pytest.mark.parametrize("ct_form", [0, 1])
+def test_advance_to_matches_the_oracle(idfx, R, ct_form):
+    nx, ny, nz = 24, 20, 16
+    prim, b, dx = smooth_ic(nx, ny, nz, 5)
+    sim, ref = pair(idfx, R, (nx, ny, nz), dx, HLLD, VANLEER, EMF_UCT, prim, b, 2, ct_form)
+    t_end = 7.3 * ref.compute_dt(0.3)
+    n_g, t_g = sim.advance_to(t_end, 0.3)
+    rc, n_r = ref.advance_to(t_end, 0.3)
+    assert rc == 0 and n_g == n_r and t_g == t_end == ref.time() == sim.time()
+    assert_state_close(sim, ref, TOL, "advance_to")
+    # already there: nothing happens; max_steps stops early
+    before = [x.clone() for x in sim.get_conserved()]
+    assert sim.advance_to(t_end, 0.3) == (0, t_end)
+    for x, y in zip(before, sim.get_conserved()):
+        assert torch.equal(x, y)
+    sim.set_state(torch.from_numpy(prim).cuda(), torch.from_numpy(b).cuda())
+    n, t = sim.advance_to(t_end, 0.3, max_steps=3)
+    assert n == 3 and 0.0 < t < t_end
+
+
+@pytest.mark.parametrize("nstages", [2, 3])
+def test_cycles_enqueued_past_t_end_change_nothing(idfx, nstages, monkeypatch):
+    """idfx_advance_to enqueues batches; a cycle that starts at t_end must hand the state on bit for bit.
+    IDFX_ADVANCE_BATCH=8 (read at bind) makes the batches overshoot: 3 real cycles, then idle ones."""
+    nx, ny, nz = 20, 12, 8
+    prim, b, dx = smooth_ic(nx, ny, nz, 9)
+    outs = []
+    for batch in (None, "8"):
+        if batch:
+            monkeypatch.setenv("IDFX_ADVANCE_BATCH", batch)
+        sim = idfx.Idfx(nx, ny, nz, dx, G53, HLLD, VANLEER, EMF_UCT, nstages=nstages)
+        sim.set_state(torch.from_numpy(prim).cuda(), torch.from_numpy(b).cuda())
+        t_end = 2.5 * sim.compute_dt(0.3)
+        n, t = sim.advance_to(t_end, 0.3)
+        assert n == 3 and t == t_end
+        outs.append([x.clone() for x in sim.get_conserved()] + [sim.get_state()[0]])
+    for x, y in zip(*outs):
+        assert torch.equal(x, y)
+
+
+def test_vector_potential_divb_on_device(idfx):
+    """After many cycles the divergence of B_ref + curl A is still one rounding of the face values."""
+    n = 24
+    prim, b, dx = smooth_ic(n, n, n, 3)
+    res = {}
+    for form in (0, 1):
+        sim = idfx.Idfx(n, n, n, dx, G53, HLLD, VANLEER, EMF_UCT, ct_form=form)
+        sim.set_state(torch.from_numpy(prim).cuda(), torch.from_numpy(b).cuda())
+        sim.advance(300, 0.3)
+        assert sim.status() == 0
+        bf = sim.get_conserved()[1]
+        div = (torch.roll(bf[0], -1, 2) - bf[0]) + (torch.roll(bf[1], -1, 1) - bf[1]) + (torch.roll(bf[2], -1, 0) - bf[2])
+        res[form] = float(div.abs().max() / bf.abs().max())
+    print("div B / |B| after 300 cycles: face form %.2e, potential form %.2e" % (res[0], res[1]))
+    assert res[1] <= 8 * 2.2e-16 and res[0] < 1e-13
+
+
+def test_orszag_tang_3d_run(idfx, R):
+    """The paper's performance workload (3D Orszag-Tang, HLLD + PLM + E^c + RK2) at 32^3 to t = 0.1 on both
+    sides: same number of cycles, same final time, fields within the bar."""
+    n = 32
+    prim, b = inputs.orszag_tang_3d(n)
+    sim, ref = pair(idfx, R, (n, n, n), 1.0 / n, HLLD, VANLEER, EMF_UCT, prim.numpy(), b.numpy().copy())
+    n_g, t_g = sim.advance_to(0.1, 0.3)
+    rc, n_r = ref.advance_to(0.1, 0.3)
+    assert rc == 0 and sim.status() == 0 and n_g == n_r and t_g == 0.1
+    assert_state_close(sim, ref, TOL, "3D OT to t = 0.1 (%d cycles)" % n_g)
+    bf = sim.get_conserved()[1]
+    div = (torch.roll(bf[0], -1, 2) - bf[0]) + (torch.roll(bf[1], -1, 1) - bf[1]) + (torch.roll(bf[2], -1, 0) - bf[2])
+    assert float(div.abs().max() / bf.abs().max()) < 1e-13
+
+
+def test_pressure_floor_matches_the_oracle(idfx, R):
+    """3D Orszag-Tang at 32^3 with a floor placed inside the range the flow reaches (p_min ~ 0.016 by t = 0.25), so
+    that it acts on many cells: same cells floored, same fields."""
+    n, floor = 32, 0.03
+    prim, b = inputs.orszag_tang_3d(n)
+    nx = ny = nz = n
+    sim = idfx.Idfx(nx, ny, nz, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT, pressure_floor=floor)
+    sim.set_state(prim.contiguous().cuda(), b.contiguous().cuda())
+    ref = R.Oracle(nx, ny, nz, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT, pressure_floor=floor)
+    ref.set_state(prim.numpy(), b.numpy().copy())
+    n_g, _ = sim.advance_to(0.25, 0.3)
+    rc, n_r = ref.advance_to(0.25, 0.3)
+    assert rc == 0 and sim.status() == 0 and n_g == n_r
+    assert_state_close(sim, ref, TOL, "floored run")
+    assert ref.floor_count() > 100 and abs(sim.floor_count() - ref.floor_count()) <= 2
+    assert float(sim.get_state()[0][4].min()) == floor
+    # off by default: the same run without the floor is flagged or stays above it
+    sim0 = idfx.Idfx(nx, ny, nz, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT)
+    sim0.set_state(prim.contiguous().cuda(), b.contiguous().cuda())
+    sim0.advance_to(0.25, 0.3)
+    assert sim0.floor_count() == 0 and float(sim0.get_state()[0][4].min()) < floor

@@ -226,3 +226,36 @@ def test_advance_to_lands_on_t_end(R):
     o.set_state(prim, b)
     rc, k = o.advance_to(t_end, 0.3, max_steps=2)
     assert k == 2 and 0.0 < o.time() < t_end
+
+
+# =================================================================================================
+# optional pressure floor (reading G20; off by default, G13)
+# =================================================================================================
+def test_pressure_floor_closed_form_and_inert_when_not_needed(R):
+    """A uniform moving magnetised state below the floor: the first stage raises every cell to the floor and rewrites
+    E = p_floor/(gamma-1) + rho v^2/2 + B^2/2; nothing else changes (uniform states have no flux divergence) and the
+    cells are not counted twice.  With pressures above the floor the option changes no bit."""
+    n, floor = 6, 1e-4
+    prim = np.zeros((5, n, n, n))
+    prim[0], prim[1], prim[2], prim[4] = 1.3, 0.3, -0.2, 1e-7
+    b = np.zeros((3, n, n, n))
+    b[0], b[1], b[2] = 0.5, -0.25, 0.1
+    o = R.Oracle(n, n, n, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT, pressure_floor=floor)
+    o.set_state(prim, b)
+    assert o.get_state()[0][4].min() == floor and o.floor_count() == n ** 3
+    o.set_state(prim, b)
+    assert o.step(1e-3) == 0
+    u, bf = o.get_conserved()
+    e_want = floor / (G53 - 1) + 0.5 * 1.3 * (0.09 + 0.04) + 0.5 * (0.25 + 0.0625 + 0.01)
+    assert np.abs(u[4] - e_want).max() <= 4e-16 and o.floor_count() == n ** 3
+    np.testing.assert_array_equal(bf, b)
+    np.testing.assert_allclose(o.get_state()[0][4], floor, rtol=1e-9)
+    prim2, b2 = smooth_mhd_ic(8, seed=2)
+    outs = []
+    for fl in (0.0, 1e-6):
+        o = R.Oracle(8, 8, 8, 0.125, G53, HLLD, VANLEER, EMF_UCT, pressure_floor=fl)
+        o.set_state(prim2, b2)
+        assert o.advance(3, 0.3) == 0 and o.floor_count() == 0
+        outs.append(o.get_conserved())
+    for x, y in zip(*outs):
+        np.testing.assert_array_equal(x, y)
