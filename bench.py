@@ -49,8 +49,9 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5",
-                    help="config1..config5 (BASELINE.json), or ot3d: the paper's own 3D Orszag-Tang run to --t-end (PAPER.md:346)")
-    ap.add_argument("--t-end", type=float, default=1.0, help="ot3d only")
+                    help="config1..config5 (BASELINE.json); ot3d: the paper's own 3D Orszag-Tang run to --t-end (PAPER.md:346); "
+                         "sedov: its Cartesian Sedov-Taylor blast, HD, HLL, to --t-end (PAPER.md:253)")
+    ap.add_argument("--t-end", type=float, default=None, help="ot3d (default 1.0) and sedov (default 0.1) only")
     ap.add_argument("--n", type=int, default=None, help="override the grid size (development only)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -313,12 +314,20 @@ def run_ot3d(args):
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
     dev = torch.device("cuda", 0)
-    n = args.n or 256
-    prim, bface = inputs.orszag_tang_3d(n, device=dev)
-    prim, bface = prim.contiguous(), bface.contiguous()
-    # pressure floor 1e-5: without any fix this run meets p < 0 in a handful of cells before t = 1 (reading G20)
-    sim = idfx.Idfx(n, n, n, 1.0 / n, inputs.GAMMA, inputs.SOLVER_HLLD, inputs.LIMITER_VANLEER, inputs.EMF_UCT_CONTACT, device=dev,
-                    pressure_floor=1e-5)
+    sedov = args.workload == "sedov"
+    n = args.n or (512 if sedov else 256)
+    t_end = args.t_end if args.t_end is not None else (0.1 if sedov else 1.0)
+    if sedov:
+        prim, bface = inputs.sedov(n, device=dev)[0], None
+        sim = idfx.Idfx(n, n, n, 1.0 / n, inputs.GAMMA, inputs.SOLVER_HLL, inputs.LIMITER_VANLEER, inputs.EMF_NONE, device=dev)
+        what = "sedov: the paper's Cartesian Sedov-Taylor blast (PAPER.md:253), %d^3 periodic, HD, HLL + PLM van Leer + RK2" % n
+    else:
+        prim, bface = inputs.orszag_tang_3d(n, device=dev)
+        prim, bface = prim.contiguous(), bface.contiguous()
+        # pressure floor 1e-5: without any fix this run meets p < 0 in a handful of cells before t = 1 (reading G20)
+        sim = idfx.Idfx(n, n, n, 1.0 / n, inputs.GAMMA, inputs.SOLVER_HLLD, inputs.LIMITER_VANLEER, inputs.EMF_UCT_CONTACT,
+                        device=dev, pressure_floor=1e-5)
+        what = "ot3d: the paper's 3D Orszag-Tang performance test, %d^3, HLLD + PLM van Leer + CT upwind-contact + RK2" % n
     sim.set_state(prim, bface)
     sim.advance(max(args.warmup, 3), 0.3)
     sim.set_state(prim, bface)          # back to t = 0
@@ -328,34 +337,43 @@ def run_ot3d(args):
     l0 = sim.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    cycles, t = sim.advance_to(args.t_end, 0.3)
+    cycles, t = sim.advance_to(t_end, 0.3)
     e1.record()
     torch.cuda.synchronize()
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
-    assert sim.status() == 0 and t == args.t_end
-    bf = sim.get_conserved()[1]
-    div = (torch.roll(bf[0], -1, 2) - bf[0]) + (torch.roll(bf[1], -1, 1) - bf[1]) + (torch.roll(bf[2], -1, 0) - bf[2])
+    assert sim.status() == 0 and t == t_end
+    extra = {}
+    if sedov:
+        rho = sim.get_state()[0][0]
+        c = n // 2
+        extra = {"shock_radius": (int(torch.argmax(rho[c, c, c:])) + 0.5) / n,
+                 "shock_radius_self_similar": 1.152 * (t_end ** 2) ** 0.2, "rho_max": float(rho.max())}
+    else:
+        bf = sim.get_conserved()[1]
+        div = (torch.roll(bf[0], -1, 2) - bf[0]) + (torch.roll(bf[1], -1, 1) - bf[1]) + (torch.roll(bf[2], -1, 0) - bf[2])
+        extra = {"max_divB_over_maxB": float(div.abs().max() / bf.abs().max()), "pressure_floor": 1e-5,
+                 "cells_floored": sim.floor_count()}
     value = n ** 3 * cycles / (ms * 1e-3)
-    print(json.dumps({
+    out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": cycles, "warmup": max(args.warmup, 3),
         "ms_per_step": ms / cycles, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": value / 1.21e8, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "ot3d: the paper's 3D Orszag-Tang performance test, %d^3, HLLD + PLM van Leer + CT upwind-contact + "
-                               "RK2, CFL 0.3, t = 0 .. %g (idfx_advance_to, host reads the device clock between batches)" % (n, args.t_end),
-                   "grid": [n, n, n], "t_end": args.t_end, "cycles": cycles,
-                   "baseline": "1.21e8 cell/s per V100 at 256^3 per GPU (Tab. 4, PAPER.md:389): other hardware, context only"},
+        "vs_baseline": None if sedov else value / 1.21e8, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": what + ", CFL 0.3, t = 0 .. %g (idfx_advance_to, host reads the device clock between batches)" % t_end,
+                   "grid": [n, n, n], "t_end": t_end, "cycles": cycles,
+                   "baseline": "the paper prints no throughput for this test" if sedov else
+                               "1.21e8 cell/s per V100 at 256^3 per GPU (Tab. 4, PAPER.md:389): other hardware, context only"},
         "gpu_launches": sim.launch_count() - l0, "clocks": clocks,
-        "max_divB_over_maxB": float(div.abs().max() / bf.abs().max()),
-        "pressure_floor": 1e-5, "cells_floored": sim.floor_count(),
-    }))
+    }
+    out.update(extra)
+    print(json.dumps(out))
 
 
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
-    elif args.workload == "ot3d":
+    elif args.workload in ("ot3d", "sedov"):
         run_ot3d(args)
     else:
         run_ours(args)

@@ -24,7 +24,8 @@
 // DESIGN.md "Readings"): the limiter flavour (G2), the Davis wave-speed estimate (G5), the HLLD
 // degeneracy threshold (G6), the Roe fallback/degenerate-eigenvector conventions (G7), the face→cell
 // mapping of c_max in dt (G8), un-lagged dt (G9), the reference E^c state (G10), and the LimO3 constants
-// (1.6, r = 1, eps = 1e-12; G18: PAPER.md:79 only names the scheme of Cada & Torrilhon 2009).
+// (1.6, r = 1, eps = 1e-12; G18: PAPER.md:79 only names the scheme of Cada & Torrilhon 2009), and the composition of the
+// 2D-HLL EMF beyond its plane-parallel limit (G21: PAPER.md:109 only names Mignone & Del Zanna 2021).
 //
 // Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC idfxref.cpp -o libidfxref.so
 #include <algorithm>
@@ -43,7 +44,7 @@ enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_
 enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3 };
 enum { OPT_INTEGRATOR = 0, OPT_CT_FORM = 1, OPT_PRESSURE_FLOOR = 2 };  // idfxref_set_option / idfxref_set_option_real
 enum { CT_FACE = 0, CT_POTENTIAL = 1 };
-enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3 };
+enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3, EMF_UCT_HLL = 4 };
 enum { OK = 0, ERR_INVALID_ARG = -1, ERR_UNSUPPORTED = -2, ERR_UNPHYSICAL = -5 };
 
 // ---------------------------------------------------------------------------------------------
@@ -533,6 +534,9 @@ struct Ctx {
   Arr F[3][7];                      // face fluxes per direction in that direction's local ordering
   Arr cf[3];                        // c_face per direction
   Arr E[3];                         // edge EMFs: E[0] at (i, j-1/2, k-1/2), E[1] at (i-1/2, j, k-1/2), E[2] at (i-1/2, j-1/2, k)
+  Arr Vt[3][2], Al[3][2];           // EMF_UCT_HLL: per d-face, the HLL-weighted transverse velocities (components d+1, d+2)
+                                    // and the one-sided speeds alpha+ = max(0, S_R), alpha- = max(0, -S_L)
+  const Arr* Bstage;                // face field of the stage input (edge_emf reads it for EMF_UCT_HLL)
   int nstages;                      // 1 Euler, 2 RK2, 3 RK3 (Tab. 1)
   int ct_form;                      // CT_FACE: Eq. 6; CT_POTENTIAL: Eq. 7-8
   Arr A[3], A0[3], As[3], Bref[3];  // CT_POTENTIAL: edge potential accumulated since set_state (same places as E),
@@ -620,6 +624,11 @@ void sweep(Ctx& c, int d, const Arr Bf[3], bool want_flux) {
   lo[a] = 0; hi[a] = c.n[a];
   lo[b] = -1; hi[b] = c.n[b];
   lo[e] = -1; hi[e] = c.n[e];
+  if (c.emf == EMF_UCT_HLL) {  // the 2D-HLL EMF reconstructs face quantities across two more transverse faces
+    lo[b] = lo[e] = -NG;
+    hi[b] = c.n[b] + NG - 1;
+    hi[e] = c.n[e] + NG - 1;
+  }
   const size_t sa = c.st[a];
   const Arr* q[7] = {&c.V[0], &c.V[1 + a], &c.V[1 + b], &c.V[1 + e], &c.V[4], &c.V[5 + b], &c.V[5 + e]};
   const int nq = c.mhd ? 7 : 5;
@@ -643,6 +652,18 @@ void sweep(Ctx& c, int d, const Arr Bf[3], bool want_flux) {
           c.roe_fallbacks += riemann(c.solver, c.g, WL, WR, Bn, F, cface);
           for (int n = 0; n < 7; ++n) c.F[d][n][i0] = F[n];
           c.cf[d][i0] = cface;
+          if (c.emf == EMF_UCT_HLL) {
+            // G21 (Mignone & Del Zanna 2021, HLL case): with the Davis speeds of this face, alpha+ = max(0, S_R),
+            // alpha- = max(0, -S_L); the face carries the HLL-weighted transverse velocities
+            // (alpha+ v_t^L + alpha- v_t^R)/(alpha+ + alpha-), which is how v_t enters the HLL flux of the normal field
+            double SL, SR;
+            davis_speeds(WL, WR, Bn, c.g, SL, SR);
+            const double ap = std::max(0.0, SR), am = std::max(0.0, -SL);
+            c.Al[d][0][i0] = ap;
+            c.Al[d][1][i0] = am;
+            c.Vt[d][0][i0] = (ap * WL[2] + am * WR[2]) / (ap + am);
+            c.Vt[d][1][i0] = (ap * WL[3] + am * WR[3]) / (ap + am);
+          }
         } else {
           double SL, SR;
           davis_speeds(WL, WR, Bn, c.g, SL, SR);
@@ -680,6 +701,32 @@ void edge_emf(Ctx& c, int comp) {
       for (ijk[0] = lo[0]; ijk[0] <= hi[0]; ++ijk[0]) {
         const size_t P = c.at(ijk[0], ijk[1], ijk[2]);
         double e = 0.25 * (Ea(P) + Ea(P - eb) + Eb(P) + Eb(P - ea));
+        if (c.emf == EMF_UCT_HLL) {
+          // 2D HLL EMF (G21).  E_c = -(v_a B_b - v_b B_a) at the edge (a-1/2, b-1/2):
+          //   E_c = -[al_a+ (v_a B_b)^W + al_a- (v_a B_b)^E - al_a+ al_a- (B_b^E - B_b^W)] / (al_a+ + al_a-)
+          //         +[al_b+ (v_b B_a)^S + al_b- (v_b B_a)^N - al_b+ al_b- (B_a^N - B_a^S)] / (al_b+ + al_b-)
+          // W/E: the staggered B_b and the face velocity v_a of the b-faces on either side of the edge, reconstructed
+          // along a with the scheme's limiter; S/N likewise along b on the a-faces; al_a+- the larger of the two
+          // a-faces that touch the edge (and al_b+- of the two b-faces).
+          const double* Bb = c.Bstage[b].data();   // on b-faces
+          const double* Ba = c.Bstage[a].data();   // on a-faces
+          const double* va_f = c.Vt[b][1].data();  // v_a on b-faces (b-sweep local order: n = b, t1 = c, t2 = a)
+          const double* vb_f = c.Vt[a][0].data();  // v_b on a-faces (a-sweep local order: n = a, t1 = b, t2 = c)
+          double unused, BbW, BbE, vaW, vaE, BaS, BaN, vbS, vbN;
+          reconstruct(c.limiter, Bb[P - 2 * ea], Bb[P - ea], Bb[P], c.dx, unused, BbW);
+          reconstruct(c.limiter, Bb[P - ea], Bb[P], Bb[P + ea], c.dx, BbE, unused);
+          reconstruct(c.limiter, va_f[P - 2 * ea], va_f[P - ea], va_f[P], c.dx, unused, vaW);
+          reconstruct(c.limiter, va_f[P - ea], va_f[P], va_f[P + ea], c.dx, vaE, unused);
+          reconstruct(c.limiter, Ba[P - 2 * eb], Ba[P - eb], Ba[P], c.dx, unused, BaS);
+          reconstruct(c.limiter, Ba[P - eb], Ba[P], Ba[P + eb], c.dx, BaN, unused);
+          reconstruct(c.limiter, vb_f[P - 2 * eb], vb_f[P - eb], vb_f[P], c.dx, unused, vbS);
+          reconstruct(c.limiter, vb_f[P - eb], vb_f[P], vb_f[P + eb], c.dx, vbN, unused);
+          const double aap = std::max(c.Al[a][0][P - eb], c.Al[a][0][P]), aam = std::max(c.Al[a][1][P - eb], c.Al[a][1][P]);
+          const double abp = std::max(c.Al[b][0][P - ea], c.Al[b][0][P]), abm = std::max(c.Al[b][1][P - ea], c.Al[b][1][P]);
+          const double term_a = (aap * vaW * BbW + aam * vaE * BbE - aap * aam * (BbE - BbW)) / (aap + aam);
+          const double term_b = (abp * vbS * BaS + abm * vbN * BaN - abp * abm * (BaN - BaS)) / (abp + abm);
+          e = -term_a + term_b;
+        }
         if (c.emf == EMF_UCT0) {
           // E^0 of Gardiner & Stone 2005: the E^c construction with the two candidate gradients
           // averaged instead of upwinded, which collapses to (1/2) sum of the four face values - (1/4) sum of the
@@ -715,6 +762,7 @@ void stage(Ctx& c, Arr Uin[5], Arr Bin[3], const Arr Ain[3], double dt, Arr Uout
   if (c.mhd)
     for (int n = 0; n < 3; ++n) fill_periodic(c, Bin[n]);
   compute_prims(c, Uin, Bin);
+  c.Bstage = Bin;
   for (int d = 0; d < 3; ++d) sweep(c, d, Bin, true);
   // a5 / Eq. 5: flux divergence; local flux ordering (rho, m_n, m_t1, m_t2, E) -> global momentum
   const double dtdx = dt / c.dx;
@@ -850,7 +898,7 @@ struct idfxref_ctx {
 IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, double gamma, int solver,
                                         int limiter, int emf_mode) {
   if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(gamma > 1.0)) return nullptr;
-  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 3 || emf_mode < 0 || emf_mode > 3) return nullptr;
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 3 || emf_mode < 0 || emf_mode > 4) return nullptr;
   const bool mhd = emf_mode != EMF_NONE;
   if (mhd && solver == SOLVER_HLLC) return nullptr;
   if (!mhd && solver == SOLVER_HLLD) return nullptr;
@@ -870,7 +918,13 @@ IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, doubl
     for (int n = 0; n < 7; ++n) c.F[d][n].assign(c.N, 0.0);
     c.cf[d].assign(c.N, 0.0);
     c.E[d].assign(c.N, 0.0);
+    if (emf_mode == EMF_UCT_HLL)
+      for (int m = 0; m < 2; ++m) {
+        c.Vt[d][m].assign(c.N, 0.0);
+        c.Al[d][m].assign(c.N, 0.0);
+      }
   }
+  c.Bstage = nullptr;
   c.nstages = 2; c.ct_form = CT_FACE; c.t = 0.0; c.pfloor = 0.0; c.nfloor = 0;
   c.last_dt = 0.0; c.status = OK; c.roe_fallbacks = 0;
   return h;

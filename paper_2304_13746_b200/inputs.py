@@ -16,7 +16,7 @@ import numpy as np
 import torch
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
-LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER = 0, 1, 2
+LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3 = 0, 1, 2, 3
 EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0 = 0, 1, 2, 3
 
 GAMMA = 5.0 / 3.0
@@ -134,6 +134,22 @@ def orszag_tang_3d(n, device="cpu"):
     bface[1] = (b0 * torch.sin(2 * two_pi * X)).expand(n, n, n)
     bface[2] = (b0 * (torch.cos(two_pi * X) + torch.sin(two_pi * Y))).expand(n, n, n)
     return prim, bface
+
+
+def sedov(n, r_i=None, device="cpu"):
+    """The paper's Cartesian Sedov-Taylor blast: rho = 1, P = 1e-2 at rest, gamma = 5/3, and an energy
+    E = 1 deposited as pressure in the cells whose centres lie within r_i of the box centre (periodic unit cube; the
+    paper does not print r_i: 3.5 cells unless given).  Returns (prim, the deposited energy as discretised = 1)."""
+    r_i = 3.5 / n if r_i is None else r_i
+    x = (torch.arange(n, dtype=torch.float64, device=device) + 0.5) / n - 0.5
+    r2 = x.view(1, 1, n) ** 2 + x.view(1, n, 1) ** 2 + x.view(n, 1, 1) ** 2
+    inside = r2 < r_i * r_i
+    n_in = int(inside.sum())
+    prim = torch.zeros((5, n, n, n), dtype=torch.float64, device=device)
+    prim[0] = 1.0
+    prim[4] = 1e-2
+    prim[4][inside] = (GAMMA - 1.0) * 1.0 / (n_in * (1.0 / n) ** 3)
+    return prim, n_in
 
 
 def turbulence_hd(n, seed, kmax, mach, device="cpu"):

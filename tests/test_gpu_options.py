@@ -158,3 +158,31 @@ def test_pressure_floor_matches_the_oracle(idfx, R):
     sim0.set_state(prim.contiguous().cuda(), b.contiguous().cuda())
     sim0.advance_to(0.25, 0.3)
     assert sim0.floor_count() == 0 and float(sim0.get_state()[0][4].min()) < floor
+
+
+def test_sedov_blast_parity_and_radius(idfx, R):
+    """The paper's Cartesian Sedov test (HLL + PLM + RK2, periodic): parity with the oracle at 32^3, and at
+    128^3 the shock radius against the self-similar solution r = 1.152 (E t^2 / rho)^(1/5)."""
+    n = 32
+    prim, _ = inputs.sedov(n)
+    sim = idfx.Idfx(n, n, n, 1.0 / n, G53, HLL, VANLEER, EMF_NONE)
+    sim.set_state(prim.cuda())
+    ref = R.Oracle(n, n, n, 1.0 / n, G53, HLL, VANLEER, EMF_NONE)
+    ref.set_state(prim.numpy())
+    n_g, t_g = sim.advance_to(0.01, 0.3)
+    rc, n_r = ref.advance_to(0.01, 0.3)
+    assert rc == 0 and n_g == n_r and t_g == 0.01
+    assert_state_close(sim, ref, TOL, "Sedov 32^3")
+    n = 128
+    prim, _ = inputs.sedov(n, device="cuda")
+    sim = idfx.Idfx(n, n, n, 1.0 / n, G53, HLL, VANLEER, EMF_NONE)
+    sim.set_state(prim)
+    sim.advance_to(0.05, 0.3)
+    assert sim.status() == 0
+    rho = sim.get_state()[0][0]
+    r_exact = 1.152 * (0.05 ** 2) ** 0.2
+    c = n // 2
+    for line in (rho[c, c, c:], rho[c, c:, c], rho[c:, c, c]):
+        r_num = (int(torch.argmax(line)) + 0.5) / n
+        assert abs(r_num - r_exact) <= 2.0 / n, (r_num, r_exact)
+    assert float(rho.max()) > 2.5

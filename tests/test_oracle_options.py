@@ -259,3 +259,120 @@ def test_pressure_floor_closed_form_and_inert_when_not_needed(R):
         outs.append(o.get_conserved())
     for x, y in zip(*outs):
         np.testing.assert_array_equal(x, y)
+
+
+# =================================================================================================
+# Sedov-Taylor blast, HD path
+# =================================================================================================
+def test_sedov_blast_radius_and_symmetry(R):
+    """E = 1 in rho = 1: the shock sits at r = xi0 (E t^2 / rho)^(1/5) with xi0 = 1.152 for gamma = 5/3 (Sedov 1946,
+    Taylor 1950; textbook value).  40^3 cells, HLL + van Leer + RK2 as in the paper, to t = 0.02 (r = 0.241 = 9.6 cells):
+    the density maximum along the axes lies within 1.5 cells of it, the eight octants are mirror images to round-off,
+    and total energy is conserved (the deposited E plus the ambient p/(gamma-1))."""
+    from paper_2304_13746_b200 import inputs
+    n = 40
+    prim, n_in = inputs.sedov(n)
+    prim = prim.numpy()
+    o = R.Oracle(n, n, n, 1.0 / n, G53, HLL, VANLEER, EMF_NONE)
+    o.set_state(prim)
+    e0 = o.get_conserved()[0][4].sum() / n ** 3
+    assert e0 == pytest.approx(1.0 + 1e-2 / (G53 - 1) * (1 - n_in / n ** 3), rel=1e-13)
+    rc, steps = o.advance_to(0.02, 0.3)
+    assert rc == 0 and steps > 50
+    u = o.get_conserved()[0]
+    assert u[4].sum() / n ** 3 == pytest.approx(e0, rel=1e-12)
+    rho = u[0]
+    for ax in range(3):      # mirror symmetry about the centre, every axis
+        np.testing.assert_allclose(rho, np.flip(rho, ax), rtol=1e-11)
+    r_exact = 1.152 * (1.0 * 0.02 ** 2 / 1.0) ** 0.2
+    c = n // 2
+    for line in (rho[c, c, c:], rho[c, c:, c], rho[c:, c, c]):
+        r_num = (np.argmax(line) + 0.5) / n
+        assert abs(r_num - r_exact) <= 1.5 / n, (r_num, r_exact)
+    assert rho.max() > 1.8      # a strong shock, smeared over ~3 cells by HLL at this resolution (limit (gamma+1)/(gamma-1) = 4)
+
+
+# =================================================================================================
+# 2D-HLL EMF (PAPER.md:109 "2D HLL ... following the method of Mignone & Del Zanna (2021)"; reading G21)
+# =================================================================================================
+EMF_UCT_HLL = 4
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("limiter", [VANLEER, LIMO3])
+def test_emf_hll2d_plane_parallel_identity(R, axis, limiter):
+    """Plane-parallel flow along a grid axis with uniform transverse velocity: the edge EMF of the 2D-HLL scheme must be
+    the EMF of the 1D HLL flux, E_t2 = -F_n[B_t1] and E_t1 = +F_n[B_t2] (the consistency requirement that fixes its
+    weights alpha+-/(alpha+ + alpha-), its dissipation alpha+ alpha-/(alpha+ + alpha-) and the HLL-weighted face velocity)."""
+    from test_oracle_scheme import HLL as HLL_
+    n = 32
+    dx = 1.0 / n
+    x = (np.arange(n) + 0.5) * dx
+    shape = [4, 4, 4]
+    shape[2 - axis] = n
+    bc = [1, 1, 1]
+    bc[2 - axis] = n
+    X = x.reshape(bc)
+    a, b_, e = axis, (axis + 1) % 3, (axis + 2) % 3
+    prim = np.empty([5] + shape)
+    prim[0] = 1.0 + 0.3 * np.sin(2 * np.pi * X)
+    prim[1 + a] = 0.4 * np.cos(2 * np.pi * X)
+    prim[1 + b_] = 0.35
+    prim[1 + e] = -0.25
+    prim[4] = 1.0 + 0.2 * np.cos(4 * np.pi * X)
+    bf = np.empty([3] + shape)
+    bf[a] = 0.7
+    bf[b_] = 0.5 + 0.3 * np.sin(2 * np.pi * X)
+    bf[e] = -0.4 + 0.2 * np.cos(2 * np.pi * X)
+    dims = shape[::-1]
+    o = R.Oracle(dims[0], dims[1], dims[2], dx, G53, HLL_, limiter, EMF_UCT_HLL)
+    o.set_state(prim, bf)
+    o.step(o.compute_dt(0.4))
+    E = o.get_emf()
+    F, _ = o.get_flux(axis)
+    np.testing.assert_allclose(E[e], -F[5], rtol=0, atol=1e-13)   # E_t2 = -F_n[B_t1]
+    np.testing.assert_allclose(E[b_], F[6], rtol=0, atol=1e-13)   # E_t1 = +F_n[B_t2]
+    assert np.abs(E[a]).max() > 0.01                               # the third component is the transverse -(v x B), not zero
+
+
+def test_emf_hll2d_uniform_state_conservation_divb_and_symmetry(R):
+    from test_oracle_scheme import HLL as HLL_, rot_prim, rot_vector
+    n = 8
+    prim = np.empty((5, n, n, n))
+    for v, val in enumerate((1.3, 0.4, -0.7, 0.2, 0.8)):
+        prim[v] = val
+    b = np.empty((3, n, n, n))
+    for d, val in enumerate((0.5, -0.3, 0.9)):
+        b[d] = val
+    o = R.Oracle(n, n, n, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT_HLL)
+    o.set_state(prim, b)
+    o.advance(2, 0.5)
+    assert np.array_equal(o.get_conserved()[1], b)
+    np.testing.assert_allclose(o.get_emf()[:, 0, 0, 0], -np.cross([0.4, -0.7, 0.2], [0.5, -0.3, 0.9]), rtol=1e-14)
+    # smooth 3D data: conservation, div B, cyclic relabelling of the axes
+    n = 12
+    prim, b = smooth_mhd_ic(n, 7)
+    o = R.Oracle(n, n, n, 1.0 / n, G53, HLL_, VANLEER, EMF_UCT_HLL)
+    o.set_state(prim, b)
+    c0, b0 = o.get_conserved()
+    assert o.advance(3, 0.4) == 0
+    c1, b1 = o.get_conserved()
+    for v in range(5):
+        assert abs(c1[v].sum() - c0[v].sum()) <= 1e-13 * max(np.abs(c0[v]).sum(), 1.0)
+    for d in range(3):
+        assert abs(b1[d].sum() - b0[d].sum()) <= 1e-13 * np.abs(b0[d]).sum()
+    assert np.abs(divb(b1)).max() <= 1e-13 * np.abs(b1).max() * 6
+    o2 = R.Oracle(n, n, n, 1.0 / n, G53, HLL_, VANLEER, EMF_UCT_HLL)
+    o2.set_state(rot_prim(prim), rot_vector(b))
+    o2.advance(3, 0.4)
+    p2, b2 = o2.get_state()
+    p1, _ = o.get_state()
+    np.testing.assert_allclose(p2, rot_prim(p1), rtol=0, atol=1e-13)
+    np.testing.assert_allclose(b2, rot_vector(b1), rtol=0, atol=1e-13)
+
+
+def test_emf_hll2d_linear_wave_second_order(R):
+    """Inclined fast wave, HLL fluxes + 2D-HLL EMF: the same convergence the other EMFs show (pre-asymptotic 16 -> 32)."""
+    from test_oracle_scheme import HLL as HLL_, run_linear_wave
+    errs = [run_linear_wave(R, n, "fast", HLL_, EMF_UCT_HLL) for n in (16, 32)]
+    assert errs[0] < 0.1 and math.log2(errs[0] / errs[1]) >= 1.25, errs
