@@ -179,7 +179,9 @@ struct FluxArgs {
   double* cf;    // c_face
 };
 
-template <int SOLVER, int LIM, bool MHD, bool SPEED_ONLY>
+// FMODE 0: fluxes and c_face; 1: c_face only (idfx_compute_dt); 2: what the 2D-HLL EMF needs of the face (G21):
+// F[0] = alpha+ = max(0, S_R), F[1] = alpha- = max(0, -S_L), F[2], F[3] = the HLL-weighted transverse velocities.
+template <int SOLVER, int LIM, bool MHD, int FMODE>
 __global__ void __launch_bounds__(128) k_flux_face(Geom g, FluxArgs a) {
   int i, j, k;
   if (!cell_of_thread(g, i, j, k)) return;
@@ -197,10 +199,19 @@ __global__ void __launch_bounds__(128) k_flux_face(Geom g, FluxArgs a) {
   }
   if (!MHD) WL[5] = WL[6] = WR[5] = WR[6] = 0.0;
   const double Bn = MHD ? a.bn[c] : 0.0;  // G3
-  if (SPEED_ONLY) {
+  if (FMODE == 1) {
     double SL, SR;
     outer_speeds<MHD>(WL, WR, Bn, g.gamma, SL, SR);
     a.cf[c] = fmax(fabs(SL), fabs(SR));
+  } else if (FMODE == 2) {
+    double SL, SR;
+    outer_speeds<MHD>(WL, WR, Bn, g.gamma, SL, SR);
+    const double ap = fmax(0.0, SR), am = fmax(0.0, -SL);
+    const double inv = 1.0 / (ap + am);
+    a.F[0][c] = ap;
+    a.F[1][c] = am;
+    a.F[2][c] = (ap * WL[2] + am * WR[2]) * inv;
+    a.F[3][c] = (ap * WL[3] + am * WR[3]) * inv;
   } else {
     double F[7];
     a.cf[c] = riemann<SOLVER, MHD>(WL, WR, Bn, g.gamma, F);
@@ -262,6 +273,7 @@ struct EmfArgs {
   const double* FB[3][2];  // FB[d][0] = F_d[B_t1], FB[d][1] = F_d[B_t2] on the left d-faces
   const signed char* SG[3];  // sign of the mass flux F_d[rho] on the left d-faces
   const double* Ec[3];     // cell-centred reference EMF -(v x Bc) of the stage input, with ghosts (G10)
+  const double* Eg[3];     // EMF_UCT_HLL: edge EMFs already evaluated by k_emf_hll2d
 };
 
 // E_c on the lower (a-1/2, b-1/2) edge of active cell idx, (a,b,c) cyclic (O10)
@@ -278,6 +290,7 @@ __device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& a, cons
     const double* __restrict__ Fb = a.FB[ib][1];
     const double EaP = -Fa[P], EaPb = -Fa[P + db];  // a-faces at (ia-1/2, ib) and (ia-1/2, ib-1)
     const double EbP = Fb[P], EbPa = Fb[P + da];    // b-faces at (ia, ib-1/2) and (ia-1, ib-1/2)
+    if (MODE == EMF_UCT_HLL) return a.Eg[c][P];
     double e = 0.25 * (EaP + EaPb + EbP + EbPa);
     if (MODE == EMF_UCT0) {
       // E^0: averaged instead of upwinded gradients = (1/2) sum of faces - (1/4) sum of cell-centred references
@@ -304,6 +317,74 @@ __device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& a, cons
       e += 0.125 * (Gb3 - Gb1) + 0.125 * (Ga3 - Ga1);
     }
     return e;
+}
+
+// ---------------------------------------------------------------------------------------------
+// 2D-HLL edge EMF (reading G21).  Thread (i,j,k) evaluates the three lower edges of its cell from the face
+// quantities of k_flux_face<FMODE 2> (no ghosts: indices wrap) and the staggered field (ghosts filled):
+//   E_c = -[al_a+ (v_a B_b)^W + al_a- (v_a B_b)^E - al_a+ al_a- (B_b^E - B_b^W)] / (al_a+ + al_a-)
+//         +[al_b+ (v_b B_a)^S + al_b- (v_b B_a)^N - al_b+ al_b- (B_a^N - B_a^S)] / (al_b+ + al_b-),   (a,b,c) cyclic,
+// W/E reconstructed along a on the b-faces either side of the edge, S/N along b on the a-faces.
+// ---------------------------------------------------------------------------------------------
+struct Hll2dArgs {
+  const double* H[3][4];   // per direction d: alpha+, alpha-, v_t1 (component d+1), v_t2 (component d+2) on the left d-faces
+  const double* Bf[3];
+  double* E[3];
+};
+
+template <int LIM>
+__global__ void __launch_bounds__(128) k_emf_hll2d(Geom g, Hll2dArgs h) {
+  int ijk[3];
+  if (!cell_of_thread(g, ijk[0], ijk[1], ijk[2])) return;
+  const int n[3] = {g.nx, g.ny, g.nz};
+  const long long st[3] = {1, g.sy, g.sz};
+  const long long P = g.at(ijk[0], ijk[1], ijk[2]);
+  const double dx2 = g.dx * g.dx;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const int a = (c + 1) % 3, b = (c + 2) % 3;
+    // offsets of the periodic images at -2, -1, +1 along a and along b
+    long long oa[4], ob[4];
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+      const int da = m - 2;  // -2, -1, 0, +1
+      int ia = ijk[a] + da, ib = ijk[b] + da;
+      ia = ia < 0 ? ia + n[a] : (ia >= n[a] ? ia - n[a] : ia);
+      ib = ib < 0 ? ib + n[b] : (ib >= n[b] ? ib - n[b] : ib);
+      oa[m] = P + (long long)(ia - ijk[a]) * st[a];
+      ob[m] = P + (long long)(ib - ijk[b]) * st[b];
+    }
+    const double* __restrict__ Bb = h.Bf[b];
+    const double* __restrict__ Ba = h.Bf[a];
+    const double* __restrict__ va = h.H[b][3];  // v_a on b-faces: b-sweep order (n = b, t1 = c, t2 = a)
+    const double* __restrict__ vb = h.H[a][2];  // v_b on a-faces: a-sweep order (n = a, t1 = b, t2 = c)
+    double unused, BbW, BbE, vaW, vaE, BaS, BaN, vbS, vbN;
+    {  // the staggered field has ghosts: plain offsets
+      const double q0 = Bb[P - 2 * st[a]], q1 = Bb[P - st[a]], q2 = Bb[P], q3 = Bb[P + st[a]];
+      face_values<LIM>(q1, q1 - q0, q2 - q1, dx2, unused, BbW);
+      face_values<LIM>(q2, q2 - q1, q3 - q2, dx2, BbE, unused);
+    }
+    {
+      const double q0 = va[oa[0]], q1 = va[oa[1]], q2 = va[P], q3 = va[oa[3]];
+      face_values<LIM>(q1, q1 - q0, q2 - q1, dx2, unused, vaW);
+      face_values<LIM>(q2, q2 - q1, q3 - q2, dx2, vaE, unused);
+    }
+    {
+      const double q0 = Ba[P - 2 * st[b]], q1 = Ba[P - st[b]], q2 = Ba[P], q3 = Ba[P + st[b]];
+      face_values<LIM>(q1, q1 - q0, q2 - q1, dx2, unused, BaS);
+      face_values<LIM>(q2, q2 - q1, q3 - q2, dx2, BaN, unused);
+    }
+    {
+      const double q0 = vb[ob[0]], q1 = vb[ob[1]], q2 = vb[P], q3 = vb[ob[3]];
+      face_values<LIM>(q1, q1 - q0, q2 - q1, dx2, unused, vbS);
+      face_values<LIM>(q2, q2 - q1, q3 - q2, dx2, vbN, unused);
+    }
+    const double aap = fmax(h.H[a][0][ob[1]], h.H[a][0][P]), aam = fmax(h.H[a][1][ob[1]], h.H[a][1][P]);
+    const double abp = fmax(h.H[b][0][oa[1]], h.H[b][0][P]), abm = fmax(h.H[b][1][oa[1]], h.H[b][1][P]);
+    const double term_a = (aap * vaW * BbW + aam * vaE * BbE - aap * aam * (BbE - BbW)) / (aap + aam);
+    const double term_b = (abp * vbS * BaS + abm * vbN * BaN - abp * abm * (BaN - BaS)) / (abp + abm);
+    h.E[c][P] = -term_a + term_b;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -541,10 +622,12 @@ enum {
   F_SG = 58,   // 1 slot holding three byte fields: sign of the face mass flux of the x, y, z sweeps (E^c only)
   F_CS = 59,   // 1: sum_d c_d per cell (x and y parts)
   F_COUNT = 60,
-  // vector-potential form only (idfx_set_option(IDFX_OPT_CT_FORM, IDFX_CT_POTENTIAL)):
-  F_AA = 60,   // 3 x 3: edge-potential buffers, rotating like the face-field buffers
-  F_BREF = 69, // 3: the face field given to set_state (ghosts filled)
-  F_COUNT_VP = 72
+  // optional groups, appended in this order when present (idfx_ctx::f_aa, f_bref, f_h2d, f_eg):
+  //   vector-potential form (idfx_set_option(IDFX_OPT_CT_FORM, IDFX_CT_POTENTIAL)): 3 x 3 edge-potential buffers rotating
+  //   like the face-field buffers, and the 3 face fields given to set_state (ghosts filled);
+  //   2D-HLL EMF: 3 x 4 face quantities of k_flux_face<FMODE 2> and the 3 edge EMFs
+  N_VP = 12,
+  N_H2D = 15
 };
 
 }  // namespace idfx
@@ -568,8 +651,12 @@ struct idfx_ctx {
   int nstages = 2;  // Tab. 1: 1 Euler, 2 RK2, 3 RK3
   bool vp = false;  // Eq. 7-8 instead of Eq. 6
   int fixed_batch = 0;  // IDFX_ADVANCE_BATCH: cycles per batch of idfx_advance_to (tests: forces cycles past t_end)
-  int nfields() const { return vp ? F_COUNT_VP : F_COUNT; }
-  double* abuf(int which, int d) const { return field(F_AA + 3 * which + d); }
+  int f_aa() const { return F_COUNT; }
+  int f_bref() const { return F_COUNT + 9; }
+  int f_h2d() const { return F_COUNT + (vp ? N_VP : 0); }
+  int f_eg() const { return f_h2d() + 12; }
+  int nfields() const { return F_COUNT + (vp ? N_VP : 0) + (emf == EMF_UCT_HLL ? N_H2D : 0); }
+  double* abuf(int which, int d) const { return field(f_aa() + 3 * which + d); }
   int bcur = 0;  // which of the three face-field buffers holds the current state
   int vcur = 0;  // which primitive buffer holds the stage input
   int graph_bnext[6] = {0, 0, 0, 0, 0, 0}, graph_vnext[6] = {0, 0, 0, 0, 0, 0};  // rotation state a replayed cycle leaves
@@ -716,7 +803,7 @@ int check_bound(const idfx_ctx* c) {
 // ---- standalone dt (idfx_compute_dt): signal speeds on every face, then the per-cell sum and the max ----
 template <int LIM, bool MHD>
 void launch_speed_l(idfx_ctx* c, const FluxArgs& a) {
-  k_flux_face<SOLVER_HLL, LIM, MHD, true><<<blocks_for(c->g.nc, 128), 128, 0, c->stream>>>(c->g, a);
+  k_flux_face<SOLVER_HLL, LIM, MHD, 1><<<blocks_for(c->g.nc, 128), 128, 0, c->stream>>>(c->g, a);
 }
 
 void launch_speed(idfx_ctx* c, int d, const double* const Bf[3]) {
@@ -931,8 +1018,52 @@ EmfArgs emf_args(idfx_ctx* c) {
     a.FB[d][1] = c->field(F_FB + 2 * d + 1);
     a.SG[d] = c->sgn(d);
     a.Ec[d] = c->vfield(8 + d);
+    a.Eg[d] = c->emf == EMF_UCT_HLL ? c->field(c->f_eg() + d) : nullptr;
   }
   return a;
+}
+
+// 2D-HLL EMF: face quantities of the three directions, then the edge EMFs (two passes over the stage input)
+template <int LIM>
+void launch_hll2d_l(idfx_ctx* c, const double* const Bf[3]) {
+  const Geom& g = c->g;
+  const long long st[3] = {1, g.sy, g.sz};
+  const unsigned nb = blocks_for(g.nc, 128);
+  Hll2dArgs h;
+  for (int d = 0; d < 3; ++d) {
+    const int ib = (d + 1) % 3, ie = (d + 2) % 3;
+    FluxArgs a;
+    a.q[0] = c->vfield(0);
+    a.q[1] = c->vfield(1 + d);
+    a.q[2] = c->vfield(1 + ib);
+    a.q[3] = c->vfield(1 + ie);
+    a.q[4] = c->vfield(4);
+    a.q[5] = c->vfield(5 + ib);
+    a.q[6] = c->vfield(5 + ie);
+    a.bn = Bf[d];
+    a.sd = st[d];
+    for (int n = 0; n < 7; ++n) a.F[n] = nullptr;
+    for (int m = 0; m < 4; ++m) {
+      a.F[m] = c->field(c->f_h2d() + 4 * d + m);
+      h.H[d][m] = a.F[m];
+    }
+    a.cf = nullptr;
+    h.Bf[d] = Bf[d];
+    h.E[d] = c->field(c->f_eg() + d);
+    LaunchScope ls(c, K_EMF);
+    k_flux_face<SOLVER_HLL, LIM, true, 2><<<nb, 128, 0, c->stream>>>(g, a);
+  }
+  LaunchScope ls(c, K_EMF);
+  k_emf_hll2d<LIM><<<nb, 128, 0, c->stream>>>(g, h);
+}
+
+void launch_hll2d(idfx_ctx* c, const double* const Bf[3]) {
+  switch (c->limiter) {
+    case LIM_FLAT: launch_hll2d_l<LIM_FLAT>(c, Bf); break;
+    case LIM_MINMOD: launch_hll2d_l<LIM_MINMOD>(c, Bf); break;
+    case LIM_LIMO3: launch_hll2d_l<LIM_LIMO3>(c, Bf); break;
+    default: launch_hll2d_l<LIM_VANLEER>(c, Bf);
+  }
 }
 
 void launch_fill(idfx_ctx* c, int which_b) {
@@ -987,7 +1118,7 @@ void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, d
     a.Ain[d] = c->vp ? c->abuf(bin, d) : nullptr;
     a.A0[d] = c->vp ? c->abuf(b0, d) : nullptr;
     a.Aout[d] = c->vp ? c->abuf(bout, d) : nullptr;
-    a.Bref[d] = c->vp ? c->field(F_BREF + d) : nullptr;
+    a.Bref[d] = c->vp ? c->field(c->f_bref() + d) : nullptr;
   }
   a.sc = c->sc;
   a.dt_fixed = dt_fixed;
@@ -1002,8 +1133,10 @@ void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, d
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield_out(n);
     dim3 grid((g.nx + CT_TX - 1) / CT_TX, (g.ny + CT_TY - 1) / CT_TY, (g.nz + CT_TZ - 1) / CT_TZ);
     const bool udone = ap.on;  // the TMA z sweep applied the divergence itself
+    if (c->emf == EMF_UCT_HLL) launch_hll2d(c, Bf);
     LaunchScope ls(c, K_UPDATE);
     if (c->emf == EMF_UCT) launch_ct<EMF_UCT>(c, grid, ea, a, combine, udone);
+    else if (c->emf == EMF_UCT_HLL) launch_ct<EMF_UCT_HLL>(c, grid, ea, a, combine, udone);
     else if (c->emf == EMF_UCT0) launch_ct<EMF_UCT0>(c, grid, ea, a, combine, udone);
     else launch_ct<EMF_ARITH>(c, grid, ea, a, combine, udone);
     c->vcur ^= 1;
@@ -1083,8 +1216,8 @@ int finish_set_state(idfx_ctx* c) {
   CK(cudaGetLastError());
   if (c->vp) {  // G19: the potential is counted from this state on
     const size_t fb = (size_t)c->g.np * sizeof(double);
-    CK(cudaMemsetAsync(c->field(F_AA), 0, 9 * fb, c->stream));
-    CK(cudaMemcpyAsync(c->field(F_BREF), c->bbuf(c->bcur, 0), 3 * fb, cudaMemcpyDeviceToDevice, c->stream));
+    CK(cudaMemsetAsync(c->field(c->f_aa()), 0, 9 * fb, c->stream));
+    CK(cudaMemcpyAsync(c->field(c->f_bref()), c->bbuf(c->bcur, 0), 3 * fb, cudaMemcpyDeviceToDevice, c->stream));
   }
   return reset_clock(c);
 }
@@ -1123,7 +1256,7 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
     set_err("idfx_create: need dx > 0 and gamma > 1");
     return nullptr;
   }
-  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 3 || emf_mode < 0 || emf_mode > 3) {
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 3 || emf_mode < 0 || emf_mode > 4) {
     set_err("idfx_create: unknown solver, limiter or emf_mode");
     return nullptr;
   }

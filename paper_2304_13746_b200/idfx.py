@@ -13,7 +13,7 @@ SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
 LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3 = 0, 1, 2, 3
 OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR = 0, 1, 2
 CT_FACE, CT_POTENTIAL = 0, 1
-EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0 = 0, 1, 2, 3
+EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0, EMF_UCT_HLL = 0, 1, 2, 3, 4
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_NOT_BOUND, ERR_CUDA, ERR_UNPHYSICAL = 0, -1, -2, -3, -4, -5
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

@@ -17,7 +17,7 @@ import torch
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
 LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3 = 0, 1, 2, 3
-EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0 = 0, 1, 2, 3
+EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0, EMF_UCT_HLL = 0, 1, 2, 3, 4
 
 GAMMA = 5.0 / 3.0
 

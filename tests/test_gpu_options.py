@@ -13,6 +13,7 @@ from test_gpu_parity import (EMF_ARITH, EMF_NONE, EMF_UCT, EMF_UCT0, HLL, HLLC, 
 pytestmark = pytest.mark.gpu
 
 LIMO3 = 3
+EMF_UCT_HLL = 4
 G53 = 5.0 / 3.0
 
 
@@ -31,6 +32,8 @@ OPTION_COMBOS = [
     (HLL, LIMO3, EMF_UCT0, 1, 0), (HLLD, VANLEER, EMF_UCT, 1, 0), (HLLC, LIMO3, EMF_NONE, 3, 0), (HLL, MINMOD, EMF_NONE, 1, 0),
     (ROE, LIMO3, EMF_NONE, 2, 0),
     (HLLD, VANLEER, EMF_UCT, 2, 1), (HLLD, LIMO3, EMF_UCT, 3, 1), (ROE, VANLEER, EMF_ARITH, 1, 1), (HLL, MINMOD, EMF_UCT0, 3, 1),
+    # 2D-HLL EMF
+    (HLL, VANLEER, EMF_UCT_HLL, 2, 0), (HLLD, LIMO3, EMF_UCT_HLL, 3, 0), (HLL, MINMOD, EMF_UCT_HLL, 2, 1), (ROE, VANLEER, EMF_UCT_HLL, 1, 0),
 ]
 
 

@@ -44,7 +44,7 @@ def test_create_validates_arguments(L):
         (8, 8, 8, 0.1, 1.4, 5, 2, 0),      # solver enum, one past Rusanov
         (8, 8, 8, 0.1, 1.4, 0, 5, 0),      # limiter enum
         (8, 8, 8, 0.1, 1.4, 0, 2, 9),      # emf enum
-        (8, 8, 8, 0.1, 1.4, 0, 2, 4),      # emf enum, one past E^0
+        (8, 8, 8, 0.1, 1.4, 0, 2, 5),      # emf enum, one past the 2D-HLL scheme
         (8, 8, 8, 0.1, 1.4, idfx.SOLVER_HLLC, 2, idfx.EMF_ARITHMETIC),   # HLLC is HD-only
         (8, 8, 8, 0.1, 1.4, idfx.SOLVER_HLLD, 2, idfx.EMF_NONE),         # HLLD is MHD-only
     ]
