@@ -30,6 +30,10 @@ ALGO_BYTES_PER_CELL_UPDATE = 320.0          # 40 doubles per M
 # Algorithmic work per cell per launch of each kernel class.
 # Sweeps: one PLM + HLLD face solve = 360 flops (+, -, x, /, sqrt counted once each in O3-O7, one E*, one U**).
 ALGO_FLOPS_PER_CELL = {"flux_x": 360.0, "flux_y": 360.0, "flux_z": 360.0}
+# HD (config 2, sedov): the whole stage is one kernel (csrc/hd_stage.cuh): stage 1 reads V5, writes R5 (10 doubles); later
+# stages read V5 U1 5 U0 5 and write U5 V5 (25); mean 17.5.  The stage-1 update kernel reads U5 R5 and writes U5 V5 (20).
+ALGO_BYTES_PER_CELL_HD = {"hd_stage": 8 * 17.5, "ct_update_prim": 8 * 20.0}
+ALGO_BYTES_PER_CELL_UPDATE_HD = 200.0       # 25 doubles per HD cell-update
 # Compulsory doubles read + written per cell (MHD, E^c; sg = 1-byte sign of the face mass flux):
 # x: V7+Bn | Fx5 FB2 cf1 sg; y: V7+Bn+Fx5 | R5 FB2 sg; z stage 1: V7+Bn+R5 | R5 FB2 sg (20 1/8), stage 2 also applies the
 # RK2 combine: + U1 5 + U0 5 | U5 instead of R5 (30 1/8); fused CT/update stage 1: R5 U0 5 Bin3 FB6 sg3 Ec3 | U5 B3 V11
@@ -226,6 +230,9 @@ def run_ours(args):
     hbm_peak = float(peaks["hbm_gbs"])
     fp64_tflops, fp64_tinst = idfx.probe_fp64()
     tot_ms = sum(v[0] for v in prof.values())
+    mhd = bface is not None
+    ALGO_BYTES_PER_CELL = globals()["ALGO_BYTES_PER_CELL"] if mhd else ALGO_BYTES_PER_CELL_HD
+    ALGO_FLOPS_PER_CELL = globals()["ALGO_FLOPS_PER_CELL"] if mhd else {}
     kernels = {}
     for name, (kms, cnt) in prof.items():
         if cnt == 0:
@@ -253,11 +260,12 @@ def run_ours(args):
     per_launch = {k: v["avg_ms"] for k, v in kernels.items() if k in ALGO_BYTES_PER_CELL}
     dom = max(per_launch, key=per_launch.get)
     roof = roof_of(dom)
-    dom_alu = max((k for k in per_launch if k in ALGO_FLOPS_PER_CELL), key=per_launch.get)
-    roof_alu = roof_of(dom_alu)
-    step_hbm = ALGO_BYTES_PER_CELL_UPDATE * value / world * 1e-9
+    alu_kernels = [k for k in per_launch if k in ALGO_FLOPS_PER_CELL]
+    roof_alu = roof_of(max(alu_kernels, key=per_launch.get)) if alu_kernels else None
+    step_bytes = ALGO_BYTES_PER_CELL_UPDATE if mhd else ALGO_BYTES_PER_CELL_UPDATE_HD
+    step_hbm = step_bytes * value / world * 1e-9
     roof_step = {"bound": "hbm", "achieved": step_hbm, "peak": hbm_peak, "unit": "GB/s", "frac": step_hbm / hbm_peak,
-                 "what": "whole step: 320 algorithmic B per cell-update x cell-updates/s per GPU, of %s" % peak_kind}
+                 "what": "whole step: %d algorithmic B per cell-update x cell-updates/s per GPU, of %s" % (step_bytes, peak_kind)}
 
     # ---- end to end through the C ABI with host buffers --------------------------------------------
     e2e = None
@@ -291,8 +299,11 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "%s: %d^3 periodic ideal MHD, PLM van Leer + HLLD + CT upwind-contact + RK2, CFL %.2f, "
-                                   "seeded random-phase v and B=curl A (|k|<=8, Mach 1, beta 10)" % (args.workload, n, cfl),
+            "config": {"workload": ("%s: %d^3 periodic ideal MHD, PLM van Leer + HLLD + CT upwind-contact + RK2, CFL %.2f, "
+                                    "seeded random-phase v and B=curl A (|k|<=8, Mach 1, beta 10)" % (args.workload, n, cfl))
+                       if args.workload == "config5" else
+                       "%s recipe at %d^3 (solver %d, limiter %d, emf %d), CFL %.2f" % (
+                           args.workload, n, cfg["solver"], cfg["limiter"], cfg["emf"], cfl),
                        "grid": [n, n, n], "cells_per_gpu": cells, "parallelism": "replicas x%d" % world,
                        "l2": "inputs (%.1f GB state) larger than L2, no flush needed" % (8 * 8 * cells * 1e-9)},
             "gpu_launches": launches, "clocks": clocks, "e2e": e2e,

@@ -147,7 +147,8 @@ long long idfx_launch_count(const idfx_ctx* ctx);
  * CUDA-event pair on the bound stream.  idfx_profile_enable(ctx, 1) clears the accumulators and starts,
  * (ctx, 0) stops.  idfx_profile_read synchronises and returns the summed device time in milliseconds and
  * the number of launches of kernel class kernel_id; idfx_profile_kernel_name gives the class names
- * ("flux_x", "flux_y", "flux_z", "rhs_dtmax", "edge_emf", "ct_update_prim", "ghost_fill", "state_io"), NULL past the end. */
+ * ("flux_x", "flux_y", "flux_z", "rhs_dtmax", "edge_emf", "ct_update_prim", "ghost_fill", "state_io", "hd_stage"), NULL past
+ * the end. */
 int idfx_profile_enable(idfx_ctx* ctx, int on);
 int idfx_profile_read(idfx_ctx* ctx, int kernel_id, double* h_ms_total, long long* h_launches);
 const char* idfx_profile_kernel_name(int kernel_id);

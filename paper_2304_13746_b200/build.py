@@ -8,8 +8,8 @@ import sys
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SOURCES = [os.path.join(_HERE, "csrc", "idfx.cu"), os.path.join(_HERE, "csrc", "probe.cu")]
-HEADERS = [os.path.join(_HERE, "csrc", f) for f in ("physics.cuh", "common.cuh", "flux_march.cuh", "flux_march_tma.cuh")] + [ os.path.join(os.path.dirname(_HERE), "include", "idfx.h"),
-           os.path.join(os.path.dirname(_HERE), "include", "idfx_probe.h")]
+HEADERS = sorted(os.path.join(_HERE, "csrc", f) for f in os.listdir(os.path.join(_HERE, "csrc")) if f.endswith(".cuh")) + [
+    os.path.join(os.path.dirname(_HERE), "include", "idfx.h"), os.path.join(os.path.dirname(_HERE), "include", "idfx_probe.h")]
 LIB = os.path.join(_HERE, "libidfx.so")
 
 NVCC_FLAGS = [

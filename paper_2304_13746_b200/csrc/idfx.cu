@@ -17,6 +17,7 @@
 #include "common.cuh"
 #include "physics.cuh"
 #include "flux_march.cuh"
+#include "hd_stage.cuh"
 #include "flux_march_tma.cuh"
 
 namespace idfx {
@@ -635,9 +636,9 @@ enum {
 using namespace idfx;
 
 // kernel classes for idfx_profile_* (order = idfx_profile_kernel_name)
-enum { K_FLUX_X = 0, K_FLUX_Y, K_FLUX_Z, K_RHS, K_EMF, K_UPDATE, K_FILL, K_STATE, K_COUNT };
+enum { K_FLUX_X = 0, K_FLUX_Y, K_FLUX_Z, K_RHS, K_EMF, K_UPDATE, K_FILL, K_STATE, K_HD, K_COUNT };
 static const char* const kKernelNames[K_COUNT] = {"flux_x", "flux_y", "flux_z", "rhs_dtmax", "edge_emf",
-                                                  "ct_update_prim", "ghost_fill", "state_io"};
+                                                  "ct_update_prim", "ghost_fill", "state_io", "hd_stage"};
 
 struct idfx_ctx {
   Geom g;
@@ -667,6 +668,8 @@ struct idfx_ctx {
   bool use_graph = true;
   bool use_tma = false;            // y/z sweeps stage their planes through shared memory with TMA (MHD)
   CUtensorMap mapV[3], mapB[3];    // per sweep direction (1 = y, 2 = z): boxes over the V and face-B field groups
+  bool hd_fused = false;           // HD: one kernel per stage (hd_stage.cuh); IDFX_HD_FUSED=0 keeps the three sweeps
+  CUtensorMap mapHD;               // 36 x 11 x 1 x 5 boxes over the primitive fields
   long long launches = 0;
   // optional per-kernel timing with CUDA events on the bound stream (idfx_profile_*)
   bool prof_on = false;
@@ -760,6 +763,18 @@ int make_tensor_maps(idfx_ctx* c) {
   const cuuint64_t py = g.ny + 2 * NG, pz = g.nz + 2 * NG;
   const cuuint64_t strides[3] = {(cuuint64_t)g.sy * 8, (cuuint64_t)g.sz * 8, (cuuint64_t)g.np * 8};
   const cuuint32_t es[4] = {1, 1, 1, 1};
+  if (!c->mhd) {
+    const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, 22};
+    const cuuint32_t box[4] = {(cuuint32_t)HD_BW, (cuuint32_t)HD_BH, 1u, 5u};
+    CUresult r = enc(&c->mapHD, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_V), dimV, strides, box, es,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+      set_err("cuTensorMapEncodeTiled failed");
+      return IDFX_ERR_CUDA;
+    }
+    return IDFX_OK;
+  }
   for (int d = 0; d < 3; ++d) {
     const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, 22}, dimB[4] = {(cuuint64_t)g.sy, py, pz, 9};
     // x sweep: 36 columns x 4 rows of one z plane; y sweep: 32 x 1 x 4; z sweep: 32 x 4 x 1
@@ -1092,6 +1107,57 @@ void launch_ct(idfx_ctx* c, dim3 grid, const EmfArgs& ea, const UpdateArgs& a, b
   else launch_ct_v<MODE, false>(c, grid, ea, a, stage2, udone);
 }
 
+// ---- hydrodynamics: the whole stage in one kernel (hd_stage.cuh) ----
+typedef void (*HdKernel)(Geom, HdStageArgs, const CUtensorMap);
+
+template <int SOLVER, int LIM>
+HdKernel hd_kernel_sl(bool first) {
+  return first ? (HdKernel)k_hd_stage<SOLVER, LIM, true> : (HdKernel)k_hd_stage<SOLVER, LIM, false>;
+}
+
+template <int SOLVER>
+HdKernel hd_kernel_s(int limiter, bool first) {
+  switch (limiter) {
+    case LIM_FLAT: return hd_kernel_sl<SOLVER, LIM_FLAT>(first);
+    case LIM_MINMOD: return hd_kernel_sl<SOLVER, LIM_MINMOD>(first);
+    case LIM_LIMO3: return hd_kernel_sl<SOLVER, LIM_LIMO3>(first);
+    default: return hd_kernel_sl<SOLVER, LIM_VANLEER>(first);
+  }
+}
+
+HdKernel hd_kernel(const idfx_ctx* c, bool first) {
+  switch (c->solver) {
+    case SOLVER_HLL: return hd_kernel_s<SOLVER_HLL>(c->limiter, first);
+    case SOLVER_RUSANOV: return hd_kernel_s<SOLVER_RUSANOV>(c->limiter, first);
+    case SOLVER_HLLC: return hd_kernel_s<SOLVER_HLLC>(c->limiter, first);
+    default: return hd_kernel_s<SOLVER_ROE>(c->limiter, first);
+  }
+}
+
+void launch_hd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int uout) {
+  const Geom& g = c->g;
+  HdStageArgs a;
+  a.fV0 = c->vcur ? 11 : 0;
+  const long long per_chunk = (long long)((g.nx + HD_CX - 1) / HD_CX) * ((g.ny + HD_CY - 1) / HD_CY);
+  long long nch = (148 * 2 * 8 + per_chunk - 1) / per_chunk;  // about 8 waves of 2 CTAs per SM
+  const long long maxch = g.nz / 16 > 0 ? g.nz / 16 : 1;
+  nch = nch < 1 ? 1 : (nch > maxch ? maxch : nch);
+  a.chunk = (int)((g.nz + nch - 1) / nch);
+  for (int n = 0; n < 5; ++n) {
+    a.R[n] = c->field(F_R + n);
+    a.Uin[n] = c->field(uin + n);
+    a.U0[n] = c->field(F_UA + n);
+    a.Uout[n] = c->field(uout + n);
+    a.Vout[n] = c->vfield_out(n);
+  }
+  a.sc = c->sc;
+  a.w = w;
+  a.w0 = w0;
+  dim3 grid((g.nx + HD_CX - 1) / HD_CX, (g.ny + HD_CY - 1) / HD_CY, (unsigned)((g.nz + a.chunk - 1) / a.chunk));
+  LaunchScope ls(c, K_HD);
+  hd_kernel(c, first)<<<grid, HD_THREADS, HD_SMEM_BYTES, c->stream>>>(g, a, c->mapHD);
+}
+
 // One stage S_dt (O2) followed by the RK combine of Eq. 9.  s: stage index (0-based); bin: face buffer of the stage
 // input; b0: saved face buffer; bout: destination.  Conserved fields: U_0 lives in F_UA for the whole cycle, the
 // intermediate stages in F_UB, the last stage writes the result back to F_UA.
@@ -1103,7 +1169,15 @@ void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, d
   const double w = W[c->nstages - 1][s], w0 = W0[c->nstages - 1][s];
   const double* Bf[3] = {c->bbuf(bin, 0), c->bbuf(bin, 1), c->bbuf(bin, 2)};
   const ApplyInfo ap = {combine && c->mhd && c->use_tma, w, w0, uin, uout};
-  launch_sweeps(c, Bf, want_dt, ap);
+  if (c->hd_fused) {
+    launch_hd_stage(c, !combine, w, w0, uin, uout);
+    if (combine) {  // the kernel wrote U_s, its primitives and their ghost images into the other primitive buffer
+      c->vcur ^= 1;
+      return;
+    }
+  } else {
+    launch_sweeps(c, Bf, want_dt, ap);
+  }
   UpdateArgs a;
   for (int n = 0; n < 5; ++n) {
     a.Uin[n] = c->field(uin + n);
@@ -1317,10 +1391,15 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
   c->fixed_batch = benv ? atoi(benv) : 0;
   const char* env = getenv("IDFX_TMA");
   c->use_tma = c->mhd && !(env && env[0] == '0');  // IDFX_TMA=0 selects the register-prefetch sweeps (A/B only)
-  if (c->use_tma) {
+  const char* henv = getenv("IDFX_HD_FUSED");
+  c->hd_fused = !c->mhd && !(henv && henv[0] == '0');
+  if (c->use_tma || c->hd_fused) {
     int rc = make_tensor_maps(c);
     if (rc) return rc;
   }
+  if (c->hd_fused)
+    for (int first = 0; first < 2; ++first)
+      CK(cudaFuncSetAttribute((const void*)hd_kernel(c, first != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, HD_SMEM_BYTES));
   c->bound = true;
   return IDFX_OK;
 }
