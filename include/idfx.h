@@ -76,9 +76,13 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
  *     edge-centred vector potential, dA/dt = -E, and sets B = B_ref + curl A after every stage (Eq. 7-8),
  *     so that round-off cannot accumulate in div B.  B_ref is the face field given to idfx_set_state and A counts from
  *     zero there (reading G19: a periodic A cannot carry a mean field).  MHD only; must be chosen BEFORE
- *     idfx_workspace_bytes / idfx_bind (it needs 12 more fields). */
-enum { IDFX_OPT_INTEGRATOR = 0, IDFX_OPT_CT_FORM = 1, IDFX_OPT_PRESSURE_FLOOR = 2 };
+ *     idfx_workspace_bytes / idfx_bind (it needs 12 more fields).
+ *   IDFX_OPT_BOUNDARY: IDFX_BOUNDARY_PERIODIC (default) or IDFX_BOUNDARY_OUTFLOW: zero-gradient ghost cells on all six
+ *     sides (the paper's non-periodic tests).  Hydrodynamics only (IDFX_ERR_UNSUPPORTED with a magnetic
+ *     field: the staggered field on a boundary face needs its own treatment); set it before idfx_set_state. */
+enum { IDFX_OPT_INTEGRATOR = 0, IDFX_OPT_CT_FORM = 1, IDFX_OPT_PRESSURE_FLOOR = 2, IDFX_OPT_BOUNDARY = 3 };
 enum { IDFX_CT_FACE = 0, IDFX_CT_POTENTIAL = 1 };
+enum { IDFX_BOUNDARY_PERIODIC = 0, IDFX_BOUNDARY_OUTFLOW = 1 };
 int idfx_set_option(idfx_ctx* ctx, int option, int value);
 /* Real-valued options.  IDFX_OPT_PRESSURE_FLOOR (default 0 = none, reading G13): when > 0, a pressure below it met in
  * the cons->prim conversion is raised to it and the total energy of the cell is rewritten to match (energy is then no

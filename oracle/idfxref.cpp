@@ -42,7 +42,7 @@ constexpr int NG = 2;  // ghost layers: PLM needs 2 ("number of ghos
 
 enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_RUSANOV = 4 };
 enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3 };
-enum { OPT_INTEGRATOR = 0, OPT_CT_FORM = 1, OPT_PRESSURE_FLOOR = 2 };  // idfxref_set_option / idfxref_set_option_real
+enum { OPT_INTEGRATOR = 0, OPT_CT_FORM = 1, OPT_PRESSURE_FLOOR = 2, OPT_BOUNDARY = 3 };  // idfxref_set_option / idfxref_set_option_real
 enum { CT_FACE = 0, CT_POTENTIAL = 1 };
 enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3, EMF_UCT_HLL = 4 };
 enum { OK = 0, ERR_INVALID_ARG = -1, ERR_UNSUPPORTED = -2, ERR_UNPHYSICAL = -5 };
@@ -542,6 +542,7 @@ struct Ctx {
   Arr A[3], A0[3], As[3], Bref[3];  // CT_POTENTIAL: edge potential accumulated since set_state (same places as E),
                                     // its saved and scratch copies, and the face field given to set_state (G19)
   double t;                         // time since set_state
+  int outflow;                      // 0: periodic; 1: zero-gradient ghosts on all six sides (HD only)
   double pfloor;                    // optional pressure floor (0 = none, G13); see compute_prims
   long long nfloor;                 // how often it acted since set_state
   double last_dt;
@@ -561,6 +562,27 @@ inline int pmod(int a, int n) {
 // a1 / O2(i): periodic fill, 2 layers, x then y then z (PAPER.md:233 sequential per-dimension order).
 void fill_periodic(const Ctx& c, Arr& a) {
   const int nx = c.n[0], ny = c.n[1], nz = c.n[2];
+  if (c.outflow) {  // zero gradient, same sequential order: each ghost layer copies the last active cell of its line
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int gI = 1; gI <= NG; ++gI) {
+          a[c.at(-gI, j, k)] = a[c.at(0, j, k)];
+          a[c.at(nx - 1 + gI, j, k)] = a[c.at(nx - 1, j, k)];
+        }
+    for (int k = 0; k < nz; ++k)
+      for (int gI = 1; gI <= NG; ++gI)
+        for (int i = -NG; i < nx + NG; ++i) {
+          a[c.at(i, -gI, k)] = a[c.at(i, 0, k)];
+          a[c.at(i, ny - 1 + gI, k)] = a[c.at(i, ny - 1, k)];
+        }
+    for (int gI = 1; gI <= NG; ++gI)
+      for (int j = -NG; j < ny + NG; ++j)
+        for (int i = -NG; i < nx + NG; ++i) {
+          a[c.at(i, j, -gI)] = a[c.at(i, j, 0)];
+          a[c.at(i, j, nz - 1 + gI)] = a[c.at(i, j, nz - 1)];
+        }
+    return;
+  }
   for (int k = 0; k < nz; ++k)
     for (int j = 0; j < ny; ++j)
       for (int gI = 1; gI <= NG; ++gI) {
@@ -925,7 +947,7 @@ IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, doubl
       }
   }
   c.Bstage = nullptr;
-  c.nstages = 2; c.ct_form = CT_FACE; c.t = 0.0; c.pfloor = 0.0; c.nfloor = 0;
+  c.nstages = 2; c.ct_form = CT_FACE; c.t = 0.0; c.pfloor = 0.0; c.nfloor = 0; c.outflow = 0;
   c.last_dt = 0.0; c.status = OK; c.roe_fallbacks = 0;
   return h;
 }
@@ -939,6 +961,10 @@ IDFXREF_API int idfxref_set_option(idfxref_ctx* h, int option, int value) {
   Ctx& c = h->c;
   if (option == OPT_INTEGRATOR && value >= 1 && value <= 3) {
     c.nstages = value;
+    return OK;
+  }
+  if (option == OPT_BOUNDARY && (value == 0 || (value == 1 && !c.mhd))) {
+    c.outflow = value;
     return OK;
   }
   if (option == OPT_CT_FORM && (value == CT_FACE || (value == CT_POTENTIAL && c.mhd))) {

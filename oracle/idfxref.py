@@ -16,7 +16,8 @@ _LIB = os.path.join(_HERE, "libidfxref.so")
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
 LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3 = 0, 1, 2, 3
-OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR = 0, 1, 2
+OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR, OPT_BOUNDARY = 0, 1, 2, 3
+BOUNDARY_PERIODIC, BOUNDARY_OUTFLOW = 0, 1
 CT_FACE, CT_POTENTIAL = 0, 1
 EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0, EMF_UCT_HLL = 0, 1, 2, 3, 4
 OK, ERR_UNPHYSICAL = 0, -5
@@ -98,7 +99,8 @@ def _c(a):
 class Oracle:
     """One oracle context: a periodic nx*ny*nz box (arrays are [var][nz][ny][nx])."""
 
-    def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode, nstages=2, ct_form=CT_FACE, pressure_floor=0.0):
+    def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode, nstages=2, ct_form=CT_FACE, pressure_floor=0.0,
+                 boundary=BOUNDARY_PERIODIC):
         self.L = lib()
         self.shape = (nz, ny, nx)
         self.mhd = emf_mode != EMF_NONE
@@ -111,6 +113,8 @@ class Oracle:
             raise ValueError("bad CT form")
         if pressure_floor and self.L.idfxref_set_option_real(self.h, OPT_PRESSURE_FLOOR, pressure_floor) != OK:
             raise ValueError("bad pressure floor")
+        if boundary != BOUNDARY_PERIODIC and self.L.idfxref_set_option(self.h, OPT_BOUNDARY, boundary) != OK:
+            raise ValueError("bad boundary (outflow is HD-only)")
 
     def close(self):
         if self.h:

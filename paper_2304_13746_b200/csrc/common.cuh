@@ -14,6 +14,7 @@ struct Geom {
   long long np;   // padded field size in doubles
   long long nc;   // nx*ny*nz
   double dx, gamma;
+  int outflow;    // 0: periodic box; 1: zero-gradient (outflow) ghosts on all six sides (hydrodynamics only)
   double pfloor;  // > 0: pressures below it are raised to it in cons->prim and E is rewritten (idfx_set_option_real); 0: none (G13)
   __host__ __device__ __forceinline__ long long at(int i, int j, int k) const {
     return (long long)(k + NG) * sz + (long long)(j + NG) * sy + (i + IOFF);

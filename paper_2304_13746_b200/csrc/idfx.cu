@@ -46,8 +46,9 @@ __global__ void k_unpack(Geom g, FieldList srcf, double* __restrict__ dst) {
   for (int n = 0; n < srcf.n; ++n) dst[n * g.nc + s] = srcf.f[n][c];
 }
 
-// a1: periodic ghost fill of a list of fields, one thread per ghost cell.  Every ghost cell copies from its
-// wrapped active image, which equals the sequential x, y, z fill of O2 (i).
+// a1: ghost fill of a list of fields, one thread per ghost cell.  Periodic: every ghost cell copies from its
+// wrapped active image, which equals the sequential x, y, z fill of O2 (i).  Outflow (HD only): from the
+// nearest active cell, which equals the sequential zero-gradient fill.
 __global__ void k_fill_ghost(Geom g, FieldList fl) {
   const int px = g.nx + 2 * NG, py = g.ny + 2 * NG;
   const long long nZ = 2LL * NG * py * px;             // k in ghost
@@ -76,7 +77,12 @@ __global__ void k_fill_ghost(Geom g, FieldList fl) {
   } else {
     return;
   }
-  const int is = (i + g.nx) % g.nx, js = (j + g.ny) % g.ny, ks = (k + g.nz) % g.nz;
+  int is = (i + g.nx) % g.nx, js = (j + g.ny) % g.ny, ks = (k + g.nz) % g.nz;
+  if (g.outflow) {  // zero gradient: the nearest active cell
+    is = min(max(i, 0), g.nx - 1);
+    js = min(max(j, 0), g.ny - 1);
+    ks = min(max(k, 0), g.nz - 1);
+  }
   const long long d = g.at(i, j, k), s = g.at(is, js, ks);
   for (int n = 0; n < fl.n; ++n) fl.f[n][d] = fl.f[n][s];
 }
@@ -1173,6 +1179,7 @@ void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, d
     launch_hd_stage(c, !combine, w, w0, uin, uout);
     if (combine) {  // the kernel wrote U_s, its primitives and their ghost images into the other primitive buffer
       c->vcur ^= 1;
+      if (c->g.outflow) launch_fill(c, bout);  // it writes periodic images only
       return;
     }
   } else {
@@ -1348,6 +1355,7 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
   g.dx = dx;
   g.gamma = gamma;
   g.pfloor = 0.0;
+  g.outflow = 0;
   g.sy = ((nx + IOFF + NG + 15) / 16) * 16;
   g.sz = (long long)g.sy * (ny + 2 * NG);
   g.np = ((g.sz * (nz + 2 * NG) + 31) / 32) * 32;
@@ -1656,6 +1664,15 @@ int idfx_set_option(idfx_ctx* c, int option, int value) {
   if (option == 0 /* IDFX_OPT_INTEGRATOR */ && value >= 1 && value <= 3) {
     if (value != c->nstages) drop_graphs(c);
     c->nstages = value;
+    return IDFX_OK;
+  }
+  if (option == 3 /* IDFX_OPT_BOUNDARY */ && (value == 0 || value == 1)) {
+    if (value == 1 && c->mhd) {
+      set_err("idfx_set_option: outflow boundaries are implemented for hydrodynamics only");
+      return IDFX_ERR_UNSUPPORTED;
+    }
+    if (value != c->g.outflow) drop_graphs(c);
+    c->g.outflow = value;
     return IDFX_OK;
   }
   if (option == 1 /* IDFX_OPT_CT_FORM */ && (value == 0 || value == 1)) {

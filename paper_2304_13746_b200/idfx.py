@@ -11,7 +11,8 @@ import torch
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
 LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3 = 0, 1, 2, 3
-OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR = 0, 1, 2
+OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR, OPT_BOUNDARY = 0, 1, 2, 3
+BOUNDARY_PERIODIC, BOUNDARY_OUTFLOW = 0, 1
 CT_FACE, CT_POTENTIAL = 0, 1
 EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0, EMF_UCT_HLL = 0, 1, 2, 3, 4
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_NOT_BOUND, ERR_CUDA, ERR_UNPHYSICAL = 0, -1, -2, -3, -4, -5
@@ -97,7 +98,7 @@ class Idfx:
     """One periodic nx*ny*nz box on one GPU.  Tensors are float64, [var][nz][ny][nx]."""
 
     def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode, device="cuda:0", stream=None, nstages=2,
-                 ct_form=CT_FACE, pressure_floor=0.0):
+                 ct_form=CT_FACE, pressure_floor=0.0, boundary=BOUNDARY_PERIODIC):
         self.L = lib()
         self.h = self.L.idfx_create(nx, ny, nz, dx, gamma, solver, limiter, emf_mode)
         if not self.h:
@@ -108,6 +109,8 @@ class Idfx:
             _check(self.L.idfx_set_option(self.h, OPT_CT_FORM, ct_form))
         if pressure_floor:
             _check(self.L.idfx_set_option_real(self.h, OPT_PRESSURE_FLOOR, pressure_floor))
+        if boundary != BOUNDARY_PERIODIC:
+            _check(self.L.idfx_set_option(self.h, OPT_BOUNDARY, boundary))
         if not torch.cuda.is_available():
             raise RuntimeError("idfx needs a CUDA device; there is no CPU fallback")
         self.device = torch.device(device)

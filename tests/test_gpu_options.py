@@ -189,3 +189,40 @@ def test_sedov_blast_parity_and_radius(idfx, R):
         r_num = (int(torch.argmax(line)) + 0.5) / n
         assert abs(r_num - r_exact) <= 2.0 / n, (r_num, r_exact)
     assert float(rho.max()) > 2.5
+
+
+@pytest.mark.parametrize("fused", ["1", "0"])
+def test_outflow_boundaries_hd(idfx, R, fused, monkeypatch):
+    """Zero-gradient ghosts (HD only): the paper's Sod tube with outflow ends along each axis, and a 3D blast reaching
+    the walls, against the oracle; both the fused stage kernel and the three-sweep path."""
+    monkeypatch.setenv("IDFX_HD_FUSED", fused)
+    for axis in range(3):
+        shape = [6, 5, 4]
+        shape[2 - axis] = 64
+        nz, ny, nx = shape
+        bc = [1, 1, 1]
+        bc[2 - axis] = 64
+        left = ((np.arange(64) + 0.5) / 64 < 0.5).reshape(bc)
+        prim = np.zeros([5] + shape)
+        prim[0] = np.where(left, 1.0, 0.125)
+        prim[4] = np.where(left, 1.0, 0.1)
+        sim = idfx.Idfx(nx, ny, nz, 1.0 / 64, 1.4, ROE, VANLEER, EMF_NONE, boundary=idfx.BOUNDARY_OUTFLOW)
+        sim.set_state(torch.from_numpy(prim).cuda())
+        ref = R.Oracle(nx, ny, nz, 1.0 / 64, 1.4, ROE, VANLEER, EMF_NONE, boundary=R.BOUNDARY_OUTFLOW)
+        ref.set_state(prim)
+        n_g, _ = sim.advance_to(0.2, 0.4)
+        rc, n_r = ref.advance_to(0.2, 0.4)
+        assert rc == 0 and n_g == n_r
+        assert_state_close(sim, ref, TOL, "Sod, outflow, axis %d" % axis)
+    n = 24
+    prim, _ = inputs.sedov(n)
+    sim = idfx.Idfx(n, n, n, 1.0 / n, G53, HLL, VANLEER, EMF_NONE, boundary=idfx.BOUNDARY_OUTFLOW, nstages=3)
+    sim.set_state(prim.cuda())
+    ref = R.Oracle(n, n, n, 1.0 / n, G53, HLL, VANLEER, EMF_NONE, boundary=R.BOUNDARY_OUTFLOW, nstages=3)
+    ref.set_state(prim.numpy())
+    sim.advance_to(0.2, 0.3)       # the shock (r = 0.61 at t = 0.2) has left through the walls
+    ref.advance_to(0.2, 0.3)
+    assert_state_close(sim, ref, TOL, "blast through outflow walls")
+    assert float(sim.get_conserved()[0][4].sum()) / n ** 3 < 0.9     # energy left the box
+    with pytest.raises(idfx.IdfxError):
+        idfx.Idfx(8, 8, 8, 0.125, G53, HLLD, VANLEER, EMF_UCT, boundary=idfx.BOUNDARY_OUTFLOW)
