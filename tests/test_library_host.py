@@ -66,6 +66,37 @@ def test_unbound_context_refuses_to_run(L):
     assert L.idfx_step(None, 0.1) == idfx.ERR_INVALID_ARG
 
 
+def test_options_are_validated_on_the_host(L):
+    """idfx_set_option / idfx_set_option_real touch no device memory: every rule of include/idfx.h can be checked here."""
+    hd = L.idfx_create(8, 8, 8, 0.1, 1.4, idfx.SOLVER_HLL, idfx.LIMITER_LIMO3, idfx.EMF_NONE)
+    mhd = L.idfx_create(8, 8, 8, 0.1, 1.4, idfx.SOLVER_HLLD, idfx.LIMITER_VANLEER, idfx.EMF_UCT_HLL)
+    assert hd and mhd
+    for h in (hd, mhd):
+        for stages in (1, 2, 3):
+            assert L.idfx_set_option(h, idfx.OPT_INTEGRATOR, stages) == idfx.OK
+        for bad in (0, 4, -1):
+            assert L.idfx_set_option(h, idfx.OPT_INTEGRATOR, bad) == idfx.ERR_INVALID_ARG
+        assert L.idfx_set_option(h, 99, 0) == idfx.ERR_INVALID_ARG
+        assert L.idfx_set_option_real(h, idfx.OPT_PRESSURE_FLOOR, 1e-6) == idfx.OK
+        assert L.idfx_set_option_real(h, idfx.OPT_PRESSURE_FLOOR, -1.0) == idfx.ERR_INVALID_ARG
+        assert L.idfx_set_option_real(h, idfx.OPT_INTEGRATOR, 2.0) == idfx.ERR_INVALID_ARG
+    # the vector potential needs a magnetic field, outflow boundaries must not have one
+    assert L.idfx_set_option(hd, idfx.OPT_CT_FORM, idfx.CT_POTENTIAL) == idfx.ERR_UNSUPPORTED
+    assert L.idfx_set_option(mhd, idfx.OPT_BOUNDARY, idfx.BOUNDARY_OUTFLOW) == idfx.ERR_UNSUPPORTED
+    assert L.idfx_set_option(hd, idfx.OPT_BOUNDARY, idfx.BOUNDARY_OUTFLOW) == idfx.OK
+    # the workspace grows by 12 fields with the potential (and holds 15 more for the 2D-HLL EMF)
+    w_face = L.idfx_workspace_bytes(mhd)
+    assert L.idfx_set_option(mhd, idfx.OPT_CT_FORM, idfx.CT_POTENTIAL) == idfx.OK
+    w_pot = L.idfx_workspace_bytes(mhd)
+    plain = L.idfx_create(8, 8, 8, 0.1, 1.4, idfx.SOLVER_HLLD, idfx.LIMITER_VANLEER, idfx.EMF_UCT_CONTACT)
+    w_plain = L.idfx_workspace_bytes(plain)
+    field = (w_pot - w_face) // 12
+    assert field * 12 == w_pot - w_face and w_face - w_plain == 15 * field and field >= 12 ** 3 * 8
+    for h in (hd, mhd, plain):
+        L.idfx_destroy(h)
+    assert L.idfx_set_option(None, idfx.OPT_INTEGRATOR, 2) == idfx.ERR_INVALID_ARG
+
+
 def test_binding_fails_loudly_without_gpu():
     if torch.cuda.is_available():
         pytest.skip("a GPU is present")
