@@ -226,3 +226,35 @@ def test_outflow_boundaries_hd(idfx, R, fused, monkeypatch):
     assert float(sim.get_conserved()[0][4].sum()) / n ** 3 < 0.9     # energy left the box
     with pytest.raises(idfx.IdfxError):
         idfx.Idfx(8, 8, 8, 0.125, G53, HLLD, VANLEER, EMF_UCT, boundary=idfx.BOUNDARY_OUTFLOW)
+
+
+def test_all_options_together_medium_box(idfx, R):
+    """RK3 + LimO3 + 2D-HLL EMF + vector potential + a floor on a box that spans many tiles in every direction and has
+    ragged tails (96 x 80 x 72): two cycles against the oracle."""
+    nx, ny, nz = 96, 80, 72
+    prim, b, dx = smooth_ic(nx, ny, nz, 31)
+    sim, ref = None, None
+    sim = idfx.Idfx(nx, ny, nz, dx, G53, HLLD, LIMO3, EMF_UCT_HLL, nstages=3, ct_form=1, pressure_floor=1e-8)
+    sim.set_state(torch.from_numpy(prim).cuda(), torch.from_numpy(b).cuda())
+    ref = R.Oracle(nx, ny, nz, dx, G53, HLLD, LIMO3, EMF_UCT_HLL, nstages=3, ct_form=1, pressure_floor=1e-8)
+    ref.set_state(prim, b)
+    sim.advance(2, 0.3)
+    ref.advance(2, 0.3)
+    assert abs(sim.last_dt() - ref.last_dt()) <= TOL_DT * ref.last_dt()
+    assert_state_close(sim, ref, TOL, "all options, 96 x 80 x 72")
+    assert sim.floor_count() == 0 == ref.floor_count()
+
+
+def test_hd_fused_kernel_ragged_and_chunked(idfx, R):
+    """The one-kernel HD stage on a box whose sizes are not multiples of its 31 x 7 tiles and whose z extent splits into
+    several chunks, RK3 + LimO3 + HLLC, against the oracle and against the three-sweep path."""
+    nx, ny, nz = 70, 45, 150
+    prim, _, dx = smooth_ic(nx, ny, nz, 17, mhd=False)
+    sim = idfx.Idfx(nx, ny, nz, dx, G53, HLLC, LIMO3, EMF_NONE, nstages=3)
+    sim.set_state(torch.from_numpy(prim).cuda())
+    ref = R.Oracle(nx, ny, nz, dx, G53, HLLC, LIMO3, EMF_NONE, nstages=3)
+    ref.set_state(prim)
+    sim.advance(2, 0.4)
+    ref.advance(2, 0.4)
+    assert abs(sim.last_dt() - ref.last_dt()) <= TOL_DT * ref.last_dt()
+    assert_state_close(sim, ref, TOL, "fused HD stage, 70 x 45 x 150")
