@@ -84,30 +84,40 @@ IDFX_DEV double limited_slope(double dm, double dp) {
   }
 }
 
-// LimO3 (Cada & Torrilhon 2009; reading G18): phi(theta) * dplus with theta = dminus/dplus,
-// written without the division: with s = sign(dplus), a = |dplus|, b = s dminus and P = (2a + b)/3,
-//   limited = s max(0, min(P, max(-b/2, min(2b, P, 1.6 a)))),  unlimited = (2 dplus + dminus)/3,
-// the unlimited value where eta = (dminus^2 + dplus^2)/dx^2 < 1 (smooth data), a linear blend within 1e-12 of eta = 1.
-IDFX_DEV double limo3_increment(double dminus, double dplus, double dx2) {
-  const double unl = (2.0 * dplus + dminus) * (1.0 / 3.0);
+// LimO3 (Cada & Torrilhon 2009; reading G18): the increment phi(theta) * dplus with
+// theta = dminus/dplus, limited branch, written without the division: with s = sign(dplus), a = |dplus|, b = s dminus
+// and P = (2a + b)/3,  phi dplus = s max(0, min(P, max(-b/2, min(2b, P, 1.6 a)))).
+IDFX_DEV double limo3_limited(double dminus, double dplus) {
   const double a = fabs(dplus), b = dplus < 0.0 ? -dminus : dminus;
   const double P = (2.0 * a + b) * (1.0 / 3.0);
   const double l = fmax(0.0, fmin(P, fmax(-0.5 * b, fmin(fmin(2.0 * b, P), 1.6 * a))));
-  const double lim = dplus < 0.0 ? -l : l;
-  const double num = dminus * dminus + dplus * dplus;
-  const double eps = 1e-12;
-  if (num <= (1.0 - eps) * dx2) return unl;
-  if (num >= (1.0 + eps) * dx2) return lim;
-  const double x = (num / dx2 - 1.0) / eps;  // rare: the blend zone
-  return 0.5 * ((1.0 - x) * unl + (1.0 + x) * lim);
+  return dplus < 0.0 ? -l : l;
 }
 
 // S2: values of cell i's reconstruction at its lower and upper faces; dm = q_i - q_{i-1}, dp = q_{i+1} - q_i.
+// LimO3: the smoothness measure eta = (dm^2 + dp^2)/dx^2 is shared by both faces; where eta < 1 (most cells of a resolved
+// flow) the unlimited third-order weights (2 + theta)/3 are used and the limiter is never evaluated; a linear blend
+// within 1e-12 of eta = 1 (a true division only there).
 template <int LIM>
 IDFX_DEV void face_values(double q, double dm, double dp, double dx2, double& lower, double& upper) {
   if (LIM == LIM_LIMO3) {
-    upper = q + 0.5 * limo3_increment(dm, dp, dx2);
-    lower = q - 0.5 * limo3_increment(dp, dm, dx2);
+    const double eps = 1e-12;
+    const double num = dm * dm + dp * dp;
+    double iu = (2.0 * dp + dm) * (1.0 / 3.0);  // upper face: phi(theta) dp
+    double il = (2.0 * dm + dp) * (1.0 / 3.0);  // lower face: phi(1/theta) dm
+    if (num > (1.0 - eps) * dx2) {
+      const double lu = limo3_limited(dm, dp), ll = limo3_limited(dp, dm);
+      if (num >= (1.0 + eps) * dx2) {
+        iu = lu;
+        il = ll;
+      } else {
+        const double x = (num / dx2 - 1.0) / eps;
+        iu = 0.5 * ((1.0 - x) * iu + (1.0 + x) * lu);
+        il = 0.5 * ((1.0 - x) * il + (1.0 + x) * ll);
+      }
+    }
+    upper = q + 0.5 * iu;
+    lower = q - 0.5 * il;
   } else {
     const double s = limited_slope<LIM>(dm, dp);
     lower = q - 0.5 * s;
