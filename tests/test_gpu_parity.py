@@ -243,6 +243,14 @@ def test_minimum_size_box(idfx, R):
     sim.advance(3, 0.3)
     ref.advance(3, 0.3)
     assert_state_close(sim, ref, TOL)
+    # hydrodynamics: the one-kernel stage with a box far smaller than its 31 x 7 tile and its 4-stage plane ring
+    for shape in ((4, 4, 4), (6, 4, 5)):
+        prim, _, dx = smooth_ic(*shape, 22, mhd=False)
+        sim, ref = make_pair(idfx, R, *shape, dx, 5.0 / 3.0, HLLC, MINMOD, EMF_NONE, prim, None)
+        sim.advance(3, 0.4)
+        ref.advance(3, 0.4)
+        assert abs(sim.last_dt() - ref.last_dt()) <= TOL_DT * ref.last_dt()
+        assert_state_close(sim, ref, TOL, "HD %dx%dx%d" % shape)
 
 
 def test_alternate_code_paths_in_a_subprocess(idfx):
@@ -266,5 +274,12 @@ def test_alternate_code_paths_in_a_subprocess(idfx):
     ) % (os.path.dirname(os.path.dirname(os.path.abspath(__file__))), os.path.dirname(os.path.abspath(__file__)))
     for env_add in ({"IDFX_TMA": "0"}, {"IDFX_GRAPH": "0"}, {"IDFX_TMA": "0", "IDFX_GRAPH": "0"}):
         p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300,
+                           env=dict(os.environ, **env_add))
+        assert p.returncode == 0 and "ok" in p.stdout, (env_add, p.stderr[-2000:])
+    # hydrodynamics: IDFX_HD_FUSED=0 selects the three-sweep path instead of the one-kernel stage
+    code_hd = code.replace("T.smooth_ic(37, 21, 13, 11)", "T.smooth_ic(37, 21, 13, 11, mhd=False)").replace(
+        "T.HLLD, T.VANLEER, T.EMF_UCT", "T.HLLC, T.VANLEER, T.EMF_NONE")
+    for env_add in ({"IDFX_HD_FUSED": "0"}, {"IDFX_HD_FUSED": "0", "IDFX_GRAPH": "0"}, {"IDFX_GRAPH": "0"}):
+        p = subprocess.run([sys.executable, "-c", code_hd], capture_output=True, text=True, timeout=300,
                            env=dict(os.environ, **env_add))
         assert p.returncode == 0 and "ok" in p.stdout, (env_add, p.stderr[-2000:])
