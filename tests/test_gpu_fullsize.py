@@ -142,3 +142,61 @@ def test_config5_512_windows_against_oracle(idfx, R):
         del p0, b0, c1, b1
     assert sim.status() == 0
     print("config5 512^3: worst relative window error %.3e" % worst)
+
+
+def test_config2_recipe_512_hd_windows_against_oracle(idfx, R):
+    """Hydrodynamics at 512^3 (config 2 recipe, the size bench.py --workload config2 --n 512 and the Sedov workload run
+    at) through the one-kernel stage, in the launch configuration used there: dt against the oracle on windows around the
+    fastest cells, then one cycle on 10 windows (corners of the periodic box, tile and chunk seams, random places)."""
+    name, W, M = "config2", 32, 10
+    prim, _, cfg = inputs.make(name, n=512, device="cuda")
+    n, dx, cfl = cfg["n"], cfg["dx"], cfg["cfl"]
+    sim = idfx.Idfx(n, n, n, dx, cfg["gamma"], cfg["solver"], cfg["limiter"], cfg["emf"])
+    sim.set_state(prim, None)
+    del prim
+    rng = np.random.default_rng(6)
+    origins = [(0, 0, 0), (n - 16, n - 16, n - 16), (31 * 7 - 16, 7 * 30 - 16, 128 - 16), (n - 20, 3, 250)]
+    origins += [tuple(int(x) for x in rng.integers(0, n, 3)) for _ in range(6)]
+    worst = 0.0
+    for cycle in range(2):
+        p0, _ = sim.get_state()
+        est = torch.sqrt(cfg["gamma"] * p0[4] / p0[0]) * 3 + p0[1].abs() + p0[2].abs() + p0[3].abs()
+        top = torch.topk(est.flatten(), 4096).indices.cpu().numpy()
+        del est
+        hot = []
+        for f in top:
+            kz, jy, ix = np.unravel_index(int(f), (n, n, n))
+            o = (int(ix) - W // 2, int(jy) - W // 2, int(kz) - W // 2)
+            if all(max(abs(o[0] - h[0]), abs(o[1] - h[1]), abs(o[2] - h[2])) > 6 for h in hot):
+                hot.append(o)
+            if len(hot) == 6:
+                break
+        dt_gpu = sim.compute_dt(cfl)
+        smax = 0.0
+        for o in hot:
+            ref = R.Oracle(W, W, W, dx, cfg["gamma"], cfg["solver"], cfg["limiter"], cfg["emf"])
+            ref.set_state(cut(p0, o, W).cpu().numpy())
+            ref.compute_dt(cfl)
+            s = np.zeros((W, W, W))
+            for d in range(3):
+                cface = ref.get_flux(d)[1]
+                s += np.maximum(cface, np.roll(cface, -1, 2 - d))
+            smax = max(smax, float(s[M:W - M, M:W - M, M:W - M].max()) / dx)
+        assert abs(cfl / smax - dt_gpu) <= TOL_DT * dt_gpu, (cfl / smax, dt_gpu)
+        sim.advance(1, cfl)
+        assert abs(sim.last_dt() - dt_gpu) <= 1e-14 * dt_gpu
+        c1, _ = sim.get_conserved()
+        scale_c = [float(c1[v].abs().max()) for v in range(5)]
+        for o in origins:
+            ref = R.Oracle(W, W, W, dx, cfg["gamma"], cfg["solver"], cfg["limiter"], cfg["emf"])
+            ref.set_state(cut(p0, o, W).cpu().numpy())
+            ref.step(dt_gpu)
+            rc, _ = ref.get_conserved()
+            gc = cut(c1, o, W).cpu().numpy()
+            sl = (slice(None), slice(M, W - M), slice(M, W - M), slice(M, W - M))
+            for v in range(5):
+                err = np.abs(gc[sl][v] - rc[sl][v]).max() / scale_c[v]
+                worst = max(worst, err)
+                assert err <= TOL, ("cycle", cycle, "window", o, "cons", v, err)
+    assert sim.status() == 0
+    print("config2 recipe at 512^3 (HD, fused stage kernel): worst relative error on %d windows x 2 cycles %.3e" % (len(origins), worst))
