@@ -179,6 +179,13 @@ __global__ void __launch_bounds__(HD_THREADS, IDFX_MINB_HD) k_hd_stage(Geom g, H
 #pragma unroll
       for (int n = 0; n < 5; ++n) qp[n] = t[ZQ[n]];
     }
+    if (!FIRST && complete && s < s1) {  // the conserved inputs of cell s are needed one plane from now
+#pragma unroll
+      for (int n = 0; n < 5; ++n) {
+        prefetch_l1(a.Uin[n] + c);
+        prefetch_l1(a.U0[n] + c);
+      }
+    }
     // ---- z face s-1/2: closes cell s-1 ----
     double WR[7], WLn[7], F[7];
 #pragma unroll
