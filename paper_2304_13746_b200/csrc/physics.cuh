@@ -141,6 +141,18 @@ IDFX_DEV void face_values(double q, double dm, double dp, double dx2, double& lo
     }
     upper = q + 0.5 * iu;
     lower = q - 0.5 * il;
+  } else if (LIM == LIM_VANLEER) {
+    // half the harmonic-mean slope, dm dp / (dm + dp): the same bits as 0.5 * limited_slope (powers of two are exact),
+    // one multiplication less; at an extremum the quotient (possibly 0/0) is discarded by the select
+    const double prod = dm * dp;
+#ifdef IDFX_PRECISE_MATH
+    const double h = prod > 0.0 ? prod / (dm + dp) : 0.0;
+#else
+    const double hq = prod * rcp(dm + dp);
+    const double h = prod > 0.0 ? hq : 0.0;
+#endif
+    lower = q - h;
+    upper = q + h;
   } else {
     const double s = limited_slope<LIM>(dm, dp);
     lower = q - 0.5 * s;
@@ -192,10 +204,11 @@ IDFX_DEV double signal_speed(const double W[7], double Bn, double g) {
   const double ir = rcp(W[0]);
   const double a2 = g * W[4] * ir;
   if (!MHD) return sqrt_pos(a2);
-  const double bn2 = Bn * Bn * ir;
-  const double b2 = bn2 + (W[5] * W[5] + W[6] * W[6]) * ir;
-  const double s = a2 + b2;
-  const double disc = fmax(s * s - 4.0 * a2 * bn2, 0.0);
+  // (a2 + b2)^2 - 4 a2 bn2 written as (a2 - b2)^2 + 4 a2 bt2: a sum of non-negative terms, no clamp needed
+  const double bt2 = (W[5] * W[5] + W[6] * W[6]) * ir;
+  const double b2 = Bn * Bn * ir + bt2;
+  const double s = a2 + b2, d = a2 - b2;
+  const double disc = fma(d, d, 4.0 * a2 * bt2);
   return sqrt_pos(0.5 * (s + sqrt_nn(disc)));
 }
 
@@ -376,20 +389,21 @@ IDFX_DEV bool roe_inner(const double WL[7], const double WR[7], double Bn, const
 // combination are evaluated only for the side K the selection of O7 picks (K = L when S_L >= 0, R when S_R <= 0).
 IDFX_DEV double hlld_onesided(const double WL[7], const double WR[7], double Bn, double g, double F[7]) {
   const double Bn2 = Bn * Bn;
-  const double pbL = 0.5 * (Bn2 + WL[5] * WL[5] + WL[6] * WL[6]);
-  const double pbR = 0.5 * (Bn2 + WR[5] * WR[5] + WR[6] * WR[6]);
+  const double bt2L = WL[5] * WL[5] + WL[6] * WL[6], bt2R = WR[5] * WR[5] + WR[6] * WR[6];
+  const double b2L = Bn2 + bt2L, b2R = Bn2 + bt2R;
+  const double pbL = 0.5 * b2L, pbR = 0.5 * b2R;
   const double pTL = WL[4] + pbL, pTR = WR[4] + pbR;
   const double uL = WL[1], uR = WR[1];
   double cL, cR;
-  {
+  {  // fast speed; (a2 + b2)^2 - 4 a2 bn2 = (a2 - b2)^2 + 4 a2 bt2 is a sum of non-negative terms (no clamp)
     const double ir = rcp(WL[0]);
-    const double a2 = g * WL[4] * ir, bn2 = Bn2 * ir, sm = a2 + 2.0 * pbL * ir;
-    cL = sqrt_pos(0.5 * (sm + sqrt_nn(fmax(sm * sm - 4.0 * a2 * bn2, 0.0))));
+    const double a2 = g * WL[4] * ir, sm = fma(b2L, ir, a2), dm = fma(-b2L, ir, a2);
+    cL = sqrt_pos(0.5 * (sm + sqrt_nn(fma(dm, dm, 4.0 * a2 * (bt2L * ir)))));
   }
   {
     const double ir = rcp(WR[0]);
-    const double a2 = g * WR[4] * ir, bn2 = Bn2 * ir, sm = a2 + 2.0 * pbR * ir;
-    cR = sqrt_pos(0.5 * (sm + sqrt_nn(fmax(sm * sm - 4.0 * a2 * bn2, 0.0))));
+    const double a2 = g * WR[4] * ir, sm = fma(b2R, ir, a2), dm = fma(-b2R, ir, a2);
+    cR = sqrt_pos(0.5 * (sm + sqrt_nn(fma(dm, dm, 4.0 * a2 * (bt2R * ir)))));
   }
   const double SL = fmin(uL - cL, uR - cR), SR = fmax(uL + cL, uR + cR);
   const double cface = fmax(fabs(SL), fabs(SR));
