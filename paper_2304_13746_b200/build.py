@@ -1,34 +1,65 @@
 """Builds libidfx.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2304_13746_b200.build [--force]
+    python -m paper_2304_13746_b200.build [--force] [-v]
+
+Translation units: csrc/idfx.cu (C ABI, state kernels, fused CT/update kernel), csrc/probe.cu, and csrc/sweeps_inst.cu once
+per (Riemann solver, reconstruction) pair, compiled in parallel as separate nvcc processes.  No -split-compile: with it
+the code nvcc 12.9 generates for the register-bound sweep kernels (where their loads are scheduled, hence 0 to 96 bytes
+of spills) was found to change from one build of the same source to the next and with the core count of the build
+machine; a z sweep at 512^3 then takes 5.8 or 6.9 ms.  One process per unit is deterministic.
 """
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = [os.path.join(_HERE, "csrc", "idfx.cu"), os.path.join(_HERE, "csrc", "probe.cu")]
-HEADERS = sorted(os.path.join(_HERE, "csrc", f) for f in os.listdir(os.path.join(_HERE, "csrc")) if f.endswith(".cuh")) + [
+_CSRC = os.path.join(_HERE, "csrc")
+_OBJ = os.path.join(_HERE, "build")
+SOURCES = [os.path.join(_CSRC, f) for f in ("idfx.cu", "probe.cu", "sweeps_inst.cu")]
+HEADERS = sorted(os.path.join(_CSRC, f) for f in os.listdir(_CSRC) if f.endswith(".cuh")) + [
     os.path.join(os.path.dirname(_HERE), "include", "idfx.h"), os.path.join(os.path.dirname(_HERE), "include", "idfx_probe.h")]
 LIB = os.path.join(_HERE, "libidfx.so")
 
-NVCC_FLAGS = [
-    "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
-    "-split-compile", "0",   # the kernels of one translation unit are optimised in parallel (same code, half the build time)
-]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
+              "-Xfatbin", "-compress-all"]
+SOLVERS = (0, 1, 2, 3, 4)   # HLL, HLLC, HLLD, Roe, Rusanov (csrc/physics.cuh)
+LIMITERS = (0, 1, 2, 3)     # flat, minmod, van Leer, LimO3
 
 
-def build(force=False, verbose=False):
-    deps = SOURCES + HEADERS
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
-        return LIB
+def _units(obj_dir):
+    """(object path, nvcc arguments) of every translation unit, the longest first"""
+    units = [(os.path.join(obj_dir, "idfx.o"), ["-c", SOURCES[0]])]
+    for s in sorted(SOLVERS, key=lambda s: s != 3):   # Roe takes longest
+        for l in reversed(LIMITERS):
+            units.append((os.path.join(obj_dir, "sweeps_%d_%d.o" % (s, l)),
+                          ["-DIDFX_INST_SOLVER=%d" % s, "-DIDFX_INST_LIM=%d" % l, "-c", SOURCES[2]]))
+    units.append((os.path.join(obj_dir, "probe.o"), ["-c", SOURCES[1]]))
+    return units
+
+
+def build(force=False, verbose=False, extra_flags=(), lib=LIB, obj_dir=_OBJ):
+    """extra_flags / lib / obj_dir: development builds of variants (-D switches) next to the product library"""
+    deps = SOURCES + HEADERS + [os.path.abspath(__file__)]
+    if not force and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in deps):
+        return lib
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + SOURCES + ["-o", tmp]
-    subprocess.check_call(cmd)
-    os.replace(tmp, LIB)
-    return LIB
+    os.makedirs(obj_dir, exist_ok=True)
+    units = _units(obj_dir)
+
+    def compile_one(unit):
+        obj, args = unit
+        cmd = [nvcc] + NVCC_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else []) + args + ["-o", obj]
+        subprocess.check_call(cmd)
+        return obj
+
+    workers = max(2, os.cpu_count() or 4)
+    with ThreadPoolExecutor(max_workers=workers) as pool:
+        objs = list(pool.map(compile_one, units))
+    tmp = lib + ".tmp.%d" % os.getpid()
+    subprocess.check_call([nvcc, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a"] + objs + ["-o", tmp])
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":

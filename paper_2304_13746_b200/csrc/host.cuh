@@ -1,0 +1,160 @@
+// host.cuh — host-side context of the idfx CUDA path, shared by the translation units of libidfx.so:
+// idfx.cu (C ABI, state kernels, fused CT/update kernel) and sweeps_inst.cu (the flux sweeps, compiled once per
+// Riemann solver and reconstruction so that the code generated for one combination does not depend on the others).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <vector>
+
+#include "../../include/idfx.h"
+#include "common.cuh"
+#include "physics.cuh"
+#include "flux_march.cuh"
+#include "hd_stage.cuh"
+#include "flux_march_tma.cuh"
+
+namespace idfx {
+
+// field slots in the workspace
+enum {
+  F_UA = 0,    // 5: conserved state at the start of the cycle (and its result)
+  F_UB = 5,    // 5: stage-1 state
+  F_BA = 10,   // 3 x 3: face-field buffers that rotate between B0 / B1 / result
+  F_BB = 13,
+  F_BC = 16,
+  F_V = 19,    // 11: primitives, cell-centred B and Ec = -(v x Bc) of the stage input
+  F_V2 = 30,   // 11: second buffer (MHD: the fused CT/update kernel reads the stage input while writing the result)
+  F_R = 41,    // 5: flux divergence
+  F_FB = 46,   // 6: face fluxes of B, [d][0..1]
+  F_FX = 52,   // 5: x-face fluxes of (rho, m, E); F_FX+0 doubles as the x mass flux
+  F_CFX = 57,  // 1: c_face of the x sweep
+  F_SG = 58,   // 1 slot holding three byte fields: sign of the face mass flux of the x, y, z sweeps (E^c only)
+  F_CS = 59,   // 1: sum_d c_d per cell (x and y parts)
+  F_COUNT = 60,
+  // optional groups, appended in this order when present (idfx_ctx::f_aa, f_bref, f_h2d, f_eg):
+  //   vector-potential form (idfx_set_option(IDFX_OPT_CT_FORM, IDFX_CT_POTENTIAL)): 3 x 3 edge-potential buffers rotating
+  //   like the face-field buffers, and the 3 face fields given to set_state (ghosts filled);
+  //   2D-HLL EMF: 3 x 4 face quantities of k_flux_face<FMODE 2> and the 3 edge EMFs
+  N_VP = 12,
+  N_H2D = 15
+};
+
+}  // namespace idfx
+
+using namespace idfx;  // internal header: the context below is written in the library's own names
+
+// kernel classes for idfx_profile_* (order = idfx_profile_kernel_name)
+enum { K_FLUX_X = 0, K_FLUX_Y, K_FLUX_Z, K_RHS, K_EMF, K_UPDATE, K_FILL, K_STATE, K_HD, K_COUNT };
+static const char* const kKernelNames[K_COUNT] = {"flux_x", "flux_y", "flux_z", "rhs_dtmax", "edge_emf",
+                                                  "ct_update_prim", "ghost_fill", "state_io", "hd_stage"};
+
+struct idfx_ctx {
+  idfx::Geom g;
+  int solver, limiter, emf;
+  bool mhd;
+  double* ws = nullptr;
+  size_t ws_bytes = 0;
+  cudaStream_t stream = nullptr;
+  bool bound = false;
+  idfx::DevScalars* sc = nullptr;
+  int nstages = 2;  // Tab. 1: 1 Euler, 2 RK2, 3 RK3
+  bool vp = false;  // Eq. 7-8 instead of Eq. 6
+  int fixed_batch = 0;  // IDFX_ADVANCE_BATCH: cycles per batch of idfx_advance_to (tests: forces cycles past t_end)
+  int f_aa() const { return F_COUNT; }
+  int f_bref() const { return F_COUNT + 9; }
+  int f_h2d() const { return F_COUNT + (vp ? N_VP : 0); }
+  int f_eg() const { return f_h2d() + 12; }
+  int nfields() const { return F_COUNT + (vp ? N_VP : 0) + (emf == EMF_UCT_HLL ? N_H2D : 0); }
+  double* abuf(int which, int d) const { return field(f_aa() + 3 * which + d); }
+  int bcur = 0;  // which of the three face-field buffers holds the current state
+  int vcur = 0;  // which primitive buffer holds the stage input
+  int graph_bnext[6] = {0, 0, 0, 0, 0, 0}, graph_vnext[6] = {0, 0, 0, 0, 0, 0};  // rotation state a replayed cycle leaves
+  // one captured CUDA graph per buffer rotation state (3 face-field rotations x 2 primitive buffers)
+  cudaGraphExec_t graph[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  long long graph_launches[6] = {0, 0, 0, 0, 0, 0};
+  double graph_cfl = 0.0;
+  bool use_graph = true;
+  bool use_tma = false;            // y/z sweeps stage their planes through shared memory with TMA (MHD)
+  CUtensorMap mapV[3], mapB[3];    // per sweep direction (1 = y, 2 = z): boxes over the V and face-B field groups
+  bool hd_fused = false;           // HD: one kernel per stage (hd_stage.cuh); IDFX_HD_FUSED=0 keeps the three sweeps
+  CUtensorMap mapHD;               // 36 x 11 x 1 x 5 boxes over the primitive fields
+  long long launches = 0;
+  // optional per-kernel timing with CUDA events on the bound stream (idfx_profile_*)
+  bool prof_on = false;
+  struct ProfRec { cudaEvent_t a, b; int id; };
+  std::vector<ProfRec> prof_pending;
+  std::vector<cudaEvent_t> prof_free;
+  double prof_ms[K_COUNT] = {0};
+  long long prof_n[K_COUNT] = {0};
+  double* field(int slot) const { return ws + (size_t)slot * (size_t)g.np; }
+  double* bbuf(int which, int d) const { return field(F_BA + 3 * which + d); }
+  signed char* sgn(int d) const { return (signed char*)field(F_SG) + (size_t)d * (size_t)g.np; }
+  double* vfield(int n) const { return field((vcur ? F_V2 : F_V) + n); }
+  double* vfield_out(int n) const { return field((vcur ? F_V : F_V2) + n); }
+};
+
+namespace idfx {
+inline cudaEvent_t prof_event(idfx_ctx* c) {
+  if (!c->prof_free.empty()) {
+    cudaEvent_t e = c->prof_free.back();
+    c->prof_free.pop_back();
+    return e;
+  }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+inline void prof_drain(idfx_ctx* c) {
+  for (auto& r : c->prof_pending) {
+    float ms = 0.f;
+    cudaEventSynchronize(r.b);
+    cudaEventElapsedTime(&ms, r.a, r.b);
+    c->prof_ms[r.id] += ms;
+    c->prof_n[r.id] += 1;
+    c->prof_free.push_back(r.a);
+    c->prof_free.push_back(r.b);
+  }
+  c->prof_pending.clear();
+}
+// brackets one kernel launch: counts it and, when profiling is on, times it with an event pair
+struct LaunchScope {
+  idfx_ctx* c;
+  int id;
+  cudaEvent_t a = nullptr;
+  LaunchScope(idfx_ctx* c_, int id_) : c(c_), id(id_) {
+    if (c->prof_on) {
+      a = prof_event(c);
+      cudaEventRecord(a, c->stream);
+    }
+  }
+  ~LaunchScope() {
+    c->launches++;
+    if (c->prof_on) {
+      cudaEvent_t b = prof_event(c);
+      cudaEventRecord(b, c->stream);
+      c->prof_pending.push_back({a, b, id});
+      if (c->prof_pending.size() >= 4096) prof_drain(c);
+    }
+  }
+};
+
+inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+
+// ---- the three flux sweeps of one stage --------------------------------------------------------
+struct ApplyInfo {
+  bool on;  // stages >= 2 with the TMA sweeps: the z sweep applies the divergence and the RK combine itself
+  double w, w0;
+  int uin, uout;  // first slots of the stage-input and result conserved fields
+};
+
+// The three flux sweeps of one stage (x, then y and z marching), defined and explicitly instantiated in sweeps_inst.cu.
+template <int SOLVER, int LIM, bool MHD>
+void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const ApplyInfo& ap);
+
+// Hydrodynamics: the whole stage in one kernel (hd_stage.cuh), same translation units.
+typedef void (*HdKernel)(Geom, HdStageArgs, const CUtensorMap);
+template <int SOLVER, int LIM>
+HdKernel hd_kernel_sl(bool first);
+
+}  // namespace idfx

@@ -16,7 +16,7 @@
 #include "../../include/idfx.h"
 #include "common.cuh"
 #include "physics.cuh"
-#include "flux_march.cuh"
+#include "flux_march.cuh"      // argument structs of the sweep kernels (the kernels are instantiated in sweeps_inst.cu)
 #include "hd_stage.cuh"
 #include "flux_march_tma.cuh"
 
@@ -276,6 +276,22 @@ __global__ void __launch_bounds__(128) k_rhs(Geom g, RhsArgs a) {
 //   E[0] = E_x(i, j-1/2, k-1/2), E[1] = E_y(i-1/2, j, k-1/2), E[2] = E_z(i-1/2, j-1/2, k).
 // For component c with (a,b,c) cyclic:  E_c^(a) = -F_a[B_b] = -FB[a][0],  E_c^(b) = +F_b[B_a] = +FB[b][1].
 // ---------------------------------------------------------------------------------------------
+// read-only load of data no thread of the running kernel writes (ld.global.nc): the compiler may then move it across the
+// kernel's stores, which lets the update phase of k_ct_update issue loads of several cells at once.  Used for the flux
+// divergence, the face fluxes and signs, the stage-input face field and E^c, the saved face field: none of these
+// buffers is ever the destination of the same launch (run_stage)
+#ifndef IDFX_CT_LDG
+#define IDFX_CT_LDG 1
+#endif
+template <typename T>
+__device__ __forceinline__ T ldro(const T* p) {
+#if IDFX_CT_LDG
+  return __ldg(p);
+#else
+  return *p;
+#endif
+}
+
 struct EmfArgs {
   const double* FB[3][2];  // FB[d][0] = F_d[B_t1], FB[d][1] = F_d[B_t2] on the left d-faces
   const signed char* SG[3];  // sign of the mass flux F_d[rho] on the left d-faces
@@ -295,22 +311,23 @@ __device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& a, cons
     const long long db = idx[ib] == 0 ? (long long)(n[ib] - 1) * st[ib] : -st[ib];
     const double* __restrict__ Fa = a.FB[ia][0];
     const double* __restrict__ Fb = a.FB[ib][1];
-    const double EaP = -Fa[P], EaPb = -Fa[P + db];  // a-faces at (ia-1/2, ib) and (ia-1/2, ib-1)
-    const double EbP = Fb[P], EbPa = Fb[P + da];    // b-faces at (ia, ib-1/2) and (ia-1, ib-1/2)
+    const double EaP = -ldro(Fa + P), EaPb = -ldro(Fa + P + db);  // a-faces at (ia-1/2, ib) and (ia-1/2, ib-1)
+    const double EbP = ldro(Fb + P), EbPa = ldro(Fb + P + da);    // b-faces at (ia, ib-1/2) and (ia-1, ib-1/2)
     if (MODE == EMF_UCT_HLL) return a.Eg[c][P];
     double e = 0.25 * (EaP + EaPb + EbP + EbPa);
     if (MODE == EMF_UCT0) {
       // E^0: averaged instead of upwinded gradients = (1/2) sum of faces - (1/4) sum of cell-centred references
       const double* __restrict__ Ecc = a.Ec[c];
       e = 0.5 * (EaP + EaPb + EbP + EbPa) -
-          0.25 * (Ecc[P] + Ecc[P - st[ia]] + Ecc[P - st[ib]] + Ecc[P - st[ia] - st[ib]]);
+          0.25 * (ldro(Ecc + P) + ldro(Ecc + P - st[ia]) + ldro(Ecc + P - st[ib]) + ldro(Ecc + P - st[ia] - st[ib]));
     }
     if (MODE == EMF_UCT) {
       // cell-centred reference EMF of the stage input (G10), stored with ghosts next to the primitives
       const double* __restrict__ Ecc = a.Ec[c];
-      const double Ec = Ecc[P], Eca = Ecc[P - st[ia]], Ecb = Ecc[P - st[ib]], Ecab = Ecc[P - st[ia] - st[ib]];
-      const int fa = a.SG[ia][P], fab = a.SG[ia][P + db];  // sign of the mass flux through the two a-faces
-      const int fb = a.SG[ib][P], fba = a.SG[ib][P + da];  // and the two b-faces
+      const double Ec = ldro(Ecc + P), Eca = ldro(Ecc + P - st[ia]), Ecb = ldro(Ecc + P - st[ib]);
+      const double Ecab = ldro(Ecc + P - st[ia] - st[ib]);
+      const int fa = ldro(a.SG[ia] + P), fab = ldro(a.SG[ia] + P + db);  // sign of the mass flux through the two a-faces
+      const int fb = ldro(a.SG[ib] + P), fba = ldro(a.SG[ib] + P + da);  // and the two b-faces
       // d/db on the a-face, quarter points ib-1/4 (cells P-a | P) and ib-3/4 (cells P-a-b | P-b)
       const double gbp_m = 2.0 * (Eca - EbPa), gbp_p = 2.0 * (Ec - EbP);
       const double gbm_m = 2.0 * (EbPa - Ecab), gbm_p = 2.0 * (EbP - Ecb);
@@ -477,7 +494,9 @@ constexpr int CT_LX = CT_TX + 1, CT_LY = CT_TY + 1, CT_LZ = CT_TZ + 1;
 // UDONE: the conserved state was already combined by the z sweep (stages >= 2); only read it back for the primitives.
 // VP: vector-potential form (Eq. 7-8): the lattice holds the new potential A = w (A_in - dt E) + w0 A_0 instead of E
 // and the face field is B_ref + curl A, so its divergence is one rounding of the face values at any time.
-template <int MODE, bool STAGE2, bool UDONE, bool VP>
+// NCU: the conserved fields this launch reads are not written by it (the host checks the buffers, launch_ct_v), so
+// they too can be loaded read-only.
+template <int MODE, bool STAGE2, bool UDONE, bool VP, bool NCU>
 __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, EmfArgs ea, UpdateArgs a) {
   __shared__ double sE[3][CT_LZ][CT_LY][CT_LX];
   const int i0 = blockIdx.x * CT_TX, j0 = blockIdx.y * CT_TY, k0 = blockIdx.z * CT_TZ;
@@ -531,11 +550,18 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
     double u[5];
 #pragma unroll
     for (int n = 0; n < 5; ++n) {
+      // the result may be written over the stage input or over U_0 (Euler, RK3): plain loads then
       if (UDONE) {
-        u[n] = a.Uout[n][c];
+        u[n] = NCU ? ldro(a.Uout[n] + c) : a.Uout[n][c];
       } else {
-        const double us = a.Uin[n][c] - dtdx * a.R[n][c];
-        u[n] = STAGE2 ? (idle ? a.U0[n][c] : a.w0 * a.U0[n][c] + a.w * us) : us;
+        const double uin = NCU ? ldro(a.Uin[n] + c) : a.Uin[n][c];
+        const double us = uin - dtdx * ldro(a.R[n] + c);
+        if (STAGE2) {
+          const double u0 = NCU ? ldro(a.U0[n] + c) : a.U0[n][c];
+          u[n] = idle ? u0 : a.w0 * u0 + a.w * us;
+        } else {
+          u[n] = us;
+        }
         a.Uout[n][c] = u[n];
       }
     }
@@ -553,14 +579,15 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
     for (int d = 0; d < 3; ++d) {
       double bl, br;
       if (VP) {
-        bl = a.Bref[d][c] + curlL[d] / g.dx;  // Eq. 8
-        br = a.Bref[d][c + st[d]] + curlR[d] / g.dx;
+        bl = ldro(a.Bref[d] + c) + curlL[d] / g.dx;  // Eq. 8
+        br = ldro(a.Bref[d] + c + st[d]) + curlR[d] / g.dx;
       } else {
-        bl = a.Bin[d][c] - dtdx * curlL[d];  // Eq. 6
-        br = a.Bin[d][c + st[d]] - dtdx * curlR[d];
+        bl = ldro(a.Bin[d] + c) - dtdx * curlL[d];  // Eq. 6
+        br = ldro(a.Bin[d] + c + st[d]) - dtdx * curlR[d];
         if (STAGE2) {
-          bl = idle ? a.B0[d][c] : a.w0 * a.B0[d][c] + a.w * bl;
-          br = idle ? a.B0[d][c + st[d]] : a.w0 * a.B0[d][c + st[d]] + a.w * br;
+          const double b0l = ldro(a.B0[d] + c), b0r = ldro(a.B0[d] + c + st[d]);
+          bl = idle ? b0l : a.w0 * b0l + a.w * bl;
+          br = idle ? b0r : a.w0 * b0r + a.w * br;
         }
       }
       v[5 + d] = 0.5 * (bl + br);
@@ -613,129 +640,11 @@ thread_local char g_err[512] = "";
 
 void set_err(const char* fmt, const char* a = "", const char* b = "") { snprintf(g_err, sizeof(g_err), fmt, a, b); }
 
-// field slots in the workspace
-enum {
-  F_UA = 0,    // 5: conserved state at the start of the cycle (and its result)
-  F_UB = 5,    // 5: stage-1 state
-  F_BA = 10,   // 3 x 3: face-field buffers that rotate between B0 / B1 / result
-  F_BB = 13,
-  F_BC = 16,
-  F_V = 19,    // 11: primitives, cell-centred B and Ec = -(v x Bc) of the stage input
-  F_V2 = 30,   // 11: second buffer (MHD: the fused CT/update kernel reads the stage input while writing the result)
-  F_R = 41,    // 5: flux divergence
-  F_FB = 46,   // 6: face fluxes of B, [d][0..1]
-  F_FX = 52,   // 5: x-face fluxes of (rho, m, E); F_FX+0 doubles as the x mass flux
-  F_CFX = 57,  // 1: c_face of the x sweep
-  F_SG = 58,   // 1 slot holding three byte fields: sign of the face mass flux of the x, y, z sweeps (E^c only)
-  F_CS = 59,   // 1: sum_d c_d per cell (x and y parts)
-  F_COUNT = 60,
-  // optional groups, appended in this order when present (idfx_ctx::f_aa, f_bref, f_h2d, f_eg):
-  //   vector-potential form (idfx_set_option(IDFX_OPT_CT_FORM, IDFX_CT_POTENTIAL)): 3 x 3 edge-potential buffers rotating
-  //   like the face-field buffers, and the 3 face fields given to set_state (ghosts filled);
-  //   2D-HLL EMF: 3 x 4 face quantities of k_flux_face<FMODE 2> and the 3 edge EMFs
-  N_VP = 12,
-  N_H2D = 15
-};
-
 }  // namespace idfx
 
+#include "host.cuh"
+
 using namespace idfx;
-
-// kernel classes for idfx_profile_* (order = idfx_profile_kernel_name)
-enum { K_FLUX_X = 0, K_FLUX_Y, K_FLUX_Z, K_RHS, K_EMF, K_UPDATE, K_FILL, K_STATE, K_HD, K_COUNT };
-static const char* const kKernelNames[K_COUNT] = {"flux_x", "flux_y", "flux_z", "rhs_dtmax", "edge_emf",
-                                                  "ct_update_prim", "ghost_fill", "state_io", "hd_stage"};
-
-struct idfx_ctx {
-  Geom g;
-  int solver, limiter, emf;
-  bool mhd;
-  double* ws = nullptr;
-  size_t ws_bytes = 0;
-  cudaStream_t stream = nullptr;
-  bool bound = false;
-  DevScalars* sc = nullptr;
-  int nstages = 2;  // Tab. 1: 1 Euler, 2 RK2, 3 RK3
-  bool vp = false;  // Eq. 7-8 instead of Eq. 6
-  int fixed_batch = 0;  // IDFX_ADVANCE_BATCH: cycles per batch of idfx_advance_to (tests: forces cycles past t_end)
-  int f_aa() const { return F_COUNT; }
-  int f_bref() const { return F_COUNT + 9; }
-  int f_h2d() const { return F_COUNT + (vp ? N_VP : 0); }
-  int f_eg() const { return f_h2d() + 12; }
-  int nfields() const { return F_COUNT + (vp ? N_VP : 0) + (emf == EMF_UCT_HLL ? N_H2D : 0); }
-  double* abuf(int which, int d) const { return field(f_aa() + 3 * which + d); }
-  int bcur = 0;  // which of the three face-field buffers holds the current state
-  int vcur = 0;  // which primitive buffer holds the stage input
-  int graph_bnext[6] = {0, 0, 0, 0, 0, 0}, graph_vnext[6] = {0, 0, 0, 0, 0, 0};  // rotation state a replayed cycle leaves
-  // one captured CUDA graph per buffer rotation state (3 face-field rotations x 2 primitive buffers)
-  cudaGraphExec_t graph[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-  long long graph_launches[6] = {0, 0, 0, 0, 0, 0};
-  double graph_cfl = 0.0;
-  bool use_graph = true;
-  bool use_tma = false;            // y/z sweeps stage their planes through shared memory with TMA (MHD)
-  CUtensorMap mapV[3], mapB[3];    // per sweep direction (1 = y, 2 = z): boxes over the V and face-B field groups
-  bool hd_fused = false;           // HD: one kernel per stage (hd_stage.cuh); IDFX_HD_FUSED=0 keeps the three sweeps
-  CUtensorMap mapHD;               // 36 x 11 x 1 x 5 boxes over the primitive fields
-  long long launches = 0;
-  // optional per-kernel timing with CUDA events on the bound stream (idfx_profile_*)
-  bool prof_on = false;
-  struct ProfRec { cudaEvent_t a, b; int id; };
-  std::vector<ProfRec> prof_pending;
-  std::vector<cudaEvent_t> prof_free;
-  double prof_ms[K_COUNT] = {0};
-  long long prof_n[K_COUNT] = {0};
-  double* field(int slot) const { return ws + (size_t)slot * (size_t)g.np; }
-  double* bbuf(int which, int d) const { return field(F_BA + 3 * which + d); }
-  signed char* sgn(int d) const { return (signed char*)field(F_SG) + (size_t)d * (size_t)g.np; }
-  double* vfield(int n) const { return field((vcur ? F_V2 : F_V) + n); }
-  double* vfield_out(int n) const { return field((vcur ? F_V : F_V2) + n); }
-};
-
-namespace {
-cudaEvent_t prof_event(idfx_ctx* c) {
-  if (!c->prof_free.empty()) {
-    cudaEvent_t e = c->prof_free.back();
-    c->prof_free.pop_back();
-    return e;
-  }
-  cudaEvent_t e = nullptr;
-  cudaEventCreate(&e);
-  return e;
-}
-void prof_drain(idfx_ctx* c) {
-  for (auto& r : c->prof_pending) {
-    float ms = 0.f;
-    cudaEventSynchronize(r.b);
-    cudaEventElapsedTime(&ms, r.a, r.b);
-    c->prof_ms[r.id] += ms;
-    c->prof_n[r.id] += 1;
-    c->prof_free.push_back(r.a);
-    c->prof_free.push_back(r.b);
-  }
-  c->prof_pending.clear();
-}
-// brackets one kernel launch: counts it and, when profiling is on, times it with an event pair
-struct LaunchScope {
-  idfx_ctx* c;
-  int id;
-  cudaEvent_t a = nullptr;
-  LaunchScope(idfx_ctx* c_, int id_) : c(c_), id(id_) {
-    if (c->prof_on) {
-      a = prof_event(c);
-      cudaEventRecord(a, c->stream);
-    }
-  }
-  ~LaunchScope() {
-    c->launches++;
-    if (c->prof_on) {
-      cudaEvent_t b = prof_event(c);
-      cudaEventRecord(b, c->stream);
-      c->prof_pending.push_back({a, b, id});
-      if (c->prof_pending.size() >= 4096) prof_drain(c);
-    }
-  }
-};
-}  // namespace
 
 #define CK(call)                                                          \
   do {                                                                    \
@@ -748,7 +657,6 @@ struct LaunchScope {
 
 namespace {
 
-inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -868,146 +776,6 @@ void launch_dtmax(idfx_ctx* c) {
   k_rhs<false, true><<<blocks_for(c->g.nc, 128), 128, 0, c->stream>>>(c->g, a);
 }
 
-template <int SOLVER, int LIM, bool MHD>
-void launch_x_tma(idfx_ctx* c, dim3 grid, const FluxXTArgs& ta) {
-  if constexpr (MHD) k_flux_x_tma<SOLVER, LIM><<<grid, 128, 0, c->stream>>>(c->g, ta, c->mapV[0], c->mapB[0]);
-}
-
-template <int SOLVER, int LIM, bool MHD>
-void launch_march_tma(idfx_ctx* c, int d, dim3 grid, const FluxTArgs& ta, bool want_dt, bool uct, bool apply) {
-  if constexpr (MHD) {
-    const Geom& g = c->g;
-    if (d == 1) {
-      if (want_dt) k_flux_march_tma<SOLVER, LIM, 1, true, true, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
-      else if (uct) k_flux_march_tma<SOLVER, LIM, 1, false, true, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
-      else k_flux_march_tma<SOLVER, LIM, 1, false, false, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[1], c->mapB[1]);
-    } else if (apply) {
-      if (uct) k_flux_march_tma<SOLVER, LIM, 2, false, true, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
-      else k_flux_march_tma<SOLVER, LIM, 2, false, false, true><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
-    } else {
-      if (want_dt) k_flux_march_tma<SOLVER, LIM, 2, true, true, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
-      else if (uct) k_flux_march_tma<SOLVER, LIM, 2, false, true, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
-      else k_flux_march_tma<SOLVER, LIM, 2, false, false, false><<<grid, 128, 0, c->stream>>>(g, ta, c->mapV[2], c->mapB[2]);
-    }
-  }
-}
-
-// ---- the three flux sweeps of one stage --------------------------------------------------------
-struct ApplyInfo {
-  bool on;  // stages >= 2 with the TMA sweeps: the z sweep applies the divergence and the RK combine itself
-  double w, w0;
-  int uin, uout;  // first slots of the stage-input and result conserved fields
-};
-
-template <int SOLVER, int LIM, bool MHD>
-void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const ApplyInfo& ap) {
-  const Geom& g = c->g;
-  const bool uct = c->emf == EMF_UCT;
-  {  // x: faces 0..nx of every row
-    FluxXArgs a;
-    a.q[0] = c->vfield(0);
-    a.q[1] = c->vfield(1);
-    a.q[2] = c->vfield(2);
-    a.q[3] = c->vfield(3);
-    a.q[4] = c->vfield(4);
-    a.q[5] = c->vfield(6);
-    a.q[6] = c->vfield(7);
-    a.bn = MHD ? Bf[0] : nullptr;
-    for (int n = 0; n < 5; ++n) a.FH[n] = c->field(F_FX + n);
-    a.FB[0] = c->field(F_FB + 0);
-    a.FB[1] = c->field(F_FB + 1);
-    a.cf = want_dt ? c->field(F_CFX) : nullptr;
-    a.sg = uct ? c->sgn(0) : nullptr;
-    const int gx = (g.nx + 1 + 30) / 31;
-    const long long nrows = (long long)g.ny * g.nz;
-    long long rpw = gx * nrows / 9472;
-    rpw = rpw < 1 ? 1 : (rpw > 32 ? 32 : rpw);
-    a.rows_per_warp = (int)rpw;
-    dim3 grid(gx, (unsigned)((nrows + 4 * rpw - 1) / (4 * rpw)));
-    LaunchScope ls(c, K_FLUX_X);
-    // Measured: the TMA rows win up to 256^3 (0.64 vs 0.69 ms), but at 512^3 their 36-column boxes for 31 faces cost
-    // 23 GB instead of 18 GB of DRAM traffic per launch and lose (5.6 vs 4.9 ms under ncu): long rows use the shuffle kernel.
-    if (MHD && c->use_tma && g.nx <= 384) {
-      FluxXTArgs ta;
-      ta.fV0 = c->vcur ? 11 : 0;
-      ta.fB = (int)((Bf[0] - c->field(F_BA)) / g.np);
-      for (int n = 0; n < 5; ++n) ta.FH[n] = a.FH[n];
-      ta.FB[0] = a.FB[0];
-      ta.FB[1] = a.FB[1];
-      ta.cf = a.cf;
-      ta.sg = a.sg;
-      const long long per_chunk = (long long)gx * ((g.ny + 3) / 4);
-      long long nch = (148 * 16 + per_chunk - 1) / per_chunk;
-      const long long maxch = g.nz / 8 > 0 ? g.nz / 8 : 1;
-      nch = nch < 1 ? 1 : (nch > maxch ? maxch : nch);
-      ta.chunk = (int)((g.nz + nch - 1) / nch);
-      dim3 tgrid(gx, (g.ny + 3) / 4, (unsigned)((g.nz + ta.chunk - 1) / ta.chunk));
-      launch_x_tma<SOLVER, LIM, MHD>(c, tgrid, ta);
-    } else {
-      k_flux_x<SOLVER, LIM, MHD><<<grid, 128, 0, c->stream>>>(g, a);
-    }
-  }
-  for (int d = 1; d < 3; ++d) {  // y then z: marching pencils
-    const int ib = (d + 1) % 3, ie = (d + 2) % 3;
-    FluxMArgs a;
-    a.q[0] = c->vfield(0);
-    a.q[1] = c->vfield(1 + d);
-    a.q[2] = c->vfield(1 + ib);
-    a.q[3] = c->vfield(1 + ie);
-    a.q[4] = c->vfield(4);
-    a.q[5] = c->vfield(5 + ib);
-    a.q[6] = c->vfield(5 + ie);
-    a.bn = MHD ? Bf[d] : nullptr;
-    a.sd = d == 1 ? g.sy : g.sz;
-    a.st = d == 1 ? g.sz : g.sy;
-    a.ns = d == 1 ? g.ny : g.nz;
-    a.nt = d == 1 ? g.nz : g.ny;
-    for (int n = 0; n < 5; ++n) {
-      a.FX[n] = c->field(F_FX + n);
-      a.R[n] = c->field(F_R + n);
-    }
-    a.cfx = c->field(F_CFX);
-    a.csum = c->field(F_CS);
-    a.FB[0] = c->field(F_FB + 2 * d);
-    a.FB[1] = c->field(F_FB + 2 * d + 1);
-    a.SG = c->sgn(d);
-    a.sc = c->sc;
-    const long long per_chunk = (long long)((g.nx + 31) / 32) * ((a.nt + 3) / 4);
-    long long nch = (148 * 16 + per_chunk - 1) / per_chunk;
-    const long long maxch = a.ns / 8 > 0 ? a.ns / 8 : 1;
-    nch = nch < 1 ? 1 : (nch > maxch ? maxch : nch);
-    a.chunk = (int)((a.ns + nch - 1) / nch);
-    dim3 grid((g.nx + 31) / 32, (a.nt + 3) / 4, (unsigned)((a.ns + a.chunk - 1) / a.chunk));
-    LaunchScope ls(c, K_FLUX_X + d);
-    if (MHD && c->use_tma) {
-      FluxTArgs ta;
-      ta.fV0 = c->vcur ? 11 : 0;
-      ta.fB = (int)((Bf[d] - c->field(F_BA)) / g.np);
-      ta.ns = a.ns; ta.nt = a.nt; ta.chunk = a.chunk; ta.sd = a.sd; ta.st = a.st;
-      for (int n = 0; n < 5; ++n) { ta.FX[n] = a.FX[n]; ta.R[n] = a.R[n]; }
-      ta.cfx = a.cfx; ta.csum = a.csum; ta.FB[0] = a.FB[0]; ta.FB[1] = a.FB[1]; ta.SG = a.SG; ta.sc = a.sc;
-      for (int n = 0; n < 5; ++n) {
-        ta.Uin[n] = c->field(ap.uin + n);
-        ta.U0[n] = c->field(F_UA + n);
-        ta.Uout[n] = c->field(ap.uout + n);
-      }
-      ta.w = ap.w;
-      ta.w0 = ap.w0;
-      launch_march_tma<SOLVER, LIM, MHD>(c, d, grid, ta, want_dt, uct, ap.on && d == 2);
-      continue;
-    }
-    if (d == 1) {
-      if (want_dt) k_flux_march<SOLVER, LIM, MHD, 1, true, true><<<grid, 128, 0, c->stream>>>(g, a);
-      else if (uct) k_flux_march<SOLVER, LIM, MHD, 1, false, true><<<grid, 128, 0, c->stream>>>(g, a);
-      else k_flux_march<SOLVER, LIM, MHD, 1, false, false><<<grid, 128, 0, c->stream>>>(g, a);
-    } else {
-      if (want_dt) k_flux_march<SOLVER, LIM, MHD, 2, true, true><<<grid, 128, 0, c->stream>>>(g, a);
-      else if (uct) k_flux_march<SOLVER, LIM, MHD, 2, false, true><<<grid, 128, 0, c->stream>>>(g, a);
-      else k_flux_march<SOLVER, LIM, MHD, 2, false, false><<<grid, 128, 0, c->stream>>>(g, a);
-    }
-  }
-}
-
 template <int SOLVER, bool MHD>
 void launch_sweeps_s(idfx_ctx* c, const double* const Bf[3], bool want_dt, const ApplyInfo& ap) {
   switch (c->limiter) {
@@ -1100,11 +868,22 @@ void launch_fill(idfx_ctx* c, int which_b) {
   k_fill_ghost<<<blocks_for(nt, 128), 128, 0, c->stream>>>(g, fl);
 }
 
+template <int MODE, bool VP, bool NCU>
+void launch_ct_n(idfx_ctx* c, dim3 grid, const EmfArgs& ea, const UpdateArgs& a, bool stage2, bool udone) {
+  if (udone) k_ct_update<MODE, true, true, VP, NCU><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
+  else if (stage2) k_ct_update<MODE, true, false, VP, NCU><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
+  else k_ct_update<MODE, false, false, VP, NCU><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
+}
+
 template <int MODE, bool VP>
 void launch_ct_v(idfx_ctx* c, dim3 grid, const EmfArgs& ea, const UpdateArgs& a, bool stage2, bool udone) {
-  if (udone) k_ct_update<MODE, true, true, VP><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
-  else if (stage2) k_ct_update<MODE, true, false, VP><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
-  else k_ct_update<MODE, false, false, VP><<<grid, CT_THREADS, 0, c->stream>>>(c->g, ea, a);
+  // read-only loads of the conserved fields only when this launch writes none of the buffers it reads them from: the
+  // stage input and U_0 differ from the destination, and the pressure floor (which rewrites E in place) is off
+  bool ncu;
+  if (udone) ncu = !(c->g.pfloor > 0.0);
+  else ncu = a.Uin[0] != a.Uout[0] && (!stage2 || a.U0[0] != a.Uout[0]);
+  if (ncu) launch_ct_n<MODE, VP, true>(c, grid, ea, a, stage2, udone);
+  else launch_ct_n<MODE, VP, false>(c, grid, ea, a, stage2, udone);
 }
 
 template <int MODE>
@@ -1113,14 +892,7 @@ void launch_ct(idfx_ctx* c, dim3 grid, const EmfArgs& ea, const UpdateArgs& a, b
   else launch_ct_v<MODE, false>(c, grid, ea, a, stage2, udone);
 }
 
-// ---- hydrodynamics: the whole stage in one kernel (hd_stage.cuh) ----
-typedef void (*HdKernel)(Geom, HdStageArgs, const CUtensorMap);
-
-template <int SOLVER, int LIM>
-HdKernel hd_kernel_sl(bool first) {
-  return first ? (HdKernel)k_hd_stage<SOLVER, LIM, true> : (HdKernel)k_hd_stage<SOLVER, LIM, false>;
-}
-
+// ---- hydrodynamics: the whole stage in one kernel (hd_stage.cuh; instantiated in sweeps_inst.cu) ----
 template <int SOLVER>
 HdKernel hd_kernel_s(int limiter, bool first) {
   switch (limiter) {
