@@ -21,6 +21,9 @@ namespace idfx {
 #ifndef IDFX_TMA_PF
 #define IDFX_TMA_PF 1                    // L1 prefetch of the next plane's directly loaded fields
 #endif
+#ifndef IDFX_PF_DIST
+#define IDFX_PF_DIST 1                   // planes ahead
+#endif
 constexpr int TMA_NST = 5;               // ring stages
 constexpr int TMA_SLACK = 2;             // a stage is refilled two planes after it was consumed
 constexpr int TMA_PLANE_V = 8 * 4 * 32;  // doubles of the primitive box (8 fields x 4 rows x 32 columns)
@@ -157,14 +160,15 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
     consume(s - s0 + 3, qp, Bnn);  // plane s+1
     if (active) {
       const long long cu = c - sd;  // cell s-1, completed by this face
-      if (IDFX_TMA_PF && s + 1 < s1) {
+      if (IDFX_TMA_PF && s + IDFX_PF_DIST < s1) {
+        const long long cpf = c + (IDFX_PF_DIST - 1) * sd;
 #pragma unroll
-        for (int n = 0; n < 5; ++n) prefetch_l1(DIR == 1 ? a.FX[n] + c + 1 : a.R[n] + c);
+        for (int n = 0; n < 5; ++n) prefetch_l1(DIR == 1 ? a.FX[n] + cpf + 1 : a.R[n] + cpf);
         if (APPLY) {
 #pragma unroll
           for (int n = 0; n < 5; ++n) {
-            prefetch_l1(a.Uin[n] + c);
-            prefetch_l1(a.U0[n] + c);
+            prefetch_l1(a.Uin[n] + cpf);
+            prefetch_l1(a.U0[n] + cpf);
           }
         }
       }
