@@ -38,10 +38,10 @@
 
 namespace {
 
-constexpr int NG = 2;  // ghost layers: PLM needs 2 ("number of ghost cells ... adjusted")
+constexpr int NG = 3;  // ghost layers: PLM and LimO3 need 2, PPM 3 ("number of ghost cells ... adjusted")
 
 enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_RUSANOV = 4 };
-enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3 };
+enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3, LIM_PPM = 4 };
 enum { OPT_INTEGRATOR = 0, OPT_CT_FORM = 1, OPT_PRESSURE_FLOOR = 2, OPT_BOUNDARY = 3 };  // idfxref_set_option / idfxref_set_option_real
 enum { CT_FACE = 0, CT_POTENTIAL = 1 };
 enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3, EMF_UCT_HLL = 4 };
@@ -515,6 +515,62 @@ void reconstruct(int limiter, double qm, double q0, double qp, double dx, double
   upper = q0 + 0.5 * s;
 }
 
+// PPM ("piecewise parabolic reconstruction using an extremum-preserving limiter (4th order accurate on
+// regularly spaced grids, Colella & Woodward 1984; Colella & Sekora 2008)"; only named there: reading G22).  On a uniform
+// grid, with a_j the cell values:
+//  (1) interface value, CW84 Eq. 1.9:  a_{j+1/2} = 7/12 (a_j + a_{j+1}) - 1/12 (a_{j-1} + a_{j+2});
+//  (2) CS08 Sec. 2.3: where a_{j+1/2} does not lie between a_j and a_{j+1} it is replaced by
+//      (a_j + a_{j+1})/2 - D2lim/6, with D2 = 3 (a_j - 2 a_{j+1/2} + a_{j+1}), D2L = a_{j-1} - 2 a_j + a_{j+1},
+//      D2R = a_j - 2 a_{j+1} + a_{j+2}, and D2lim = s min(C |D2L|, C |D2R|, |D2|) when the three share the sign s, else 0;
+//  (3) CS08 Sec. 2.4, parabola of cell j with edge values a- = a_{j-1/2}, a+ = a_{j+1/2}:
+//      at a local extremum ((a+ - a_j)(a_j - a-) <= 0 or (a_{j+1} - a_j)(a_j - a_{j-1}) <= 0) both edge deviations are scaled
+//      by D2lim/D2f, D2f = 6 (a+ - 2 a_j + a-), D2lim = s min(|D2f|, C |D2L|, C |D2C|, C |D2R|) from the second differences
+//      of the cell values centred at j-1, j, j+1 when all four share the sign s, else 0 (a smooth extremum keeps its
+//      parabola, a non-smooth one is flattened); elsewhere the CW84 overshoot rule, one side at a time:
+//      |a+ - a_j| >= 2 |a- - a_j|  ->  a+ = a_j - 2 (a- - a_j), and the mirror image.  C = 1.25.
+double ppm_interface(double am1, double a0, double ap1, double ap2) {
+  const double C = 1.25;
+  double f = (7.0 * (a0 + ap1) - (am1 + ap2)) / 12.0;
+  if ((f - a0) * (ap1 - f) < 0.0) {
+    const double D2 = 3.0 * (a0 - 2.0 * f + ap1);
+    const double D2L = am1 - 2.0 * a0 + ap1;
+    const double D2R = a0 - 2.0 * ap1 + ap2;
+    double D2lim = 0.0;
+    if (D2 > 0.0 && D2L > 0.0 && D2R > 0.0) D2lim = std::min(std::min(C * D2L, C * D2R), D2);
+    if (D2 < 0.0 && D2L < 0.0 && D2R < 0.0) D2lim = -std::min(std::min(-C * D2L, -C * D2R), -D2);
+    f = 0.5 * (a0 + ap1) - D2lim / 6.0;
+  }
+  return f;
+}
+
+// a[0..4] = a_{j-2} .. a_{j+2}; values of cell j's limited parabola at its lower and upper faces
+void ppm_faces(const double a[5], double& lower, double& upper) {
+  const double C = 1.25;
+  const double a0 = a[2];
+  double am = ppm_interface(a[0], a[1], a[2], a[3]);
+  double ap = ppm_interface(a[1], a[2], a[3], a[4]);
+  const double dm = a0 - am, dp = ap - a0;
+  if (dm * dp <= 0.0 || (a[3] - a0) * (a0 - a[1]) <= 0.0) {
+    const double D2f = 6.0 * (ap - 2.0 * a0 + am);
+    const double D2L = a[0] - 2.0 * a[1] + a[2];
+    const double D2C = a[1] - 2.0 * a[2] + a[3];
+    const double D2R = a[2] - 2.0 * a[3] + a[4];
+    double D2lim = 0.0;
+    if (D2f > 0.0 && D2L > 0.0 && D2C > 0.0 && D2R > 0.0)
+      D2lim = std::min(std::min(C * D2L, C * D2R), std::min(C * D2C, D2f));
+    if (D2f < 0.0 && D2L < 0.0 && D2C < 0.0 && D2R < 0.0)
+      D2lim = -std::min(std::min(-C * D2L, -C * D2R), std::min(-C * D2C, -D2f));
+    const double ratio = (D2f == 0.0) ? 0.0 : D2lim / D2f;
+    ap = a0 + dp * ratio;
+    am = a0 - dm * ratio;
+  } else {
+    if (std::fabs(dp) >= 2.0 * std::fabs(dm)) ap = a0 + 2.0 * dm;
+    if (std::fabs(dm) >= 2.0 * std::fabs(dp)) am = a0 - 2.0 * dp;
+  }
+  lower = am;
+  upper = ap;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Grid-level scheme
 // ---------------------------------------------------------------------------------------------
@@ -664,6 +720,12 @@ void sweep(Ctx& c, int d, const Arr Bf[3], bool want_flux) {
           const double* v = q[n]->data();
           const double qm2 = v[i0 - 2 * sa], qm1 = v[i0 - sa], q0 = v[i0], qp1 = v[i0 + sa];
           double lo_unused, hi_unused;
+          if (c.limiter == LIM_PPM) {  // five-cell stencils: cells i-3 .. i+1 and i-2 .. i+2
+            const double sL[5] = {v[i0 - 3 * sa], qm2, qm1, q0, qp1}, sR[5] = {qm2, qm1, q0, qp1, v[i0 + 2 * sa]};
+            ppm_faces(sL, lo_unused, WL[n]);
+            ppm_faces(sR, WR[n], hi_unused);
+            continue;
+          }
           reconstruct(c.limiter, qm2, qm1, q0, c.dx, lo_unused, WL[n]);   // cell i-1 at its upper face
           reconstruct(c.limiter, qm1, q0, qp1, c.dx, WR[n], hi_unused);   // cell i at its lower face
         }
@@ -920,7 +982,8 @@ struct idfxref_ctx {
 IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, double gamma, int solver,
                                         int limiter, int emf_mode) {
   if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(gamma > 1.0)) return nullptr;
-  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 3 || emf_mode < 0 || emf_mode > 4) return nullptr;
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 4 || emf_mode < 0 || emf_mode > 4) return nullptr;
+  if (limiter == LIM_PPM && emf_mode == EMF_UCT_HLL) return nullptr;  // the 2D-HLL EMF reconstructs with 3-cell stencils only
   const bool mhd = emf_mode != EMF_NONE;
   if (mhd && solver == SOLVER_HLLC) return nullptr;
   if (!mhd && solver == SOLVER_HLLD) return nullptr;
@@ -1122,6 +1185,9 @@ IDFXREF_API void idfxref_reconstruct(int limiter, double qm, double q0, double q
                                      double* upper) {
   reconstruct(limiter, qm, q0, qp, dx, *lower, *upper);
 }
+
+// Point-wise PPM for the pins: a[0..4] = a_{j-2} .. a_{j+2}.
+IDFXREF_API void idfxref_ppm_faces(const double* a, double* lower, double* upper) { ppm_faces(a, *lower, *upper); }
 
 IDFXREF_API int idfxref_last_dt(const idfxref_ctx* h, double* dt_out) {
   if (!h || !dt_out) return ERR_INVALID_ARG;

@@ -84,6 +84,8 @@ def lib():
         L.idfxref_get_potential.argtypes = [vp, dp]
         L.idfxref_reconstruct.argtypes = [ci, cd, cd, cd, cd, dp, dp]
         L.idfxref_reconstruct.restype = None
+        L.idfxref_ppm_faces.argtypes = [dp, dp, dp]
+        L.idfxref_ppm_faces.restype = None
         _lib = L
     return _lib
 
@@ -246,6 +248,15 @@ def reconstruct(limiter, qm, q0, qp, dx):
     """(value at the lower face, value at the upper face) of cell i's reconstruction."""
     lo, hi = ctypes.c_double(), ctypes.c_double()
     lib().idfxref_reconstruct(limiter, qm, q0, qp, dx, ctypes.byref(lo), ctypes.byref(hi))
+    return lo.value, hi.value
+
+
+def ppm_faces(a5):
+    """(value at the lower face, value at the upper face) of cell j's PPM parabola from (a_{j-2}, ..., a_{j+2})."""
+    a = np.ascontiguousarray(a5, dtype=np.float64)
+    assert a.shape == (5,)
+    lo, hi = ctypes.c_double(), ctypes.c_double()
+    lib().idfxref_ppm_faces(_p(a), ctypes.byref(lo), ctypes.byref(hi))
     return lo.value, hi.value
 
 

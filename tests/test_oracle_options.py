@@ -118,7 +118,7 @@ def test_limo3_symmetries_and_bounds(R):
         lo_r, hi_r = R.reconstruct(LIMO3, qp, q0, qm, dx)      # mirror image
         assert (lo, hi) == (hi_r, lo_r)
         lo_n, hi_n = R.reconstruct(LIMO3, -qm, -q0, -qp, dx)   # odd in the data
-        assert (lo_n, hi_n) == (-lo, -hi)
+        assert (lo_n, hi_n) == (-lo, -hi)                   # exactly: every operation is odd
         lo_s, hi_s = R.reconstruct(LIMO3, qm + 1.0, q0 + 1.0, qp + 1.0, dx)
         assert lo_s == pytest.approx(lo + 1.0, abs=1e-12 * max(1.0, abs(q0))) and hi_s == pytest.approx(hi + 1.0, abs=1e-12 * max(1.0, abs(q0)))
         if (qm - q0) ** 2 + (qp - q0) ** 2 > 1.01 * dx * dx:   # limited: 0 <= phi <= 1.6, and monotone data stay bounded
@@ -445,3 +445,121 @@ def test_outflow_lets_a_uniform_flow_and_a_pulse_leave(R):
     assert np.abs(out[0] - 1.0).max() < 1e-6 and np.abs(out[1] - 2.0).max() < 1e-6
     with pytest.raises(ValueError):
         R.Oracle(8, 8, 8, 0.125, G53, HLLD, VANLEER, EMF_UCT, boundary=R.BOUNDARY_OUTFLOW)
+
+
+# =================================================================================================
+# PPM with the extremum-preserving limiter (Colella & Woodward 1984; Colella & Sekora 2008; reading G22)
+# =================================================================================================
+PPM = 4
+
+
+def _cell_averages(F, xc, dx):
+    """exact cell averages from the antiderivative F"""
+    return np.array([(F(x + 0.5 * dx) - F(x - 0.5 * dx)) / dx for x in xc])
+
+
+def test_ppm_is_exact_for_cell_averages_of_a_monotone_cubic(R):
+    """The interface formula 7/12, -1/12 reproduces the point values of a cubic from its cell averages, and where the
+    data are smooth and monotone no limiter acts (fourth order on regular grids)."""
+    f = lambda x: 2.0 + x + 0.3 * x ** 2 + 0.1 * x ** 3
+    F = lambda x: 2.0 * x + x ** 2 / 2 + 0.1 * x ** 3 + 0.025 * x ** 4
+    for dx in (0.2, 0.05):
+        for x0 in (0.3, 1.0, -0.2):
+            xc = x0 + dx * np.arange(-2, 3)
+            lo, hi = R.ppm_faces(_cell_averages(F, xc, dx))
+            # the averages are differences of the antiderivative divided by dx: their own rounding is ~ 1e-16 |F| / dx
+            assert abs(lo - f(x0 - 0.5 * dx)) <= 2e-13 and abs(hi - f(x0 + 0.5 * dx)) <= 2e-13
+    a = 3.0 - 0.7 * np.arange(5.0)            # linear and constant data come back exactly
+    lo, hi = R.ppm_faces(a)
+    assert abs(lo - (a[2] + 0.35)) <= 1e-15 and abs(hi - (a[2] - 0.35)) <= 1e-15
+    assert R.ppm_faces(np.full(5, 1.25)) == (1.25, 1.25)
+
+
+def test_ppm_keeps_a_smooth_extremum_and_flattens_a_rough_one(R):
+    """What 'extremum-preserving' means (Colella & Sekora 2008): the cell holding the maximum of a parabola keeps the exact
+    edge values (the 1984 limiter would set both to the cell value); an isolated spike is flattened."""
+    for dx in (0.1, 0.01):
+        F = lambda x: x - x ** 3 / 3                      # f = 1 - x^2, maximum inside cell j
+        for shift in (0.0, 0.2 * dx, -0.3 * dx):
+            xc = shift + dx * np.arange(-2, 3)
+            a = _cell_averages(F, xc, dx)
+            lo, hi = R.ppm_faces(a)
+            assert abs(lo - (1 - (shift - 0.5 * dx) ** 2)) <= 2e-13 and abs(hi - (1 - (shift + 0.5 * dx) ** 2)) <= 2e-13
+            assert max(lo, hi) < a[2] or shift != 0.0     # not flattened
+    assert R.ppm_faces(np.array([0.0, 0.0, 1.0, 0.0, 0.0])) == (1.0, 1.0)
+    assert R.ppm_faces(np.array([1.0, 1.0, 0.0, 1.0, 1.0])) == (0.0, 0.0)
+    # a smooth extremum whose neighbouring second differences are much smaller is limited to 1.25 times them
+    a = np.array([-0.01, 0.0, 1.0, 0.0, -0.01])           # D2C = -2, D2L = D2R = 1.01: signs differ -> flat
+    assert R.ppm_faces(a) == (1.0, 1.0)
+
+
+def test_ppm_is_monotone_at_discontinuities_and_symmetric(R):
+    rng = np.random.default_rng(5)
+    step = np.array([0.0, 0.0, 0.0, 1.0, 1.0, 1.0, 1.0])
+    for j in range(2, 5):                                   # every cell of a step keeps its faces inside [0, 1]
+        lo, hi = R.ppm_faces(step[j - 2:j + 3])
+        assert 0.0 <= lo <= 1.0 and 0.0 <= hi <= 1.0 and lo <= hi
+    for _ in range(3000):
+        a = rng.normal(size=5) * rng.choice([1e-3, 1.0, 30.0])
+        lo, hi = R.ppm_faces(a)
+        lo_r, hi_r = R.ppm_faces(a[::-1].copy())            # mirror image
+        tol = 8e-16 * np.abs(a).max()                      # sums are formed in a fixed order: symmetric up to rounding
+        assert abs(lo_r - hi) <= tol and abs(hi_r - lo) <= tol
+        lo_n, hi_n = R.ppm_faces(-a)                        # odd in the data
+        assert (lo_n, hi_n) == (-lo, -hi)                   # exactly: every operation is odd
+        if (a[3] - a[2]) * (a[2] - a[1]) > 0 and (a[2] - a[1]) * (a[1] - a[0]) > 0 and (a[4] - a[3]) * (a[3] - a[2]) > 0:
+            # monotone data: the parabola is monotone (no new extremum inside the cell) and stays between the neighbours
+            assert min(a[1], a[2]) - 1e-15 <= lo <= max(a[1], a[2]) + 1e-15
+            assert min(a[2], a[3]) - 1e-15 <= hi <= max(a[2], a[3]) + 1e-15
+            assert abs(hi - a[2]) <= 2 * abs(a[2] - lo) + 1e-15 and abs(a[2] - lo) <= 2 * abs(hi - a[2]) + 1e-15
+        else:   # next to an extremum an edge value may leave the range of its two cells (that is the point of the 2008
+            # limiter: the extremum of the underlying function lies between the cell values) but only by a bounded amount
+            span = a.max() - a.min()
+            assert abs(lo - a[2]) <= span and abs(hi - a[2]) <= span
+
+
+def test_ppm_face_values_converge_at_fourth_order(R):
+    errs = []
+    for n in (16, 32, 64):
+        dx = 1.0 / n
+        F = lambda x: -np.cos(2 * np.pi * x) / (2 * np.pi) + 2 * x     # f = sin(2 pi x) + 2
+        x0 = 0.1
+        xc = x0 + dx * np.arange(-2, 3)
+        lo, hi = R.ppm_faces(_cell_averages(F, xc, dx))
+        errs.append(abs(hi - (np.sin(2 * np.pi * (x0 + 0.5 * dx)) + 2)))
+    assert math.log2(errs[0] / errs[1]) > 3.7 and math.log2(errs[1] / errs[2]) > 3.7, errs
+
+
+@pytest.mark.parametrize("kind", ["fast", "alfven"])
+def test_rk3_ppm_linear_wave_converges_like_the_integrator(R, kind):
+    """PPM with RK3 (Fig. 8): third-order convergence at moderate resolution and an error well below the
+    second-order scheme's."""
+    errs = [run_wave_1d(R, n, PPM, 3, kind) for n in (32, 64)]
+    assert math.log2(errs[0] / errs[1]) >= 2.8, errs
+    assert errs[1] < 0.2 * run_wave_1d(R, 64, VANLEER, 2, kind)
+
+
+def test_ppm_scheme_conserves_and_keeps_divb(R):
+    from paper_2304_13746_b200 import inputs
+    prim, bface, cfg = inputs.make("config3", n=12)
+    o = R.Oracle(12, 12, 12, cfg["dx"], cfg["gamma"], HLLD, PPM, EMF_UCT, nstages=3)
+    o.set_state(prim.numpy(), bface.numpy())
+    c0, b0 = o.get_conserved()
+    o.advance(6, 0.3)
+    c1, b1 = o.get_conserved()
+    for v in range(5):
+        assert abs(c1[v].sum() - c0[v].sum()) <= 1e-13 * max(np.abs(c0[v]).sum(), 1.0)
+    for d in range(3):
+        assert abs(b1[d].sum() - b0[d].sum()) <= 1e-13 * np.abs(b0).sum()
+    div = sum(np.roll(b1[d], -1, axis=2 - d) - b1[d] for d in range(3)) / cfg["dx"]
+    assert np.abs(div).max() * cfg["dx"] <= 1e-13 * np.abs(b1).max()
+    # a uniform state is a fixed point, bit for bit
+    prim[:] = prim[:, :1, :1, :1]
+    bface[:] = 0.3
+    o.set_state(prim.numpy(), bface.numpy())
+    o.advance(2, 0.3)
+    p2, b2 = o.get_state()
+    assert (p2 == p2[:, :1, :1, :1]).all() and (b2 == 0.3).all()
+    # refused with the 2D-HLL EMF (3-cell edge reconstruction only)
+    with pytest.raises(Exception):
+        R.Oracle(12, 12, 12, cfg["dx"], cfg["gamma"], HLL, PPM, 4)
