@@ -288,7 +288,7 @@ def run_ours(args):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        sn, ssteps = 128, 2
+        sn, ssteps = 128, 5   # about 13 s of oracle work on one host core
         rate, el = oracle_rate(args.workload, sn, ssteps, 0)
         cpu = {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": el,
                "sample": "%s recipe at %d^3, %d steps (oracle/idfxref.cpp as it stands, 1 thread of %d host cores)" % (

@@ -49,7 +49,11 @@ typedef struct idfx_ctx idfx_ctx;
 enum { IDFX_SOLVER_HLL = 0, IDFX_SOLVER_HLLC = 1, IDFX_SOLVER_HLLD = 2, IDFX_SOLVER_ROE = 3, IDFX_SOLVER_RUSANOV = 4 };
 /* Reconstruction: flat (1st order), PLM with minmod or van Leer (harmonic mean, G2) slopes, and the compact
  * third-order LimO3 of Cada & Torrilhon 2009 (same 3-cell stencil and 2 ghost layers; constants in reading G18). */
-enum { IDFX_LIMITER_FLAT = 0, IDFX_LIMITER_MINMOD = 1, IDFX_LIMITER_VANLEER = 2, IDFX_LIMITER_LIMO3 = 3 };
+enum { IDFX_LIMITER_FLAT = 0, IDFX_LIMITER_MINMOD = 1, IDFX_LIMITER_VANLEER = 2, IDFX_LIMITER_LIMO3 = 3,
+       /* piecewise parabolic with the extremum-preserving limiter (Colella & Woodward 1984, Colella & Sekora
+        * 2008; reading G22): five-cell stencils, evaluated outside the tuned sweeps (one kernel per direction plus a
+        * divergence pass; +18 workspace fields); periodic boxes only, not with IDFX_EMF_UCT_HLL */
+       IDFX_LIMITER_PPM = 4 };
 /* EMF reconstruction: arithmetic average of the face fluxes, the E^0 and E^c (upwind-contact)
  * schemes of Gardiner & Stone 2005, and the 2D HLL Riemann solver at the edges after Mignone & Del Zanna 2021 (reading G21;
  * consistent in the plane-parallel limit with the HLL face solver).  IDFX_EMF_NONE selects hydrodynamics (no magnetic

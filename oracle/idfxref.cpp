@@ -25,7 +25,9 @@
 // degeneracy threshold (G6), the Roe fallback/degenerate-eigenvector conventions (G7), the face→cell
 // mapping of c_max in dt (G8), un-lagged dt (G9), the reference E^c state (G10), and the LimO3 constants
 // (1.6, r = 1, eps = 1e-12; G18: PAPER.md:79 only names the scheme of Cada & Torrilhon 2009), and the composition of the
-// 2D-HLL EMF beyond its plane-parallel limit (G21: PAPER.md:109 only names Mignone & Del Zanna 2021).
+// 2D-HLL EMF beyond its plane-parallel limit (G21: PAPER.md:109 only names Mignone & Del Zanna 2021), and the form of the PPM
+// limiter (G22: PAPER.md:79 only names Colella & Woodward 1984 and Colella & Sekora 2008; pinned here by what the
+// construction must do: exact for cubics, smooth extrema kept, steps monotone, fourth-order face values).
 //
 // Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC idfxref.cpp -o libidfxref.so
 #include <algorithm>

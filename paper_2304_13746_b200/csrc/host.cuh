@@ -36,8 +36,10 @@ enum {
   //   vector-potential form (idfx_set_option(IDFX_OPT_CT_FORM, IDFX_CT_POTENTIAL)): 3 x 3 edge-potential buffers rotating
   //   like the face-field buffers, and the 3 face fields given to set_state (ghosts filled);
   //   2D-HLL EMF: 3 x 4 face quantities of k_flux_face<FMODE 2> and the 3 edge EMFs
+  //   PPM: 3 x 5 face fluxes of (rho, m, E) and the 3 c_face fields of k_flux_face_ppm
   N_VP = 12,
-  N_H2D = 15
+  N_H2D = 15,
+  N_GEN = 18
 };
 
 }  // namespace idfx
@@ -65,7 +67,8 @@ struct idfx_ctx {
   int f_bref() const { return F_COUNT + 9; }
   int f_h2d() const { return F_COUNT + (vp ? N_VP : 0); }
   int f_eg() const { return f_h2d() + 12; }
-  int nfields() const { return F_COUNT + (vp ? N_VP : 0) + (emf == EMF_UCT_HLL ? N_H2D : 0); }
+  int f_gen() const { return f_h2d() + (emf == EMF_UCT_HLL ? N_H2D : 0); }
+  int nfields() const { return f_gen() + (limiter == LIM_PPM ? N_GEN : 0); }
   double* abuf(int which, int d) const { return field(f_aa() + 3 * which + d); }
   int bcur = 0;  // which of the three face-field buffers holds the current state
   int vcur = 0;  // which primitive buffer holds the stage input

@@ -228,6 +228,66 @@ __global__ void __launch_bounds__(128) k_flux_face(Geom g, FluxArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// PPM (reading G22) outside the tuned sweeps: the same left-face solve with five-cell stencils.  The fields
+// carry two ghost layers and PPM reaches three cells back, so positions along the sweep are wrapped (periodic boxes only).
+// Along the six cells id-3 .. id+2 there are five interfaces; each is evaluated once and shared by the two parabolas.
+// FMODE 0: fluxes (hydro part to F[0..4], field part to F[5..6]), c_face and the sign of the mass flux; 1: c_face only.
+// ---------------------------------------------------------------------------------------------
+struct FluxPpmArgs {
+  const double* q[7];
+  const double* bn;
+  long long sd;
+  int dir;
+  double* F[7];
+  double* cf;
+  signed char* sg;  // null unless the upwind-contact EMF needs it
+};
+
+template <int SOLVER, bool MHD, int FMODE>
+__global__ void __launch_bounds__(128) k_flux_face_ppm(Geom g, FluxPpmArgs a) {
+  int ijk[3];
+  if (!cell_of_thread(g, ijk[0], ijk[1], ijk[2])) return;
+  const long long c = g.at(ijk[0], ijk[1], ijk[2]);
+  const int nd = a.dir == 0 ? g.nx : (a.dir == 1 ? g.ny : g.nz), id = ijk[a.dir];
+  long long off[6];
+#pragma unroll
+  for (int m = 0; m < 6; ++m) {
+    int w = id + m - 3;
+    w = w < 0 ? w + nd : (w >= nd ? w - nd : w);
+    off[m] = c + (long long)(w - id) * a.sd;
+  }
+  constexpr int NQ = MHD ? 7 : 5;
+  double WL[7], WR[7];
+#pragma unroll
+  for (int n = 0; n < NQ; ++n) {
+    const double* __restrict__ q = a.q[n];
+    double v[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) v[m] = q[off[m]];
+    // interfaces between v[1]|v[2], v[2]|v[3] (the face being solved), v[3]|v[4]
+    const double e12 = ppm_edge(v[0], v[1], v[2], v[3]);
+    const double e23 = ppm_edge(v[1], v[2], v[3], v[4]);
+    const double e34 = ppm_edge(v[2], v[3], v[4], v[5]);
+    double unused;
+    ppm_limit(v, e12, e23, unused, WL[n]);       // cell id-1 (v[2]) at its upper face
+    ppm_limit(v + 1, e23, e34, WR[n], unused);   // cell id (v[3]) at its lower face
+  }
+  if (!MHD) WL[5] = WL[6] = WR[5] = WR[6] = 0.0;
+  const double Bn = MHD ? a.bn[c] : 0.0;  // G3
+  if (FMODE == 1) {
+    double SL, SR;
+    outer_speeds<MHD>(WL, WR, Bn, g.gamma, SL, SR);
+    a.cf[c] = fmax(fabs(SL), fabs(SR));
+  } else {
+    double F[7];
+    a.cf[c] = riemann<SOLVER, MHD>(WL, WR, Bn, g.gamma, F);
+#pragma unroll
+    for (int n = 0; n < NQ; ++n) a.F[n][c] = F[n];
+    if (a.sg) a.sg[c] = flux_sign(F[0]);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // a5: flux divergence R = sum_d [F_d(i+1/2) - F_d(i-1/2)] (Eq. 5); a9: block max of sum_d c_d/dx
 // ---------------------------------------------------------------------------------------------
 struct RhsArgs {
@@ -751,6 +811,15 @@ void launch_speed(idfx_ctx* c, int d, const double* const Bf[3]) {
   for (int n = 0; n < 7; ++n) a.F[n] = nullptr;
   a.cf = c->field(F_R + d);  // scratch: R is dead between cycles
   LaunchScope ls(c, K_FLUX_X + d);
+  if (c->limiter == LIM_PPM) {
+    FluxPpmArgs pa;
+    for (int n = 0; n < 7; ++n) { pa.q[n] = a.q[n]; pa.F[n] = nullptr; }
+    pa.bn = a.bn; pa.sd = a.sd; pa.dir = d; pa.cf = a.cf; pa.sg = nullptr;
+    const unsigned nb = blocks_for(c->g.nc, 128);
+    if (c->mhd) k_flux_face_ppm<SOLVER_HLL, true, 1><<<nb, 128, 0, c->stream>>>(c->g, pa);
+    else k_flux_face_ppm<SOLVER_HLL, false, 1><<<nb, 128, 0, c->stream>>>(c->g, pa);
+    return;
+  }
   if (c->mhd) {
     if (c->limiter == LIM_FLAT) launch_speed_l<LIM_FLAT, true>(c, a);
     else if (c->limiter == LIM_MINMOD) launch_speed_l<LIM_MINMOD, true>(c, a);
@@ -774,6 +843,59 @@ void launch_dtmax(idfx_ctx* c) {
   a.sc = c->sc;
   LaunchScope ls(c, K_RHS);
   k_rhs<false, true><<<blocks_for(c->g.nc, 128), 128, 0, c->stream>>>(c->g, a);
+}
+
+// ---- PPM: face fluxes of the three directions into their own fields, then divergence and dt (k_rhs) ----
+template <int SOLVER, bool MHD>
+void launch_ppm_s(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
+  const Geom& g = c->g;
+  const long long st[3] = {1, g.sy, g.sz};
+  const unsigned nb = blocks_for(g.nc, 128);
+  RhsArgs r;
+  for (int d = 0; d < 3; ++d) {
+    const int ib = (d + 1) % 3, ie = (d + 2) % 3;
+    FluxPpmArgs a;
+    a.q[0] = c->vfield(0);
+    a.q[1] = c->vfield(1 + d);
+    a.q[2] = c->vfield(1 + ib);
+    a.q[3] = c->vfield(1 + ie);
+    a.q[4] = c->vfield(4);
+    a.q[5] = c->vfield(5 + ib);
+    a.q[6] = c->vfield(5 + ie);
+    a.bn = MHD ? Bf[d] : nullptr;
+    a.sd = st[d];
+    a.dir = d;
+    for (int n = 0; n < 5; ++n) {
+      a.F[n] = c->field(c->f_gen() + 5 * d + n);
+      r.F[d][n] = a.F[n];
+    }
+    a.F[5] = c->field(F_FB + 2 * d);
+    a.F[6] = c->field(F_FB + 2 * d + 1);
+    a.cf = c->field(c->f_gen() + 15 + d);
+    r.cf[d] = a.cf;
+    a.sg = c->emf == EMF_UCT ? c->sgn(d) : nullptr;
+    LaunchScope ls(c, K_FLUX_X + d);
+    k_flux_face_ppm<SOLVER, MHD, 0><<<nb, 128, 0, c->stream>>>(g, a);
+  }
+  for (int n = 0; n < 5; ++n) r.R[n] = c->field(F_R + n);
+  r.sc = c->sc;
+  LaunchScope ls(c, K_RHS);
+  if (want_dt) k_rhs<true, true><<<nb, 128, 0, c->stream>>>(g, r);
+  else k_rhs<true, false><<<nb, 128, 0, c->stream>>>(g, r);
+}
+
+void launch_ppm(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
+  if (c->mhd) {
+    if (c->solver == SOLVER_HLL) launch_ppm_s<SOLVER_HLL, true>(c, Bf, want_dt);
+    else if (c->solver == SOLVER_RUSANOV) launch_ppm_s<SOLVER_RUSANOV, true>(c, Bf, want_dt);
+    else if (c->solver == SOLVER_HLLD) launch_ppm_s<SOLVER_HLLD, true>(c, Bf, want_dt);
+    else launch_ppm_s<SOLVER_ROE, true>(c, Bf, want_dt);
+  } else {
+    if (c->solver == SOLVER_HLL) launch_ppm_s<SOLVER_HLL, false>(c, Bf, want_dt);
+    else if (c->solver == SOLVER_RUSANOV) launch_ppm_s<SOLVER_RUSANOV, false>(c, Bf, want_dt);
+    else if (c->solver == SOLVER_HLLC) launch_ppm_s<SOLVER_HLLC, false>(c, Bf, want_dt);
+    else launch_ppm_s<SOLVER_ROE, false>(c, Bf, want_dt);
+  }
 }
 
 template <int SOLVER, bool MHD>
@@ -946,8 +1068,11 @@ void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, d
   const int uin = s == 0 ? F_UA : F_UB, uout = last ? F_UA : F_UB;
   const double w = W[c->nstages - 1][s], w0 = W0[c->nstages - 1][s];
   const double* Bf[3] = {c->bbuf(bin, 0), c->bbuf(bin, 1), c->bbuf(bin, 2)};
-  const ApplyInfo ap = {combine && c->mhd && c->use_tma, w, w0, uin, uout};
-  if (c->hd_fused) {
+  const bool ppm = c->limiter == LIM_PPM;
+  const ApplyInfo ap = {combine && c->mhd && c->use_tma && !ppm, w, w0, uin, uout};
+  if (ppm) {
+    launch_ppm(c, Bf, want_dt);
+  } else if (c->hd_fused) {
     launch_hd_stage(c, !combine, w, w0, uin, uout);
     if (combine) {  // the kernel wrote U_s, its primitives and their ghost images into the other primitive buffer
       c->vcur ^= 1;
@@ -1109,8 +1234,12 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
     set_err("idfx_create: need dx > 0 and gamma > 1");
     return nullptr;
   }
-  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 3 || emf_mode < 0 || emf_mode > 4) {
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 4 || emf_mode < 0 || emf_mode > 4) {
     set_err("idfx_create: unknown solver, limiter or emf_mode");
+    return nullptr;
+  }
+  if (limiter == LIM_PPM && emf_mode == EMF_UCT_HLL) {
+    set_err("idfx_create: unsupported combination (the 2D-HLL EMF reconstructs with three-cell stencils, not PPM)");
     return nullptr;
   }
   const bool mhd = emf_mode != EMF_NONE;
@@ -1172,7 +1301,8 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
   const char* env = getenv("IDFX_TMA");
   c->use_tma = c->mhd && !(env && env[0] == '0');  // IDFX_TMA=0 selects the register-prefetch sweeps (A/B only)
   const char* henv = getenv("IDFX_HD_FUSED");
-  c->hd_fused = !c->mhd && !(henv && henv[0] == '0');
+  c->hd_fused = !c->mhd && !(henv && henv[0] == '0') && c->limiter != LIM_PPM;
+  if (c->limiter == LIM_PPM) c->use_tma = false;  // PPM runs through k_flux_face_ppm / k_rhs
   if (c->use_tma || c->hd_fused) {
     int rc = make_tensor_maps(c);
     if (rc) return rc;
@@ -1441,6 +1571,10 @@ int idfx_set_option(idfx_ctx* c, int option, int value) {
   if (option == 3 /* IDFX_OPT_BOUNDARY */ && (value == 0 || value == 1)) {
     if (value == 1 && c->mhd) {
       set_err("idfx_set_option: outflow boundaries are implemented for hydrodynamics only");
+      return IDFX_ERR_UNSUPPORTED;
+    }
+    if (value == 1 && c->limiter == LIM_PPM) {
+      set_err("idfx_set_option: PPM is implemented for periodic boxes only");
       return IDFX_ERR_UNSUPPORTED;
     }
     if (value != c->g.outflow) drop_graphs(c);

@@ -14,7 +14,7 @@
 namespace idfx {
 
 enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_RUSANOV = 4 };
-enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3 };
+enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3, LIM_PPM = 4 };
 enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3, EMF_UCT_HLL = 4 };
 
 #define IDFX_DEV __device__ __forceinline__
@@ -157,6 +157,41 @@ IDFX_DEV void face_values(double q, double dm, double dp, double dx2, double& lo
     const double s = limited_slope<LIM>(dm, dp);
     lower = q - 0.5 * s;
     upper = q + 0.5 * s;
+  }
+}
+
+// PPM with the extremum-preserving limiter (Colella & Woodward 1984, Colella & Sekora 2008; DESIGN.md reading
+// G22), uniform grid.  Interface value between cells 0 and 1 from cells -1 .. 2: fourth-order average, and where that is
+// not between its two cells the second-difference-limited replacement.
+IDFX_DEV double ppm_edge(double am1, double a0, double ap1, double ap2) {
+  const double mid = a0 + ap1;
+  double f = (7.0 / 12.0) * mid - (1.0 / 12.0) * (am1 + ap2);
+  if ((f - a0) * (ap1 - f) < 0.0) {
+    const double d2 = 3.0 * (mid - 2.0 * f), d2l = (am1 + ap1) - 2.0 * a0, d2r = (a0 + ap2) - 2.0 * ap1;
+    const bool same = d2 * d2l > 0.0 && d2 * d2r > 0.0;
+    const double mag = fmin(fabs(d2), 1.25 * fmin(fabs(d2l), fabs(d2r)));
+    f = 0.5 * mid - (same ? copysign(mag, d2) : 0.0) * (1.0 / 6.0);
+  }
+  return f;
+}
+
+// Limited parabola of the cell with value a0 and raw edge values em (lower), ep (upper); q[0..4] = cells -2 .. +2.
+// At an extremum both edge deviations shrink by D2lim/D2f; elsewhere an edge further than twice the other from a0 is
+// pulled in (one side at a time).
+IDFX_DEV void ppm_limit(const double q[5], double em, double ep, double& lower, double& upper) {
+  const double a0 = q[2];
+  const double dm = a0 - em, dp = ep - a0;
+  if (dm * dp <= 0.0 || (q[3] - a0) * (a0 - q[1]) <= 0.0) {
+    const double d2f = 6.0 * ((ep + em) - 2.0 * a0);
+    const double d2l = (q[0] + q[2]) - 2.0 * q[1], d2c = (q[1] + q[3]) - 2.0 * q[2], d2r = (q[2] + q[4]) - 2.0 * q[3];
+    const bool same = d2f * d2l > 0.0 && d2f * d2c > 0.0 && d2f * d2r > 0.0;
+    const double mag = fmin(fabs(d2f), 1.25 * fmin(fabs(d2c), fmin(fabs(d2l), fabs(d2r))));
+    const double ratio = same ? mag / fabs(d2f) : 0.0;   // d2f != 0 whenever same
+    lower = a0 - dm * ratio;
+    upper = a0 + dp * ratio;
+  } else {
+    upper = fabs(dp) >= 2.0 * fabs(dm) ? a0 + 2.0 * dm : ep;
+    lower = fabs(dm) >= 2.0 * fabs(dp) ? a0 - 2.0 * dp : em;
   }
 }
 

@@ -10,7 +10,7 @@ import os
 import torch
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
-LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3 = 0, 1, 2, 3
+LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3, LIMITER_PPM = 0, 1, 2, 3, 4
 OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR, OPT_BOUNDARY = 0, 1, 2, 3
 BOUNDARY_PERIODIC, BOUNDARY_OUTFLOW = 0, 1
 CT_FACE, CT_POTENTIAL = 0, 1

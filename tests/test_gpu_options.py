@@ -13,6 +13,7 @@ from test_gpu_parity import (EMF_ARITH, EMF_NONE, EMF_UCT, EMF_UCT0, HLL, HLLC, 
 pytestmark = pytest.mark.gpu
 
 LIMO3 = 3
+PPM = 4
 EMF_UCT_HLL = 4
 G53 = 5.0 / 3.0
 
@@ -32,6 +33,9 @@ OPTION_COMBOS = [
     (HLL, LIMO3, EMF_UCT0, 1, 0), (HLLD, VANLEER, EMF_UCT, 1, 0), (HLLC, LIMO3, EMF_NONE, 3, 0), (HLL, MINMOD, EMF_NONE, 1, 0),
     (ROE, LIMO3, EMF_NONE, 2, 0),
     (HLLD, VANLEER, EMF_UCT, 2, 1), (HLLD, LIMO3, EMF_UCT, 3, 1), (ROE, VANLEER, EMF_ARITH, 1, 1), (HLL, MINMOD, EMF_UCT0, 3, 1),
+    # PPM (five-cell stencils, evaluated by k_flux_face_ppm + k_rhs)
+    (HLLD, PPM, EMF_UCT, 3, 0), (HLLD, PPM, EMF_UCT, 2, 0), (ROE, PPM, EMF_ARITH, 3, 0), (HLL, PPM, EMF_UCT0, 1, 1),
+    (HLLC, PPM, EMF_NONE, 3, 0), (ROE, PPM, EMF_NONE, 2, 0),
     # 2D-HLL EMF
     (HLL, VANLEER, EMF_UCT_HLL, 2, 0), (HLLD, LIMO3, EMF_UCT_HLL, 3, 0), (HLL, MINMOD, EMF_UCT_HLL, 2, 1), (ROE, VANLEER, EMF_UCT_HLL, 1, 0),
 ]
@@ -66,6 +70,36 @@ def test_limo3_on_steep_data(idfx, R):
     d = np.diff(p[0], axis=2)
     eta = (d[:, :, 1:] ** 2 + d[:, :, :-1] ** 2) / cfg["dx"] ** 2
     assert (eta > 1).any() and (eta < 1).any()      # both branches were exercised
+
+
+def test_ppm_on_steep_data(idfx, R):
+    """Random-phase Mach-1 turbulence at 40^3: after a few cycles the flow has smooth and non-smooth extrema, clipped
+    interface values and overshooting parabolas, i.e. every branch of the PPM limiter (G22); the oracle follows the
+    formulas as printed, the kernel shares the five interfaces of a stencil between its two parabolas."""
+    prim, b, cfg = inputs.make("config3", n=40)
+    sim, ref = pair(idfx, R, (40, 40, 40), cfg["dx"], HLLD, PPM, EMF_UCT, prim.numpy(), b.numpy(), 3, 0)
+    for _ in range(3):
+        sim.advance(2, 0.3)
+        ref.advance(2, 0.3)
+        assert abs(sim.last_dt() - ref.last_dt()) <= TOL_DT * ref.last_dt()
+    assert_state_close(sim, ref, TOL, "config3 recipe, PPM + RK3")
+    assert sim.status() == 0 and ref.status() == 0
+    assert abs(sim.compute_dt(0.3) - ref.compute_dt(0.3)) <= TOL_DT * ref.compute_dt(0.3)   # standalone dt, PPM states
+    # smallest box (the stencil wraps around the whole box) and hydrodynamics
+    for shape, solver, emf in (((4, 4, 4), HLLD, EMF_UCT), ((5, 4, 7), HLLC, EMF_NONE)):
+        prim, b, dx = smooth_ic(*shape, 3, emf != EMF_NONE)
+        sim, ref = pair(idfx, R, shape, dx, solver, PPM, emf, prim, b, 3, 0)
+        sim.advance(3, 0.3)
+        ref.advance(3, 0.3)
+        assert_state_close(sim, ref, TOL, "PPM %s" % (shape,))
+
+
+def test_ppm_refused_where_not_implemented(idfx):
+    with pytest.raises(Exception):
+        idfx.Idfx(8, 8, 8, 0.125, G53, HLL, PPM, EMF_UCT_HLL)
+    with pytest.raises(idfx.IdfxError) as e:
+        idfx.Idfx(8, 8, 8, 0.125, G53, HLLC, PPM, EMF_NONE, boundary=idfx.BOUNDARY_OUTFLOW)
+    assert e.value.code == idfx.ERR_UNSUPPORTED
 
 
 @pytest.mark.parametrize("ct_form", [0, 1])
