@@ -21,8 +21,10 @@ HEADERS = sorted(os.path.join(_CSRC, f) for f in os.listdir(_CSRC) if f.endswith
     os.path.join(os.path.dirname(_HERE), "include", "idfx.h"), os.path.join(os.path.dirname(_HERE), "include", "idfx_probe.h")]
 LIB = os.path.join(_HERE, "libidfx.so")
 
+# --register-usage-level=3 (default 5): ptxas keeps the fused CT/update kernel at 64 registers without its 16-32 B of spills
+# (9.55 -> 9.1 ms at 512^3) and the sweeps at 150-168 registers with fewer spills (same speed)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
-              "-Xfatbin", "-compress-all"]
+              "-Xfatbin", "-compress-all", "-Xptxas", "--register-usage-level=3"]
 SOLVERS = (0, 1, 2, 3, 4)   # HLL, HLLC, HLLD, Roe, Rusanov (csrc/physics.cuh)
 LIMITERS = (0, 1, 2, 3)     # flat, minmod, van Leer, LimO3
 
