@@ -66,8 +66,20 @@ __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a
       for (int n = 0; n < NQ; ++n) qen[n] = a.q[n][e];
     }
   };
-  fetch(r);
+#ifndef IDFX_X_PF_L1
+#define IDFX_X_PF_L1 0   // 1: the next row is prefetched into L1 (no registers) instead of into registers
+#endif
+  if (!IDFX_X_PF_L1) fetch(r);
   for (; r < rend; ++r) {
+    if (IDFX_X_PF_L1) {
+      fetch(r);
+      if (r + 1 < rend) {
+        const long long cn = g.at(cl, (r + 1) % g.ny, (r + 1) / g.ny);
+#pragma unroll
+        for (int n = 0; n < NQ; ++n) prefetch_l1(a.q[n] + cn);
+        if (MHD) prefetch_l1(a.bn + cn);
+      }
+    }
     double q[7], qe[7], Bn = bnn;
 #pragma unroll
     for (int n = 0; n < NQ; ++n) {
@@ -75,7 +87,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a
       qe[n] = qen[n];
     }
     const long long c = g.at(cl, r % g.ny, r / g.ny);
-    if (r + 1 < rend) fetch(r + 1);
+    if (!IDFX_X_PF_L1 && r + 1 < rend) fetch(r + 1);
     double WL[7], WR[7];
 #pragma unroll
     for (int n = 0; n < NQ; ++n) {

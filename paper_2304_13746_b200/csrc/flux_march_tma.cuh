@@ -155,6 +155,13 @@ __global__ void __launch_bounds__(128, IDFX_MINB_T) k_flux_march_tma(Geom g, Flu
   long long c = g.at(min(i, g.nx - 1), 0, 0) + (long long)min(t, a.nt - 1) * a.st + (long long)s0 * a.sd;
   const long long sd = a.sd;
   double Fp[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, cfp = 0.0;
+  // z sweeps: two planes per trip, so that the carried state (left face state, forward differences, previous flux) needs
+  // no register-to-register rotation (5.66 -> 5.50 ms at 512^3; the y sweep is slower that way, 5.17 -> 5.25 ms)
+#ifndef IDFX_MARCH_UNROLL_Z
+#define IDFX_MARCH_UNROLL_Z 2
+#endif
+  constexpr int UNROLL = DIR == 2 ? IDFX_MARCH_UNROLL_Z : 1;
+#pragma unroll UNROLL
   for (int s = s0; s <= s1; ++s, c += sd) {
     double qp[7], Bnn;
     consume(s - s0 + 3, qp, Bnn);  // plane s+1
