@@ -45,9 +45,10 @@ __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a
   const int f0 = 31 * blockIdx.x;
   const int ci = f0 - 1 + lane;
   const int nrows = g.ny * g.nz;
-  int r = (blockIdx.y * 4 + warp) * a.rows_per_warp;
-  const int rend = min(r + a.rows_per_warp, nrows);
-  if (r >= rend) return;
+  // The trip count comes from a kernel argument, so it is uniform as far as the compiler can prove, and no lane leaves
+  // the loop early: the warp shuffles below then compile to plain SHFL (with a per-warp row range they were wrapped in
+  // WARPSYNC.COLLECTIVE / ENDCOLLECTIVE pairs, 84 instructions per row).  Rows past the end are clamped and not stored.
+  const int rbase = (blockIdx.y * 4 + warp) * a.rows_per_warp;
   const int cl = min(ci, g.nx + 1);               // clamp the load column into the padded row
   const int ce = lane == 0 ? ci - 1 : min(ci + 1, g.nx + 1);  // edge lanes fetch the neighbour outside the window
   const bool edge = lane == 0 || lane == 31;
@@ -55,6 +56,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a
 
   double qn[7], qen[7], bnn = 0.0;  // next row (prefetched)
   auto fetch = [&](int row) {
+    row = min(row, nrows - 1);
     const int j = row % g.ny, k = row / g.ny;
     const long long c = g.at(cl, j, k);
 #pragma unroll
@@ -69,12 +71,16 @@ __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a
 #ifndef IDFX_X_PF_L1
 #define IDFX_X_PF_L1 0   // 1: the next row is prefetched into L1 (no registers) instead of into registers
 #endif
-  if (!IDFX_X_PF_L1) fetch(r);
-  for (; r < rend; ++r) {
+  if (!IDFX_X_PF_L1) fetch(rbase);
+  for (int it = 0; it < a.rows_per_warp; ++it) {
+    const int r = rbase + it;
+    const bool rowok = r < nrows;
+    const int rr = min(r, nrows - 1);
     if (IDFX_X_PF_L1) {
       fetch(r);
-      if (r + 1 < rend) {
-        const long long cn = g.at(cl, (r + 1) % g.ny, (r + 1) / g.ny);
+      if (it + 1 < a.rows_per_warp) {
+        const int rn = min(r + 1, nrows - 1);
+        const long long cn = g.at(cl, rn % g.ny, rn / g.ny);
 #pragma unroll
         for (int n = 0; n < NQ; ++n) prefetch_l1(a.q[n] + cn);
         if (MHD) prefetch_l1(a.bn + cn);
@@ -86,8 +92,8 @@ __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a
       q[n] = qn[n];
       qe[n] = qen[n];
     }
-    const long long c = g.at(cl, r % g.ny, r / g.ny);
-    if (!IDFX_X_PF_L1 && r + 1 < rend) fetch(r + 1);
+    const long long c = g.at(cl, rr % g.ny, rr / g.ny);
+    if (!IDFX_X_PF_L1 && it + 1 < a.rows_per_warp) fetch(r + 1);
     double WL[7], WR[7];
 #pragma unroll
     for (int n = 0; n < NQ; ++n) {
@@ -100,7 +106,7 @@ __global__ void __launch_bounds__(128, IDFX_MINB_X) k_flux_x(Geom g, FluxXArgs a
       WL[n] = __shfl_up_sync(0xffffffffu, up, 1);
     }
     if (!MHD) WL[5] = WL[6] = WR[5] = WR[6] = 0.0;
-    if (solve) {
+    if (solve && rowok) {
       double F[7];
       const double cface = riemann<SOLVER, MHD>(WL, WR, MHD ? Bn : 0.0, g.gamma, F);
 #pragma unroll
