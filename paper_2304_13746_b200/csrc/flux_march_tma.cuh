@@ -321,6 +321,7 @@ __global__ void __launch_bounds__(128, 4) k_flux_x_tma(Geom g, FluxXTArgs a, con
   for (int p = 0; p < np; ++p, c += g.sz) {
     const int st = p % TX_NST;
     mbar_wait(&full[st], (p / TX_NST) & 1);
+    __syncwarp();  // the lanes leave the wait loop one by one: reconverge once here rather than around every shuffle below
     const double* r = ring[st];
     double WL[7], WR[7];
 #pragma unroll
