@@ -43,7 +43,7 @@ ALGO_BYTES_PER_CELL = {"flux_x": 8 * 16.125, "flux_y": 8 * 20.125, "flux_z": 8 *
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (mean of the stage-1 and stage-2 launch) from the committed
 # ncu --set full capture of this command at 512^3 (profiles/r01_ncu_full_512.md); only valid for that workload
-NCU_TRAFFIC_BYTES_512 = {"flux_x": 17.43e9, "flux_y": 25.60e9, "flux_z": 30.34e9, "ct_update_prim": 44.81e9}
+NCU_TRAFFIC_BYTES_512 = {"flux_x": 17.43e9, "flux_y": 25.80e9, "flux_z": 30.37e9, "ct_update_prim": 43.20e9}
 
 
 def parse_args():
