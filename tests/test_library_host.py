@@ -97,6 +97,23 @@ def test_options_are_validated_on_the_host(L):
     assert L.idfx_set_option(None, idfx.OPT_INTEGRATOR, 2) == idfx.ERR_INVALID_ARG
 
 
+def test_ppm_rules_on_the_host(L):
+    """PPM (limiter 4): refused with the 2D-HLL EMF and with outflow boundaries, 18 more workspace fields (include/idfx.h)."""
+    assert not L.idfx_create(8, 8, 8, 0.1, 1.4, idfx.SOLVER_HLL, idfx.LIMITER_PPM, idfx.EMF_UCT_HLL)
+    assert b"PPM" in L.idfx_last_error()
+    assert not L.idfx_create(8, 8, 8, 0.1, 1.4, idfx.SOLVER_HLL, 5, idfx.EMF_NONE)
+    ppm = L.idfx_create(8, 8, 8, 0.1, 1.4, idfx.SOLVER_HLLD, idfx.LIMITER_PPM, idfx.EMF_UCT_CONTACT)
+    plm = L.idfx_create(8, 8, 8, 0.1, 1.4, idfx.SOLVER_HLLD, idfx.LIMITER_VANLEER, idfx.EMF_UCT_CONTACT)
+    hd = L.idfx_create(8, 8, 8, 0.1, 1.4, idfx.SOLVER_HLLC, idfx.LIMITER_PPM, idfx.EMF_NONE)
+    assert ppm and plm and hd
+    extra = L.idfx_workspace_bytes(ppm) - L.idfx_workspace_bytes(plm)
+    assert extra % 18 == 0 and extra // 18 >= 12 ** 3 * 8
+    assert L.idfx_set_option(hd, idfx.OPT_BOUNDARY, idfx.BOUNDARY_OUTFLOW) == idfx.ERR_UNSUPPORTED
+    assert L.idfx_set_option(hd, idfx.OPT_INTEGRATOR, 3) == idfx.OK
+    for h in (ppm, plm, hd):
+        L.idfx_destroy(h)
+
+
 def test_binding_fails_loudly_without_gpu():
     if torch.cuda.is_available():
         pytest.skip("a GPU is present")
