@@ -496,7 +496,7 @@ struct UpdateArgs {
 
 // Hydrodynamics: apply the flux divergence, RK2 combine, cons->prim.  (MHD uses k_ct_update below.)
 template <bool STAGE2>
-__global__ void __launch_bounds__(128) k_update_hd(Geom g, UpdateArgs a) {
+__global__ void __launch_bounds__(128, 16) k_update_hd(Geom g, UpdateArgs a) {  // 32 registers: full occupancy for a pure stream
   int i, j, k;
   if (!cell_of_thread(g, i, j, k)) return;
   const long long c = g.at(i, j, k);
