@@ -65,6 +65,8 @@ __device__ __forceinline__ void publish_dt(DevScalars* sc, double dt, bool lands
   if (dt > 0.0) sc->ncycles += 1;
 }
 
+// pulls a line into L1 ahead of its use; costs no register
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // sign of a face mass flux as one byte (+1, -1, 0): all the upwind-contact EMF needs of it (G10)

@@ -23,9 +23,6 @@
 
 namespace idfx {
 
-// pulls a line into L1 ahead of its use; costs no register
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-
 struct FluxXArgs {
   const double* q[7];  // rho, vx, vy, vz, p, Bc_y, Bc_z
   const double* bn;    // B_x on x-faces

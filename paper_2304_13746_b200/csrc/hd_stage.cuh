@@ -15,7 +15,7 @@
 #include <cstdint>
 
 #include "common.cuh"
-#include "flux_march_tma.cuh"
+#include "tma.cuh"
 #include "physics.cuh"
 
 namespace idfx {

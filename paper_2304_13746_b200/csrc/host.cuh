@@ -12,6 +12,7 @@
 #include "physics.cuh"
 #include "flux_march.cuh"
 #include "hd_stage.cuh"
+#include "mhd_stage.cuh"
 #include "flux_march_tma.cuh"
 
 namespace idfx {
@@ -47,9 +48,9 @@ enum {
 using namespace idfx;  // internal header: the context below is written in the library's own names
 
 // kernel classes for idfx_profile_* (order = idfx_profile_kernel_name)
-enum { K_FLUX_X = 0, K_FLUX_Y, K_FLUX_Z, K_RHS, K_EMF, K_UPDATE, K_FILL, K_STATE, K_HD, K_COUNT };
+enum { K_FLUX_X = 0, K_FLUX_Y, K_FLUX_Z, K_RHS, K_EMF, K_UPDATE, K_FILL, K_STATE, K_HD, K_MHD, K_COUNT };
 static const char* const kKernelNames[K_COUNT] = {"flux_x", "flux_y", "flux_z", "rhs_dtmax", "edge_emf",
-                                                  "ct_update_prim", "ghost_fill", "state_io", "hd_stage"};
+                                                  "ct_update_prim", "ghost_fill", "state_io", "hd_stage", "mhd_stage"};
 
 struct idfx_ctx {
   idfx::Geom g;
@@ -82,6 +83,8 @@ struct idfx_ctx {
   CUtensorMap mapV[3], mapB[3];    // per sweep direction (1 = y, 2 = z): boxes over the V and face-B field groups
   bool hd_fused = false;           // HD: one kernel per stage (hd_stage.cuh); IDFX_HD_FUSED=0 keeps the three sweeps
   CUtensorMap mapHD;               // 36 x 11 x 1 x 5 boxes over the primitive fields
+  bool mhd_fused = false;          // MHD: the three sweeps of a stage in one kernel (mhd_stage.cuh)
+  CUtensorMap mapMV, mapMB;        // 36 x (TY+3) x 1 x 8 boxes over the primitives, x 3 over the face-field buffers
   long long launches = 0;
   // optional per-kernel timing with CUDA events on the bound stream (idfx_profile_*)
   bool prof_on = false;
@@ -159,5 +162,10 @@ void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const
 typedef void (*HdKernel)(Geom, HdStageArgs, const CUtensorMap);
 template <int SOLVER, int LIM>
 HdKernel hd_kernel_sl(bool first);
+
+// MHD: the three sweeps of a stage in one kernel (mhd_stage.cuh), same translation units.
+typedef void (*MhdKernel)(Geom, MhdStageArgs, const CUtensorMap, const CUtensorMap);
+template <int SOLVER, int LIM>
+MhdKernel mhd_kernel_sl(bool first, int emf_mode);
 
 }  // namespace idfx

@@ -18,6 +18,7 @@
 #include "physics.cuh"
 #include "flux_march.cuh"      // argument structs of the sweep kernels (the kernels are instantiated in sweeps_inst.cu)
 #include "hd_stage.cuh"
+#include "mhd_stage.cuh"
 #include "flux_march_tma.cuh"
 
 namespace idfx {
@@ -359,56 +360,67 @@ struct EmfArgs {
   const double* Eg[3];     // EMF_UCT_HLL: edge EMFs already evaluated by k_emf_hll2d
 };
 
-// E_c on the lower (a-1/2, b-1/2) edge of active cell idx, (a,b,c) cyclic (O10)
+// E_c on the lower (a-1/2, b-1/2) edge of active cell idx, (a, b, c) cyclic (Gardiner & Stone 2005).
+// Written in "quadrant form".  Four faces meet at the edge: the a-faces of rows ib-1 and ib (they carry E^(a) = -F_a[B_b])
+// and the b-faces of columns ia-1 and ia (E^(b) = +F_b[B_a]); four cells touch it, (column, row) in {ia-1, ia} x {ib-1, ib}.
+//   arithmetic:  E = mean of the four face values
+//   E^c:         every face also looks sideways into one of its two cells -- the one its mass flux comes from -- and adds
+//                a quarter of (transverse face value on that cell's side of the edge - cell-centred reference value):
+//                  a-face of row r, donor column k:  E^(b)[k] - E^ref[k][r]
+//                  b-face of column k, donor row r:  E^(a)[r] - E^ref[k][r]
+//                which is Gardiner & Stone's (dx/8)(dE/dx at the two quarter points) with the one-sided differences
+//                2 (E_face - E_ref) and 2 (E_ref - E_face) written out and summed; a vanishing mass flux weighs both cells 1/2
+//   E^0:         the same with both cells weighted 1/2 on every face
+// The donor weight of the lower cell is (1 + s)/2 with s the stored sign of the mass flux (+1, -1, 0), so the upwind choice
+// is arithmetic on {0, 1/2, 1} rather than a branch.
 template <int MODE>
-__device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& a, const int idx[3], int c) {
-  const int n[3] = {g.nx, g.ny, g.nz};
-  const long long st[3] = {1, g.sy, g.sz};
+__device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& A, const int idx[3], int c) {
+  if (MODE == EMF_UCT_HLL) return A.Eg[c][g.at(idx[0], idx[1], idx[2])];
+  const int a = (c + 1) % 3, b = (c + 2) % 3;
+  const int ext[3] = {g.nx, g.ny, g.nz};
+  const long long step[3] = {1, g.sy, g.sz};
   const long long P = g.at(idx[0], idx[1], idx[2]);
-    const int ia = (c + 1) % 3, ib = (c + 2) % 3;
-    // periodic images of the neighbours one step down in a and in b (flux arrays have no ghosts)
-    const long long da = idx[ia] == 0 ? (long long)(n[ia] - 1) * st[ia] : -st[ia];
-    const long long db = idx[ib] == 0 ? (long long)(n[ib] - 1) * st[ib] : -st[ib];
-    const double* __restrict__ Fa = a.FB[ia][0];
-    const double* __restrict__ Fb = a.FB[ib][1];
-    const double EaP = -ldro(Fa + P), EaPb = -ldro(Fa + P + db);  // a-faces at (ia-1/2, ib) and (ia-1/2, ib-1)
-    const double EbP = ldro(Fb + P), EbPa = ldro(Fb + P + da);    // b-faces at (ia, ib-1/2) and (ia-1, ib-1/2)
-    if (MODE == EMF_UCT_HLL) return a.Eg[c][P];
-    double e = 0.25 * (EaP + EaPb + EbP + EbPa);
-    if (MODE == EMF_UCT0) {
-      // E^0: averaged instead of upwinded gradients = (1/2) sum of faces - (1/4) sum of cell-centred references
-      const double* __restrict__ Ecc = a.Ec[c];
-      e = 0.5 * (EaP + EaPb + EbP + EbPa) -
-          0.25 * (ldro(Ecc + P) + ldro(Ecc + P - st[ia]) + ldro(Ecc + P - st[ib]) + ldro(Ecc + P - st[ia] - st[ib]));
-    }
-    if (MODE == EMF_UCT) {
-      // cell-centred reference EMF of the stage input (G10), stored with ghosts next to the primitives
-      const double* __restrict__ Ecc = a.Ec[c];
-      const double Ec = ldro(Ecc + P), Eca = ldro(Ecc + P - st[ia]), Ecb = ldro(Ecc + P - st[ib]);
-      const double Ecab = ldro(Ecc + P - st[ia] - st[ib]);
-      const int fa = ldro(a.SG[ia] + P), fab = ldro(a.SG[ia] + P + db);  // sign of the mass flux through the two a-faces
-      const int fb = ldro(a.SG[ib] + P), fba = ldro(a.SG[ib] + P + da);  // and the two b-faces
-      // d/db on the a-face, quarter points ib-1/4 (cells P-a | P) and ib-3/4 (cells P-a-b | P-b)
-      const double gbp_m = 2.0 * (Eca - EbPa), gbp_p = 2.0 * (Ec - EbP);
-      const double gbm_m = 2.0 * (EbPa - Ecab), gbm_p = 2.0 * (EbP - Ecb);
-      const double Gb1 = fa > 0 ? gbp_m : (fa < 0 ? gbp_p : 0.5 * (gbp_m + gbp_p));
-      const double Gb3 = fab > 0 ? gbm_m : (fab < 0 ? gbm_p : 0.5 * (gbm_m + gbm_p));
-      // d/da on the b-face, quarter points ia-1/4 (cells P-b | P) and ia-3/4 (cells P-a-b | P-a)
-      const double gap_m = 2.0 * (Ecb - EaPb), gap_p = 2.0 * (Ec - EaP);
-      const double gam_m = 2.0 * (EaPb - Ecab), gam_p = 2.0 * (EaP - Eca);
-      const double Ga1 = fb > 0 ? gap_m : (fb < 0 ? gap_p : 0.5 * (gap_m + gap_p));
-      const double Ga3 = fba > 0 ? gam_m : (fba < 0 ? gam_p : 0.5 * (gam_m + gam_p));
-      e += 0.125 * (Gb3 - Gb1) + 0.125 * (Ga3 - Ga1);
-    }
-    return e;
+  // one step down in a / in b: flux and sign arrays carry no ghosts (their periodic image is taken), cell arrays do
+  const long long downA = idx[a] == 0 ? (long long)(ext[a] - 1) * step[a] : -step[a];
+  const long long downB = idx[b] == 0 ? (long long)(ext[b] - 1) * step[b] : -step[b];
+  const double* __restrict__ fluxA = A.FB[a][0];  // F_a[B_b]
+  const double* __restrict__ fluxB = A.FB[b][1];  // F_b[B_a]
+  const double onA[2] = {-ldro(fluxA + P + downB), -ldro(fluxA + P)};  // by row:    ib-1, ib
+  const double onB[2] = {ldro(fluxB + P + downA), ldro(fluxB + P)};    // by column: ia-1, ia
+  const double mean = 0.25 * ((onA[0] + onA[1]) + (onB[0] + onB[1]));
+  if (MODE == EMF_ARITH) return mean;
+  const double* __restrict__ ref = A.Ec[c];  // -(v x Bc)_c of the stage input, with ghosts (G10)
+  double cell[2][2];                         // [column][row]
+  cell[1][1] = ldro(ref + P);
+  cell[0][1] = ldro(ref + P - step[a]);
+  cell[1][0] = ldro(ref + P - step[b]);
+  cell[0][0] = ldro(ref + P - step[a] - step[b]);
+  double wA[2] = {0.5, 0.5}, wB[2] = {0.5, 0.5};  // weight of the LOWER cell: column ia-1 for the a-faces, row ib-1 for the b-faces
+  if (MODE == EMF_UCT) {
+    wA[0] = 0.5 + 0.5 * (double)ldro(A.SG[a] + P + downB);
+    wA[1] = 0.5 + 0.5 * (double)ldro(A.SG[a] + P);
+    wB[0] = 0.5 + 0.5 * (double)ldro(A.SG[b] + P + downA);
+    wB[1] = 0.5 + 0.5 * (double)ldro(A.SG[b] + P);
+  }
+  double side = 0.0;
+#pragma unroll
+  for (int r = 0; r < 2; ++r)  // a-face of row r
+    side += wA[r] * (onB[0] - cell[0][r]) + (1.0 - wA[r]) * (onB[1] - cell[1][r]);
+#pragma unroll
+  for (int k = 0; k < 2; ++k)  // b-face of column k
+    side += wB[k] * (onA[0] - cell[k][0]) + (1.0 - wB[k]) * (onA[1] - cell[k][1]);
+  return mean + 0.25 * side;
 }
 
 // ---------------------------------------------------------------------------------------------
-// 2D-HLL edge EMF (reading G21).  Thread (i,j,k) evaluates the three lower edges of its cell from the face
-// quantities of k_flux_face<FMODE 2> (no ghosts: indices wrap) and the staggered field (ghosts filled):
-//   E_c = -[al_a+ (v_a B_b)^W + al_a- (v_a B_b)^E - al_a+ al_a- (B_b^E - B_b^W)] / (al_a+ + al_a-)
-//         +[al_b+ (v_b B_a)^S + al_b- (v_b B_a)^N - al_b+ al_b- (B_a^N - B_a^S)] / (al_b+ + al_b-),   (a,b,c) cyclic,
-// W/E reconstructed along a on the b-faces either side of the edge, S/N along b on the a-faces.
+// 2D-HLL edge EMF (reading G21).  Thread (i, j, k) evaluates the three lower edges of its cell.  At an edge
+// along c the induction flux v_a B_b is transported across the edge along a, and v_b B_a along b; each is a one-dimensional
+// HLL flux of a staggered field between its two edge-side values:
+//   T(q; lo, hi) = [al+ q_lo (v_lo + al-) + al- q_hi (v_hi - al+)] / (al+ + al-)      (= the HLL average of v q, regrouped)
+//   E_c = -T(B_b along a) + T(B_a along b)
+// with lo / hi the staggered field and the face velocity reconstructed to the edge from either side, and al+- the larger
+// one-sided speed of the two faces normal to the transport direction that touch the edge.  Inputs: the face quantities of
+// k_flux_face<FMODE 2> (no ghosts: indices wrap) and the staggered field (ghosts filled).
 // ---------------------------------------------------------------------------------------------
 struct Hll2dArgs {
   const double* H[3][4];   // per direction d: alpha+, alpha-, v_t1 (component d+1), v_t2 (component d+2) on the left d-faces
@@ -416,58 +428,54 @@ struct Hll2dArgs {
   double* E[3];
 };
 
+// values at the point between samples m1 and p0 of a line of four samples, seen from below and from above (S2 along the line)
+template <int LIM>
+__device__ __forceinline__ void edge_sides(double m2, double m1, double p0, double p1, double dx2, double& below, double& above) {
+  double drop;
+  face_values<LIM>(m1, m1 - m2, p0 - m1, dx2, drop, below);
+  face_values<LIM>(p0, p0 - m1, p1 - p0, dx2, above, drop);
+}
+
+__device__ __forceinline__ double hll_transport(double alp, double alm, double v_lo, double q_lo, double v_hi, double q_hi) {
+  return (alp * q_lo * (v_lo + alm) + alm * q_hi * (v_hi - alp)) / (alp + alm);
+}
+
 template <int LIM>
 __global__ void __launch_bounds__(128) k_emf_hll2d(Geom g, Hll2dArgs h) {
-  int ijk[3];
-  if (!cell_of_thread(g, ijk[0], ijk[1], ijk[2])) return;
-  const int n[3] = {g.nx, g.ny, g.nz};
-  const long long st[3] = {1, g.sy, g.sz};
-  const long long P = g.at(ijk[0], ijk[1], ijk[2]);
+  int cellidx[3];
+  if (!cell_of_thread(g, cellidx[0], cellidx[1], cellidx[2])) return;
+  const int ext[3] = {g.nx, g.ny, g.nz};
+  const long long step[3] = {1, g.sy, g.sz};
+  const long long P = g.at(cellidx[0], cellidx[1], cellidx[2]);
   const double dx2 = g.dx * g.dx;
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    const int a = (c + 1) % 3, b = (c + 2) % 3;
-    // offsets of the periodic images at -2, -1, +1 along a and along b
-    long long oa[4], ob[4];
+    double T[2];  // transport along a = c+1 (of B_b), along b = c+2 (of B_a)
 #pragma unroll
-    for (int m = 0; m < 4; ++m) {
-      const int da = m - 2;  // -2, -1, 0, +1
-      int ia = ijk[a] + da, ib = ijk[b] + da;
-      ia = ia < 0 ? ia + n[a] : (ia >= n[a] ? ia - n[a] : ia);
-      ib = ib < 0 ? ib + n[b] : (ib >= n[b] ? ib - n[b] : ib);
-      oa[m] = P + (long long)(ia - ijk[a]) * st[a];
-      ob[m] = P + (long long)(ib - ijk[b]) * st[b];
+    for (int leg = 0; leg < 2; ++leg) {
+      const int along = (c + 1 + leg) % 3;   // direction of the transport across the edge
+      const int other = (c + 2 - leg) % 3;   // component of the staggered field carried = normal of the faces it lives on
+      // periodic images of the face samples at -2, -1, +1 along `along` (ghost-free arrays)
+      long long w[4];
+#pragma unroll
+      for (int m = 0; m < 4; ++m) {
+        int t = cellidx[along] + m - 2;
+        t = t < 0 ? t + ext[along] : (t >= ext[along] ? t - ext[along] : t);
+        w[m] = P + (long long)(t - cellidx[along]) * step[along];
+      }
+      // velocity component `along` on the `other`-faces: slot 2 of that sweep is component other+1, slot 3 is other+2
+      const double* __restrict__ vel = h.H[other][(along - other + 3) % 3 == 1 ? 2 : 3];
+      const double* __restrict__ fld = h.Bf[other];
+      double q_lo, q_hi, v_lo, v_hi;
+      edge_sides<LIM>(fld[P - 2 * step[along]], fld[P - step[along]], fld[P], fld[P + step[along]], dx2, q_lo, q_hi);
+      edge_sides<LIM>(vel[w[0]], vel[w[1]], vel[P], vel[w[3]], dx2, v_lo, v_hi);
+      // the two `along`-faces touching the edge are neighbours in `other`
+      const int t = cellidx[other] - 1;
+      const long long nb = P + (long long)((t < 0 ? t + ext[other] : t) - cellidx[other]) * step[other];
+      const double alp = fmax(h.H[along][0][nb], h.H[along][0][P]), alm = fmax(h.H[along][1][nb], h.H[along][1][P]);
+      T[leg] = hll_transport(alp, alm, v_lo, q_lo, v_hi, q_hi);
     }
-    const double* __restrict__ Bb = h.Bf[b];
-    const double* __restrict__ Ba = h.Bf[a];
-    const double* __restrict__ va = h.H[b][3];  // v_a on b-faces: b-sweep order (n = b, t1 = c, t2 = a)
-    const double* __restrict__ vb = h.H[a][2];  // v_b on a-faces: a-sweep order (n = a, t1 = b, t2 = c)
-    double unused, BbW, BbE, vaW, vaE, BaS, BaN, vbS, vbN;
-    {  // the staggered field has ghosts: plain offsets
-      const double q0 = Bb[P - 2 * st[a]], q1 = Bb[P - st[a]], q2 = Bb[P], q3 = Bb[P + st[a]];
-      face_values<LIM>(q1, q1 - q0, q2 - q1, dx2, unused, BbW);
-      face_values<LIM>(q2, q2 - q1, q3 - q2, dx2, BbE, unused);
-    }
-    {
-      const double q0 = va[oa[0]], q1 = va[oa[1]], q2 = va[P], q3 = va[oa[3]];
-      face_values<LIM>(q1, q1 - q0, q2 - q1, dx2, unused, vaW);
-      face_values<LIM>(q2, q2 - q1, q3 - q2, dx2, vaE, unused);
-    }
-    {
-      const double q0 = Ba[P - 2 * st[b]], q1 = Ba[P - st[b]], q2 = Ba[P], q3 = Ba[P + st[b]];
-      face_values<LIM>(q1, q1 - q0, q2 - q1, dx2, unused, BaS);
-      face_values<LIM>(q2, q2 - q1, q3 - q2, dx2, BaN, unused);
-    }
-    {
-      const double q0 = vb[ob[0]], q1 = vb[ob[1]], q2 = vb[P], q3 = vb[ob[3]];
-      face_values<LIM>(q1, q1 - q0, q2 - q1, dx2, unused, vbS);
-      face_values<LIM>(q2, q2 - q1, q3 - q2, dx2, vbN, unused);
-    }
-    const double aap = fmax(h.H[a][0][ob[1]], h.H[a][0][P]), aam = fmax(h.H[a][1][ob[1]], h.H[a][1][P]);
-    const double abp = fmax(h.H[b][0][oa[1]], h.H[b][0][P]), abm = fmax(h.H[b][1][oa[1]], h.H[b][1][P]);
-    const double term_a = (aap * vaW * BbW + aam * vaE * BbE - aap * aam * (BbE - BbW)) / (aap + aam);
-    const double term_b = (abp * vbS * BaS + abm * vbN * BaN - abp * abm * (BaN - BaS)) / (abp + abm);
-    h.E[c][P] = -term_a + term_b;
+    h.E[c][P] = T[1] - T[0];
   }
 }
 
@@ -674,8 +682,10 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
     v[10] = v[2] * v[5] - v[1] * v[6];
     if (!(u[0] > 0.0) || !(v[4] > 0.0)) a.sc->flag = 1;
     const long long gz = k < NG ? (long long)g.nz * g.sz : (k >= g.nz - NG ? -(long long)g.nz * g.sz : 0);
+    const bool want_ec = a.V[8] != nullptr;  // only the separate sweeps read the reference EMF back
 #pragma unroll
-    for (int n = 0; n < 11; ++n) a.V[n][c] = v[n];
+    for (int n = 0; n < 11; ++n)
+      if (n < 8 || want_ec) a.V[n][c] = v[n];
     if (gx != 0 || gy != 0 || gz != 0) {
 #pragma unroll
       for (int m = 1; m < 8; ++m) {
@@ -683,7 +693,8 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
         const bool ok = (!(m & 1) || gx != 0) && (!(m & 2) || gy != 0) && (!(m & 4) || gz != 0);
         if (ok) {
 #pragma unroll
-          for (int n = 0; n < 11; ++n) a.V[n][c + off] = v[n];
+          for (int n = 0; n < 11; ++n)
+            if (n < 8 || want_ec) a.V[n][c + off] = v[n];
         }
       }
     }
@@ -753,6 +764,20 @@ int make_tensor_maps(idfx_ctx* c) {
       return IDFX_ERR_CUDA;
     }
     return IDFX_OK;
+  }
+  if (c->mhd_fused) {
+    const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, 22}, dimB[4] = {(cuuint64_t)g.sy, py, pz, 9};
+    const cuuint32_t boxV[4] = {(cuuint32_t)MS_BW, (cuuint32_t)MS_BH, 1u, 8u}, boxB[4] = {(cuuint32_t)MS_BWB, (cuuint32_t)MS_TY, 1u, 3u};
+    CUresult r1 = enc(&c->mapMV, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_V), dimV, strides, boxV, es,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r2 = enc(&c->mapMB, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_BA), dimB, strides, boxB, es,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r1 != CUDA_SUCCESS || r2 != CUDA_SUCCESS) {
+      set_err("cuTensorMapEncodeTiled failed");
+      return IDFX_ERR_CUDA;
+    }
   }
   for (int d = 0; d < 3; ++d) {
     const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, 22}, dimB[4] = {(cuuint64_t)g.sy, py, pz, 9};
@@ -934,7 +959,8 @@ EmfArgs emf_args(idfx_ctx* c) {
     a.FB[d][1] = c->field(F_FB + 2 * d + 1);
     a.SG[d] = c->sgn(d);
     a.Ec[d] = c->vfield(8 + d);
-    a.Eg[d] = c->emf == EMF_UCT_HLL ? c->field(c->f_eg() + d) : nullptr;
+    // edge EMFs already evaluated: by k_emf_hll2d (2D-HLL), or by the one-kernel stage (mhd_stage.cuh)
+    a.Eg[d] = c->emf == EMF_UCT_HLL ? c->field(c->f_eg() + d) : (c->mhd_fused ? c->field(F_FB + d) : nullptr);
   }
   return a;
 }
@@ -1063,6 +1089,53 @@ void launch_hd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int 
   hd_kernel(c, first)<<<grid, HD_THREADS, HD_SMEM_BYTES, c->stream>>>(g, a, c->mapHD);
 }
 
+// ---- MHD: the three sweeps of a stage in one kernel (mhd_stage.cuh; instantiated in sweeps_inst.cu) ----
+template <int SOLVER>
+MhdKernel mhd_kernel_s(int limiter, bool first, int mode) {
+  switch (limiter) {
+    case LIM_FLAT: return mhd_kernel_sl<SOLVER, LIM_FLAT>(first, mode);
+    case LIM_MINMOD: return mhd_kernel_sl<SOLVER, LIM_MINMOD>(first, mode);
+    case LIM_LIMO3: return mhd_kernel_sl<SOLVER, LIM_LIMO3>(first, mode);
+    default: return mhd_kernel_sl<SOLVER, LIM_VANLEER>(first, mode);
+  }
+}
+
+// mode: the edge EMF the kernel evaluates (arithmetic, E^c, E^0); the 2D-HLL EMF comes from its own kernels afterwards
+MhdKernel mhd_kernel(const idfx_ctx* c, bool first, int mode) {
+  switch (c->solver) {
+    case SOLVER_HLL: return mhd_kernel_s<SOLVER_HLL>(c->limiter, first, mode);
+    case SOLVER_RUSANOV: return mhd_kernel_s<SOLVER_RUSANOV>(c->limiter, first, mode);
+    case SOLVER_HLLD: return mhd_kernel_s<SOLVER_HLLD>(c->limiter, first, mode);
+    default: return mhd_kernel_s<SOLVER_ROE>(c->limiter, first, mode);
+  }
+}
+
+void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int uout, int bin) {
+  const Geom& g = c->g;
+  MhdStageArgs a;
+  a.fV0 = c->vcur ? 11 : 0;
+  a.fB0 = 3 * bin;
+  const long long per_chunk = (long long)((g.nx + MS_CX - 1) / MS_CX) * ((g.ny + MS_CY - 1) / MS_CY);
+  long long nch = (148 * 24 + per_chunk - 1) / per_chunk;  // about 24 waves of one CTA per SM: a short last wave
+  const long long maxch = g.nz / 16 > 0 ? g.nz / 16 : 1;
+  nch = nch < 1 ? 1 : (nch > maxch ? maxch : nch);
+  a.chunk = (int)((g.nz + nch - 1) / nch);
+  for (int n = 0; n < 5; ++n) {
+    a.R[n] = c->field(F_R + n);
+    a.Uin[n] = c->field(uin + n);
+    a.U0[n] = c->field(F_UA + n);
+    a.Uout[n] = c->field(uout + n);
+  }
+  for (int d = 0; d < 3; ++d) a.E[d] = c->field(F_FB + d);  // the edge lattice lives in the first three face-flux slots
+  a.sc = c->sc;
+  a.w = w;
+  a.w0 = w0;
+  dim3 grid((g.nx + MS_CX - 1) / MS_CX, (g.ny + MS_CY - 1) / MS_CY, (unsigned)((g.nz + a.chunk - 1) / a.chunk));
+  LaunchScope ls(c, K_MHD);
+  mhd_kernel(c, first, c->emf == EMF_UCT_HLL ? EMF_ARITH : c->emf)<<<grid, MS_THREADS, MS_SMEM_BYTES, c->stream>>>(g, a, c->mapMV,
+                                                                                                                 c->mapMB);
+}
+
 // One stage S_dt (O2) followed by the RK combine of Eq. 9.  s: stage index (0-based); bin: face buffer of the stage
 // input; b0: saved face buffer; bout: destination.  Conserved fields: U_0 lives in F_UA for the whole cycle, the
 // intermediate stages in F_UB, the last stage writes the result back to F_UA.
@@ -1074,9 +1147,11 @@ void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, d
   const double w = W[c->nstages - 1][s], w0 = W0[c->nstages - 1][s];
   const double* Bf[3] = {c->bbuf(bin, 0), c->bbuf(bin, 1), c->bbuf(bin, 2)};
   const bool ppm = c->limiter == LIM_PPM;
-  const ApplyInfo ap = {combine && c->mhd && c->use_tma && !ppm, w, w0, uin, uout};
+  const ApplyInfo ap = {combine && c->mhd && (c->use_tma || c->mhd_fused) && !ppm, w, w0, uin, uout};
   if (ppm) {
     launch_ppm(c, Bf, want_dt);
+  } else if (c->mhd_fused) {
+    launch_mhd_stage(c, !combine, w, w0, uin, uout, bin);
   } else if (c->hd_fused) {
     launch_hd_stage(c, !combine, w, w0, uin, uout);
     if (combine) {  // the kernel wrote U_s, its primitives and their ghost images into the other primitive buffer
@@ -1114,12 +1189,14 @@ void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, d
     // EMFs of neighbouring tiles still read the stage-input primitives while this tile writes the result's
     const EmfArgs ea = emf_args(c);
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield_out(n);
+    if (c->mhd_fused)  // the one-kernel stage forms -(v x Bc) itself
+      for (int n = 8; n < 11; ++n) a.V[n] = nullptr;
     dim3 grid((g.nx + CT_TX - 1) / CT_TX, (g.ny + CT_TY - 1) / CT_TY, (g.nz + CT_TZ - 1) / CT_TZ);
     const bool udone = ap.on;  // the TMA z sweep applied the divergence itself
     if (c->emf == EMF_UCT_HLL) launch_hll2d(c, Bf);
     LaunchScope ls(c, K_UPDATE);
-    if (c->emf == EMF_UCT) launch_ct<EMF_UCT>(c, grid, ea, a, combine, udone);
-    else if (c->emf == EMF_UCT_HLL) launch_ct<EMF_UCT_HLL>(c, grid, ea, a, combine, udone);
+    if (c->mhd_fused || c->emf == EMF_UCT_HLL) launch_ct<EMF_UCT_HLL>(c, grid, ea, a, combine, udone);  // lattice read from memory
+    else if (c->emf == EMF_UCT) launch_ct<EMF_UCT>(c, grid, ea, a, combine, udone);
     else if (c->emf == EMF_UCT0) launch_ct<EMF_UCT0>(c, grid, ea, a, combine, udone);
     else launch_ct<EMF_ARITH>(c, grid, ea, a, combine, udone);
     c->vcur ^= 1;
@@ -1308,13 +1385,19 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
   const char* henv = getenv("IDFX_HD_FUSED");
   c->hd_fused = !c->mhd && !(henv && henv[0] == '0') && c->limiter != LIM_PPM;
   if (c->limiter == LIM_PPM) c->use_tma = false;  // PPM runs through k_flux_face_ppm / k_rhs
-  if (c->use_tma || c->hd_fused) {
+  const char* menv = getenv("IDFX_MHD_FUSED");
+  c->mhd_fused = c->mhd && !(menv && menv[0] == '0') && c->limiter != LIM_PPM;
+  if (c->use_tma || c->hd_fused || c->mhd_fused) {
     int rc = make_tensor_maps(c);
     if (rc) return rc;
   }
   if (c->hd_fused)
     for (int first = 0; first < 2; ++first)
       CK(cudaFuncSetAttribute((const void*)hd_kernel(c, first != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, HD_SMEM_BYTES));
+  if (c->mhd_fused)
+    for (int first = 0; first < 2; ++first)
+      CK(cudaFuncSetAttribute((const void*)mhd_kernel(c, first != 0, c->emf == EMF_UCT_HLL ? EMF_ARITH : c->emf),
+                              cudaFuncAttributeMaxDynamicSharedMemorySize, MS_SMEM_BYTES));
   c->bound = true;
   return IDFX_OK;
 }

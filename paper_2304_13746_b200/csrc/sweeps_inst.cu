@@ -150,9 +150,19 @@ HdKernel hd_kernel_sl(bool first) {
   return first ? (HdKernel)k_hd_stage<SOLVER, LIM, true> : (HdKernel)k_hd_stage<SOLVER, LIM, false>;
 }
 
+template <int SOLVER, int LIM>
+MhdKernel mhd_kernel_sl(bool first, int emf_mode) {
+  switch (emf_mode) {
+    case EMF_UCT: return first ? (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_UCT, true> : (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_UCT, false>;
+    case EMF_UCT0: return first ? (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_UCT0, true> : (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_UCT0, false>;
+    default: return first ? (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_ARITH, true> : (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_ARITH, false>;
+  }
+}
+
 // MHD: every solver but HLLC; hydrodynamics: every solver but HLLD (idfx_create refuses the other combinations)
 #if IDFX_INST_SOLVER != 1
 template void launch_sweeps_t<IDFX_INST_SOLVER, IDFX_INST_LIM, true>(idfx_ctx*, const double* const[3], bool, const ApplyInfo&);
+template MhdKernel mhd_kernel_sl<IDFX_INST_SOLVER, IDFX_INST_LIM>(bool, int);
 #endif
 #if IDFX_INST_SOLVER != 2
 template void launch_sweeps_t<IDFX_INST_SOLVER, IDFX_INST_LIM, false>(idfx_ctx*, const double* const[3], bool, const ApplyInfo&);
