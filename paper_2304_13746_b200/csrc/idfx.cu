@@ -497,6 +497,7 @@ struct UpdateArgs {
   const double* A0[3];
   double* Aout[3];
   const double* Bref[3];  // and the face field the potential is counted from (ghosts filled)
+  int store_u;            // first stage: 0 = U_1 is needed for the primitives only (rk2_keeps_no_u1)
   double dt_fixed;        // > 0: use it; otherwise dt = cfl / smax (first stage; later stages read sc->dt_used)
   double cfl;
   double w, w0;           // Eq. 9: U_s = w U* + w0 U_0 (stages >= 2)
@@ -635,7 +636,7 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
         } else {
           u[n] = us;
         }
-        a.Uout[n][c] = u[n];
+        if (STAGE2 || a.store_u) a.Uout[n][c] = u[n];
       }
     }
     const double ex00 = sE[0][lk][lj][li], ex10 = sE[0][lk][lj + 1][li];
@@ -1110,6 +1111,10 @@ MhdKernel mhd_kernel(const idfx_ctx* c, bool first, int mode) {
   }
 }
 
+// RK2 without a stored U_1 (one-kernel stages, no pressure floor): the first stage's update kernel keeps U_1 in registers
+// for the primitives only, and the second stage rebuilds it from U_0 and R_1, which it reads instead of U_1
+bool rk2_keeps_no_u1(const idfx_ctx* c) { return c->mhd_fused && c->nstages == 2 && !(c->g.pfloor > 0.0); }
+
 void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int uout, int bin) {
   const Geom& g = c->g;
   MhdStageArgs a;
@@ -1122,10 +1127,11 @@ void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int
   a.chunk = (int)((g.nz + nch - 1) / nch);
   for (int n = 0; n < 5; ++n) {
     a.R[n] = c->field(F_R + n);
-    a.Uin[n] = c->field(uin + n);
+    a.Uin[n] = c->field((rk2_keeps_no_u1(c) ? F_R : uin) + n);
     a.U0[n] = c->field(F_UA + n);
     a.Uout[n] = c->field(uout + n);
   }
+  a.uin_is_r = rk2_keeps_no_u1(c) ? 1 : 0;
   for (int d = 0; d < 3; ++d) a.E[d] = c->field(F_FB + d);  // the edge lattice lives in the first three face-flux slots
   a.sc = c->sc;
   a.w = w;
@@ -1183,6 +1189,7 @@ void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, d
   a.cfl = cfl;
   a.w = w;
   a.w0 = w0;
+  a.store_u = !(s == 0 && rk2_keeps_no_u1(c));
   const Geom& g = c->g;
   if (c->mhd) {
     // edge EMFs + CT + RK combine + cons->prim + ghost images in one kernel; V is double-buffered because the

@@ -15,8 +15,8 @@
 // and row TY-1 only supply faces to their lower neighbours.
 //   all stages  : E_x, E_y, E_z on the edge lattice (three doubles per cell) for the CT update in k_ct_update
 //   first stage : R = flux divergence (dt is not known before the whole grid has been swept), max_cells sum_d c_d / dx
-//   later stages: U_s = w0 U_0 + w (U_{s-1} - dt/dx R) applied at once (Eq. 9); U_{s-1} and U_0 of the cell are staged by
-//                 cp.async one plane ahead, so no register waits for them
+//   later stages: U_s = w0 U_0 + w (U_{s-1} - dt/dx R) applied at once (Eq. 9); U_{s-1} and U_0 of the cell are loaded
+//                 ahead of the EMF evaluation and used behind it
 // Per cell and stage the kernel reads 11 doubles and writes 8 (later stages: reads 21), against 57 (67) for the three
 // separate sweeps with their x-flux, partial-divergence, face-flux and sign arrays.
 #pragma once
@@ -67,8 +67,7 @@ constexpr int MS_SLAB = MS_TY * MS_TX;                            // one exchang
 constexpr int MS_EXS_DOUBLES = EX_ND * MS_SLAB;
 constexpr int MS_EXL_DOUBLES = EL_ND * MS_SLAB + MS_SLAB / 2;
 constexpr int MS_EXCH_BYTES = (2 * MS_EXS_DOUBLES + 3 * MS_EXL_DOUBLES) * 8;
-constexpr int MS_USTAGE_BYTES = 10 * MS_SLAB * 8;                 // U_{s-1} and U_0 of the cell being closed (later stages)
-constexpr int MS_SMEM_BYTES = MS_RING_BYTES + MS_EXCH_BYTES + MS_USTAGE_BYTES + MS_NST * 8 + 128;
+constexpr int MS_SMEM_BYTES = MS_RING_BYTES + MS_EXCH_BYTES + MS_NST * 8 + 128;
 static_assert((8 * MS_FIELD * 8) % 128 == 0, "the face-field box must land on a 128-byte boundary behind the primitives");
 static_assert(MS_SMEM_BYTES <= 227 * 1024, "ring + exchange area exceed the shared memory of an SM");
 
@@ -79,7 +78,8 @@ struct MhdStageArgs {
   double* R[5];
   double* E[3];   // edge EMFs, lower-edge indexing: E[0](i,j,k) = E_x(i, j-1/2, k-1/2), E[1] = E_y(i-1/2, j, k-1/2), E[2] = E_z(i-1/2, j-1/2, k)
   DevScalars* sc;
-  const double* Uin[5];
+  const double* Uin[5];  // U_{s-1}; or, with uin_is_r, the first stage's divergence R_1 (RK2: U_1 = U_0 - dt/dx R_1 is never stored)
+  int uin_is_r;
   const double* U0[5];
   double* Uout[5];
   double w, w0;
@@ -131,11 +131,6 @@ __device__ __forceinline__ double ms_edge(const double onA[2], const double onB[
   return mean + 0.25 * side;
 }
 
-__device__ __forceinline__ void cp_async_8(void* smem_dst, const void* gsrc) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
 // MODE: EMF_ARITH, EMF_UCT (upwind-contact) or EMF_UCT0
 template <int SOLVER, int LIM, int MODE, bool FIRST>
 __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArgs a, const __grid_constant__ CUtensorMap mapV,
@@ -145,8 +140,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
   unsigned char* ms_smem = ms_smem_raw + ((128u - (smem_u32(ms_smem_raw) & 127u)) & 127u);
   double (*ring)[MS_STRIDE] = reinterpret_cast<double (*)[MS_STRIDE]>(ms_smem);
   double* exch = reinterpret_cast<double*>(ms_smem + MS_RING_BYTES);
-  double* ustage = reinterpret_cast<double*>(ms_smem + MS_RING_BYTES + MS_EXCH_BYTES);
-  uint64_t* full = reinterpret_cast<uint64_t*>(ms_smem + MS_RING_BYTES + MS_EXCH_BYTES + MS_USTAGE_BYTES);
+  uint64_t* full = reinterpret_cast<uint64_t*>(ms_smem + MS_RING_BYTES + MS_EXCH_BYTES);
   const double dx2 = g.dx * g.dx;
   const int lx = threadIdx.x & 31, ly = threadIdx.x >> 5;
   const int x0 = blockIdx.x * MS_CX, y0 = blockIdx.y * MS_CY;
@@ -295,31 +289,43 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
     __syncthreads();  // the exchange set of this plane is complete; nobody reads plane s of the ring any more
     refill(p);
     if (!complete || s < s0) continue;  // (no barrier below this line)
-    // ---- close cell s-1 ----
+    // ---- close cell s-1: its divergence is complete.  First stage: store it.  Later stages: Eq. 9 at once; the loads of
+    // U_{s-1} and U_0 are issued here and used behind the EMF evaluation below, which hides their latency ----
+    const long long cu = c - g.sz;
+    double rt[5], uin[5], u0[5];
     if (s > s0) {
-      const long long cu = c - g.sz;
+#pragma unroll
+      for (int n = 0; n < 5; ++n) rt[n] = acc[n] + Fz[n];
       if (FIRST) {
 #pragma unroll
-        for (int n = 0; n < 5; ++n) a.R[n][cu] = acc[n] + Fz[n];
+        for (int n = 0; n < 5; ++n) a.R[n][cu] = rt[n];
         smax = fmax(smax, csxy + fmax(cfzp, cfz));  // G8
       } else {
-        // staged by this thread one iteration ago
-        cp_async_wait_all();
-        const double* us = ustage + se;
 #pragma unroll
         for (int n = 0; n < 5; ++n) {
-          const double u0 = us[(5 + n) * MS_SLAB];
-          a.Uout[n][cu] = dtdx == 0.0 ? u0 : a.w0 * u0 + a.w * (us[n * MS_SLAB] - dtdx * (acc[n] + Fz[n]));  // Eq. 9
+          uin[n] = a.Uin[n][cu];
+          u0[n] = a.U0[n][cu];
         }
       }
     }
-    if (s == s1) break;
-    if (!FIRST) {  // U_{s-1}, U_0 of cell s: needed when the cell is closed, one plane from now
-      double* us = ustage + se;
+    auto apply = [&]() {
+      if (FIRST || s == s0) return;
 #pragma unroll
       for (int n = 0; n < 5; ++n) {
-        cp_async_8(us + n * MS_SLAB, a.Uin[n] + c);
-        cp_async_8(us + (5 + n) * MS_SLAB, a.U0[n] + c);
+        // RK2 keeps no copy of U_1: it is U_0 - dt/dx R_1, with R_1 in place of U_{s-1} (same expression as k_ct_update's)
+        const double us = a.uin_is_r ? u0[n] - dtdx * uin[n] : uin[n];
+        a.Uout[n][cu] = dtdx == 0.0 ? u0[n] : a.w0 * u0[n] + a.w * (us - dtdx * rt[n]);  // Eq. 9
+      }
+    };
+    if (s == s1) {
+      apply();
+      break;
+    }
+    if (!FIRST) {  // the same lines of the next plane, on their way to L2
+#pragma unroll
+      for (int n = 0; n < 5; ++n) {
+        prefetch_l2(a.Uin[n] + c);
+        prefetch_l2(a.U0[n] + c);
       }
     }
     // ---- cell s: x and y parts of its divergence, minus its lower z flux ----
@@ -393,6 +399,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
       }
       a.E[1][c + up_x] = ms_edge<MODE>(onA, onB, cl, wA, wB);
     }
+    apply();
   }
   if (FIRST) {
     const double m = block_max_ms(complete ? smax / g.dx : 0.0);
