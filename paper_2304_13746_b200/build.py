@@ -2,7 +2,7 @@
 
     python -m paper_2304_13746_b200.build [--force] [-v]
 
-Translation units: csrc/idfx.cu (C ABI, state kernels, fused CT/update kernel), csrc/probe.cu, and csrc/sweeps_inst.cu once
+Translation units: csrc/idfx.cu (C ABI, state kernels, fused CT/update kernel), csrc/probe.cu, and csrc/stage_inst.cu once
 per (Riemann solver, reconstruction) pair, compiled in parallel as separate nvcc processes.  No -split-compile: with it
 the code nvcc 12.9 generates for the register-bound sweep kernels (where their loads are scheduled, hence 0 to 96 bytes
 of spills) was found to change from one build of the same source to the next and with the core count of the build
@@ -16,7 +16,7 @@ from concurrent.futures import ThreadPoolExecutor
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _OBJ = os.path.join(_HERE, "build")
-SOURCES = [os.path.join(_CSRC, f) for f in ("idfx.cu", "probe.cu", "sweeps_inst.cu")]
+SOURCES = [os.path.join(_CSRC, f) for f in ("idfx.cu", "probe.cu", "stage_inst.cu")]
 HEADERS = sorted(os.path.join(_CSRC, f) for f in os.listdir(_CSRC) if f.endswith(".cuh")) + [
     os.path.join(os.path.dirname(_HERE), "include", "idfx.h"), os.path.join(os.path.dirname(_HERE), "include", "idfx_probe.h")]
 LIB = os.path.join(_HERE, "libidfx.so")
@@ -34,7 +34,7 @@ def _units(obj_dir):
     units = [(os.path.join(obj_dir, "idfx.o"), ["-c", SOURCES[0]])]
     for s in sorted(SOLVERS, key=lambda s: s != 3):   # Roe takes longest
         for l in reversed(LIMITERS):
-            units.append((os.path.join(obj_dir, "sweeps_%d_%d.o" % (s, l)),
+            units.append((os.path.join(obj_dir, "stage_%d_%d.o" % (s, l)),
                           ["-DIDFX_INST_SOLVER=%d" % s, "-DIDFX_INST_LIM=%d" % l, "-c", SOURCES[2]]))
     units.append((os.path.join(obj_dir, "probe.o"), ["-c", SOURCES[1]]))
     return units

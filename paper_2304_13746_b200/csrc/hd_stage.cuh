@@ -32,9 +32,7 @@ constexpr int HD_STRIDE = (HD_PLANE + 15) / 16 * 16;  // doubles between ring st
 constexpr int HD_RING_BYTES = HD_NST * HD_STRIDE * 8;
 constexpr int HD_EXCH_BYTES = 2 * 6 * HD_TY * HD_TX * 8;
 constexpr int HD_SMEM_BYTES = HD_RING_BYTES + HD_EXCH_BYTES + 2 * HD_NST * 8 + 128;
-#ifndef IDFX_MINB_HD
-#define IDFX_MINB_HD 2
-#endif
+constexpr int HD_MINB = 2;  // CTAs per SM
 
 struct HdStageArgs {
   int fV0;        // first field of the stage-input primitives inside the tensor map (0 or 11)
@@ -78,7 +76,7 @@ __device__ __forceinline__ double hd_face(const double qm2[5], const double qm1[
 }
 
 template <int SOLVER, int LIM, bool FIRST>
-__global__ void __launch_bounds__(HD_THREADS, IDFX_MINB_HD) k_hd_stage(Geom g, HdStageArgs a, const __grid_constant__ CUtensorMap mapV) {
+__global__ void __launch_bounds__(HD_THREADS, HD_MINB) k_hd_stage(Geom g, HdStageArgs a, const __grid_constant__ CUtensorMap mapV) {
   // dynamic shared memory (HD_SMEM_BYTES, above the 48 KB static limit): the plane ring, the exchange array of the lower
   // y-face fluxes and c_face (double-buffered), the barriers
   extern __shared__ __align__(128) unsigned char hd_smem_raw[];

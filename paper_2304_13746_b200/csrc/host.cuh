@@ -1,5 +1,5 @@
 // host.cuh — host-side context of the idfx CUDA path, shared by the translation units of libidfx.so:
-// idfx.cu (C ABI, state kernels, fused CT/update kernel) and sweeps_inst.cu (the flux sweeps, compiled once per
+// idfx.cu (C ABI, state kernels, fused CT/update kernel) and stage_inst.cu (the one-kernel stages, compiled once per
 // Riemann solver and reconstruction so that the code generated for one combination does not depend on the others).
 #pragma once
 #include <cuda.h>
@@ -10,10 +10,8 @@
 #include "../../include/idfx.h"
 #include "common.cuh"
 #include "physics.cuh"
-#include "flux_march.cuh"
 #include "hd_stage.cuh"
 #include "mhd_stage.cuh"
-#include "flux_march_tma.cuh"
 
 namespace idfx {
 
@@ -27,12 +25,9 @@ enum {
   F_V = 19,    // 11: primitives, cell-centred B and Ec = -(v x Bc) of the stage input
   F_V2 = 30,   // 11: second buffer (MHD: the fused CT/update kernel reads the stage input while writing the result)
   F_R = 41,    // 5: flux divergence
-  F_FB = 46,   // 6: face fluxes of B, [d][0..1]
-  F_FX = 52,   // 5: x-face fluxes of (rho, m, E); F_FX+0 doubles as the x mass flux
-  F_CFX = 57,  // 1: c_face of the x sweep
-  F_SG = 58,   // 1 slot holding three byte fields: sign of the face mass flux of the x, y, z sweeps (E^c only)
-  F_CS = 59,   // 1: sum_d c_d per cell (x and y parts)
-  F_COUNT = 60,
+  F_FB = 46,   // 6: the edge EMFs E_x, E_y, E_z of the one-kernel MHD stage in the first three; PPM: face fluxes of B, [d][0..1]
+  F_SG = 52,   // 1 slot holding three byte fields: sign of the face mass flux per direction (PPM with E^c only)
+  F_COUNT = 53,
   // optional groups, appended in this order when present (idfx_ctx::f_aa, f_bref, f_h2d, f_eg):
   //   vector-potential form (idfx_set_option(IDFX_OPT_CT_FORM, IDFX_CT_POTENTIAL)): 3 x 3 edge-potential buffers rotating
   //   like the face-field buffers, and the 3 face fields given to set_state (ghosts filled);
@@ -79,12 +74,9 @@ struct idfx_ctx {
   long long graph_launches[6] = {0, 0, 0, 0, 0, 0};
   double graph_cfl = 0.0;
   bool use_graph = true;
-  bool use_tma = false;            // y/z sweeps stage their planes through shared memory with TMA (MHD)
-  CUtensorMap mapV[3], mapB[3];    // per sweep direction (1 = y, 2 = z): boxes over the V and face-B field groups
-  bool hd_fused = false;           // HD: one kernel per stage (hd_stage.cuh); IDFX_HD_FUSED=0 keeps the three sweeps
-  CUtensorMap mapHD;               // 36 x 11 x 1 x 5 boxes over the primitive fields
-  bool mhd_fused = false;          // MHD: the three sweeps of a stage in one kernel (mhd_stage.cuh)
-  CUtensorMap mapMV, mapMB;        // 36 x (TY+3) x 1 x 8 boxes over the primitives, x 3 over the face-field buffers
+  bool fused = false;              // one kernel per stage (hd_stage.cuh, mhd_stage.cuh): every reconstruction but PPM
+  CUtensorMap mapHD;               // HD: 36 x 11 x 1 x 5 boxes over the primitive fields
+  CUtensorMap mapMV, mapMB;        // MHD: 36 x (TY+3) x 1 x 8 boxes over the primitives, 34 x TY x 1 x 3 over the face-field buffers
   long long launches = 0;
   // optional per-kernel timing with CUDA events on the bound stream (idfx_profile_*)
   bool prof_on = false;
@@ -147,18 +139,7 @@ struct LaunchScope {
 
 inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
-// ---- the three flux sweeps of one stage --------------------------------------------------------
-struct ApplyInfo {
-  bool on;  // stages >= 2 with the TMA sweeps: the z sweep applies the divergence and the RK combine itself
-  double w, w0;
-  int uin, uout;  // first slots of the stage-input and result conserved fields
-};
-
-// The three flux sweeps of one stage (x, then y and z marching), defined and explicitly instantiated in sweeps_inst.cu.
-template <int SOLVER, int LIM, bool MHD>
-void launch_sweeps_t(idfx_ctx* c, const double* const Bf[3], bool want_dt, const ApplyInfo& ap);
-
-// Hydrodynamics: the whole stage in one kernel (hd_stage.cuh), same translation units.
+// Hydrodynamics: the whole stage in one kernel (hd_stage.cuh); defined and explicitly instantiated in stage_inst.cu.
 typedef void (*HdKernel)(Geom, HdStageArgs, const CUtensorMap);
 template <int SOLVER, int LIM>
 HdKernel hd_kernel_sl(bool first);

@@ -16,10 +16,8 @@
 #include "../../include/idfx.h"
 #include "common.cuh"
 #include "physics.cuh"
-#include "flux_march.cuh"      // argument structs of the sweep kernels (the kernels are instantiated in sweeps_inst.cu)
 #include "hd_stage.cuh"
 #include "mhd_stage.cuh"
-#include "flux_march_tma.cuh"
 
 namespace idfx {
 
@@ -341,16 +339,9 @@ __global__ void __launch_bounds__(128) k_rhs(Geom g, RhsArgs a) {
 // kernel's stores, which lets the update phase of k_ct_update issue loads of several cells at once.  Used for the flux
 // divergence, the face fluxes and signs, the stage-input face field and E^c, the saved face field: none of these
 // buffers is ever the destination of the same launch (run_stage)
-#ifndef IDFX_CT_LDG
-#define IDFX_CT_LDG 1
-#endif
 template <typename T>
 __device__ __forceinline__ T ldro(const T* p) {
-#if IDFX_CT_LDG
   return __ldg(p);
-#else
-  return *p;
-#endif
 }
 
 struct EmfArgs {
@@ -543,25 +534,10 @@ __global__ void __launch_bounds__(128, 16) k_update_hd(Geom g, UpdateArgs a) {  
 // edges read from shared memory, so the edge EMFs never travel to HBM; the result's ghost images (V and the new
 // face field) are written by the owners of the boundary cells, which replaces the separate ghost-fill pass.
 // ---------------------------------------------------------------------------------------------
-#ifndef IDFX_CT_TX
-#define IDFX_CT_TX 32
-#define IDFX_CT_TY 4
-#define IDFX_CT_TZ 8
-#endif
-constexpr int CT_TX = IDFX_CT_TX, CT_TY = IDFX_CT_TY, CT_TZ = IDFX_CT_TZ;
-#ifndef IDFX_CT_ZSPLIT
-#define IDFX_CT_ZSPLIT 2   // threads per (i, j) column of the tile in the update phase
-#endif
-constexpr int CT_ZSPLIT = IDFX_CT_ZSPLIT;
+constexpr int CT_TX = 32, CT_TY = 4, CT_TZ = 8;
+constexpr int CT_ZSPLIT = 2;  // threads per (i, j) column of the tile in the update phase
 constexpr int CT_THREADS = CT_TX * CT_TY * CT_ZSPLIT;
-#ifndef IDFX_MINB_CT
-#define IDFX_MINB_CT (8 / IDFX_CT_ZSPLIT)
-#endif
-#ifndef IDFX_CT_UNROLL
-#define IDFX_CT_UNROLL 1
-#endif
-#define IDFX_PRAGMA_(x) _Pragma(#x)
-#define IDFX_UNROLL(n) IDFX_PRAGMA_(unroll n)
+constexpr int CT_MINB = 4;    // CTAs per SM
 constexpr int CT_LX = CT_TX + 1, CT_LY = CT_TY + 1, CT_LZ = CT_TZ + 1;
 
 // UDONE: the conserved state was already combined by the z sweep (stages >= 2); only read it back for the primitives.
@@ -570,7 +546,7 @@ constexpr int CT_LX = CT_TX + 1, CT_LY = CT_TY + 1, CT_LZ = CT_TZ + 1;
 // NCU: the conserved fields this launch reads are not written by it (the host checks the buffers, launch_ct_v), so
 // they too can be loaded read-only.
 template <int MODE, bool STAGE2, bool UDONE, bool VP, bool NCU>
-__global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, EmfArgs ea, UpdateArgs a) {
+__global__ void __launch_bounds__(CT_THREADS, CT_MINB) k_ct_update(Geom g, EmfArgs ea, UpdateArgs a) {
   __shared__ double sE[3][CT_LZ][CT_LY][CT_LX];
   const int i0 = blockIdx.x * CT_TX, j0 = blockIdx.y * CT_TY, k0 = blockIdx.z * CT_TZ;
   double dt;
@@ -583,7 +559,7 @@ __global__ void __launch_bounds__(CT_THREADS, IDFX_MINB_CT) k_ct_update(Geom g, 
   }
   const bool idle = STAGE2 && dt == 0.0;  // a cycle at t_end (idfx_advance_to ran past it): hand U_0 on unchanged
   // ---- phase 1: edge lattice ----
-  IDFX_UNROLL(IDFX_CT_UNROLL)
+#pragma unroll 1
   for (int p = threadIdx.x; p < CT_LZ * CT_LY * CT_LX; p += CT_THREADS) {
     const int li = p % CT_LX, lj = (p / CT_LX) % CT_LY, lk = p / (CT_LX * CT_LY);
     const int I = i0 + li, J = j0 + lj, K = k0 + lk;
@@ -739,8 +715,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-// 4D tensor maps (x, y, z, field) over groups of equally spaced padded fields; one box = one sweep plane of a
-// 32 x 4 strip of pencils.
+// 4D tensor maps (x, y, z, field) over groups of equally spaced padded fields; one box = one z plane of a tile with its halo.
 int make_tensor_maps(idfx_ctx* c) {
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
@@ -766,7 +741,7 @@ int make_tensor_maps(idfx_ctx* c) {
     }
     return IDFX_OK;
   }
-  if (c->mhd_fused) {
+  {
     const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, 22}, dimB[4] = {(cuuint64_t)g.sy, py, pz, 9};
     const cuuint32_t boxV[4] = {(cuuint32_t)MS_BW, (cuuint32_t)MS_BH, 1u, 8u}, boxB[4] = {(cuuint32_t)MS_BWB, (cuuint32_t)MS_TY, 1u, 3u};
     CUresult r1 = enc(&c->mapMV, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_V), dimV, strides, boxV, es,
@@ -774,24 +749,6 @@ int make_tensor_maps(idfx_ctx* c) {
                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     CUresult r2 = enc(&c->mapMB, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_BA), dimB, strides, boxB, es,
                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r1 != CUDA_SUCCESS || r2 != CUDA_SUCCESS) {
-      set_err("cuTensorMapEncodeTiled failed");
-      return IDFX_ERR_CUDA;
-    }
-  }
-  for (int d = 0; d < 3; ++d) {
-    const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, 22}, dimB[4] = {(cuuint64_t)g.sy, py, pz, 9};
-    // x sweep: 36 columns x 4 rows of one z plane; y sweep: 32 x 1 x 4; z sweep: 32 x 4 x 1
-    const cuuint32_t bx = d == 0 ? (cuuint32_t)TX_W : 32u, by = d == 1 ? 1u : 4u, bz = d == 1 ? 4u : 1u;
-    const cuuint32_t boxV[4] = {bx, by, bz, 8};
-    const cuuint32_t boxB[4] = {bx, by, bz, 1};
-    const CUtensorMapL2promotion promo = d == 0 ? CU_TENSOR_MAP_L2_PROMOTION_NONE : CU_TENSOR_MAP_L2_PROMOTION_L2_256B;
-    CUresult r1 = enc(&c->mapV[d], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_V), dimV, strides, boxV, es,
-                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
-                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    CUresult r2 = enc(&c->mapB[d], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_BA), dimB, strides, boxB, es,
-                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r1 != CUDA_SUCCESS || r2 != CUDA_SUCCESS) {
       set_err("cuTensorMapEncodeTiled failed");
@@ -929,30 +886,6 @@ void launch_ppm(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
   }
 }
 
-template <int SOLVER, bool MHD>
-void launch_sweeps_s(idfx_ctx* c, const double* const Bf[3], bool want_dt, const ApplyInfo& ap) {
-  switch (c->limiter) {
-    case LIM_FLAT: launch_sweeps_t<SOLVER, LIM_FLAT, MHD>(c, Bf, want_dt, ap); break;
-    case LIM_MINMOD: launch_sweeps_t<SOLVER, LIM_MINMOD, MHD>(c, Bf, want_dt, ap); break;
-    case LIM_LIMO3: launch_sweeps_t<SOLVER, LIM_LIMO3, MHD>(c, Bf, want_dt, ap); break;
-    default: launch_sweeps_t<SOLVER, LIM_VANLEER, MHD>(c, Bf, want_dt, ap);
-  }
-}
-
-void launch_sweeps(idfx_ctx* c, const double* const Bf[3], bool want_dt, const ApplyInfo& ap) {
-  if (c->mhd) {
-    if (c->solver == SOLVER_HLL) launch_sweeps_s<SOLVER_HLL, true>(c, Bf, want_dt, ap);
-    else if (c->solver == SOLVER_RUSANOV) launch_sweeps_s<SOLVER_RUSANOV, true>(c, Bf, want_dt, ap);
-    else if (c->solver == SOLVER_HLLD) launch_sweeps_s<SOLVER_HLLD, true>(c, Bf, want_dt, ap);
-    else launch_sweeps_s<SOLVER_ROE, true>(c, Bf, want_dt, ap);
-  } else {
-    if (c->solver == SOLVER_HLL) launch_sweeps_s<SOLVER_HLL, false>(c, Bf, want_dt, ap);
-    else if (c->solver == SOLVER_RUSANOV) launch_sweeps_s<SOLVER_RUSANOV, false>(c, Bf, want_dt, ap);
-    else if (c->solver == SOLVER_HLLC) launch_sweeps_s<SOLVER_HLLC, false>(c, Bf, want_dt, ap);
-    else launch_sweeps_s<SOLVER_ROE, false>(c, Bf, want_dt, ap);
-  }
-}
-
 EmfArgs emf_args(idfx_ctx* c) {
   EmfArgs a;
   for (int d = 0; d < 3; ++d) {
@@ -961,7 +894,7 @@ EmfArgs emf_args(idfx_ctx* c) {
     a.SG[d] = c->sgn(d);
     a.Ec[d] = c->vfield(8 + d);
     // edge EMFs already evaluated: by k_emf_hll2d (2D-HLL), or by the one-kernel stage (mhd_stage.cuh)
-    a.Eg[d] = c->emf == EMF_UCT_HLL ? c->field(c->f_eg() + d) : (c->mhd_fused ? c->field(F_FB + d) : nullptr);
+    a.Eg[d] = c->emf == EMF_UCT_HLL ? c->field(c->f_eg() + d) : (c->fused ? c->field(F_FB + d) : nullptr);
   }
   return a;
 }
@@ -1113,7 +1046,7 @@ MhdKernel mhd_kernel(const idfx_ctx* c, bool first, int mode) {
 
 // RK2 without a stored U_1 (one-kernel stages, no pressure floor): the first stage's update kernel keeps U_1 in registers
 // for the primitives only, and the second stage rebuilds it from U_0 and R_1, which it reads instead of U_1
-bool rk2_keeps_no_u1(const idfx_ctx* c) { return c->mhd_fused && c->nstages == 2 && !(c->g.pfloor > 0.0); }
+bool rk2_keeps_no_u1(const idfx_ctx* c) { return c->mhd && c->fused && c->nstages == 2 && !(c->g.pfloor > 0.0); }
 
 void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int uout, int bin) {
   const Geom& g = c->g;
@@ -1152,21 +1085,17 @@ void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, d
   const int uin = s == 0 ? F_UA : F_UB, uout = last ? F_UA : F_UB;
   const double w = W[c->nstages - 1][s], w0 = W0[c->nstages - 1][s];
   const double* Bf[3] = {c->bbuf(bin, 0), c->bbuf(bin, 1), c->bbuf(bin, 2)};
-  const bool ppm = c->limiter == LIM_PPM;
-  const ApplyInfo ap = {combine && c->mhd && (c->use_tma || c->mhd_fused) && !ppm, w, w0, uin, uout};
-  if (ppm) {
+  if (!c->fused) {  // PPM: generic face-flux kernels, divergence and dt in k_rhs
     launch_ppm(c, Bf, want_dt);
-  } else if (c->mhd_fused) {
+  } else if (c->mhd) {
     launch_mhd_stage(c, !combine, w, w0, uin, uout, bin);
-  } else if (c->hd_fused) {
+  } else {
     launch_hd_stage(c, !combine, w, w0, uin, uout);
     if (combine) {  // the kernel wrote U_s, its primitives and their ghost images into the other primitive buffer
       c->vcur ^= 1;
       if (c->g.outflow) launch_fill(c, bout);  // it writes periodic images only
       return;
     }
-  } else {
-    launch_sweeps(c, Bf, want_dt, ap);
   }
   UpdateArgs a;
   for (int n = 0; n < 5; ++n) {
@@ -1196,13 +1125,13 @@ void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, d
     // EMFs of neighbouring tiles still read the stage-input primitives while this tile writes the result's
     const EmfArgs ea = emf_args(c);
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield_out(n);
-    if (c->mhd_fused)  // the one-kernel stage forms -(v x Bc) itself
+    if (c->fused)  // the one-kernel stage forms -(v x Bc) itself
       for (int n = 8; n < 11; ++n) a.V[n] = nullptr;
     dim3 grid((g.nx + CT_TX - 1) / CT_TX, (g.ny + CT_TY - 1) / CT_TY, (g.nz + CT_TZ - 1) / CT_TZ);
-    const bool udone = ap.on;  // the TMA z sweep applied the divergence itself
+    const bool udone = combine && c->fused;  // the one-kernel stage applied the divergence itself
     if (c->emf == EMF_UCT_HLL) launch_hll2d(c, Bf);
     LaunchScope ls(c, K_UPDATE);
-    if (c->mhd_fused || c->emf == EMF_UCT_HLL) launch_ct<EMF_UCT_HLL>(c, grid, ea, a, combine, udone);  // lattice read from memory
+    if (c->fused || c->emf == EMF_UCT_HLL) launch_ct<EMF_UCT_HLL>(c, grid, ea, a, combine, udone);  // lattice read from memory
     else if (c->emf == EMF_UCT) launch_ct<EMF_UCT>(c, grid, ea, a, combine, udone);
     else if (c->emf == EMF_UCT0) launch_ct<EMF_UCT0>(c, grid, ea, a, combine, udone);
     else launch_ct<EMF_ARITH>(c, grid, ea, a, combine, udone);
@@ -1387,21 +1316,15 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
                  c->stream != cudaStreamPerThread;
   const char* benv = getenv("IDFX_ADVANCE_BATCH");
   c->fixed_batch = benv ? atoi(benv) : 0;
-  const char* env = getenv("IDFX_TMA");
-  c->use_tma = c->mhd && !(env && env[0] == '0');  // IDFX_TMA=0 selects the register-prefetch sweeps (A/B only)
-  const char* henv = getenv("IDFX_HD_FUSED");
-  c->hd_fused = !c->mhd && !(henv && henv[0] == '0') && c->limiter != LIM_PPM;
-  if (c->limiter == LIM_PPM) c->use_tma = false;  // PPM runs through k_flux_face_ppm / k_rhs
-  const char* menv = getenv("IDFX_MHD_FUSED");
-  c->mhd_fused = c->mhd && !(menv && menv[0] == '0') && c->limiter != LIM_PPM;
-  if (c->use_tma || c->hd_fused || c->mhd_fused) {
+  c->fused = c->limiter != LIM_PPM;  // PPM (five-cell stencils) runs through k_flux_face_ppm / k_rhs
+  if (c->fused) {
     int rc = make_tensor_maps(c);
     if (rc) return rc;
   }
-  if (c->hd_fused)
+  if (c->fused && !c->mhd)
     for (int first = 0; first < 2; ++first)
       CK(cudaFuncSetAttribute((const void*)hd_kernel(c, first != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, HD_SMEM_BYTES));
-  if (c->mhd_fused)
+  if (c->fused && c->mhd)
     for (int first = 0; first < 2; ++first)
       CK(cudaFuncSetAttribute((const void*)mhd_kernel(c, first != 0, c->emf == EMF_UCT_HLL ? EMF_ARITH : c->emf),
                               cudaFuncAttributeMaxDynamicSharedMemorySize, MS_SMEM_BYTES));

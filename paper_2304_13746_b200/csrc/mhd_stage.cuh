@@ -30,13 +30,7 @@
 
 namespace idfx {
 
-#ifndef IDFX_MHD_TY
-#define IDFX_MHD_TY 12
-#endif
-#ifndef IDFX_MHD_NST
-#define IDFX_MHD_NST 2
-#endif
-constexpr int MS_TX = 32, MS_TY = IDFX_MHD_TY;       // threads
+constexpr int MS_TX = 32, MS_TY = 12;                // threads: 12 warps, 3 per scheduler, 168 registers each
 constexpr int MS_CX = MS_TX - 1, MS_CY = MS_TY - 1;  // cells a tile completes
 constexpr int MS_BW = 36, MS_BH = MS_TY + 3;         // box: columns x0-2-sh .., rows y0-2 .. y0+TY
 constexpr int MS_FIELD = MS_BW * MS_BH;              // doubles of one primitive field of a plane (rho, v, p, Bc: 8 fields)
@@ -44,7 +38,7 @@ constexpr int MS_BWB = 34;                           // the staggered field is n
 constexpr int MS_FIELD_B = MS_BWB * MS_TY;           // doubles of one face-field component of a plane (Bx_f, By_f, Bz_f)
 constexpr int MS_PLANE = 8 * MS_FIELD + 3 * MS_FIELD_B;
 constexpr uint32_t MS_BYTES_V = 8 * MS_FIELD * 8, MS_BYTES_B = 3 * MS_FIELD_B * 8;
-constexpr int MS_NST = IDFX_MHD_NST;
+constexpr int MS_NST = 2;                            // ring stages: the plane being solved and the next one
 constexpr int MS_THREADS = MS_TX * MS_TY;
 constexpr int MS_STRIDE = (MS_PLANE + 15) / 16 * 16;  // doubles between ring stages: TMA destinations are 128-byte aligned
 constexpr int MS_RING_BYTES = MS_NST * MS_STRIDE * 8;
@@ -309,12 +303,14 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
       }
     }
     auto apply = [&]() {
-      if (FIRST || s == s0) return;
+      if constexpr (!FIRST) {
+        if (s == s0) return;
 #pragma unroll
-      for (int n = 0; n < 5; ++n) {
-        // RK2 keeps no copy of U_1: it is U_0 - dt/dx R_1, with R_1 in place of U_{s-1} (same expression as k_ct_update's)
-        const double us = a.uin_is_r ? u0[n] - dtdx * uin[n] : uin[n];
-        a.Uout[n][cu] = dtdx == 0.0 ? u0[n] : a.w0 * u0[n] + a.w * (us - dtdx * rt[n]);  // Eq. 9
+        for (int n = 0; n < 5; ++n) {
+          // RK2 keeps no copy of U_1: it is U_0 - dt/dx R_1, with R_1 in place of U_{s-1} (same expression as k_ct_update's)
+          const double us = a.uin_is_r ? u0[n] - dtdx * uin[n] : uin[n];
+          a.Uout[n][cu] = dtdx == 0.0 ? u0[n] : a.w0 * u0[n] + a.w * (us - dtdx * rt[n]);  // Eq. 9
+        }
       }
     };
     if (s == s1) {

@@ -20,8 +20,7 @@ enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3, EMF_UCT_HLL = 4 }
 #define IDFX_DEV __device__ __forceinline__
 
 // Reciprocal and square root without the IEEE slow paths: hardware seed (upper 32 bits, ~2^-20) refined by one
-// third-order step in fp64 (the series in the residual e up to e^2, truncation ~ e^3 < 2^-57), result within ~1 ulp;
-// -DIDFX_NEWTON2 keeps the former two Newton steps (one more fp64 instruction per call).  All operands on this path are normal, finite and non-negative
+// third-order step in fp64 (the series in the residual e up to e^2, truncation ~ e^3 < 2^-57), result within ~1 ulp.  All operands on this path are normal, finite and non-negative
 // where a root is taken; zero is handled explicitly.  -DIDFX_PRECISE_MATH restores the correctly rounded forms.
 IDFX_DEV double rcp(double x) {
 #ifdef IDFX_PRECISE_MATH
@@ -29,15 +28,8 @@ IDFX_DEV double rcp(double x) {
 #else
   double y;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-#ifdef IDFX_NEWTON2
-  double e = fma(-x, y, 1.0);
-  y = fma(y, e, y);
-  e = fma(-x, y, 1.0);
-  return fma(y, e, y);
-#else
   const double e = fma(-x, y, 1.0);     // 1/x = y (1 + e + e^2 + O(e^3)), |e| <~ 2^-20
   return fma(y, fma(e, e, e), y);
-#endif
 #endif
 }
 
@@ -49,15 +41,8 @@ IDFX_DEV double rsqrt_pos(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   const double h = 0.5 * x;
-#ifdef IDFX_NEWTON2
-  double e = fma(-h * y, y, 0.5);  // (1 - x y^2)/2
-  y = fma(y, e, y);
-  e = fma(-h * y, y, 0.5);
-  return fma(y, e, y);
-#else
   const double e = fma(-h * y, y, 0.5);  // (1 - x y^2)/2;  x^-1/2 = y (1 + e + 3/2 e^2 + O(e^3))
   return fma(y, fma(1.5 * e, e, e), y);
-#endif
 #endif
 }
 
@@ -65,8 +50,6 @@ IDFX_DEV double rsqrt_pos(double x) {
 IDFX_DEV double sqrt_nn(double x) {
 #ifdef IDFX_PRECISE_MATH
   return sqrt(x);
-#elif defined(IDFX_NEWTON2)
-  return x * rsqrt_pos(fmax(x, 1e-300));
 #else
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(fmax(x, 1e-300)));
@@ -80,8 +63,6 @@ IDFX_DEV double sqrt_nn(double x) {
 IDFX_DEV double sqrt_pos(double x) {
 #ifdef IDFX_PRECISE_MATH
   return sqrt(x);
-#elif defined(IDFX_NEWTON2)
-  return x * rsqrt_pos(x);
 #else
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));

@@ -225,11 +225,9 @@ def test_sedov_blast_parity_and_radius(idfx, R):
     assert float(rho.max()) > 2.5
 
 
-@pytest.mark.parametrize("fused", ["1", "0"])
-def test_outflow_boundaries_hd(idfx, R, fused, monkeypatch):
-    """Zero-gradient ghosts (HD only): the paper's Sod tube with outflow ends along each axis, and a 3D blast reaching
-    the walls, against the oracle; both the fused stage kernel and the three-sweep path."""
-    monkeypatch.setenv("IDFX_HD_FUSED", fused)
+def test_outflow_boundaries_hd(idfx, R):
+    """Zero-gradient ghosts (HD): the paper's Sod tube with outflow ends along each axis, and a 3D blast reaching
+    the walls, against the oracle."""
     for axis in range(3):
         shape = [6, 5, 4]
         shape[2 - axis] = 64

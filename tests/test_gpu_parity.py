@@ -254,8 +254,8 @@ def test_minimum_size_box(idfx, R):
 
 
 def test_alternate_code_paths_in_a_subprocess(idfx):
-    """IDFX_TMA=0 (register-prefetch sweeps + separate R path in stage 2) and IDFX_GRAPH=0 (no CUDA-graph replay) are
-    A/B switches read at idfx_bind; run one MHD parity case under each in a fresh process."""
+    """IDFX_GRAPH=0 (no CUDA-graph replay: every cycle enqueued kernel by kernel) is read at idfx_bind; run one MHD and
+    one HD parity case under it in a fresh process."""
     import os
     import subprocess
     import sys
@@ -272,14 +272,13 @@ def test_alternate_code_paths_in_a_subprocess(idfx):
         "assert abs(sim.last_dt() - ref.last_dt()) <= T.TOL_DT * ref.last_dt()\n"
         "print('ok')\n"
     ) % (os.path.dirname(os.path.dirname(os.path.abspath(__file__))), os.path.dirname(os.path.abspath(__file__)))
-    for env_add in ({"IDFX_TMA": "0"}, {"IDFX_GRAPH": "0"}, {"IDFX_TMA": "0", "IDFX_GRAPH": "0"}):
+    for env_add in ({"IDFX_GRAPH": "0"},):
         p = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300,
                            env=dict(os.environ, **env_add))
         assert p.returncode == 0 and "ok" in p.stdout, (env_add, p.stderr[-2000:])
-    # hydrodynamics: IDFX_HD_FUSED=0 selects the three-sweep path instead of the one-kernel stage
     code_hd = code.replace("T.smooth_ic(37, 21, 13, 11)", "T.smooth_ic(37, 21, 13, 11, mhd=False)").replace(
         "T.HLLD, T.VANLEER, T.EMF_UCT", "T.HLLC, T.VANLEER, T.EMF_NONE")
-    for env_add in ({"IDFX_HD_FUSED": "0"}, {"IDFX_HD_FUSED": "0", "IDFX_GRAPH": "0"}, {"IDFX_GRAPH": "0"}):
+    for env_add in ({"IDFX_GRAPH": "0"},):
         p = subprocess.run([sys.executable, "-c", code_hd], capture_output=True, text=True, timeout=300,
                            env=dict(os.environ, **env_add))
         assert p.returncode == 0 and "ok" in p.stdout, (env_add, p.stderr[-2000:])
