@@ -100,7 +100,9 @@ int idfx_floor_count(idfx_ctx* ctx, long long* h_count_out); /* synchronises */
 size_t idfx_workspace_bytes(const idfx_ctx* ctx);
 
 /* Binds a caller-owned device workspace (>= idfx_workspace_bytes, 256-byte aligned) and a stream.
- * Zeroes the workspace on that stream.  Must precede every call below. */
+ * Zeroes the workspace on that stream.  Must precede every call below.  The stream and every device pointer passed to
+ * later calls must belong to the device that holds the workspace; the calls themselves may be made with any device
+ * current in the calling thread (the library switches to the workspace's device and restores the caller's). */
 int idfx_bind(idfx_ctx* ctx, void* d_workspace, size_t bytes, void* cuda_stream);
 
 /* Copy-in of the state (O1): Bc from faces, then conserved variables from the primitives.

@@ -217,9 +217,12 @@ __global__ void __launch_bounds__(HD_THREADS, HD_MINB) k_hd_stage(Geom g, HdStag
         const double vx = u[1] * ir, vy = u[2] * ir, vz = u[3] * ir;
         double pr = (g.gamma - 1.0) * (u[4] - 0.5 * u[0] * (vx * vx + vy * vy + vz * vz));
         if (g.pfloor > 0.0 && pr < g.pfloor) {
+          const bool acts = pr < g.pfloor * (1.0 - 1e-9);  // a cell floored before recomputes to the floor within rounding
           pr = g.pfloor;
-          u[4] = pr / (g.gamma - 1.0) + 0.5 * u[0] * (vx * vx + vy * vy + vz * vz);
-          atomicAdd(&a.sc->nfloor, 1ull);
+          if (acts) {
+            u[4] = pr / (g.gamma - 1.0) + 0.5 * u[0] * (vx * vx + vy * vy + vz * vz);
+            atomicAdd(&a.sc->nfloor, 1ull);
+          }
         }
         if (!(u[0] > 0.0) || !(pr > 0.0)) a.sc->flag = 1;
 #pragma unroll

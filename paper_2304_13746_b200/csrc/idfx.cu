@@ -142,7 +142,11 @@ __device__ __forceinline__ void prim_from_cons(double gm1, double rho, double mx
 __device__ __forceinline__ bool pressure_floor(const Geom& g, DevScalars* sc, double rho, double vx, double vy, double vz,
                                                double bx, double by, double bz, double& p, double& E) {
   if (!(g.pfloor > 0.0) || !(p < g.pfloor)) return false;
+  // a cell floored before recomputes to the floor within rounding: it is not floored (or counted) again, so a cycle that
+  // changes nothing (idfx_advance_to past t_end) leaves the count alone too
+  const bool acts = p < g.pfloor * (1.0 - 1e-9);
   p = g.pfloor;
+  if (!acts) return false;
   E = p / (g.gamma - 1.0) + 0.5 * rho * (vx * vx + vy * vy + vz * vz) + 0.5 * (bx * bx + by * by + bz * bz);
   atomicAdd(&sc->nfloor, 1ull);
   return true;
@@ -765,6 +769,19 @@ void drop_graphs(idfx_ctx* c) {
   }
 }
 
+// Every ABI call runs on the device that holds the workspace, whatever device is current in the calling thread, and
+// leaves the caller's current device as it found it.
+struct DeviceScope {
+  int prev = -1;
+  explicit DeviceScope(int dev) {
+    if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) cudaSetDevice(dev);
+    else prev = -1;
+  }
+  ~DeviceScope() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
 int check_bound(const idfx_ctx* c) {
   if (!c) {
     set_err("null context");
@@ -1300,6 +1317,14 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
     set_err("idfx_bind: workspace too small or not 256-byte aligned");
     return IDFX_ERR_INVALID_ARG;
   }
+  cudaPointerAttributes attr;
+  if (cudaPointerGetAttributes(&attr, d_workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+    cudaGetLastError();
+    set_err("idfx_bind: the workspace is not device memory");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  c->device = attr.device;
+  DeviceScope on_device(c->device);
   c->ws = (double*)d_workspace;
   c->ws_bytes = bytes;
   c->stream = (cudaStream_t)cuda_stream;
@@ -1335,6 +1360,7 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
 int idfx_set_state(idfx_ctx* c, const double* d_prim, const double* d_bface) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!d_prim || (c->mhd && !d_bface)) {
     set_err("idfx_set_state: null state pointer");
     return IDFX_ERR_INVALID_ARG;
@@ -1359,6 +1385,7 @@ int idfx_set_state(idfx_ctx* c, const double* d_prim, const double* d_bface) {
 int idfx_set_state_host(idfx_ctx* c, const double* h_prim, const double* h_bface) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!h_prim || (c->mhd && !h_bface)) {
     set_err("idfx_set_state_host: null state pointer");
     return IDFX_ERR_INVALID_ARG;
@@ -1377,6 +1404,7 @@ int idfx_set_state_host(idfx_ctx* c, const double* h_prim, const double* h_bface
 int idfx_get_state(idfx_ctx* c, double* d_prim, double* d_bface) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!d_prim) {
     set_err("idfx_get_state: null output");
     return IDFX_ERR_INVALID_ARG;
@@ -1403,6 +1431,7 @@ int idfx_get_state(idfx_ctx* c, double* d_prim, double* d_bface) {
 int idfx_get_state_host(idfx_ctx* c, double* h_prim, double* h_bface) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!h_prim) {
     set_err("idfx_get_state_host: null output");
     return IDFX_ERR_INVALID_ARG;
@@ -1421,6 +1450,7 @@ int idfx_get_state_host(idfx_ctx* c, double* h_prim, double* h_bface) {
 int idfx_get_conserved(idfx_ctx* c, double* d_cons, double* d_bface) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!d_cons) {
     set_err("idfx_get_conserved: null output");
     return IDFX_ERR_INVALID_ARG;
@@ -1446,6 +1476,7 @@ int idfx_get_conserved(idfx_ctx* c, double* d_cons, double* d_bface) {
 int idfx_compute_dt(idfx_ctx* c, double cfl, double* h_dt_out) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!h_dt_out || !(cfl > 0.0) || !(cfl < 1.0)) {
     set_err("idfx_compute_dt: need 0 < cfl < 1 and a non-null output");
     return IDFX_ERR_INVALID_ARG;
@@ -1467,6 +1498,7 @@ int idfx_compute_dt(idfx_ctx* c, double cfl, double* h_dt_out) {
 int idfx_step(idfx_ctx* c, double dt) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!(dt > 0.0)) {
     set_err("idfx_step: dt must be > 0");
     return IDFX_ERR_INVALID_ARG;
@@ -1526,6 +1558,7 @@ static int read_scalars(idfx_ctx* c, DevScalars* h) {
 int idfx_advance(idfx_ctx* c, int nsteps, double cfl) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (nsteps < 0 || !(cfl > 0.0) || !(cfl < 1.0)) {
     set_err("idfx_advance: need nsteps >= 0 and 0 < cfl < 1");
     return IDFX_ERR_INVALID_ARG;
@@ -1536,6 +1569,7 @@ int idfx_advance(idfx_ctx* c, int nsteps, double cfl) {
 int idfx_advance_to(idfx_ctx* c, double t_end, double cfl, int max_steps, int* h_nsteps_out, double* h_t_out) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (max_steps < 0 || !(cfl > 0.0) || !(cfl < 1.0) || !(t_end == t_end)) {
     set_err("idfx_advance_to: need max_steps >= 0, 0 < cfl < 1 and a t_end that is not NaN");
     return IDFX_ERR_INVALID_ARG;
@@ -1569,6 +1603,7 @@ int idfx_advance_to(idfx_ctx* c, double t_end, double cfl, int max_steps, int* h
 int idfx_time(idfx_ctx* c, double* h_t_out) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!h_t_out) return IDFX_ERR_INVALID_ARG;
   DevScalars h;
   if ((rc = read_scalars(c, &h))) return rc;
@@ -1632,6 +1667,7 @@ int idfx_set_option_real(idfx_ctx* c, int option, double value) {
 int idfx_floor_count(idfx_ctx* c, long long* h_count_out) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!h_count_out) return IDFX_ERR_INVALID_ARG;
   DevScalars h;
   if ((rc = read_scalars(c, &h))) return rc;
@@ -1642,6 +1678,7 @@ int idfx_floor_count(idfx_ctx* c, long long* h_count_out) {
 int idfx_get_potential(idfx_ctx* c, double* d_pot) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!c->vp || !d_pot) {
     set_err("idfx_get_potential: needs IDFX_CT_POTENTIAL and a non-null output");
     return IDFX_ERR_INVALID_ARG;
@@ -1659,6 +1696,7 @@ int idfx_get_potential(idfx_ctx* c, double* d_pot) {
 int idfx_last_dt(idfx_ctx* c, double* h_dt_out) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (!h_dt_out) return IDFX_ERR_INVALID_ARG;
   CK(cudaMemcpyAsync(h_dt_out, &c->sc->dt_used, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
@@ -1668,6 +1706,7 @@ int idfx_last_dt(idfx_ctx* c, double* h_dt_out) {
 int idfx_status(idfx_ctx* c) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   int flag = 0;
   CK(cudaMemcpyAsync(&flag, &c->sc->flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
@@ -1683,6 +1722,7 @@ long long idfx_launch_count(const idfx_ctx* c) { return c ? c->launches : 0; }
 int idfx_profile_enable(idfx_ctx* c, int on) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   prof_drain(c);
   for (int k = 0; k < K_COUNT; ++k) {
     c->prof_ms[k] = 0.0;
@@ -1695,6 +1735,7 @@ int idfx_profile_enable(idfx_ctx* c, int on) {
 int idfx_profile_read(idfx_ctx* c, int kernel_id, double* h_ms_total, long long* h_launches) {
   int rc = check_bound(c);
   if (rc) return rc;
+  DeviceScope on_device(c->device);
   if (kernel_id < 0 || kernel_id >= K_COUNT || !h_ms_total || !h_launches) {
     set_err("idfx_profile_read: bad kernel id or null output");
     return IDFX_ERR_INVALID_ARG;
@@ -1711,6 +1752,7 @@ const char* idfx_profile_kernel_name(int kernel_id) {
 
 void idfx_destroy(idfx_ctx* c) {
   if (!c) return;
+  DeviceScope on_device(c->device);
   prof_drain(c);
   drop_graphs(c);
   for (cudaEvent_t e : c->prof_free) cudaEventDestroy(e);

@@ -6,7 +6,10 @@
   outputs one by one: a 32^3 window cut out of the GPU state before a cycle, advanced by the oracle as a small
   periodic box with the same dt, agrees with the full computation on every cell further than 10 cells from the
   window boundary (domain of dependence of one RK2 cycle: <= 8 cells).  dt at full size is checked through the
-  per-cell signal-speed sums the oracle computes on windows around the fastest cells.
+  per-cell signal-speed sums the oracle computes on windows around the fastest cells.  Checked cycles: the first two,
+  the eleventh and the twenty-second (the last one bench.py times: 2-3 warm-up + 20); windows sit on the corners of the
+  periodic box, on the seams of the 31 x 11 tiles and z chunks of k_mhd_stage and of the 32 x 4 x 8 tiles of k_ct_update,
+  and at random places.
 """
 import os
 
@@ -35,7 +38,9 @@ def test_full_config_against_oracle_samples(idfx, name):
     if not os.path.exists(path):
         pytest.skip("golden samples for %s not generated (tests/golden/make_config_goldens.py)" % name)
     gold = np.load(path)
-    prim, b, cfg = inputs.make(name, device="cuda")
+    # the SAME arrays the goldens were computed from: synthesised on the CPU (as make_config_goldens.py does), then copied
+    prim, b, cfg = inputs.make(name)
+    prim, b = prim.cuda(), (None if b is None else b.cuda())
     n = cfg["n"]
     assert n == int(gold["n"]) and cfg["steps"] == int(gold["steps"])
     sim = idfx.Idfx(n, n, n, cfg["dx"], cfg["gamma"], cfg["solver"], cfg["limiter"], cfg["emf"])
@@ -84,9 +89,16 @@ def test_config5_512_windows_against_oracle(idfx, R):
     del prim, b
     rng = np.random.default_rng(5)
     origins = [(0, 0, 0), (n - 16, n - 16, n - 16), (n - 20, 3, 250), (100, n - 12, n - 30)]
-    origins += [tuple(int(x) for x in rng.integers(0, n, 3)) for _ in range(8)]
+    # seams of the launch configuration at 512^3: x tiles start at 31 m (the last, partial one at 496), y tiles at 11 m
+    # (last at 506), z chunks of 103 planes (5 chunks); k_ct_update tiles at multiples of (32, 4, 8)
+    origins += [(31 * 5 - 16, 11 * 9 - 16, 103 - 16), (496 - 16, 506 - 16, 412 - 16), (31 * 11 - 16, 11 * 30 - 16, 309 - 16),
+                (32 * 7 - 16, 4 * 50 - 16, 8 * 33 - 16)]
+    origins += [tuple(int(x) for x in rng.integers(0, n, 3)) for _ in range(6)]
     worst = 0.0
-    for cycle in range(2):
+    done = 0
+    for cycle in (0, 1, 10, 21):
+        sim.advance(cycle - done, cfl)
+        done = cycle + 1
         p0, b0 = sim.get_state()
         # ---- dt at full size: windows around the cells with the largest cell-centred estimate ----
         rho, pr = p0[0], p0[4]

@@ -197,6 +197,24 @@ def test_pressure_floor_matches_the_oracle(idfx, R):
     assert sim0.floor_count() == 0 and float(sim0.get_state()[0][4].min()) < floor
 
 
+def test_floor_count_does_not_depend_on_the_batch_size(idfx, monkeypatch):
+    """Cycles enqueued past t_end (IDFX_ADVANCE_BATCH=16 forces them) meet the already floored cells again: they must not
+    be floored or counted a second time, so the count is the same as with batches that do not overshoot."""
+    n, floor = 32, 0.03
+    prim, b = inputs.orszag_tang_3d(n)
+    counts, states = [], []
+    for batch in (None, "16"):
+        if batch:
+            monkeypatch.setenv("IDFX_ADVANCE_BATCH", batch)
+        sim = idfx.Idfx(n, n, n, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT, pressure_floor=floor)
+        sim.set_state(prim.contiguous().cuda(), b.contiguous().cuda())
+        sim.advance_to(0.25, 0.3)
+        counts.append(sim.floor_count())
+        states.append(sim.get_conserved()[0].clone())
+    assert counts[0] == counts[1] > 100, counts
+    assert torch.equal(states[0], states[1])
+
+
 def test_sedov_blast_parity_and_radius(idfx, R):
     """The paper's Cartesian Sedov test (HLL + PLM + RK2, periodic): parity with the oracle at 32^3, and at
     128^3 the shock radius against the self-similar solution r = 1.152 (E t^2 / rho)^(1/5)."""

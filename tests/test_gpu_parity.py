@@ -114,6 +114,35 @@ def test_every_scheme_combination_ragged_box(idfx, R, solver, limiter, emf):
     assert ref.roe_fallbacks() == 0
 
 
+# Thin boxes that are long in ONE direction: the whole oracle runs on them in a second, and the long direction crosses
+# every kind of seam of the launch configuration used at 512^3 -- the 31-cell x tiles of the one-kernel stages (nx = 385 =
+# 12 x 31 + 13 and nx = 400 end in a partial tile, nx = 512 is the headline row length), their 11-row (MHD) / 7-row (HD) y
+# tiles, their z chunks (nz = 100: several chunks of >= 16 planes per CTA) and the 32 x 4 x 8 tiles of k_ct_update.
+THIN_BOXES = [(400, 12, 10), (385, 12, 10), (512, 12, 10), (10, 130, 12), (12, 10, 100), (70, 30, 40)]
+THIN_SCHEMES = [(HLLD, VANLEER, EMF_UCT), (ROE, VANLEER, EMF_UCT), (HLL, VANLEER, EMF_UCT), (HLLD, MINMOD, EMF_ARITH),
+                (HLLC, VANLEER, EMF_NONE)]
+
+
+@pytest.mark.parametrize("solver,limiter,emf", THIN_SCHEMES)
+@pytest.mark.parametrize("shape", THIN_BOXES)
+def test_tile_and_chunk_seams_on_thin_boxes(idfx, R, shape, solver, limiter, emf):
+    nx, ny, nz = shape
+    prim, b, dx = smooth_ic(nx, ny, nz, 23, emf != EMF_NONE)
+    if b is not None:
+        # smooth_ic differentiates its potential with dx = 1 / (longest side): across the short sides of a thin box the
+        # field would be (longest / shortest) times stronger (beta << 1); scale the varying part back
+        mean = np.array([0.4, -0.3, 0.2]).reshape(3, 1, 1, 1)
+        b = mean + (b - mean) * (min(shape) / max(shape))
+    sim, ref = make_pair(idfx, R, nx, ny, nz, dx, 5.0 / 3.0, solver, limiter, emf, prim, b)
+    for s in range(4):
+        sim.advance(1, 0.4)
+        ref.advance(1, 0.4)
+        assert abs(sim.last_dt() - ref.last_dt()) <= TOL_DT * ref.last_dt(), "dt of cycle %d" % s
+        assert_state_close(sim, ref, TOL, "%dx%dx%d cycle %d" % (nx, ny, nz, s))
+    assert sim.status() == 0 and ref.status() == 0
+    assert float(sim.get_state()[0][4].min()) > 0.2   # a well-behaved flow: the comparison is not of two blow-ups
+
+
 def run_config(idfx, R, name, n=None, steps=None):
     prim, b, cfg = inputs.make(name, n=n)
     N = cfg["n"]
