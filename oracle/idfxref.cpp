@@ -600,7 +600,11 @@ struct Ctx {
   Arr A[3], A0[3], As[3], Bref[3];  // CT_POTENTIAL: edge potential accumulated since set_state (same places as E),
                                     // its saved and scratch copies, and the face field given to set_state (G19)
   double t;                         // time since set_state
-  int outflow;                      // 0: periodic; 1: zero-gradient ghosts on all six sides (HD only)
+  int outflow;                      // 0: periodic; 1: zero-gradient ghosts on all six sides.  With a
+                                    // magnetic field (reading G23) the staggered components are zero-gradient too: every ghost
+                                    // face copies the nearest active face of its line, the upper boundary face (index n, not
+                                    // part of the state) included; it is not evolved, and div B is kept on the cells whose six
+                                    // faces all belong to the state
   double pfloor;                    // optional pressure floor (0 = none, G13); see compute_prims
   long long nfloor;                 // how often it acted since set_state
   double last_dt;
@@ -1028,11 +1032,14 @@ IDFXREF_API int idfxref_set_option(idfxref_ctx* h, int option, int value) {
     c.nstages = value;
     return OK;
   }
-  if (option == OPT_BOUNDARY && (value == 0 || (value == 1 && !c.mhd))) {
+  if (option == OPT_BOUNDARY && (value == 0 || value == 1)) {
+    // with a magnetic field: face CT, three-cell reconstructions and the face-flux EMFs only (the 2D-HLL EMF and PPM reach
+    // further into the ghost zones, the vector potential has no zero-gradient form)
+    if (value == 1 && c.mhd && (c.emf == EMF_UCT_HLL || c.limiter == LIM_PPM || c.ct_form == CT_POTENTIAL)) return ERR_UNSUPPORTED;
     c.outflow = value;
     return OK;
   }
-  if (option == OPT_CT_FORM && (value == CT_FACE || (value == CT_POTENTIAL && c.mhd))) {
+  if (option == OPT_CT_FORM && (value == CT_FACE || (value == CT_POTENTIAL && c.mhd && !c.outflow))) {
     c.ct_form = value;
     if (value == CT_POTENTIAL)
       for (int d = 0; d < 3; ++d) {

@@ -116,7 +116,7 @@ class Oracle:
         if pressure_floor and self.L.idfxref_set_option_real(self.h, OPT_PRESSURE_FLOOR, pressure_floor) != OK:
             raise ValueError("bad pressure floor")
         if boundary != BOUNDARY_PERIODIC and self.L.idfxref_set_option(self.h, OPT_BOUNDARY, boundary) != OK:
-            raise ValueError("bad boundary (outflow is HD-only)")
+            raise ValueError("bad boundary (with a magnetic field: outflow needs face CT, no PPM, no 2D-HLL EMF)")
 
     def close(self):
         if self.h:
