@@ -16,9 +16,10 @@ from concurrent.futures import ThreadPoolExecutor
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _OBJ = os.path.join(_HERE, "build")
-SOURCES = [os.path.join(_CSRC, f) for f in ("idfx.cu", "probe.cu", "stage_inst.cu")]
+SOURCES = [os.path.join(_CSRC, f) for f in ("idfx.cu", "probe.cu", "stage_inst.cu", "noalloc.cu")]
 HEADERS = sorted(os.path.join(_CSRC, f) for f in os.listdir(_CSRC) if f.endswith(".cuh")) + [
-    os.path.join(os.path.dirname(_HERE), "include", "idfx.h"), os.path.join(os.path.dirname(_HERE), "include", "idfx_probe.h")]
+    os.path.join(os.path.dirname(_HERE), "include", "idfx.h"), os.path.join(os.path.dirname(_HERE), "include", "idfx_probe.h"),
+    os.path.join(os.path.dirname(_HERE), "include", "idfx_noalloc.h")]
 LIB = os.path.join(_HERE, "libidfx.so")
 
 # --register-usage-level=3 (default 5): ptxas keeps the fused CT/update kernel at 64 registers without its 16-32 B of spills
@@ -37,6 +38,7 @@ def _units(obj_dir):
             units.append((os.path.join(obj_dir, "stage_%d_%d.o" % (s, l)),
                           ["-DIDFX_INST_SOLVER=%d" % s, "-DIDFX_INST_LIM=%d" % l, "-c", SOURCES[2]]))
     units.append((os.path.join(obj_dir, "probe.o"), ["-c", SOURCES[1]]))
+    units.append((os.path.join(obj_dir, "noalloc.o"), ["-c", SOURCES[3]]))
     return units
 
 

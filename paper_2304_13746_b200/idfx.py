@@ -28,6 +28,7 @@ SYMBOLS = (
     "idfx_profile_enable", "idfx_profile_read", "idfx_profile_kernel_name",
     "idfx_set_option", "idfx_advance_to", "idfx_time", "idfx_get_potential", "idfx_set_option_real", "idfx_floor_count",
     "idfx_probe_fp64",
+    "idfx_noalloc_compute_dt", "idfx_noalloc_last_error",
 )
 
 _lib = None
@@ -73,6 +74,8 @@ def lib():
         L.idfx_profile_kernel_name.argtypes = [ci]
         L.idfx_profile_kernel_name.restype = ctypes.c_char_p
         L.idfx_probe_fp64.argtypes = [vp, ci, dp, dp]
+        L.idfx_noalloc_compute_dt.argtypes = [ci, ci, ci, cd, cd, ci, vp, vp, cd, vp, vp]
+        L.idfx_noalloc_last_error.restype = ctypes.c_char_p
         L.idfx_last_error.restype = ctypes.c_char_p
         L.idfx_destroy.argtypes = [vp]
         L.idfx_destroy.restype = None
@@ -92,6 +95,29 @@ def probe_fp64(repeats=5):
     if rc != OK:
         raise IdfxError(rc, "fp64 probe failed")
     return tf.value, ti.value
+
+
+NOALLOC_MAX_CELLS = 262144   # include/idfx_noalloc.h
+
+
+def noalloc_compute_dt(prim, bface, dx, gamma, limiter, cfl, out=None):
+    """The CFL step of a periodic box given as contiguous device tensors, through the entry point that allocates nothing
+    (include/idfx_noalloc.h; at most NOALLOC_MAX_CELLS cells; calls that overlap on the GPU race on its static scratch).
+    `out`: a one-element float64 device tensor for the result (made here when None: that allocation is torch's, the
+    library call itself allocates nothing).  Enqueued on torch's current stream; returns `out` without synchronising."""
+    assert prim.is_cuda and prim.dtype == torch.float64 and prim.is_contiguous() and prim.shape[0] == 5
+    nz, ny, nx = prim.shape[1:]
+    if bface is not None:
+        assert bface.is_cuda and bface.dtype == torch.float64 and bface.is_contiguous() and tuple(bface.shape) == (3, nz, ny, nx)
+    if out is None:
+        out = torch.empty(1, dtype=torch.float64, device=prim.device)
+    with torch.cuda.device(prim.device):
+        rc = lib().idfx_noalloc_compute_dt(nx, ny, nz, dx, gamma, limiter, prim.data_ptr(),
+                                           bface.data_ptr() if bface is not None else None, cfl,
+                                           torch.cuda.current_stream(prim.device).cuda_stream, out.data_ptr())
+    if rc != OK:
+        raise IdfxError(rc, lib().idfx_noalloc_last_error().decode())
+    return out
 
 
 class Idfx:
