@@ -82,9 +82,19 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
  *     zero there (reading G19: a periodic A cannot carry a mean field).  MHD only; must be chosen BEFORE
  *     idfx_workspace_bytes / idfx_bind (it needs 12 more fields).
  *   IDFX_OPT_BOUNDARY: IDFX_BOUNDARY_PERIODIC (default) or IDFX_BOUNDARY_OUTFLOW: zero-gradient ghost cells on all six
- *     sides (the paper's non-periodic tests).  Hydrodynamics only (IDFX_ERR_UNSUPPORTED with a magnetic
- *     field: the staggered field on a boundary face needs its own treatment); set it before idfx_set_state. */
-enum { IDFX_OPT_INTEGRATOR = 0, IDFX_OPT_CT_FORM = 1, IDFX_OPT_PRESSURE_FLOOR = 2, IDFX_OPT_BOUNDARY = 3 };
+ *     sides (the paper's non-periodic tests).  With a magnetic field (reading G23) the staggered
+ *     components are zero-gradient as well: every ghost face copies the nearest face of the state along its line, the
+ *     upper boundary face (index n, not part of the state) included.  Needs a three-cell reconstruction (not PPM), a
+ *     face-flux EMF (not IDFX_EMF_UCT_HLL) and IDFX_CT_FACE (IDFX_ERR_UNSUPPORTED otherwise); set it before idfx_set_state.
+ *   IDFX_OPT_EXCHANGE_DIRS: bit d set = the ghost layers of direction d (0 = x, 1 = y, 2 = z) are the cells of a
+ *     neighbouring sub-box of a domain decomposition and arrive through idfx_halo_unpack.  The context
+ *     then never wraps periodically along d, and the CALLER drives every cycle through the staged calls below.  Same
+ *     restrictions as outflow; must be chosen BEFORE idfx_bind.
+ *   IDFX_OPT_OUTFLOW_SIDES: for a sub-box of a decomposed box with outflow boundaries: bit 2 d + side (side 0 lower,
+ *     1 upper) set = that side of the sub-box is a wall of the whole box (its ghosts are then filled with
+ *     idfx_halo_fill(d, side, 1) by the caller).  Every direction of such a run must be exchanged or walled. */
+enum { IDFX_OPT_INTEGRATOR = 0, IDFX_OPT_CT_FORM = 1, IDFX_OPT_PRESSURE_FLOOR = 2, IDFX_OPT_BOUNDARY = 3, IDFX_OPT_EXCHANGE_DIRS = 4,
+       IDFX_OPT_OUTFLOW_SIDES = 5 };
 enum { IDFX_CT_FACE = 0, IDFX_CT_POTENTIAL = 1 };
 enum { IDFX_BOUNDARY_PERIODIC = 0, IDFX_BOUNDARY_OUTFLOW = 1 };
 int idfx_set_option(idfx_ctx* ctx, int option, int value);
@@ -143,6 +153,37 @@ int idfx_time(idfx_ctx* ctx, double* h_t_out);
 /* IDFX_CT_POTENTIAL only: the edge potential accumulated since idfx_set_state, d_pot[c][k][j][i] = A_c on the lower
  * edges of cell (i,j,k): A_x at (i, j-1/2, k-1/2), A_y at (i-1/2, j, k-1/2), A_z at (i-1/2, j-1/2, k). */
 int idfx_get_potential(idfx_ctx* ctx, double* d_pot);
+
+/* ---- The cycle in pieces, for a domain decomposition over several contexts (one per GPU) -------
+ * One sub-box per context, IDFX_OPT_EXCHANGE_DIRS set.  Per cycle, identically on every sub-box:
+ *     idfx_cycle_begin(dt <= 0, cfl)
+ *     for s in 0 .. stages-1:
+ *         idfx_stage_flux(s)                  reconstruct -> Riemann -> divergence -> edge EMFs; s = 0 also reduces the
+ *                                             sub-box's max_cells sum_d c_d/dx into 8 bytes of the workspace
+ *         [s = 0: max over all sub-boxes of those 8 bytes, written back in place: Eq. 10's "entire integration volume"]
+ *         idfx_stage_update(s)                CT, RK combine, cons -> prim of the stage result (no ghost layer is written)
+ *         for d in x, y, z (this order fills edges and corners):
+ *             exchanged d:  idfx_halo_pack(d, side) on both sides -> the neighbours -> idfx_halo_unpack(d, side)
+ *             otherwise:    idfx_halo_fill(d, side, zero_gradient) on both sides
+ *     idfx_cycle_end()
+ * A slab carries the primitives (with Bc) and the face field of the stage result: idfx_halo_count(d) doubles, layout
+ * [field][z][y][x] of the two layers, spanning the ghost layers of the directions below d.  What one sub-box packs on its
+ * upper side is what its upper neighbour unpacks on its lower side.  Setting the state: idfx_set_state (copy-in only),
+ * the same ghost sequence (the face field must reach the ghosts before Bc is formed), idfx_set_state_finish, the ghost
+ * sequence again.  Every sub-box then computes bit for bit what the undecomposed box computes (tests/test_gpu_decomp.py).
+ * The staged calls also work without exchanged directions (they are what idfx_step runs).
+ * idfx_dt_reduce_offset: byte offset inside the bound workspace of the 8-byte reduction word; it holds a non-negative
+ * double, so an elementwise MAX of doubles over the sub-boxes is the reduction.  All on the bound stream, none synchronises. */
+int       idfx_cycle_begin(idfx_ctx* ctx, double dt, double cfl);   /* dt > 0: fixed step; else the CFL step */
+int       idfx_stage_flux(idfx_ctx* ctx, int stage);
+int       idfx_stage_update(idfx_ctx* ctx, int stage);
+int       idfx_cycle_end(idfx_ctx* ctx);
+size_t    idfx_dt_reduce_offset(const idfx_ctx* ctx);
+int       idfx_set_state_finish(idfx_ctx* ctx);
+long long idfx_halo_count(const idfx_ctx* ctx, int dir);
+int       idfx_halo_pack(idfx_ctx* ctx, int dir, int side, double* d_buf);          /* side 0: lower, 1: upper */
+int       idfx_halo_unpack(idfx_ctx* ctx, int dir, int side, const double* d_buf);
+int       idfx_halo_fill(idfx_ctx* ctx, int dir, int side, int zero_gradient);      /* periodic image, or the nearest layer */
 
 /* dt used by the most recent cycle (synchronises). */
 int idfx_last_dt(idfx_ctx* ctx, double* h_dt_out);

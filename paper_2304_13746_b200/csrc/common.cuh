@@ -14,7 +14,11 @@ struct Geom {
   long long np;   // padded field size in doubles
   long long nc;   // nx*ny*nz
   double dx, gamma;
-  int outflow;    // 0: periodic box; 1: zero-gradient (outflow) ghosts on all six sides (hydrodynamics only)
+  int outflow;    // bit 2 d + side set: that side (0 lower, 1 upper) of direction d is an outflow wall with zero-gradient ghosts;
+                  // 0: none (periodic box, or a sub-box inside a decomposed one); 0x3f: all six sides
+  int open;       // bit d set: the kernels do not wrap periodically along direction d -- the edge lattice keeps its plane of
+                  // index n, nobody writes periodic ghost images, and the ghost layers are filled by a separate pass
+                  // (zero-gradient copies for outflow, the neighbour's cells under a domain decomposition).  0: periodic box
   double pfloor;  // > 0: pressures below it are raised to it in cons->prim and E is rewritten (idfx_set_option_real); 0: none (G13)
   __host__ __device__ __forceinline__ long long at(int i, int j, int k) const {
     return (long long)(k + NG) * sz + (long long)(j + NG) * sy + (i + IOFF);

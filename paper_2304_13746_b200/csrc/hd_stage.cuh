@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(HD_THREADS, HD_MINB) k_hd_stage(Geom g, HdStag
         const long long gz = k < NG ? (long long)g.nz * g.sz : (k >= g.nz - NG ? -(long long)g.nz * g.sz : 0);
 #pragma unroll
         for (int n = 0; n < 5; ++n) a.Vout[n][cu] = v[n];
-        if (!g.outflow && (gx != 0 || gy != 0 || gz != 0)) {
+        if (!g.open && (gx != 0 || gy != 0 || gz != 0)) {
 #pragma unroll
           for (int m = 1; m < 8; ++m) {
             const long long off = ((m & 1) ? gx : 0) + ((m & 2) ? gy : 0) + ((m & 4) ? gz : 0);

@@ -67,6 +67,11 @@ struct idfx_ctx {
   int f_gen() const { return f_h2d() + (emf == EMF_UCT_HLL ? N_H2D : 0); }
   int nfields() const { return f_gen() + (limiter == LIM_PPM ? N_GEN : 0); }
   double* abuf(int which, int d) const { return field(f_aa() + 3 * which + d); }
+  int exch = 0;  // bit d set: the ghost layers of direction d come from a neighbouring sub-box (idfx_halo_*), the caller
+                 // drives the cycle through the staged calls
+  // the running cycle (cycle_begin .. cycle_end)
+  double cyc_dt_fixed = 0.0, cyc_cfl = 0.0;
+  int cyc_b0 = 0, cyc_bin = 0;  // saved face buffer; face buffer of the next stage's input (= bcur between cycles)
   int bcur = 0;  // which of the three face-field buffers holds the current state
   int vcur = 0;  // which primitive buffer holds the stage input
   int graph_bnext[6] = {0, 0, 0, 0, 0, 0}, graph_vnext[6] = {0, 0, 0, 0, 0, 0};  // rotation state a replayed cycle leaves

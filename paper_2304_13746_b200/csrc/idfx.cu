@@ -86,6 +86,64 @@ __global__ void k_fill_ghost(Geom g, FieldList fl) {
   for (int n = 0; n < fl.n; ++n) fl.f[n][d] = fl.f[n][s];
 }
 
+// a1 one direction and one side at a time ("sequential x -> y -> z exchange", the order that also gets
+// edges and corners right): a slab of NG layers normal to direction d that spans the active cells of the directions
+// above d and the whole padded extent of the directions below it.
+//   SLAB_COPY   ghost slab <- a slab of the same field (periodic image, or with `clamp` the nearest active layer)
+//   SLAB_PACK   the NG active layers next to the side -> a contiguous buffer [field][z][y][x of the slab]
+//   SLAB_UNPACK a contiguous buffer -> the ghost slab of that side
+// Under a domain decomposition the buffer packed on one rank's upper side is unpacked on its upper neighbour's lower side.
+enum { SLAB_COPY = 0, SLAB_PACK = 1, SLAB_UNPACK = 2 };
+
+struct SlabGeom {
+  int lo[3], ext[3];  // first index and extent of the slab in x, y, z (ext[d] = NG)
+  int d, src0, clamp; // SLAB_COPY: first source layer along d, or the one layer every ghost layer copies
+  long long count;    // cells of the slab
+};
+
+inline SlabGeom slab_geom(const Geom& g, int d, int side, int mode, int clamp) {
+  SlabGeom s;
+  const int n[3] = {g.nx, g.ny, g.nz};
+  for (int q = 0; q < 3; ++q) {
+    s.lo[q] = q < d ? -NG : 0;
+    s.ext[q] = q < d ? n[q] + 2 * NG : n[q];
+  }
+  s.ext[d] = NG;
+  s.d = d;
+  s.clamp = clamp;
+  if (mode == SLAB_PACK) {
+    s.lo[d] = side ? n[d] - NG : 0;
+    s.src0 = 0;
+  } else {
+    s.lo[d] = side ? n[d] : -NG;
+    s.src0 = clamp ? (side ? n[d] - 1 : 0) : (side ? 0 : n[d] - NG);
+  }
+  s.count = (long long)s.ext[0] * s.ext[1] * s.ext[2];
+  return s;
+}
+
+template <int MODE>
+__global__ void k_slab(Geom g, SlabGeom sg, FieldList fl, double* __restrict__ buf) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= sg.count) return;
+  int l[3];
+  l[0] = (int)(t % sg.ext[0]);
+  const long long r = t / sg.ext[0];
+  l[1] = (int)(r % sg.ext[1]);
+  l[2] = (int)(r / sg.ext[1]);
+  int idx[3] = {sg.lo[0] + l[0], sg.lo[1] + l[1], sg.lo[2] + l[2]};
+  const long long cell = g.at(idx[0], idx[1], idx[2]);
+  if (MODE == SLAB_COPY) {
+    idx[sg.d] = sg.clamp ? sg.src0 : sg.src0 + l[sg.d];
+    const long long src = g.at(idx[0], idx[1], idx[2]);
+    for (int n = 0; n < fl.n; ++n) fl.f[n][cell] = fl.f[n][src];
+  } else if (MODE == SLAB_PACK) {
+    for (int n = 0; n < fl.n; ++n) buf[n * sg.count + t] = fl.f[n][cell];
+  } else {
+    for (int n = 0; n < fl.n; ++n) fl.f[n][cell] = buf[n * sg.count + t];
+  }
+}
+
 // ---------------------------------------------------------------------------------------------
 // a2: cell-centred B and cons <-> prim
 // ---------------------------------------------------------------------------------------------
@@ -104,10 +162,11 @@ __global__ void k_cons_from_prim(Geom g, StateArgs a) {
   const long long c = g.at(i, j, k);
   double bx = 0.0, by = 0.0, bz = 0.0;
   if (MHD) {
-    // right faces through the periodic image (face ghosts are not filled yet)
-    bx = 0.5 * (a.Bf[0][c] + a.Bf[0][g.at(i + 1 == g.nx ? 0 : i + 1, j, k)]);
-    by = 0.5 * (a.Bf[1][c] + a.Bf[1][g.at(i, j + 1 == g.ny ? 0 : j + 1, k)]);
-    bz = 0.5 * (a.Bf[2][c] + a.Bf[2][g.at(i, j, k + 1 == g.nz ? 0 : k + 1)]);
+    // right faces through the periodic image (face ghosts are not filled yet); along an open direction the ghost face,
+    // which is filled before this kernel runs
+    bx = 0.5 * (a.Bf[0][c] + a.Bf[0][g.at(i + 1 == g.nx && !(g.open & 1) ? 0 : i + 1, j, k)]);
+    by = 0.5 * (a.Bf[1][c] + a.Bf[1][g.at(i, j + 1 == g.ny && !(g.open & 2) ? 0 : j + 1, k)]);
+    bz = 0.5 * (a.Bf[2][c] + a.Bf[2][g.at(i, j, k + 1 == g.nz && !(g.open & 4) ? 0 : k + 1)]);
     a.V[5][c] = bx;
     a.V[6][c] = by;
     a.V[7][c] = bz;
@@ -568,8 +627,8 @@ __global__ void __launch_bounds__(CT_THREADS, CT_MINB) k_ct_update(Geom g, EmfAr
     const int li = p % CT_LX, lj = (p / CT_LX) % CT_LY, lk = p / (CT_LX * CT_LY);
     const int I = i0 + li, J = j0 + lj, K = k0 + lk;
     if (I > g.nx || J > g.ny || K > g.nz) continue;
-    // periodic image of lattice index n is index 0
-    const int idx[3] = {I == g.nx ? 0 : I, J == g.ny ? 0 : J, K == g.nz ? 0 : K};
+    // periodic image of lattice index n is index 0; along an open direction the lattice keeps its own plane n
+    const int idx[3] = {I == g.nx && !(g.open & 1) ? 0 : I, J == g.ny && !(g.open & 2) ? 0 : J, K == g.nz && !(g.open & 4) ? 0 : K};
     const bool on[3] = {li < CT_TX, lj < CT_TY, lk < CT_TZ};
     const bool owned = on[0] && on[1] && on[2] && I < g.nx && J < g.ny && K < g.nz;
     const long long P = g.at(idx[0], idx[1], idx[2]);
@@ -592,9 +651,10 @@ __global__ void __launch_bounds__(CT_THREADS, CT_MINB) k_ct_update(Geom g, EmfAr
   if (i >= g.nx || j >= g.ny) return;
   const double dtdx = dt / g.dx;
   const long long st[3] = {1, g.sy, g.sz};
-  // ghost images of this column in x and y
-  const long long gx = i < NG ? (long long)g.nx : (i >= g.nx - NG ? -(long long)g.nx : 0);
-  const long long gy = j < NG ? (long long)g.ny * g.sy : (j >= g.ny - NG ? -(long long)g.ny * g.sy : 0);
+  // ghost images of this column in x and y (none with an open side: a fill pass follows then)
+  const long long gx = g.open ? 0 : (i < NG ? (long long)g.nx : (i >= g.nx - NG ? -(long long)g.nx : 0));
+  const long long gy = g.open ? 0 : (j < NG ? (long long)g.ny * g.sy : (j >= g.ny - NG ? -(long long)g.ny * g.sy : 0));
+  const int nd[3] = {g.nx, g.ny, g.nz};
 #pragma unroll
   for (int lkk = 0; lkk < CT_TZ / CT_ZSPLIT; ++lkk) {
     const int lk = lz * (CT_TZ / CT_ZSPLIT) + lkk;
@@ -644,10 +704,12 @@ __global__ void __launch_bounds__(CT_THREADS, CT_MINB) k_ct_update(Geom g, EmfAr
           br = idle ? b0r : a.w0 * b0r + a.w * br;
         }
       }
+      // outflow (G23): the upper boundary face is not part of the state, it copies the last active face
+      if (((g.outflow >> (2 * d + 1)) & 1) && (d == 0 ? i : (d == 1 ? j : k)) == nd[d] - 1) br = bl;
       v[5 + d] = 0.5 * (bl + br);
       a.Bout[d][c] = bl;
       // images of the new face value
-      const long long gz = k < NG ? (long long)g.nz * g.sz : (k >= g.nz - NG ? -(long long)g.nz * g.sz : 0);
+      const long long gz = g.open ? 0 : (k < NG ? (long long)g.nz * g.sz : (k >= g.nz - NG ? -(long long)g.nz * g.sz : 0));
 #pragma unroll
       for (int m = 1; m < 8; ++m) {
         const long long off = ((m & 1) ? gx : 0) + ((m & 2) ? gy : 0) + ((m & 4) ? gz : 0);
@@ -662,7 +724,7 @@ __global__ void __launch_bounds__(CT_THREADS, CT_MINB) k_ct_update(Geom g, EmfAr
     v[9] = v[1] * v[7] - v[3] * v[5];
     v[10] = v[2] * v[5] - v[1] * v[6];
     if (!(u[0] > 0.0) || !(v[4] > 0.0)) a.sc->flag = 1;
-    const long long gz = k < NG ? (long long)g.nz * g.sz : (k >= g.nz - NG ? -(long long)g.nz * g.sz : 0);
+    const long long gz = g.open ? 0 : (k < NG ? (long long)g.nz * g.sz : (k >= g.nz - NG ? -(long long)g.nz * g.sz : 0));
     const bool want_ec = a.V[8] != nullptr;  // only the separate sweeps read the reference EMF back
 #pragma unroll
     for (int n = 0; n < 11; ++n)
@@ -1070,7 +1132,9 @@ void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int
   MhdStageArgs a;
   a.fV0 = c->vcur ? 11 : 0;
   a.fB0 = 3 * bin;
-  const long long per_chunk = (long long)((g.nx + MS_CX - 1) / MS_CX) * ((g.ny + MS_CY - 1) / MS_CY);
+  // along an open direction the tiles start at cell -1 (mhd_stage.cuh)
+  const int tx = (g.nx + (g.open & 1) + MS_CX - 1) / MS_CX, ty = (g.ny + ((g.open >> 1) & 1) + MS_CY - 1) / MS_CY;
+  const long long per_chunk = (long long)tx * ty;
   long long nch = (148 * 24 + per_chunk - 1) / per_chunk;  // about 24 waves of one CTA per SM: a short last wave
   const long long maxch = g.nz / 16 > 0 ? g.nz / 16 : 1;
   nch = nch < 1 ? 1 : (nch > maxch ? maxch : nch);
@@ -1086,100 +1150,133 @@ void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int
   a.sc = c->sc;
   a.w = w;
   a.w0 = w0;
-  dim3 grid((g.nx + MS_CX - 1) / MS_CX, (g.ny + MS_CY - 1) / MS_CY, (unsigned)((g.nz + a.chunk - 1) / a.chunk));
+  dim3 grid(tx, ty, (unsigned)((g.nz + a.chunk - 1) / a.chunk));
   LaunchScope ls(c, K_MHD);
   mhd_kernel(c, first, c->emf == EMF_UCT_HLL ? EMF_ARITH : c->emf)<<<grid, MS_THREADS, MS_SMEM_BYTES, c->stream>>>(g, a, c->mapMV,
                                                                                                                  c->mapMB);
 }
 
-// One stage S_dt (O2) followed by the RK combine of Eq. 9.  s: stage index (0-based); bin: face buffer of the stage
-// input; b0: saved face buffer; bout: destination.  Conserved fields: U_0 lives in F_UA for the whole cycle, the
-// intermediate stages in F_UB, the last stage writes the result back to F_UA.
-void run_stage(idfx_ctx* c, int s, int bin, int b0, int bout, double dt_fixed, double cfl, bool want_dt) {
+// ---- one cycle, in pieces: cycle_begin, then per stage stage_flux -> stage_update (-> ghost fill), then cycle_end.
+// idfx_step / idfx_advance run them back to back (run_cycle); a domain-decomposed run drives them through the staged ABI
+// with its halo exchange and the reduction of dt in between.
+// Conserved fields: U_0 lives in F_UA for the whole cycle, the intermediate stages in F_UB, the last stage writes the
+// result back to F_UA.  Face field: three buffers rotate, never writing the saved one (b0) nor the stage input.
+struct StagePlan {
+  bool combine, last;
+  int uin, uout, bin, b0, bout;
+  double w, w0;
+};
+
+StagePlan plan_stage(const idfx_ctx* c, int s) {
   static const double W[3][3] = {{1.0, 0.0, 0.0}, {1.0, 0.5, 0.0}, {1.0, 0.25, 2.0 / 3.0}};      // Tab. 1
   static const double W0[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.5, 0.0}, {0.0, 0.75, 1.0 / 3.0}};
-  const bool combine = s > 0, last = s == c->nstages - 1;
-  const int uin = s == 0 ? F_UA : F_UB, uout = last ? F_UA : F_UB;
-  const double w = W[c->nstages - 1][s], w0 = W0[c->nstages - 1][s];
-  const double* Bf[3] = {c->bbuf(bin, 0), c->bbuf(bin, 1), c->bbuf(bin, 2)};
-  if (!c->fused) {  // PPM: generic face-flux kernels, divergence and dt in k_rhs
-    launch_ppm(c, Bf, want_dt);
-  } else if (c->mhd) {
-    launch_mhd_stage(c, !combine, w, w0, uin, uout, bin);
-  } else {
-    launch_hd_stage(c, !combine, w, w0, uin, uout);
-    if (combine) {  // the kernel wrote U_s, its primitives and their ghost images into the other primitive buffer
-      c->vcur ^= 1;
-      if (c->g.outflow) launch_fill(c, bout);  // it writes periodic images only
-      return;
-    }
+  StagePlan p;
+  p.combine = s > 0;
+  p.last = s == c->nstages - 1;
+  p.uin = s == 0 ? F_UA : F_UB;
+  p.uout = p.last ? F_UA : F_UB;
+  p.w = W[c->nstages - 1][s];
+  p.w0 = W0[c->nstages - 1][s];
+  p.b0 = c->cyc_b0;
+  p.bin = c->cyc_bin;
+  const int b1 = (p.b0 + 1) % 3, b2 = (p.b0 + 2) % 3;
+  p.bout = p.bin == b1 ? b2 : b1;
+  return p;
+}
+
+// dt_fixed > 0: that dt; otherwise dt = cfl / max found by stage 1, shortened to land on t_end (never leaves the device)
+void cycle_begin(idfx_ctx* c, double dt_fixed, double cfl) {
+  c->cyc_dt_fixed = dt_fixed;
+  c->cyc_cfl = cfl;
+  c->cyc_b0 = c->cyc_bin = c->bcur;
+  LaunchScope ls(c, K_STATE);
+  k_cycle_begin<<<1, 32, 0, c->stream>>>(c->sc);
+}
+
+// a3 - a6 of stage s: reconstruct -> Riemann -> flux divergence (-> edge EMFs); stage 0 also reduces max sum_d c_d / dx
+void stage_flux(idfx_ctx* c, int s) {
+  const StagePlan p = plan_stage(c, s);
+  const double* Bf[3] = {c->bbuf(p.bin, 0), c->bbuf(p.bin, 1), c->bbuf(p.bin, 2)};
+  if (!c->fused) launch_ppm(c, Bf, s == 0 && !(c->cyc_dt_fixed > 0.0));  // PPM: generic face-flux kernels, divergence and dt in k_rhs
+  else if (c->mhd) launch_mhd_stage(c, !p.combine, p.w, p.w0, p.uin, p.uout, p.bin);
+  else launch_hd_stage(c, !p.combine, p.w, p.w0, p.uin, p.uout);
+}
+
+// a7, a8, a2 of stage s (and the ghost images or the local ghost fill a1 of its result); rotates the buffers
+void stage_update(idfx_ctx* c, int s) {
+  const StagePlan p = plan_stage(c, s);
+  const Geom& g = c->g;
+  c->cyc_bin = p.bout;
+  if (c->fused && !c->mhd && p.combine) {
+    // the HD stage kernel wrote U_s, its primitives and (periodic box) their ghost images into the other primitive buffer
+    c->vcur ^= 1;
+    if (g.open && !c->exch) launch_fill(c, p.bout);
+    return;
   }
   UpdateArgs a;
   for (int n = 0; n < 5; ++n) {
-    a.Uin[n] = c->field(uin + n);
+    a.Uin[n] = c->field(p.uin + n);
     a.U0[n] = c->field(F_UA + n);
     a.R[n] = c->field(F_R + n);
-    a.Uout[n] = c->field(uout + n);
+    a.Uout[n] = c->field(p.uout + n);
   }
   for (int d = 0; d < 3; ++d) {
-    a.Bin[d] = c->bbuf(bin, d);
-    a.B0[d] = c->bbuf(b0, d);
-    a.Bout[d] = c->bbuf(bout, d);
-    a.Ain[d] = c->vp ? c->abuf(bin, d) : nullptr;
-    a.A0[d] = c->vp ? c->abuf(b0, d) : nullptr;
-    a.Aout[d] = c->vp ? c->abuf(bout, d) : nullptr;
+    a.Bin[d] = c->bbuf(p.bin, d);
+    a.B0[d] = c->bbuf(p.b0, d);
+    a.Bout[d] = c->bbuf(p.bout, d);
+    a.Ain[d] = c->vp ? c->abuf(p.bin, d) : nullptr;
+    a.A0[d] = c->vp ? c->abuf(p.b0, d) : nullptr;
+    a.Aout[d] = c->vp ? c->abuf(p.bout, d) : nullptr;
     a.Bref[d] = c->vp ? c->field(c->f_bref() + d) : nullptr;
   }
   a.sc = c->sc;
-  a.dt_fixed = dt_fixed;
-  a.cfl = cfl;
-  a.w = w;
-  a.w0 = w0;
+  a.dt_fixed = c->cyc_dt_fixed;
+  a.cfl = c->cyc_cfl;
+  a.w = p.w;
+  a.w0 = p.w0;
   a.store_u = !(s == 0 && rk2_keeps_no_u1(c));
-  const Geom& g = c->g;
   if (c->mhd) {
-    // edge EMFs + CT + RK combine + cons->prim + ghost images in one kernel; V is double-buffered because the
-    // EMFs of neighbouring tiles still read the stage-input primitives while this tile writes the result's
+    // CT + RK combine + cons->prim + ghost images in one kernel; V is double-buffered because neighbouring tiles still
+    // read the stage-input primitives while this tile writes the result's
     const EmfArgs ea = emf_args(c);
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield_out(n);
     if (c->fused)  // the one-kernel stage forms -(v x Bc) itself
       for (int n = 8; n < 11; ++n) a.V[n] = nullptr;
     dim3 grid((g.nx + CT_TX - 1) / CT_TX, (g.ny + CT_TY - 1) / CT_TY, (g.nz + CT_TZ - 1) / CT_TZ);
-    const bool udone = combine && c->fused;  // the one-kernel stage applied the divergence itself
-    if (c->emf == EMF_UCT_HLL) launch_hll2d(c, Bf);
-    LaunchScope ls(c, K_UPDATE);
-    if (c->fused || c->emf == EMF_UCT_HLL) launch_ct<EMF_UCT_HLL>(c, grid, ea, a, combine, udone);  // lattice read from memory
-    else if (c->emf == EMF_UCT) launch_ct<EMF_UCT>(c, grid, ea, a, combine, udone);
-    else if (c->emf == EMF_UCT0) launch_ct<EMF_UCT0>(c, grid, ea, a, combine, udone);
-    else launch_ct<EMF_ARITH>(c, grid, ea, a, combine, udone);
+    const bool udone = p.combine && c->fused;  // the one-kernel stage applied the divergence itself
+    if (c->emf == EMF_UCT_HLL) {
+      const double* Bf[3] = {c->bbuf(p.bin, 0), c->bbuf(p.bin, 1), c->bbuf(p.bin, 2)};
+      launch_hll2d(c, Bf);
+    }
+    {
+      LaunchScope ls(c, K_UPDATE);
+      if (c->fused || c->emf == EMF_UCT_HLL) launch_ct<EMF_UCT_HLL>(c, grid, ea, a, p.combine, udone);  // lattice read from memory
+      else if (c->emf == EMF_UCT) launch_ct<EMF_UCT>(c, grid, ea, a, p.combine, udone);
+      else if (c->emf == EMF_UCT0) launch_ct<EMF_UCT0>(c, grid, ea, a, p.combine, udone);
+      else launch_ct<EMF_ARITH>(c, grid, ea, a, p.combine, udone);
+    }
     c->vcur ^= 1;
+    if (g.open && !c->exch) launch_fill(c, p.bout);  // no images were written
   } else {
     for (int n = 0; n < 11; ++n) a.V[n] = c->vfield(n);
     {
       LaunchScope ls(c, K_UPDATE);
-      if (combine) k_update_hd<true><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
+      if (p.combine) k_update_hd<true><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
       else k_update_hd<false><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
     }
-    launch_fill(c, bout);
+    if (!c->exch) launch_fill(c, p.bout);
   }
 }
 
-// One cycle of the integrator.  dt_fixed > 0: that dt; otherwise dt = cfl / max found by stage 1, shortened to land on
-// t_end (never leaves the device).
+void cycle_end(idfx_ctx* c) { c->bcur = c->cyc_bin; }
+
 int run_cycle(idfx_ctx* c, double dt_fixed, double cfl) {
-  const bool want_dt = !(dt_fixed > 0.0);
-  {
-    LaunchScope ls(c, K_STATE);
-    k_cycle_begin<<<1, 32, 0, c->stream>>>(c->sc);
-  }
-  const int b0 = c->bcur, b1 = (c->bcur + 1) % 3, b2 = (c->bcur + 2) % 3;
-  int bin = b0;
+  cycle_begin(c, dt_fixed, cfl);
   for (int s = 0; s < c->nstages; ++s) {
-    const int bout = bin == b1 ? b2 : b1;  // never b0 (saved) and never the stage input
-    run_stage(c, s, bin, b0, bout, dt_fixed, cfl, want_dt && s == 0);
-    bin = bout;
+    stage_flux(c, s);
+    stage_update(c, s);
   }
-  c->bcur = bin;
+  cycle_end(c);
   CK(cudaGetLastError());
   return IDFX_OK;
 }
@@ -1221,11 +1318,15 @@ int finish_set_state(idfx_ctx* c) {
   for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
   a.sc = c->sc;
   const unsigned nb = blocks_for(c->g.nc, 128);
+  // open sides: Bc of the last cell needs the ghost face beyond it (its caller has filled the face ghosts when they come
+  // from a neighbour; zero-gradient ones are filled here)
+  if (c->mhd && c->g.open && !c->exch) launch_fill(c, c->bcur);
   { LaunchScope ls(c, K_STATE);
   if (c->mhd) k_cons_from_prim<true><<<nb, 128, 0, c->stream>>>(c->g, a);
   else k_cons_from_prim<false><<<nb, 128, 0, c->stream>>>(c->g, a);
   }
-  launch_fill(c, c->bcur);
+  c->cyc_bin = c->bcur;
+  if (!c->exch) launch_fill(c, c->bcur);
   CK(cudaGetLastError());
   if (c->vp) {  // G19: the potential is counted from this state on
     const size_t fb = (size_t)c->g.np * sizeof(double);
@@ -1292,6 +1393,7 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
   g.gamma = gamma;
   g.pfloor = 0.0;
   g.outflow = 0;
+  g.open = 0;
   g.sy = ((nx + IOFF + NG + 15) / 16) * 16;
   g.sz = (long long)g.sy * (ny + 2 * NG);
   g.np = ((g.sz * (nz + 2 * NG) + 31) / 32) * 32;
@@ -1379,6 +1481,19 @@ int idfx_set_state(idfx_ctx* c, const double* d_prim, const double* d_bface) {
     k_pack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_bface);
     }
   }
+  c->cyc_bin = c->bcur;
+  if (c->exch) return IDFX_OK;  // the caller exchanges the face ghosts, then calls idfx_set_state_finish
+  return finish_set_state(c);
+}
+
+int idfx_set_state_finish(idfx_ctx* c) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  DeviceScope on_device(c->device);
+  if (!c->exch) {
+    set_err("idfx_set_state_finish: only with exchanged directions (idfx_set_state is complete otherwise)");
+    return IDFX_ERR_INVALID_ARG;
+  }
   return finish_set_state(c);
 }
 
@@ -1396,7 +1511,8 @@ int idfx_set_state_host(idfx_ctx* c, const double* h_prim, const double* h_bface
     for (int d = 0; d < 3; ++d)
       if ((rc = copy3d(c, c->bbuf(c->bcur, d), h_bface + (size_t)d * c->g.nc, nullptr, cudaMemcpyHostToDevice)))
         return rc;
-  if ((rc = finish_set_state(c))) return rc;
+  c->cyc_bin = c->bcur;
+  if (!c->exch && (rc = finish_set_state(c))) return rc;
   CK(cudaStreamSynchronize(c->stream));  // the caller may reuse its host buffers as soon as this returns
   return IDFX_OK;
 }
@@ -1482,9 +1598,16 @@ int idfx_compute_dt(idfx_ctx* c, double cfl, double* h_dt_out) {
     return IDFX_ERR_INVALID_ARG;
   }
   CK(cudaMemsetAsync(&c->sc->smax_bits, 0, sizeof(unsigned long long), c->stream));
-  const double* Bf[3] = {c->bbuf(c->bcur, 0), c->bbuf(c->bcur, 1), c->bbuf(c->bcur, 2)};
-  for (int d = 0; d < 3; ++d) launch_speed(c, d, Bf);
-  launch_dtmax(c);
+  if (c->fused) {
+    // the first-stage kernel itself, run for its reduction only (its divergence and EMFs land in scratch that is dead
+    // between cycles): the same arithmetic, tile for tile, as the dt a cycle would take, on any kind of boundary
+    if (c->mhd) launch_mhd_stage(c, true, 1.0, 0.0, F_UA, F_UB, c->bcur);
+    else launch_hd_stage(c, true, 1.0, 0.0, F_UA, F_UB);
+  } else {
+    const double* Bf[3] = {c->bbuf(c->bcur, 0), c->bbuf(c->bcur, 1), c->bbuf(c->bcur, 2)};
+    for (int d = 0; d < 3; ++d) launch_speed(c, d, Bf);
+    launch_dtmax(c);
+  }
   CK(cudaGetLastError());
   unsigned long long bits = 0;
   CK(cudaMemcpyAsync(&bits, &c->sc->smax_bits, sizeof(bits), cudaMemcpyDeviceToHost, c->stream));
@@ -1503,12 +1626,20 @@ int idfx_step(idfx_ctx* c, double dt) {
     set_err("idfx_step: dt must be > 0");
     return IDFX_ERR_INVALID_ARG;
   }
+  if (c->exch) {
+    set_err("idfx_step: with exchanged directions the cycle is driven through idfx_cycle_begin / idfx_stage_* / idfx_halo_*");
+    return IDFX_ERR_UNSUPPORTED;
+  }
   return run_cycle(c, dt, 0.0);
 }
 
 // nsteps cycles with the CFL step, replayed from CUDA graphs where possible
 static int advance_cycles(idfx_ctx* c, int nsteps, double cfl) {
   int rc;
+  if (c->exch) {
+    set_err("idfx_advance: with exchanged directions the cycle is driven through idfx_cycle_begin / idfx_stage_* / idfx_halo_*");
+    return IDFX_ERR_UNSUPPORTED;
+  }
   if (c->graph_cfl != cfl) {
     drop_graphs(c);
     c->graph_cfl = cfl;
@@ -1622,16 +1753,35 @@ int idfx_set_option(idfx_ctx* c, int option, int value) {
     return IDFX_OK;
   }
   if (option == 3 /* IDFX_OPT_BOUNDARY */ && (value == 0 || value == 1)) {
-    if (value == 1 && c->mhd) {
-      set_err("idfx_set_option: outflow boundaries are implemented for hydrodynamics only");
+    if (value == 1 && (c->limiter == LIM_PPM || c->emf == EMF_UCT_HLL || c->vp)) {
+      set_err("idfx_set_option: outflow boundaries need a three-cell reconstruction, a face-flux EMF and the face form of CT");
       return IDFX_ERR_UNSUPPORTED;
     }
-    if (value == 1 && c->limiter == LIM_PPM) {
-      set_err("idfx_set_option: PPM is implemented for periodic boxes only");
-      return IDFX_ERR_UNSUPPORTED;
+    drop_graphs(c);
+    c->g.outflow = value ? 0x3f : 0;
+    c->g.open = (value ? 7 : 0) | c->exch;
+    return IDFX_OK;
+  }
+  if (option == 5 /* IDFX_OPT_OUTFLOW_SIDES */ && value >= 0 && value <= 0x3f) {
+    if (!c->exch) {
+      set_err("idfx_set_option: per-side walls are for sub-boxes of a decomposed box (IDFX_OPT_EXCHANGE_DIRS first)");
+      return IDFX_ERR_INVALID_ARG;
     }
-    if (value != c->g.outflow) drop_graphs(c);
+    drop_graphs(c);
     c->g.outflow = value;
+    return IDFX_OK;
+  }
+  if (option == 4 /* IDFX_OPT_EXCHANGE_DIRS */ && value >= 0 && value <= 7) {
+    if (c->bound) {
+      set_err("idfx_set_option: the exchanged directions must be chosen before idfx_bind");
+      return IDFX_ERR_INVALID_ARG;
+    }
+    if (value && (c->limiter == LIM_PPM || c->emf == EMF_UCT_HLL || c->vp)) {
+      set_err("idfx_set_option: halo exchange needs a three-cell reconstruction, a face-flux EMF and the face form of CT");
+      return IDFX_ERR_UNSUPPORTED;
+    }
+    c->exch = value;
+    c->g.open = (c->g.outflow ? 7 : 0) | value;
     return IDFX_OK;
   }
   if (option == 1 /* IDFX_OPT_CT_FORM */ && (value == 0 || value == 1)) {
@@ -1639,8 +1789,8 @@ int idfx_set_option(idfx_ctx* c, int option, int value) {
       set_err("idfx_set_option: the CT form must be chosen before idfx_bind");
       return IDFX_ERR_INVALID_ARG;
     }
-    if (value == 1 && !c->mhd) {
-      set_err("idfx_set_option: the vector-potential form needs a magnetic field");
+    if (value == 1 && (!c->mhd || c->g.open)) {
+      set_err("idfx_set_option: the vector-potential form needs a magnetic field and a periodic box");
       return IDFX_ERR_UNSUPPORTED;
     }
     c->vp = value == 1;
@@ -1691,6 +1841,103 @@ int idfx_get_potential(idfx_ctx* c, double* d_pot) {
   }
   CK(cudaGetLastError());
   return IDFX_OK;
+}
+
+// ---- the cycle in pieces, and the halo slabs (domain decomposition) ----
+int idfx_cycle_begin(idfx_ctx* c, double dt, double cfl) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  DeviceScope on_device(c->device);
+  if (!(dt > 0.0) && (!(cfl > 0.0) || !(cfl < 1.0))) {
+    set_err("idfx_cycle_begin: need dt > 0, or dt <= 0 and 0 < cfl < 1");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  cycle_begin(c, dt > 0.0 ? dt : 0.0, cfl);
+  CK(cudaGetLastError());
+  return IDFX_OK;
+}
+
+static int check_stage(idfx_ctx* c, int stage, const char* who) {
+  if (stage < 0 || stage >= c->nstages) {
+    set_err("%s: no such stage", who);
+    return IDFX_ERR_INVALID_ARG;
+  }
+  return IDFX_OK;
+}
+
+int idfx_stage_flux(idfx_ctx* c, int stage) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  DeviceScope on_device(c->device);
+  if ((rc = check_stage(c, stage, "idfx_stage_flux"))) return rc;
+  stage_flux(c, stage);
+  CK(cudaGetLastError());
+  return IDFX_OK;
+}
+
+int idfx_stage_update(idfx_ctx* c, int stage) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  DeviceScope on_device(c->device);
+  if ((rc = check_stage(c, stage, "idfx_stage_update"))) return rc;
+  stage_update(c, stage);
+  CK(cudaGetLastError());
+  return IDFX_OK;
+}
+
+int idfx_cycle_end(idfx_ctx* c) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  cycle_end(c);
+  return IDFX_OK;
+}
+
+size_t idfx_dt_reduce_offset(const idfx_ctx* c) {
+  if (!c || !c->bound) return 0;
+  return (size_t)((const char*)&c->sc->smax_bits - (const char*)c->ws);
+}
+
+// the fields a halo slab carries: the primitives of the stage input (with Bc) and its face field
+static FieldList halo_fields(const idfx_ctx* c) {
+  FieldList fl;
+  fl.n = 0;
+  const int nv = c->mhd ? (c->fused ? 8 : 11) : 5;
+  for (int n = 0; n < nv; ++n) fl.f[fl.n++] = c->vfield(n);
+  if (c->mhd)
+    for (int d = 0; d < 3; ++d) fl.f[fl.n++] = c->bbuf(c->cyc_bin, d);
+  return fl;
+}
+
+long long idfx_halo_count(const idfx_ctx* c, int dir) {
+  if (!c || !c->bound || dir < 0 || dir > 2) return 0;
+  return (long long)halo_fields(c).n * slab_geom(c->g, dir, 0, SLAB_PACK, 0).count;
+}
+
+static int halo_op(idfx_ctx* c, int dir, int side, int mode, int clamp, double* d_buf, const char* who) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  DeviceScope on_device(c->device);
+  if (dir < 0 || dir > 2 || side < 0 || side > 1 || (mode != SLAB_COPY && !d_buf)) {
+    set_err("%s: need 0 <= dir <= 2, side 0 (lower) or 1 (upper) and a device buffer", who);
+    return IDFX_ERR_INVALID_ARG;
+  }
+  const SlabGeom sg = slab_geom(c->g, dir, side, mode, clamp);
+  const FieldList fl = halo_fields(c);
+  const unsigned nb = blocks_for(sg.count, 128);
+  LaunchScope ls(c, K_FILL);
+  if (mode == SLAB_COPY) k_slab<SLAB_COPY><<<nb, 128, 0, c->stream>>>(c->g, sg, fl, nullptr);
+  else if (mode == SLAB_PACK) k_slab<SLAB_PACK><<<nb, 128, 0, c->stream>>>(c->g, sg, fl, d_buf);
+  else k_slab<SLAB_UNPACK><<<nb, 128, 0, c->stream>>>(c->g, sg, fl, d_buf);
+  CK(cudaGetLastError());
+  return IDFX_OK;
+}
+
+int idfx_halo_pack(idfx_ctx* c, int dir, int side, double* d_buf) { return halo_op(c, dir, side, SLAB_PACK, 0, d_buf, "idfx_halo_pack"); }
+int idfx_halo_unpack(idfx_ctx* c, int dir, int side, const double* d_buf) {
+  return halo_op(c, dir, side, SLAB_UNPACK, 0, const_cast<double*>(d_buf), "idfx_halo_unpack");
+}
+int idfx_halo_fill(idfx_ctx* c, int dir, int side, int zero_gradient) {
+  return halo_op(c, dir, side, SLAB_COPY, zero_gradient ? 1 : 0, nullptr, "idfx_halo_fill");
 }
 
 int idfx_last_dt(idfx_ctx* c, double* h_dt_out) {

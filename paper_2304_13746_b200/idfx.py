@@ -11,7 +11,7 @@ import torch
 
 SOLVER_HLL, SOLVER_HLLC, SOLVER_HLLD, SOLVER_ROE, SOLVER_RUSANOV = 0, 1, 2, 3, 4
 LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3, LIMITER_PPM = 0, 1, 2, 3, 4
-OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR, OPT_BOUNDARY = 0, 1, 2, 3
+OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR, OPT_BOUNDARY, OPT_EXCHANGE_DIRS, OPT_OUTFLOW_SIDES = 0, 1, 2, 3, 4, 5
 BOUNDARY_PERIODIC, BOUNDARY_OUTFLOW = 0, 1
 CT_FACE, CT_POTENTIAL = 0, 1
 EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0, EMF_UCT_HLL = 0, 1, 2, 3, 4
@@ -29,6 +29,8 @@ SYMBOLS = (
     "idfx_set_option", "idfx_advance_to", "idfx_time", "idfx_get_potential", "idfx_set_option_real", "idfx_floor_count",
     "idfx_probe_fp64",
     "idfx_noalloc_compute_dt", "idfx_noalloc_last_error",
+    "idfx_cycle_begin", "idfx_stage_flux", "idfx_stage_update", "idfx_cycle_end", "idfx_dt_reduce_offset",
+    "idfx_set_state_finish", "idfx_halo_count", "idfx_halo_pack", "idfx_halo_unpack", "idfx_halo_fill",
 )
 
 _lib = None
@@ -74,6 +76,18 @@ def lib():
         L.idfx_profile_kernel_name.argtypes = [ci]
         L.idfx_profile_kernel_name.restype = ctypes.c_char_p
         L.idfx_probe_fp64.argtypes = [vp, ci, dp, dp]
+        L.idfx_cycle_begin.argtypes = [vp, cd, cd]
+        L.idfx_stage_flux.argtypes = [vp, ci]
+        L.idfx_stage_update.argtypes = [vp, ci]
+        L.idfx_cycle_end.argtypes = [vp]
+        L.idfx_dt_reduce_offset.argtypes = [vp]
+        L.idfx_dt_reduce_offset.restype = sz
+        L.idfx_set_state_finish.argtypes = [vp]
+        L.idfx_halo_count.argtypes = [vp, ci]
+        L.idfx_halo_count.restype = ctypes.c_longlong
+        L.idfx_halo_pack.argtypes = [vp, ci, ci, vp]
+        L.idfx_halo_unpack.argtypes = [vp, ci, ci, vp]
+        L.idfx_halo_fill.argtypes = [vp, ci, ci, ci]
         L.idfx_noalloc_compute_dt.argtypes = [ci, ci, ci, cd, cd, ci, vp, vp, cd, vp, vp]
         L.idfx_noalloc_last_error.restype = ctypes.c_char_p
         L.idfx_last_error.restype = ctypes.c_char_p
@@ -124,7 +138,7 @@ class Idfx:
     """One periodic nx*ny*nz box on one GPU.  Tensors are float64, [var][nz][ny][nx]."""
 
     def __init__(self, nx, ny, nz, dx, gamma, solver, limiter, emf_mode, device="cuda:0", stream=None, nstages=2,
-                 ct_form=CT_FACE, pressure_floor=0.0, boundary=BOUNDARY_PERIODIC):
+                 ct_form=CT_FACE, pressure_floor=0.0, boundary=BOUNDARY_PERIODIC, exchange_dirs=0, outflow_sides=0):
         self.L = lib()
         self.h = self.L.idfx_create(nx, ny, nz, dx, gamma, solver, limiter, emf_mode)
         if not self.h:
@@ -137,6 +151,11 @@ class Idfx:
             _check(self.L.idfx_set_option_real(self.h, OPT_PRESSURE_FLOOR, pressure_floor))
         if boundary != BOUNDARY_PERIODIC:
             _check(self.L.idfx_set_option(self.h, OPT_BOUNDARY, boundary))
+        if exchange_dirs:
+            _check(self.L.idfx_set_option(self.h, OPT_EXCHANGE_DIRS, exchange_dirs))
+        if outflow_sides:
+            _check(self.L.idfx_set_option(self.h, OPT_OUTFLOW_SIDES, outflow_sides))
+        self.nstages = nstages
         if not torch.cuda.is_available():
             raise RuntimeError("idfx needs a CUDA device; there is no CPU fallback")
         self.device = torch.device(device)
@@ -226,6 +245,56 @@ class Idfx:
 
     def set_integrator(self, nstages):
         _check(self.L.idfx_set_option(self.h, OPT_INTEGRATOR, nstages))
+        self.nstages = nstages
+
+    # ---- the cycle in pieces and the halo slabs (include/idfx.h, "The cycle in pieces"; driven by decomp.py) ----
+    def cycle_begin(self, dt, cfl):
+        with self._ordered():
+            _check(self.L.idfx_cycle_begin(self.h, dt, cfl))
+
+    def stage_flux(self, stage):
+        with self._ordered():
+            _check(self.L.idfx_stage_flux(self.h, stage))
+
+    def stage_update(self, stage):
+        with self._ordered():
+            _check(self.L.idfx_stage_update(self.h, stage))
+
+    def cycle_end(self):
+        _check(self.L.idfx_cycle_end(self.h))
+
+    def set_state_finish(self):
+        with self._ordered():
+            _check(self.L.idfx_set_state_finish(self.h))
+
+    def dt_word(self):
+        """The 8 bytes of the workspace that hold max_cells sum_d c_d/dx of the running cycle, as a float64 view."""
+        off = self.L.idfx_dt_reduce_offset(self.h)
+        return self.workspace[off:off + 8].view(torch.float64)
+
+    def halo_count(self, d):
+        return self.L.idfx_halo_count(self.h, d)
+
+    def new_buffer(self, count):
+        return torch.empty(count, dtype=torch.float64, device=self.device)
+
+    def adopt(self, buf):
+        """A neighbour's packed slab, on this context's device (a peer copy when the neighbour lives on another GPU)."""
+        return buf if buf.device == self.device else buf.to(self.device)
+
+    def halo_pack(self, d, side, buf):
+        assert buf.is_cuda and buf.dtype == torch.float64 and buf.is_contiguous() and buf.numel() >= self.halo_count(d)
+        with self._ordered():
+            _check(self.L.idfx_halo_pack(self.h, d, side, buf.data_ptr()))
+
+    def halo_unpack(self, d, side, buf):
+        assert buf.is_cuda and buf.dtype == torch.float64 and buf.is_contiguous() and buf.numel() >= self.halo_count(d)
+        with self._ordered():
+            _check(self.L.idfx_halo_unpack(self.h, d, side, buf.data_ptr()))
+
+    def halo_fill(self, d, side, zero_gradient):
+        with self._ordered():
+            _check(self.L.idfx_halo_fill(self.h, d, side, 1 if zero_gradient else 0))
 
     def advance_to(self, t_end, cfl, max_steps=(1 << 31) - 1):
         """Returns (number of cycles taken, time reached)."""
