@@ -94,6 +94,7 @@ def parse_args():
                          "sedov: its Cartesian Sedov-Taylor blast, HD, HLL, to --t-end (PAPER.md:253)")
     ap.add_argument("--t-end", type=float, default=None, help="ot3d (default 1.0) and sedov (default 0.1) only")
     ap.add_argument("--n", type=int, default=None, help="override the grid size (development only)")
+    ap.add_argument("--repeats", type=int, default=REPEATS, help="timed repeats of the K cycles from the same initial state")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -245,7 +246,7 @@ def run_ours(args):
     # line reports the MEDIAN repeat as value / ms_per_step and lists them all.
     sampler = ClockSampler(local)
     reps = []
-    for r in range(REPEATS):
+    for r in range(max(args.repeats, 1)):
         if r:
             sim.set_state(prim, bface)
         sim.advance(W, cfl)
@@ -264,7 +265,7 @@ def run_ours(args):
     clocks = sampler.stop()
     ms = statistics.median(reps)
     value = aggregate_rate(cells, K, world, ms * 1e-3)
-    repeats = {"n": REPEATS, "ms_per_step": [t / K for t in reps], "best_ms_per_step": min(reps) / K,
+    repeats = {"n": len(reps), "ms_per_step": [t / K for t in reps], "best_ms_per_step": min(reps) / K,
                "median_ms_per_step": ms / K, "what": "each repeat: set_state(same input), %d warm-up, %d timed cycles" % (W, K)}
 
     # ---- per-kernel durations over K more steps (CUDA events around every launch, on the launch stream) ----

@@ -153,6 +153,6 @@ HdKernel hd_kernel_sl(bool first);
 // MHD: the three sweeps of a stage in one kernel (mhd_stage.cuh), same translation units.
 typedef void (*MhdKernel)(Geom, MhdStageArgs, const CUtensorMap, const CUtensorMap);
 template <int SOLVER, int LIM>
-MhdKernel mhd_kernel_sl(bool first, int emf_mode);
+MhdKernel mhd_kernel_sl(bool first, int emf_mode, bool open);
 
 }  // namespace idfx

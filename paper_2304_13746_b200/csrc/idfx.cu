@@ -1104,22 +1104,22 @@ void launch_hd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int 
 
 // ---- MHD: the three sweeps of a stage in one kernel (mhd_stage.cuh; instantiated in sweeps_inst.cu) ----
 template <int SOLVER>
-MhdKernel mhd_kernel_s(int limiter, bool first, int mode) {
+MhdKernel mhd_kernel_s(int limiter, bool first, int mode, bool open) {
   switch (limiter) {
-    case LIM_FLAT: return mhd_kernel_sl<SOLVER, LIM_FLAT>(first, mode);
-    case LIM_MINMOD: return mhd_kernel_sl<SOLVER, LIM_MINMOD>(first, mode);
-    case LIM_LIMO3: return mhd_kernel_sl<SOLVER, LIM_LIMO3>(first, mode);
-    default: return mhd_kernel_sl<SOLVER, LIM_VANLEER>(first, mode);
+    case LIM_FLAT: return mhd_kernel_sl<SOLVER, LIM_FLAT>(first, mode, open);
+    case LIM_MINMOD: return mhd_kernel_sl<SOLVER, LIM_MINMOD>(first, mode, open);
+    case LIM_LIMO3: return mhd_kernel_sl<SOLVER, LIM_LIMO3>(first, mode, open);
+    default: return mhd_kernel_sl<SOLVER, LIM_VANLEER>(first, mode, open);
   }
 }
 
 // mode: the edge EMF the kernel evaluates (arithmetic, E^c, E^0); the 2D-HLL EMF comes from its own kernels afterwards
-MhdKernel mhd_kernel(const idfx_ctx* c, bool first, int mode) {
+MhdKernel mhd_kernel(const idfx_ctx* c, bool first, int mode, bool open) {
   switch (c->solver) {
-    case SOLVER_HLL: return mhd_kernel_s<SOLVER_HLL>(c->limiter, first, mode);
-    case SOLVER_RUSANOV: return mhd_kernel_s<SOLVER_RUSANOV>(c->limiter, first, mode);
-    case SOLVER_HLLD: return mhd_kernel_s<SOLVER_HLLD>(c->limiter, first, mode);
-    default: return mhd_kernel_s<SOLVER_ROE>(c->limiter, first, mode);
+    case SOLVER_HLL: return mhd_kernel_s<SOLVER_HLL>(c->limiter, first, mode, open);
+    case SOLVER_RUSANOV: return mhd_kernel_s<SOLVER_RUSANOV>(c->limiter, first, mode, open);
+    case SOLVER_HLLD: return mhd_kernel_s<SOLVER_HLLD>(c->limiter, first, mode, open);
+    default: return mhd_kernel_s<SOLVER_ROE>(c->limiter, first, mode, open);
   }
 }
 
@@ -1152,7 +1152,7 @@ void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int
   a.w0 = w0;
   dim3 grid(tx, ty, (unsigned)((g.nz + a.chunk - 1) / a.chunk));
   LaunchScope ls(c, K_MHD);
-  mhd_kernel(c, first, c->emf == EMF_UCT_HLL ? EMF_ARITH : c->emf)<<<grid, MS_THREADS, MS_SMEM_BYTES, c->stream>>>(g, a, c->mapMV,
+  mhd_kernel(c, first, c->emf == EMF_UCT_HLL ? EMF_ARITH : c->emf, g.open != 0)<<<grid, MS_THREADS, MS_SMEM_BYTES, c->stream>>>(g, a, c->mapMV,
                                                                                                                  c->mapMB);
 }
 
@@ -1452,8 +1452,8 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
     for (int first = 0; first < 2; ++first)
       CK(cudaFuncSetAttribute((const void*)hd_kernel(c, first != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, HD_SMEM_BYTES));
   if (c->fused && c->mhd)
-    for (int first = 0; first < 2; ++first)
-      CK(cudaFuncSetAttribute((const void*)mhd_kernel(c, first != 0, c->emf == EMF_UCT_HLL ? EMF_ARITH : c->emf),
+    for (int v = 0; v < 4; ++v)  // first / later stage x periodic / open (the boundary option may still change after bind)
+      CK(cudaFuncSetAttribute((const void*)mhd_kernel(c, (v & 1) != 0, c->emf == EMF_UCT_HLL ? EMF_ARITH : c->emf, (v & 2) != 0),
                               cudaFuncAttributeMaxDynamicSharedMemorySize, MS_SMEM_BYTES));
   c->bound = true;
   return IDFX_OK;

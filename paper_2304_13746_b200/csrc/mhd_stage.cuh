@@ -125,8 +125,9 @@ __device__ __forceinline__ double ms_edge(const double onA[2], const double onB[
   return mean + 0.25 * side;
 }
 
-// MODE: EMF_ARITH, EMF_UCT (upwind-contact) or EMF_UCT0
-template <int SOLVER, int LIM, int MODE, bool FIRST>
+// MODE: EMF_ARITH, EMF_UCT (upwind-contact) or EMF_UCT0.  OPEN: some direction does not wrap (Geom::open); the periodic box
+// is its own instantiation so that none of the open-side bookkeeping is in its instruction stream.
+template <int SOLVER, int LIM, int MODE, bool FIRST, bool OPEN>
 __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArgs a, const __grid_constant__ CUtensorMap mapV,
                                                               const __grid_constant__ CUtensorMap mapB) {
   extern __shared__ __align__(128) unsigned char ms_smem_raw[];
@@ -139,14 +140,14 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
   const int lx = threadIdx.x & 31, ly = threadIdx.x >> 5;
   // Along an open direction (Geom::open) the tiles start one cell below the box: the ghost cell -1 is nobody's cell, but the
   // edges at index 0 are its UPPER edges, and on a periodic side they belong to cell n-1 of the far end instead.
-  const int ox = g.open & 1, oy = (g.open >> 1) & 1, oz = (g.open >> 2) & 1;
+  const int ox = OPEN ? g.open & 1 : 0, oy = OPEN ? (g.open >> 1) & 1 : 0, oz = OPEN ? (g.open >> 2) & 1 : 0;
   const int x0 = blockIdx.x * MS_CX - ox, y0 = blockIdx.y * MS_CY - oy;
   const int i = x0 + lx, j = y0 + ly;
   const int s0 = blockIdx.z * a.chunk;
   const int s1 = min(s0 + a.chunk, g.nz);
   const int np = s1 - s0 + 4;  // planes s0-2 .. s1+1; plane p of the ring is z plane s0 - 2 + p
   const bool in_tile = ly < MS_CY && j < g.ny && lx < MS_CX && i < g.nx;  // this thread owns the upper edges of its cell
-  const bool complete = in_tile && i >= 0 && j >= 0;                      // and the cell itself
+  const bool complete = in_tile && (!OPEN || (i >= 0 && j >= 0));         // and the cell itself
   const bool live_row = j <= g.ny;  // warp-uniform; rows above the upper boundary face (last tile only) have nothing to supply
   if (threadIdx.x == 0) {
 #pragma unroll
@@ -193,7 +194,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
   refill(0);
   wait_plane(1);  // every later plane is waited for one iteration ahead, by the z solve
   // periodic image of the upper neighbours (edges are stored under the index of the cell whose LOWER edge they are)
-  const long long c_row = g.at(min(max(i, -1), g.nx - 1), min(max(j, -1), g.ny - 1), 0);
+  const long long c_row = g.at(min(i, g.nx - 1), min(j, g.ny - 1), 0);
   const long long up_x = !ox && i + 1 >= g.nx ? 1 - (long long)g.nx : 1;
   const long long up_y = !oy && j + 1 >= g.ny ? (1 - (long long)g.ny) * g.sy : (long long)g.sy;
   double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};  // cell s-1: divergence of its x and y faces minus its lower z flux (global order)
@@ -213,7 +214,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
     int wcode = 0;  // donor weights of this thread's three faces: 2 bits each, sign + 1
     double dFx[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, cfx2 = 0.0, FyO[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, cfy = 0.0;
     // ---- y and x faces of plane s (the last chunk of an open z direction: also of the ghost plane nz, for the lattice plane nz) ----
-    const bool xy = s < s1 || (oz && s == g.nz);
+    const bool xy = s < s1 || (OPEN && oz && s == g.nz);
     if (xy && live_row) {
       {
         // y: local order (rho, vy, vz, vx, p, Bcz, Bcx), normal field B_y on the lower y face
@@ -323,7 +324,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
       apply();
       break;
     }
-    if (!FIRST && complete && s < s1) {  // the same lines of the next plane, on their way to L2
+    if (!FIRST && (!OPEN || (complete && s < s1))) {  // the same lines of the next plane, on their way to L2
 #pragma unroll
       for (int n = 0; n < 5; ++n) {
         prefetch_l2(a.Uin[n] + c);
@@ -331,7 +332,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
       }
     }
     // ---- cell s: x and y parts of its divergence, minus its lower z flux ----
-    if (s < s1) {
+    if (!OPEN || s < s1) {
       const double* up = ex + se + MS_TX;  // row ly + 1; y sweep: (n, t1, t2) = (y, z, x)
       acc[0] = dFx[0] + (up[(EX_FY + 0) * MS_SLAB] - FyO[0]) - Fz[0];
       acc[2] = dFx[2] + (up[(EX_FY + 1) * MS_SLAB] - FyO[1]) - Fz[2];
@@ -363,7 +364,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
         wB[0] = wgt(wts[e01], 2);
         wB[1] = wgt(wts[e11], 2);
       }
-      if (s < s1) a.E[2][c + up_x + up_y] = ms_edge<MODE>(onA, onB, cl, wA, wB);
+      if (!OPEN || s < s1) a.E[2][c + up_x + up_y] = ms_edge<MODE>(onA, onB, cl, wA, wB);
       // E_x(i, j+1/2, s-1/2): a = y, b = z.  y faces (j+1/2) of planes s-1, s carry -F_y[B_z]; z faces (s-1/2) of rows j, j+1 carry +F_z[B_y]
       onA[0] = -elp[EL_YBZ * MS_SLAB + e01];
       onA[1] = -el[EL_YBZ * MS_SLAB + e01];
@@ -381,7 +382,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
         wB[0] = wgt(wts[e00], 4);
         wB[1] = wgt(wts[e01], 4);
       }
-      if (i >= 0) a.E[0][c + up_y] = ms_edge<MODE>(onA, onB, cl, wA, wB);
+      if (!OPEN || i >= 0) a.E[0][c + up_y] = ms_edge<MODE>(onA, onB, cl, wA, wB);
       // E_y(i+1/2, j, s-1/2): a = z, b = x.  z faces (s-1/2) of columns i, i+1 carry -F_z[B_x]; x faces (i+1/2) of planes s-1, s carry +F_x[B_z]
       onA[0] = -ex[(EX_ZB + 0) * MS_SLAB + e00];
       onA[1] = -ex[(EX_ZB + 0) * MS_SLAB + e10];
@@ -399,7 +400,7 @@ __global__ void __launch_bounds__(MS_THREADS, 1) k_mhd_stage(Geom g, MhdStageArg
         wB[0] = wgt(wtsp[e10], 0);
         wB[1] = wgt(wts[e10], 0);
       }
-      if (j >= 0) a.E[1][c + up_x] = ms_edge<MODE>(onA, onB, cl, wA, wB);
+      if (!OPEN || j >= 0) a.E[1][c + up_x] = ms_edge<MODE>(onA, onB, cl, wA, wB);
     }
     apply();
   }

@@ -17,18 +17,24 @@ HdKernel hd_kernel_sl(bool first) {
   return first ? (HdKernel)k_hd_stage<SOLVER, LIM, true> : (HdKernel)k_hd_stage<SOLVER, LIM, false>;
 }
 
+template <int SOLVER, int LIM, int MODE>
+MhdKernel mhd_kernel_m(bool first, bool open) {
+  if (open) return first ? (MhdKernel)k_mhd_stage<SOLVER, LIM, MODE, true, true> : (MhdKernel)k_mhd_stage<SOLVER, LIM, MODE, false, true>;
+  return first ? (MhdKernel)k_mhd_stage<SOLVER, LIM, MODE, true, false> : (MhdKernel)k_mhd_stage<SOLVER, LIM, MODE, false, false>;
+}
+
 template <int SOLVER, int LIM>
-MhdKernel mhd_kernel_sl(bool first, int emf_mode) {
+MhdKernel mhd_kernel_sl(bool first, int emf_mode, bool open) {
   switch (emf_mode) {
-    case EMF_UCT: return first ? (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_UCT, true> : (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_UCT, false>;
-    case EMF_UCT0: return first ? (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_UCT0, true> : (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_UCT0, false>;
-    default: return first ? (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_ARITH, true> : (MhdKernel)k_mhd_stage<SOLVER, LIM, EMF_ARITH, false>;
+    case EMF_UCT: return mhd_kernel_m<SOLVER, LIM, EMF_UCT>(first, open);
+    case EMF_UCT0: return mhd_kernel_m<SOLVER, LIM, EMF_UCT0>(first, open);
+    default: return mhd_kernel_m<SOLVER, LIM, EMF_ARITH>(first, open);
   }
 }
 
 // MHD: every solver but HLLC; hydrodynamics: every solver but HLLD (idfx_create refuses the other combinations)
 #if IDFX_INST_SOLVER != 1
-template MhdKernel mhd_kernel_sl<IDFX_INST_SOLVER, IDFX_INST_LIM>(bool, int);
+template MhdKernel mhd_kernel_sl<IDFX_INST_SOLVER, IDFX_INST_LIM>(bool, int, bool);
 #endif
 #if IDFX_INST_SOLVER != 2
 template HdKernel hd_kernel_sl<IDFX_INST_SOLVER, IDFX_INST_LIM>(bool);

@@ -274,8 +274,11 @@ def test_outflow_boundaries_hd(idfx, R):
     ref.advance_to(0.2, 0.3)
     assert_state_close(sim, ref, TOL, "blast through outflow walls")
     assert float(sim.get_conserved()[0][4].sum()) / n ** 3 < 0.9     # energy left the box
+    # with a magnetic field (tests/test_gpu_decomp.py): face-flux EMFs and the face form of CT only
     with pytest.raises(idfx.IdfxError):
-        idfx.Idfx(8, 8, 8, 0.125, G53, HLLD, VANLEER, EMF_UCT, boundary=idfx.BOUNDARY_OUTFLOW)
+        idfx.Idfx(8, 8, 8, 0.125, G53, HLLD, VANLEER, EMF_UCT_HLL, boundary=idfx.BOUNDARY_OUTFLOW)
+    with pytest.raises(idfx.IdfxError):
+        idfx.Idfx(8, 8, 8, 0.125, G53, HLLD, VANLEER, EMF_UCT, ct_form=1, boundary=idfx.BOUNDARY_OUTFLOW)
 
 
 def test_all_options_together_medium_box(idfx, R):
