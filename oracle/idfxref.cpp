@@ -46,7 +46,7 @@ enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_
 enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3, LIM_PPM = 4 };
 enum { OPT_INTEGRATOR = 0, OPT_CT_FORM = 1, OPT_PRESSURE_FLOOR = 2, OPT_BOUNDARY = 3 };  // idfxref_set_option / idfxref_set_option_real
 enum { CT_FACE = 0, CT_POTENTIAL = 1 };
-enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3, EMF_UCT_HLL = 4 };
+enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3, EMF_UCT_HLL = 4, EMF_UCT_HLLD = 5 };
 enum { OK = 0, ERR_INVALID_ARG = -1, ERR_UNSUPPORTED = -2, ERR_UNPHYSICAL = -5 };
 
 // ---------------------------------------------------------------------------------------------
@@ -284,6 +284,75 @@ void hlld_flux(const double WL[7], const double WR[7], double Bn, const double U
   } else {
     for (int n = 0; n < 7; ++n)
       F[n] = FR[n] + f.SsR * f.UssR[n] - (f.SsR - SR) * f.UsR[n] - SR * UR[n];
+  }
+}
+
+// 2D-HLLD EMF, face part ("2D ... HLLD Riemann solvers ... following the method of Mignone & Del Zanna
+// (2021)"; reading G24).  In every region of the HLLD fan the flux of a transverse field component is LINEAR in the two
+// face states and can be written, for t = t1, t2 alike,
+//     F_n[B_t] = a_L u_L B_t,L + a_R u_R B_t,R - (d_R B_t,R - d_L B_t,L) - vbar_t B_n ,      a_L + a_R = 1,
+// i.e. an upwinded transport of B_t along n plus the stretching of B_n by an effective transverse velocity.  With
+// h_K = [rho_K (S_K-u_K)^2 - B_n^2]/d_K, g_K = B_n (S_M-u_K)/d_K (B*_t,K = h_K B_t,K, v*_t,K = v_t,K - g_K B_t,K; G6: h = 1, g = 0),
+// s_K = sqrt(rho*_K), sgn = sign(B_n), sigma_K = S*_K s_K/(s_L+s_R), and the regions in the order of O7:
+//   L  : a_L = 1, d = 0, vbar = v_L                           R  : mirror image
+//   L* : a_L = 1, d_L = S_L (h_L - 1), d_R = 0, vbar = v_L    R* : a_R = 1, d_R = -S_R (h_R - 1), d_L = 0, vbar = v_R
+//   L**: a_L = 1, d_L = S_L (h_L - 1) - sigma_L (h_L - s_R sgn g_L), d_R = -sigma_L (h_R - s_R sgn g_R)
+//   R**: a_R = 1, d_R = -S_R (h_R - 1) + sigma_R (h_R + s_L sgn g_R), d_L = sigma_R (h_L + s_L sgn g_L)
+//   both **: vbar = (s_L v_L + s_R v_R)/(s_L+s_R) - S_M s_L s_R (v_R - v_L) / ((s_L+s_R) |B_n|)
+// (write out F = F*_K + S*_K (B**_t - B*_t,K) with the double-star states of O7 and collect the terms; the |B_n| part of
+// S*_K turns v_K into the density-weighted mean, the S_M part is the last term; |S_M| <= |B_n|/s_K inside the ** fan).
+// For equal states h = 1, g = 0 and d_L = d_R, as consistency demands.  out = (a_L, d_L, d_R, vbar_t1, vbar_t2).
+void hlld_uct_coeffs(const double WL[7], const double WR[7], double Bn, double g, double out[5]) {
+  double UL[7], UR[7], SL, SR;
+  cons_from_prim(WL, Bn, g, UL);
+  cons_from_prim(WR, Bn, g, UR);
+  davis_speeds(WL, WR, Bn, g, SL, SR);
+  if (SL >= 0.0) {
+    out[0] = 1.0; out[1] = 0.0; out[2] = 0.0; out[3] = WL[2]; out[4] = WL[3];
+    return;
+  }
+  if (SR <= 0.0) {
+    out[0] = 0.0; out[1] = 0.0; out[2] = 0.0; out[3] = WR[2]; out[4] = WR[3];
+    return;
+  }
+  HlldFan f;
+  hlld_fan(WL, WR, Bn, UL, UR, SL, SR, f);
+  const double SM = f.SM;
+  double h[2], gk[2];
+  const double* W[2] = {WL, WR};
+  const double SK[2] = {SL, SR};
+  for (int K = 0; K < 2; ++K) {
+    const double r = W[K][0], u = W[K][1];
+    const double dK = r * (SK[K] - u) * (SK[K] - SM) - Bn * Bn;
+    if (std::fabs(dK) < 1e-12 * r * (SK[K] - u) * (SK[K] - u)) {  // G6
+      h[K] = 1.0;
+      gk[K] = 0.0;
+    } else {
+      h[K] = (r * (SK[K] - u) * (SK[K] - u) - Bn * Bn) / dK;
+      gk[K] = Bn * (SM - u) / dK;
+    }
+  }
+  const double sL = std::sqrt(f.UsL[0]), sR = std::sqrt(f.UsR[0]);
+  const double sgn = (Bn >= 0.0) ? 1.0 : -1.0;
+  if (f.SsL >= 0.0) {
+    out[0] = 1.0; out[1] = SL * (h[0] - 1.0); out[2] = 0.0; out[3] = WL[2]; out[4] = WL[3];
+  } else if (f.SsR <= 0.0) {
+    out[0] = 0.0; out[1] = 0.0; out[2] = -SR * (h[1] - 1.0); out[3] = WR[2]; out[4] = WR[3];
+  } else {
+    if (SM >= 0.0) {
+      const double sig = f.SsL * sL / (sL + sR);
+      out[0] = 1.0;
+      out[1] = SL * (h[0] - 1.0) - sig * (h[0] - sR * sgn * gk[0]);
+      out[2] = -sig * (h[1] - sR * sgn * gk[1]);
+    } else {
+      const double sig = f.SsR * sR / (sL + sR);
+      out[0] = 0.0;
+      out[2] = -SR * (h[1] - 1.0) + sig * (h[1] + sL * sgn * gk[1]);
+      out[1] = sig * (h[0] + sL * sgn * gk[0]);
+    }
+    const double theta = -SM * sL * sR / ((sL + sR) * std::fabs(Bn));  // |B_n| > 0 here: the ** fan has zero width otherwise
+    out[3] = (sL * WL[2] + sR * WR[2]) / (sL + sR) + theta * (WR[2] - WL[2]);
+    out[4] = (sL * WL[3] + sR * WR[3]) / (sL + sR) + theta * (WR[3] - WL[3]);
   }
 }
 
@@ -594,7 +663,8 @@ struct Ctx {
   Arr E[3];                         // edge EMFs: E[0] at (i, j-1/2, k-1/2), E[1] at (i-1/2, j, k-1/2), E[2] at (i-1/2, j-1/2, k)
   Arr Vt[3][2], Al[3][2];           // EMF_UCT_HLL: per d-face, the HLL-weighted transverse velocities (components d+1, d+2)
                                     // and the one-sided speeds alpha+ = max(0, S_R), alpha- = max(0, -S_L)
-  const Arr* Bstage;                // face field of the stage input (edge_emf reads it for EMF_UCT_HLL)
+  Arr Hc[3][5];                     // EMF_UCT_HLLD: per d-face (a_L, d_L, d_R, vbar_t1, vbar_t2) of hlld_uct_coeffs
+  const Arr* Bstage;                // face field of the stage input (edge_emf reads it for EMF_UCT_HLL / EMF_UCT_HLLD)
   int nstages;                      // 1 Euler, 2 RK2, 3 RK3 (Tab. 1)
   int ct_form;                      // CT_FACE: Eq. 6; CT_POTENTIAL: Eq. 7-8
   Arr A[3], A0[3], As[3], Bref[3];  // CT_POTENTIAL: edge potential accumulated since set_state (same places as E),
@@ -708,7 +778,7 @@ void sweep(Ctx& c, int d, const Arr Bf[3], bool want_flux) {
   lo[a] = 0; hi[a] = c.n[a];
   lo[b] = -1; hi[b] = c.n[b];
   lo[e] = -1; hi[e] = c.n[e];
-  if (c.emf == EMF_UCT_HLL) {  // the 2D-HLL EMF reconstructs face quantities across two more transverse faces
+  if (c.emf == EMF_UCT_HLL || c.emf == EMF_UCT_HLLD) {  // the 2D EMFs reconstruct face quantities across two more transverse faces
     lo[b] = lo[e] = -NG;
     hi[b] = c.n[b] + NG - 1;
     hi[e] = c.n[e] + NG - 1;
@@ -753,6 +823,11 @@ void sweep(Ctx& c, int d, const Arr Bf[3], bool want_flux) {
             c.Al[d][1][i0] = am;
             c.Vt[d][0][i0] = (ap * WL[2] + am * WR[2]) / (ap + am);
             c.Vt[d][1][i0] = (ap * WL[3] + am * WR[3]) / (ap + am);
+          }
+          if (c.emf == EMF_UCT_HLLD) {
+            double co[5];
+            hlld_uct_coeffs(WL, WR, Bn, c.g, co);
+            for (int m = 0; m < 5; ++m) c.Hc[d][m][i0] = co[m];
           }
         } else {
           double SL, SR;
@@ -816,6 +891,33 @@ void edge_emf(Ctx& c, int comp) {
           const double term_a = (aap * vaW * BbW + aam * vaE * BbE - aap * aam * (BbE - BbW)) / (aap + aam);
           const double term_b = (abp * vbS * BaS + abm * vbN * BaN - abp * abm * (BaN - BaS)) / (abp + abm);
           e = -term_a + term_b;
+        }
+        if (c.emf == EMF_UCT_HLLD) {
+          // 2D HLLD EMF (G24): the two transports of the 2D-HLL EMF with the coefficients of hlld_uct_coeffs,
+          //   E_c = -[aL_a (v_a B_b)^W + aR_a (v_a B_b)^E - (dR_a B_b^E - dL_a B_b^W)]
+          //         +[aL_b (v_b B_a)^S + aR_b (v_b B_a)^N - (dR_b B_a^N - dL_b B_a^S)]
+          // W/E: staggered B_b and the effective velocity vbar_a of the b-faces on either side of the edge, reconstructed
+          // along a; S/N likewise along b on the a-faces; coefficients: the mean of the two faces that touch the edge.
+          const double* Bb = c.Bstage[b].data();
+          const double* Ba = c.Bstage[a].data();
+          const double* va_f = c.Hc[b][4].data();  // vbar_a on b-faces (b-sweep local order: n = b, t1 = c, t2 = a)
+          const double* vb_f = c.Hc[a][3].data();  // vbar_b on a-faces (a-sweep local order: n = a, t1 = b, t2 = c)
+          double unused, BbW, BbE, vaW, vaE, BaS, BaN, vbS, vbN;
+          reconstruct(c.limiter, Bb[P - 2 * ea], Bb[P - ea], Bb[P], c.dx, unused, BbW);
+          reconstruct(c.limiter, Bb[P - ea], Bb[P], Bb[P + ea], c.dx, BbE, unused);
+          reconstruct(c.limiter, va_f[P - 2 * ea], va_f[P - ea], va_f[P], c.dx, unused, vaW);
+          reconstruct(c.limiter, va_f[P - ea], va_f[P], va_f[P + ea], c.dx, vaE, unused);
+          reconstruct(c.limiter, Ba[P - 2 * eb], Ba[P - eb], Ba[P], c.dx, unused, BaS);
+          reconstruct(c.limiter, Ba[P - eb], Ba[P], Ba[P + eb], c.dx, BaN, unused);
+          reconstruct(c.limiter, vb_f[P - 2 * eb], vb_f[P - eb], vb_f[P], c.dx, unused, vbS);
+          reconstruct(c.limiter, vb_f[P - eb], vb_f[P], vb_f[P + eb], c.dx, vbN, unused);
+          const double aLa = 0.5 * (c.Hc[a][0][P - eb] + c.Hc[a][0][P]), dLa = 0.5 * (c.Hc[a][1][P - eb] + c.Hc[a][1][P]);
+          const double dRa = 0.5 * (c.Hc[a][2][P - eb] + c.Hc[a][2][P]);
+          const double aLb = 0.5 * (c.Hc[b][0][P - ea] + c.Hc[b][0][P]), dLb = 0.5 * (c.Hc[b][1][P - ea] + c.Hc[b][1][P]);
+          const double dRb = 0.5 * (c.Hc[b][2][P - ea] + c.Hc[b][2][P]);
+          const double Ta = aLa * vaW * BbW + (1.0 - aLa) * vaE * BbE - (dRa * BbE - dLa * BbW);
+          const double Tb = aLb * vbS * BaS + (1.0 - aLb) * vbN * BaN - (dRb * BaN - dLb * BaS);
+          e = -Ta + Tb;
         }
         if (c.emf == EMF_UCT0) {
           // E^0 of Gardiner & Stone 2005: the E^c construction with the two candidate gradients
@@ -988,8 +1090,9 @@ struct idfxref_ctx {
 IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, double gamma, int solver,
                                         int limiter, int emf_mode) {
   if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0.0) || !(gamma > 1.0)) return nullptr;
-  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 4 || emf_mode < 0 || emf_mode > 4) return nullptr;
-  if (limiter == LIM_PPM && emf_mode == EMF_UCT_HLL) return nullptr;  // the 2D-HLL EMF reconstructs with 3-cell stencils only
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 4 || emf_mode < 0 || emf_mode > 5) return nullptr;
+  if (limiter == LIM_PPM && (emf_mode == EMF_UCT_HLL || emf_mode == EMF_UCT_HLLD)) return nullptr;  // the 2D EMFs reconstruct with 3-cell stencils only
+  if (emf_mode == EMF_UCT_HLLD && solver != SOLVER_HLLD) return nullptr;  // its coefficients are those of the HLLD face solve
   const bool mhd = emf_mode != EMF_NONE;
   if (mhd && solver == SOLVER_HLLC) return nullptr;
   if (!mhd && solver == SOLVER_HLLD) return nullptr;
@@ -1009,6 +1112,8 @@ IDFXREF_API idfxref_ctx* idfxref_create(int nx, int ny, int nz, double dx, doubl
     for (int n = 0; n < 7; ++n) c.F[d][n].assign(c.N, 0.0);
     c.cf[d].assign(c.N, 0.0);
     c.E[d].assign(c.N, 0.0);
+    if (emf_mode == EMF_UCT_HLLD)
+      for (int m = 0; m < 5; ++m) c.Hc[d][m].assign(c.N, 0.0);
     if (emf_mode == EMF_UCT_HLL)
       for (int m = 0; m < 2; ++m) {
         c.Vt[d][m].assign(c.N, 0.0);
@@ -1035,7 +1140,7 @@ IDFXREF_API int idfxref_set_option(idfxref_ctx* h, int option, int value) {
   if (option == OPT_BOUNDARY && (value == 0 || value == 1)) {
     // with a magnetic field: face CT, three-cell reconstructions and the face-flux EMFs only (the 2D-HLL EMF and PPM reach
     // further into the ghost zones, the vector potential has no zero-gradient form)
-    if (value == 1 && c.mhd && (c.emf == EMF_UCT_HLL || c.limiter == LIM_PPM || c.ct_form == CT_POTENTIAL)) return ERR_UNSUPPORTED;
+    if (value == 1 && c.mhd && (c.emf == EMF_UCT_HLL || c.emf == EMF_UCT_HLLD || c.limiter == LIM_PPM || c.ct_form == CT_POTENTIAL)) return ERR_UNSUPPORTED;
     c.outflow = value;
     return OK;
   }
@@ -1260,6 +1365,10 @@ IDFXREF_API void idfxref_flux_from_cons(double gamma, const double* U, double Bn
 IDFXREF_API int idfxref_riemann(int solver, double gamma, const double* WL, const double* WR, double Bn,
                                 double* F, double* cface) {
   return riemann(solver, gamma, WL, WR, Bn, F, *cface);
+}
+// out[5] = (a_L, d_L, d_R, vbar_t1, vbar_t2) of the 2D-HLLD EMF (G24)
+IDFXREF_API void idfxref_hlld_uct_coeffs(double gamma, const double* WL, const double* WR, double Bn, double* out) {
+  hlld_uct_coeffs(WL, WR, Bn, gamma, out);
 }
 IDFXREF_API void idfxref_wave_speeds(double gamma, const double* WL, const double* WR, double Bn, double* SL,
                                      double* SR) {

@@ -19,7 +19,7 @@ LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3 = 0, 1, 2, 3
 OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR, OPT_BOUNDARY = 0, 1, 2, 3
 BOUNDARY_PERIODIC, BOUNDARY_OUTFLOW = 0, 1
 CT_FACE, CT_POTENTIAL = 0, 1
-EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0, EMF_UCT_HLL = 0, 1, 2, 3, 4
+EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0, EMF_UCT_HLL, EMF_UCT_HLLD = 0, 1, 2, 3, 4, 5
 OK, ERR_UNPHYSICAL = 0, -5
 
 _lib = None
@@ -68,6 +68,8 @@ def lib():
         L.idfxref_riemann.argtypes = [ci, cd, dp, dp, cd, dp, dp]
         L.idfxref_wave_speeds.argtypes = [cd, dp, dp, cd, dp, dp]
         L.idfxref_wave_speeds.restype = None
+        L.idfxref_hlld_uct_coeffs.argtypes = [cd, dp, dp, cd, dp]
+        L.idfxref_hlld_uct_coeffs.restype = None
         L.idfxref_slope.argtypes = [ci, cd, cd]
         L.idfxref_slope.restype = cd
         L.idfxref_hllc_fan.argtypes = [cd, dp, dp, dp, dp]
@@ -238,6 +240,13 @@ def wave_speeds(gamma, WL, WR, Bn=0.0):
     sl, sr = ctypes.c_double(), ctypes.c_double()
     lib().idfxref_wave_speeds(gamma, _p(_v7(WL)), _p(_v7(WR)), Bn, ctypes.byref(sl), ctypes.byref(sr))
     return sl.value, sr.value
+
+
+def hlld_uct_coeffs(gamma, WL, WR, Bn):
+    """(a_L, d_L, d_R, vbar_t1, vbar_t2) of the 2D-HLLD EMF at one face (reading G24)."""
+    out = np.empty(5)
+    lib().idfxref_hlld_uct_coeffs(gamma, _p(_v7(WL)), _p(_v7(WR)), Bn, _p(out))
+    return out
 
 
 def slope(limiter, dm, dp):

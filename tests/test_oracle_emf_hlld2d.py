@@ -1,0 +1,174 @@
+"""Pins of the 2D-HLLD edge EMF ("2D ... HLLD Riemann solvers ... following the method of Mignone & Del Zanna
+(2021)"; reading G24 of DESIGN.md).  The face part is a decomposition of the (already pinned) HLLD flux of the transverse
+field, F_n[B_t] = a_L u_L B_t,L + a_R u_R B_t,R - (d_R B_t,R - d_L B_t,L) - vbar_t B_n; the edge part transports the two
+staggered components with those coefficients.  What fixes it:
+  * the decomposition reproduces the HLLD flux of both transverse components in every region of the fan (random states
+    spanning all six regions), with a_L + a_R = 1 and d_L = d_R for equal states;
+  * plane-parallel flow along x, y and z: the edge EMF is the EMF of the 1D HLLD flux (the design requirement);
+  * uniform state: -v x B and nothing moves; conservation, div B, cyclic relabelling of the axes; second-order linear waves.
+"""
+import math
+
+import numpy as np
+import pytest
+
+HLL, HLLD = 0, 2
+VANLEER, LIMO3 = 2, 3
+EMF_UCT, EMF_UCT_HLLD = 2, 5
+G53 = 5.0 / 3.0
+
+
+def random_pair(rng, jump, supersonic=0.0):
+    WL = np.array([1.0 + 0.5 * rng.random(), rng.normal(0, 0.6) + supersonic, rng.normal(0, 0.6), rng.normal(0, 0.6),
+                   0.6 + 0.6 * rng.random(), rng.normal(0, 0.8), rng.normal(0, 0.8)])
+    WR = WL * (1.0 + jump * rng.uniform(-1, 1, 7)) + jump * rng.normal(0, 0.3, 7)
+    WR[0], WR[4] = abs(WR[0]) + 0.05, abs(WR[4]) + 0.05
+    return WL, WR
+
+
+def region_of(R, WL, WR, Bn):
+    S, _ = R.hlld_fan(G53, WL, WR, Bn)
+    SL, SsL, SM, SsR, SR = S
+    if SL >= 0: return "L"
+    if SR <= 0: return "R"
+    if SsL >= 0: return "L*"
+    if SsR <= 0: return "R*"
+    return "L**" if SM >= 0 else "R**"
+
+
+def test_decomposition_reproduces_the_hlld_flux_in_every_region(R):
+    rng = np.random.default_rng(8)
+    seen = {}
+    worst = 0.0
+    for k in range(6000):
+        WL, WR = random_pair(rng, 0.3, supersonic=rng.choice([0.0, 0.0, 2.5, -2.5]))
+        Bn = rng.normal(0, 0.7) if k % 7 else 0.0
+        F, _, _ = R.riemann(HLLD, G53, WL, WR, Bn)
+        aL, dL, dR, vt1, vt2 = R.hlld_uct_coeffs(G53, WL, WR, Bn)
+        assert aL in (0.0, 1.0)
+        for t, vt in ((5, vt1), (6, vt2)):
+            want = aL * WL[1] * WL[t] + (1 - aL) * WR[1] * WR[t] - (dR * WR[t] - dL * WL[t]) - vt * Bn
+            scale = max(np.abs(F).max(), 1.0)
+            worst = max(worst, abs(F[t] - want) / scale)
+        reg = region_of(R, WL, WR, Bn)
+        seen[reg] = seen.get(reg, 0) + 1
+    assert worst <= 1e-13, worst
+    assert set(seen) == {"L", "R", "L*", "R*", "L**", "R**"} and min(seen.values()) >= 20, seen
+
+
+def test_equal_states_give_a_consistent_upwind_transport(R):
+    """L = R: d_L = d_R (no net dissipation), vbar = the state's transverse velocity, a_L by the sign of u."""
+    rng = np.random.default_rng(9)
+    for _ in range(300):
+        W, _ = random_pair(rng, 0.0)
+        Bn = rng.normal(0, 0.7)
+        aL, dL, dR, vt1, vt2 = R.hlld_uct_coeffs(G53, W, W, Bn)
+        assert abs(dL - dR) <= 1e-13 * max(1.0, abs(dL)) and dL >= -1e-14
+        assert abs(vt1 - W[2]) <= 1e-13 and abs(vt2 - W[3]) <= 1e-13
+        assert aL == (1.0 if W[1] >= 0 else 0.0)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("limiter", [VANLEER, LIMO3])
+def test_emf_hlld2d_plane_parallel_identity(R, axis, limiter):
+    """Plane-parallel flow along a grid axis with uniform transverse velocity: E_t2 = -F_n[B_t1] and E_t1 = +F_n[B_t2] with the
+    HLLD fluxes.  The wave has both signs of u and of the contact speed, so faces lie in starred regions on both sides."""
+    n = 32
+    dx = 1.0 / n
+    x = (np.arange(n) + 0.5) * dx
+    shape = [4, 4, 4]
+    shape[2 - axis] = n
+    bc = [1, 1, 1]
+    bc[2 - axis] = n
+    X = x.reshape(bc)
+    a, b_, e = axis, (axis + 1) % 3, (axis + 2) % 3
+    prim = np.empty([5] + shape)
+    prim[0] = 1.0 + 0.3 * np.sin(2 * np.pi * X)
+    prim[1 + a] = 0.4 * np.cos(2 * np.pi * X)
+    prim[1 + b_] = 0.35
+    prim[1 + e] = -0.25
+    prim[4] = 1.0 + 0.2 * np.cos(4 * np.pi * X)
+    bf = np.empty([3] + shape)
+    bf[a] = 0.7
+    bf[b_] = 0.5 + 0.3 * np.sin(2 * np.pi * X)
+    bf[e] = -0.4 + 0.2 * np.cos(2 * np.pi * X)
+    dims = shape[::-1]
+    out = {}
+    for emf in (EMF_UCT_HLLD, EMF_UCT):
+        o = R.Oracle(dims[0], dims[1], dims[2], dx, G53, HLLD, limiter, emf)
+        o.set_state(prim, bf)
+        o.step(o.compute_dt(0.4))
+        out[emf] = (o.get_emf(), o.get_flux(axis)[0])
+    E, F = out[EMF_UCT_HLLD]
+    np.testing.assert_allclose(E[e], -F[5], rtol=0, atol=1e-13)   # E_t2 = -F_n[B_t1]
+    np.testing.assert_allclose(E[b_], F[6], rtol=0, atol=1e-13)   # E_t1 = +F_n[B_t2]
+    assert np.abs(E[a]).max() > 0.01
+    regions = set()
+    for i in range(n):                                             # the faces of this run do visit starred regions
+        idx = [0, 0, 0]
+        idx[2 - axis] = i
+        regions.add(bool(abs(F[5][tuple(idx)]) > 0))
+    assert regions == {True}
+
+
+def test_emf_hlld2d_uniform_state_conservation_divb_and_symmetry(R):
+    from test_oracle_scheme import divb, rot_prim, rot_vector, smooth_mhd_ic
+    n = 8
+    prim = np.empty((5, n, n, n))
+    for v, val in enumerate((1.3, 0.4, -0.7, 0.2, 0.8)):
+        prim[v] = val
+    b = np.empty((3, n, n, n))
+    for d, val in enumerate((0.5, -0.3, 0.9)):
+        b[d] = val
+    o = R.Oracle(n, n, n, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT_HLLD)
+    o.set_state(prim, b)
+    o.advance(2, 0.5)
+    assert np.array_equal(o.get_conserved()[1], b)
+    np.testing.assert_allclose(o.get_emf()[:, 0, 0, 0], -np.cross([0.4, -0.7, 0.2], [0.5, -0.3, 0.9]), rtol=1e-14)
+    n = 12
+    prim, b = smooth_mhd_ic(n, 7)
+    o = R.Oracle(n, n, n, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT_HLLD)
+    o.set_state(prim, b)
+    c0, b0 = o.get_conserved()
+    assert o.advance(3, 0.4) == 0
+    c1, b1 = o.get_conserved()
+    for v in range(5):
+        assert abs(c1[v].sum() - c0[v].sum()) <= 1e-13 * max(np.abs(c0[v]).sum(), 1.0)
+    for d in range(3):
+        assert abs(b1[d].sum() - b0[d].sum()) <= 1e-13 * np.abs(b0[d]).sum()
+    assert np.abs(divb(b1)).max() <= 1e-13 * np.abs(b1).max() * 6
+    o2 = R.Oracle(n, n, n, 1.0 / n, G53, HLLD, VANLEER, EMF_UCT_HLLD)
+    o2.set_state(rot_prim(prim), rot_vector(b))
+    o2.advance(3, 0.4)
+    p2, b2 = o2.get_state()
+    p1, _ = o.get_state()
+    np.testing.assert_allclose(p2, rot_prim(p1), rtol=0, atol=1e-13)
+    np.testing.assert_allclose(b2, rot_vector(b1), rtol=0, atol=1e-13)
+    # a different EMF than the upwind-contact one, by a truncation-error amount that shrinks with the resolution
+    diffs = []
+    for m in (12, 24):
+        prim, b = smooth_mhd_ic(m, 7)
+        res = []
+        for emf in (EMF_UCT_HLLD, EMF_UCT):
+            o3 = R.Oracle(m, m, m, 1.0 / m, G53, HLLD, VANLEER, emf)
+            o3.set_state(prim, b)
+            o3.advance(3, 0.4)
+            res.append(o3.get_conserved()[1])
+        diffs.append(np.abs(res[0] - res[1]).max() / np.abs(res[1]).max())
+    assert 1e-6 < diffs[1] < 0.4 * diffs[0] < 0.04, diffs
+
+
+@pytest.mark.parametrize("kind", ["fast", "alfven"])
+def test_emf_hlld2d_linear_wave_second_order(R, kind):
+    from test_oracle_scheme import run_linear_wave
+    errs = [run_linear_wave(R, n, kind, HLLD, EMF_UCT_HLLD) for n in (16, 32)]
+    ref = run_linear_wave(R, 32, kind, HLLD, EMF_UCT)
+    assert errs[0] < 0.1 and math.log2(errs[0] / errs[1]) >= 1.25, errs
+    assert errs[1] < 1.5 * ref, (errs, ref)
+
+
+def test_rejected_combinations(R):
+    with pytest.raises(ValueError):
+        R.Oracle(8, 8, 8, 0.125, G53, HLL, VANLEER, EMF_UCT_HLLD)      # its coefficients are the HLLD solve's
+    with pytest.raises(ValueError):
+        R.Oracle(8, 8, 8, 0.125, G53, HLLD, 4, EMF_UCT_HLLD)           # PPM
