@@ -56,9 +56,11 @@ enum { IDFX_LIMITER_FLAT = 0, IDFX_LIMITER_MINMOD = 1, IDFX_LIMITER_VANLEER = 2,
        IDFX_LIMITER_PPM = 4 };
 /* EMF reconstruction: arithmetic average of the face fluxes, the E^0 and E^c (upwind-contact)
  * schemes of Gardiner & Stone 2005, and the 2D HLL Riemann solver at the edges after Mignone & Del Zanna 2021 (reading G21;
- * consistent in the plane-parallel limit with the HLL face solver).  IDFX_EMF_NONE selects hydrodynamics (no magnetic
- * field at all). */
-enum { IDFX_EMF_NONE = 0, IDFX_EMF_ARITHMETIC = 1, IDFX_EMF_UCT_CONTACT = 2, IDFX_EMF_UCT_0 = 3, IDFX_EMF_UCT_HLL = 4 };
+ * consistent in the plane-parallel limit with the HLL face solver) and its HLLD counterpart (reading G24: the same two
+ * transports with the response coefficients of the HLLD face solves; plane-parallel limit = the 1D HLLD flux; with
+ * IDFX_SOLVER_HLLD only).  IDFX_EMF_NONE selects hydrodynamics (no magnetic field at all). */
+enum { IDFX_EMF_NONE = 0, IDFX_EMF_ARITHMETIC = 1, IDFX_EMF_UCT_CONTACT = 2, IDFX_EMF_UCT_0 = 3, IDFX_EMF_UCT_HLL = 4,
+       IDFX_EMF_UCT_HLLD = 5 };
 enum {
   IDFX_OK = 0,
   IDFX_ERR_INVALID_ARG = -1,

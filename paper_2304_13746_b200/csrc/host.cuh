@@ -35,6 +35,7 @@ enum {
   //   PPM: 3 x 5 face fluxes of (rho, m, E) and the 3 c_face fields of k_flux_face_ppm
   N_VP = 12,
   N_H2D = 15,
+  N_H2D_D = 18,   // 2D-HLLD EMF: 3 x 5 face quantities and the 3 edge EMFs
   N_GEN = 18
 };
 
@@ -63,8 +64,9 @@ struct idfx_ctx {
   int f_aa() const { return F_COUNT; }
   int f_bref() const { return F_COUNT + 9; }
   int f_h2d() const { return F_COUNT + (vp ? N_VP : 0); }
-  int f_eg() const { return f_h2d() + 12; }
-  int f_gen() const { return f_h2d() + (emf == EMF_UCT_HLL ? N_H2D : 0); }
+  bool emf2d() const { return emf == EMF_UCT_HLL || emf == EMF_UCT_HLLD; }  // edge EMFs from their own kernels (k_emf_hll2d)
+  int f_eg() const { return f_h2d() + (emf == EMF_UCT_HLLD ? 15 : 12); }
+  int f_gen() const { return f_h2d() + (emf == EMF_UCT_HLL ? N_H2D : (emf == EMF_UCT_HLLD ? N_H2D_D : 0)); }
   int nfields() const { return f_gen() + (limiter == LIM_PPM ? N_GEN : 0); }
   double* abuf(int which, int d) const { return field(f_aa() + 3 * which + d); }
   int exch = 0;  // bit d set: the ghost layers of direction d come from a neighbouring sub-box (idfx_halo_*), the caller

@@ -249,7 +249,8 @@ struct FluxArgs {
 };
 
 // FMODE 0: fluxes and c_face; 1: c_face only (idfx_compute_dt); 2: what the 2D-HLL EMF needs of the face (G21):
-// F[0] = alpha+ = max(0, S_R), F[1] = alpha- = max(0, -S_L), F[2], F[3] = the HLL-weighted transverse velocities.
+// F[0] = alpha+ = max(0, S_R), F[1] = alpha- = max(0, -S_L), F[2], F[3] = the HLL-weighted transverse velocities;
+// 3: what the 2D-HLLD EMF needs (G24, hlld_uct_face): F[0] = dirL, F[1] = kL, F[2] = kR, F[3], F[4] = the effective velocities.
 template <int SOLVER, int LIM, bool MHD, int FMODE>
 __global__ void __launch_bounds__(128) k_flux_face(Geom g, FluxArgs a) {
   int i, j, k;
@@ -281,6 +282,14 @@ __global__ void __launch_bounds__(128) k_flux_face(Geom g, FluxArgs a) {
     a.F[1][c] = am;
     a.F[2][c] = (ap * WL[2] + am * WR[2]) * inv;
     a.F[3][c] = (ap * WL[3] + am * WR[3]) * inv;
+  } else if (FMODE == 3) {
+    double dirL, kL, kR, vt1, vt2;
+    hlld_uct_face(WL, WR, Bn, g.gamma, dirL, kL, kR, vt1, vt2);
+    a.F[0][c] = dirL;
+    a.F[1][c] = kL;
+    a.F[2][c] = kR;
+    a.F[3][c] = vt1;
+    a.F[4][c] = vt2;
   } else {
     double F[7];
     a.cf[c] = riemann<SOLVER, MHD>(WL, WR, Bn, g.gamma, F);
@@ -477,7 +486,9 @@ __device__ __forceinline__ double edge_emf(const Geom& g, const EmfArgs& A, cons
 // k_flux_face<FMODE 2> (no ghosts: indices wrap) and the staggered field (ghosts filled).
 // ---------------------------------------------------------------------------------------------
 struct Hll2dArgs {
-  const double* H[3][4];   // per direction d: alpha+, alpha-, v_t1 (component d+1), v_t2 (component d+2) on the left d-faces
+  // per direction d, on the left d-faces: 2D-HLL: alpha+, alpha-, v_t1 (component d+1), v_t2 (component d+2);
+  // 2D-HLLD: dirL, kL, kR, vt1, vt2 of hlld_uct_face
+  const double* H[3][5];
   const double* Bf[3];
   double* E[3];
 };
@@ -494,7 +505,13 @@ __device__ __forceinline__ double hll_transport(double alp, double alm, double v
   return (alp * q_lo * (v_lo + alm) + alm * q_hi * (v_hi - alp)) / (alp + alm);
 }
 
-template <int LIM>
+// 2D-HLLD (reading G24): the transport of staggered component q across the edge with the response of the HLLD face solves
+// normal to it: plain upwind transport by the reconstructed face velocity on the side the contact points from, plus kL q_lo - kR q_hi
+__device__ __forceinline__ double hlld_transport(double dirL, double kL, double kR, double v_lo, double q_lo, double v_hi, double q_hi) {
+  return q_lo * (dirL * v_lo + kL) + q_hi * ((1.0 - dirL) * v_hi - kR);
+}
+
+template <int LIM, bool HLLD>
 __global__ void __launch_bounds__(128) k_emf_hll2d(Geom g, Hll2dArgs h) {
   int cellidx[3];
   if (!cell_of_thread(g, cellidx[0], cellidx[1], cellidx[2])) return;
@@ -518,7 +535,7 @@ __global__ void __launch_bounds__(128) k_emf_hll2d(Geom g, Hll2dArgs h) {
         w[m] = P + (long long)(t - cellidx[along]) * step[along];
       }
       // velocity component `along` on the `other`-faces: slot 2 of that sweep is component other+1, slot 3 is other+2
-      const double* __restrict__ vel = h.H[other][(along - other + 3) % 3 == 1 ? 2 : 3];
+      const double* __restrict__ vel = h.H[other][((along - other + 3) % 3 == 1 ? 2 : 3) + (HLLD ? 1 : 0)];
       const double* __restrict__ fld = h.Bf[other];
       double q_lo, q_hi, v_lo, v_hi;
       edge_sides<LIM>(fld[P - 2 * step[along]], fld[P - step[along]], fld[P], fld[P + step[along]], dx2, q_lo, q_hi);
@@ -526,8 +543,14 @@ __global__ void __launch_bounds__(128) k_emf_hll2d(Geom g, Hll2dArgs h) {
       // the two `along`-faces touching the edge are neighbours in `other`
       const int t = cellidx[other] - 1;
       const long long nb = P + (long long)((t < 0 ? t + ext[other] : t) - cellidx[other]) * step[other];
-      const double alp = fmax(h.H[along][0][nb], h.H[along][0][P]), alm = fmax(h.H[along][1][nb], h.H[along][1][P]);
-      T[leg] = hll_transport(alp, alm, v_lo, q_lo, v_hi, q_hi);
+      if (HLLD) {  // the mean response of the two faces
+        const double dirL = 0.5 * (h.H[along][0][nb] + h.H[along][0][P]);
+        const double kL = 0.5 * (h.H[along][1][nb] + h.H[along][1][P]), kR = 0.5 * (h.H[along][2][nb] + h.H[along][2][P]);
+        T[leg] = hlld_transport(dirL, kL, kR, v_lo, q_lo, v_hi, q_hi);
+      } else {
+        const double alp = fmax(h.H[along][0][nb], h.H[along][0][P]), alm = fmax(h.H[along][1][nb], h.H[along][1][P]);
+        T[leg] = hll_transport(alp, alm, v_lo, q_lo, v_hi, q_hi);
+      }
     }
     h.E[c][P] = T[1] - T[0];
   }
@@ -973,7 +996,7 @@ EmfArgs emf_args(idfx_ctx* c) {
     a.SG[d] = c->sgn(d);
     a.Ec[d] = c->vfield(8 + d);
     // edge EMFs already evaluated: by k_emf_hll2d (2D-HLL), or by the one-kernel stage (mhd_stage.cuh)
-    a.Eg[d] = c->emf == EMF_UCT_HLL ? c->field(c->f_eg() + d) : (c->fused ? c->field(F_FB + d) : nullptr);
+    a.Eg[d] = c->emf2d() ? c->field(c->f_eg() + d) : (c->fused ? c->field(F_FB + d) : nullptr);
   }
   return a;
 }
@@ -981,6 +1004,8 @@ EmfArgs emf_args(idfx_ctx* c) {
 // 2D-HLL EMF: face quantities of the three directions, then the edge EMFs (two passes over the stage input)
 template <int LIM>
 void launch_hll2d_l(idfx_ctx* c, const double* const Bf[3]) {
+  const bool hlld = c->emf == EMF_UCT_HLLD;
+  const int nq = hlld ? 5 : 4;  // face quantities per direction
   const Geom& g = c->g;
   const long long st[3] = {1, g.sy, g.sz};
   const unsigned nb = blocks_for(g.nc, 128);
@@ -998,18 +1023,20 @@ void launch_hll2d_l(idfx_ctx* c, const double* const Bf[3]) {
     a.bn = Bf[d];
     a.sd = st[d];
     for (int n = 0; n < 7; ++n) a.F[n] = nullptr;
-    for (int m = 0; m < 4; ++m) {
-      a.F[m] = c->field(c->f_h2d() + 4 * d + m);
+    for (int m = 0; m < nq; ++m) {
+      a.F[m] = c->field(c->f_h2d() + nq * d + m);
       h.H[d][m] = a.F[m];
     }
     a.cf = nullptr;
     h.Bf[d] = Bf[d];
     h.E[d] = c->field(c->f_eg() + d);
     LaunchScope ls(c, K_EMF);
-    k_flux_face<SOLVER_HLL, LIM, true, 2><<<nb, 128, 0, c->stream>>>(g, a);
+    if (hlld) k_flux_face<SOLVER_HLL, LIM, true, 3><<<nb, 128, 0, c->stream>>>(g, a);
+    else k_flux_face<SOLVER_HLL, LIM, true, 2><<<nb, 128, 0, c->stream>>>(g, a);
   }
   LaunchScope ls(c, K_EMF);
-  k_emf_hll2d<LIM><<<nb, 128, 0, c->stream>>>(g, h);
+  if (hlld) k_emf_hll2d<LIM, true><<<nb, 128, 0, c->stream>>>(g, h);
+  else k_emf_hll2d<LIM, false><<<nb, 128, 0, c->stream>>>(g, h);
 }
 
 void launch_hll2d(idfx_ctx* c, const double* const Bf[3]) {
@@ -1152,7 +1179,7 @@ void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int
   a.w0 = w0;
   dim3 grid(tx, ty, (unsigned)((g.nz + a.chunk - 1) / a.chunk));
   LaunchScope ls(c, K_MHD);
-  mhd_kernel(c, first, c->emf == EMF_UCT_HLL ? EMF_ARITH : c->emf, g.open != 0)<<<grid, MS_THREADS, MS_SMEM_BYTES, c->stream>>>(g, a, c->mapMV,
+  mhd_kernel(c, first, c->emf2d() ? EMF_ARITH : c->emf, g.open != 0)<<<grid, MS_THREADS, MS_SMEM_BYTES, c->stream>>>(g, a, c->mapMV,
                                                                                                                  c->mapMB);
 }
 
@@ -1244,13 +1271,13 @@ void stage_update(idfx_ctx* c, int s) {
       for (int n = 8; n < 11; ++n) a.V[n] = nullptr;
     dim3 grid((g.nx + CT_TX - 1) / CT_TX, (g.ny + CT_TY - 1) / CT_TY, (g.nz + CT_TZ - 1) / CT_TZ);
     const bool udone = p.combine && c->fused;  // the one-kernel stage applied the divergence itself
-    if (c->emf == EMF_UCT_HLL) {
+    if (c->emf2d()) {
       const double* Bf[3] = {c->bbuf(p.bin, 0), c->bbuf(p.bin, 1), c->bbuf(p.bin, 2)};
       launch_hll2d(c, Bf);
     }
     {
       LaunchScope ls(c, K_UPDATE);
-      if (c->fused || c->emf == EMF_UCT_HLL) launch_ct<EMF_UCT_HLL>(c, grid, ea, a, p.combine, udone);  // lattice read from memory
+      if (c->fused || c->emf2d()) launch_ct<EMF_UCT_HLL>(c, grid, ea, a, p.combine, udone);  // lattice read from memory
       else if (c->emf == EMF_UCT) launch_ct<EMF_UCT>(c, grid, ea, a, p.combine, udone);
       else if (c->emf == EMF_UCT0) launch_ct<EMF_UCT0>(c, grid, ea, a, p.combine, udone);
       else launch_ct<EMF_ARITH>(c, grid, ea, a, p.combine, udone);
@@ -1370,12 +1397,16 @@ idfx_ctx* idfx_create(int nx, int ny, int nz, double dx, double gamma, int solve
     set_err("idfx_create: need dx > 0 and gamma > 1");
     return nullptr;
   }
-  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 4 || emf_mode < 0 || emf_mode > 4) {
+  if (solver < 0 || solver > 4 || limiter < 0 || limiter > 4 || emf_mode < 0 || emf_mode > 5) {
     set_err("idfx_create: unknown solver, limiter or emf_mode");
     return nullptr;
   }
-  if (limiter == LIM_PPM && emf_mode == EMF_UCT_HLL) {
-    set_err("idfx_create: unsupported combination (the 2D-HLL EMF reconstructs with three-cell stencils, not PPM)");
+  if (limiter == LIM_PPM && (emf_mode == EMF_UCT_HLL || emf_mode == EMF_UCT_HLLD)) {
+    set_err("idfx_create: unsupported combination (the 2D-HLL / HLLD EMFs reconstruct with three-cell stencils, not PPM)");
+    return nullptr;
+  }
+  if (emf_mode == EMF_UCT_HLLD && solver != SOLVER_HLLD) {
+    set_err("idfx_create: unsupported combination (the 2D-HLLD EMF takes its coefficients from HLLD face solves)");
     return nullptr;
   }
   const bool mhd = emf_mode != EMF_NONE;
@@ -1453,7 +1484,7 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
       CK(cudaFuncSetAttribute((const void*)hd_kernel(c, first != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, HD_SMEM_BYTES));
   if (c->fused && c->mhd)
     for (int v = 0; v < 4; ++v)  // first / later stage x periodic / open (the boundary option may still change after bind)
-      CK(cudaFuncSetAttribute((const void*)mhd_kernel(c, (v & 1) != 0, c->emf == EMF_UCT_HLL ? EMF_ARITH : c->emf, (v & 2) != 0),
+      CK(cudaFuncSetAttribute((const void*)mhd_kernel(c, (v & 1) != 0, c->emf2d() ? EMF_ARITH : c->emf, (v & 2) != 0),
                               cudaFuncAttributeMaxDynamicSharedMemorySize, MS_SMEM_BYTES));
   c->bound = true;
   return IDFX_OK;
@@ -1753,7 +1784,7 @@ int idfx_set_option(idfx_ctx* c, int option, int value) {
     return IDFX_OK;
   }
   if (option == 3 /* IDFX_OPT_BOUNDARY */ && (value == 0 || value == 1)) {
-    if (value == 1 && (c->limiter == LIM_PPM || c->emf == EMF_UCT_HLL || c->vp)) {
+    if (value == 1 && (c->limiter == LIM_PPM || c->emf2d() || c->vp)) {
       set_err("idfx_set_option: outflow boundaries need a three-cell reconstruction, a face-flux EMF and the face form of CT");
       return IDFX_ERR_UNSUPPORTED;
     }
@@ -1776,7 +1807,7 @@ int idfx_set_option(idfx_ctx* c, int option, int value) {
       set_err("idfx_set_option: the exchanged directions must be chosen before idfx_bind");
       return IDFX_ERR_INVALID_ARG;
     }
-    if (value && (c->limiter == LIM_PPM || c->emf == EMF_UCT_HLL || c->vp)) {
+    if (value && (c->limiter == LIM_PPM || c->emf2d() || c->vp)) {
       set_err("idfx_set_option: halo exchange needs a three-cell reconstruction, a face-flux EMF and the face form of CT");
       return IDFX_ERR_UNSUPPORTED;
     }

@@ -15,7 +15,7 @@ namespace idfx {
 
 enum { SOLVER_HLL = 0, SOLVER_HLLC = 1, SOLVER_HLLD = 2, SOLVER_ROE = 3, SOLVER_RUSANOV = 4 };
 enum { LIM_FLAT = 0, LIM_MINMOD = 1, LIM_VANLEER = 2, LIM_LIMO3 = 3, LIM_PPM = 4 };
-enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3, EMF_UCT_HLL = 4 };
+enum { EMF_NONE = 0, EMF_ARITH = 1, EMF_UCT = 2, EMF_UCT0 = 3, EMF_UCT_HLL = 4, EMF_UCT_HLLD = 5 };
 
 #define IDFX_DEV __device__ __forceinline__
 
@@ -520,6 +520,57 @@ IDFX_DEV double hlld_onesided(const double WL[7], const double WR[7], double Bn,
     F[n] = pure ? FK[n] : f;
   }
   return cface;
+}
+
+// What the 2D-HLLD edge EMF needs of a face (reading G24): how the HLLD flux of a transverse field
+// component responds to the two face values of that component and to the normal field,
+//     F_n[B_t] = (u_L dirL + kL) B_t,L + (u_R (1 - dirL) - kR) B_t,R - vt B_n .
+// dirL says whether the face lies left of the contact; (kL, kR) is the response that is not plain upwind transport; vt slides
+// from v_L to v_R across the double-star fan.  One formula for all regions: a side's outer shock contributes
+// eK = S_K (h_K - 1) once the face is inside the fan, and inside the double-star fan both sides add -z h_K + m g_K with
+// z = +-S*_K s_K / (s_L + s_R) (+ left of the contact, - right) and m = +-z s_O sgn(B_n), s_O the root density of the other side.
+IDFX_DEV void hlld_uct_face(const double WL[7], const double WR[7], double Bn, double g, double& dirL, double& kL, double& kR,
+                            double& vt1, double& vt2) {
+  double SL, SR;
+  outer_speeds<true>(WL, WR, Bn, g, SL, SR);
+  const double Bn2 = Bn * Bn;
+  const double pTL = WL[4] + 0.5 * (Bn2 + WL[5] * WL[5] + WL[6] * WL[6]);
+  const double pTR = WR[4] + 0.5 * (Bn2 + WR[5] * WR[5] + WR[6] * WR[6]);
+  const double mL = WL[0] * (SL - WL[1]), mR = WR[0] * (SR - WR[1]);  // mass fluxes through the outer waves
+  const double SM = (mR * WR[1] - mL * WL[1] - pTR + pTL) / (mR - mL);
+  // per side: compression of the transverse field h, coupling g between B_t and v_t, root of the star density
+  double hK[2], gK[2], sK[2];
+  {
+    const double m[2] = {mL, mR}, S[2] = {SL, SR}, u[2] = {WL[1], WR[1]};
+#pragma unroll
+    for (int K = 0; K < 2; ++K) {
+      const double den = m[K] * (S[K] - SM) - Bn2;
+      const bool flat = fabs(den) < 1e-12 * m[K] * (S[K] - u[K]);  // G6
+      hK[K] = flat ? 1.0 : (m[K] * (S[K] - u[K]) - Bn2) / den;
+      gK[K] = flat ? 0.0 : Bn * (SM - u[K]) / den;
+      sK[K] = sqrt(m[K] / (S[K] - SM));
+    }
+  }
+  const double aB = fabs(Bn);
+  const double SsL = SM - aB / sK[0], SsR = SM + aB / sK[1];
+  // where the face lies (the order of O7)
+  const bool outerL = SL >= 0.0, outerR = !outerL && SR <= 0.0;
+  const bool starL = !outerL && !outerR && SsL >= 0.0, starR = !outerL && !outerR && !starL && SsR <= 0.0;
+  const bool inner = !outerL && !outerR && !starL && !starR;
+  const bool left = outerL || starL || (inner && SM >= 0.0);
+  dirL = left ? 1.0 : 0.0;
+  const bool fan = !outerL && !outerR;
+  const double eL = (fan && left) ? SL * (hK[0] - 1.0) : 0.0;
+  const double eR = (fan && !left) ? SR * (hK[1] - 1.0) : 0.0;
+  const double ssum = sK[0] + sK[1];
+  const double z = inner ? (left ? SsL * sK[0] : -SsR * sK[1]) / ssum : 0.0;
+  const double m = (left ? z * sK[1] : -z * sK[0]) * (Bn >= 0.0 ? 1.0 : -1.0);
+  kL = eL - z * hK[0] + m * gK[0];
+  kR = -eR - z * hK[1] + m * gK[1];
+  // share of v_R in the effective transverse velocity
+  const double om = inner ? sK[1] * (1.0 - SM * sK[0] / aB) / ssum : (left ? 0.0 : 1.0);
+  vt1 = WL[2] + om * (WR[2] - WL[2]);
+  vt2 = WL[3] + om * (WR[3] - WL[3]);
 }
 
 // One Riemann problem.  Returns the flux in F and c_face = max(|S_L|,|S_R|).

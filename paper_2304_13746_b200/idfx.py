@@ -14,7 +14,7 @@ LIMITER_FLAT, LIMITER_MINMOD, LIMITER_VANLEER, LIMITER_LIMO3, LIMITER_PPM = 0, 1
 OPT_INTEGRATOR, OPT_CT_FORM, OPT_PRESSURE_FLOOR, OPT_BOUNDARY, OPT_EXCHANGE_DIRS, OPT_OUTFLOW_SIDES = 0, 1, 2, 3, 4, 5
 BOUNDARY_PERIODIC, BOUNDARY_OUTFLOW = 0, 1
 CT_FACE, CT_POTENTIAL = 0, 1
-EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0, EMF_UCT_HLL = 0, 1, 2, 3, 4
+EMF_NONE, EMF_ARITHMETIC, EMF_UCT_CONTACT, EMF_UCT_0, EMF_UCT_HLL, EMF_UCT_HLLD = 0, 1, 2, 3, 4, 5
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_NOT_BOUND, ERR_CUDA, ERR_UNPHYSICAL = 0, -1, -2, -3, -4, -5
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

@@ -15,6 +15,7 @@ pytestmark = pytest.mark.gpu
 LIMO3 = 3
 PPM = 4
 EMF_UCT_HLL = 4
+EMF_UCT_HLLD = 5
 G53 = 5.0 / 3.0
 
 
@@ -38,6 +39,8 @@ OPTION_COMBOS = [
     (HLLC, PPM, EMF_NONE, 3, 0), (ROE, PPM, EMF_NONE, 2, 0),
     # 2D-HLL EMF
     (HLL, VANLEER, EMF_UCT_HLL, 2, 0), (HLLD, LIMO3, EMF_UCT_HLL, 3, 0), (HLL, MINMOD, EMF_UCT_HLL, 2, 1), (ROE, VANLEER, EMF_UCT_HLL, 1, 0),
+    # 2D-HLLD EMF (reading G24)
+    (HLLD, VANLEER, EMF_UCT_HLLD, 2, 0), (HLLD, LIMO3, EMF_UCT_HLLD, 3, 0), (HLLD, MINMOD, EMF_UCT_HLLD, 2, 1), (HLLD, VANLEER, EMF_UCT_HLLD, 1, 0),
 ]
 
 
@@ -311,3 +314,19 @@ def test_hd_fused_kernel_ragged_and_chunked(idfx, R):
     ref.advance(2, 0.4)
     assert abs(sim.last_dt() - ref.last_dt()) <= TOL_DT * ref.last_dt()
     assert_state_close(sim, ref, TOL, "fused HD stage, 70 x 45 x 150")
+
+
+def test_emf_hlld2d_on_turbulence_all_fan_regions(idfx, R):
+    """Mach-1 turbulence at 40^3 after a few cycles puts faces into every region of the HLLD fan (supersonic, starred and
+    double-starred on both sides): the 2D-HLLD EMF of the CUDA path (unified response form) against the oracle's region by
+    region coefficients."""
+    prim, b, cfg = inputs.make("config3", n=40)
+    sim, ref = pair(idfx, R, (40, 40, 40), cfg["dx"], HLLD, VANLEER, EMF_UCT_HLLD, prim.numpy(), b.numpy(), 2, 0)
+    sim.advance(6, 0.3)
+    ref.advance(6, 0.3)
+    assert sim.status() == 0 and ref.status() == 0
+    assert abs(sim.last_dt() - ref.last_dt()) <= TOL_DT * ref.last_dt()
+    assert_state_close(sim, ref, TOL, "2D-HLLD EMF, 40^3 turbulence")
+    bf = sim.get_conserved()[1]
+    div = (torch.roll(bf[0], -1, 2) - bf[0]) + (torch.roll(bf[1], -1, 1) - bf[1]) + (torch.roll(bf[2], -1, 0) - bf[2])
+    assert float(div.abs().max() / bf.abs().max()) <= 1e-13
