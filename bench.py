@@ -95,6 +95,9 @@ def parse_args():
     ap.add_argument("--t-end", type=float, default=None, help="ot3d (default 1.0) and sedov (default 0.1) only")
     ap.add_argument("--n", type=int, default=None, help="override the grid size (development only)")
     ap.add_argument("--repeats", type=int, default=REPEATS, help="timed repeats of the K cycles from the same initial state")
+    ap.add_argument("--decompose", default=None, metavar="PXxPYxPZ",
+                    help="domain decomposition (PAPER.md:229-233): the box is PX x PY x PZ sub-boxes of n^3 cells each (weak scaling), "
+                         "one per rank over NCCL under torchrun (PX*PY*PZ = --gpus), or all on the one GPU when --gpus 1")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -375,6 +378,84 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_decomposed(args):
+    """One box split into sub-boxes that exchange two-cell halos every stage and share one dt (decomp.py).  Weak scaling:
+    every sub-box is the n^3 workload box (the random-phase fields are periodic, so the global state is their periodic
+    continuation and every exchanged slab carries real data)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2304_13746_b200 import decomp, idfx, inputs
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dims = tuple(int(x) for x in args.decompose.lower().split("x"))
+    nsub = dims[0] * dims[1] * dims[2]
+    assert len(dims) == 3 and (world == nsub or world == 1), "--decompose PXxPYxPZ needs PX*PY*PZ ranks, or one rank"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    prim, bface, cfg = inputs.make(args.workload, n=args.n, device=dev)
+    n, cfl = cfg["n"], cfg["cfl"]
+    mine = [rank] if world > 1 else list(range(nsub))
+    boxes = []
+    for r in mine:
+        sim = idfx.Idfx(n, n, n, cfg["dx"], cfg["gamma"], cfg["solver"], cfg["limiter"], cfg["emf"], device=dev,
+                        exchange_dirs=decomp.exchange_dirs(dims))
+        boxes.append(sim)
+    link = decomp.DistLink(boxes[0], dims) if world > 1 else decomp.LocalLink(boxes, dims)
+    dec = decomp.Decomposition(link)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def reset():
+        for sim in boxes:
+            sim.set_state(prim, bface)
+        dec.finish_set_state()
+
+    K, W = args.steps, max(args.warmup, 0)
+    sampler = ClockSampler(local)
+    reps = []
+    for r in range(max(args.repeats, 1)):
+        reset()
+        dec.advance(W, cfl)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if r == 0:
+            sampler.start()
+        barrier()
+        l0 = sum(b.launch_count() for b in boxes)
+        e0.record()
+        dec.advance(K, cfl)
+        e1.record()
+        barrier()
+        launches = sum(b.launch_count() for b in boxes) - l0
+        assert all(b.status() == 0 for b in boxes)
+        reps.append(max_over_ranks(e0.elapsed_time(e1), world, dev))
+    clocks = sampler.stop()
+    ms = statistics.median(reps)
+    cells = n ** 3 * nsub
+    halo = sum(2 * boxes[0].halo_count(d) * 8 for d in range(3) if dims[d] > 1) * boxes[0].nstages
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": cells * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": "%s recipe, %d^3 cells per sub-box, %s sub-boxes (domain decomposition, halo exchange every stage, "
+                                   "one dt for the whole box), CFL %.2f" % (args.workload, n, args.decompose, cfl),
+                       "grid": [n * dims[0], n * dims[1], n * dims[2]], "cells_per_gpu": cells // world,
+                       "parallelism": "domain decomposition %s over %d GPU(s), %s" % (
+                           args.decompose, world, "NCCL isend/irecv + all_reduce(MAX)" if world > 1 else "sub-boxes on one device"),
+                       "halo_bytes_sent_per_subbox_per_step": halo},
+            "gpu_launches": launches, "clocks": clocks,
+            "repeats": {"n": len(reps), "ms_per_step": [t / K for t in reps]},
+        }))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_ot3d(args):
     """The paper's performance test itself (Tab. 4): 3D Orszag-Tang, HLLD + PLM van Leer + E^c + RK2, run
     from t = 0 to t_end with the CFL step (idfx_advance_to), 256^3 per GPU unless --n says otherwise.  One rank."""
@@ -442,6 +523,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.decompose:
+        run_decomposed(args)
     elif args.workload in ("ot3d", "sedov"):
         run_ot3d(args)
     else:

@@ -56,6 +56,7 @@ struct idfx_ctx {
   size_t ws_bytes = 0;
   cudaStream_t stream = nullptr;
   int device = -1;  // the device that holds the workspace (idfx_bind); every call runs there
+  int sms = 148;    // its SM count
   bool bound = false;
   idfx::DevScalars* sc = nullptr;
   int nstages = 2;  // Tab. 1: 1 Euler, 2 RK2, 3 RK3

@@ -1161,10 +1161,20 @@ void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int
   a.fB0 = 3 * bin;
   // along an open direction the tiles start at cell -1 (mhd_stage.cuh)
   const int tx = (g.nx + (g.open & 1) + MS_CX - 1) / MS_CX, ty = (g.ny + ((g.open >> 1) & 1) + MS_CY - 1) / MS_CY;
+  // z planes per CTA: one CTA per SM runs at a time, so the launch takes ceil(CTAs / SMs) rounds of (chunk + 1) plane
+  // iterations (every chunk re-solves the plane below it for its lowest edges); take the chunk count with the shortest
+  // launch among those that give at least two rounds
   const long long per_chunk = (long long)tx * ty;
-  long long nch = (148 * 24 + per_chunk - 1) / per_chunk;  // about 24 waves of one CTA per SM: a short last wave
   const long long maxch = g.nz / 16 > 0 ? g.nz / 16 : 1;
-  nch = nch < 1 ? 1 : (nch > maxch ? maxch : nch);
+  long long nch = 1, best = -1;
+  for (long long k = 1; k <= maxch; ++k) {
+    const long long chunk = (g.nz + k - 1) / k, ctas = per_chunk * ((g.nz + chunk - 1) / chunk);
+    const long long rounds = (ctas + c->sms - 1) / c->sms, cost = rounds * (chunk + 1);
+    if ((rounds >= 2 || k == maxch) && (best < 0 || cost < best)) {
+      best = cost;
+      nch = k;
+    }
+  }
   a.chunk = (int)((g.nz + nch - 1) / nch);
   for (int n = 0; n < 5; ++n) {
     a.R[n] = c->field(F_R + n);
@@ -1458,6 +1468,7 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
   }
   c->device = attr.device;
   DeviceScope on_device(c->device);
+  if (cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || c->sms < 1) c->sms = 148;
   c->ws = (double*)d_workspace;
   c->ws_bytes = bytes;
   c->stream = (cudaStream_t)cuda_stream;
