@@ -61,7 +61,7 @@ def build(force=False, verbose=False, extra_flags=(), lib=LIB, obj_dir=_OBJ):
     with ThreadPoolExecutor(max_workers=workers) as pool:
         objs = list(pool.map(compile_one, units))
     tmp = lib + ".tmp.%d" % os.getpid()
-    subprocess.check_call([nvcc, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a"] + objs + ["-o", tmp])
+    subprocess.check_call([nvcc, "-shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a"] + objs + ["-ldl", "-o", tmp])
     os.replace(tmp, lib)
     return lib
 

@@ -5,6 +5,7 @@
 // column IOFF = 16 (a 128-byte boundary) with ghost columns 14,15 and nx+16,nx+17; pitch is a multiple of
 // 16 doubles.  All fields live in the caller's workspace.
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>  // header-only; ranges cost nothing unless a profiler (nsys, ncu --nvtx) is attached
 
 #include <cstddef>
 #include <cstdio>
@@ -1225,7 +1226,15 @@ StagePlan plan_stage(const idfx_ctx* c, int s) {
 }
 
 // dt_fixed > 0: that dt; otherwise dt = cfl / max found by stage 1, shortened to land on t_end (never leaves the device)
+// NVTX range per cycle piece: "idfx cycle" > "stage s flux" / "stage s update"; under CUDA-graph replay
+// only the capture shows them, run with IDFX_GRAPH=0 for a per-stage timeline
+struct NvtxScope {
+  explicit NvtxScope(const char* name) { nvtxRangePushA(name); }
+  ~NvtxScope() { nvtxRangePop(); }
+};
+
 void cycle_begin(idfx_ctx* c, double dt_fixed, double cfl) {
+  NvtxScope range("idfx cycle_begin");
   c->cyc_dt_fixed = dt_fixed;
   c->cyc_cfl = cfl;
   c->cyc_b0 = c->cyc_bin = c->bcur;
@@ -1235,6 +1244,8 @@ void cycle_begin(idfx_ctx* c, double dt_fixed, double cfl) {
 
 // a3 - a6 of stage s: reconstruct -> Riemann -> flux divergence (-> edge EMFs); stage 0 also reduces max sum_d c_d / dx
 void stage_flux(idfx_ctx* c, int s) {
+  static const char* const names[3] = {"idfx stage 1 flux+emf", "idfx stage 2 flux+emf", "idfx stage 3 flux+emf"};
+  NvtxScope range(names[s]);
   const StagePlan p = plan_stage(c, s);
   const double* Bf[3] = {c->bbuf(p.bin, 0), c->bbuf(p.bin, 1), c->bbuf(p.bin, 2)};
   if (!c->fused) launch_ppm(c, Bf, s == 0 && !(c->cyc_dt_fixed > 0.0));  // PPM: generic face-flux kernels, divergence and dt in k_rhs
@@ -1244,6 +1255,8 @@ void stage_flux(idfx_ctx* c, int s) {
 
 // a7, a8, a2 of stage s (and the ghost images or the local ghost fill a1 of its result); rotates the buffers
 void stage_update(idfx_ctx* c, int s) {
+  static const char* const names[3] = {"idfx stage 1 ct+update", "idfx stage 2 ct+update", "idfx stage 3 ct+update"};
+  NvtxScope range(names[s]);
   const StagePlan p = plan_stage(c, s);
   const Geom& g = c->g;
   c->cyc_bin = p.bout;
