@@ -186,6 +186,11 @@ long long idfx_halo_count(const idfx_ctx* ctx, int dir);
 int       idfx_halo_pack(idfx_ctx* ctx, int dir, int side, double* d_buf);          /* side 0: lower, 1: upper */
 int       idfx_halo_unpack(idfx_ctx* ctx, int dir, int side, const double* d_buf);
 int       idfx_halo_fill(idfx_ctx* ctx, int dir, int side, int zero_gradient);      /* periodic image, or the nearest layer */
+/* Pack and unpack in one launch when the neighbour is a context of the SAME process: the two active layers next to `side`
+ * of ctx are written straight into the ghost layers of the opposite side of `neighbour` (peer stores over NVLink when it is
+ * bound on another, peer-accessible device; IDFX_ERR_UNSUPPORTED when it is not).  Enqueued on ctx's stream: the caller
+ * orders it after the neighbour's last use of those ghost layers and before its next one. */
+int       idfx_halo_push(idfx_ctx* ctx, int dir, int side, idfx_ctx* neighbour);
 
 /* dt used by the most recent cycle (synchronises). */
 int idfx_last_dt(idfx_ctx* ctx, double* h_dt_out);

@@ -145,6 +145,20 @@ __global__ void k_slab(Geom g, SlabGeom sg, FieldList fl, double* __restrict__ b
   }
 }
 
+// Pack and unpack in one: the NG active layers next to one side of a sub-box go straight into the ghost layers of the
+// opposite side of its neighbour.  The neighbour's fields may live on another GPU of the same process: the stores are then
+// peer stores over NVLink (coalesced along x, no staging buffer, one launch per slab instead of two).
+__global__ void k_slab_push(Geom gs, SlabGeom from, FieldList fs, Geom gd, SlabGeom to, FieldList fd) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= from.count) return;
+  const int l0 = (int)(t % from.ext[0]);
+  const long long r = t / from.ext[0];
+  const int l1 = (int)(r % from.ext[1]), l2 = (int)(r / from.ext[1]);
+  const long long src = gs.at(from.lo[0] + l0, from.lo[1] + l1, from.lo[2] + l2);
+  const long long dst = gd.at(to.lo[0] + l0, to.lo[1] + l1, to.lo[2] + l2);
+  for (int n = 0; n < fs.n; ++n) fd.f[n][dst] = fs.f[n][src];
+}
+
 // ---------------------------------------------------------------------------------------------
 // a2: cell-centred B and cons <-> prim
 // ---------------------------------------------------------------------------------------------
@@ -1996,6 +2010,38 @@ int idfx_halo_unpack(idfx_ctx* c, int dir, int side, const double* d_buf) {
 }
 int idfx_halo_fill(idfx_ctx* c, int dir, int side, int zero_gradient) {
   return halo_op(c, dir, side, SLAB_COPY, zero_gradient ? 1 : 0, nullptr, "idfx_halo_fill");
+}
+
+int idfx_halo_push(idfx_ctx* c, int dir, int side, idfx_ctx* nb) {
+  int rc = check_bound(c);
+  if (rc) return rc;
+  if ((rc = check_bound(nb))) return rc;
+  DeviceScope on_device(c->device);
+  if (dir < 0 || dir > 2 || side < 0 || side > 1) {
+    set_err("idfx_halo_push: need 0 <= dir <= 2 and side 0 (lower) or 1 (upper)");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  const SlabGeom from = slab_geom(c->g, dir, side, SLAB_PACK, 0), to = slab_geom(nb->g, dir, 1 - side, SLAB_UNPACK, 0);
+  const FieldList fs = halo_fields(c), fd = halo_fields(nb);
+  if (from.ext[0] != to.ext[0] || from.ext[1] != to.ext[1] || from.ext[2] != to.ext[2] || fs.n != fd.n) {
+    set_err("idfx_halo_push: the two sub-boxes do not share the face they meet at (extents or scheme differ)");
+    return IDFX_ERR_INVALID_ARG;
+  }
+  if (nb->device != c->device) {  // peer stores: once per pair of devices
+    int can = 0;
+    CK(cudaDeviceCanAccessPeer(&can, c->device, nb->device));
+    if (!can) {
+      set_err("idfx_halo_push: device of the neighbour is not peer-accessible (use idfx_halo_pack / unpack and a transport)");
+      return IDFX_ERR_UNSUPPORTED;
+    }
+    const cudaError_t e = cudaDeviceEnablePeerAccess(nb->device, 0);
+    if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) CK(e);
+    cudaGetLastError();
+  }
+  LaunchScope ls(c, K_FILL);
+  k_slab_push<<<blocks_for(from.count, 128), 128, 0, c->stream>>>(c->g, from, fs, nb->g, to, fd);
+  CK(cudaGetLastError());
+  return IDFX_OK;
 }
 
 int idfx_last_dt(idfx_ctx* c, double* h_dt_out) {

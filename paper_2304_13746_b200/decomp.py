@@ -69,10 +69,13 @@ def exchange_dirs(dims):
 class LocalLink:
     """All sub-boxes in this process: boxes[rank]."""
 
-    def __init__(self, boxes, dims, periodic=True):
+    def __init__(self, boxes, dims, periodic=True, push=True):
         assert len(boxes) == dims[0] * dims[1] * dims[2]
         self.boxes, self.dims, self.periodic = boxes, dims, periodic
         self.ranks = list(range(len(boxes)))
+        # contexts of one process can write each other's ghost layers directly (idfx_halo_push: one launch per slab,
+        # peer stores over NVLink between devices); otherwise pack -> buffer -> unpack
+        self.push = push and all(hasattr(b, "halo_push") for b in boxes)
 
     def local(self):
         return list(zip(self.ranks, self.boxes))
@@ -86,6 +89,17 @@ class LocalLink:
             w.copy_(m)
 
     def exchange(self, d):
+        if self.push:
+            # a push reads active layers (and ghost layers of the directions already exchanged) and writes ghost layers of
+            # direction d only, so the pushes of one direction do not depend on one another
+            for r, b in self.local():
+                for side in (0, 1):
+                    nb = neighbour(r, self.dims, d, side, self.periodic)
+                    if nb is None:
+                        b.halo_fill(d, side, True)
+                    else:
+                        b.halo_push(d, side, self.boxes[nb])
+            return
         # pack every slab first (a box's upper and lower slabs come from disjoint layers, and nobody's ghosts are touched
         # until all are packed), then unpack
         packed = {}

@@ -30,7 +30,7 @@ SYMBOLS = (
     "idfx_probe_fp64",
     "idfx_noalloc_compute_dt", "idfx_noalloc_last_error",
     "idfx_cycle_begin", "idfx_stage_flux", "idfx_stage_update", "idfx_cycle_end", "idfx_dt_reduce_offset",
-    "idfx_set_state_finish", "idfx_halo_count", "idfx_halo_pack", "idfx_halo_unpack", "idfx_halo_fill",
+    "idfx_set_state_finish", "idfx_halo_count", "idfx_halo_pack", "idfx_halo_unpack", "idfx_halo_fill", "idfx_halo_push",
 )
 
 _lib = None
@@ -88,6 +88,7 @@ def lib():
         L.idfx_halo_pack.argtypes = [vp, ci, ci, vp]
         L.idfx_halo_unpack.argtypes = [vp, ci, ci, vp]
         L.idfx_halo_fill.argtypes = [vp, ci, ci, ci]
+        L.idfx_halo_push.argtypes = [vp, ci, ci, vp]
         L.idfx_noalloc_compute_dt.argtypes = [ci, ci, ci, cd, cd, ci, vp, vp, cd, vp, vp]
         L.idfx_noalloc_last_error.restype = ctypes.c_char_p
         L.idfx_last_error.restype = ctypes.c_char_p
@@ -291,6 +292,18 @@ class Idfx:
         assert buf.is_cuda and buf.dtype == torch.float64 and buf.is_contiguous() and buf.numel() >= self.halo_count(d)
         with self._ordered():
             _check(self.L.idfx_halo_unpack(self.h, d, side, buf.data_ptr()))
+
+    def halo_push(self, d, side, neighbour):
+        """My two layers next to `side` straight into `neighbour`'s ghost layers of the opposite side (same process)."""
+        nb_cur = torch.cuda.current_stream(neighbour.device)
+        if nb_cur != neighbour.stream:
+            nb_cur.wait_stream(neighbour.stream)      # the neighbour is done with its ghost layers
+        with self._ordered():
+            if neighbour.device != self.device:
+                self.stream.wait_stream(nb_cur)
+            _check(self.L.idfx_halo_push(self.h, d, side, neighbour.h))
+        if neighbour.device != self.device:
+            nb_cur.wait_stream(self.stream)
 
     def halo_fill(self, d, side, zero_gradient):
         with self._ordered():

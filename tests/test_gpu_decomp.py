@@ -36,7 +36,7 @@ def smooth(shape, seed, mhd):
     return torch.from_numpy(prim).cuda(), (None if b is None else torch.from_numpy(b).cuda()), dx
 
 
-def run_decomposed(idfx, shape, dims, dx, scheme, prim, b, cycles, cfl, periodic=True, nstages=2):
+def run_decomposed(idfx, shape, dims, dx, scheme, prim, b, cycles, cfl, periodic=True, nstages=2, push=True):
     solver, limiter, emf = scheme
     nranks = dims[0] * dims[1] * dims[2]
     boxes, slices = [], []
@@ -50,7 +50,7 @@ def run_decomposed(idfx, shape, dims, dx, scheme, prim, b, cycles, cfl, periodic
         sim.set_state(prim[sl].contiguous(), None if b is None else b[sl].contiguous())
         boxes.append(sim)
         slices.append(sl)
-    dec = decomp.Decomposition(decomp.LocalLink(boxes, dims, periodic))
+    dec = decomp.Decomposition(decomp.LocalLink(boxes, dims, periodic, push=push))
     dec.finish_set_state()
     dec.advance(cycles, cfl)
     cons = torch.empty_like(prim)
@@ -178,3 +178,14 @@ def test_hd_outflow_compute_dt_matches_advance(idfx, R):
         sim.advance(1, 0.4)
         ref.advance(1, 0.4)
         assert sim.last_dt() == dt
+
+
+@pytest.mark.parametrize("periodic", [True, False])
+def test_pack_unpack_path_equals_the_push_path(idfx, periodic):
+    """The slab exchange through buffers (idfx_halo_pack / unpack: what a transport between processes carries) and the
+    direct push into the neighbour's ghost layers give the same bits."""
+    shape, dims, scheme = (37, 26, 19), (2, 2, 2), (HLLD, VANLEER, EMF_UCT)
+    prim, b, dx = smooth(shape, 47, True)
+    res = [run_decomposed(idfx, shape, dims, dx, scheme, prim, b, 2, 0.4, periodic=periodic, push=p) for p in (True, False)]
+    assert res[0][2] == res[1][2]
+    assert torch.equal(res[0][0], res[1][0]) and torch.equal(res[0][1], res[1][1])
