@@ -120,9 +120,10 @@ class LocalLink:
 class DistLink:
     """One sub-box per torch.distributed rank."""
 
-    def __init__(self, box, dims, periodic=True, group=None):
+    def __init__(self, box, dims, periodic=True, group=None, tags=True):
         import torch.distributed as dist
         self.dist, self.group = dist, group
+        self.tags = tags          # False: every message with tag 0, i.e. matched by order alone as NCCL does (tests)
         self.box, self.dims, self.periodic = box, dims, periodic
         self.rank = dist.get_rank(group)
         assert dist.get_world_size(group) == dims[0] * dims[1] * dims[2]
@@ -135,24 +136,27 @@ class DistLink:
 
     def exchange(self, d):
         b, dist = self.box, self.dist
+        nbs = [neighbour(self.rank, self.dims, d, side, self.periodic) for side in (0, 1)]
         send = [b.new_buffer(b.halo_count(d)) for _ in (0, 1)]
-        recv = [b.new_buffer(b.halo_count(d)) for _ in (0, 1)]
+        recv = [b.new_buffer(b.halo_count(d)) for _ in (0, 1)]   # recv[side]: what goes into my ghost layers of that side
         ops = []
+        # NCCL has no tags: between two ranks the k-th send matches the k-th receive.  Everybody sends its lower slab, then its
+        # upper slab; the lower slab of my upper neighbour fills my upper ghosts, so receives are posted upper first.  (With
+        # two ranks along a periodic direction both neighbours are the same peer, and only this order pairs them correctly;
+        # gloo also honours the tags.)
         for side in (0, 1):
-            nb = neighbour(self.rank, self.dims, d, side, self.periodic)
-            if nb is None:
+            if nbs[side] is None:
                 continue
             b.halo_pack(d, side, send[side])
-            if nb == self.rank:            # cannot happen with dims[d] > 1; kept for a one-rank group
-                recv[1 - side].copy_(send[side])
-                continue
-            ops.append(dist.P2POp(dist.isend, send[side], nb, self.group, tag=2 * d + side))
-            ops.append(dist.P2POp(dist.irecv, recv[side], nb, self.group, tag=2 * d + (1 - side)))
+            ops.append(dist.P2POp(dist.isend, send[side], nbs[side], self.group, tag=(2 * d + side) if self.tags else 0))
+        for side in (1, 0):
+            if nbs[side] is not None:
+                ops.append(dist.P2POp(dist.irecv, recv[side], nbs[side], self.group, tag=(2 * d + (1 - side)) if self.tags else 0))
         if ops:
             for w in dist.batch_isend_irecv(ops):
                 w.wait()
         for side in (0, 1):
-            if neighbour(self.rank, self.dims, d, side, self.periodic) is None:
+            if nbs[side] is None:
                 b.halo_fill(d, side, True)
             else:
                 b.halo_unpack(d, side, recv[side])

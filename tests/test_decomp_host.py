@@ -172,7 +172,7 @@ def test_local_link_reproduces_the_single_box(dims, periodic):
             assert sorted(set(f)) == [0, 1, 2] and f == sorted(f)
 
 
-def _worker(rank, world, port, dims, periodic, path):
+def _worker(rank, world, port, dims, periodic, path, tags=True):
     import torch.distributed as dist
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
@@ -181,7 +181,7 @@ def _worker(rank, world, port, dims, periodic, path):
     (x0, nx), (y0, ny), (z0, nz) = decomp.sub_box(rank, dims, shape)
     sl = (slice(None), slice(z0, z0 + nz), slice(y0, y0 + ny), slice(x0, x0 + nx))
     box = HostBox(field[sl])
-    dec = decomp.Decomposition(decomp.DistLink(box, dims, periodic))
+    dec = decomp.Decomposition(decomp.DistLink(box, dims, periodic, tags=tags))
     dec.finish_set_state()
     dec.advance(2, 0.3)
     np.save(path % rank, box.active())
@@ -193,6 +193,20 @@ def _worker(rank, world, port, dims, periodic, path):
 def test_dist_link_over_gloo_world_size_2(tmp_path, dims, periodic, port):
     path = str(tmp_path / "rank%d.npy")
     mp.spawn(_worker, args=(2, port, dims, periodic, path), nprocs=2, join=True)
+    field = whole_field((13, 10, 9))
+    one, _ = run_local(field, (1, 1, 1), periodic)
+    for rank in range(2):
+        (x0, nx), (y0, ny), (z0, nz) = decomp.sub_box(rank, dims, field.shape[:0:-1])
+        assert np.array_equal(np.load(path % rank), one[:, z0:z0 + nz, y0:y0 + ny, x0:x0 + nx])
+
+
+def test_dist_link_pairs_messages_by_order_alone(tmp_path):
+    """NCCL has no tags: between two ranks the k-th send meets the k-th receive.  With two ranks along a periodic direction
+    both neighbours of a rank are the same peer, so only the right posting order delivers each slab to the right side.
+    All tags equal makes gloo match by order too."""
+    dims, periodic = (2, 1, 1), True
+    path = str(tmp_path / "rank%d.npy")
+    mp.spawn(_worker, args=(2, 29547, dims, periodic, path, False), nprocs=2, join=True)
     field = whole_field((13, 10, 9))
     one, _ = run_local(field, (1, 1, 1), periodic)
     for rank in range(2):
