@@ -39,7 +39,8 @@ struct HdStageArgs {
   int chunk;      // z planes per CTA
   double* R[5];
   DevScalars* sc;
-  const double* Uin[5];
+  const double* Uin[5];  // U_{s-1}; or, with uin_is_r, the first stage's divergence R_1 (RK2: U_1 = U_0 - dt/dx R_1 is never stored)
+  int uin_is_r;
   const double* U0[5];
   double* Uout[5];
   double* Vout[5];
@@ -211,7 +212,9 @@ __global__ void __launch_bounds__(HD_THREADS, HD_MINB) k_hd_stage(Geom g, HdStag
 #pragma unroll
         for (int n = 0; n < 5; ++n) {
           const double u0 = a.U0[n][cu];
-          u[n] = dtdx == 0.0 ? u0 : a.w0 * u0 + a.w * (a.Uin[n][cu] - dtdx * rt[n]);  // Eq. 9
+          const double uin = a.Uin[n][cu];
+          const double us = a.uin_is_r ? u0 - dtdx * uin : uin;
+          u[n] = dtdx == 0.0 ? u0 : a.w0 * u0 + a.w * (us - dtdx * rt[n]);  // Eq. 9
         }
         const double ir = 1.0 / u[0];
         const double vx = u[1] * ir, vy = u[2] * ir, vz = u[3] * ir;

@@ -615,7 +615,7 @@ __global__ void __launch_bounds__(128, 16) k_update_hd(Geom g, UpdateArgs a) {  
   for (int n = 0; n < 5; ++n) {
     const double us = a.Uin[n][c] - dtdx * a.R[n][c];
     u[n] = STAGE2 ? (dt == 0.0 ? a.U0[n][c] : a.w0 * a.U0[n][c] + a.w * us) : us;
-    a.Uout[n][c] = u[n];
+    if (STAGE2 || a.store_u) a.Uout[n][c] = u[n];
   }
   double vx, vy, vz, p;
   prim_from_cons(g.gamma - 1.0, u[0], u[1], u[2], u[3], u[4], 0.0, 0.0, 0.0, vx, vy, vz, p);
@@ -1120,6 +1120,10 @@ HdKernel hd_kernel(const idfx_ctx* c, bool first) {
   }
 }
 
+// RK2 without a stored U_1 (one-kernel stages, no pressure floor): the first stage's update kernel keeps U_1 in registers
+// for the primitives only, and the second stage rebuilds it from U_0 and R_1, which it reads instead of U_1
+bool rk2_keeps_no_u1(const idfx_ctx* c) { return c->fused && c->nstages == 2 && !(c->g.pfloor > 0.0); }
+
 void launch_hd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int uout) {
   const Geom& g = c->g;
   HdStageArgs a;
@@ -1131,11 +1135,12 @@ void launch_hd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int 
   a.chunk = (int)((g.nz + nch - 1) / nch);
   for (int n = 0; n < 5; ++n) {
     a.R[n] = c->field(F_R + n);
-    a.Uin[n] = c->field(uin + n);
+    a.Uin[n] = c->field((rk2_keeps_no_u1(c) ? F_R : uin) + n);
     a.U0[n] = c->field(F_UA + n);
     a.Uout[n] = c->field(uout + n);
     a.Vout[n] = c->vfield_out(n);
   }
+  a.uin_is_r = rk2_keeps_no_u1(c) ? 1 : 0;
   a.sc = c->sc;
   a.w = w;
   a.w0 = w0;
@@ -1164,10 +1169,6 @@ MhdKernel mhd_kernel(const idfx_ctx* c, bool first, int mode, bool open) {
     default: return mhd_kernel_s<SOLVER_ROE>(c->limiter, first, mode, open);
   }
 }
-
-// RK2 without a stored U_1 (one-kernel stages, no pressure floor): the first stage's update kernel keeps U_1 in registers
-// for the primitives only, and the second stage rebuilds it from U_0 and R_1, which it reads instead of U_1
-bool rk2_keeps_no_u1(const idfx_ctx* c) { return c->mhd && c->fused && c->nstages == 2 && !(c->g.pfloor > 0.0); }
 
 void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int uout, int bin) {
   const Geom& g = c->g;
