@@ -308,7 +308,10 @@ def run_ours(args):
         alu = {"kernel": name, "bound": "alu", "achieved": k["algo_TFLOPs"], "peak": fp64_peak, "unit": "TFLOP/s",
                "frac": k["algo_TFLOPs"] / fp64_peak, "traffic": k.get("ncu_dram_bytes"),
                "peak_source": "148 SMs x 64 fp64 FMA lanes x 2 flops x %.0f MHz (maximum SM clock, MEASURED_PEAKS.json); the DFMA "
-                              "probe of this run is in fp64_probe" % sm_max_mhz, "hbm_frac": hbm["frac"]}
+                              "probe of this run is in fp64_probe" % sm_max_mhz, "hbm_frac": hbm["frac"],
+               # the same algorithmic operations against the instruction rate of the pipe (one operation per instruction, FMA or not):
+               # a code whose operations are mostly not fused cannot exceed 0.5 of the FMA peak above
+               "ops_per_inst_slot_frac": k["algo_TFLOPs"] / (0.5 * fp64_peak)}
         return alu
     if n == 512 and args.workload == "config5":
         traffic = ncu_traffic()   # committed ncu capture of this command, quoted only while csrc/ is unchanged

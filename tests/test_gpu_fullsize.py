@@ -87,6 +87,10 @@ def test_config5_512_windows_against_oracle(idfx, R):
     sim = idfx.Idfx(n, n, n, dx, cfg["gamma"], cfg["solver"], cfg["limiter"], cfg["emf"])
     sim.set_state(prim, b)
     del prim, b
+    c_start, b_start = sim.get_conserved()
+    sums0 = [float(c_start[v].sum()) for v in range(5)] + [float(b_start[d].sum()) for d in range(3)]
+    abs0 = [float(c_start[v].abs().sum()) for v in range(5)] + [float(b_start[d].abs().sum()) for d in range(3)]
+    del c_start, b_start
     rng = np.random.default_rng(5)
     origins = [(0, 0, 0), (n - 16, n - 16, n - 16), (n - 20, 3, 250), (100, n - 12, n - 30)]
     # seams of the launch configuration at 512^3: x tiles start at 31 m (the last, partial one at 496), y tiles at 11 m
@@ -153,7 +157,15 @@ def test_config5_512_windows_against_oracle(idfx, R):
             assert err <= TOL, ("cycle", cycle, "window", o, "bface", err)
         del p0, b0, c1, b1
     assert sim.status() == 0
-    print("config5 512^3: worst relative window error %.3e" % worst)
+    # properties that hold at any size, on the whole box after the 22 cycles: conservation on the periodic box and div B
+    c_end, b_end = sim.get_conserved()
+    sums1 = [float(c_end[v].sum()) for v in range(5)] + [float(b_end[d].sum()) for d in range(3)]
+    for s0, s1, a0 in zip(sums0, sums1, abs0):
+        assert abs(s1 - s0) <= 1e-11 * a0, (s0, s1, a0)     # 1.3e8 cells summed in fp64: ~1e-13 of the absolute sum per pass
+    div = (torch.roll(b_end[0], -1, 2) - b_end[0]) + (torch.roll(b_end[1], -1, 1) - b_end[1]) + (torch.roll(b_end[2], -1, 0) - b_end[2])
+    divb = float(div.abs().max() / b_end.abs().max())
+    assert divb <= 1e-13, divb
+    print("config5 512^3: worst relative window error %.3e; after 22 cycles max|div B| dx / max|B| = %.2e, conserved sums within 1e-11" % (worst, divb))
 
 
 def test_config2_recipe_512_hd_windows_against_oracle(idfx, R):
