@@ -65,6 +65,8 @@ def run_decomposed(idfx, shape, dims, dx, scheme, prim, b, cycles, cfl, periodic
 
 
 CASES = [
+    ((8, 8, 8), (2, 2, 2), (HLLD, VANLEER, EMF_UCT), 2),          # 4^3 sub-boxes: the minimum size, every tile partial
+    ((9, 8, 13), (2, 1, 3), (HLLC, VANLEER, EMF_NONE), 3),
     ((40, 24, 16), (2, 1, 1), (HLLD, VANLEER, EMF_UCT), 2),
     ((40, 24, 16), (1, 2, 1), (HLLD, VANLEER, EMF_UCT), 2),
     ((40, 24, 16), (1, 1, 2), (HLLD, VANLEER, EMF_UCT), 2),
@@ -112,6 +114,7 @@ def test_staged_calls_equal_advance_on_a_periodic_box(idfx):
 
 
 OUTFLOW_CASES = [
+    ((8, 9, 8), (2, 2, 2), (HLLD, MINMOD, EMF_UCT), 2),
     ((40, 24, 16), (2, 1, 1), (HLLD, VANLEER, EMF_UCT), 2),
     ((37, 26, 19), (2, 2, 2), (HLLD, VANLEER, EMF_UCT), 2),
     ((40, 24, 16), (1, 2, 2), (ROE, MINMOD, EMF_ARITH), 3),
