@@ -16,18 +16,24 @@
 // fan-integral identity; HLLC p* continuity; isolated contact and rotational discontinuities; Roe
 // L·R=I, A·r=λr against a finite-difference Jacobian, Σλαr = F_R−F_L; MHD-Roe(B=0) = 5-wave HD Roe;
 // Rusanov = HLL with symmetric speeds; limiter properties; exact Sod solution along x, y, z; direction symmetry; uniform state; conservation;
-// div B; Eᶜ plane-parallel identity; RK2 amplification factor; closed-form dt; 2nd-order convergence of
-// linear fast/Alfvén waves.  Options (tests/test_oracle_options.py): Euler/RK2/RK3 amplification polynomials and temporal
-// order; LimO3 exact for parabolas, bounded at jumps, 3rd-order linear-wave convergence with RK3; vector-potential CT
-// equal to face CT up to rounding with div B that does not accumulate; advance_to lands on t_end.
-// PARITY UNPINNED (the paper fixes none of these and prints no number that depends on them, see
-// DESIGN.md "Readings"): the limiter flavour (G2), the Davis wave-speed estimate (G5), the HLLD
-// degeneracy threshold (G6), the Roe fallback/degenerate-eigenvector conventions (G7), the face→cell
-// mapping of c_max in dt (G8), un-lagged dt (G9), the reference E^c state (G10), and the LimO3 constants
-// (1.6, r = 1, eps = 1e-12; G18: PAPER.md:79 only names the scheme of Cada & Torrilhon 2009), and the composition of the
-// 2D-HLL EMF beyond its plane-parallel limit (G21: PAPER.md:109 only names Mignone & Del Zanna 2021), and the form of the PPM
-// limiter (G22: PAPER.md:79 only names Colella & Woodward 1984 and Colella & Sekora 2008; pinned here by what the
-// construction must do: exact for cubics, smooth extrema kept, steps monotone, fourth-order face values).
+// div B; Eᶜ plane-parallel identity AND its upwind-side rule (test_oracle_emf_upwind.py: domain of dependence of a one-edge
+// potential bump in supersonic flow for every sign quadrant and edge family, donor-cell closed form, field-loop advection,
+// zero mass flux => mean = E^0); RK2 amplification factor; closed-form dt; 2nd-order convergence of
+// linear fast/Alfvén waves.  Options (tests/test_oracle_options.py, test_oracle_emf_hlld2d.py): Euler/RK2/RK3 amplification
+// polynomials and temporal order; LimO3 exact for parabolas, bounded at jumps, 3rd-order linear-wave convergence with RK3;
+// vector-potential CT equal to face CT up to rounding with div B that does not accumulate; advance_to lands on t_end; 2D-HLL and
+// 2D-HLLD EMFs: plane-parallel limit = the 1D HLL / HLLD flux EMF along x, y, z, and for HLLD the coefficient decomposition
+// reproduces the pinned HLLD flux in all six fan regions; outflow boundaries with a magnetic field: Brio-Wu tube stays 1D and
+// equals the periodic double tube away from the ends, fixed point, div B on interior cells.
+// PARITY UNPINNED (the paper fixes none of these CHOICES and prints no number that depends on them, see
+// DESIGN.md "Readings"; each has pins that a wrong implementation of the stated reading fails): the limiter flavour (G2),
+// the Davis wave-speed estimate (G5), the HLLD degeneracy threshold (G6), the Roe fallback/degenerate-eigenvector conventions
+// (G7), the face→cell mapping of c_max in dt (G8), un-lagged dt (G9), the reference state of E^c (G10: -v x Bc of the stage
+// input), the LimO3 constants (1.6, r = 1, eps = 1e-12; G18: PAPER.md:79 only names the scheme of Cada & Torrilhon 2009), the
+// composition of the 2D-HLL and 2D-HLLD EMFs beyond their plane-parallel limit (G21, G24: PAPER.md:109 only names Mignone &
+// Del Zanna 2021), the form of the PPM limiter (G22: PAPER.md:79 only names Colella & Woodward 1984 and Colella & Sekora 2008;
+// pinned here by what the construction must do: exact for cubics, smooth extrema kept, steps monotone, fourth-order face
+// values), and the zero-gradient continuation of the staggered field at outflow boundaries (G23).
 //
 // Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC idfxref.cpp -o libidfxref.so
 #include <algorithm>
