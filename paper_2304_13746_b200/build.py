@@ -4,9 +4,9 @@
 
 Translation units: csrc/idfx.cu (C ABI, state kernels, fused CT/update kernel), csrc/probe.cu, and csrc/stage_inst.cu once
 per (Riemann solver, reconstruction) pair, compiled in parallel as separate nvcc processes.  No -split-compile: with it
-the code nvcc 12.9 generates for the register-bound sweep kernels (where their loads are scheduled, hence 0 to 96 bytes
-of spills) was found to change from one build of the same source to the next and with the core count of the build
-machine; a z sweep at 512^3 then takes 5.8 or 6.9 ms.  One process per unit is deterministic.
+the code nvcc 12.9 generates for register-bound kernels (where their loads are scheduled, hence 0 to 96 bytes
+of spills) was found in round 1 to change from one build of the same source to the next and with the core count of the build
+machine (a 512^3 sweep then took 5.8 or 6.9 ms).  One process per unit is deterministic.
 """
 import os
 import subprocess

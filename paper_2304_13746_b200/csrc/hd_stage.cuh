@@ -3,7 +3,7 @@
 // no intermediate field at all: a CTA of 32 x 8 threads owns a column of (x, y) tiles and marches along z; every z plane
 // of the five primitive fields arrives once, with its two-cell halo, as one TMA box (36 x 11 x 5 doubles) in a 4-stage
 // shared-memory ring.  Thread (lx, ly) owns cell (x0 + lx, y0 + ly) of the plane and solves the three LOWER faces of its
-// cell: the x and y faces from the plane in shared memory, the z face by marching (registers, as in flux_march.cuh).
+// cell: the x and y faces from the plane in shared memory, the z face by marching (left state, forward differences and previous flux in registers).
 // The upper x face comes from lane lx + 1 by shuffle, the upper y face from row ly + 1 through a small double-buffered
 // exchange array, the upper z face one plane later: every Riemann problem inside a tile is solved once.  Lane 31 and
 // row 7 only supply faces (tiles advance by 31 x 7 cells), which costs 15 % of the x/y solves and nothing in HBM traffic.

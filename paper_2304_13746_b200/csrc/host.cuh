@@ -153,7 +153,7 @@ typedef void (*HdKernel)(Geom, HdStageArgs, const CUtensorMap);
 template <int SOLVER, int LIM>
 HdKernel hd_kernel_sl(bool first);
 
-// MHD: the three sweeps of a stage in one kernel (mhd_stage.cuh), same translation units.
+// MHD: the three sweeps and the edge EMFs of a stage in one kernel (mhd_stage.cuh), same translation units.
 typedef void (*MhdKernel)(Geom, MhdStageArgs, const CUtensorMap, const CUtensorMap);
 template <int SOLVER, int LIM>
 MhdKernel mhd_kernel_sl(bool first, int emf_mode, bool open);

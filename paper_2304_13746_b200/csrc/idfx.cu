@@ -263,7 +263,7 @@ struct FluxArgs {
   double* cf;    // c_face
 };
 
-// FMODE 0: fluxes and c_face; 1: c_face only (idfx_compute_dt); 2: what the 2D-HLL EMF needs of the face (G21):
+// FMODE 0: fluxes and c_face; 1: c_face only; 2: what the 2D-HLL EMF needs of the face (G21):
 // F[0] = alpha+ = max(0, S_R), F[1] = alpha- = max(0, -S_L), F[2], F[3] = the HLL-weighted transverse velocities;
 // 3: what the 2D-HLLD EMF needs (G24, hlld_uct_face): F[0] = dirL, F[1] = kL, F[2] = kR, F[3], F[4] = the effective velocities.
 template <int SOLVER, int LIM, bool MHD, int FMODE>
@@ -641,7 +641,7 @@ constexpr int CT_THREADS = CT_TX * CT_TY * CT_ZSPLIT;
 constexpr int CT_MINB = 4;    // CTAs per SM
 constexpr int CT_LX = CT_TX + 1, CT_LY = CT_TY + 1, CT_LZ = CT_TZ + 1;
 
-// UDONE: the conserved state was already combined by the z sweep (stages >= 2); only read it back for the primitives.
+// UDONE: the conserved state was already combined by the stage kernel (stages >= 2); only read it back for the primitives.
 // VP: vector-potential form (Eq. 7-8): the lattice holds the new potential A = w (A_in - dt E) + w0 A_0 instead of E
 // and the face field is B_ref + curl A, so its divergence is one rounding of the face values at any time.
 // NCU: the conserved fields this launch reads are not written by it (the host checks the buffers, launch_ct_v), so
@@ -763,7 +763,7 @@ __global__ void __launch_bounds__(CT_THREADS, CT_MINB) k_ct_update(Geom g, EmfAr
     v[10] = v[2] * v[5] - v[1] * v[6];
     if (!(u[0] > 0.0) || !(v[4] > 0.0)) a.sc->flag = 1;
     const long long gz = g.open ? 0 : (k < NG ? (long long)g.nz * g.sz : (k >= g.nz - NG ? -(long long)g.nz * g.sz : 0));
-    const bool want_ec = a.V[8] != nullptr;  // only the separate sweeps read the reference EMF back
+    const bool want_ec = a.V[8] != nullptr;  // only the PPM path (edge_emf above) reads the reference EMF back
 #pragma unroll
     for (int n = 0; n < 11; ++n)
       if (n < 8 || want_ec) a.V[n][c] = v[n];
@@ -894,48 +894,29 @@ int check_bound(const idfx_ctx* c) {
   return IDFX_OK;
 }
 
-// ---- standalone dt (idfx_compute_dt): signal speeds on every face, then the per-cell sum and the max ----
-template <int LIM, bool MHD>
-void launch_speed_l(idfx_ctx* c, const FluxArgs& a) {
-  k_flux_face<SOLVER_HLL, LIM, MHD, 1><<<blocks_for(c->g.nc, 128), 128, 0, c->stream>>>(c->g, a);
-}
-
+// ---- standalone dt with PPM (idfx_compute_dt; the other reconstructions run their first-stage kernel for its reduction):
+// signal speeds on every face, then the per-cell sum and the max ----
 void launch_speed(idfx_ctx* c, int d, const double* const Bf[3]) {
-  const int ia = d, ib = (d + 1) % 3, ie = (d + 2) % 3;
+  const int ib = (d + 1) % 3, ie = (d + 2) % 3;
   const long long st[3] = {1, c->g.sy, c->g.sz};
-  FluxArgs a;
-  a.q[0] = c->vfield(0);
-  a.q[1] = c->vfield(1 + ia);
-  a.q[2] = c->vfield(1 + ib);
-  a.q[3] = c->vfield(1 + ie);
-  a.q[4] = c->vfield(4);
-  a.q[5] = c->vfield(5 + ib);
-  a.q[6] = c->vfield(5 + ie);
-  a.bn = c->mhd ? Bf[ia] : nullptr;
-  a.sd = st[d];
-  for (int n = 0; n < 7; ++n) a.F[n] = nullptr;
-  a.cf = c->field(F_R + d);  // scratch: R is dead between cycles
+  FluxPpmArgs pa;
+  pa.q[0] = c->vfield(0);
+  pa.q[1] = c->vfield(1 + d);
+  pa.q[2] = c->vfield(1 + ib);
+  pa.q[3] = c->vfield(1 + ie);
+  pa.q[4] = c->vfield(4);
+  pa.q[5] = c->vfield(5 + ib);
+  pa.q[6] = c->vfield(5 + ie);
+  for (int n = 0; n < 7; ++n) pa.F[n] = nullptr;
+  pa.bn = c->mhd ? Bf[d] : nullptr;
+  pa.sd = st[d];
+  pa.dir = d;
+  pa.cf = c->field(F_R + d);  // scratch: R is dead between cycles
+  pa.sg = nullptr;
   LaunchScope ls(c, K_FLUX_X + d);
-  if (c->limiter == LIM_PPM) {
-    FluxPpmArgs pa;
-    for (int n = 0; n < 7; ++n) { pa.q[n] = a.q[n]; pa.F[n] = nullptr; }
-    pa.bn = a.bn; pa.sd = a.sd; pa.dir = d; pa.cf = a.cf; pa.sg = nullptr;
-    const unsigned nb = blocks_for(c->g.nc, 128);
-    if (c->mhd) k_flux_face_ppm<SOLVER_HLL, true, 1><<<nb, 128, 0, c->stream>>>(c->g, pa);
-    else k_flux_face_ppm<SOLVER_HLL, false, 1><<<nb, 128, 0, c->stream>>>(c->g, pa);
-    return;
-  }
-  if (c->mhd) {
-    if (c->limiter == LIM_FLAT) launch_speed_l<LIM_FLAT, true>(c, a);
-    else if (c->limiter == LIM_MINMOD) launch_speed_l<LIM_MINMOD, true>(c, a);
-    else if (c->limiter == LIM_LIMO3) launch_speed_l<LIM_LIMO3, true>(c, a);
-    else launch_speed_l<LIM_VANLEER, true>(c, a);
-  } else {
-    if (c->limiter == LIM_FLAT) launch_speed_l<LIM_FLAT, false>(c, a);
-    else if (c->limiter == LIM_MINMOD) launch_speed_l<LIM_MINMOD, false>(c, a);
-    else if (c->limiter == LIM_LIMO3) launch_speed_l<LIM_LIMO3, false>(c, a);
-    else launch_speed_l<LIM_VANLEER, false>(c, a);
-  }
+  const unsigned nb = blocks_for(c->g.nc, 128);
+  if (c->mhd) k_flux_face_ppm<SOLVER_HLL, true, 1><<<nb, 128, 0, c->stream>>>(c->g, pa);
+  else k_flux_face_ppm<SOLVER_HLL, false, 1><<<nb, 128, 0, c->stream>>>(c->g, pa);
 }
 
 void launch_dtmax(idfx_ctx* c) {
@@ -1100,7 +1081,7 @@ void launch_ct(idfx_ctx* c, dim3 grid, const EmfArgs& ea, const UpdateArgs& a, b
   else launch_ct_v<MODE, false>(c, grid, ea, a, stage2, udone);
 }
 
-// ---- hydrodynamics: the whole stage in one kernel (hd_stage.cuh; instantiated in sweeps_inst.cu) ----
+// ---- hydrodynamics: the whole stage in one kernel (hd_stage.cuh; instantiated in stage_inst.cu) ----
 template <int SOLVER>
 HdKernel hd_kernel_s(int limiter, bool first) {
   switch (limiter) {
@@ -1149,7 +1130,7 @@ void launch_hd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int 
   hd_kernel(c, first)<<<grid, HD_THREADS, HD_SMEM_BYTES, c->stream>>>(g, a, c->mapHD);
 }
 
-// ---- MHD: the three sweeps of a stage in one kernel (mhd_stage.cuh; instantiated in sweeps_inst.cu) ----
+// ---- MHD: the three sweeps and the edge EMFs of a stage in one kernel (mhd_stage.cuh; instantiated in stage_inst.cu) ----
 template <int SOLVER>
 MhdKernel mhd_kernel_s(int limiter, bool first, int mode, bool open) {
   switch (limiter) {

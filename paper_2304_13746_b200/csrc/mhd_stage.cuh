@@ -18,7 +18,7 @@
 //   later stages: U_s = w0 U_0 + w (U_{s-1} - dt/dx R) applied at once (Eq. 9); U_{s-1} and U_0 of the cell are loaded
 //                 ahead of the EMF evaluation and used behind it
 // Per cell and stage the kernel reads 11 doubles and writes 8 (later stages: reads 21), against 57 (67) for the three
-// separate sweeps with their x-flux, partial-divergence, face-flux and sign arrays.
+// separate sweeps of round 1 with their x-flux, partial-divergence, face-flux and sign arrays.
 #pragma once
 #include <cuda.h>
 

@@ -1,5 +1,5 @@
 // tma.cuh — one-line PTX wrappers: mbarrier (init / expect-tx / arrive / parity wait) and the 4D TMA tile load
-// (cp.async.bulk.tensor) that the staged kernels (flux_march_tma.cuh, hd_stage.cuh, mhd_stage.cuh) are built from.
+// (cp.async.bulk.tensor) that the staged kernels (hd_stage.cuh, mhd_stage.cuh) are built from.
 #pragma once
 #include <cuda.h>
 
