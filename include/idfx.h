@@ -108,7 +108,9 @@ int idfx_set_option(idfx_ctx* ctx, int option, int value);
 int idfx_set_option_real(idfx_ctx* ctx, int option, double value);
 int idfx_floor_count(idfx_ctx* ctx, long long* h_count_out); /* synchronises */
 
-/* Device bytes the caller must supply to idfx_bind (internal padded state, stage buffers, fluxes, EMFs). */
+/* Device bytes the caller must supply to idfx_bind (internal padded state, stage buffers, divergence, edge EMFs): 43 padded
+ * fields of (nx + 18 rounded up to 16) * (ny + 4) * (nz + 4) doubles for MHD, 25 for hydrodynamics, more with PPM, the
+ * vector-potential form (choose it first) or the 2D EMFs; DESIGN.md section 6.  No call touches memory outside it. */
 size_t idfx_workspace_bytes(const idfx_ctx* ctx);
 
 /* Binds a caller-owned device workspace (>= idfx_workspace_bytes, 256-byte aligned) and a stream.

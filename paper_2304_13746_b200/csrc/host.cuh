@@ -22,12 +22,13 @@ enum {
   F_BA = 10,   // 3 x 3: face-field buffers that rotate between B0 / B1 / result
   F_BB = 13,
   F_BC = 16,
-  F_V = 19,    // 11: primitives, cell-centred B and Ec = -(v x Bc) of the stage input
-  F_V2 = 30,   // 11: second buffer (MHD: the fused CT/update kernel reads the stage input while writing the result)
-  F_R = 41,    // 5: flux divergence
-  F_FB = 46,   // 6: the edge EMFs E_x, E_y, E_z of the one-kernel MHD stage in the first three; PPM: face fluxes of B, [d][0..1]
-  F_SG = 52,   // 1 slot holding three byte fields: sign of the face mass flux per direction (PPM with E^c only)
-  F_COUNT = 53,
+  // then, at offsets that depend on what the context needs (idfx_ctx::f_v .. f_count; hydrodynamics has no face field,
+  // only PPM reads -(v x Bc), face fluxes of B and sign bytes back from memory):
+  //   V, V2  2 x nv(): primitives, cell-centred B (MHD) and Ec = -(v x Bc) (PPM) of the stage input, double-buffered
+  //          (the update kernels read the stage input of neighbouring tiles while writing the result)
+  //   R      5: flux divergence
+  //   FB     nfb(): the edge EMFs E_x, E_y, E_z of the one-kernel MHD stage in the first three; PPM: face fluxes of B, [d][0..1]
+  //   SG     nsg(): 1 slot holding three byte fields, the sign of the face mass flux per direction (PPM with E^c only)
   // optional groups, appended in this order when present (idfx_ctx::f_aa, f_bref, f_h2d, f_eg):
   //   vector-potential form (idfx_set_option(IDFX_OPT_CT_FORM, IDFX_CT_POTENTIAL)): 3 x 3 edge-potential buffers rotating
   //   like the face-field buffers, and the 3 face fields given to set_state (ghosts filled);
@@ -62,9 +63,19 @@ struct idfx_ctx {
   int nstages = 2;  // Tab. 1: 1 Euler, 2 RK2, 3 RK3
   bool vp = false;  // Eq. 7-8 instead of Eq. 6
   int fixed_batch = 0;  // IDFX_ADVANCE_BATCH: cycles per batch of idfx_advance_to (tests: forces cycles past t_end)
-  int f_aa() const { return F_COUNT; }
-  int f_bref() const { return F_COUNT + 9; }
-  int f_h2d() const { return F_COUNT + (vp ? N_VP : 0); }
+  int nbf() const { return mhd ? 9 : 0; }
+  int nv() const { return mhd ? (limiter == LIM_PPM ? 11 : 8) : 5; }
+  int nfb() const { return limiter == LIM_PPM ? 6 : (mhd ? 3 : 0); }
+  int nsg() const { return limiter == LIM_PPM ? 1 : 0; }
+  int f_v() const { return F_BA + nbf(); }
+  int f_v2() const { return f_v() + nv(); }
+  int f_r() const { return f_v2() + nv(); }
+  int f_fb() const { return f_r() + 5; }
+  int f_sg() const { return f_fb() + nfb(); }
+  int f_count() const { return f_sg() + nsg(); }
+  int f_aa() const { return f_count(); }
+  int f_bref() const { return f_count() + 9; }
+  int f_h2d() const { return f_count() + (vp ? N_VP : 0); }
   bool emf2d() const { return emf == EMF_UCT_HLL || emf == EMF_UCT_HLLD; }  // edge EMFs from their own kernels (k_emf_hll2d)
   int f_eg() const { return f_h2d() + (emf == EMF_UCT_HLLD ? 15 : 12); }
   int f_gen() const { return f_h2d() + (emf == EMF_UCT_HLL ? N_H2D : (emf == EMF_UCT_HLLD ? N_H2D_D : 0)); }
@@ -96,9 +107,9 @@ struct idfx_ctx {
   long long prof_n[K_COUNT] = {0};
   double* field(int slot) const { return ws + (size_t)slot * (size_t)g.np; }
   double* bbuf(int which, int d) const { return field(F_BA + 3 * which + d); }
-  signed char* sgn(int d) const { return (signed char*)field(F_SG) + (size_t)d * (size_t)g.np; }
-  double* vfield(int n) const { return field((vcur ? F_V2 : F_V) + n); }
-  double* vfield_out(int n) const { return field((vcur ? F_V : F_V2) + n); }
+  signed char* sgn(int d) const { return (signed char*)field(f_sg()) + (size_t)d * (size_t)g.np; }
+  double* vfield(int n) const { return field((vcur ? f_v2() : f_v()) + n); }
+  double* vfield_out(int n) const { return field((vcur ? f_v() : f_v2()) + n); }
 };
 
 namespace idfx {

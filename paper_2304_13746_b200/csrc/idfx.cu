@@ -187,7 +187,7 @@ __global__ void k_cons_from_prim(Geom g, StateArgs a) {
     a.V[7][c] = bz;
   }
   const double rho = a.V[0][c], vx = a.V[1][c], vy = a.V[2][c], vz = a.V[3][c], p = a.V[4][c];
-  if (MHD) {
+  if (MHD && a.V[8]) {  // only PPM keeps -(v x Bc) in memory
     a.V[8][c] = vz * by - vy * bz;
     a.V[9][c] = vx * bz - vz * bx;
     a.V[10][c] = vy * bx - vx * by;
@@ -834,9 +834,9 @@ int make_tensor_maps(idfx_ctx* c) {
   const cuuint64_t strides[3] = {(cuuint64_t)g.sy * 8, (cuuint64_t)g.sz * 8, (cuuint64_t)g.np * 8};
   const cuuint32_t es[4] = {1, 1, 1, 1};
   if (!c->mhd) {
-    const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, 22};
+    const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, (cuuint64_t)(2 * c->nv())};
     const cuuint32_t box[4] = {(cuuint32_t)HD_BW, (cuuint32_t)HD_BH, 1u, 5u};
-    CUresult r = enc(&c->mapHD, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_V), dimV, strides, box, es,
+    CUresult r = enc(&c->mapHD, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(c->f_v()), dimV, strides, box, es,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
@@ -846,9 +846,9 @@ int make_tensor_maps(idfx_ctx* c) {
     return IDFX_OK;
   }
   {
-    const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, 22}, dimB[4] = {(cuuint64_t)g.sy, py, pz, 9};
+    const cuuint64_t dimV[4] = {(cuuint64_t)g.sy, py, pz, (cuuint64_t)(2 * c->nv())}, dimB[4] = {(cuuint64_t)g.sy, py, pz, 9};
     const cuuint32_t boxV[4] = {(cuuint32_t)MS_BW, (cuuint32_t)MS_BH, 1u, 8u}, boxB[4] = {(cuuint32_t)MS_BWB, (cuuint32_t)MS_TY, 1u, 3u};
-    CUresult r1 = enc(&c->mapMV, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_V), dimV, strides, boxV, es,
+    CUresult r1 = enc(&c->mapMV, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(c->f_v()), dimV, strides, boxV, es,
                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     CUresult r2 = enc(&c->mapMB, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_BA), dimB, strides, boxB, es,
@@ -911,7 +911,7 @@ void launch_speed(idfx_ctx* c, int d, const double* const Bf[3]) {
   pa.bn = c->mhd ? Bf[d] : nullptr;
   pa.sd = st[d];
   pa.dir = d;
-  pa.cf = c->field(F_R + d);  // scratch: R is dead between cycles
+  pa.cf = c->field(c->f_r() + d);  // scratch: R is dead between cycles
   pa.sg = nullptr;
   LaunchScope ls(c, K_FLUX_X + d);
   const unsigned nb = blocks_for(c->g.nc, 128);
@@ -923,7 +923,7 @@ void launch_dtmax(idfx_ctx* c) {
   RhsArgs a;
   for (int d = 0; d < 3; ++d) {
     for (int n = 0; n < 5; ++n) a.F[d][n] = nullptr;
-    a.cf[d] = c->field(F_R + d);
+    a.cf[d] = c->field(c->f_r() + d);
   }
   for (int n = 0; n < 5; ++n) a.R[n] = nullptr;
   a.sc = c->sc;
@@ -955,15 +955,15 @@ void launch_ppm_s(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
       a.F[n] = c->field(c->f_gen() + 5 * d + n);
       r.F[d][n] = a.F[n];
     }
-    a.F[5] = c->field(F_FB + 2 * d);
-    a.F[6] = c->field(F_FB + 2 * d + 1);
+    a.F[5] = c->field(c->f_fb() + 2 * d);
+    a.F[6] = c->field(c->f_fb() + 2 * d + 1);
     a.cf = c->field(c->f_gen() + 15 + d);
     r.cf[d] = a.cf;
     a.sg = c->emf == EMF_UCT ? c->sgn(d) : nullptr;
     LaunchScope ls(c, K_FLUX_X + d);
     k_flux_face_ppm<SOLVER, MHD, 0><<<nb, 128, 0, c->stream>>>(g, a);
   }
-  for (int n = 0; n < 5; ++n) r.R[n] = c->field(F_R + n);
+  for (int n = 0; n < 5; ++n) r.R[n] = c->field(c->f_r() + n);
   r.sc = c->sc;
   LaunchScope ls(c, K_RHS);
   if (want_dt) k_rhs<true, true><<<nb, 128, 0, c->stream>>>(g, r);
@@ -987,12 +987,12 @@ void launch_ppm(idfx_ctx* c, const double* const Bf[3], bool want_dt) {
 EmfArgs emf_args(idfx_ctx* c) {
   EmfArgs a;
   for (int d = 0; d < 3; ++d) {
-    a.FB[d][0] = c->field(F_FB + 2 * d);
-    a.FB[d][1] = c->field(F_FB + 2 * d + 1);
+    a.FB[d][0] = c->field(c->f_fb() + 2 * d);
+    a.FB[d][1] = c->field(c->f_fb() + 2 * d + 1);
     a.SG[d] = c->sgn(d);
-    a.Ec[d] = c->vfield(8 + d);
+    a.Ec[d] = c->nv() > 8 ? c->vfield(8 + d) : nullptr;
     // edge EMFs already evaluated: by k_emf_hll2d (2D-HLL), or by the one-kernel stage (mhd_stage.cuh)
-    a.Eg[d] = c->emf2d() ? c->field(c->f_eg() + d) : (c->fused ? c->field(F_FB + d) : nullptr);
+    a.Eg[d] = c->emf2d() ? c->field(c->f_eg() + d) : (c->fused ? c->field(c->f_fb() + d) : nullptr);
   }
   return a;
 }
@@ -1047,7 +1047,7 @@ void launch_hll2d(idfx_ctx* c, const double* const Bf[3]) {
 void launch_fill(idfx_ctx* c, int which_b) {
   FieldList fl;
   fl.n = 0;
-  for (int n = 0; n < (c->mhd ? 11 : 5); ++n) fl.f[fl.n++] = c->vfield(n);
+  for (int n = 0; n < c->nv(); ++n) fl.f[fl.n++] = c->vfield(n);
   if (c->mhd)
     for (int d = 0; d < 3; ++d) fl.f[fl.n++] = c->bbuf(which_b, d);
   const Geom& g = c->g;
@@ -1108,15 +1108,15 @@ bool rk2_keeps_no_u1(const idfx_ctx* c) { return c->fused && c->nstages == 2 && 
 void launch_hd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int uout) {
   const Geom& g = c->g;
   HdStageArgs a;
-  a.fV0 = c->vcur ? 11 : 0;
+  a.fV0 = c->vcur ? c->nv() : 0;
   const long long per_chunk = (long long)((g.nx + HD_CX - 1) / HD_CX) * ((g.ny + HD_CY - 1) / HD_CY);
   long long nch = (148 * 2 * 8 + per_chunk - 1) / per_chunk;  // about 8 waves of 2 CTAs per SM
   const long long maxch = g.nz / 16 > 0 ? g.nz / 16 : 1;
   nch = nch < 1 ? 1 : (nch > maxch ? maxch : nch);
   a.chunk = (int)((g.nz + nch - 1) / nch);
   for (int n = 0; n < 5; ++n) {
-    a.R[n] = c->field(F_R + n);
-    a.Uin[n] = c->field((rk2_keeps_no_u1(c) ? F_R : uin) + n);
+    a.R[n] = c->field(c->f_r() + n);
+    a.Uin[n] = c->field((rk2_keeps_no_u1(c) ? c->f_r() : uin) + n);
     a.U0[n] = c->field(F_UA + n);
     a.Uout[n] = c->field(uout + n);
     a.Vout[n] = c->vfield_out(n);
@@ -1154,7 +1154,7 @@ MhdKernel mhd_kernel(const idfx_ctx* c, bool first, int mode, bool open) {
 void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int uout, int bin) {
   const Geom& g = c->g;
   MhdStageArgs a;
-  a.fV0 = c->vcur ? 11 : 0;
+  a.fV0 = c->vcur ? c->nv() : 0;
   a.fB0 = 3 * bin;
   // along an open direction the tiles start at cell -1 (mhd_stage.cuh)
   const int tx = (g.nx + (g.open & 1) + MS_CX - 1) / MS_CX, ty = (g.ny + ((g.open >> 1) & 1) + MS_CY - 1) / MS_CY;
@@ -1177,13 +1177,13 @@ void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int
     }
   a.chunk = (int)((g.nz + nch - 1) / nch);
   for (int n = 0; n < 5; ++n) {
-    a.R[n] = c->field(F_R + n);
-    a.Uin[n] = c->field((rk2_keeps_no_u1(c) ? F_R : uin) + n);
+    a.R[n] = c->field(c->f_r() + n);
+    a.Uin[n] = c->field((rk2_keeps_no_u1(c) ? c->f_r() : uin) + n);
     a.U0[n] = c->field(F_UA + n);
     a.Uout[n] = c->field(uout + n);
   }
   a.uin_is_r = rk2_keeps_no_u1(c) ? 1 : 0;
-  for (int d = 0; d < 3; ++d) a.E[d] = c->field(F_FB + d);  // the edge lattice lives in the first three face-flux slots
+  for (int d = 0; d < 3; ++d) a.E[d] = c->field(c->f_fb() + d);  // the edge lattice lives in the first three face-flux slots
   a.sc = c->sc;
   a.w = w;
   a.w0 = w0;
@@ -1266,7 +1266,7 @@ void stage_update(idfx_ctx* c, int s) {
   for (int n = 0; n < 5; ++n) {
     a.Uin[n] = c->field(p.uin + n);
     a.U0[n] = c->field(F_UA + n);
-    a.R[n] = c->field(F_R + n);
+    a.R[n] = c->field(c->f_r() + n);
     a.Uout[n] = c->field(p.uout + n);
   }
   for (int d = 0; d < 3; ++d) {
@@ -1288,9 +1288,8 @@ void stage_update(idfx_ctx* c, int s) {
     // CT + RK combine + cons->prim + ghost images in one kernel; V is double-buffered because neighbouring tiles still
     // read the stage-input primitives while this tile writes the result's
     const EmfArgs ea = emf_args(c);
-    for (int n = 0; n < 11; ++n) a.V[n] = c->vfield_out(n);
-    if (c->fused)  // the one-kernel stage forms -(v x Bc) itself
-      for (int n = 8; n < 11; ++n) a.V[n] = nullptr;
+    // -(v x Bc) is stored for PPM only: the one-kernel stage forms it itself
+    for (int n = 0; n < 11; ++n) a.V[n] = n < c->nv() ? c->vfield_out(n) : nullptr;
     dim3 grid((g.nx + CT_TX - 1) / CT_TX, (g.ny + CT_TY - 1) / CT_TY, (g.nz + CT_TZ - 1) / CT_TZ);
     const bool udone = p.combine && c->fused;  // the one-kernel stage applied the divergence itself
     if (c->emf2d()) {
@@ -1307,7 +1306,7 @@ void stage_update(idfx_ctx* c, int s) {
     c->vcur ^= 1;
     if (g.open && !c->exch) launch_fill(c, p.bout);  // no images were written
   } else {
-    for (int n = 0; n < 11; ++n) a.V[n] = c->vfield(n);
+    for (int n = 0; n < 11; ++n) a.V[n] = n < c->nv() ? c->vfield(n) : nullptr;
     {
       LaunchScope ls(c, K_UPDATE);
       if (p.combine) k_update_hd<true><<<blocks_for(g.nc, 128), 128, 0, c->stream>>>(g, a);
@@ -1363,7 +1362,7 @@ int reset_clock(idfx_ctx* c) {
 int finish_set_state(idfx_ctx* c) {
   StateArgs a;
   for (int n = 0; n < 5; ++n) a.U[n] = c->field(F_UA + n);
-  for (int n = 0; n < 11; ++n) a.V[n] = c->vfield(n);
+  for (int n = 0; n < 11; ++n) a.V[n] = n < c->nv() ? c->vfield(n) : nullptr;
   for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
   a.sc = c->sc;
   const unsigned nb = blocks_for(c->g.nc, 128);
@@ -1389,7 +1388,7 @@ int refresh_prims(idfx_ctx* c) {
   StateArgs a;
   for (int n = 0; n < 5; ++n) a.U[n] = c->field(F_UA + n);
   for (int n = 0; n < 11; ++n) a.V[n] = nullptr;
-  for (int n = 0; n < 5; ++n) a.V[n] = c->field(F_R + n);  // scratch: R is dead between cycles
+  for (int n = 0; n < 5; ++n) a.V[n] = c->field(c->f_r() + n);  // scratch: R is dead between cycles
   for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
   a.sc = c->sc;
   const unsigned nb = blocks_for(c->g.nc, 128);
@@ -1583,7 +1582,7 @@ int idfx_get_state(idfx_ctx* c, double* d_prim, double* d_bface) {
   const unsigned nb = blocks_for(c->g.nc, 128);
   FieldList fl;
   fl.n = 5;
-  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(F_R + n);
+  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(c->f_r() + n);
   { LaunchScope ls(c, K_STATE);
   k_unpack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_prim);
   }
@@ -1608,7 +1607,7 @@ int idfx_get_state_host(idfx_ctx* c, double* h_prim, double* h_bface) {
   }
   if ((rc = refresh_prims(c))) return rc;
   for (int n = 0; n < 5; ++n)
-    if ((rc = copy3d(c, c->field(F_R + n), nullptr, h_prim + (size_t)n * c->g.nc, cudaMemcpyDeviceToHost))) return rc;
+    if ((rc = copy3d(c, c->field(c->f_r() + n), nullptr, h_prim + (size_t)n * c->g.nc, cudaMemcpyDeviceToHost))) return rc;
   if (c->mhd && h_bface)
     for (int d = 0; d < 3; ++d)
       if ((rc = copy3d(c, c->bbuf(c->bcur, d), nullptr, h_bface + (size_t)d * c->g.nc, cudaMemcpyDeviceToHost)))
@@ -1955,8 +1954,7 @@ size_t idfx_dt_reduce_offset(const idfx_ctx* c) {
 static FieldList halo_fields(const idfx_ctx* c) {
   FieldList fl;
   fl.n = 0;
-  const int nv = c->mhd ? (c->fused ? 8 : 11) : 5;
-  for (int n = 0; n < nv; ++n) fl.f[fl.n++] = c->vfield(n);
+  for (int n = 0; n < c->nv(); ++n) fl.f[fl.n++] = c->vfield(n);
   if (c->mhd)
     for (int d = 0; d < 3; ++d) fl.f[fl.n++] = c->bbuf(c->cyc_bin, d);
   return fl;
