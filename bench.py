@@ -36,9 +36,11 @@ ALGO_FLOPS_PER_CELL = {"mhd_stage": 3 * 360.0 + 3 * 42.0 + 9.0 + 25.0 + 10.0}
 #   ct_update_prim stage 1: R5 U_0 5 Bin3 E3 | B3 V8 (27; U_1 is not stored);  stage 2: U5 Bin3 B0 3 E3 | B3 V8 (25)
 # = 100 doubles = 800 B per cell-update for the whole cycle.
 ALGO_BYTES_PER_CELL = {"mhd_stage": 8 * 24.0, "ct_update_prim": 8 * 26.0}
-# HD (config 2, sedov): the whole stage is one kernel (csrc/hd_stage.cuh): stage 1 reads V5, writes R5 (10 doubles); later
-# stages read V5 U1 5 U0 5 and write U5 V5 (25); mean 17.5.  The stage-1 update kernel reads U5 R5 and writes U5 V5 (20).
-ALGO_BYTES_PER_CELL_HD = {"hd_stage": 8 * 17.5, "ct_update_prim": 8 * 20.0}
+# HD (config 2, sedov): RK2 cycles on a periodic box read the conserved fields (csrc/hd_stage_u.cuh): stage 1 reads U_0 5 and
+# writes R_1 5 (10 doubles), stage 2 reads U_0 5 R_1 5 and writes U5 (15); mean 12.5 = the 25 doubles of SURVEY.md §8(d) per
+# cell-update.  (The first cycle after set_state and the other integrators go through csrc/hd_stage.cuh and k_update_hd:
+# 10 + 25 + 15 doubles.)
+ALGO_BYTES_PER_CELL_HD = {"hd_stage": 8 * 12.5, "ct_update_prim": 8 * 15.0}
 ALGO_BYTES_PER_CELL_UPDATE_HD = 200.0       # 25 doubles per HD cell-update
 # fp64 issue peak of the board: 148 SMs x 64 fp64 FMA lanes x 2 flops x the maximum SM clock
 FP64_LANES = 148 * 64

@@ -60,6 +60,26 @@ __device__ __forceinline__ double block_max_hd(double v) {
   return m;
 }
 
+// The pointwise arithmetic of the hydrodynamic update, written with explicit roundings: three kernels form the same
+// quantities (k_update_hd, k_hd_stage, k_hd_stage_u) and must get the same bits whatever the compiler would contract around
+// them, so that the two kinds of cycle (and decomposed against undecomposed runs) stay interchangeable bit for bit.
+// a5 of the first stage: U_1 = U_0 - dt/dx R_1
+__device__ __forceinline__ double hd_apply(double u0, double dtdx, double r) { return __fma_rn(-dtdx, r, u0); }
+// Eq. 9: U_s = w0 U_0 + w (U_{s-1} - dt/dx R)
+__device__ __forceinline__ double hd_combine(double w0, double u0, double w, double us, double dtdx, double r) {
+  return __fma_rn(w0, u0, __dmul_rn(w, __fma_rn(-dtdx, r, us)));
+}
+// a2: (rho, v, p) of (rho, m, E)
+__device__ __forceinline__ void hd_prims(double gm1, const double u[5], double v[5]) {
+  const double ir = __ddiv_rn(1.0, u[0]);
+  v[0] = u[0];
+  v[1] = __dmul_rn(u[1], ir);
+  v[2] = __dmul_rn(u[2], ir);
+  v[3] = __dmul_rn(u[3], ir);
+  const double v2 = __fma_rn(v[3], v[3], __fma_rn(v[2], v[2], __dmul_rn(v[1], v[1])));
+  v[4] = __dmul_rn(gm1, __fma_rn(__dmul_rn(-0.5, u[0]), v2, u[4]));
+}
+
 // Lower face of the cell whose stencil (two cells below, one above, along one direction) is q[0..3][5 fields] in the
 // sweep's local order (rho, u_n, u_t1, u_t2, p); returns c_face.
 template <int SOLVER, int LIM>
@@ -213,12 +233,13 @@ __global__ void __launch_bounds__(HD_THREADS, HD_MINB) k_hd_stage(Geom g, HdStag
         for (int n = 0; n < 5; ++n) {
           const double u0 = a.U0[n][cu];
           const double uin = a.Uin[n][cu];
-          const double us = a.uin_is_r ? u0 - dtdx * uin : uin;
-          u[n] = dtdx == 0.0 ? u0 : a.w0 * u0 + a.w * (us - dtdx * rt[n]);  // Eq. 9
+          const double us = a.uin_is_r ? hd_apply(u0, dtdx, uin) : uin;
+          u[n] = dtdx == 0.0 ? u0 : hd_combine(a.w0, u0, a.w, us, dtdx, rt[n]);  // Eq. 9
         }
-        const double ir = 1.0 / u[0];
-        const double vx = u[1] * ir, vy = u[2] * ir, vz = u[3] * ir;
-        double pr = (g.gamma - 1.0) * (u[4] - 0.5 * u[0] * (vx * vx + vy * vy + vz * vz));
+        double v[5];
+        hd_prims(g.gamma - 1.0, u, v);
+        const double vx = v[1], vy = v[2], vz = v[3];
+        double pr = v[4];
         if (g.pfloor > 0.0 && pr < g.pfloor) {
           const bool acts = pr < g.pfloor * (1.0 - 1e-9);  // a cell floored before recomputes to the floor within rounding
           pr = g.pfloor;
@@ -230,7 +251,7 @@ __global__ void __launch_bounds__(HD_THREADS, HD_MINB) k_hd_stage(Geom g, HdStag
         if (!(u[0] > 0.0) || !(pr > 0.0)) a.sc->flag = 1;
 #pragma unroll
         for (int n = 0; n < 5; ++n) a.Uout[n][cu] = u[n];
-        const double v[5] = {u[0], vx, vy, vz, pr};
+        v[4] = pr;
         const int k = s - 1;
         const long long gz = k < NG ? (long long)g.nz * g.sz : (k >= g.nz - NG ? -(long long)g.nz * g.sz : 0);
 #pragma unroll

@@ -11,14 +11,15 @@
 #include "common.cuh"
 #include "physics.cuh"
 #include "hd_stage.cuh"
+#include "hd_stage_u.cuh"
 #include "mhd_stage.cuh"
 
 namespace idfx {
 
 // field slots in the workspace
 enum {
-  F_UA = 0,    // 5: conserved state at the start of the cycle (and its result)
-  F_UB = 5,    // 5: stage-1 state
+  F_UA = 0,    // 5 + 5: conserved state at the start of the cycle (and its result), and the stage-1 state (RK3) or the
+  F_UB = 5,    //        result of a hydrodynamic cycle fed with the conserved fields; idfx_ctx::f_u / f_ub say which is which
   F_BA = 10,   // 3 x 3: face-field buffers that rotate between B0 / B1 / result
   F_BB = 13,
   F_BC = 16,
@@ -88,14 +89,26 @@ struct idfx_ctx {
   int cyc_b0 = 0, cyc_bin = 0;  // saved face buffer; face buffer of the next stage's input (= bcur between cycles)
   int bcur = 0;  // which of the three face-field buffers holds the current state
   int vcur = 0;  // which primitive buffer holds the stage input
-  int graph_bnext[6] = {0, 0, 0, 0, 0, 0}, graph_vnext[6] = {0, 0, 0, 0, 0, 0};  // rotation state a replayed cycle leaves
-  // one captured CUDA graph per buffer rotation state (3 face-field rotations x 2 primitive buffers)
-  cudaGraphExec_t graph[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-  long long graph_launches[6] = {0, 0, 0, 0, 0, 0};
+  // one captured CUDA graph per buffer rotation state (3 face-field rotations x 2 primitive buffers) and one for the
+  // hydrodynamic cycle fed with the conserved fields per role of the two conserved buffers
+  static constexpr int N_GRAPHS = 8;
+  int graph_bnext[N_GRAPHS] = {0}, graph_vnext[N_GRAPHS] = {0};  // rotation state a replayed cycle leaves
+  int graph_ucur[N_GRAPHS] = {0};                                // conserved-buffer roles a graph was captured with
+  cudaGraphExec_t graph[N_GRAPHS] = {nullptr};
+  long long graph_launches[N_GRAPHS] = {0};
   double graph_cfl = 0.0;
   bool use_graph = true;
   bool fused = false;              // one kernel per stage (hd_stage.cuh, mhd_stage.cuh): every reconstruction but PPM
   CUtensorMap mapHD;               // HD: 36 x 11 x 1 x 5 boxes over the primitive fields
+  CUtensorMap mapHU, mapHR;        // the same boxes over U_A and over R (hd_stage_u.cuh)
+  // hydrodynamic RK2 cycles fed with the conserved fields (hd_stage_u.cuh) never write the primitive buffers:
+  bool v_given = true;    // V holds the caller's primitives (set_state): the next cycle reconstructs from exactly those
+  bool v_stale = false;   // V is older than U_A
+  bool ug_valid = false;  // the ghost layers of U_A hold its periodic images
+  bool cyc_ufed = false;  // the running cycle is of that kind
+  int ucur = 0;           // which conserved buffer holds the state (only those cycles swap them)
+  int f_u() const { return ucur ? F_UB : F_UA; }
+  int f_ub() const { return ucur ? F_UA : F_UB; }
   CUtensorMap mapMV, mapMB;        // MHD: 36 x (TY+3) x 1 x 8 boxes over the primitives, 34 x TY x 1 x 3 over the face-field buffers
   long long launches = 0;
   // optional per-kernel timing with CUDA events on the bound stream (idfx_profile_*)
@@ -163,6 +176,10 @@ inline unsigned blocks_for(long long n, int bs) { return (unsigned)((n + bs - 1)
 typedef void (*HdKernel)(Geom, HdStageArgs, const CUtensorMap);
 template <int SOLVER, int LIM>
 HdKernel hd_kernel_sl(bool first);
+
+typedef void (*HdKernelU)(Geom, HdStageArgs, const CUtensorMap, const CUtensorMap);
+template <int SOLVER, int LIM>
+HdKernelU hd_kernel_u_sl(bool first);
 
 // MHD: the three sweeps and the edge EMFs of a stage in one kernel (mhd_stage.cuh), same translation units.
 typedef void (*MhdKernel)(Geom, MhdStageArgs, const CUtensorMap, const CUtensorMap);

@@ -49,35 +49,40 @@ __global__ void k_unpack(Geom g, FieldList srcf, double* __restrict__ dst) {
 // a1: ghost fill of a list of fields, one thread per ghost cell.  Periodic: every ghost cell copies from its
 // wrapped active image, which equals the sequential x, y, z fill of O2 (i).  Outflow (HD only): from the
 // nearest active cell, which equals the sequential zero-gradient fill.
-__global__ void k_fill_ghost(Geom g, FieldList fl) {
-  const int px = g.nx + 2 * NG, py = g.ny + 2 * NG;
-  const long long nZ = 2LL * NG * py * px;             // k in ghost
-  const long long nY = (long long)g.nz * 2 * NG * px;  // k active, j in ghost
-  const long long nX = (long long)g.nz * g.ny * 2 * NG;
-  long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+// T: unsigned int wherever the count of ghost cells fits (64-bit divisions cost an order of magnitude more).
+template <typename T>
+__device__ __forceinline__ void fill_ghost_cell(const Geom& g, const FieldList& fl) {
+  const T px = (T)(g.nx + 2 * NG), py = (T)(g.ny + 2 * NG);
+  const T nZ = (T)(2 * NG) * py * px;             // k in ghost
+  const T nY = (T)g.nz * (T)(2 * NG) * px;        // k active, j in ghost
+  const T nX = (T)g.nz * (T)g.ny * (T)(2 * NG);
+  T t = (T)blockIdx.x * (T)blockDim.x + (T)threadIdx.x;
   int i, j, k;
   if (t < nZ) {
     i = (int)(t % px) - NG;
-    const long long r = t / px;
+    const T r = t / px;
     j = (int)(r % py) - NG;
     const int kk = (int)(r / py);
     k = kk < NG ? kk - NG : g.nz + kk - NG;
   } else if ((t -= nZ) < nY) {
     i = (int)(t % px) - NG;
-    const long long r = t / px;
-    const int jj = (int)(r % (2 * NG));
+    const T r = t / px;
+    const int jj = (int)(r % (T)(2 * NG));
     j = jj < NG ? jj - NG : g.ny + jj - NG;
-    k = (int)(r / (2 * NG));
+    k = (int)(r / (T)(2 * NG));
   } else if ((t -= nY) < nX) {
-    const int ii = (int)(t % (2 * NG));
+    const int ii = (int)(t % (T)(2 * NG));
     i = ii < NG ? ii - NG : g.nx + ii - NG;
-    const long long r = t / (2 * NG);
-    j = (int)(r % g.ny);
-    k = (int)(r / g.ny);
+    const T r = t / (T)(2 * NG);
+    j = (int)(r % (T)g.ny);
+    k = (int)(r / (T)g.ny);
   } else {
     return;
   }
-  int is = (i + g.nx) % g.nx, js = (j + g.ny) % g.ny, ks = (k + g.nz) % g.nz;
+  // the wrapped active image (extents are at least 2 NG, so one box length is enough)
+  int is = i < 0 ? i + g.nx : (i >= g.nx ? i - g.nx : i);
+  int js = j < 0 ? j + g.ny : (j >= g.ny ? j - g.ny : j);
+  int ks = k < 0 ? k + g.nz : (k >= g.nz ? k - g.nz : k);
   if (g.outflow) {  // zero gradient: the nearest active cell
     is = min(max(i, 0), g.nx - 1);
     js = min(max(j, 0), g.ny - 1);
@@ -85,6 +90,23 @@ __global__ void k_fill_ghost(Geom g, FieldList fl) {
   }
   const long long d = g.at(i, j, k), s = g.at(is, js, ks);
   for (int n = 0; n < fl.n; ++n) fl.f[n][d] = fl.f[n][s];
+}
+
+template <typename T>
+__global__ void k_fill_ghost(Geom g, FieldList fl) {
+  fill_ghost_cell<T>(g, fl);
+}
+
+// the same fill after the first stage of a cycle whose stages read the conserved fields (hd_stage_u.cuh): there is no update
+// kernel between the stages, so one thread of this launch publishes the dt the reduction of the stage just found
+template <typename T>
+__global__ void k_fill_ghost_dt(Geom g, FieldList fl, DevScalars* sc, double dt_fixed, double cfl) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    bool lands;
+    const double dt = first_stage_dt(sc, dt_fixed, cfl, lands);
+    publish_dt(sc, dt, lands);
+  }
+  fill_ghost_cell<T>(g, fl);
 }
 
 // a1 one direction and one side at a time ("sequential x -> y -> z exchange", the order that also gets
@@ -240,7 +262,14 @@ __global__ void k_prim_from_cons(Geom g, StateArgs a) {
   }
   double vx, vy, vz, p;
   const double rho = a.U[0][c];
-  prim_from_cons(g.gamma - 1.0, rho, a.U[1][c], a.U[2][c], a.U[3][c], a.U[4][c], bx, by, bz, vx, vy, vz, p);
+  if (MHD) {
+    prim_from_cons(g.gamma - 1.0, rho, a.U[1][c], a.U[2][c], a.U[3][c], a.U[4][c], bx, by, bz, vx, vy, vz, p);
+  } else {  // the bits the stage kernels form (hd_stage.cuh)
+    const double u[5] = {rho, a.U[1][c], a.U[2][c], a.U[3][c], a.U[4][c]};
+    double v[5];
+    hd_prims(g.gamma - 1.0, u, v);
+    vx = v[1], vy = v[2], vz = v[3], p = v[4];
+  }
   if (g.pfloor > 0.0 && p < g.pfloor) p = g.pfloor;  // a floored cell recomputes to the floor within rounding
   a.V[0][c] = rho;
   a.V[1][c] = vx;
@@ -613,12 +642,14 @@ __global__ void __launch_bounds__(128, 16) k_update_hd(Geom g, UpdateArgs a) {  
   double u[5];
 #pragma unroll
   for (int n = 0; n < 5; ++n) {
-    const double us = a.Uin[n][c] - dtdx * a.R[n][c];
-    u[n] = STAGE2 ? (dt == 0.0 ? a.U0[n][c] : a.w0 * a.U0[n][c] + a.w * us) : us;
+    // (the pointwise arithmetic of hd_stage.cuh: the stage kernels form the same quantities and must get the same bits)
+    if (STAGE2) u[n] = dt == 0.0 ? a.U0[n][c] : hd_combine(a.w0, a.U0[n][c], a.w, a.Uin[n][c], dtdx, a.R[n][c]);
+    else u[n] = hd_apply(a.Uin[n][c], dtdx, a.R[n][c]);
     if (STAGE2 || a.store_u) a.Uout[n][c] = u[n];
   }
-  double vx, vy, vz, p;
-  prim_from_cons(g.gamma - 1.0, u[0], u[1], u[2], u[3], u[4], 0.0, 0.0, 0.0, vx, vy, vz, p);
+  double v[5];
+  hd_prims(g.gamma - 1.0, u, v);
+  double vx = v[1], vy = v[2], vz = v[3], p = v[4];
   if (pressure_floor(g, a.sc, u[0], vx, vy, vz, 0.0, 0.0, 0.0, p, u[4])) a.Uout[4][c] = u[4];
   if (!(u[0] > 0.0) || !(p > 0.0)) a.sc->flag = 1;
   a.V[0][c] = u[0];
@@ -839,7 +870,14 @@ int make_tensor_maps(idfx_ctx* c) {
     CUresult r = enc(&c->mapHD, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(c->f_v()), dimV, strides, box, es,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
+    const cuuint64_t dimU[4] = {(cuuint64_t)g.sy, py, pz, 5}, dimUU[4] = {(cuuint64_t)g.sy, py, pz, 10};
+    CUresult ru = enc(&c->mapHU, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(F_UA), dimUU, strides, box, es,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult rr = enc(&c->mapHR, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->field(c->f_r()), dimU, strides, box, es,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS || ru != CUDA_SUCCESS || rr != CUDA_SUCCESS) {
       set_err("cuTensorMapEncodeTiled failed");
       return IDFX_ERR_CUDA;
     }
@@ -863,7 +901,7 @@ int make_tensor_maps(idfx_ctx* c) {
 }
 
 void drop_graphs(idfx_ctx* c) {
-  for (int k = 0; k < 6; ++k) {
+  for (int k = 0; k < idfx_ctx::N_GRAPHS; ++k) {
     if (c->graph[k]) cudaGraphExecDestroy(c->graph[k]);
     c->graph[k] = nullptr;
   }
@@ -1044,17 +1082,37 @@ void launch_hll2d(idfx_ctx* c, const double* const Bf[3]) {
   }
 }
 
+// a1 of a list of fields; publish: also the dt of the running cycle (k_fill_ghost_dt)
+void launch_fill_list(idfx_ctx* c, const FieldList& fl, bool publish) {
+  const Geom& g = c->g;
+  const long long px = g.nx + 2 * NG, py = g.ny + 2 * NG;
+  const long long nt = 2LL * NG * py * px + (long long)g.nz * 2 * NG * px + (long long)g.nz * g.ny * 2 * NG;
+  const unsigned nb = blocks_for(nt, 128);
+  LaunchScope ls(c, K_FILL);
+  if (nt + 128 < (1LL << 31)) {
+    if (publish) k_fill_ghost_dt<unsigned int><<<nb, 128, 0, c->stream>>>(g, fl, c->sc, c->cyc_dt_fixed, c->cyc_cfl);
+    else k_fill_ghost<unsigned int><<<nb, 128, 0, c->stream>>>(g, fl);
+  } else {
+    if (publish) k_fill_ghost_dt<long long><<<nb, 128, 0, c->stream>>>(g, fl, c->sc, c->cyc_dt_fixed, c->cyc_cfl);
+    else k_fill_ghost<long long><<<nb, 128, 0, c->stream>>>(g, fl);
+  }
+}
+
+// ghost layers of five consecutive fields
+void launch_fill_five(idfx_ctx* c, int first_field, bool publish) {
+  FieldList fl;
+  fl.n = 5;
+  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(first_field + n);
+  launch_fill_list(c, fl, publish);
+}
+
 void launch_fill(idfx_ctx* c, int which_b) {
   FieldList fl;
   fl.n = 0;
   for (int n = 0; n < c->nv(); ++n) fl.f[fl.n++] = c->vfield(n);
   if (c->mhd)
     for (int d = 0; d < 3; ++d) fl.f[fl.n++] = c->bbuf(which_b, d);
-  const Geom& g = c->g;
-  const long long px = g.nx + 2 * NG, py = g.ny + 2 * NG;
-  const long long nt = 2LL * NG * py * px + (long long)g.nz * 2 * NG * px + (long long)g.nz * g.ny * 2 * NG;
-  LaunchScope ls(c, K_FILL);
-  k_fill_ghost<<<blocks_for(nt, 128), 128, 0, c->stream>>>(g, fl);
+  launch_fill_list(c, fl, false);
 }
 
 template <int MODE, bool VP, bool NCU>
@@ -1101,6 +1159,25 @@ HdKernel hd_kernel(const idfx_ctx* c, bool first) {
   }
 }
 
+template <int SOLVER>
+HdKernelU hd_kernel_u_s(int limiter, bool first) {
+  switch (limiter) {
+    case LIM_FLAT: return hd_kernel_u_sl<SOLVER, LIM_FLAT>(first);
+    case LIM_MINMOD: return hd_kernel_u_sl<SOLVER, LIM_MINMOD>(first);
+    case LIM_LIMO3: return hd_kernel_u_sl<SOLVER, LIM_LIMO3>(first);
+    default: return hd_kernel_u_sl<SOLVER, LIM_VANLEER>(first);
+  }
+}
+
+HdKernelU hd_kernel_u(const idfx_ctx* c, bool first) {
+  switch (c->solver) {
+    case SOLVER_HLL: return hd_kernel_u_s<SOLVER_HLL>(c->limiter, first);
+    case SOLVER_RUSANOV: return hd_kernel_u_s<SOLVER_RUSANOV>(c->limiter, first);
+    case SOLVER_HLLC: return hd_kernel_u_s<SOLVER_HLLC>(c->limiter, first);
+    default: return hd_kernel_u_s<SOLVER_ROE>(c->limiter, first);
+  }
+}
+
 // RK2 without a stored U_1 (one-kernel stages, no pressure floor): the first stage's update kernel keeps U_1 in registers
 // for the primitives only, and the second stage rebuilds it from U_0 and R_1, which it reads instead of U_1
 bool rk2_keeps_no_u1(const idfx_ctx* c) { return c->fused && c->nstages == 2 && !(c->g.pfloor > 0.0); }
@@ -1117,7 +1194,7 @@ void launch_hd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int 
   for (int n = 0; n < 5; ++n) {
     a.R[n] = c->field(c->f_r() + n);
     a.Uin[n] = c->field((rk2_keeps_no_u1(c) ? c->f_r() : uin) + n);
-    a.U0[n] = c->field(F_UA + n);
+    a.U0[n] = c->field(c->f_u() + n);
     a.Uout[n] = c->field(uout + n);
     a.Vout[n] = c->vfield_out(n);
   }
@@ -1128,6 +1205,37 @@ void launch_hd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int 
   dim3 grid((g.nx + HD_CX - 1) / HD_CX, (g.ny + HD_CY - 1) / HD_CY, (unsigned)((g.nz + a.chunk - 1) / a.chunk));
   LaunchScope ls(c, K_HD);
   hd_kernel(c, first)<<<grid, HD_THREADS, HD_SMEM_BYTES, c->stream>>>(g, a, c->mapHD);
+}
+
+// Hydrodynamic RK2 on a periodic box without pressure floor and without neighbours: the stages read the conserved fields
+// (hd_stage_u.cuh).  The first cycle after set_state still reconstructs from the caller's primitives as given.
+bool hd_ufed(const idfx_ctx* c) {
+  return c->fused && !c->mhd && c->nstages == 2 && !(c->g.pfloor > 0.0) && !c->g.open && !c->exch && !c->v_given;
+}
+
+void launch_hd_stage_u(idfx_ctx* c, bool first, double w, double w0) {
+  const Geom& g = c->g;
+  HdStageArgs a;
+  a.fV0 = c->ucur ? 5 : 0;  // U_0 inside the map over both conserved buffers
+  const long long per_chunk = (long long)((g.nx + HD_CX - 1) / HD_CX) * ((g.ny + HD_CY - 1) / HD_CY);
+  long long nch = (148 * 2 * 8 + per_chunk - 1) / per_chunk;  // about 8 waves of 2 CTAs per SM
+  const long long maxch = g.nz / 16 > 0 ? g.nz / 16 : 1;
+  nch = nch < 1 ? 1 : (nch > maxch ? maxch : nch);
+  a.chunk = (int)((g.nz + nch - 1) / nch);
+  for (int n = 0; n < 5; ++n) {
+    a.R[n] = c->field(c->f_r() + n);
+    a.Uin[n] = c->field(c->f_r() + n);
+    a.U0[n] = c->field(c->f_u() + n);
+    a.Uout[n] = c->field(c->f_ub() + n);
+    a.Vout[n] = nullptr;
+  }
+  a.uin_is_r = 1;
+  a.sc = c->sc;
+  a.w = w;
+  a.w0 = w0;
+  dim3 grid((g.nx + HD_CX - 1) / HD_CX, (g.ny + HD_CY - 1) / HD_CY, (unsigned)((g.nz + a.chunk - 1) / a.chunk));
+  LaunchScope ls(c, K_HD);
+  hd_kernel_u(c, first)<<<grid, HD_THREADS, HDU_SMEM_BYTES, c->stream>>>(g, a, c->mapHU, c->mapHR);
 }
 
 // ---- MHD: the three sweeps and the edge EMFs of a stage in one kernel (mhd_stage.cuh; instantiated in stage_inst.cu) ----
@@ -1179,7 +1287,7 @@ void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int
   for (int n = 0; n < 5; ++n) {
     a.R[n] = c->field(c->f_r() + n);
     a.Uin[n] = c->field((rk2_keeps_no_u1(c) ? c->f_r() : uin) + n);
-    a.U0[n] = c->field(F_UA + n);
+    a.U0[n] = c->field(c->f_u() + n);
     a.Uout[n] = c->field(uout + n);
   }
   a.uin_is_r = rk2_keeps_no_u1(c) ? 1 : 0;
@@ -1196,8 +1304,10 @@ void launch_mhd_stage(idfx_ctx* c, bool first, double w, double w0, int uin, int
 // ---- one cycle, in pieces: cycle_begin, then per stage stage_flux -> stage_update (-> ghost fill), then cycle_end.
 // idfx_step / idfx_advance run them back to back (run_cycle); a domain-decomposed run drives them through the staged ABI
 // with its halo exchange and the reduction of dt in between.
-// Conserved fields: U_0 lives in F_UA for the whole cycle, the intermediate stages in F_UB, the last stage writes the
-// result back to F_UA.  Face field: three buffers rotate, never writing the saved one (b0) nor the stage input.
+// Conserved fields: U_0 lives in one of the two conserved buffers (idfx_ctx::f_u) for the whole cycle, the intermediate
+// stages in the other (f_ub), the last stage writes the result back over U_0 -- except in the hydrodynamic cycle fed with
+// the conserved fields (hd_stage_u.cuh), whose second stage still reads the halo of U_0 in neighbouring tiles while it
+// writes: its result goes to the other buffer and the two swap roles.  Face field: three buffers rotate, never writing the saved one (b0) nor the stage input.
 struct StagePlan {
   bool combine, last;
   int uin, uout, bin, b0, bout;
@@ -1210,8 +1320,8 @@ StagePlan plan_stage(const idfx_ctx* c, int s) {
   StagePlan p;
   p.combine = s > 0;
   p.last = s == c->nstages - 1;
-  p.uin = s == 0 ? F_UA : F_UB;
-  p.uout = p.last ? F_UA : F_UB;
+  p.uin = s == 0 ? c->f_u() : c->f_ub();
+  p.uout = p.last ? c->f_u() : c->f_ub();
   p.w = W[c->nstages - 1][s];
   p.w0 = W0[c->nstages - 1][s];
   p.b0 = c->cyc_b0;
@@ -1229,6 +1339,29 @@ struct NvtxScope {
   ~NvtxScope() { nvtxRangePop(); }
 };
 
+int ensure_v(idfx_ctx* c);
+
+// Before every cycle, outside any graph capture: decides which kind of cycle runs and brings the fields it reads up to date.
+int prepare_cycle(idfx_ctx* c) {
+  c->cyc_ufed = hd_ufed(c);
+  if (c->cyc_ufed) {
+    if (!c->ug_valid) {  // the cycle before wrote U without its ghost layers
+      launch_fill_five(c, c->f_u(), false);
+      c->ug_valid = true;
+    }
+    return IDFX_OK;
+  }
+  return ensure_v(c);
+}
+
+// the flags a finished cycle leaves (cycle_end, or the replay of its graph)
+void after_cycle(idfx_ctx* c) {
+  if (c->cyc_ufed) c->ucur ^= 1;
+  c->v_stale = c->cyc_ufed;
+  c->ug_valid = c->cyc_ufed;
+  c->v_given = false;
+}
+
 void cycle_begin(idfx_ctx* c, double dt_fixed, double cfl) {
   NvtxScope range("idfx cycle_begin");
   c->cyc_dt_fixed = dt_fixed;
@@ -1243,6 +1376,10 @@ void stage_flux(idfx_ctx* c, int s) {
   static const char* const names[3] = {"idfx stage 1 flux+emf", "idfx stage 2 flux+emf", "idfx stage 3 flux+emf"};
   NvtxScope range(names[s]);
   const StagePlan p = plan_stage(c, s);
+  if (c->cyc_ufed) {
+    launch_hd_stage_u(c, !p.combine, p.w, p.w0);
+    return;
+  }
   const double* Bf[3] = {c->bbuf(p.bin, 0), c->bbuf(p.bin, 1), c->bbuf(p.bin, 2)};
   if (!c->fused) launch_ppm(c, Bf, s == 0 && !(c->cyc_dt_fixed > 0.0));  // PPM: generic face-flux kernels, divergence and dt in k_rhs
   else if (c->mhd) launch_mhd_stage(c, !p.combine, p.w, p.w0, p.uin, p.uout, p.bin);
@@ -1256,6 +1393,12 @@ void stage_update(idfx_ctx* c, int s) {
   const StagePlan p = plan_stage(c, s);
   const Geom& g = c->g;
   c->cyc_bin = p.bout;
+  if (c->cyc_ufed) {
+    // a1 of what the stage wrote: R_1 (and the dt of the cycle, now that the whole box has been reduced), or the result
+    if (!p.combine) launch_fill_five(c, c->f_r(), true);
+    else launch_fill_five(c, c->f_ub(), false);
+    return;
+  }
   if (c->fused && !c->mhd && p.combine) {
     // the HD stage kernel wrote U_s, its primitives and (periodic box) their ghost images into the other primitive buffer
     c->vcur ^= 1;
@@ -1265,7 +1408,7 @@ void stage_update(idfx_ctx* c, int s) {
   UpdateArgs a;
   for (int n = 0; n < 5; ++n) {
     a.Uin[n] = c->field(p.uin + n);
-    a.U0[n] = c->field(F_UA + n);
+    a.U0[n] = c->field(c->f_u() + n);
     a.R[n] = c->field(c->f_r() + n);
     a.Uout[n] = c->field(p.uout + n);
   }
@@ -1316,7 +1459,10 @@ void stage_update(idfx_ctx* c, int s) {
   }
 }
 
-void cycle_end(idfx_ctx* c) { c->bcur = c->cyc_bin; }
+void cycle_end(idfx_ctx* c) {
+  c->bcur = c->cyc_bin;
+  after_cycle(c);
+}
 
 int run_cycle(idfx_ctx* c, double dt_fixed, double cfl) {
   cycle_begin(c, dt_fixed, cfl);
@@ -1361,7 +1507,7 @@ int reset_clock(idfx_ctx* c) {
 // after the primitives (V[0..4]) and the face field (current buffer, active part) are in place
 int finish_set_state(idfx_ctx* c) {
   StateArgs a;
-  for (int n = 0; n < 5; ++n) a.U[n] = c->field(F_UA + n);
+  for (int n = 0; n < 5; ++n) a.U[n] = c->field(c->f_u() + n);
   for (int n = 0; n < 11; ++n) a.V[n] = n < c->nv() ? c->vfield(n) : nullptr;
   for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
   a.sc = c->sc;
@@ -1375,6 +1521,9 @@ int finish_set_state(idfx_ctx* c) {
   }
   c->cyc_bin = c->bcur;
   if (!c->exch) launch_fill(c, c->bcur);
+  c->v_given = true;  // the next cycle reconstructs from exactly these primitives
+  c->v_stale = false;
+  c->ug_valid = false;
   CK(cudaGetLastError());
   if (c->vp) {  // G19: the potential is counted from this state on
     const size_t fb = (size_t)c->g.np * sizeof(double);
@@ -1386,7 +1535,7 @@ int finish_set_state(idfx_ctx* c) {
 
 int refresh_prims(idfx_ctx* c) {
   StateArgs a;
-  for (int n = 0; n < 5; ++n) a.U[n] = c->field(F_UA + n);
+  for (int n = 0; n < 5; ++n) a.U[n] = c->field(c->f_u() + n);
   for (int n = 0; n < 11; ++n) a.V[n] = nullptr;
   for (int n = 0; n < 5; ++n) a.V[n] = c->field(c->f_r() + n);  // scratch: R is dead between cycles
   for (int d = 0; d < 3; ++d) a.Bf[d] = c->bbuf(c->bcur, d);
@@ -1396,6 +1545,25 @@ int refresh_prims(idfx_ctx* c) {
   if (c->mhd) k_prim_from_cons<true><<<nb, 128, 0, c->stream>>>(c->g, a);
   else k_prim_from_cons<false><<<nb, 128, 0, c->stream>>>(c->g, a);
   }
+  CK(cudaGetLastError());
+  return IDFX_OK;
+}
+
+// Hydrodynamic cycles fed with the conserved fields leave the primitive buffer behind: bring it (and its ghost layers) up to
+// date before anything reads it (a cycle of the other kind after an option changed)
+int ensure_v(idfx_ctx* c) {
+  if (!c->v_stale) return IDFX_OK;
+  StateArgs a;
+  for (int n = 0; n < 5; ++n) a.U[n] = c->field(c->f_u() + n);
+  for (int n = 0; n < 11; ++n) a.V[n] = n < 5 ? c->vfield(n) : nullptr;
+  for (int d = 0; d < 3; ++d) a.Bf[d] = nullptr;
+  a.sc = c->sc;
+  {
+    LaunchScope ls(c, K_STATE);
+    k_prim_from_cons<false><<<blocks_for(c->g.nc, 128), 128, 0, c->stream>>>(c->g, a);
+  }
+  launch_fill(c, c->bcur);
+  c->v_stale = false;
   CK(cudaGetLastError());
   return IDFX_OK;
 }
@@ -1486,6 +1654,9 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
   c->sc = (DevScalars*)(c->ws + (size_t)c->nfields() * (size_t)c->g.np);
   c->bcur = 0;
   c->vcur = 0;
+  c->ucur = 0;
+  c->v_given = true;
+  c->v_stale = c->ug_valid = c->cyc_ufed = false;
   c->launches = 0;
   CK(cudaMemsetAsync(d_workspace, 0, idfx_workspace_bytes(c), c->stream));
   if (int rc = reset_clock(c)) return rc;
@@ -1503,7 +1674,10 @@ int idfx_bind(idfx_ctx* c, void* d_workspace, size_t bytes, void* cuda_stream) {
   }
   if (c->fused && !c->mhd)
     for (int first = 0; first < 2; ++first)
+    {
       CK(cudaFuncSetAttribute((const void*)hd_kernel(c, first != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, HD_SMEM_BYTES));
+      CK(cudaFuncSetAttribute((const void*)hd_kernel_u(c, first != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, HDU_SMEM_BYTES));
+    }
   if (c->fused && c->mhd)
     for (int v = 0; v < 4; ++v)  // first / later stage x periodic / open (the boundary option may still change after bind)
       CK(cudaFuncSetAttribute((const void*)mhd_kernel(c, (v & 1) != 0, c->emf2d() ? EMF_ARITH : c->emf, (v & 2) != 0),
@@ -1627,7 +1801,7 @@ int idfx_get_conserved(idfx_ctx* c, double* d_cons, double* d_bface) {
   const unsigned nb = blocks_for(c->g.nc, 128);
   FieldList fl;
   fl.n = 5;
-  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(F_UA + n);
+  for (int n = 0; n < 5; ++n) fl.f[n] = c->field(c->f_u() + n);
   { LaunchScope ls(c, K_STATE);
   k_unpack<<<nb, 128, 0, c->stream>>>(c->g, fl, d_cons);
   }
@@ -1654,8 +1828,9 @@ int idfx_compute_dt(idfx_ctx* c, double cfl, double* h_dt_out) {
   if (c->fused) {
     // the first-stage kernel itself, run for its reduction only (its divergence and EMFs land in scratch that is dead
     // between cycles): the same arithmetic, tile for tile, as the dt a cycle would take, on any kind of boundary
-    if (c->mhd) launch_mhd_stage(c, true, 1.0, 0.0, F_UA, F_UB, c->bcur);
-    else launch_hd_stage(c, true, 1.0, 0.0, F_UA, F_UB);
+    if (c->mhd) launch_mhd_stage(c, true, 1.0, 0.0, c->f_u(), c->f_ub(), c->bcur);
+    else if (c->v_stale) launch_hd_stage_u(c, true, 1.0, 0.0);  // the conserved fields (with ghosts) are what is current
+    else launch_hd_stage(c, true, 1.0, 0.0, c->f_u(), c->f_ub());
   } else {
     const double* Bf[3] = {c->bbuf(c->bcur, 0), c->bbuf(c->bcur, 1), c->bbuf(c->bcur, 2)};
     for (int d = 0; d < 3; ++d) launch_speed(c, d, Bf);
@@ -1683,6 +1858,7 @@ int idfx_step(idfx_ctx* c, double dt) {
     set_err("idfx_step: with exchanged directions the cycle is driven through idfx_cycle_begin / idfx_stage_* / idfx_halo_*");
     return IDFX_ERR_UNSUPPORTED;
   }
+  if ((rc = prepare_cycle(c))) return rc;
   return run_cycle(c, dt, 0.0);
 }
 
@@ -1698,15 +1874,24 @@ static int advance_cycles(idfx_ctx* c, int nsteps, double cfl) {
     c->graph_cfl = cfl;
   }
   for (int s = 0; s < nsteps; ++s) {
+    if ((rc = prepare_cycle(c))) return rc;
     if (!c->use_graph || c->prof_on) {
       if ((rc = run_cycle(c, 0.0, cfl))) return rc;
       continue;
     }
     // the cycle is a fixed sequence of kernels whose arguments depend only on the buffer rotation state: capture it
     // once per state, then replay (dt and the clock never leave the device, so nothing else varies)
-    const int key = c->bcur * 2 + c->vcur;
+    // (a cycle fed with the conserved fields rotates only those; the other kind never runs with them swapped unless such
+    // cycles came before it, and then its graphs are captured anew)
+    const int key = c->cyc_ufed ? 6 + c->ucur : c->bcur * 2 + c->vcur;
+    if (c->graph[key] && c->graph_ucur[key] != c->ucur) {
+      cudaGraphExecDestroy(c->graph[key]);
+      c->graph[key] = nullptr;
+    }
     if (!c->graph[key]) {
-      const int b = c->bcur, v = c->vcur;
+      const int b = c->bcur, v = c->vcur, u = c->ucur;
+      const bool vg = c->v_given, vs = c->v_stale, ug = c->ug_valid;
+      c->graph_ucur[key] = u;
       const long long l0 = c->launches;
       cudaGraph_t gr = nullptr;
       CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
@@ -1724,11 +1909,16 @@ static int advance_cycles(idfx_ctx* c, int nsteps, double cfl) {
       c->graph_vnext[key] = c->vcur;
       c->bcur = b;
       c->vcur = v;
+      c->ucur = u;
+      c->v_given = vg;
+      c->v_stale = vs;
+      c->ug_valid = ug;
     }
     CK(cudaGraphLaunch(c->graph[key], c->stream));
     c->launches += c->graph_launches[key];
     c->bcur = c->graph_bnext[key];  // as run_cycle leaves them
     c->vcur = c->graph_vnext[key];
+    after_cycle(c);
   }
   return IDFX_OK;
 }
@@ -1905,6 +2095,7 @@ int idfx_cycle_begin(idfx_ctx* c, double dt, double cfl) {
     set_err("idfx_cycle_begin: need dt > 0, or dt <= 0 and 0 < cfl < 1");
     return IDFX_ERR_INVALID_ARG;
   }
+  if ((rc = prepare_cycle(c))) return rc;
   cycle_begin(c, dt > 0.0 ? dt : 0.0, cfl);
   CK(cudaGetLastError());
   return IDFX_OK;

@@ -1,4 +1,4 @@
-// stage_inst.cu — the one-kernel stages (hd_stage.cuh, mhd_stage.cuh) of one (Riemann solver, reconstruction) pair.
+// stage_inst.cu — the one-kernel stages (hd_stage.cuh, hd_stage_u.cuh, mhd_stage.cuh) of one (Riemann solver, reconstruction) pair.
 // build.py compiles this file once per pair (-DIDFX_INST_SOLVER=s -DIDFX_INST_LIM=l), each into its own object: the
 // register allocation of these kernels sits at the edge of their occupancy target (168 registers for 384 threads) and
 // was found to change with the other kernels of the translation unit and with nvcc's -split-compile partitioning, i.e.
@@ -15,6 +15,11 @@ namespace idfx {
 template <int SOLVER, int LIM>
 HdKernel hd_kernel_sl(bool first) {
   return first ? (HdKernel)k_hd_stage<SOLVER, LIM, true> : (HdKernel)k_hd_stage<SOLVER, LIM, false>;
+}
+
+template <int SOLVER, int LIM>
+HdKernelU hd_kernel_u_sl(bool first) {
+  return first ? (HdKernelU)k_hd_stage_u<SOLVER, LIM, true> : (HdKernelU)k_hd_stage_u<SOLVER, LIM, false>;
 }
 
 template <int SOLVER, int LIM, int MODE>
@@ -38,6 +43,7 @@ template MhdKernel mhd_kernel_sl<IDFX_INST_SOLVER, IDFX_INST_LIM>(bool, int, boo
 #endif
 #if IDFX_INST_SOLVER != 2
 template HdKernel hd_kernel_sl<IDFX_INST_SOLVER, IDFX_INST_LIM>(bool);
+template HdKernelU hd_kernel_u_sl<IDFX_INST_SOLVER, IDFX_INST_LIM>(bool);
 #endif
 
 }  // namespace idfx

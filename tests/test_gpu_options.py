@@ -330,3 +330,53 @@ def test_emf_hlld2d_on_turbulence_all_fan_regions(idfx, R):
     bf = sim.get_conserved()[1]
     div = (torch.roll(bf[0], -1, 2) - bf[0]) + (torch.roll(bf[1], -1, 1) - bf[1]) + (torch.roll(bf[2], -1, 0) - bf[2])
     assert float(div.abs().max() / bf.abs().max()) <= 1e-13
+
+
+@pytest.mark.parametrize("solver,limiter", [(HLLC, VANLEER), (ROE, MINMOD), (HLL, LIMO3)])
+def test_hd_cycles_fed_with_the_conserved_fields(idfx, R, solver, limiter):
+    """Hydrodynamic RK2 cycles on a periodic box read the conserved fields and never write the primitive buffers
+    (csrc/hd_stage_u.cuh), except the first cycle after set_state, which reconstructs from the caller's primitives as given.
+    Every way in and out of that mode against the oracle: graph replay and single steps, compute_dt and get_state in
+    between, a switch to RK3 and back, fixed steps, and a second set_state.  The box
+    spans several 31 x 7 tiles, partial ones and three z chunks."""
+    nx, ny, nz = 70, 45, 50
+    prim, _, dx = smooth_ic(nx, ny, nz, 29, mhd=False)
+    sim = idfx.Idfx(nx, ny, nz, dx, G53, solver, limiter, EMF_NONE)
+    ref = R.Oracle(nx, ny, nz, dx, G53, solver, limiter, EMF_NONE)
+    sim.set_state(torch.from_numpy(prim).cuda())
+    ref.set_state(prim)
+
+    def both(what, *args):
+        getattr(sim, what)(*args)
+        getattr(ref, what)(*args)
+
+    def check(tag):
+        assert abs(sim.last_dt() - ref.last_dt()) <= TOL_DT * ref.last_dt(), tag
+        assert_state_close(sim, ref, TOL, tag)
+        dg, dr = sim.compute_dt(0.4), ref.compute_dt(0.4)
+        assert abs(dg - dr) <= TOL_DT * dr, tag + ": compute_dt"
+
+    both("advance", 4, 0.4)                      # one cycle from the given primitives, three from the conserved fields
+    check("4 cycles")
+    both("advance", 1, 0.4)                      # compute_dt and get_state in between must not have disturbed anything
+    check("5 cycles")
+    dt = 0.5 * ref.last_dt()
+    both("step", dt)                             # outside the graphs
+    both("step", dt)
+    check("fixed steps")
+    sim.set_integrator(3)                        # RK3 needs the primitive buffers again ...
+    assert ref.L.idfxref_set_option(ref.h, 0, 3) == 0
+    both("advance", 2, 0.4)
+    check("RK3")
+    sim.set_integrator(2)                        # ... and RK2 drops them again, with the conserved buffers swapped or not
+    assert ref.L.idfxref_set_option(ref.h, 0, 2) == 0
+    both("advance", 3, 0.4)
+    check("RK2 again")
+    sim.set_state(torch.from_numpy(prim).cuda())
+    ref.set_state(prim)
+    both("advance", 3, 0.4)
+    check("after a second set_state")
+    assert sim.status() == 0 and ref.status() == 0
+    cons_g = sim.get_conserved()[0].cpu().numpy()
+    cons_r = ref.get_conserved()[0]
+    assert np.abs(cons_g - cons_r).max() <= TOL * np.abs(cons_r).max()
