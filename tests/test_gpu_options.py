@@ -372,6 +372,14 @@ def test_hd_cycles_fed_with_the_conserved_fields(idfx, R, solver, limiter):
     assert ref.L.idfxref_set_option(ref.h, 0, 2) == 0
     both("advance", 3, 0.4)
     check("RK2 again")
+    for _ in range(2):                           # the same cycles through the staged calls (include/idfx.h)
+        sim.cycle_begin(0.0, 0.4)
+        for stage in range(2):
+            sim.stage_flux(stage)
+            sim.stage_update(stage)
+        sim.cycle_end()
+    ref.advance(2, 0.4)
+    check("staged calls")
     sim.set_state(torch.from_numpy(prim).cuda())
     ref.set_state(prim)
     both("advance", 3, 0.4)
