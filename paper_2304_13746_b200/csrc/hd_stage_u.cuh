@@ -6,7 +6,8 @@
 // What is gone from the cycle: the update kernel between the stages (10 doubles read, 5 written per cell), the primitives
 // the second stage wrote for the next cycle (5) and read back (5 + halo).  The halo of R_1 and of the result U comes from
 // the ghost-fill kernel (a1) after each stage; the one after the first stage also publishes the dt of the cycle.
-// (Measured at 512^3: images written by the owners of the boundary cells inside these kernels, as the MHD update kernel
+// (Measured at 512^3: alternating the two landing slots in the first stage, one plane more of look-ahead, changes nothing:
+// the kernels do not wait for their loads.  Images written by the owners of the boundary cells inside these kernels, as the MHD update kernel
 // does, cost the stage kernels 3 %, more than the two fill launches take: 16.84 against 16.72 ms per cycle.)
 //   first stage : R_1 = flux divergence of prim(U_0), max_cells sum_d c_d / dx
 //   second stage: U = w0 U_0 + w (U_1 - dt/dx R_2) (Eq. 9), written to the OTHER conserved buffer: neighbouring tiles still

@@ -89,7 +89,14 @@ __device__ __forceinline__ void fill_ghost_cell(const Geom& g, const FieldList& 
     ks = min(max(k, 0), g.nz - 1);
   }
   const long long d = g.at(i, j, k), s = g.at(is, js, ks);
-  for (int n = 0; n < fl.n; ++n) fl.f[n][d] = fl.f[n][s];
+  // all loads first: a ghost cell is one strided access per field, and the copy is bound by how many are in flight
+  double v[14];
+#pragma unroll
+  for (int n = 0; n < 14; ++n)
+    if (n < fl.n) v[n] = fl.f[n][s];
+#pragma unroll
+  for (int n = 0; n < 14; ++n)
+    if (n < fl.n) fl.f[n][d] = v[n];
 }
 
 template <typename T>
