@@ -2171,6 +2171,7 @@ static int halo_op(idfx_ctx* c, int dir, int side, int mode, int clamp, double* 
     set_err("%s: need 0 <= dir <= 2, side 0 (lower) or 1 (upper) and a device buffer", who);
     return IDFX_ERR_INVALID_ARG;
   }
+  if ((rc = ensure_v(c))) return rc;  // the slabs are cut from the primitive buffer
   const SlabGeom sg = slab_geom(c->g, dir, side, mode, clamp);
   const FieldList fl = halo_fields(c);
   const unsigned nb = blocks_for(sg.count, 128);
@@ -2199,6 +2200,7 @@ int idfx_halo_push(idfx_ctx* c, int dir, int side, idfx_ctx* nb) {
     set_err("idfx_halo_push: need 0 <= dir <= 2 and side 0 (lower) or 1 (upper)");
     return IDFX_ERR_INVALID_ARG;
   }
+  if ((rc = ensure_v(c))) return rc;  // the slab is cut from the primitive buffer
   const SlabGeom from = slab_geom(c->g, dir, side, SLAB_PACK, 0), to = slab_geom(nb->g, dir, 1 - side, SLAB_UNPACK, 0);
   const FieldList fs = halo_fields(c), fd = halo_fields(nb);
   if (from.ext[0] != to.ext[0] || from.ext[1] != to.ext[1] || from.ext[2] != to.ext[2] || fs.n != fd.n) {
