@@ -325,6 +325,10 @@ def run_ours(args):
     roof = roof_of(dom)
     hbm_kernels = [k for k in per_class if k not in ALGO_FLOPS_PER_CELL]
     roof_hbm = roof_of(max(hbm_kernels, key=per_class.get)) if hbm_kernels else None
+    if not mhd:
+        # bench.py holds no flop count for the hydrodynamic stage kernels, so their line is the HBM one; ncu shows them bound
+        # by fp64 issue since they read the conserved fields (profiles/r02_ncu_full_512.md: 58-62 % of the pipe, 1.5-2.2 TB/s)
+        roof["note"] = "hd_stage is bound by fp64 issue, not HBM (profiles/r02_ncu_full_512.md); no flop model for it here"
     step_bytes = ALGO_BYTES_PER_CELL_UPDATE if mhd else ALGO_BYTES_PER_CELL_UPDATE_HD
     step_hbm = step_bytes * value / world * 1e-9
     roof_step = {"bound": "hbm", "achieved": step_hbm, "peak": hbm_peak, "unit": "GB/s", "frac": step_hbm / hbm_peak,
